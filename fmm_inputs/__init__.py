@@ -1,0 +1,304 @@
+"""Seeded synthetic inputs for the FMM cell-to-cell interaction step.
+
+This module is the ONLY code shared by the CPU oracle (``oracle/``) and the CUDA
+path (``paper_2101_08226_b200/``).  It holds none of the method's arithmetic
+(no Green's-function tensors, no stencil, no M2L): it only manufactures the
+per-cell multipole moments that the interaction step takes as *input*.
+
+What the inputs stand in for
+----------------------------
+The paper measures on stationary n=3/2 polytropes (§3.5;
+scaling runs §5: 128^3 = 4096 sub-grids, 256^3 = 32768 sub-grids of
+8x8x8 cells) and on a q<1 binary (§4).  Its input decks (Zenodo, L1144-1146)
+are not available, so seeded synthetic fields of the same shape are used:
+Lane-Emden n=1.5 density profiles on the unit cube with the 1e-10 ambient
+floor of Eq. 36 (L325-327).
+
+Cell model
+----------
+"The multipoles of each cell are composed of the multipoles of its child
+cells" (L125).  Every cell is 8 child point masses at
+x_cell + (+-h/4, +-h/4, +-h/4); the cell's raw Cartesian moments about its
+centre of mass,  M^(n) = sum_p m_p (y_p - z)^{(x) n},  n = 0..3, are the 20
+unique components in lexicographic order
+  [0] [x y z] [xx xy xz yy yz zz] [xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz]
+with no factorials or multiplicities folded in.  The expansion centre is
+handed over as the OFFSET  delta = z - x_cell  (3 doubles per cell).
+
+Array layout (both outputs): component-major SoA, C order, x fastest:
+  moments[20][nz][ny][nx],  com_off[3][nz][ny][nx].
+
+Random numbers: SplitMix64 counter stream, u = (x >> 11) * 2^-53.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+
+DEFAULT_SEED = 20210108
+
+# unique-component index tables (lexicographic), exported for tests/harness
+IDX2 = [(0, 0), (0, 1), (0, 2), (1, 1), (1, 2), (2, 2)]
+IDX3 = [(0, 0, 0), (0, 0, 1), (0, 0, 2), (0, 1, 1), (0, 1, 2), (0, 2, 2),
+        (1, 1, 1), (1, 1, 2), (1, 2, 2), (2, 2, 2)]
+
+_GOLDEN = np.uint64(0x9E3779B97F4A7C15)
+_MIX1 = np.uint64(0xBF58476D1CE4E5B9)
+_MIX2 = np.uint64(0x94D049BB133111EB)
+
+
+def splitmix64(seed: int, count: int, offset: int = 0) -> np.ndarray:
+    """``count`` SplitMix64 outputs, draws number offset+1 .. offset+count of the stream."""
+    with np.errstate(over="ignore"):
+        idx = np.arange(offset + 1, offset + count + 1, dtype=np.uint64)
+        z = np.uint64(seed & 0xFFFFFFFFFFFFFFFF) + idx * _GOLDEN
+        z = (z ^ (z >> np.uint64(30))) * _MIX1
+        z = (z ^ (z >> np.uint64(27))) * _MIX2
+        z = z ^ (z >> np.uint64(31))
+    return z
+
+
+def uniform01(seed: int, count: int, offset: int = 0) -> np.ndarray:
+    """Doubles in [0,1): (x >> 11) * 2^-53."""
+    return (splitmix64(seed, count, offset) >> np.uint64(11)).astype(np.float64) * (2.0 ** -53)
+
+
+# --------------------------------------------------------------------------------------
+# Lane-Emden n = 1.5 profile (Eq. 43 / §3.5: polytropic index n = 3/2)
+# --------------------------------------------------------------------------------------
+_LE_CACHE = {}
+
+
+def lane_emden(n: float = 1.5, dxi: float = 1.0e-4):
+    """Integrate theta'' + 2 theta'/xi + theta^n = 0 by RK4.
+
+    Returns (xi_grid, theta_grid, xi1) with theta(xi1) = 0 the first zero
+    (xi1 = 3.65375... for n = 1.5)."""
+    key = (n, dxi)
+    if key in _LE_CACHE:
+        return _LE_CACHE[key]
+
+    def rhs(xi, th, ph):
+        return ph, -(max(th, 0.0) ** n) - 2.0 * ph / xi
+
+    xi = dxi
+    th = 1.0 - xi * xi / 6.0 + n * xi ** 4 / 120.0
+    ph = -xi / 3.0 + n * xi ** 3 / 30.0
+    xs, ths = [0.0, xi], [1.0, th]
+    xi1 = None
+    while True:
+        k1t, k1p = rhs(xi, th, ph)
+        k2t, k2p = rhs(xi + 0.5 * dxi, th + 0.5 * dxi * k1t, ph + 0.5 * dxi * k1p)
+        k3t, k3p = rhs(xi + 0.5 * dxi, th + 0.5 * dxi * k2t, ph + 0.5 * dxi * k2p)
+        k4t, k4p = rhs(xi + dxi, th + dxi * k3t, ph + dxi * k3p)
+        th_new = th + dxi * (k1t + 2 * k2t + 2 * k3t + k4t) / 6.0
+        ph_new = ph + dxi * (k1p + 2 * k2p + 2 * k3p + k4p) / 6.0
+        xi_new = xi + dxi
+        if th_new <= 0.0:
+            xi1 = xi + dxi * th / (th - th_new)
+            xs.append(xi_new)
+            ths.append(0.0)
+            break
+        xi, th, ph = xi_new, th_new, ph_new
+        xs.append(xi)
+        ths.append(th)
+    out = (np.asarray(xs), np.asarray(ths), float(xi1))
+    _LE_CACHE[key] = out
+    return out
+
+
+def polytrope_density(r: np.ndarray, radius: float, rho_c: float) -> np.ndarray:
+    """rho(r) = rho_c * theta_LE(xi1 r / radius)^1.5 inside the star, 0 outside."""
+    xs, ths, xi1 = lane_emden()
+    xi = np.asarray(r) * (xi1 / radius)
+    th = np.interp(xi, xs, ths, right=0.0)
+    th = np.where(xi < xi1, np.maximum(th, 0.0), 0.0)
+    return rho_c * th ** 1.5
+
+
+# --------------------------------------------------------------------------------------
+# fields
+# --------------------------------------------------------------------------------------
+@dataclass
+class Star:
+    centre: tuple
+    radius: float
+    rho_c: float
+
+
+FLOOR = 1.0e-10  # ambient density floor, PAPER.md L325-327 (Eq. 36)
+
+SINGLE_STAR = [Star((0.5, 0.5, 0.5), 0.4, 1.0)]
+# M ~ rho_c R^3 for a fixed polytropic index, so M2/M1 = 0.7 needs rho_c2 = 0.7 (0.15/0.12)^3
+BINARY = [Star((0.3, 0.5, 0.5), 0.15, 1.0), Star((0.7, 0.5, 0.5), 0.12, 0.7 * (0.15 / 0.12) ** 3)]
+
+
+def field_density(stars, x, y, z):
+    rho = np.zeros(np.broadcast(x, y, z).shape)
+    for s in stars:
+        r = np.sqrt((x - s.centre[0]) ** 2 + (y - s.centre[1]) ** 2 + (z - s.centre[2]) ** 2)
+        rho = rho + polytrope_density(r, s.radius, s.rho_c)
+    return np.maximum(rho, FLOOR)
+
+
+# --------------------------------------------------------------------------------------
+# cells from 8 child point masses
+# --------------------------------------------------------------------------------------
+# child c = bx + 2 by + 4 bz, sign s = 2 b - 1
+CHILD_SIGNS = np.array([[2 * ((c >> a) & 1) - 1 for a in range(3)] for c in range(8)], dtype=np.float64)
+
+
+def cells_from_children(child_mass: np.ndarray, h: float):
+    """P2M of the 8-child cell model.
+
+    child_mass: [8][...cells...] masses of the children at +-h/4 offsets.
+    Returns (moments[20][...], com_off[3][...])."""
+    shape = child_mass.shape[1:]
+    q = 0.25 * h
+    m0 = child_mass.sum(axis=0)
+    com = np.zeros((3,) + shape)
+    for c in range(8):
+        for a in range(3):
+            com[a] += child_mass[c] * (CHILD_SIGNS[c, a] * q)
+    com /= m0
+    mom = np.zeros((20,) + shape)
+    mom[0] = m0
+    for c in range(8):
+        d = [CHILD_SIGNS[c, a] * q - com[a] for a in range(3)]
+        m = child_mass[c]
+        for a in range(3):
+            mom[1 + a] += m * d[a]
+        for t, (a, b) in enumerate(IDX2):
+            mom[4 + t] += m * d[a] * d[b]
+        for t, (a, b, e) in enumerate(IDX3):
+            mom[10 + t] += m * d[a] * d[b] * d[e]
+    return mom, com
+
+
+@dataclass
+class Workload:
+    name: str
+    n: tuple            # (nx, ny, nz) cells
+    h: float
+    theta: float
+    kind: str           # "multipole" | "monopole"
+    am_correction: bool
+    out_lo: tuple       # target region, cells (x, y, z)
+    out_hi: tuple
+    moments: np.ndarray             # [20][nz][ny][nx]  (monopole: [1][nz][ny][nx])
+    com_off: Optional[np.ndarray]   # [3][nz][ny][nx]   (monopole: None)
+    child_mass: Optional[np.ndarray] = None  # [8][nz][ny][nx], kept only on request (brute force)
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def out_shape(self):
+        return tuple(self.out_hi[a] - self.out_lo[a] for a in range(3))
+
+
+def _cell_axis(n, h):
+    return (np.arange(n, dtype=np.float64) + 0.5) * h
+
+
+def _star_children(stars, n, h, kslice, factor=None):
+    """Child masses [8][kz][ny][nx] for z-layers kslice, sampled on the 2n lattice."""
+    nx, ny, nz = n
+    xc = _cell_axis(nx, h)[None, None, :]
+    yc = _cell_axis(ny, h)[None, :, None]
+    zc = _cell_axis(nz, h)[kslice][:, None, None]
+    q = 0.25 * h
+    cm = np.empty((8, zc.shape[0], ny, nx))
+    vol = (0.5 * h) ** 3
+    for c in range(8):
+        sx, sy, sz = CHILD_SIGNS[c]
+        cm[c] = field_density(stars, xc + sx * q, yc + sy * q, zc + sz * q) * vol
+    if factor is not None:
+        cm *= factor[None]
+    return cm
+
+
+def _uniform_field(name, stars, ncell, theta, seed, perturb, keep_children=False, kind="multipole",
+                   dtype_out=np.float64):
+    n = (ncell, ncell, ncell)
+    h = 1.0 / ncell
+    ncells = ncell ** 3
+    factor = None
+    if perturb is not None:
+        lo, hi = perturb
+        factor = (lo + (hi - lo) * uniform01(seed, ncells)).reshape(ncell, ncell, ncell)
+    if kind == "monopole":
+        xc = _cell_axis(ncell, h)
+        mass = np.empty((1, ncell, ncell, ncell))
+        chunk = max(1, min(ncell, (1 << 22) // (ncell * ncell)))
+        for k0 in range(0, ncell, chunk):
+            ks = slice(k0, min(ncell, k0 + chunk))
+            rho = field_density(stars, xc[None, None, :], xc[None, :, None], xc[ks][:, None, None])
+            mass[0, ks] = rho * h ** 3
+        if factor is not None:
+            mass[0] *= factor
+        return Workload(name, n, h, theta, "monopole", False, (0, 0, 0), n, mass, None,
+                        meta={"seed": seed, "stars": len(stars)})
+    mom = np.empty((20, ncell, ncell, ncell))
+    com = np.empty((3, ncell, ncell, ncell))
+    children = np.empty((8, ncell, ncell, ncell)) if keep_children else None
+    chunk = max(1, min(ncell, (1 << 21) // (ncell * ncell)))
+    for k0 in range(0, ncell, chunk):
+        ks = slice(k0, min(ncell, k0 + chunk))
+        cm = _star_children(stars, n, h, ks, None if factor is None else factor[ks])
+        m, c = cells_from_children(cm, h)
+        mom[:, ks] = m
+        com[:, ks] = c
+        if keep_children:
+            children[:, ks] = cm
+    return Workload(name, n, h, theta, "multipole", True, (0, 0, 0), n, mom, com, children,
+                    meta={"seed": seed, "stars": len(stars)})
+
+
+def config1(seed: int = DEFAULT_SEED, theta: float = 0.5, ncell: int = 24, keep_children: bool = True,
+            out_lo=None, out_hi=None) -> Workload:
+    """cfg 1: one 8^3 sub-grid + its 26 neighbours (24^3 cells, h = 1/24), random cells.
+
+    rho ~ U(0.5,1.5), m = rho h^3; alpha ~ U(-0.4,0.4)^3; child masses
+    (m/8) prod_c (1 + alpha_c s_c)  =>  COM offset = alpha h/4 ~ U(-0.1h, 0.1h)."""
+    h = 1.0 / ncell
+    ncells = ncell ** 3
+    u = uniform01(seed, 4 * ncells).reshape(ncell, ncell, ncell, 4)
+    m = (0.5 + u[..., 0]) * h ** 3
+    alpha = -0.4 + 0.8 * u[..., 1:4]
+    cm = np.empty((8, ncell, ncell, ncell))
+    for c in range(8):
+        w = np.ones((ncell, ncell, ncell))
+        for a in range(3):
+            w = w * (1.0 + alpha[..., a] * CHILD_SIGNS[c, a])
+        cm[c] = (m / 8.0) * w
+    mom, com = cells_from_children(cm, h)
+    n = (ncell,) * 3
+    if out_lo is None:
+        out_lo, out_hi = ((8, 8, 8), (16, 16, 16)) if ncell == 24 else ((0, 0, 0), n)
+    return Workload("cfg1_random_%d" % ncell, n, h, theta, "multipole", True, tuple(out_lo), tuple(out_hi),
+                    mom, com, cm if keep_children else None, meta={"seed": seed})
+
+
+def config2(seed: int = DEFAULT_SEED, theta: float = 0.5, ncell: int = 32, keep_children: bool = False) -> Workload:
+    """cfg 2: single n=1.5 polytrope (R = 0.4, centred), ncell^3 cells on the unit cube."""
+    return _uniform_field("cfg2_polytrope_%d" % ncell, SINGLE_STAR, ncell, theta, seed, None, keep_children)
+
+
+def config3(seed: int = DEFAULT_SEED, theta: float = 0.5, ncell: int = 128, keep_children: bool = False) -> Workload:
+    """cfg 3: two-polytrope binary, per-cell factor ~U(0.99,1.01), ncell^3 cells (paper: 128^3, L1004)."""
+    return _uniform_field("cfg3_binary_%d" % ncell, BINARY, ncell, theta, seed, (0.99, 1.01), keep_children)
+
+
+def config4(seed: int = DEFAULT_SEED, theta: float = 0.5, ncell: int = 128) -> Workload:
+    """cfg 4: monopole (leaf) variant on the cfg-3 field: m = h^3 rho(x_cell) * factor."""
+    return _uniform_field("cfg4_monopole_%d" % ncell, BINARY, ncell, theta, seed, (0.99, 1.01), kind="monopole")
+
+
+def config5(seed: int = DEFAULT_SEED, theta: float = 0.5, ncell: int = 256, keep_children: bool = False) -> Workload:
+    """cfg 5: binary with 1e-8 density noise, ncell^3 cells (paper: 256^3 = 32768 sub-grids, L986)."""
+    return _uniform_field("cfg5_binary_%d" % ncell, BINARY, ncell, theta, seed,
+                          (1.0 - 1.0e-8, 1.0 + 1.0e-8), keep_children)
+
+
+CONFIGS = {"cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5}

@@ -1,0 +1,442 @@
+/*
+ * fmm_oracle.c -- plain, slow, obviously-correct CPU oracle of the same-level FMM
+ * cell-to-cell interaction step of Octo-Tiger's gravity solver.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference leg may build, load or call it.  It
+ * shares no code, header, table or constant with the CUDA path under
+ * paper_2101_08226_b200/ and neither includes the other.
+ *
+ * What it follows (PAPER.md = arxiv 2101.08226, section 2.2):
+ *   - "variant of the Cartesian FMM described by Dehnen (2000) ... conserves linear
+ *     momentum to machine precision ... Both multipole and expansions are relative to
+ *     cell centres" (L125);
+ *   - the angular-momentum extension that "works by adding an additional higher order
+ *     multipoles which is used to calculate a correction to the calculated force" while
+ *     "preserving linear momentum conservation" (L127);
+ *   - the opening criterion, Eq. 15 (L131-135): theta' = dx/|x_A - x_B| < theta  <=>  well
+ *     separated; two cells interact here "when they are well separated from each other,
+ *     but their respective parents are not well separated";
+ *   - isolated boundary: the FMM ignores the domain boundary (L321); G = 1 (L363).
+ * The paper prints no FMM formulas (it defers to Dehnen 2000 / Marcello et al. 2016), so
+ * the formulas are the readings listed in DESIGN.md ("Readings of the paper") and
+ * SURVEY.md section 8(c), restated here step by step with FULL (non-unique) tensors:
+ *
+ *   Green's function g(R) = -1/|R| and its derivative tensors D^(n) = d^n g / dR^n,
+ *     d0=-1/r, d1=1/r^3, d2=-3/r^5, d3=15/r^7, d4=-105/r^9,
+ *     D0 = d0;  D1_i = d1 R_i;  D2_ij = d1 d_ij + d2 R_i R_j;
+ *     D3_ijk = d2 (d_ij R_k + d_ik R_j + d_jk R_i) + d3 R_i R_j R_k;
+ *     D4_ijkl = d2 (d_ij d_kl + d_ik d_jl + d_il d_jk)
+ *             + d3 (d_ij R_k R_l + d_ik R_j R_l + d_il R_j R_k + d_jk R_i R_l + d_jl R_i R_k + d_kl R_i R_j)
+ *             + d4 R_i R_j R_k R_l.
+ *   For target A and every partner B of its stencil (R = z_A - z_B, expansion centres =
+ *   centres of mass handed over as offsets delta from the geometric cell centre):
+ *     L0       += M_B D0 - M1_B.D1 + 1/2 M2_B:D2 - 1/6 M3_B:.D3
+ *     L1_i     += M_B D1_i - M1_B,j D2_ij + 1/2 M2_B,jk D3_ijk
+ *     L2_ij    += M_B D2_ij - M1_B,k D3_ijk
+ *     L3_ijk   += M_B D3_ijk                                   (truncation n + m <= 3)
+ *     correction (L127):  n3 = M3_B - (M_B/M_A) M3_A ;  dL1_i += -1/6 n3_jkl D4_ijkl
+ *   Monopole (leaf) variant: R = geometric centre difference,
+ *     phi += -m_B/|R| ;  g_i += -m_B R_i/|R|^3.
+ *
+ * Precision: every per-pair term is formed in IEEE double; the running sums over the
+ * partners are `long double` (x87 80-bit on this host) so the oracle's own summation
+ * error stays out of the 1e-12 parity budget.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): stencil counts and theta_min
+ * (L137), worked example W1, symbolic derivatives of -1/r (sympy), order-of-convergence
+ * against direct summation over point masses, Newton's third law (L125), angular-momentum
+ * conservation with the correction on and its violation with it off (L127), point-mass
+ * and uniform-sphere closed forms.  No function here is "parity unpinned".
+ *
+ * Layouts: moments [20][nz][ny][nx] (monopole: [1][nz][ny][nx]), com_off [3][nz][ny][nx],
+ * outputs SoA over the output region: L [20][oz][oy][ox], Lcorr [3][oz][oy][ox],
+ * monopole out [4][oz][oy][ox] = (phi, gx, gy, gz).  x is the fastest index.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_OK 0
+#define ORC_EINVAL 1
+#define ORC_EMASS 2
+
+/* ---------------------------------------------------------------------------------- */
+/* Opening criterion, Eq. 15 (L131-135).  Distances are in units of the cell width, so  */
+/* theta' = 1/|Delta|;  "theta' < theta"  <=>  |Delta|^2 theta^2 > 1  (strict, L135).   */
+/* ---------------------------------------------------------------------------------- */
+static int well_separated(long d2, double theta) { return (double)d2 * theta * theta > 1.0; }
+
+/* parent index of a cell index: floor(i/2), also for negative i */
+static int parent_of(int i) { return (i >= 0) ? (i / 2) : -((-i + 1) / 2); }
+
+/* Is Delta a partner of a cell with parity (px,py,pz)?  Cells well separated (L135),      */
+/* parents not well separated; a parent is never well separated from itself (Delta_I = 0). */
+static int is_partner(int px, int py, int pz, int dx, int dy, int dz, double theta)
+{
+    long d2 = (long)dx * dx + (long)dy * dy + (long)dz * dz;
+    if (d2 == 0 || !well_separated(d2, theta)) return 0;
+    int Ix = parent_of(px + dx) - parent_of(px);
+    int Iy = parent_of(py + dy) - parent_of(py);
+    int Iz = parent_of(pz + dz) - parent_of(pz);
+    long D2 = (long)Ix * Ix + (long)Iy * Iy + (long)Iz * Iz;
+    if (D2 > 0 && well_separated(D2, theta)) return 0;
+    return 1;
+}
+
+/* search range that certainly contains the stencil: parents within 1/theta parent cells */
+static int search_reach(double theta) { return 2 * (int)floor(1.0 / theta) + 3; }
+
+/* Stencil of parity class parity = px + 2 py + 4 pz, in lexicographic (dz, dy, dx) order. */
+/* dxyz receives up to cap triples (dx,dy,dz); *count is always the full count.           */
+int fmm_oracle_stencil(double theta, int parity, int cap, int *count, signed char *dxyz)
+{
+    if (!(theta > 0.0 && theta < 1.0) || parity < 0 || parity > 7 || !count) return ORC_EINVAL;
+    int px = parity & 1, py = (parity >> 1) & 1, pz = (parity >> 2) & 1;
+    int S = search_reach(theta), c = 0;
+    if (S > 127) return ORC_EINVAL;
+    for (int dz = -S; dz <= S; ++dz)
+        for (int dy = -S; dy <= S; ++dy)
+            for (int dx = -S; dx <= S; ++dx)
+                if (is_partner(px, py, pz, dx, dy, dz, theta)) {
+                    if (dxyz && c < cap) {
+                        dxyz[3 * c + 0] = (signed char)dx;
+                        dxyz[3 * c + 1] = (signed char)dy;
+                        dxyz[3 * c + 2] = (signed char)dz;
+                    }
+                    ++c;
+                }
+    *count = c;
+    return ORC_OK;
+}
+
+/* ---------------------------------------------------------------------------------- */
+/* unique <-> full tensors, lexicographic unique order                                   */
+/* ---------------------------------------------------------------------------------- */
+static void sort3(int *a, int *b, int *c)
+{
+    int t;
+    if (*a > *b) { t = *a; *a = *b; *b = t; }
+    if (*b > *c) { t = *b; *b = *c; *c = t; }
+    if (*a > *b) { t = *a; *a = *b; *b = t; }
+}
+/* position of sorted (i<=j) in [xx xy xz yy yz zz] */
+static int u2(int i, int j)
+{
+    if (i > j) { int t = i; i = j; j = t; }
+    static const int tab[3][3] = {{0, 1, 2}, {-1, 3, 4}, {-1, -1, 5}};
+    return tab[i][j];
+}
+/* position of sorted (i<=j<=k) in [xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz] */
+static int u3(int i, int j, int k)
+{
+    sort3(&i, &j, &k);
+    static const int tab[3][3][3] = {
+        {{0, 1, 2}, {-1, 3, 4}, {-1, -1, 5}},
+        {{-1, -1, -1}, {-1, 6, 7}, {-1, -1, 8}},
+        {{-1, -1, -1}, {-1, -1, -1}, {-1, -1, 9}}};
+    return tab[i][j][k];
+}
+
+static double kd(int i, int j) { return i == j ? 1.0 : 0.0; }
+
+/* Green's-function derivative tensors of g = -1/|R| (closed forms in the header).       */
+static void green_tensors(const double R[3], double *D0, double D1[3], double D2[3][3],
+                          double D3[3][3][3], double D4[3][3][3][3])
+{
+    double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2];
+    double r = sqrt(r2);
+    double d0 = -1.0 / r;
+    double d1 = 1.0 / (r2 * r);
+    double d2 = -3.0 / (r2 * r2 * r);
+    double d3 = 15.0 / (r2 * r2 * r2 * r);
+    double d4 = -105.0 / (r2 * r2 * r2 * r2 * r);
+    *D0 = d0;
+    for (int i = 0; i < 3; ++i) {
+        D1[i] = d1 * R[i];
+        for (int j = 0; j < 3; ++j) {
+            D2[i][j] = d1 * kd(i, j) + d2 * R[i] * R[j];
+            for (int k = 0; k < 3; ++k) {
+                D3[i][j][k] = d2 * (kd(i, j) * R[k] + kd(i, k) * R[j] + kd(j, k) * R[i]) + d3 * R[i] * R[j] * R[k];
+                if (D4)
+                    for (int l = 0; l < 3; ++l)
+                        D4[i][j][k][l] =
+                            d2 * (kd(i, j) * kd(k, l) + kd(i, k) * kd(j, l) + kd(i, l) * kd(j, k)) +
+                            d3 * (kd(i, j) * R[k] * R[l] + kd(i, k) * R[j] * R[l] + kd(i, l) * R[j] * R[k] +
+                                  kd(j, k) * R[i] * R[l] + kd(j, l) * R[i] * R[k] + kd(k, l) * R[i] * R[j]) +
+                            d4 * R[i] * R[j] * R[k] * R[l];
+            }
+        }
+    }
+}
+
+/* flattened export of the tensors for the symbolic-derivative pin: 1+3+9+27+81 = 121 */
+int fmm_oracle_green(const double R[3], double out[121])
+{
+    double D0, D1[3], D2[3][3], D3[3][3][3], D4[3][3][3][3];
+    if (!R || !out) return ORC_EINVAL;
+    green_tensors(R, &D0, D1, D2, D3, D4);
+    out[0] = D0;
+    memcpy(out + 1, D1, sizeof D1);
+    memcpy(out + 4, D2, sizeof D2);
+    memcpy(out + 13, D3, sizeof D3);
+    memcpy(out + 40, D4, sizeof D4);
+    return ORC_OK;
+}
+
+/* One ordered pair A <- B.  MB = 20 unique source moments; MA0, MA3 = target mass and    */
+/* unique third moments (used by the correction only).  term[20] and cterm[3] receive     */
+/* this pair's contribution, formed in double.                                            */
+static void pair_terms(const double R[3], const double MB[20], double MA0, const double MA3[10],
+                       int correction, double term[20], double cterm[3])
+{
+    double D0, D1[3], D2[3][3], D3[3][3][3], D4[3][3][3][3];
+    green_tensors(R, &D0, D1, D2, D3, correction ? D4 : NULL);
+
+    double M0 = MB[0], M1[3], M2[3][3], M3[3][3][3];
+    for (int i = 0; i < 3; ++i) {
+        M1[i] = MB[1 + i];
+        for (int j = 0; j < 3; ++j) {
+            M2[i][j] = MB[4 + u2(i, j)];
+            for (int k = 0; k < 3; ++k) M3[i][j][k] = MB[10 + u3(i, j, k)];
+        }
+    }
+
+    /* L0 += M D0 - M1.D1 + 1/2 M2:D2 - 1/6 M3:.D3 */
+    double s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    for (int i = 0; i < 3; ++i) {
+        s1 += M1[i] * D1[i];
+        for (int j = 0; j < 3; ++j) {
+            s2 += M2[i][j] * D2[i][j];
+            for (int k = 0; k < 3; ++k) s3 += M3[i][j][k] * D3[i][j][k];
+        }
+    }
+    term[0] = M0 * D0 - s1 + 0.5 * s2 - s3 / 6.0;
+
+    /* L1_i += M D1_i - M1_j D2_ij + 1/2 M2_jk D3_ijk */
+    for (int i = 0; i < 3; ++i) {
+        double a = 0.0, b = 0.0;
+        for (int j = 0; j < 3; ++j) {
+            a += M1[j] * D2[i][j];
+            for (int k = 0; k < 3; ++k) b += M2[j][k] * D3[i][j][k];
+        }
+        term[1 + i] = M0 * D1[i] - a + 0.5 * b;
+    }
+
+    /* L2_ij += M D2_ij - M1_k D3_ijk   (unique components i <= j) */
+    for (int i = 0; i < 3; ++i)
+        for (int j = i; j < 3; ++j) {
+            double a = 0.0;
+            for (int k = 0; k < 3; ++k) a += M1[k] * D3[i][j][k];
+            term[4 + u2(i, j)] = M0 * D2[i][j] - a;
+        }
+
+    /* L3_ijk += M D3_ijk   (unique components i <= j <= k) */
+    for (int i = 0; i < 3; ++i)
+        for (int j = i; j < 3; ++j)
+            for (int k = j; k < 3; ++k) term[10 + u3(i, j, k)] = M0 * D3[i][j][k];
+
+    /* correction (L127):  n3 = M3_B - (M_B/M_A) M3_A ;  dL1_i += -1/6 n3_jkl D4_ijkl */
+    cterm[0] = cterm[1] = cterm[2] = 0.0;
+    if (correction) {
+        double q = M0 / MA0;
+        for (int i = 0; i < 3; ++i) {
+            double c = 0.0;
+            for (int j = 0; j < 3; ++j)
+                for (int k = 0; k < 3; ++k)
+                    for (int l = 0; l < 3; ++l) {
+                        double n3 = M3[j][k][l] - q * MA3[u3(j, k, l)];
+                        c += n3 * D4[i][j][k][l];
+                    }
+            cterm[i] = -c / 6.0;
+        }
+    }
+}
+
+/* single ordered pair, for the worked example W1 and closed-form pins */
+int fmm_oracle_pair(const double R[3], const double MB[20], double MA0, const double MA3[10],
+                    int correction, double L[20], double dL1[3])
+{
+    if (!R || !MB || !L || !dL1) return ORC_EINVAL;
+    if (correction && (!MA3 || !(MA0 > 0.0))) return ORC_EMASS;
+    pair_terms(R, MB, MA0, MA3, correction, L, dL1);
+    return ORC_OK;
+}
+
+static int check_region(const int n[3], const int lo[3], const int hi[3])
+{
+    for (int a = 0; a < 3; ++a)
+        if (n[a] <= 0 || lo[a] < 0 || hi[a] > n[a] || lo[a] >= hi[a]) return 0;
+    return 1;
+}
+
+/* Build the 8 per-parity partner lists once. */
+typedef struct { int count[8]; signed char *d[8]; } stencil_set;
+
+static int build_stencils(double theta, stencil_set *S)
+{
+    memset(S, 0, sizeof *S);
+    for (int p = 0; p < 8; ++p) {
+        int c = 0;
+        if (fmm_oracle_stencil(theta, p, 0, &c, NULL) != ORC_OK) return ORC_EINVAL;
+        S->d[p] = (signed char *)malloc((size_t)3 * (c > 0 ? c : 1));
+        if (!S->d[p]) return ORC_EINVAL;
+        fmm_oracle_stencil(theta, p, c, &S->count[p], S->d[p]);
+    }
+    return ORC_OK;
+}
+static void free_stencils(stencil_set *S) { for (int p = 0; p < 8; ++p) free(S->d[p]); }
+
+/*
+ * The interaction step for multipole cells.
+ * For every target cell A in [out_lo, out_hi): loop over its parity class's partner list
+ * in the fixed (dz,dy,dx) order, skip partners outside the grid (isolated, L321),
+ * R_c = (double)(i_A,c - i_B,c) * h + (delta_A,c - delta_B,c), accumulate.
+ * L gets the correction folded into L1 when enabled; Lcorr (may be NULL) gets it alone.
+ * n_interactions (may be NULL) receives the number of ordered in-domain pairs.
+ */
+int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                  double theta, int am_correction, const double *moments,
+                                  const double *com_off, double *L, double *Lcorr,
+                                  unsigned long long *n_interactions)
+{
+    if (!n || !out_lo || !out_hi || !moments || !com_off || !L || !(h > 0.0)) return ORC_EINVAL;
+    if (!check_region(n, out_lo, out_hi)) return ORC_EINVAL;
+    stencil_set S;
+    if (build_stencils(theta, &S) != ORC_OK) return ORC_EINVAL;
+
+    const size_t nx = n[0], ny = n[1], nz = n[2], ncell = nx * ny * nz;
+    const size_t ox = out_hi[0] - out_lo[0], oy = out_hi[1] - out_lo[1], oz = out_hi[2] - out_lo[2];
+    const size_t ocell = ox * oy * oz;
+    unsigned long long total = 0;
+    int bad_mass = 0;
+
+#pragma omp parallel for collapse(2) schedule(dynamic, 1) reduction(+ : total) reduction(| : bad_mass)
+    for (int k = out_lo[2]; k < out_hi[2]; ++k)
+        for (int j = out_lo[1]; j < out_hi[1]; ++j)
+            for (int i = out_lo[0]; i < out_hi[0]; ++i) {
+                const size_t a = ((size_t)k * ny + j) * nx + i;
+                const int p = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
+                long double acc[20], cacc[3] = {0.0L, 0.0L, 0.0L};
+                for (int c = 0; c < 20; ++c) acc[c] = 0.0L;
+                double MA3[10], MA0 = moments[a], dA[3];
+                for (int c = 0; c < 10; ++c) MA3[c] = moments[(size_t)(10 + c) * ncell + a];
+                for (int c = 0; c < 3; ++c) dA[c] = com_off[(size_t)c * ncell + a];
+                if (am_correction && !(MA0 > 0.0)) bad_mass |= 1;
+
+                for (int s = 0; s < S.count[p]; ++s) {
+                    const int dx = S.d[p][3 * s], dy = S.d[p][3 * s + 1], dz = S.d[p][3 * s + 2];
+                    const int bi = i + dx, bj = j + dy, bk = k + dz;
+                    if (bi < 0 || bj < 0 || bk < 0 || bi >= (int)nx || bj >= (int)ny || bk >= (int)nz) continue;
+                    const size_t b = ((size_t)bk * ny + bj) * nx + bi;
+                    double MB[20], R[3], term[20], cterm[3];
+                    for (int c = 0; c < 20; ++c) MB[c] = moments[(size_t)c * ncell + b];
+                    R[0] = (double)(i - bi) * h + (dA[0] - com_off[0 * ncell + b]);
+                    R[1] = (double)(j - bj) * h + (dA[1] - com_off[1 * ncell + b]);
+                    R[2] = (double)(k - bk) * h + (dA[2] - com_off[2 * ncell + b]);
+                    pair_terms(R, MB, MA0, MA3, am_correction && MA0 > 0.0, term, cterm);
+                    for (int c = 0; c < 20; ++c) acc[c] += (long double)term[c];
+                    for (int c = 0; c < 3; ++c) cacc[c] += (long double)cterm[c];
+                    ++total;
+                }
+                const size_t o = ((size_t)(k - out_lo[2]) * oy + (j - out_lo[1])) * ox + (i - out_lo[0]);
+                if (am_correction)
+                    for (int c = 0; c < 3; ++c) acc[1 + c] += cacc[c];
+                for (int c = 0; c < 20; ++c) L[(size_t)c * ocell + o] = (double)acc[c];
+                if (Lcorr)
+                    for (int c = 0; c < 3; ++c) Lcorr[(size_t)c * ocell + o] = (double)cacc[c];
+            }
+    free_stencils(&S);
+    if (n_interactions) *n_interactions = total;
+    return bad_mass ? ORC_EMASS : ORC_OK;
+}
+
+/*
+ * Monopole (leaf) variant (BASELINE.json config 4): every cell is the
+ * point mass m at its geometric centre; the same stencil; G = 1 (L363):
+ *   phi_A = -sum_B m_B/|R| ,  g_A = -sum_B m_B R/|R|^3 ,  R = x_A - x_B = (i_A - i_B) h.
+ * out = [4][oz][oy][ox] = (phi, gx, gy, gz).
+ */
+int fmm_oracle_interact_monopole(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                 double theta, const double *mass, double *out,
+                                 unsigned long long *n_interactions)
+{
+    if (!n || !out_lo || !out_hi || !mass || !out || !(h > 0.0)) return ORC_EINVAL;
+    if (!check_region(n, out_lo, out_hi)) return ORC_EINVAL;
+    stencil_set S;
+    if (build_stencils(theta, &S) != ORC_OK) return ORC_EINVAL;
+    const size_t nx = n[0], ny = n[1], nz = n[2];
+    const size_t ox = out_hi[0] - out_lo[0], oy = out_hi[1] - out_lo[1], oz = out_hi[2] - out_lo[2];
+    const size_t ocell = ox * oy * oz;
+    unsigned long long total = 0;
+
+#pragma omp parallel for collapse(2) schedule(dynamic, 1) reduction(+ : total)
+    for (int k = out_lo[2]; k < out_hi[2]; ++k)
+        for (int j = out_lo[1]; j < out_hi[1]; ++j)
+            for (int i = out_lo[0]; i < out_hi[0]; ++i) {
+                const int p = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
+                long double acc[4] = {0.0L, 0.0L, 0.0L, 0.0L};
+                for (int s = 0; s < S.count[p]; ++s) {
+                    const int bi = i + S.d[p][3 * s], bj = j + S.d[p][3 * s + 1], bk = k + S.d[p][3 * s + 2];
+                    if (bi < 0 || bj < 0 || bk < 0 || bi >= (int)nx || bj >= (int)ny || bk >= (int)nz) continue;
+                    const double m = mass[((size_t)bk * ny + bj) * nx + bi];
+                    double R[3] = {(double)(i - bi) * h, (double)(j - bj) * h, (double)(k - bk) * h};
+                    double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2];
+                    double r = sqrt(r2);
+                    acc[0] += (long double)(-m / r);
+                    for (int c = 0; c < 3; ++c) acc[1 + c] += (long double)(-m * R[c] / (r2 * r));
+                    ++total;
+                }
+                const size_t o = ((size_t)(k - out_lo[2]) * oy + (j - out_lo[1])) * ox + (i - out_lo[0]);
+                for (int c = 0; c < 4; ++c) out[(size_t)c * ocell + o] = (double)acc[c];
+            }
+    free_stencils(&S);
+    if (n_interactions) *n_interactions = total;
+    return ORC_OK;
+}
+
+/* Number of ordered in-domain pairs for a region, by enumeration on the index grid. */
+int fmm_oracle_interaction_count(const int n[3], const int out_lo[3], const int out_hi[3], double theta,
+                                 unsigned long long *count)
+{
+    if (!n || !out_lo || !out_hi || !count || !check_region(n, out_lo, out_hi)) return ORC_EINVAL;
+    stencil_set S;
+    if (build_stencils(theta, &S) != ORC_OK) return ORC_EINVAL;
+    unsigned long long total = 0;
+#pragma omp parallel for collapse(2) reduction(+ : total)
+    for (int k = out_lo[2]; k < out_hi[2]; ++k)
+        for (int j = out_lo[1]; j < out_hi[1]; ++j)
+            for (int i = out_lo[0]; i < out_hi[0]; ++i) {
+                const int p = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
+                for (int s = 0; s < S.count[p]; ++s) {
+                    const int bi = i + S.d[p][3 * s], bj = j + S.d[p][3 * s + 1], bk = k + S.d[p][3 * s + 2];
+                    if (bi < 0 || bj < 0 || bk < 0 || bi >= n[0] || bj >= n[1] || bk >= n[2]) continue;
+                    ++total;
+                }
+            }
+    free_stencils(&S);
+    *count = total;
+    return ORC_OK;
+}
+
+int fmm_oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void fmm_oracle_set_num_threads(int t)
+{
+#ifdef _OPENMP
+    if (t > 0) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}

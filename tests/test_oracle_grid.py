@@ -1,0 +1,188 @@
+"""Grid-level pins of the oracle -- CPU only.
+
+Expected values are fixed by the paper's statements, not by the oracle:
+  * "conserves linear momentum to machine precision"  -> sum_A F_A = 0;
+  * with the correction "conserve both angular and linear momentum to machine precision" (L127),
+    visibly violated without it (L670, Fig. 12)                        -> sum_A T_A = 0 on / != 0 off;
+  * the expansion approximates the direct sum over the constituents of the same partner set to
+    the truncation error of an order-3 FMM                            -> brute force on tiny grids;
+  * isolated boundary (L321): partners outside the grid contribute nothing.
+"""
+import numpy as np
+import pytest
+
+import fmm_inputs as fi
+import oracle
+from helpers import cell_forces_and_torques
+
+
+def _closed(ncell, theta, seed=11, correction=True):
+    w = fi.config1(seed=seed, theta=theta, ncell=ncell)
+    L, Lc, cnt = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, am_correction=correction)
+    return w, L, Lc, cnt
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.35, 0.7])
+def test_newtons_third_law(theta):
+    w, L, Lc, _ = _closed(12, theta)
+    F, _ = cell_forces_and_torques(w.moments, w.com_off, L, w.h)
+    rel = np.abs(F.sum(axis=(1, 2, 3))).max() / np.abs(F).sum()
+    assert rel < 2e-15, rel
+    # also without the correction: the base method already conserves linear momentum (L125)
+    w, L0, _, _ = _closed(12, theta, correction=False)
+    F0, _ = cell_forces_and_torques(w.moments, w.com_off, L0, w.h)
+    assert np.abs(F0.sum(axis=(1, 2, 3))).max() / np.abs(F0).sum() < 2e-15
+    np.testing.assert_allclose(L[1:4] - Lc, L0[1:4], rtol=0, atol=1e-15 * np.abs(L0[1:4]).max())
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.35, 0.7])
+def test_angular_momentum_with_and_without_correction(theta):
+    w, L, _, _ = _closed(12, theta, correction=True)
+    F, T = cell_forces_and_torques(w.moments, w.com_off, L, w.h)
+    scale = np.abs(np.cross(np.stack(np.meshgrid(*[np.arange(12) * w.h] * 3, indexing="ij")), F, axis=0)).sum()
+    on = np.abs(T.sum(axis=(1, 2, 3))).max() / scale
+    w, L0, _, _ = _closed(12, theta, correction=False)
+    _, T0 = cell_forces_and_torques(w.moments, w.com_off, L0, w.h)
+    off = np.abs(T0.sum(axis=(1, 2, 3))).max() / scale
+    assert on < 5e-15, on
+    assert off > 1e-9, off            # the test is sensitive: the uncorrected method does violate it
+    assert off > 1e4 * on
+
+
+def test_polytrope_field_conservation():
+    """Same invariants on the polytrope-shaped field of config 2 (reduced to 16^3 for the CPU)."""
+    w = fi.config2(ncell=16)
+    L, _, cnt = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off)
+    assert cnt == oracle.interaction_count(w.n, 0.5)
+    F, T = cell_forces_and_torques(w.moments, w.com_off, L, w.h)
+    assert np.abs(F.sum(axis=(1, 2, 3))).max() / np.abs(F).sum() < 2e-15
+    assert np.abs(T.sum(axis=(1, 2, 3))).max() / np.abs(T).sum() < 5e-14
+
+
+def _direct_over_children(w, theta, targets):
+    """phi and grad phi at z_A from the CHILD point masses of the same partner set."""
+    nx, ny, nz = w.n
+    h = w.h
+    q = 0.25 * h
+    out = {}
+    for (i, j, k) in targets:
+        p = (i & 1) + 2 * (j & 1) + 4 * (k & 1)
+        zA = (np.array([i, j, k]) + 0.5) * h + w.com_off[:, k, j, i]
+        phi, grad = 0.0, np.zeros(3)
+        for dx, dy, dz in oracle.stencil(theta, p).astype(int):
+            bi, bj, bk = i + dx, j + dy, k + dz
+            if not (0 <= bi < nx and 0 <= bj < ny and 0 <= bk < nz):
+                continue
+            xc = (np.array([bi, bj, bk]) + 0.5) * h
+            for c in range(8):
+                y = xc + fi.CHILD_SIGNS[c] * q
+                m = w.child_mass[c, bk, bj, bi]
+                R = zA - y
+                r = np.linalg.norm(R)
+                phi += -m / r
+                grad += m * R / r ** 3
+        out[(i, j, k)] = (phi, grad)
+    return out
+
+
+@pytest.mark.parametrize("theta,tol0,tol1", [(0.5, 6e-5, 5e-3), (0.35, 3e-5, 3e-3), (0.7, 4e-4, 2e-2)])
+def test_brute_force_over_constituents(theta, tol0, tol1):
+    """P8: L0, L1 against the direct sum over the partners' child masses (truncation error only)."""
+    w = fi.config1(seed=5, theta=theta, ncell=12)
+    L, _, _ = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, am_correction=False)
+    targets = [(0, 0, 0), (5, 6, 7), (6, 5, 4), (11, 3, 8), (4, 4, 4), (7, 7, 7)]
+    ref = _direct_over_children(w, theta, targets)
+    e0 = max(abs(L[0, k, j, i] - ref[(i, j, k)][0]) / abs(ref[(i, j, k)][0]) for (i, j, k) in targets)
+    gmax = max(np.abs(ref[t][1]).max() for t in targets)
+    e1 = max(np.abs(L[1:4, k, j, i] - ref[(i, j, k)][1]).max() for (i, j, k) in targets) / gmax
+    assert e0 < tol0, e0
+    assert e1 < tol1, e1
+    assert e0 > 1e-9      # it IS a truncated expansion, not the exact sum
+
+
+def test_error_falls_as_orders_are_switched_on():
+    """P8 (second half): monopole-only sources -> +M2 -> +M3 must reduce the L0 error."""
+    theta = 0.5
+    w = fi.config1(seed=5, theta=theta, ncell=12)
+    targets = [(5, 6, 7), (6, 5, 4), (4, 4, 4), (7, 7, 7), (2, 9, 6)]
+    ref = _direct_over_children(w, theta, targets)
+    errs = []
+    for keep in (1, 10, 20):
+        mom = w.moments.copy()
+        mom[keep:] = 0.0
+        L, _, _ = oracle.interact_multipole(w.n, w.h, theta, mom, w.com_off, am_correction=False)
+        errs.append(max(abs(L[0, k, j, i] - ref[(i, j, k)][0]) / abs(ref[(i, j, k)][0]) for (i, j, k) in targets))
+    assert errs[0] > errs[1] > errs[2], errs
+
+
+def test_isolated_boundary_and_output_region():
+    """L321: the solve ignores everything outside the grid.  Embedding the grid in a larger one
+    filled with zero-mass cells must not change any coefficient; and an output sub-region equals
+    the corresponding slice of the full result."""
+    w = fi.config1(seed=2, ncell=8, out_lo=(0, 0, 0), out_hi=(8, 8, 8))
+    L, Lc, cnt = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off)
+    big_m = np.zeros((20, 24, 24, 24))
+    big_c = np.zeros((3, 24, 24, 24))
+    big_m[:, 8:16, 8:16, 8:16] = w.moments
+    big_c[:, 8:16, 8:16, 8:16] = w.com_off
+    Lb, Lcb, cntb = oracle.interact_multipole((24, 24, 24), w.h, 0.5, big_m, big_c, (8, 8, 8), (16, 16, 16))
+    assert cntb == 118272 and cnt < cntb
+    np.testing.assert_allclose(Lb, L, rtol=0, atol=1e-15 * np.abs(L).max())
+    np.testing.assert_allclose(Lcb, Lc, rtol=0, atol=1e-15 * np.abs(Lc).max())
+    Ls, _, _ = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off, (0, 0, 2), (8, 8, 6))
+    np.testing.assert_array_equal(Ls, L[:, 2:6])
+
+
+def test_scaling_and_mass_ratio_consistency():
+    """P10: doubling every mass doubles L and Lcorr (the ratio M_B/M_A is unchanged)."""
+    w = fi.config1(seed=9, ncell=8, out_lo=(0, 0, 0), out_hi=(8, 8, 8))
+    L, Lc, _ = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off)
+    L2, Lc2, _ = oracle.interact_multipole(w.n, w.h, 0.5, 2.0 * w.moments, w.com_off)
+    np.testing.assert_allclose(L2, 2.0 * L, rtol=1e-15)
+    np.testing.assert_allclose(Lc2, 2.0 * Lc, rtol=1e-15)
+
+
+def test_correction_needs_positive_target_mass():
+    w = fi.config1(seed=9, ncell=8, out_lo=(0, 0, 0), out_hi=(8, 8, 8))
+    mom = w.moments.copy()
+    mom[0, 3, 3, 3] = 0.0
+    with pytest.raises(RuntimeError):
+        oracle.interact_multipole(w.n, w.h, 0.5, mom, w.com_off, am_correction=True)
+    oracle.interact_multipole(w.n, w.h, 0.5, mom, w.com_off, am_correction=False)
+
+
+# ------------------------------------------------------------------ monopole variant
+def test_monopole_matches_plain_direct_sum():
+    """Config-4 kernel against numpy: phi = -sum m/|R|, g = -sum m R/|R|^3 over the stencil."""
+    rng = np.random.default_rng(1)
+    n, h, theta = 10, 0.1, 0.5
+    mass = rng.uniform(0.5, 1.5, (n, n, n))
+    out, cnt = oracle.interact_monopole((n, n, n), h, theta, mass)
+    assert cnt == oracle.interaction_count((n, n, n), theta)
+    for (i, j, k) in [(0, 0, 0), (4, 5, 6), (9, 2, 7), (5, 5, 5)]:
+        p = (i & 1) + 2 * (j & 1) + 4 * (k & 1)
+        phi, g = 0.0, np.zeros(3)
+        for dx, dy, dz in oracle.stencil(theta, p).astype(int):
+            bi, bj, bk = i + dx, j + dy, k + dz
+            if 0 <= bi < n and 0 <= bj < n and 0 <= bk < n:
+                R = -np.array([dx, dy, dz]) * h
+                r = np.linalg.norm(R)
+                phi -= mass[bk, bj, bi] / r
+                g -= mass[bk, bj, bi] * R / r ** 3
+        np.testing.assert_allclose(out[0, k, j, i], phi, rtol=1e-14)
+        np.testing.assert_allclose(out[1:4, k, j, i], g, rtol=0, atol=1e-14 * np.abs(out[1:4]).max())
+
+
+def test_monopole_zero_net_force_and_multipole_limit():
+    """sum m_A g_A = 0 to machine precision (config 4's check); and the multipole entry point with
+    pure monopoles at the geometric centres gives L0 = phi, L1 = -g."""
+    w = fi.config4(ncell=16)
+    mass = w.moments[0]
+    out, _ = oracle.interact_monopole(w.n, w.h, 0.5, mass)
+    tot = (mass[None] * out[1:4]).sum(axis=(1, 2, 3))
+    assert np.abs(tot).max() / np.abs(mass[None] * out[1:4]).sum() < 2e-15
+    mom = np.zeros((20,) + mass.shape)
+    mom[0] = mass
+    L, _, _ = oracle.interact_multipole(w.n, w.h, 0.5, mom, np.zeros((3,) + mass.shape), am_correction=False)
+    np.testing.assert_allclose(L[0], out[0], rtol=1e-14)
+    np.testing.assert_allclose(-L[1:4], out[1:4], rtol=0, atol=1e-14 * np.abs(out[1:4]).max())
