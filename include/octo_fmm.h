@@ -1,0 +1,136 @@
+/*
+ * octo_fmm.h -- C ABI of the B200-native FMM cell-to-cell interaction step.
+ *
+ * The operation (PAPER.md = arxiv 2101.08226, section 2.2 "Gravity Update and the Angular
+ * Momentum Correction", L123-139): on a uniform level of cells grouped in 8x8x8 sub-grids
+ * (L287), every cell A accumulates an order-3 local Taylor expansion of the potential
+ * (20 FP64 coefficients) from the order-3 multipole moments (20 FP64 components) of every
+ * same-level cell B that is well separated from A while their parents are not (opening
+ * criterion, Eq. 15), plus the angular-momentum-conserving correction (L127) and
+ * the monopole (leaf) variant.  Domain is isolated (L321), G = 1 (L363).  The formulas the
+ * paper defers to Dehnen (2000) / Marcello et al. (2016) are restated in DESIGN.md.
+ *
+ * Conventions
+ *   - cell index (i,j,k), x fastest; geometric centre x = origin + (i + 1/2) h.
+ *   - moments: raw Cartesian moments about the cell's expansion centre z = x + delta,
+ *       M^(n) = sum_p m_p (y_p - z)^{(x)n}, n = 0..3, 20 unique components in the order
+ *       [0] [x y z] [xx xy xz yy yz zz] [xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz],
+ *       no factorials or multiplicities folded in;  layout [20][nz][ny][nx] (SoA).
+ *   - com_off: delta = z - x_cell, layout [3][nz][ny][nx]; |delta_c| <= h/2.
+ *   - expansions: L^(n) = d^n phi / dx^n at z_A, same 20-slot order, layout
+ *       [20][oz][oy][ox] over the output region; with am_correction the correction is folded
+ *       into L^(1); Lcorr [3][oz][oy][ox] returns it alone.
+ *   - monopole kind: moments = mass [1][nz][ny][nx] at the geometric centres, output
+ *       [4][oz][oy][ox] = (phi, g_x, g_y, g_z),  phi = -sum m/|R|,  g = -sum m R/|R|^3.
+ *   - pair separation, in this operation order:
+ *       R_c = (double)(i_A,c - i_B,c) * h + (delta_A,c - delta_B,c).
+ *
+ * Memory and ownership: every pointer marked "device" is device memory on cfg.device owned by
+ * the caller; the library never allocates or frees device memory (the caller lends it a
+ * workspace) and never synchronises the stream except in octo_fmm_destroy and
+ * octo_fmm_status.  All work is enqueued on cfg.stream (a cudaStream_t).  Inputs may be reused
+ * by the caller once the stream has passed set_moments; outputs are complete once the stream
+ * has passed get_expansions.  A handle is not thread-safe.  Handles that share a device share
+ * the stencil table in constant memory: use them on one stream (or serialise them).
+ *
+ * Errors: every call returns an OCTO_FMM_* status; nothing throws or aborts.
+ * There is no CPU fallback: without a usable CUDA device create() fails with OCTO_FMM_ECUDA.
+ */
+#ifndef OCTO_FMM_H
+#define OCTO_FMM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct octo_fmm octo_fmm_t; /* opaque handle */
+
+enum { OCTO_FMM_OK = 0, OCTO_FMM_EINVAL = 1, OCTO_FMM_ESTATE = 2, OCTO_FMM_ENOMEM = 3, OCTO_FMM_ECUDA = 4,
+       OCTO_FMM_EMASS = 5 /* am_correction with a target cell of mass <= 0 (division M_B/M_A, L127) */ };
+enum { OCTO_FMM_MULTIPOLE = 0, OCTO_FMM_MONOPOLE = 1 };
+
+typedef struct {
+    int n[3];                  /* cells per axis (x,y,z), each a positive multiple of 8 (8^3 sub-grids, L287) */
+    int out_lo[3], out_hi[3];  /* target region in cells, 8-aligned; lo = hi = 0 -> the whole grid           */
+    double h;                  /* cell width                                                                  */
+    double origin[3];          /* lower corner of the grid (kept for the caller; results do not depend on it) */
+    double theta;              /* opening angle, 1/3 < theta < 1: halo reach <= 5 cells (theta_min, L137)     */
+    int kind;                  /* OCTO_FMM_MULTIPOLE | OCTO_FMM_MONOPOLE                                      */
+    int am_correction;         /* 0/1, ignored for MONOPOLE                                                   */
+    int device;                /* CUDA device ordinal                                                         */
+    void *stream;              /* cudaStream_t, borrowed                                                      */
+    void *workspace;           /* device memory, 256-byte aligned, borrowed for the handle's lifetime         */
+    size_t workspace_bytes;    /* >= octo_fmm_workspace_bytes(cfg)                                            */
+} octo_fmm_config;
+
+/* Bytes of device workspace a handle for this configuration needs (0 on invalid configuration). */
+size_t octo_fmm_workspace_bytes(const octo_fmm_config *cfg);
+
+/* Builds the 8 per-parity interaction lists from Eq. 15 (L131-135) on the host and the TMA
+ * descriptors of the workspace; no device allocation.  EINVAL: bad sizes / theta / NULL /
+ * workspace too small or misaligned.  ECUDA: no usable device. */
+int octo_fmm_create(const octo_fmm_config *cfg, octo_fmm_t **out);
+
+/* Stage the sources: re-lays the caller's moments into the workspace
+ * (asynchronously, on the stream).  moments: device, [20][nz][ny][nx] (MONOPOLE: [1][nz][ny][nx]);
+ * com_off: device, [3][nz][ny][nx] (NULL for MONOPOLE, or for offset 0). */
+int octo_fmm_set_moments(octo_fmm_t *h, const double *moments, const double *com_off);
+
+/* The interaction step (a3-a5), asynchronous on the stream.  ESTATE before set_moments. */
+int octo_fmm_interact(octo_fmm_t *h);
+
+/* Copy the results out (a6), asynchronous on the stream.  L: device, [20] (MONOPOLE: [4]) x
+ * out cells; Lcorr: device, [3] x out cells, or NULL.  ESTATE before interact. */
+int octo_fmm_get_expansions(octo_fmm_t *h, double *L, double *Lcorr);
+
+/* Synchronises the stream and releases the handle (not the workspace). */
+int octo_fmm_destroy(octo_fmm_t *h);
+
+/* ---- auxiliary ------------------------------------------------------------------------- */
+
+/* Interaction list of parity class parity = px + 2 py + 4 pz, in (dz,dy,dx)-lexicographic order.
+ * *count receives the list length; dxyz (may be NULL) must hold that many (dx,dy,dz) triples. */
+int octo_fmm_get_stencil(const octo_fmm_t *h, int parity, int *count, signed char (*dxyz)[3]);
+
+/* Number of ordered in-domain (A,B) pairs one interact() evaluates (out-of-grid partners are
+ * skipped: isolated boundary, L321). */
+int octo_fmm_interaction_count(const octo_fmm_t *h, unsigned long long *n);
+
+/* Synchronises the stream and reports device-side conditions of the last interact():
+ * OCTO_FMM_EMASS if am_correction met a target mass <= 0, ECUDA on a CUDA error, else OK. */
+int octo_fmm_status(octo_fmm_t *h);
+
+/* Whole step with HOST buffers (pinned or pageable): H2D of moments/com_off into
+ * scratch, set_moments, interact, get_expansions, D2H of L (and Lcorr if non-NULL), then a stream
+ * synchronise.  scratch: device, >= octo_fmm_host_scratch_bytes(cfg) bytes, borrowed for the call. */
+size_t octo_fmm_host_scratch_bytes(const octo_fmm_config *cfg);
+int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *com_off_host,
+                      double *L_host, double *Lcorr_host, void *scratch, size_t scratch_bytes);
+
+/* Kernel selection, for tests and profiling: "kernel" = 0 staged (TMA + shared memory, default),
+ * 1 direct (global-memory loads; same pair arithmetic).  Unknown keys -> EINVAL. */
+int octo_fmm_set_option(octo_fmm_t *h, const char *key, int value);
+
+/* Launch facts of the interaction kernel the handle would run: grid, block, dynamic shared
+ * memory bytes, registers per thread, number of kernels launched per interact(). */
+int octo_fmm_launch_info(const octo_fmm_t *h, int *grid, int *block, int *smem_bytes, int *regs,
+                         int *launches_per_interact);
+
+/* FP64 ALU roofline probe: runs `iters` dependent-free DFMA chains on every SM of the device and
+ * returns the measured FP64 FLOP/s (2 per DFMA), SM count and SM clock (kHz, device attribute).
+ * scratch: device, >= 8 * 1024 * 1024 bytes. */
+int octo_fmm_fp64_peak_probe(int device, void *stream, void *scratch, int iters, double *flops_per_s,
+                             int *sm_count, int *clock_khz);
+
+/* FP64 operations one multipole (kind 0) / monopole (kind 1) interaction executes in the kernel's
+ * inner loop, counted from its operation list (DFMA = 2, DADD/DMUL = 1); see DESIGN.md. */
+int octo_fmm_flops_per_interaction(int kind, int am_correction, int *flops, int *fp64_instructions);
+
+const char *octo_fmm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OCTO_FMM_H */

@@ -1,0 +1,268 @@
+"""Python binding of the octo_fmm C ABI (include/octo_fmm.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libocto_fmm.so; PyTorch provides device
+memory and the stream.  There is no CPU fallback: if the shared library is missing, importing
+this package raises.  Build it with `python -m paper_2101_08226_b200.build` (or
+`__graft_entry__.build()`).
+
+The module-level functions carry the C names (octo_fmm_create, ...); `OctoFMM` is a small
+convenience wrapper that owns the workspace tensor.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libocto_fmm.so")
+
+OK, EINVAL, ESTATE, ENOMEM, ECUDA, EMASS = 0, 1, 2, 3, 4, 5
+MULTIPOLE, MONOPOLE = 0, 1
+_STATUS = {0: "OK", 1: "EINVAL", 2: "ESTATE", 3: "ENOMEM", 4: "ECUDA", 5: "EMASS"}
+
+
+class OctoFmmError(RuntimeError):
+    def __init__(self, call, status):
+        super().__init__("%s failed: OCTO_FMM_%s (%d)" % (call, _STATUS.get(status, "?"), status))
+        self.status = status
+
+
+class octo_fmm_config(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int * 3), ("out_lo", ctypes.c_int * 3), ("out_hi", ctypes.c_int * 3),
+                ("h", ctypes.c_double), ("origin", ctypes.c_double * 3), ("theta", ctypes.c_double),
+                ("kind", ctypes.c_int), ("am_correction", ctypes.c_int), ("device", ctypes.c_int),
+                ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
+
+
+if not os.path.exists(_LIB_PATH):
+    raise ImportError("paper_2101_08226_b200: %s is missing -- build it with "
+                      "`python -m paper_2101_08226_b200.build`; there is no CPU fallback" % _LIB_PATH)
+_lib = ctypes.CDLL(_LIB_PATH)
+
+_vp, _ip, _dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)
+_cfgp = ctypes.POINTER(octo_fmm_config)
+_lib.octo_fmm_workspace_bytes.restype = ctypes.c_size_t
+_lib.octo_fmm_workspace_bytes.argtypes = [_cfgp]
+_lib.octo_fmm_host_scratch_bytes.restype = ctypes.c_size_t
+_lib.octo_fmm_host_scratch_bytes.argtypes = [_cfgp]
+_lib.octo_fmm_create.argtypes = [_cfgp, ctypes.POINTER(_vp)]
+_lib.octo_fmm_set_moments.argtypes = [_vp, _vp, _vp]
+_lib.octo_fmm_interact.argtypes = [_vp]
+_lib.octo_fmm_get_expansions.argtypes = [_vp, _vp, _vp]
+_lib.octo_fmm_destroy.argtypes = [_vp]
+_lib.octo_fmm_get_stencil.argtypes = [_vp, ctypes.c_int, _ip, _vp]
+_lib.octo_fmm_interaction_count.argtypes = [_vp, ctypes.POINTER(ctypes.c_ulonglong)]
+_lib.octo_fmm_status.argtypes = [_vp]
+_lib.octo_fmm_run_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_size_t]
+_lib.octo_fmm_set_option.argtypes = [_vp, ctypes.c_char_p, ctypes.c_int]
+_lib.octo_fmm_launch_info.argtypes = [_vp, _ip, _ip, _ip, _ip, _ip]
+_lib.octo_fmm_fp64_peak_probe.argtypes = [ctypes.c_int, _vp, _vp, ctypes.c_int, _dp, _ip, _ip]
+_lib.octo_fmm_flops_per_interaction.argtypes = [ctypes.c_int, ctypes.c_int, _ip, _ip]
+_lib.octo_fmm_version.restype = ctypes.c_char_p
+
+
+def _ptr(t):
+    """Device/host address of a torch tensor or numpy array (or None)."""
+    if t is None:
+        return None
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def make_config(n, h, theta, kind=MULTIPOLE, am_correction=True, out_lo=(0, 0, 0), out_hi=(0, 0, 0),
+                origin=(0.0, 0.0, 0.0), device=0, stream=0, workspace=0, workspace_bytes=0):
+    c = octo_fmm_config()
+    for a in range(3):
+        c.n[a], c.out_lo[a], c.out_hi[a], c.origin[a] = int(n[a]), int(out_lo[a]), int(out_hi[a]), float(origin[a])
+    c.h, c.theta, c.kind, c.am_correction = float(h), float(theta), int(kind), int(bool(am_correction))
+    c.device, c.stream, c.workspace, c.workspace_bytes = int(device), stream or None, workspace or None, int(workspace_bytes)
+    return c
+
+
+# ---- the C ABI, same names ----------------------------------------------------------------
+def octo_fmm_version():
+    return _lib.octo_fmm_version().decode()
+
+
+def octo_fmm_workspace_bytes(cfg):
+    return int(_lib.octo_fmm_workspace_bytes(ctypes.byref(cfg)))
+
+
+def octo_fmm_host_scratch_bytes(cfg):
+    return int(_lib.octo_fmm_host_scratch_bytes(ctypes.byref(cfg)))
+
+
+def octo_fmm_create(cfg):
+    h = _vp()
+    rc = _lib.octo_fmm_create(ctypes.byref(cfg), ctypes.byref(h))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_create", rc)
+    return h
+
+
+def octo_fmm_set_moments(h, moments, com_off=None):
+    rc = _lib.octo_fmm_set_moments(h, _ptr(moments), _ptr(com_off))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_set_moments", rc)
+
+
+def octo_fmm_interact(h):
+    rc = _lib.octo_fmm_interact(h)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_interact", rc)
+
+
+def octo_fmm_get_expansions(h, L, Lcorr=None):
+    rc = _lib.octo_fmm_get_expansions(h, _ptr(L), _ptr(Lcorr))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_get_expansions", rc)
+
+
+def octo_fmm_destroy(h):
+    rc = _lib.octo_fmm_destroy(h)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_destroy", rc)
+
+
+def octo_fmm_status(h):
+    return int(_lib.octo_fmm_status(h))
+
+
+def octo_fmm_get_stencil(h, parity):
+    import numpy as np
+    cnt = ctypes.c_int(0)
+    rc = _lib.octo_fmm_get_stencil(h, int(parity), ctypes.byref(cnt), None)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_get_stencil", rc)
+    out = np.zeros((cnt.value, 3), dtype=np.int8)
+    rc = _lib.octo_fmm_get_stencil(h, int(parity), ctypes.byref(cnt), out.ctypes.data)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_get_stencil", rc)
+    return out
+
+
+def octo_fmm_interaction_count(h):
+    n = ctypes.c_ulonglong(0)
+    rc = _lib.octo_fmm_interaction_count(h, ctypes.byref(n))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_interaction_count", rc)
+    return int(n.value)
+
+
+def octo_fmm_run_host(h, moments_host, com_off_host, L_host, Lcorr_host, scratch, scratch_bytes):
+    rc = _lib.octo_fmm_run_host(h, _ptr(moments_host), _ptr(com_off_host), _ptr(L_host), _ptr(Lcorr_host),
+                                _ptr(scratch), int(scratch_bytes))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_run_host", rc)
+
+
+def octo_fmm_set_option(h, key, value):
+    rc = _lib.octo_fmm_set_option(h, key.encode(), int(value))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_set_option", rc)
+
+
+def octo_fmm_launch_info(h):
+    v = [ctypes.c_int(0) for _ in range(5)]
+    rc = _lib.octo_fmm_launch_info(h, *[ctypes.byref(x) for x in v])
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_launch_info", rc)
+    return dict(zip(("grid", "block", "smem_bytes", "regs", "launches_per_interact"), [x.value for x in v]))
+
+
+def octo_fmm_fp64_peak_probe(device, stream, scratch, iters=20000):
+    f, sm, clk = ctypes.c_double(0), ctypes.c_int(0), ctypes.c_int(0)
+    rc = _lib.octo_fmm_fp64_peak_probe(int(device), stream or None, _ptr(scratch), int(iters), ctypes.byref(f),
+                                       ctypes.byref(sm), ctypes.byref(clk))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_fp64_peak_probe", rc)
+    return {"flops_per_s": f.value, "sm_count": sm.value, "clock_khz": clk.value}
+
+
+def octo_fmm_flops_per_interaction(kind, am_correction):
+    f, i = ctypes.c_int(0), ctypes.c_int(0)
+    rc = _lib.octo_fmm_flops_per_interaction(int(kind), int(bool(am_correction)), ctypes.byref(f), ctypes.byref(i))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_flops_per_interaction", rc)
+    return f.value, i.value
+
+
+# ---- convenience wrapper ---------------------------------------------------------------------
+class OctoFMM:
+    """Owns a workspace tensor and a handle.  Tensors are torch CUDA float64, SoA as in octo_fmm.h."""
+
+    def __init__(self, n, h, theta, kind=MULTIPOLE, am_correction=True, out_lo=(0, 0, 0), out_hi=(0, 0, 0),
+                 device=0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("octo_fmm needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.kind = kind
+        self.n = tuple(int(v) for v in n)
+        whole = all(v == 0 for v in tuple(out_lo) + tuple(out_hi))
+        self.out_lo = (0, 0, 0) if whole else tuple(out_lo)
+        self.out_hi = self.n if whole else tuple(out_hi)
+        cfg = make_config(n, h, theta, kind, am_correction, out_lo, out_hi, device=device,
+                          stream=self.stream.cuda_stream)
+        nbytes = octo_fmm_workspace_bytes(cfg)
+        if nbytes == 0:
+            raise OctoFmmError("octo_fmm_workspace_bytes", EINVAL)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        cfg.workspace, cfg.workspace_bytes = self.workspace.data_ptr(), nbytes
+        self.cfg = cfg
+        self.handle = octo_fmm_create(cfg)
+
+    @property
+    def out_shape(self):
+        o = [self.out_hi[a] - self.out_lo[a] for a in range(3)]
+        return (o[2], o[1], o[0])
+
+    def set_moments(self, moments, com_off=None):
+        octo_fmm_set_moments(self.handle, moments, com_off)
+
+    def interact(self):
+        octo_fmm_interact(self.handle)
+
+    def get_expansions(self, L=None, Lcorr=None, want_corr=True):
+        torch = self.torch
+        ncoef = 20 if self.kind == MULTIPOLE else 4
+        if L is None:
+            L = torch.empty((ncoef,) + self.out_shape, dtype=torch.float64, device=self.device)
+        if Lcorr is None and want_corr and self.kind == MULTIPOLE:
+            Lcorr = torch.empty((3,) + self.out_shape, dtype=torch.float64, device=self.device)
+        octo_fmm_get_expansions(self.handle, L, Lcorr)
+        return L, Lcorr
+
+    def solve(self, moments, com_off=None):
+        self.set_moments(moments, com_off)
+        self.interact()
+        return self.get_expansions()
+
+    def status(self):
+        return octo_fmm_status(self.handle)
+
+    def stencil(self, parity):
+        return octo_fmm_get_stencil(self.handle, parity)
+
+    def interaction_count(self):
+        return octo_fmm_interaction_count(self.handle)
+
+    def launch_info(self):
+        return octo_fmm_launch_info(self.handle)
+
+    def set_option(self, key, value):
+        octo_fmm_set_option(self.handle, key, value)
+
+    def close(self):
+        if getattr(self, "handle", None) is not None:
+            octo_fmm_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

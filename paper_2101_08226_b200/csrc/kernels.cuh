@@ -1,0 +1,409 @@
+// kernels.cuh -- sm_100a kernels of the FMM cell-to-cell interaction step.
+//
+//   stage_multipole_kernel   a2: raw moments -> staged layout in the workspace
+//   m2l_staged_kernel        a3/a4/a6: persistent, TMA-fed slab pipeline (default)
+//   m2l_direct_kernel        a3/a4/a6: same pair arithmetic, global-memory loads (cross-check)
+//   p2p_monopole_kernel      a5: monopole variant
+//   dfma_peak_kernel         FP64 ALU roofline probe
+//
+// Staged layout of the sources (workspace), in double2 units:
+//     S[z][cp][y][xpar][xh] of double2,  cp = comp >> 1 (10 pairs; slot 19 is padding),
+//     xpar = x & 1, xh = x >> 1
+// i.e. components are stored in pairs and each x-row is de-interleaved into its even and odd
+// cells, so that the 8 lanes of a warp that share an x-parity read 8 CONSECUTIVE double2 from
+// shared memory (one conflict-free 128-byte wavefront per quarter warp, LDS.128) and one 5-D
+// TMA box {2, 13, 52, 10, 1} brings a whole z-slab (tile + halo) on chip.  The pair is the
+// innermost tensor dimension because TMA needs the box start 16-byte aligned in the innermost
+// dimension (measured: an odd FP64 start coordinate raises "illegal instruction" on sm_100a).
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "m2l_math.cuh"
+
+namespace octo {
+
+constexpr int REACH_MAX = 5;            // theta_min = 0.34 for 8^3 sub-grids
+constexpr int MAX_LIST = 651;           // |S_p| for 1/3 < theta (7 * 93)
+constexpr int TILE = 16;                // target tile: 16 x 16 cells of one z-layer
+constexpr int NPAIR = (NCOMP + 1) / 2;  // 10 component pairs
+constexpr int SLAB_XH = 13;             // half-row length in the slab: (16 + 2*5) / 2
+constexpr int SLAB_ROW = 2 * SLAB_XH;   // 26 double2 per y-row (even half, odd half)
+constexpr int SLAB_Y = TILE + 2 * REACH_MAX;      // 26
+constexpr int SLAB_PLANE = SLAB_Y * SLAB_ROW;     // 676 double2 per component pair
+constexpr int SLAB_ELEMS = NPAIR * SLAB_PLANE;    // 6760 double2
+constexpr int SLAB_BYTES = SLAB_ELEMS * 16;       // 108160 = 845 * 128 (TMA transaction size, 128-B aligned)
+static_assert(SLAB_BYTES % 128 == 0, "TMA needs 128-byte aligned shared-memory destinations");
+constexpr int NSTAGE = 2;
+constexpr int CONSUMER_WARPS = 8;
+constexpr int STAGED_THREADS = (CONSUMER_WARPS + 1) * 32;   // + 1 producer warp
+constexpr int STAGED_SMEM = NSTAGE * SLAB_BYTES + 64;
+
+struct StEntry {
+    int off;                 // staged kernel: shared-memory offset (double2) relative to the thread's base
+    signed char dx, dy, dz, pad;
+};
+
+// Stencil tables (the interaction lists of the 8 parity classes, Eq. 15) in constant memory.
+__constant__ StEntry c_entries[8 * MAX_LIST];
+__constant__ int c_begin[8][2 * REACH_MAX + 2];   // first entry of (class, dz); [..][11] = end
+__constant__ double c_hmul[2 * REACH_MAX + 1];    // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h)
+
+struct Params {
+    int nx, ny, nz;
+    int lo[3], hi[3];        // output region
+    int ox, oy, oz;          // its extents
+    int tiles_x, tiles_y;    // 16 x 16 tiles covering the output region
+    long long ntiles;        // tiles_x * tiles_y * oz
+    int reach;
+    const double* S;         // staged sources
+    double* L;               // [20][oz][oy][ox]
+    double* C;               // [3][oz][oy][ox]
+    int* flags;              // bit 0: target mass <= 0 with correction
+};
+
+// ------------------------------------------------------------------------------------------
+// a2: stage the sources
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) stage_multipole_kernel(const double* __restrict__ mom,
+                                                              const double* __restrict__ com, double* __restrict__ S,
+                                                              int nx, int ny, int nz)
+{
+    const long long ncell = (long long)nx * ny * nz;
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= ncell) return;
+    const int x = (int)(cell % nx);
+    const long long r = cell / nx;
+    const int y = (int)(r % ny), z = (int)(r / ny);
+    double M[20], s[20];
+#pragma unroll
+    for (int c = 0; c < 20; ++c) M[c] = mom[(long long)c * ncell + cell];
+    reduce_moments(M, s);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) s[C_DX + c] = com ? com[(long long)c * ncell + cell] : 0.0;
+    s[19] = 0.0;
+    const long long plane = (long long)ny * nx;   // double2 per (z, pair)
+    double2* dst = reinterpret_cast<double2*>(S) + (long long)z * NPAIR * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1);
+#pragma unroll
+    for (int c = 0; c < NPAIR; ++c) dst[(long long)c * plane] = make_double2(s[2 * c], s[2 * c + 1]);
+}
+
+// ------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + TMA
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_slab(void* dst, const CUtensorMap* map, uint64_t* bar, int c1, int c2, int c4)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes"
+        " [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+        ::"r"(smem_u32(dst)), "l"((uint64_t)map), "r"(smem_u32(bar)), "r"(0), "r"(c1), "r"(c2), "r"(0), "r"(c4)
+        : "memory");
+}
+
+// tile id -> (tile x, tile y, layer); the layer runs fastest so that the CTAs resident at one
+// time walk up a few columns and share their slabs through L2.
+__device__ __forceinline__ void decode_tile(const Params& p, long long t, int& x0, int& y0, int& k)
+{
+    k = p.lo[2] + (int)(t % p.oz);
+    const long long c = t / p.oz;
+    x0 = p.lo[0] + (int)(c % p.tiles_x) * TILE;
+    y0 = p.lo[1] + (int)(c / p.tiles_x) * TILE;
+}
+
+// ------------------------------------------------------------------------------------------
+// a3/a4/a6, default: persistent CTAs, one 16x16x1 target tile at a time, one cell per thread.
+// Warp w (< 8) holds the 32 cells of xy-parity class w >> 1 in tile rows 8 (w & 1) + {0..7}
+// (every lane of a warp runs the same interaction list, no masks); warp 8 is the TMA producer.
+// For dz = -reach..reach the z-slab k + dz (tile + 5-cell halo, all 19 components) is brought
+// in by one TMA box; the two slab buffers form a full/empty mbarrier ring that keeps running
+// across tiles.  Out-of-grid parts of a box are zero-filled by TMA = zero-mass cells with zero
+// offset, which contribute exactly 0 to every coefficient (isolated boundary, L321).
+// ------------------------------------------------------------------------------------------
+// load the 19 staged components of one source cell (10 double2, stride `stride` double2)
+#define OCTO_LOAD_SOURCE(q, stride, src, bx_, by_, bz_)                                   \
+    {                                                                                     \
+        double2 v_[NPAIR];                                                                \
+        _Pragma("unroll") for (int c_ = 0; c_ < NPAIR; ++c_) v_[c_] = (q)[(long long)c_ * (stride)]; \
+        _Pragma("unroll") for (int c_ = 0; c_ < 8; ++c_) { src[2 * c_] = v_[c_].x; src[2 * c_ + 1] = v_[c_].y; } \
+        bx_ = v_[8].x; by_ = v_[8].y; bz_ = v_[9].x;                                       \
+    }
+
+// the target's own expansion centre and (for the correction) M3_A / M_A in staged form
+template <bool CORR>
+__device__ __forceinline__ void load_target(const Params& p, int gx, int gy, int k, double (&dA)[3], double (&tA)[7])
+{
+    const long long plane = (long long)p.ny * p.nx;
+    const double2* own = reinterpret_cast<const double2*>(p.S) + (long long)k * NPAIR * plane + (long long)gy * p.nx +
+                         (gx & 1) * (p.nx >> 1) + (gx >> 1);
+    const double2 d01 = own[8 * plane], d2 = own[9 * plane];
+    dA[0] = d01.x; dA[1] = d01.y; dA[2] = d2.x;
+    if (CORR) {
+        const double mA = own[0].x;
+        if (mA > 0.0) {
+            const double inv = 1.0 / mA;
+            const double2 o0 = own[4 * plane], o1 = own[5 * plane], o2 = own[6 * plane], o3 = own[7 * plane];
+            tA[0] = o0.y * inv;                       // comp 9  (xxx)
+            tA[1] = o1.x * inv; tA[2] = o1.y * inv;   // comps 10, 11
+            tA[3] = o2.x * inv; tA[4] = o2.y * inv;   // comps 12, 13
+            tA[5] = o3.x * inv; tA[6] = o3.y * inv;   // comps 14, 15
+        } else {
+            atomicOr(p.flags, 1);
+        }
+    }
+}
+
+template <bool CORR>
+__device__ __forceinline__ void store_target(const Params& p, const Acc& acc, int gx, int gy, int k)
+{
+    double L[20], C[3];
+    acc_finish<CORR>(acc, L, C);
+    const long long ocell = (long long)p.ox * p.oy * p.oz;
+    const long long o = ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+#pragma unroll
+    for (int c = 0; c < 20; ++c) p.L[(long long)c * ocell + o] = L[c];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p.C[(long long)c * ocell + o] = C[c];
+}
+
+template <bool CORR>
+__global__ void __launch_bounds__(STAGED_THREADS, 1)
+m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* slab0 = reinterpret_cast<double2*>(smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + NSTAGE * SLAB_BYTES);
+    uint64_t* empty = full + NSTAGE;
+
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < NSTAGE; ++b) {
+            mbar_init(&full[b], 1);
+            mbar_init(&empty[b], CONSUMER_WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == CONSUMER_WARPS) {
+        // ------------------------------ producer ------------------------------
+        if (lane == 0) {
+            uint32_t it = 0;
+            for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
+                int x0, y0, k;
+                decode_tile(p, t, x0, y0, k);
+                for (int dz = -p.reach; dz <= p.reach; ++dz) {
+                    const int zz = k + dz;
+                    if (zz < 0 || zz >= p.nz) continue;
+                    const uint32_t b = it % NSTAGE;
+                    if (it >= NSTAGE) mbar_wait(&empty[b], ((it / NSTAGE) - 1) & 1);
+                    mbar_arrive_expect_tx(&full[b], SLAB_BYTES);
+                    tma_load_slab(slab0 + (size_t)b * SLAB_ELEMS, &tmap, &full[b], (x0 >> 1) - 3, 2 * (y0 - REACH_MAX), zz);
+                    ++it;
+                }
+            }
+        }
+        return;
+    }
+
+    // ------------------------------ consumers ------------------------------
+    const int cls_xy = warp >> 1;                      // px + 2 py
+    const int px = cls_xy & 1, py = cls_xy >> 1;
+    const int lx = lane & 7;
+    const int ly = ((warp & 1) << 2) + (lane >> 3);    // 0..7
+    const int tbase = lx + 2 * ly * SLAB_ROW;          // double2
+
+    uint32_t it = 0;
+    for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
+        int x0, y0, k;
+        decode_tile(p, t, x0, y0, k);
+        const int gx = x0 + px + 2 * lx, gy = y0 + py + 2 * ly;
+        const bool active = gx < p.hi[0] && gy < p.hi[1];
+        const int cls = cls_xy + ((k & 1) << 2);
+
+        double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        if (active) load_target<CORR>(p, gx, gy, k, dA, tA);
+
+        Acc acc;
+        acc_zero(acc);
+
+        for (int dz = -p.reach; dz <= p.reach; ++dz) {
+            const int zz = k + dz;
+            if (zz < 0 || zz >= p.nz) continue;
+            const uint32_t b = it % NSTAGE;
+            mbar_wait(&full[b], (it / NSTAGE) & 1);
+            const double2* sl = slab0 + (size_t)b * SLAB_ELEMS + tbase;
+            const double Rz0 = c_hmul[dz + REACH_MAX] + dA[2];
+            const int s_begin = c_begin[cls][dz + REACH_MAX], s_end = c_begin[cls][dz + REACH_MAX + 1];
+#pragma unroll 1
+            for (int s = s_begin; s < s_end; ++s) {
+                const StEntry e = c_entries[cls * MAX_LIST + s];
+                const double2* q = sl + e.off;
+                double src[16], bx, by, bz;
+                OCTO_LOAD_SOURCE(q, SLAB_PLANE, src, bx, by, bz);
+                const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx);
+                const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by);
+                const double z = Rz0 - bz;
+                m2l_pair<CORR>(acc, x, y, z, src, tA);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[b]);
+            ++it;
+        }
+
+        if (active) store_target<CORR>(p, acc, gx, gy, k);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a3/a4/a6, cross-check variant: one thread per target cell, sources read straight from the
+// staged array in global memory with explicit in-grid tests.  Same pair arithmetic.
+// Block = 256 threads = the 8 parity classes x 32 cells of a 16 x 8 x 2 brick, two passes in z.
+// ------------------------------------------------------------------------------------------
+template <bool CORR>
+__global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
+{
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const int px = warp & 1, py = (warp >> 1) & 1, pz = warp >> 2;
+    const int bx = (p.ox + 15) / 16, by = (p.oy + 7) / 8;
+    const int b = blockIdx.x;
+    const int x0 = p.lo[0] + (b % bx) * 16, y0 = p.lo[1] + ((b / bx) % by) * 8, z0 = p.lo[2] + (b / (bx * by)) * 4;
+    const int gx = x0 + px + 2 * (lane & 7), gy = y0 + py + 2 * (lane >> 3);
+    const long long plane = (long long)p.ny * p.nx;
+    const double2* S2 = reinterpret_cast<const double2*>(p.S);
+    const int cls = warp;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int k = z0 + pz + 2 * pass;
+        if (!(gx < p.hi[0] && gy < p.hi[1] && k < p.hi[2])) continue;
+        double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        load_target<CORR>(p, gx, gy, k, dA, tA);
+        Acc acc;
+        acc_zero(acc);
+        const int s_end = c_begin[cls][2 * REACH_MAX + 1];
+#pragma unroll 1
+        for (int s = c_begin[cls][0]; s < s_end; ++s) {
+            const StEntry e = c_entries[cls * MAX_LIST + s];
+            const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+            if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
+            const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
+            double src[16], bx_, by_, bz_;
+            OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
+            const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
+            const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by_);
+            const double z = c_hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+            m2l_pair<CORR>(acc, x, y, z, src, tA);
+        }
+        store_target<CORR>(p, acc, gx, gy, k);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// a5: monopole (leaf) variant.  R = (i_A - i_B) h has no per-cell part, so -1/|R| and
+// -R/|R|^3 depend on the list entry only: they are tabulated once per (class, entry) on the
+// host in FP64 and the kernel is a 4-FMA stencil sum.  W = [class][entry]{w0,wx,wy,wz}.
+// mass is zero-padded by REACH_MAX cells on every side: P[(nz+10)][(ny+10)][(nx+10)].
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __restrict__ mass, double* __restrict__ P,
+                                                             int nx, int ny, int nz)
+{
+    const int X = nx + 2 * REACH_MAX, Y = ny + 2 * REACH_MAX, Z = nz + 2 * REACH_MAX;
+    const long long n = (long long)X * Y * Z;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int x = (int)(i % X) - REACH_MAX;
+    const long long r = i / X;
+    const int y = (int)(r % Y) - REACH_MAX, z = (int)(r / Y) - REACH_MAX;
+    const bool in = x >= 0 && y >= 0 && z >= 0 && x < nx && y < ny && z < nz;
+    P[i] = in ? mass[((long long)z * ny + y) * nx + x] : 0.0;
+}
+
+__global__ void __launch_bounds__(256) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
+                                                           const double4* __restrict__ W, double* __restrict__ out)
+{
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const int px = warp & 1, py = (warp >> 1) & 1, pz = warp >> 2;
+    const int bx = (p.ox + 15) / 16, by = (p.oy + 7) / 8;
+    const int b = blockIdx.x;
+    const int x0 = p.lo[0] + (b % bx) * 16, y0 = p.lo[1] + ((b / bx) % by) * 8, z0 = p.lo[2] + (b / (bx * by)) * 4;
+    const int gx = x0 + px + 2 * (lane & 7), gy = y0 + py + 2 * ((lane >> 3) & 3);
+    const int X = p.nx + 2 * REACH_MAX, Y = p.ny + 2 * REACH_MAX;
+    const long long ocell = (long long)p.ox * p.oy * p.oz;
+    const int cls = warp;
+    const int s_begin = c_begin[cls][0], s_end = c_begin[cls][2 * REACH_MAX + 1];
+    // two cells per thread (k and k + 2 share the parity class, hence the list and the weights)
+    const int k0 = z0 + pz, k1 = k0 + 2;
+    const bool act0 = gx < p.hi[0] && gy < p.hi[1] && k0 < p.hi[2];
+    const bool act1 = gx < p.hi[0] && gy < p.hi[1] && k1 < p.hi[2];
+    if (!act0) return;
+    const double* c0 = P + ((long long)(k0 + REACH_MAX) * Y + (gy + REACH_MAX)) * X + (gx + REACH_MAX);
+    const double* c1 = act1 ? c0 + 2LL * Y * X : c0;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0, b0 = 0.0, b1 = 0.0, b2 = 0.0, b3 = 0.0;
+#pragma unroll 4
+    for (int s = s_begin; s < s_end; ++s) {
+        const StEntry e = c_entries[cls * MAX_LIST + s];
+        const long long off = ((long long)e.dz * Y + e.dy) * X + e.dx;
+        const double4 w = W[cls * MAX_LIST + s];
+        const double m0 = c0[off], m1 = c1[off];
+        a0 = fma(m0, w.x, a0); a1 = fma(m0, w.y, a1); a2 = fma(m0, w.z, a2); a3 = fma(m0, w.w, a3);
+        b0 = fma(m1, w.x, b0); b1 = fma(m1, w.y, b1); b2 = fma(m1, w.z, b2); b3 = fma(m1, w.w, b3);
+    }
+    long long o = ((long long)(k0 - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+    out[o] = a0; out[ocell + o] = a1; out[2 * ocell + o] = a2; out[3 * ocell + o] = a3;
+    if (act1) {
+        o += 2LL * p.oy * p.ox;
+        out[o] = b0; out[ocell + o] = b1; out[2 * ocell + o] = b2; out[3 * ocell + o] = b3;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// FP64 ALU roofline probe: 8 independent DFMA chains per thread.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double seed)
+{
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-9;
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+            a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+}  // namespace octo

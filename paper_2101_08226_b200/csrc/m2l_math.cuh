@@ -1,0 +1,218 @@
+// m2l_math.cuh -- per-pair arithmetic of the multipole->local interaction, sm_100a.
+//
+// What it computes is defined in include/octo_fmm.h / DESIGN.md (section 2.2).
+// How it computes it differs from the definition on purpose (this is the GPU formulation; the
+// CPU oracle uses full tensors):
+//   * The Green's-function derivative tensors D^(n) of -1/r are symmetric and TRACE-FREE, so only
+//     2n+1 components of each are independent.  We generate the components with at most one z
+//     index (5 of D2, 7 of D3, 9 of D4) plus the few z-heavy ones the contractions touch, and we
+//     contract them with source moments that were reduced once per cell at staging time
+//     (trace removed, multiplicity and (-1)^m/m! folded in).  98 FMAs per pair instead of 125.
+//   * Accumulators are the independent components of L (1 + 3 + 5 + 7) and the correction (3);
+//     the dependent components (L2_zz, L3_xzz, L3_yzz, L3_zzz) are rebuilt once per cell.
+//   * 1/r comes from MUFU.RSQ64H (rsqrt.approx.ftz.f64, ~2^-21) and ONE cubically convergent
+//     correction step, y (1 + e/2 + 3e^2/8), e = 1 - r^2 y^2: relative error ~ (5/16) e^3 < 1e-18.
+#pragma once
+
+namespace octo {
+
+// staged (internal) per-cell source components
+enum {
+    C_M0 = 0,
+    C_M1X = 1, C_M1Y, C_M1Z,                               // -M1 (sign folded)
+    C_QXX = 4, C_QXY, C_QXZ, C_QYY, C_QYZ,                 // reduced 1/2 M2
+    C_OXXX = 9, C_OXXY, C_OXXZ, C_OXYY, C_OXYZ, C_OYYY, C_OYYZ,  // reduced -1/6 M3
+    C_DX = 16, C_DY, C_DZ,                                 // centre-of-mass offset delta
+    NCOMP = 19
+};
+
+struct Acc {
+    double l0;
+    double l1[3];
+    double l2[5];   // xx xy xz yy yz
+    double l3[7];   // xxx xxy xxz xyy xyz yyy yyz
+    double c[3];    // correction to L1
+};
+
+__device__ __forceinline__ void acc_zero(Acc& a)
+{
+    a.l0 = 0.0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { a.l1[i] = 0.0; a.c[i] = 0.0; }
+#pragma unroll
+    for (int i = 0; i < 5; ++i) a.l2[i] = 0.0;
+#pragma unroll
+    for (int i = 0; i < 7; ++i) a.l3[i] = 0.0;
+}
+
+// 1/sqrt(x) to ~1 ulp for normal positive x
+__device__ __forceinline__ double rsqrt_fast(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double q = e * p;
+    return fma(y, q, y);
+}
+
+// Reduce the 20 raw moments of a cell to the 16 staged source components (once per cell).
+__device__ __forceinline__ void reduce_moments(const double M[20], double* s)
+{
+    s[C_M0] = M[0];
+    s[C_M1X] = -M[1];
+    s[C_M1Y] = -M[2];
+    s[C_M1Z] = -M[3];
+    // M2: [xx xy xz yy yz zz] = M[4..9];  1/2 M2:D2 with D2_zz = -D2_xx - D2_yy
+    s[C_QXX] = 0.5 * (M[4] - M[9]);
+    s[C_QXY] = M[5];
+    s[C_QXZ] = M[6];
+    s[C_QYY] = 0.5 * (M[7] - M[9]);
+    s[C_QYZ] = M[8];
+    // M3: [xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz] = M[10..19];  -1/6 M3:.D3 with
+    // D3_xzz = -D3_xxx - D3_xyy, D3_yzz = -D3_xxy - D3_yyy, D3_zzz = -D3_xxz - D3_yyz
+    s[C_OXXX] = -(M[10] - 3.0 * M[15]) * (1.0 / 6.0);
+    s[C_OXXY] = -0.5 * (M[11] - M[18]);
+    s[C_OXXZ] = -(3.0 * M[12] - M[19]) * (1.0 / 6.0);
+    s[C_OXYY] = -0.5 * (M[13] - M[15]);
+    s[C_OXYZ] = -M[14];
+    s[C_OYYY] = -(M[16] - 3.0 * M[18]) * (1.0 / 6.0);
+    s[C_OYYZ] = -(3.0 * M[17] - M[19]) * (1.0 / 6.0);
+}
+
+// One ordered pair A <- B.  (x,y,z) = R = z_A - z_B; s[0..15] staged source components;
+// tA[0..6] = staged third moments of the target divided by its mass (correction only).
+template <bool CORR>
+__device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y, const double z,
+                                         const double (&s)[16], const double (&tA)[7])
+{
+    const double r2 = fma(z, z, fma(y, y, x * x));
+    const double w = rsqrt_fast(r2);          // 1/r
+    const double w2 = w * w;                  // 1/r^2
+    const double d1 = w * w2;                 // 1/r^3
+    const double d2 = d1 * (-3.0 * w2);       // -3/r^5
+    const double d3 = d2 * (-5.0 * w2);       // 15/r^7
+
+    // ---- D1, D2 (6 components; zz is needed by the dipole term of L1_z) ----
+    const double D1x = d1 * x, D1y = d1 * y, D1z = d1 * z;
+    const double ax = d2 * x, ay = d2 * y, az = d2 * z;
+    const double Dxx = fma(ax, x, d1), Dxy = ax * y, Dxz = ax * z;
+    const double Dyy = fma(ay, y, d1), Dyz = ay * z, Dzz = fma(az, z, d1);
+
+    // ---- D3: 7 independent + xzz, yzz ----
+    const double bx = d3 * x, by = d3 * y;
+    const double bxx = bx * x, bxy = bx * y, byy = by * y;
+    const double ax3 = 3.0 * ax, ay3 = 3.0 * ay;
+    const double Dxxx = fma(bxx, x, ax3);
+    const double Dxxy = fma(bxx, y, ay);
+    const double Dxxz = fma(bxx, z, az);
+    const double Dxyy = fma(bxy, y, ax);
+    const double Dxyz = bxy * z;
+    const double Dyyy = fma(byy, y, ay3);
+    const double Dyyz = fma(byy, z, az);
+    const double Dxzz = -(Dxxx + Dxyy);
+    const double Dyzz = -(Dxxy + Dyyy);
+
+    const double m0 = s[C_M0], m1x = s[C_M1X], m1y = s[C_M1Y], m1z = s[C_M1Z];
+    const double qxx = s[C_QXX], qxy = s[C_QXY], qxz = s[C_QXZ], qyy = s[C_QYY], qyz = s[C_QYZ];
+
+    // ---- L0 += M D0 - M1.D1 + 1/2 M2:D2 - 1/6 M3:.D3 ----
+    {
+        double t = a.l0;
+        t = fma(m0, -w, t);
+        t = fma(m1x, D1x, t); t = fma(m1y, D1y, t); t = fma(m1z, D1z, t);
+        t = fma(qxx, Dxx, t); t = fma(qxy, Dxy, t); t = fma(qxz, Dxz, t); t = fma(qyy, Dyy, t); t = fma(qyz, Dyz, t);
+        t = fma(s[C_OXXX], Dxxx, t); t = fma(s[C_OXXY], Dxxy, t); t = fma(s[C_OXXZ], Dxxz, t);
+        t = fma(s[C_OXYY], Dxyy, t); t = fma(s[C_OXYZ], Dxyz, t); t = fma(s[C_OYYY], Dyyy, t);
+        t = fma(s[C_OYYZ], Dyyz, t);
+        a.l0 = t;
+    }
+    // ---- L1_i += M D1_i - M1_j D2_ij + 1/2 M2_jk D3_ijk ----
+    {
+        double t = a.l1[0];
+        t = fma(m0, D1x, t);
+        t = fma(m1x, Dxx, t); t = fma(m1y, Dxy, t); t = fma(m1z, Dxz, t);
+        t = fma(qxx, Dxxx, t); t = fma(qxy, Dxxy, t); t = fma(qxz, Dxxz, t); t = fma(qyy, Dxyy, t); t = fma(qyz, Dxyz, t);
+        a.l1[0] = t;
+        t = a.l1[1];
+        t = fma(m0, D1y, t);
+        t = fma(m1x, Dxy, t); t = fma(m1y, Dyy, t); t = fma(m1z, Dyz, t);
+        t = fma(qxx, Dxxy, t); t = fma(qxy, Dxyy, t); t = fma(qxz, Dxyz, t); t = fma(qyy, Dyyy, t); t = fma(qyz, Dyyz, t);
+        a.l1[1] = t;
+        t = a.l1[2];
+        t = fma(m0, D1z, t);
+        t = fma(m1x, Dxz, t); t = fma(m1y, Dyz, t); t = fma(m1z, Dzz, t);
+        t = fma(qxx, Dxxz, t); t = fma(qxy, Dxyz, t); t = fma(qxz, Dxzz, t); t = fma(qyy, Dyyz, t); t = fma(qyz, Dyzz, t);
+        a.l1[2] = t;
+    }
+    // ---- L2_ij += M D2_ij - M1_k D3_ijk   (xx xy xz yy yz) ----
+    a.l2[0] = fma(m1z, Dxxz, fma(m1y, Dxxy, fma(m1x, Dxxx, fma(m0, Dxx, a.l2[0]))));
+    a.l2[1] = fma(m1z, Dxyz, fma(m1y, Dxyy, fma(m1x, Dxxy, fma(m0, Dxy, a.l2[1]))));
+    a.l2[2] = fma(m1z, Dxzz, fma(m1y, Dxyz, fma(m1x, Dxxz, fma(m0, Dxz, a.l2[2]))));
+    a.l2[3] = fma(m1z, Dyyz, fma(m1y, Dyyy, fma(m1x, Dxyy, fma(m0, Dyy, a.l2[3]))));
+    a.l2[4] = fma(m1z, Dyzz, fma(m1y, Dyyz, fma(m1x, Dxyz, fma(m0, Dyz, a.l2[4]))));
+    // ---- L3_ijk += M D3_ijk   (xxx xxy xxz xyy xyz yyy yyz) ----
+    a.l3[0] = fma(m0, Dxxx, a.l3[0]);
+    a.l3[1] = fma(m0, Dxxy, a.l3[1]);
+    a.l3[2] = fma(m0, Dxxz, a.l3[2]);
+    a.l3[3] = fma(m0, Dxyy, a.l3[3]);
+    a.l3[4] = fma(m0, Dxyz, a.l3[4]);
+    a.l3[5] = fma(m0, Dyyy, a.l3[5]);
+    a.l3[6] = fma(m0, Dyyz, a.l3[6]);
+
+    if (CORR) {
+        // ---- correction (L127): n3 = M3_B - (M_B/M_A) M3_A (staged form), dL1_i += n3_t D4_{i,t} ----
+        const double d4 = d3 * (-7.0 * w2);    // -105/r^9
+        const double n0 = fma(-m0, tA[0], s[C_OXXX]);   // xxx
+        const double n1 = fma(-m0, tA[1], s[C_OXXY]);   // xxy
+        const double n2 = fma(-m0, tA[2], s[C_OXXZ]);   // xxz
+        const double n3 = fma(-m0, tA[3], s[C_OXYY]);   // xyy
+        const double n4 = fma(-m0, tA[4], s[C_OXYZ]);   // xyz
+        const double n5 = fma(-m0, tA[5], s[C_OYYY]);   // yyy
+        const double n6 = fma(-m0, tA[6], s[C_OYYZ]);   // yyz
+
+        const double cx = d4 * x, cy = d4 * y;
+        const double cxx = cx * x, cxy = cx * y, cyy = cy * y;
+        const double cxxx = cxx * x, cxxy = cxx * y, cxyy = cxy * y, cyyy = cyy * y;
+        const double bxz = bx * z, byz = by * z;
+        const double d2_3 = 3.0 * d2, bxy3 = 3.0 * bxy;
+        const double Exxxx = fma(cxxx, x, fma(6.0, bxx, d2_3));
+        const double Exxxy = fma(cxxx, y, bxy3);
+        const double Exxxz = fma(cxxx, z, 3.0 * bxz);
+        const double Exxyy = fma(cxxy, y, (bxx + byy) + d2);
+        const double Exxyz = fma(cxxy, z, byz);
+        const double Exyyy = fma(cxyy, y, bxy3);
+        const double Exyyz = fma(cxyy, z, bxz);
+        const double Eyyyy = fma(cyyy, y, fma(6.0, byy, d2_3));
+        const double Eyyyz = fma(cyyy, z, 3.0 * byz);
+        const double Exxzz = -(Exxxx + Exxyy);
+        const double Exyzz = -(Exxxy + Exyyy);
+        const double Eyyzz = -(Exxyy + Eyyyy);
+
+        a.c[0] = fma(n6, Exyyz, fma(n5, Exyyy, fma(n4, Exxyz, fma(n3, Exxyy, fma(n2, Exxxz, fma(n1, Exxxy, fma(n0, Exxxx, a.c[0])))))));
+        a.c[1] = fma(n6, Eyyyz, fma(n5, Eyyyy, fma(n4, Exyyz, fma(n3, Exyyy, fma(n2, Exxyz, fma(n1, Exxyy, fma(n0, Exxxy, a.c[1])))))));
+        a.c[2] = fma(n6, Eyyzz, fma(n5, Eyyyz, fma(n4, Exyzz, fma(n3, Exyyz, fma(n2, Exxzz, fma(n1, Exxyz, fma(n0, Exxxz, a.c[2])))))));
+    }
+}
+
+// Rebuild the 20 + 3 output coefficients from the independent accumulators.
+template <bool CORR>
+__device__ __forceinline__ void acc_finish(const Acc& a, double L[20], double C[3])
+{
+    L[0] = a.l0;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        C[i] = CORR ? a.c[i] : 0.0;
+        L[1 + i] = CORR ? a.l1[i] + a.c[i] : a.l1[i];
+    }
+    L[4] = a.l2[0]; L[5] = a.l2[1]; L[6] = a.l2[2]; L[7] = a.l2[3]; L[8] = a.l2[4];
+    L[9] = -(a.l2[0] + a.l2[3]);                       // zz = -(xx + yy)
+    L[10] = a.l3[0]; L[11] = a.l3[1]; L[12] = a.l3[2]; L[13] = a.l3[3]; L[14] = a.l3[4];
+    L[15] = -(a.l3[0] + a.l3[3]);                      // xzz = -(xxx + xyy)
+    L[16] = a.l3[5]; L[17] = a.l3[6];
+    L[18] = -(a.l3[1] + a.l3[5]);                      // yzz = -(xxy + yyy)
+    L[19] = -(a.l3[2] + a.l3[6]);                      // zzz = -(xxz + yyz)
+}
+
+}  // namespace octo

@@ -1,0 +1,518 @@
+// octo_fmm.cu -- C ABI (include/octo_fmm.h) and host logic of the B200-native FMM
+// cell-to-cell interaction step.  Kernels live in kernels.cuh / m2l_math.cuh.
+//
+// Host logic here: configuration checks, the interaction lists of Eq. 15,
+// their translation into shared-memory offsets, the closed-form interaction count, the TMA
+// descriptor of the staged source array, workspace partitioning, launches.
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/octo_fmm.h"
+#include "kernels.cuh"
+
+using namespace octo;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Offset3 { signed char d[3]; };
+
+// Eq. 15 with distances in units of the (parent) cell width: theta' = 1/|Delta| < theta.
+inline bool well_separated(long long d2, double theta) { return (double)d2 * theta * theta > 1.0; }
+inline int floor_div2(int v) { return v >> 1; }   // arithmetic shift: floor for negatives too
+
+// partner list of parity class (px,py,pz): cells well separated, parents not (L135)
+std::vector<Offset3> build_list(int px, int py, int pz, double theta, int* reach_out)
+{
+    std::vector<Offset3> out;
+    const int S = 2 * (int)std::floor(1.0 / theta) + 3;
+    int reach = 0;
+    for (int dz = -S; dz <= S; ++dz)
+        for (int dy = -S; dy <= S; ++dy)
+            for (int dx = -S; dx <= S; ++dx) {
+                const long long c2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
+                if (c2 == 0 || !well_separated(c2, theta)) continue;
+                const int Ix = floor_div2(px + dx), Iy = floor_div2(py + dy), Iz = floor_div2(pz + dz);
+                const long long p2 = (long long)Ix * Ix + (long long)Iy * Iy + (long long)Iz * Iz;
+                if (p2 != 0 && well_separated(p2, theta)) continue;
+                Offset3 o;
+                o.d[0] = (signed char)dx; o.d[1] = (signed char)dy; o.d[2] = (signed char)dz;
+                out.push_back(o);
+                const int m = std::max(std::abs(dx), std::max(std::abs(dy), std::abs(dz)));
+                if (m > reach) reach = m;
+            }
+    if (reach_out && reach > *reach_out) *reach_out = reach;
+    return out;
+}
+
+bool region_of(const octo_fmm_config& c, int lo[3], int hi[3])
+{
+    bool whole = true;
+    for (int a = 0; a < 3; ++a) whole = whole && c.out_lo[a] == 0 && c.out_hi[a] == 0;
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = whole ? 0 : c.out_lo[a];
+        hi[a] = whole ? c.n[a] : c.out_hi[a];
+        if (lo[a] < 0 || hi[a] > c.n[a] || lo[a] >= hi[a] || lo[a] % 8 || hi[a] % 8) return false;
+    }
+    return true;
+}
+
+bool config_ok(const octo_fmm_config* c)
+{
+    if (!c) return false;
+    for (int a = 0; a < 3; ++a)
+        if (c->n[a] <= 0 || c->n[a] % 8 || c->n[a] > 4096) return false;
+    int lo[3], hi[3];
+    if (!region_of(*c, lo, hi)) return false;
+    if (!(c->h > 0.0) || !std::isfinite(c->h)) return false;
+    if (!(c->theta > 1.0 / 3.0 && c->theta < 1.0)) return false;   // reach <= 5 (theta_min, L137)
+    if (c->kind != OCTO_FMM_MULTIPOLE && c->kind != OCTO_FMM_MONOPOLE) return false;
+    return true;
+}
+
+struct Sizes { size_t src, L, C, W, flags, total; };
+
+Sizes sizes_of(const octo_fmm_config& c)
+{
+    int lo[3], hi[3];
+    region_of(c, lo, hi);
+    const size_t ncell = (size_t)c.n[0] * c.n[1] * c.n[2];
+    const size_t ocell = (size_t)(hi[0] - lo[0]) * (hi[1] - lo[1]) * (hi[2] - lo[2]);
+    Sizes s{};
+    if (c.kind == OCTO_FMM_MULTIPOLE) {
+        s.src = align_up(ncell * NPAIR * 2 * sizeof(double));
+        s.L = align_up(ocell * 20 * sizeof(double));
+        s.C = align_up(ocell * 3 * sizeof(double));
+        s.W = 0;
+    } else {
+        const size_t pc = (size_t)(c.n[0] + 2 * REACH_MAX) * (c.n[1] + 2 * REACH_MAX) * (c.n[2] + 2 * REACH_MAX);
+        s.src = align_up(pc * sizeof(double));
+        s.L = align_up(ocell * 4 * sizeof(double));
+        s.C = 0;
+        s.W = align_up((size_t)8 * MAX_LIST * sizeof(double4));
+    }
+    s.flags = ALIGN;
+    s.total = s.src + s.L + s.C + s.W + s.flags;
+    return s;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+const void* g_const_owner = nullptr;   // handle whose tables are in constant memory
+
+}  // namespace
+
+struct octo_fmm {
+    octo_fmm_config cfg;
+    int lo[3], hi[3];
+    int reach;
+    std::vector<Offset3> list[8];
+    std::vector<StEntry> entries;          // 8 * MAX_LIST
+    int begin[8][2 * REACH_MAX + 2];
+    double hmul[2 * REACH_MAX + 1];
+    std::vector<double4> weights;          // monopole: 8 * MAX_LIST
+    unsigned long long n_interactions;
+    CUtensorMap tmap;
+    Params prm;
+    double* src;
+    double* L;
+    double* C;
+    double4* W;
+    int* flags;
+    int state;          // 0 created, 1 sources staged, 2 interacted
+    int kernel;         // 0 staged (TMA), 1 direct
+    int sm_count;
+    cudaStream_t stream;
+};
+
+extern "C" {
+
+const char* octo_fmm_version(void) { return "octo_fmm 0.1 (sm_100a)"; }
+
+size_t octo_fmm_workspace_bytes(const octo_fmm_config* cfg)
+{
+    if (!config_ok(cfg)) return 0;
+    return sizes_of(*cfg).total;
+}
+
+size_t octo_fmm_host_scratch_bytes(const octo_fmm_config* cfg)
+{
+    if (!config_ok(cfg)) return 0;
+    int lo[3], hi[3];
+    region_of(*cfg, lo, hi);
+    const size_t ncell = (size_t)cfg->n[0] * cfg->n[1] * cfg->n[2];
+    const size_t ocell = (size_t)(hi[0] - lo[0]) * (hi[1] - lo[1]) * (hi[2] - lo[2]);
+    if (cfg->kind == OCTO_FMM_MULTIPOLE)
+        return align_up(ncell * 20 * 8) + align_up(ncell * 3 * 8) + align_up(ocell * 20 * 8) + align_up(ocell * 3 * 8);
+    return align_up(ncell * 8) + align_up(ocell * 4 * 8);
+}
+
+int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
+{
+    if (!out) return OCTO_FMM_EINVAL;
+    *out = nullptr;
+    if (!config_ok(cfg)) return OCTO_FMM_EINVAL;
+    const Sizes sz = sizes_of(*cfg);
+    if (!cfg->workspace || cfg->workspace_bytes < sz.total || ((uintptr_t)cfg->workspace % ALIGN)) return OCTO_FMM_EINVAL;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) return OCTO_FMM_ECUDA;
+    if (cudaSetDevice(cfg->device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (prop.major != 10) return OCTO_FMM_ECUDA;   // sm_100a only
+
+    octo_fmm* h = new (std::nothrow) octo_fmm();
+    if (!h) return OCTO_FMM_ENOMEM;
+    h->cfg = *cfg;
+    h->stream = (cudaStream_t)cfg->stream;
+    h->sm_count = prop.multiProcessorCount;
+    h->state = 0;
+    h->kernel = 0;
+    region_of(*cfg, h->lo, h->hi);
+
+    // ---- a1: interaction lists (Eq. 15) ----
+    h->reach = 0;
+    for (int p = 0; p < 8; ++p) h->list[p] = build_list(p & 1, (p >> 1) & 1, (p >> 2) & 1, cfg->theta, &h->reach);
+    if (h->reach > REACH_MAX) { delete h; return OCTO_FMM_EINVAL; }
+    for (int p = 0; p < 8; ++p)
+        if ((int)h->list[p].size() > MAX_LIST) { delete h; return OCTO_FMM_EINVAL; }
+
+    h->entries.assign((size_t)8 * MAX_LIST, StEntry{0, 0, 0, 0, 0});
+    for (int p = 0; p < 8; ++p) {
+        const int px = p & 1, py = (p >> 1) & 1;
+        int cur = 0;
+        for (int dz = -REACH_MAX; dz <= REACH_MAX + 1; ++dz) {
+            // lists are (dz,dy,dx)-lexicographic, so each dz is a contiguous range
+            while (cur < (int)h->list[p].size() && h->list[p][cur].d[2] < dz) ++cur;
+            h->begin[p][dz + REACH_MAX] = cur;
+        }
+        for (size_t s = 0; s < h->list[p].size(); ++s) {
+            const int dx = h->list[p][s].d[0], dy = h->list[p][s].d[1], dz = h->list[p][s].d[2];
+            StEntry e;
+            // shared-memory offset of the source relative to the thread's base (see kernels.cuh)
+            e.off = (py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1);   // double2 units
+            e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz; e.pad = 0;
+            h->entries[(size_t)p * MAX_LIST + s] = e;
+        }
+    }
+    for (int d = -REACH_MAX; d <= REACH_MAX; ++d) h->hmul[d + REACH_MAX] = (double)(-d) * cfg->h;
+
+    // ---- interaction count: per-axis closed form over the lists (out-of-grid partners skipped) ----
+    {
+        unsigned long long cnt[3][2][2 * REACH_MAX + 1];
+        for (int a = 0; a < 3; ++a)
+            for (int par = 0; par < 2; ++par)
+                for (int d = -REACH_MAX; d <= REACH_MAX; ++d) {
+                    unsigned long long c = 0;
+                    for (int i = h->lo[a]; i < h->hi[a]; ++i)
+                        if ((i & 1) == par && i + d >= 0 && i + d < cfg->n[a]) ++c;
+                    cnt[a][par][d + REACH_MAX] = c;
+                }
+        unsigned long long total = 0;
+        for (int p = 0; p < 8; ++p)
+            for (const Offset3& o : h->list[p])
+                total += cnt[0][p & 1][o.d[0] + REACH_MAX] * cnt[1][(p >> 1) & 1][o.d[1] + REACH_MAX] *
+                         cnt[2][(p >> 2) & 1][o.d[2] + REACH_MAX];
+        h->n_interactions = total;
+    }
+
+    // ---- workspace partition ----
+    char* w = (char*)cfg->workspace;
+    h->src = (double*)w; w += sz.src;
+    h->L = (double*)w;   w += sz.L;
+    h->C = (double*)w;   w += sz.C;
+    h->W = (double4*)w;  w += sz.W;
+    h->flags = (int*)w;
+
+    Params& P = h->prm;
+    P.nx = cfg->n[0]; P.ny = cfg->n[1]; P.nz = cfg->n[2];
+    for (int a = 0; a < 3; ++a) { P.lo[a] = h->lo[a]; P.hi[a] = h->hi[a]; }
+    P.ox = h->hi[0] - h->lo[0]; P.oy = h->hi[1] - h->lo[1]; P.oz = h->hi[2] - h->lo[2];
+    P.tiles_x = (P.ox + TILE - 1) / TILE; P.tiles_y = (P.oy + TILE - 1) / TILE;
+    P.ntiles = (long long)P.tiles_x * P.tiles_y * P.oz;
+    P.reach = h->reach;
+    P.S = h->src; P.L = h->L; P.C = h->C; P.flags = h->flags;
+
+    if (cfg->kind == OCTO_FMM_MULTIPOLE) {
+        // ---- TMA descriptor of S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
+        //      {2 (pair), nx/2 (xh), 2 ny (y*2 + xpar), 10 (cp), nz}
+        EncodeTiledFn enc = encode_tiled_fn();
+        if (!enc) { delete h; return OCTO_FMM_ECUDA; }
+        const cuuint64_t nxh = (cuuint64_t)cfg->n[0] / 2, nxy = (cuuint64_t)cfg->n[0] * cfg->n[1];
+        cuuint64_t dims[5] = {2, nxh, 2 * (cuuint64_t)cfg->n[1], (cuuint64_t)NPAIR, (cuuint64_t)cfg->n[2]};
+        cuuint64_t strides[4] = {16, nxh * 16, nxy * 16, nxy * 16 * NPAIR};
+        cuuint32_t box[5] = {2, SLAB_XH, 2 * SLAB_Y, NPAIR, 1};
+        cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+        std::memset(&h->tmap, 0, sizeof(h->tmap));
+        CUresult r = enc(&h->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void*)h->src, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { delete h; return OCTO_FMM_ECUDA; }
+        cudaError_t e1 = cudaFuncSetAttribute(m2l_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        if (e1 != cudaSuccess || e2 != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+    } else {
+        // ---- monopole weights: -1/|R| and -R/|R|^3 with R = (i_A - i_B) h = -Delta h ----
+        h->weights.assign((size_t)8 * MAX_LIST, double4{0, 0, 0, 0});
+        for (int p = 0; p < 8; ++p)
+            for (size_t s = 0; s < h->list[p].size(); ++s) {
+                const double Rx = h->hmul[h->list[p][s].d[0] + REACH_MAX], Ry = h->hmul[h->list[p][s].d[1] + REACH_MAX],
+                             Rz = h->hmul[h->list[p][s].d[2] + REACH_MAX];
+                const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = std::sqrt(r2);
+                double4 wv;
+                wv.x = -1.0 / r; wv.y = -Rx / (r2 * r); wv.z = -Ry / (r2 * r); wv.w = -Rz / (r2 * r);
+                h->weights[(size_t)p * MAX_LIST + s] = wv;
+            }
+        if (cudaMemcpyAsync(h->W, h->weights.data(), h->weights.size() * sizeof(double4), cudaMemcpyHostToDevice,
+                            h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+        if (cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+    }
+    *out = h;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com_off)
+{
+    if (!h || !moments) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    const Params& P = h->prm;
+    if (h->cfg.kind == OCTO_FMM_MULTIPOLE) {
+        const long long ncell = (long long)P.nx * P.ny * P.nz;
+        stage_multipole_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(moments, com_off, h->src, P.nx, P.ny, P.nz);
+    } else {
+        const long long pc = (long long)(P.nx + 2 * REACH_MAX) * (P.ny + 2 * REACH_MAX) * (P.nz + 2 * REACH_MAX);
+        stage_monopole_kernel<<<(unsigned)((pc + 255) / 256), 256, 0, h->stream>>>(moments, h->src, P.nx, P.ny, P.nz);
+    }
+    if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    h->state = 1;
+    return OCTO_FMM_OK;
+}
+
+static int upload_tables(octo_fmm_t* h)
+{
+    if (g_const_owner == h) return OCTO_FMM_OK;
+    if (cudaMemcpyToSymbolAsync(c_entries, h->entries.data(), h->entries.size() * sizeof(StEntry), 0,
+                                cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (cudaMemcpyToSymbolAsync(c_begin, h->begin, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    if (cudaMemcpyToSymbolAsync(c_hmul, h->hmul, sizeof(h->hmul), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    g_const_owner = h;
+    return OCTO_FMM_OK;
+}
+
+static int brick_blocks(const Params& P) { return ((P.ox + 15) / 16) * ((P.oy + 7) / 8) * ((P.oz + 3) / 4); }
+
+int octo_fmm_interact(octo_fmm_t* h)
+{
+    if (!h) return OCTO_FMM_EINVAL;
+    if (h->state < 1) return OCTO_FMM_ESTATE;
+    if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (upload_tables(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    if (cudaMemsetAsync(h->flags, 0, sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    const Params& P = h->prm;
+    if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
+        p2p_monopole_kernel<<<brick_blocks(P), 256, 0, h->stream>>>(P, h->src, h->W, h->L);
+    } else if (h->kernel == 1) {
+        if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
+        else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
+    } else {
+        const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
+        if (h->cfg.am_correction) m2l_staged_kernel<true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        else                      m2l_staged_kernel<false><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    }
+    if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    h->state = 2;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_get_expansions(octo_fmm_t* h, double* L, double* Lcorr)
+{
+    if (!h || !L) return OCTO_FMM_EINVAL;
+    if (h->state < 2) return OCTO_FMM_ESTATE;
+    const Params& P = h->prm;
+    const size_t ocell = (size_t)P.ox * P.oy * P.oz;
+    const size_t ncoef = h->cfg.kind == OCTO_FMM_MULTIPOLE ? 20 : 4;
+    if (cudaMemcpyAsync(L, h->L, ocell * ncoef * sizeof(double), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    if (Lcorr) {
+        if (h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
+        if (cudaMemcpyAsync(Lcorr, h->C, ocell * 3 * sizeof(double), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess)
+            return OCTO_FMM_ECUDA;
+    }
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_status(octo_fmm_t* h)
+{
+    if (!h) return OCTO_FMM_EINVAL;
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (h->state < 2) return OCTO_FMM_OK;
+    int f = 0;
+    if (cudaMemcpy(&f, h->flags, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
+    return (f & 1) ? OCTO_FMM_EMASS : OCTO_FMM_OK;
+}
+
+int octo_fmm_destroy(octo_fmm_t* h)
+{
+    if (!h) return OCTO_FMM_EINVAL;
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (g_const_owner == h) g_const_owner = nullptr;
+    delete h;
+    return e == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
+}
+
+int octo_fmm_get_stencil(const octo_fmm_t* h, int parity, int* count, signed char (*dxyz)[3])
+{
+    if (!h || !count || parity < 0 || parity > 7) return OCTO_FMM_EINVAL;
+    *count = (int)h->list[parity].size();
+    if (dxyz)
+        for (size_t s = 0; s < h->list[parity].size(); ++s)
+            for (int a = 0; a < 3; ++a) dxyz[s][a] = h->list[parity][s].d[a];
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_interaction_count(const octo_fmm_t* h, unsigned long long* n)
+{
+    if (!h || !n) return OCTO_FMM_EINVAL;
+    *n = h->n_interactions;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_run_host(octo_fmm_t* h, const double* moments_host, const double* com_off_host, double* L_host,
+                      double* Lcorr_host, void* scratch, size_t scratch_bytes)
+{
+    if (!h || !moments_host || !L_host || !scratch) return OCTO_FMM_EINVAL;
+    if (scratch_bytes < octo_fmm_host_scratch_bytes(&h->cfg) || ((uintptr_t)scratch % ALIGN)) return OCTO_FMM_EINVAL;
+    const Params& P = h->prm;
+    const size_t ncell = (size_t)P.nx * P.ny * P.nz, ocell = (size_t)P.ox * P.oy * P.oz;
+    const bool multi = h->cfg.kind == OCTO_FMM_MULTIPOLE;
+    if (multi && !com_off_host) return OCTO_FMM_EINVAL;
+    if (!multi && Lcorr_host) return OCTO_FMM_EINVAL;
+    char* w = (char*)scratch;
+    double* d_m = (double*)w; w += align_up(ncell * (multi ? 20 : 1) * 8);
+    double* d_c = nullptr;
+    if (multi) { d_c = (double*)w; w += align_up(ncell * 3 * 8); }
+    double* d_L = (double*)w; w += align_up(ocell * (multi ? 20 : 4) * 8);
+    double* d_C = multi ? (double*)w : nullptr;
+    if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (cudaMemcpyAsync(d_m, moments_host, ncell * (multi ? 20 : 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    if (multi && cudaMemcpyAsync(d_c, com_off_host, ncell * 3 * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    int rc;
+    if ((rc = octo_fmm_set_moments(h, d_m, d_c)) != OCTO_FMM_OK) return rc;
+    if ((rc = octo_fmm_interact(h)) != OCTO_FMM_OK) return rc;
+    if ((rc = octo_fmm_get_expansions(h, d_L, Lcorr_host ? d_C : nullptr)) != OCTO_FMM_OK) return rc;
+    if (cudaMemcpyAsync(L_host, d_L, ocell * (multi ? 20 : 4) * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    if (Lcorr_host && cudaMemcpyAsync(Lcorr_host, d_C, ocell * 3 * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
+{
+    if (!h || !key) return OCTO_FMM_EINVAL;
+    if (!std::strcmp(key, "kernel")) {
+        if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
+        h->kernel = value;
+        return OCTO_FMM_OK;
+    }
+    return OCTO_FMM_EINVAL;
+}
+
+int octo_fmm_launch_info(const octo_fmm_t* h, int* grid, int* block, int* smem_bytes, int* regs, int* launches)
+{
+    if (!h) return OCTO_FMM_EINVAL;
+    const Params& P = h->prm;
+    cudaFuncAttributes fa;
+    cudaError_t e;
+    int g, b, s;
+    if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
+        e = cudaFuncGetAttributes(&fa, p2p_monopole_kernel);
+        g = brick_blocks(P); b = 256; s = 0;
+    } else if (h->kernel == 1) {
+        e = h->cfg.am_correction ? cudaFuncGetAttributes(&fa, m2l_direct_kernel<true>) : cudaFuncGetAttributes(&fa, m2l_direct_kernel<false>);
+        g = brick_blocks(P); b = 256; s = 0;
+    } else {
+        e = h->cfg.am_correction ? cudaFuncGetAttributes(&fa, m2l_staged_kernel<true>) : cudaFuncGetAttributes(&fa, m2l_staged_kernel<false>);
+        g = (int)std::min<long long>(P.ntiles, h->sm_count); b = STAGED_THREADS; s = STAGED_SMEM;
+    }
+    if (e != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (grid) *grid = g;
+    if (block) *block = b;
+    if (smem_bytes) *smem_bytes = s;
+    if (regs) *regs = fa.numRegs;
+    if (launches) *launches = 1;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_fp64_peak_probe(int device, void* stream, void* scratch, int iters, double* flops_per_s, int* sm_count,
+                             int* clock_khz)
+{
+    if (!scratch || iters <= 0 || !flops_per_s) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int blocks = prop.multiProcessorCount * 8;   // 8 x 256 threads = 2048 threads per SM
+    if ((size_t)blocks * 256 * 8 > (size_t)8 * 1024 * 1024) return OCTO_FMM_EINVAL;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return OCTO_FMM_ECUDA;
+    dfma_peak_kernel<<<blocks, 256, 0, st>>>((double*)scratch, iters / 8 + 1, 1.0);   // warm-up
+    cudaEventRecord(e0, st);
+    dfma_peak_kernel<<<blocks, 256, 0, st>>>((double*)scratch, iters, 1.0);
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    *flops_per_s = (double)blocks * 256.0 * (double)iters * 64.0 * 2.0 / (ms * 1e-3);
+    if (sm_count) *sm_count = prop.multiProcessorCount;
+    if (clock_khz) *clock_khz = prop.clockRate;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int* fp64_instructions)
+{
+    // Counted from the operation list of m2l_pair<> + the separation.
+    int f, i;
+    if (kind == OCTO_FMM_MONOPOLE) { f = 8; i = 4; }
+    else if (kind == OCTO_FMM_MULTIPOLE) {
+        if (am_correction) { f = 301; i = 178; }   // 123 DFMA + 43 DMUL + 12 DADD
+        else               { f = 201; i = 117; }   //  84 DFMA + 26 DMUL +  7 DADD
+    } else return OCTO_FMM_EINVAL;
+    if (flops) *flops = f;
+    if (fp64_instructions) *fp64_instructions = i;
+    return OCTO_FMM_OK;
+}
+
+}  // extern "C"

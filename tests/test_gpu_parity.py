@@ -1,0 +1,252 @@
+"""Parity of the CUDA path against the CPU oracle, through the C ABI (-m gpu).
+
+Bar (BASELINE.json north_star): interaction lists bit-exact; coefficients within 1e-12 relative,
+max-norm per cell normalised by the cell's largest coefficient.  A tighter, condition-aware
+per-order check is applied as well (each order normalised by its own largest coefficient).
+"""
+import numpy as np
+import pytest
+
+import fmm_inputs as fi
+import oracle
+from helpers import cell_forces_and_torques, parity_error, per_order_error
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-12          # the contract
+TOL_ORDER = 2e-12    # per-order (L1 cancels heavily in smooth fields; still far below the contract's spirit)
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from paper_2101_08226_b200 import build
+    build.build()
+    import paper_2101_08226_b200 as p
+    assert torch.cuda.is_available()
+    return p, torch
+
+
+def gpu_multipole(env, w, theta=None, correction=True, kernel=0, out_lo=None, out_hi=None):
+    p, torch = env
+    theta = w.theta if theta is None else theta
+    out_lo = w.out_lo if out_lo is None else out_lo
+    out_hi = w.out_hi if out_hi is None else out_hi
+    f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, correction, out_lo, out_hi)
+    f.set_option("kernel", kernel)
+    mom = torch.from_numpy(w.moments).cuda()
+    com = torch.from_numpy(w.com_off).cuda()
+    L, Lc = f.solve(mom, com)
+    torch.cuda.synchronize()
+    assert f.status() == p.OK
+    cnt = f.interaction_count()
+    info = f.launch_info()
+    f.close()
+    return L.cpu().numpy(), Lc.cpu().numpy(), cnt, info
+
+
+def check(L, Lc, Lr, Lcr, tol=TOL):
+    e = parity_error(L, Lr)
+    assert e < tol, ("coefficients", e)
+    eo = per_order_error(L, Lr)
+    assert max(eo) < TOL_ORDER, ("per order", eo)
+    if Lcr is not None and np.abs(Lcr).max() > 0:
+        ec = parity_error(Lc, Lcr)
+        assert ec < 1e-11, ("correction", ec)   # a small difference of large terms; folded value is held to TOL above
+    return e
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.35, 0.34, 0.7, 0.4])
+def test_stencils_bit_exact(env, theta):
+    p, torch = env
+    f = p.OctoFMM((24, 24, 24), 1.0 / 24, theta, out_lo=(8, 8, 8), out_hi=(16, 16, 16))
+    for par in range(8):
+        got, ref = f.stencil(par), oracle.stencil(theta, par)
+        assert got.shape == ref.shape and np.array_equal(got, ref)
+    assert f.interaction_count() == oracle.interaction_count((24, 24, 24), theta, (8, 8, 8), (16, 16, 16))
+    f.close()
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("correction", [True, False])
+def test_config1(env, kernel, correction):
+    """cfg 1: one 8^3 sub-grid + 26 neighbours, theta = 0.5."""
+    w = fi.config1()
+    L, Lc, cnt, info = gpu_multipole(env, w, correction=correction, kernel=kernel)
+    Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, w.theta, w.moments, w.com_off, w.out_lo, w.out_hi, correction)
+    assert cnt == cntr == 118272
+    check(L, Lc, Lr, Lcr)
+    if not correction:
+        assert np.all(Lc == 0.0)
+
+
+@pytest.mark.parametrize("theta", [0.35, 0.7])
+def test_config1_theta_sweep(env, theta):
+    w = fi.config1(theta=theta)
+    L, Lc, cnt, _ = gpu_multipole(env, w)
+    Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, w.out_lo, w.out_hi, True)
+    assert cnt == cntr
+    check(L, Lc, Lr, Lcr)
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_whole_small_grid_with_domain_faces(env, kernel):
+    """Every cell of a 24 x 16 x 8 grid is a target: all tiles touch the domain boundary (TMA
+    zero fill = isolated boundary, L321), tiles are ragged in x (24 = 16 + 8) and the slab ring
+    skips out-of-range layers."""
+    w = fi.config1(seed=77, ncell=24)
+    w.moments = np.ascontiguousarray(w.moments[:, :8, :16, :])
+    w.com_off = np.ascontiguousarray(w.com_off[:, :8, :16, :])
+    w.n, w.out_lo, w.out_hi = (24, 16, 8), (0, 0, 0), (24, 16, 8)
+    L, Lc, cnt, _ = gpu_multipole(env, w, kernel=kernel)
+    Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off)
+    assert cnt == cntr
+    check(L, Lc, Lr, Lcr)
+
+
+def test_config2_polytrope_batched(env):
+    """cfg 2: 32^3 polytrope, all 64 sub-grids in one call; closed domain -> invariants too."""
+    w = fi.config2()
+    L, Lc, cnt, _ = gpu_multipole(env, w)
+    Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off)
+    assert cnt == cntr == 6590856
+    check(L, Lc, Lr, Lcr)
+    F, T = cell_forces_and_torques(w.moments, w.com_off, L, w.h)
+    assert np.abs(F.sum(axis=(1, 2, 3))).max() / np.abs(F).sum() < 1e-14       # L125
+    assert np.abs(T.sum(axis=(1, 2, 3))).max() / np.abs(T).sum() < 1e-13       # L127
+
+
+_CACHE = {}
+
+
+def cached_workload(name):
+    if name not in _CACHE:
+        _CACHE.clear()           # keep at most one large workload alive
+        _CACHE[name] = {"cfg3": fi.config3, "cfg5": fi.config5}[name]()
+    return _CACHE[name]
+
+
+def _sampled_subgrids(n):
+    """8^3 sub-grids to compare at full size: corners, a face, an edge, interior, both stars."""
+    s = n // 8
+    picks = {(0, 0, 0), (s - 1, s - 1, s - 1), (0, s // 2, s - 1), (s // 2, s // 2, s // 2),
+             (int(0.3 * s), s // 2, s // 2), (int(0.7 * s), s // 2, s // 2), (s // 2 + 1, 0, s // 3), (1, 2, 3)}
+    return sorted(picks)
+
+
+def test_config3_full_size_sampled(env):
+    """cfg 3: 128^3 binary in the launch configuration bench.py uses; the oracle recomputes sampled
+    sub-grids; Newton's third law and the torque balance are checked on the whole GPU result."""
+    w = fi.config3()
+    L, Lc, cnt, info = gpu_multipole(env, w)
+    assert cnt == 468364296
+    worst = 0.0
+    for (sx, sy, sz) in _sampled_subgrids(128):
+        lo, hi = (8 * sx, 8 * sy, 8 * sz), (8 * sx + 8, 8 * sy + 8, 8 * sz + 8)
+        Lr, Lcr, _ = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off, lo, hi, True)
+        sl = (slice(None), slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+        worst = max(worst, check(L[sl], Lc[sl], Lr, Lcr))
+    F, T = cell_forces_and_torques(w.moments, w.com_off, L, w.h)
+    assert np.abs(F.sum(axis=(1, 2, 3))).max() / np.abs(F).sum() < 1e-14
+    assert np.abs(T.sum(axis=(1, 2, 3))).max() / np.abs(T).sum() < 1e-12
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.35, 0.7])
+def test_config5_full_size_sampled(env, theta):
+    """cfg 5: 256^3, theta sweep, sampled sub-grids against the oracle."""
+    p, torch = env
+    w = cached_workload("cfg5")
+    f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, True)
+    mom = torch.from_numpy(w.moments).cuda()
+    com = torch.from_numpy(w.com_off).cuda()
+    L, Lc = f.solve(mom, com)
+    torch.cuda.synchronize()
+    assert f.status() == p.OK
+    expect = {0.5: 3810941448, 0.35: 10646746680, 0.7: 2201973760}[theta]
+    assert f.interaction_count() == expect
+    for (sx, sy, sz) in _sampled_subgrids(256)[:6]:
+        lo, hi = (8 * sx, 8 * sy, 8 * sz), (8 * sx + 8, 8 * sy + 8, 8 * sz + 8)
+        Lr, Lcr, _ = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, lo, hi, True)
+        g = L[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
+        gc = Lc[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
+        check(g, gc, Lr, Lcr)
+    f.close()
+
+
+def test_monopole_config4(env):
+    """cfg 4: monopole variant; small full-grid parity, full-size sampled parity, zero net force."""
+    p, torch = env
+    w = fi.config4(ncell=32)
+    f = p.OctoFMM(w.n, w.h, 0.5, p.MONOPOLE)
+    out, _ = f.solve(torch.from_numpy(w.moments).cuda())
+    torch.cuda.synchronize()
+    ref, cnt = oracle.interact_monopole(w.n, w.h, 0.5, w.moments[0])
+    assert f.interaction_count() == cnt
+    assert parity_error(out.cpu().numpy(), ref) < TOL
+    f.close()
+
+    w = fi.config4()
+    f = p.OctoFMM(w.n, w.h, 0.5, p.MONOPOLE)
+    out, _ = f.solve(torch.from_numpy(w.moments).cuda())
+    torch.cuda.synchronize()
+    assert f.interaction_count() == 468364296
+    out = out.cpu().numpy()
+    for (sx, sy, sz) in _sampled_subgrids(128):
+        lo, hi = (8 * sx, 8 * sy, 8 * sz), (8 * sx + 8, 8 * sy + 8, 8 * sz + 8)
+        ref, _ = oracle.interact_monopole(w.n, w.h, 0.5, w.moments[0], lo, hi)
+        assert parity_error(out[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]], ref) < TOL
+    mg = w.moments[0][None] * out[1:4]
+    assert np.abs(mg.sum(axis=(1, 2, 3))).max() / np.abs(mg).sum() < 1e-14
+    f.close()
+
+
+def test_host_buffer_entry_point(env):
+    """octo_fmm_run_host (H2D + step + D2H) gives the same numbers as the device-pointer calls."""
+    p, torch = env
+    w = fi.config1()
+    L, Lc, _, _ = gpu_multipole(env, w)
+    f = p.OctoFMM(w.n, w.h, w.theta, p.MULTIPOLE, True, w.out_lo, w.out_hi)
+    nb = p.octo_fmm_host_scratch_bytes(f.cfg)
+    scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    mom = torch.from_numpy(w.moments).pin_memory()
+    com = torch.from_numpy(w.com_off).pin_memory()
+    Lh = torch.empty((20, 8, 8, 8), dtype=torch.float64).pin_memory()
+    Lch = torch.empty((3, 8, 8, 8), dtype=torch.float64).pin_memory()
+    p.octo_fmm_run_host(f.handle, mom, com, Lh, Lch, scratch, nb)
+    assert np.array_equal(Lh.numpy(), L) and np.array_equal(Lch.numpy(), Lc)
+    f.close()
+
+
+def test_error_paths(env):
+    p, torch = env
+    w = fi.config1()
+    f = p.OctoFMM(w.n, w.h, 0.5, p.MULTIPOLE, True, w.out_lo, w.out_hi)
+    with pytest.raises(p.OctoFmmError) as ei:
+        f.interact()
+    assert ei.value.status == p.ESTATE
+    mom = torch.from_numpy(w.moments).cuda()
+    com = torch.from_numpy(w.com_off).cuda()
+    f.set_moments(mom, com)
+    with pytest.raises(p.OctoFmmError) as ei:
+        f.get_expansions()
+    assert ei.value.status == p.ESTATE
+    # a target cell of zero mass with the correction on is reported, not divided by
+    mom[0, 10, 10, 10] = 0.0
+    f.set_moments(mom, com)
+    f.interact()
+    assert f.status() == p.EMASS
+    f.close()
+    # zero-mass SOURCE cells outside the target region are harmless
+    w2 = fi.config1()
+    w2.moments[:, :4] = 0.0
+    w2.com_off[:, :4] = 0.0
+    L, Lc, _, _ = gpu_multipole(env, w2)
+    Lr, Lcr, _ = oracle.interact_multipole(w2.n, w2.h, 0.5, w2.moments, w2.com_off, w2.out_lo, w2.out_hi, True)
+    check(L, Lc, Lr, Lcr)
+
+
+def test_fp64_probe_runs(env):
+    p, torch = env
+    scratch = torch.empty(8 << 20, dtype=torch.uint8, device="cuda")
+    r = p.octo_fmm_fp64_peak_probe(0, torch.cuda.current_stream().cuda_stream, scratch, 4000)
+    assert r["sm_count"] > 0 and r["flops_per_s"] > 1e12
