@@ -1,0 +1,357 @@
+#!/usr/bin/env python
+"""Benchmark of the FMM cell-to-cell interaction step (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfg5|cfg3|cfg2] [--theta 0.5] [--ncell 256]
+
+A "step" is one pass of the whole hot path over one batch: stage the sources (set_moments), the
+interaction kernel (interact), store/copy the expansions (get_expansions).  Default workload is
+config 5 (256^3 cells = 32768 sub-grids, two-polytrope binary, theta = 0.5, correction on), the
+configuration BASELINE.json's metric is quoted on.  Prints ONE JSON line (rank 0).
+
+N > 1 (torchrun): every rank runs an independent problem of the same shape (its own seed) --
+the path shards by sub-problem with no data-path collective ("scaling": "weak"); timing is the
+max over ranks between barriers.
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on the host cores on a
+bounded sample of the same workload; it is a deliberately plain program, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fmm_cell_interactions_per_s"
+UNIT = "interactions/s"
+FP64_LANES_PER_SM = 64        # FP64 FMA lanes per SM per clock on B200 (37.2 TFLOP/s at 148 SMs x 1965 MHz)
+
+
+def env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def make_workload(name, theta, ncell, seed):
+    import fmm_inputs as fi
+    if name == "cfg5":
+        w = fi.config5(seed=seed, theta=theta, ncell=ncell or 256)
+    elif name == "cfg3":
+        w = fi.config3(seed=seed, theta=theta, ncell=ncell or 128)
+    elif name == "cfg2":
+        w = fi.config2(seed=seed, theta=theta, ncell=ncell or 32)
+    else:
+        raise SystemExit("unknown workload " + name)
+    return w
+
+
+def sample_regions(ncell, nregions, edge=16):
+    """Stratified, deterministic sample of edge^3-cell regions (8 sub-grids each): corners,
+    faces and interior of the lattice of regions."""
+    m = ncell // edge
+    picks = []
+    i = 0
+    while len(picks) < min(nregions, m ** 3):
+        # low-discrepancy walk over the region lattice (includes (0,0,0) and boundary regions)
+        a = (i * 7) % m
+        b = (i * 11 + i // m) % m
+        c = (i * 13 + i // (m * m) + (i // 3)) % m
+        if (a, b, c) not in picks:
+            picks.append((a, b, c))
+        i += 1
+    return [((a * edge, b * edge, c * edge), ((a + 1) * edge, (b + 1) * edge, (c + 1) * edge)) for a, b, c in picks]
+
+
+def oracle_sample(w, theta, nregions):
+    """Time the oracle, as it stands, on a bounded sample of the workload.  Returns
+    (interactions, seconds, threads)."""
+    import oracle
+    regions = sample_regions(w.n[0], nregions)
+    oracle.lib()
+    t0 = time.perf_counter()
+    total = 0
+    for lo, hi in regions:
+        _, _, cnt = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, lo, hi, True)
+        total += cnt
+    return total, time.perf_counter() - t0, oracle.num_threads(), len(regions)
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1] or [r for (_, r) in self.rows[-3:]]
+        sm, smax, power, reasons = [], None, [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0]))
+                smax = float(f[1])
+                power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, val in zip(names, f[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(nme)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": smax,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, bounded sample per step."""
+    rank = env_int("RANK", 0)
+    if rank != 0:
+        return
+    w = make_workload(args.workload, args.theta, args.ncell, args.seed)
+    nreg = args.ref_regions
+    for _ in range(args.warmup):
+        oracle_sample(w, args.theta, 1)
+    tot, secs = 0, 0.0
+    threads = 1
+    for _ in range(args.steps):
+        c, s, threads, nr = oracle_sample(w, args.theta, nreg)
+        tot += c
+        secs += s
+    value = tot / secs
+    sample = "%d regions of 16^3 cells (%d sub-grids) per step of %s" % (nreg, 8 * nreg, w.name)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s theta=%g correction=on" % (w.name, args.theta), "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    world = env_int("WORLD_SIZE", 1)
+    rank = env_int("RANK", 0)
+    local = env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2101_08226_b200 import build
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2101_08226_b200 as p
+
+    # independent problem per rank (weak scaling): same shape, own seed
+    w = make_workload(args.workload, args.theta, args.ncell, args.seed + rank)
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream(dev)
+    f = p.OctoFMM(w.n, w.h, args.theta, p.MULTIPOLE, True, device=local, stream=stream)
+    n_int = f.interaction_count()
+    info = f.launch_info()
+    flops_per, instr_per = p.octo_fmm_flops_per_interaction(p.MULTIPOLE, True)
+
+    mom = torch.from_numpy(w.moments).to(dev)
+    com = torch.from_numpy(w.com_off).to(dev)
+    L = torch.empty((20,) + f.out_shape, dtype=torch.float64, device=dev)
+    Lc = torch.empty((3,) + f.out_shape, dtype=torch.float64, device=dev)
+
+    def step():
+        f.set_moments(mom, com)
+        f.interact()
+        f.get_expansions(L, Lc)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    # ---- timed region: device-resident inputs ----
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t_begin = time.perf_counter()
+    ev0.record(stream)
+    for i in range(args.steps):
+        f.set_moments(mom, com)
+        kev[i][0].record(stream)
+        f.interact()
+        kev[i][1].record(stream)
+        f.get_expansions(L, Lc)
+    ev1.record(stream)
+    barrier()
+    t_end = time.perf_counter()
+    clocks = sampler.stop(t_begin, t_end)
+    ms_total = ev0.elapsed_time(ev1)
+    kernel_ms = sum(a.elapsed_time(b) for a, b in kev) / args.steps
+    if f.status() != p.OK:
+        raise SystemExit("bench.py: device reported status %d" % f.status())
+    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total = float(tmax.item())
+    ms_per_step = ms_total / args.steps
+    value = world * n_int * args.steps / (ms_total * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (H2D + step + D2H inside the timed region) ----
+    e2e = None
+    if args.e2e_steps > 0:
+        nb = p.octo_fmm_host_scratch_bytes(f.cfg)
+        scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
+        mom_h = torch.from_numpy(w.moments).pin_memory()
+        com_h = torch.from_numpy(w.com_off).pin_memory()
+        L_h = torch.empty((20,) + f.out_shape, dtype=torch.float64).pin_memory()
+        Lc_h = torch.empty((3,) + f.out_shape, dtype=torch.float64).pin_memory()
+        p.octo_fmm_run_host(f.handle, mom_h, com_h, L_h, Lc_h, scratch, nb)       # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(args.e2e_steps):
+            p.octo_fmm_run_host(f.handle, mom_h, com_h, L_h, Lc_h, scratch, nb)
+        b.record(stream)
+        barrier()
+        e2e_ms = max(a.elapsed_time(b), 1e3 * (time.perf_counter() - t0))
+        t2 = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t2.item())
+        e2e = {"value": world * n_int * args.e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(mom_h.numel() * 8 + com_h.numel() * 8),
+               "d2h_bytes_per_step": int(L_h.numel() * 8 + Lc_h.numel() * 8),
+               "steps": args.e2e_steps, "ms_per_step": e2e_ms / args.e2e_steps,
+               "checksum_L0": float(L_h[0].sum())}
+        del scratch, mom_h, com_h, L_h, Lc_h
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the interaction kernel), FP64 ALU bound ----
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    peak_tflops = sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    probe_scratch = torch.empty(8 << 20, dtype=torch.uint8, device=dev)
+    probe = p.octo_fmm_fp64_peak_probe(local, stream.cuda_stream, probe_scratch, 40000)
+    achieved = flops_per * n_int / (kernel_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "m2l_staged_kernel<correction>", "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                "peak_source": "derived: %d SMs x %d FP64 FMA lanes x 2 x %.0f MHz (sm_max_mhz of %s)" % (
+                    sm_count, FP64_LANES_PER_SM, sm_max_mhz, "MEASURED_PEAKS.json" if peaks else "nvidia-smi"),
+                "peak_measured_dfma": probe["flops_per_s"] / 1e12,
+                "frac_of_measured_dfma": achieved / (probe["flops_per_s"] / 1e12),
+                "flops_per_interaction": flops_per, "fp64_instr_per_interaction": instr_per,
+                "fp64_pipe_issue_frac": (instr_per * n_int / (kernel_ms * 1e-3)) / (sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
+                "kernel_ms": kernel_ms, "interactions_per_launch": n_int,
+                "traffic": TRAFFIC_BYTES.get((args.workload, args.ncell or 256, args.theta)),
+                "algorithmic_bytes": int((23 + 23) * 8 * w.moments[0].size),
+                "hbm_gbs_at_algorithmic_bytes": (23 + 23) * 8 * w.moments[0].size / (kernel_ms * 1e-3) / 1e9,
+                "hbm_peak_gbs": peaks.get("hbm_gbs")}
+
+    # ---- the oracle timed beside it on this box's host cores (bounded sample) ----
+    c, s, threads, nr = oracle_sample(w, args.theta, args.ref_regions)
+    cpu_baseline = {"value": c / s, "unit": UNIT, "cores": threads, "kind": "oracle",
+                    "sample": "%d regions of 16^3 cells (%d sub-grids, %d interactions) of %s in %.1f s" % (
+                        nr, 8 * nr, c, w.name, s)}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s theta=%g correction=on (%d^3 cells, %d sub-grids of 8^3)" % (
+                w.name, args.theta, w.n[0], (w.n[0] // 8) ** 3),
+                "interactions_per_step": n_int, "l2": "inputs (%.2f GB) larger than L2" % (mom.numel() * 8 / 1e9),
+                "launch": info, "parallelism": "independent problem per GPU" if world > 1 else "single GPU"},
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
+            "gpu_launches": 2 * args.steps}
+    print(json.dumps(line))
+    f.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of the interaction kernel, one `ncu --set full` capture
+# per entry (profiles/); None until captured for that workload.
+TRAFFIC_BYTES = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--theta", type=float, default=0.5)
+    ap.add_argument("--ncell", type=int, default=0)
+    ap.add_argument("--seed", type=int, default=20210108)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--ref-regions", type=int, default=32)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
