@@ -1,8 +1,8 @@
 """Python binding of the octo_fmm C ABI (include/octo_fmm.h): argument marshalling only.
 
 Every step of the hot path runs in the CUDA kernels of libocto_fmm.so; PyTorch provides device
-memory and the stream.  There is no CPU fallback: if the shared library is missing, importing
-this package raises.  Build it with `python -m paper_2101_08226_b200.build` (or
+memory and the stream.  There is no CPU fallback: if the shared library is missing, the first
+call into the library raises ImportError.  Build it with `python -m paper_2101_08226_b200.build` (or
 `__graft_entry__.build()`).
 
 The module-level functions carry the C names (octo_fmm_create, ...); `OctoFMM` is a small
@@ -34,31 +34,49 @@ class octo_fmm_config(ctypes.Structure):
                 ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
 
 
-if not os.path.exists(_LIB_PATH):
-    raise ImportError("paper_2101_08226_b200: %s is missing -- build it with "
-                      "`python -m paper_2101_08226_b200.build`; there is no CPU fallback" % _LIB_PATH)
-_lib = ctypes.CDLL(_LIB_PATH)
+class _Library:
+    """Loads libocto_fmm.so on first use and fails loudly when it is missing (no CPU fallback).
 
-_vp, _ip, _dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)
-_cfgp = ctypes.POINTER(octo_fmm_config)
-_lib.octo_fmm_workspace_bytes.restype = ctypes.c_size_t
-_lib.octo_fmm_workspace_bytes.argtypes = [_cfgp]
-_lib.octo_fmm_host_scratch_bytes.restype = ctypes.c_size_t
-_lib.octo_fmm_host_scratch_bytes.argtypes = [_cfgp]
-_lib.octo_fmm_create.argtypes = [_cfgp, ctypes.POINTER(_vp)]
-_lib.octo_fmm_set_moments.argtypes = [_vp, _vp, _vp]
-_lib.octo_fmm_interact.argtypes = [_vp]
-_lib.octo_fmm_get_expansions.argtypes = [_vp, _vp, _vp]
-_lib.octo_fmm_destroy.argtypes = [_vp]
-_lib.octo_fmm_get_stencil.argtypes = [_vp, ctypes.c_int, _ip, _vp]
-_lib.octo_fmm_interaction_count.argtypes = [_vp, ctypes.POINTER(ctypes.c_ulonglong)]
-_lib.octo_fmm_status.argtypes = [_vp]
-_lib.octo_fmm_run_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_size_t]
-_lib.octo_fmm_set_option.argtypes = [_vp, ctypes.c_char_p, ctypes.c_int]
-_lib.octo_fmm_launch_info.argtypes = [_vp, _ip, _ip, _ip, _ip, _ip]
-_lib.octo_fmm_fp64_peak_probe.argtypes = [ctypes.c_int, _vp, _vp, ctypes.c_int, _dp, _ip, _ip]
-_lib.octo_fmm_flops_per_interaction.argtypes = [ctypes.c_int, ctypes.c_int, _ip, _ip]
-_lib.octo_fmm_version.restype = ctypes.c_char_p
+    Loading is deferred only so that `paper_2101_08226_b200.build` can be imported to produce it."""
+
+    def __init__(self):
+        self._cdll = None
+
+    def _load(self):
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError("paper_2101_08226_b200: %s is missing -- build it with "
+                              "`python -m paper_2101_08226_b200.build`; there is no CPU fallback" % _LIB_PATH)
+        lib = ctypes.CDLL(_LIB_PATH)
+        vp, ip, dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)
+        cfgp = ctypes.POINTER(octo_fmm_config)
+        lib.octo_fmm_workspace_bytes.restype = ctypes.c_size_t
+        lib.octo_fmm_workspace_bytes.argtypes = [cfgp]
+        lib.octo_fmm_host_scratch_bytes.restype = ctypes.c_size_t
+        lib.octo_fmm_host_scratch_bytes.argtypes = [cfgp]
+        lib.octo_fmm_create.argtypes = [cfgp, ctypes.POINTER(vp)]
+        lib.octo_fmm_set_moments.argtypes = [vp, vp, vp]
+        lib.octo_fmm_interact.argtypes = [vp]
+        lib.octo_fmm_get_expansions.argtypes = [vp, vp, vp]
+        lib.octo_fmm_destroy.argtypes = [vp]
+        lib.octo_fmm_get_stencil.argtypes = [vp, ctypes.c_int, ip, vp]
+        lib.octo_fmm_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
+        lib.octo_fmm_status.argtypes = [vp]
+        lib.octo_fmm_run_host.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_size_t]
+        lib.octo_fmm_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
+        lib.octo_fmm_launch_info.argtypes = [vp, ip, ip, ip, ip, ip]
+        lib.octo_fmm_fp64_peak_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, dp, ip, ip]
+        lib.octo_fmm_flops_per_interaction.argtypes = [ctypes.c_int, ctypes.c_int, ip, ip]
+        lib.octo_fmm_version.restype = ctypes.c_char_p
+        self._cdll = lib
+
+    def __getattr__(self, name):
+        if self._cdll is None:
+            self._load()
+        return getattr(self._cdll, name)
+
+
+_lib = _Library()
+_vp = ctypes.c_void_p
 
 
 def _ptr(t):
