@@ -27,19 +27,22 @@ namespace octo {
 
 constexpr int REACH_MAX = 5;            // theta_min = 0.34 for 8^3 sub-grids
 constexpr int MAX_LIST = 651;           // |S_p| for 1/3 < theta (7 * 93)
-constexpr int TILE = 16;                // target tile: 16 x 16 cells of one z-layer
+constexpr int TILE_X = 16;              // target brick of one CTA pass: 16 x 8 x 3 cells = 12 warps
+constexpr int TILE_Y = 8;
+constexpr int TILE_Z = 3;
 constexpr int NPAIR = (NCOMP + 1) / 2;  // 10 component pairs
-constexpr int SLAB_XH = 13;             // half-row length in the slab: (16 + 2*5) / 2
+constexpr int SLAB_XH = (TILE_X + 2 * REACH_MAX) / 2;   // 13: half-row length in the slab
 constexpr int SLAB_ROW = 2 * SLAB_XH;   // 26 double2 per y-row (even half, odd half)
-constexpr int SLAB_Y = TILE + 2 * REACH_MAX;      // 26
-constexpr int SLAB_PLANE = SLAB_Y * SLAB_ROW;     // 676 double2 per component pair
-constexpr int SLAB_ELEMS = NPAIR * SLAB_PLANE;    // 6760 double2
-constexpr int SLAB_BYTES = SLAB_ELEMS * 16;       // 108160 = 845 * 128 (TMA transaction size, 128-B aligned)
+constexpr int SLAB_Y = TILE_Y + 2 * REACH_MAX;    // 18
+constexpr int SLAB_PLANE = SLAB_Y * SLAB_ROW;     // 468 double2 per component pair
+constexpr int SLAB_ELEMS = NPAIR * SLAB_PLANE;    // 4680 double2
+constexpr int SLAB_BYTES = SLAB_ELEMS * 16;       // 74880 = 585 * 128 (TMA transaction size, 128-B aligned)
 static_assert(SLAB_BYTES % 128 == 0, "TMA needs 128-byte aligned shared-memory destinations");
-constexpr int NSTAGE = 2;
-constexpr int CONSUMER_WARPS = 8;
+constexpr int NSTAGE = 3;
+constexpr int CONSUMER_WARPS = 4 * TILE_Z;        // one warp per (xy-parity class, layer of the brick)
 constexpr int STAGED_THREADS = (CONSUMER_WARPS + 1) * 32;   // + 1 producer warp
 constexpr int STAGED_SMEM = NSTAGE * SLAB_BYTES + 64;
+static_assert(STAGED_SMEM <= 227 * 1024, "shared memory per CTA");
 
 struct StEntry {
     int off;                 // staged kernel: shared-memory offset (double2) relative to the thread's base
@@ -55,8 +58,8 @@ struct Params {
     int nx, ny, nz;
     int lo[3], hi[3];        // output region
     int ox, oy, oz;          // its extents
-    int tiles_x, tiles_y;    // 16 x 16 tiles covering the output region
-    long long ntiles;        // tiles_x * tiles_y * oz
+    int tiles_x, tiles_y, tiles_z;   // 16 x 8 x 3 bricks covering the output region
+    long long ntiles;        // tiles_x * tiles_y * tiles_z
     int reach;
     const double* S;         // staged sources
     double* L;               // [20][oz][oy][ox]
@@ -120,6 +123,23 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
             : "memory");
     } while (!done);
 }
+// the producer's wait: sleeps between polls so that its spin does not take issue slots from the
+// consumer warps of its sub-partition (a slab lasts ~10 us; the poll interval is ~0.25 us)
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    for (;;) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+        if (done) break;
+        __nanosleep(256);
+    }
+}
 __device__ __forceinline__ void tma_load_slab(void* dst, const CUtensorMap* map, uint64_t* bar, int c1, int c2, int c4)
 {
     asm volatile(
@@ -129,24 +149,28 @@ __device__ __forceinline__ void tma_load_slab(void* dst, const CUtensorMap* map,
         : "memory");
 }
 
-// tile id -> (tile x, tile y, layer); the layer runs fastest so that the CTAs resident at one
-// time walk up a few columns and share their slabs through L2.
-__device__ __forceinline__ void decode_tile(const Params& p, long long t, int& x0, int& y0, int& k)
+// brick id -> lower corner; z runs fastest so that the CTAs resident at one time walk up a few
+// columns and share their slabs through L2.
+__device__ __forceinline__ void decode_tile(const Params& p, long long t, int& x0, int& y0, int& k0)
 {
-    k = p.lo[2] + (int)(t % p.oz);
-    const long long c = t / p.oz;
-    x0 = p.lo[0] + (int)(c % p.tiles_x) * TILE;
-    y0 = p.lo[1] + (int)(c / p.tiles_x) * TILE;
+    k0 = p.lo[2] + (int)(t % p.tiles_z) * TILE_Z;
+    const long long c = t / p.tiles_z;
+    x0 = p.lo[0] + (int)(c % p.tiles_x) * TILE_X;
+    y0 = p.lo[1] + (int)(c / p.tiles_x) * TILE_Y;
 }
 
 // ------------------------------------------------------------------------------------------
-// a3/a4/a6, default: persistent CTAs, one 16x16x1 target tile at a time, one cell per thread.
-// Warp w (< 8) holds the 32 cells of xy-parity class w >> 1 in tile rows 8 (w & 1) + {0..7}
-// (every lane of a warp runs the same interaction list, no masks); warp 8 is the TMA producer.
-// For dz = -reach..reach the z-slab k + dz (tile + 5-cell halo, all 19 components) is brought
-// in by one TMA box; the two slab buffers form a full/empty mbarrier ring that keeps running
-// across tiles.  Out-of-grid parts of a box are zero-filled by TMA = zero-mass cells with zero
-// offset, which contribute exactly 0 to every coefficient (isolated boundary, L321).
+// a3/a4/a6, default: persistent CTAs, one 16 x 8 x 3 target brick at a time, one cell per thread.
+// Consumer warp w (< 12) holds the 32 cells of xy-parity class w & 3 in layer k0 + (w >> 2) of the
+// brick (every lane of a warp runs the same interaction list, no masks); warp 12 is the TMA
+// producer.  The z-slabs k0 - reach .. k0 + 2 + reach (brick + 5-cell halo in x and y, all 19
+// components, 74880 bytes) are brought in by one TMA box each and are shared by the three layers:
+// a warp of layer k uses slab zz with dz = zz - k when |dz| <= reach and only releases it
+// otherwise.  The three slab buffers form a full/empty mbarrier ring that keeps running across
+// bricks.  Twelve consumer warps (three per sub-partition) is what the FP64 pipe needs to stay
+// busy at the instruction-level parallelism of the pair arithmetic (profiles/r01_*.md).
+// Out-of-grid parts of a box are zero-filled by TMA = zero-mass cells with zero offset, which
+// contribute exactly 0 to every coefficient (isolated boundary, L321).
 // ------------------------------------------------------------------------------------------
 // load the 19 staged components of one source cell (10 double2, stride `stride` double2)
 #define OCTO_LOAD_SOURCE(q, stride, src, bx_, by_, bz_)                                   \
@@ -221,13 +245,12 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
         if (lane == 0) {
             uint32_t it = 0;
             for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
-                int x0, y0, k;
-                decode_tile(p, t, x0, y0, k);
-                for (int dz = -p.reach; dz <= p.reach; ++dz) {
-                    const int zz = k + dz;
-                    if (zz < 0 || zz >= p.nz) continue;
+                int x0, y0, k0;
+                decode_tile(p, t, x0, y0, k0);
+                const int z_lo = max(k0 - p.reach, 0), z_hi = min(k0 + TILE_Z - 1 + p.reach, p.nz - 1);
+                for (int zz = z_lo; zz <= z_hi; ++zz) {
                     const uint32_t b = it % NSTAGE;
-                    if (it >= NSTAGE) mbar_wait(&empty[b], ((it / NSTAGE) - 1) & 1);
+                    if (it >= NSTAGE) mbar_wait_backoff(&empty[b], ((it / NSTAGE) - 1) & 1);
                     mbar_arrive_expect_tx(&full[b], SLAB_BYTES);
                     tma_load_slab(slab0 + (size_t)b * SLAB_ELEMS, &tmap, &full[b], (x0 >> 1) - 3, 2 * (y0 - REACH_MAX), zz);
                     ++it;
@@ -238,19 +261,23 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
     }
 
     // ------------------------------ consumers ------------------------------
-    const int cls_xy = warp >> 1;                      // px + 2 py
+    const int cls_xy = warp & 3;                       // px + 2 py
+    const int layer = warp >> 2;                       // 0..2
     const int px = cls_xy & 1, py = cls_xy >> 1;
     const int lx = lane & 7;
-    const int ly = ((warp & 1) << 2) + (lane >> 3);    // 0..7
+    const int ly = lane >> 3;                          // 0..3
     const int tbase = lx + 2 * ly * SLAB_ROW;          // double2
 
     uint32_t it = 0;
     for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
-        int x0, y0, k;
-        decode_tile(p, t, x0, y0, k);
+        int x0, y0, k0;
+        decode_tile(p, t, x0, y0, k0);
+        const int k = k0 + layer;
         const int gx = x0 + px + 2 * lx, gy = y0 + py + 2 * ly;
-        const bool active = gx < p.hi[0] && gy < p.hi[1];
+        const bool layer_on = k < p.hi[2];             // warp-uniform
+        const bool active = layer_on && gx < p.hi[0] && gy < p.hi[1];
         const int cls = cls_xy + ((k & 1) << 2);
+        const int z_hi = min(k0 + TILE_Z - 1 + p.reach, p.nz - 1);
 
         double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         if (active) load_target<CORR>(p, gx, gy, k, dA, tA);
@@ -258,29 +285,65 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
         Acc acc;
         acc_zero(acc);
 
-        for (int dz = -p.reach; dz <= p.reach; ++dz) {
-            const int zz = k + dz;
-            if (zz < 0 || zz >= p.nz) continue;
-            const uint32_t b = it % NSTAGE;
-            mbar_wait(&full[b], (it / NSTAGE) & 1);
-            const double2* sl = slab0 + (size_t)b * SLAB_ELEMS + tbase;
-            const double Rz0 = c_hmul[dz + REACH_MAX] + dA[2];
-            const int s_begin = c_begin[cls][dz + REACH_MAX], s_end = c_begin[cls][dz + REACH_MAX + 1];
-#pragma unroll 1
-            for (int s = s_begin; s < s_end; ++s) {
-                const StEntry e = c_entries[cls * MAX_LIST + s];
-                const double2* q = sl + e.off;
-                double src[16], bx, by, bz;
-                OCTO_LOAD_SOURCE(q, SLAB_PLANE, src, bx, by, bz);
-                const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx);
-                const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by);
-                const double z = Rz0 - bz;
-                m2l_pair<CORR>(acc, x, y, z, src, tA);
+        // Walk the slabs dz = -reach..reach of this tile and, inside each, the list segment of
+        // (class, dz).  The loop is software-pipelined by hand: `fetch` loads pair s+1 from shared
+        // memory and runs its head (separation, r^2, 1/r) while the body of pair s executes, so the
+        // dependent head chain is hidden although only two warps share a sub-partition's FP64 pipe.
+        int zz = max(k0 - p.reach, 0) - 1;
+        int s = 0, s_end = 0;
+        bool open = false;
+        uint32_t b = 0;
+        const double2* sl = slab0;
+        double Rz0 = 0.0;
+        // make (s < s_end) true by moving on to the next slab this layer uses; every slab of the
+        // brick is waited for and released, used or not.  false at the end of the brick.
+        auto ensure = [&]() -> bool {
+            while (s >= s_end) {
+                if (open) {                        // every load from this slab has been issued
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&empty[b]);
+                    ++it;
+                    open = false;
+                }
+                if (++zz > z_hi) return false;
+                b = it % NSTAGE;
+                mbar_wait(&full[b], (it / NSTAGE) & 1);
+                open = true;
+                const int dz = zz - k;
+                if (layer_on && dz >= -p.reach && dz <= p.reach) {
+                    sl = slab0 + (size_t)b * SLAB_ELEMS + tbase;
+                    Rz0 = c_hmul[dz + REACH_MAX] + dA[2];
+                    s = cls * MAX_LIST + c_begin[cls][dz + REACH_MAX];
+                    s_end = cls * MAX_LIST + c_begin[cls][dz + REACH_MAX + 1];
+                }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[b]);
-            ++it;
+            return true;
+        };
+#define OCTO_FETCH(P)                                                                       \
+        {                                                                                   \
+            const StEntry e_ = c_entries[s];                                                \
+            ++s;                                                                            \
+            double bx_, by_, bz_;                                                           \
+            OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_);                \
+            P.x = c_hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                                \
+            P.y = c_hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                                \
+            P.z = Rz0 - bz_;                                                                \
+            P.w = pair_head(P.x, P.y, P.z);                                                 \
         }
+        struct Fetched { double src[16]; double x, y, z, w; } A, B;
+        if (ensure()) {
+            OCTO_FETCH(A);
+            for (;;) {
+                if (!ensure()) break;
+                OCTO_FETCH(B);
+                m2l_pair<CORR>(acc, A.x, A.y, A.z, A.w, A.src, tA);
+                if (!ensure()) { A = B; break; }
+                OCTO_FETCH(A);
+                m2l_pair<CORR>(acc, B.x, B.y, B.z, B.w, B.src, tA);
+            }
+            m2l_pair<CORR>(acc, A.x, A.y, A.z, A.w, A.src, tA);
+        }
+#undef OCTO_FETCH
 
         if (active) store_target<CORR>(p, acc, gx, gy, k);
     }
@@ -323,7 +386,7 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
             const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
             const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by_);
             const double z = c_hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
-            m2l_pair<CORR>(acc, x, y, z, src, tA);
+            m2l_pair<CORR>(acc, x, y, z, pair_head(x, y, z), src, tA);
         }
         store_target<CORR>(p, acc, gx, gy, k);
     }

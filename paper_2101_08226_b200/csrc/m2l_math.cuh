@@ -81,14 +81,20 @@ __device__ __forceinline__ void reduce_moments(const double M[20], double* s)
     s[C_OYYZ] = -(3.0 * M[17] - M[19]) * (1.0 / 6.0);
 }
 
-// One ordered pair A <- B.  (x,y,z) = R = z_A - z_B; s[0..15] staged source components;
-// tA[0..6] = staged third moments of the target divided by its mass (correction only).
-template <bool CORR>
-__device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y, const double z,
-                                         const double (&s)[16], const double (&tA)[7])
+// Head of one ordered pair: 1/|R|.  Kept apart from the body so that the kernels can run the
+// head of pair s+1 (a long dependent chain: r^2 -> MUFU -> correction step) under the body of pair s.
+__device__ __forceinline__ double pair_head(const double x, const double y, const double z)
 {
     const double r2 = fma(z, z, fma(y, y, x * x));
-    const double w = rsqrt_fast(r2);          // 1/r
+    return rsqrt_fast(r2);
+}
+
+// Body of one ordered pair A <- B.  (x,y,z) = R = z_A - z_B, w = 1/|R|; s[0..15] staged source
+// components; tA[0..6] = staged third moments of the target divided by its mass (correction only).
+template <bool CORR>
+__device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y, const double z, const double w,
+                                         const double (&s)[16], const double (&tA)[7])
+{
     const double w2 = w * w;                  // 1/r^2
     const double d1 = w * w2;                 // 1/r^3
     const double d2 = d1 * (-3.0 * w2);       // -3/r^5

@@ -252,8 +252,9 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     P.nx = cfg->n[0]; P.ny = cfg->n[1]; P.nz = cfg->n[2];
     for (int a = 0; a < 3; ++a) { P.lo[a] = h->lo[a]; P.hi[a] = h->hi[a]; }
     P.ox = h->hi[0] - h->lo[0]; P.oy = h->hi[1] - h->lo[1]; P.oz = h->hi[2] - h->lo[2];
-    P.tiles_x = (P.ox + TILE - 1) / TILE; P.tiles_y = (P.oy + TILE - 1) / TILE;
-    P.ntiles = (long long)P.tiles_x * P.tiles_y * P.oz;
+    P.tiles_x = (P.ox + TILE_X - 1) / TILE_X; P.tiles_y = (P.oy + TILE_Y - 1) / TILE_Y;
+    P.tiles_z = (P.oz + TILE_Z - 1) / TILE_Z;
+    P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
     P.reach = h->reach;
     P.S = h->src; P.L = h->L; P.C = h->C; P.flags = h->flags;
 
