@@ -27,7 +27,7 @@ enum {
 };
 
 struct Acc {
-    double l0;
+    double l0, l0b; // two partial sums of L0
     double l1[3];
     double l2[5];   // xx xy xz yy yz
     double l3[7];   // xxx xxy xxz xyy xyz yyy yyz
@@ -37,6 +37,7 @@ struct Acc {
 __device__ __forceinline__ void acc_zero(Acc& a)
 {
     a.l0 = 0.0;
+    a.l0b = 0.0;
 #pragma unroll
     for (int i = 0; i < 3; ++i) { a.l1[i] = 0.0; a.c[i] = 0.0; }
 #pragma unroll
@@ -100,11 +101,42 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
     const double d2 = d1 * (-3.0 * w2);       // -3/r^5
     const double d3 = d2 * (-5.0 * w2);       // 15/r^7
 
-    // ---- D1, D2 (6 components; zz is needed by the dipole term of L1_z) ----
+    const double m0 = s[C_M0], m1x = s[C_M1X], m1y = s[C_M1Y], m1z = s[C_M1Z];
+    const double qxx = s[C_QXX], qxy = s[C_QXY], qxz = s[C_QXZ], qyy = s[C_QYY], qyz = s[C_QYZ];
+    const double oxxx = s[C_OXXX], oxxy = s[C_OXXY], oxxz = s[C_OXXZ], oxyy = s[C_OXYY], oxyz = s[C_OXYZ],
+                 oyyy = s[C_OYYY], oyyz = s[C_OYYZ];
+
+    // The contractions
+    //   L0     += M D0 - M1.D1 + 1/2 M2:D2 - 1/6 M3:.D3
+    //   L1_i   += M D1_i - M1_j D2_ij + 1/2 M2_jk D3_ijk
+    //   L2_ij  += M D2_ij - M1_k D3_ijk            (xx xy xz yy yz)
+    //   L3_ijk += M D3_ijk                         (xxx xxy xxz xyy xyz yyy yyz)
+    // are written as RUNS that share one component of D, each right after that component is
+    // generated: a DFMA with three fresh register operands issues at 2/3 of the FP64 rate on
+    // sm_100 (register-read bound, measured), one that repeats an operand of the previous
+    // instruction in the same slot takes it from the operand-reuse cache and issues at full rate.
+    // Every run updates distinct accumulators; L0 alternates between two partial sums.
+
+    // ---- D0, D1 ----
+    a.l0 = fma(m0, -w, a.l0);
     const double D1x = d1 * x, D1y = d1 * y, D1z = d1 * z;
+    a.l1[0] = fma(m0, D1x, a.l1[0]);  a.l0b = fma(m1x, D1x, a.l0b);
+    a.l1[1] = fma(m0, D1y, a.l1[1]);  a.l0 = fma(m1y, D1y, a.l0);
+    a.l1[2] = fma(m0, D1z, a.l1[2]);  a.l0b = fma(m1z, D1z, a.l0b);
+
+    // ---- D2 (6 components; zz is needed by the dipole term of L1_z) ----
     const double ax = d2 * x, ay = d2 * y, az = d2 * z;
-    const double Dxx = fma(ax, x, d1), Dxy = ax * y, Dxz = ax * z;
-    const double Dyy = fma(ay, y, d1), Dyz = ay * z, Dzz = fma(az, z, d1);
+    const double Dxx = fma(ax, x, d1), Dyy = fma(ay, y, d1), Dzz = fma(az, z, d1);
+    const double Dxy = ax * y, Dxz = ax * z, Dyz = ay * z;
+    a.l2[0] = fma(m0, Dxx, a.l2[0]);  a.l1[0] = fma(m1x, Dxx, a.l1[0]);  a.l0 = fma(qxx, Dxx, a.l0);
+    a.l2[1] = fma(m0, Dxy, a.l2[1]);  a.l1[1] = fma(m1x, Dxy, a.l1[1]);  a.l1[0] = fma(m1y, Dxy, a.l1[0]);
+    a.l0b = fma(qxy, Dxy, a.l0b);
+    a.l2[2] = fma(m0, Dxz, a.l2[2]);  a.l1[2] = fma(m1x, Dxz, a.l1[2]);  a.l1[0] = fma(m1z, Dxz, a.l1[0]);
+    a.l0 = fma(qxz, Dxz, a.l0);
+    a.l2[3] = fma(m0, Dyy, a.l2[3]);  a.l1[1] = fma(m1y, Dyy, a.l1[1]);  a.l0b = fma(qyy, Dyy, a.l0b);
+    a.l2[4] = fma(m0, Dyz, a.l2[4]);  a.l1[2] = fma(m1y, Dyz, a.l1[2]);  a.l1[1] = fma(m1z, Dyz, a.l1[1]);
+    a.l0 = fma(qyz, Dyz, a.l0);
+    a.l1[2] = fma(m1z, Dzz, a.l1[2]);
 
     // ---- D3: 7 independent + xzz, yzz ----
     const double bx = d3 * x, by = d3 * y;
@@ -113,71 +145,45 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
     const double Dxxx = fma(bxx, x, ax3);
     const double Dxxy = fma(bxx, y, ay);
     const double Dxxz = fma(bxx, z, az);
+    a.l3[0] = fma(m0, Dxxx, a.l3[0]);  a.l2[0] = fma(m1x, Dxxx, a.l2[0]);  a.l1[0] = fma(qxx, Dxxx, a.l1[0]);
+    a.l0b = fma(oxxx, Dxxx, a.l0b);
+    a.l3[1] = fma(m0, Dxxy, a.l3[1]);  a.l2[1] = fma(m1x, Dxxy, a.l2[1]);  a.l2[0] = fma(m1y, Dxxy, a.l2[0]);
+    a.l1[1] = fma(qxx, Dxxy, a.l1[1]);  a.l1[0] = fma(qxy, Dxxy, a.l1[0]);  a.l0 = fma(oxxy, Dxxy, a.l0);
+    a.l3[2] = fma(m0, Dxxz, a.l3[2]);  a.l2[2] = fma(m1x, Dxxz, a.l2[2]);  a.l2[0] = fma(m1z, Dxxz, a.l2[0]);
+    a.l1[2] = fma(qxx, Dxxz, a.l1[2]);  a.l1[0] = fma(qxz, Dxxz, a.l1[0]);  a.l0b = fma(oxxz, Dxxz, a.l0b);
     const double Dxyy = fma(bxy, y, ax);
     const double Dxyz = bxy * z;
+    a.l3[3] = fma(m0, Dxyy, a.l3[3]);  a.l2[3] = fma(m1x, Dxyy, a.l2[3]);  a.l2[1] = fma(m1y, Dxyy, a.l2[1]);
+    a.l1[0] = fma(qyy, Dxyy, a.l1[0]);  a.l1[1] = fma(qxy, Dxyy, a.l1[1]);  a.l0 = fma(oxyy, Dxyy, a.l0);
+    a.l3[4] = fma(m0, Dxyz, a.l3[4]);  a.l2[4] = fma(m1x, Dxyz, a.l2[4]);  a.l2[2] = fma(m1y, Dxyz, a.l2[2]);
+    a.l2[1] = fma(m1z, Dxyz, a.l2[1]);  a.l1[0] = fma(qyz, Dxyz, a.l1[0]);  a.l1[1] = fma(qxz, Dxyz, a.l1[1]);
+    a.l1[2] = fma(qxy, Dxyz, a.l1[2]);  a.l0b = fma(oxyz, Dxyz, a.l0b);
     const double Dyyy = fma(byy, y, ay3);
     const double Dyyz = fma(byy, z, az);
+    a.l3[5] = fma(m0, Dyyy, a.l3[5]);  a.l2[3] = fma(m1y, Dyyy, a.l2[3]);  a.l1[1] = fma(qyy, Dyyy, a.l1[1]);
+    a.l0 = fma(oyyy, Dyyy, a.l0);
+    a.l3[6] = fma(m0, Dyyz, a.l3[6]);  a.l2[4] = fma(m1y, Dyyz, a.l2[4]);  a.l2[3] = fma(m1z, Dyyz, a.l2[3]);
+    a.l1[2] = fma(qyy, Dyyz, a.l1[2]);  a.l1[1] = fma(qyz, Dyyz, a.l1[1]);  a.l0b = fma(oyyz, Dyyz, a.l0b);
     const double Dxzz = -(Dxxx + Dxyy);
     const double Dyzz = -(Dxxy + Dyyy);
+    a.l2[2] = fma(m1z, Dxzz, a.l2[2]);  a.l1[2] = fma(qxz, Dxzz, a.l1[2]);
+    a.l2[4] = fma(m1z, Dyzz, a.l2[4]);  a.l1[2] = fma(qyz, Dyzz, a.l1[2]);
 
-    const double m0 = s[C_M0], m1x = s[C_M1X], m1y = s[C_M1Y], m1z = s[C_M1Z];
-    const double qxx = s[C_QXX], qxy = s[C_QXY], qxz = s[C_QXZ], qyy = s[C_QYY], qyz = s[C_QYZ];
-
-    // ---- L0 += M D0 - M1.D1 + 1/2 M2:D2 - 1/6 M3:.D3 ----
-    {
-        double t = a.l0;
-        t = fma(m0, -w, t);
-        t = fma(m1x, D1x, t); t = fma(m1y, D1y, t); t = fma(m1z, D1z, t);
-        t = fma(qxx, Dxx, t); t = fma(qxy, Dxy, t); t = fma(qxz, Dxz, t); t = fma(qyy, Dyy, t); t = fma(qyz, Dyz, t);
-        t = fma(s[C_OXXX], Dxxx, t); t = fma(s[C_OXXY], Dxxy, t); t = fma(s[C_OXXZ], Dxxz, t);
-        t = fma(s[C_OXYY], Dxyy, t); t = fma(s[C_OXYZ], Dxyz, t); t = fma(s[C_OYYY], Dyyy, t);
-        t = fma(s[C_OYYZ], Dyyz, t);
-        a.l0 = t;
+    double n0 = 0.0, n1 = 0.0, n2 = 0.0, n3 = 0.0, n4 = 0.0, n5 = 0.0, n6 = 0.0;
+    if (CORR) {
+        // n3 = O_B - M_B (O_A / M_A), L127
+        n0 = fma(-m0, tA[0], oxxx);   // xxx
+        n1 = fma(-m0, tA[1], oxxy);   // xxy
+        n2 = fma(-m0, tA[2], oxxz);   // xxz
+        n3 = fma(-m0, tA[3], oxyy);   // xyy
+        n4 = fma(-m0, tA[4], oxyz);   // xyz
+        n5 = fma(-m0, tA[5], oyyy);   // yyy
+        n6 = fma(-m0, tA[6], oyyz);   // yyz
     }
-    // ---- L1_i += M D1_i - M1_j D2_ij + 1/2 M2_jk D3_ijk ----
-    {
-        double t = a.l1[0];
-        t = fma(m0, D1x, t);
-        t = fma(m1x, Dxx, t); t = fma(m1y, Dxy, t); t = fma(m1z, Dxz, t);
-        t = fma(qxx, Dxxx, t); t = fma(qxy, Dxxy, t); t = fma(qxz, Dxxz, t); t = fma(qyy, Dxyy, t); t = fma(qyz, Dxyz, t);
-        a.l1[0] = t;
-        t = a.l1[1];
-        t = fma(m0, D1y, t);
-        t = fma(m1x, Dxy, t); t = fma(m1y, Dyy, t); t = fma(m1z, Dyz, t);
-        t = fma(qxx, Dxxy, t); t = fma(qxy, Dxyy, t); t = fma(qxz, Dxyz, t); t = fma(qyy, Dyyy, t); t = fma(qyz, Dyyz, t);
-        a.l1[1] = t;
-        t = a.l1[2];
-        t = fma(m0, D1z, t);
-        t = fma(m1x, Dxz, t); t = fma(m1y, Dyz, t); t = fma(m1z, Dzz, t);
-        t = fma(qxx, Dxxz, t); t = fma(qxy, Dxyz, t); t = fma(qxz, Dxzz, t); t = fma(qyy, Dyyz, t); t = fma(qyz, Dyzz, t);
-        a.l1[2] = t;
-    }
-    // ---- L2_ij += M D2_ij - M1_k D3_ijk   (xx xy xz yy yz) ----
-    a.l2[0] = fma(m1z, Dxxz, fma(m1y, Dxxy, fma(m1x, Dxxx, fma(m0, Dxx, a.l2[0]))));
-    a.l2[1] = fma(m1z, Dxyz, fma(m1y, Dxyy, fma(m1x, Dxxy, fma(m0, Dxy, a.l2[1]))));
-    a.l2[2] = fma(m1z, Dxzz, fma(m1y, Dxyz, fma(m1x, Dxxz, fma(m0, Dxz, a.l2[2]))));
-    a.l2[3] = fma(m1z, Dyyz, fma(m1y, Dyyy, fma(m1x, Dxyy, fma(m0, Dyy, a.l2[3]))));
-    a.l2[4] = fma(m1z, Dyzz, fma(m1y, Dyyz, fma(m1x, Dxyz, fma(m0, Dyz, a.l2[4]))));
-    // ---- L3_ijk += M D3_ijk   (xxx xxy xxz xyy xyz yyy yyz) ----
-    a.l3[0] = fma(m0, Dxxx, a.l3[0]);
-    a.l3[1] = fma(m0, Dxxy, a.l3[1]);
-    a.l3[2] = fma(m0, Dxxz, a.l3[2]);
-    a.l3[3] = fma(m0, Dxyy, a.l3[3]);
-    a.l3[4] = fma(m0, Dxyz, a.l3[4]);
-    a.l3[5] = fma(m0, Dyyy, a.l3[5]);
-    a.l3[6] = fma(m0, Dyyz, a.l3[6]);
 
     if (CORR) {
-        // ---- correction (L127): n3 = M3_B - (M_B/M_A) M3_A (staged form), dL1_i += n3_t D4_{i,t} ----
+        // ---- correction (L127): dL1_i += n3_t D4_{i,t}, runs over t ----
         const double d4 = d3 * (-7.0 * w2);    // -105/r^9
-        const double n0 = fma(-m0, tA[0], s[C_OXXX]);   // xxx
-        const double n1 = fma(-m0, tA[1], s[C_OXXY]);   // xxy
-        const double n2 = fma(-m0, tA[2], s[C_OXXZ]);   // xxz
-        const double n3 = fma(-m0, tA[3], s[C_OXYY]);   // xyy
-        const double n4 = fma(-m0, tA[4], s[C_OXYZ]);   // xyz
-        const double n5 = fma(-m0, tA[5], s[C_OYYY]);   // yyy
-        const double n6 = fma(-m0, tA[6], s[C_OYYZ]);   // yyz
-
         const double cx = d4 * x, cy = d4 * y;
         const double cxx = cx * x, cxy = cx * y, cyy = cy * y;
         const double cxxx = cxx * x, cxxy = cxx * y, cxyy = cxy * y, cyyy = cyy * y;
@@ -196,9 +202,13 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
         const double Exyzz = -(Exxxy + Exyyy);
         const double Eyyzz = -(Exxyy + Eyyyy);
 
-        a.c[0] = fma(n6, Exyyz, fma(n5, Exyyy, fma(n4, Exxyz, fma(n3, Exxyy, fma(n2, Exxxz, fma(n1, Exxxy, fma(n0, Exxxx, a.c[0])))))));
-        a.c[1] = fma(n6, Eyyyz, fma(n5, Eyyyy, fma(n4, Exyyz, fma(n3, Exyyy, fma(n2, Exxyz, fma(n1, Exxyy, fma(n0, Exxxy, a.c[1])))))));
-        a.c[2] = fma(n6, Eyyzz, fma(n5, Eyyyz, fma(n4, Exyzz, fma(n3, Exyyz, fma(n2, Exxzz, fma(n1, Exxyz, fma(n0, Exxxz, a.c[2])))))));
+        a.c[0] = fma(n0, Exxxx, a.c[0]); a.c[1] = fma(n0, Exxxy, a.c[1]); a.c[2] = fma(n0, Exxxz, a.c[2]);
+        a.c[0] = fma(n1, Exxxy, a.c[0]); a.c[1] = fma(n1, Exxyy, a.c[1]); a.c[2] = fma(n1, Exxyz, a.c[2]);
+        a.c[0] = fma(n2, Exxxz, a.c[0]); a.c[1] = fma(n2, Exxyz, a.c[1]); a.c[2] = fma(n2, Exxzz, a.c[2]);
+        a.c[0] = fma(n3, Exxyy, a.c[0]); a.c[1] = fma(n3, Exyyy, a.c[1]); a.c[2] = fma(n3, Exyyz, a.c[2]);
+        a.c[0] = fma(n4, Exxyz, a.c[0]); a.c[1] = fma(n4, Exyyz, a.c[1]); a.c[2] = fma(n4, Exyzz, a.c[2]);
+        a.c[0] = fma(n5, Exyyy, a.c[0]); a.c[1] = fma(n5, Eyyyy, a.c[1]); a.c[2] = fma(n5, Eyyyz, a.c[2]);
+        a.c[0] = fma(n6, Exyyz, a.c[0]); a.c[1] = fma(n6, Eyyyz, a.c[1]); a.c[2] = fma(n6, Eyyzz, a.c[2]);
     }
 }
 
@@ -206,7 +216,7 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
 template <bool CORR>
 __device__ __forceinline__ void acc_finish(const Acc& a, double L[20], double C[3])
 {
-    L[0] = a.l0;
+    L[0] = a.l0 + a.l0b;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         C[i] = CORR ? a.c[i] : 0.0;
