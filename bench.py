@@ -72,11 +72,11 @@ def sample_regions(ncell, nregions, edge=16):
     return [((a * edge, b * edge, c * edge), ((a + 1) * edge, (b + 1) * edge, (c + 1) * edge)) for a, b, c in picks]
 
 
-def oracle_sample(w, theta, nregions):
-    """Time the oracle, as it stands, on a bounded sample of the workload.  Returns
-    (interactions, seconds, threads)."""
+def oracle_sample(w, theta, nregions, first=0):
+    """Time the oracle, as it stands, on regions first .. first+nregions-1 of the stratified sample.
+    Returns (interactions, seconds, threads, regions)."""
     import oracle
-    regions = sample_regions(w.n[0], nregions)
+    regions = sample_regions(w.n[0], first + nregions)[first:]
     oracle.lib()
     t0 = time.perf_counter()
     total = 0
@@ -84,6 +84,28 @@ def oracle_sample(w, theta, nregions):
         _, _, cnt = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, lo, hi, True)
         total += cnt
     return total, time.perf_counter() - t0, oracle.num_threads(), len(regions)
+
+
+def oracle_sample_bounded(w, theta, target_s, pilot=4):
+    """A sample sized for about target_s seconds of oracle work: a short pilot fixes the region count."""
+    c0, s0, _, n0 = oracle_sample(w, theta, pilot)
+    per_region = max(s0 / n0, 1e-6)
+    m = (w.n[0] // 16) ** 3
+    nreg = int(max(pilot, min(m - pilot, target_s / per_region)))
+    return oracle_sample(w, theta, nreg, first=pilot if nreg + pilot <= m else 0)
+
+
+def aggregate_over_ranks(ms_local, units_local, dist=None, device=None):
+    """Whole-job numbers from per-rank ones: time = MAX over ranks, units = SUM over ranks
+    (every rank works on its own problem; there is no data-path collective)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms_local), int(units_local)
+    import torch
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    u = torch.tensor([int(units_local)], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(u.item())
 
 
 class ClockSampler:
@@ -147,15 +169,15 @@ def run_reference(args):
     if rank != 0:
         return
     w = make_workload(args.workload, args.theta, args.ncell, args.seed)
-    nreg = args.ref_regions
     for _ in range(args.warmup):
         oracle_sample(w, args.theta, 1)
-    tot, secs = 0, 0.0
+    tot, secs, nreg = 0, 0.0, 0
     threads = 1
     for _ in range(args.steps):
-        c, s, threads, nr = oracle_sample(w, args.theta, nreg)
+        c, s, threads, nr = oracle_sample_bounded(w, args.theta, args.ref_seconds)
         tot += c
         secs += s
+        nreg = nr
     value = tot / secs
     sample = "%d regions of 16^3 cells (%d sub-grids) per step of %s" % (nreg, 8 * nreg, w.name)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
@@ -203,6 +225,8 @@ def run_ours(args):
     L = torch.empty((20,) + f.out_shape, dtype=torch.float64, device=dev)
     Lc = torch.empty((3,) + f.out_shape, dtype=torch.float64, device=dev)
 
+    f.bind_outputs(L, Lc)          # interact() writes the expansions straight into the caller's buffers
+
     def step():
         f.set_moments(mom, com)
         f.interact()
@@ -240,12 +264,9 @@ def run_ours(args):
     kernel_ms = sum(a.elapsed_time(b) for a, b in kev) / args.steps
     if f.status() != p.OK:
         raise SystemExit("bench.py: device reported status %d" % f.status())
-    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total = float(tmax.item())
+    ms_total, units = aggregate_over_ranks(ms_total, n_int * args.steps, dist if world > 1 else None, dev)
     ms_per_step = ms_total / args.steps
-    value = world * n_int * args.steps / (ms_total * 1e-3)
+    value = units / (ms_total * 1e-3)
 
     # ---- end to end through the host-buffer entry point (H2D + step + D2H inside the timed region) ----
     e2e = None
@@ -266,11 +287,8 @@ def run_ours(args):
         b.record(stream)
         barrier()
         e2e_ms = max(a.elapsed_time(b), 1e3 * (time.perf_counter() - t0))
-        t2 = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t2.item())
-        e2e = {"value": world * n_int * args.e2e_steps / (e2e_ms * 1e-3), "unit": UNIT,
+        e2e_ms, e2e_units = aggregate_over_ranks(e2e_ms, n_int * args.e2e_steps, dist if world > 1 else None, dev)
+        e2e = {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": int(mom_h.numel() * 8 + com_h.numel() * 8),
                "d2h_bytes_per_step": int(L_h.numel() * 8 + Lc_h.numel() * 8),
                "steps": args.e2e_steps, "ms_per_step": e2e_ms / args.e2e_steps,
@@ -309,7 +327,7 @@ def run_ours(args):
                 "hbm_peak_gbs": peaks.get("hbm_gbs")}
 
     # ---- the oracle timed beside it on this box's host cores (bounded sample) ----
-    c, s, threads, nr = oracle_sample(w, args.theta, args.ref_regions)
+    c, s, threads, nr = oracle_sample_bounded(w, args.theta, args.ref_seconds)
     cpu_baseline = {"value": c / s, "unit": UNIT, "cores": threads, "kind": "oracle",
                     "sample": "%d regions of 16^3 cells (%d sub-grids, %d interactions) of %s in %.1f s" % (
                         nr, 8 * nr, c, w.name, s)}
@@ -345,7 +363,8 @@ def main():
     ap.add_argument("--ncell", type=int, default=0)
     ap.add_argument("--seed", type=int, default=20210108)
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--ref-regions", type=int, default=32)
+    ap.add_argument("--ref-seconds", type=float, default=12.0,
+                    help="CPU seconds of oracle work per cpu_baseline sample / per --impl reference step")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

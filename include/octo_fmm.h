@@ -85,6 +85,13 @@ int octo_fmm_interact(octo_fmm_t *h);
  * out cells; Lcorr: device, [3] x out cells, or NULL.  ESTATE before interact. */
 int octo_fmm_get_expansions(octo_fmm_t *h, double *L, double *Lcorr);
 
+/* Optional: make interact() write its results straight into caller buffers (device, same shapes
+ * as get_expansions; with Lcorr = NULL the correction alone stays in the workspace).  A later
+ * get_expansions() with the same pointers then copies nothing.  L = NULL
+ * restores the default (results kept in the workspace).  The buffers must stay valid until
+ * the stream has passed the interact() calls that use them. */
+int octo_fmm_bind_outputs(octo_fmm_t *h, double *L, double *Lcorr);
+
 /* Synchronises the stream and releases the handle (not the workspace). */
 int octo_fmm_destroy(octo_fmm_t *h);
 
@@ -103,8 +110,8 @@ int octo_fmm_interaction_count(const octo_fmm_t *h, unsigned long long *n);
 int octo_fmm_status(octo_fmm_t *h);
 
 /* Whole step with HOST buffers (pinned or pageable): H2D of moments/com_off into
- * scratch, set_moments, interact, get_expansions, D2H of L (and Lcorr if non-NULL), then a stream
- * synchronise.  scratch: device, >= octo_fmm_host_scratch_bytes(cfg) bytes, borrowed for the call. */
+ * scratch, set_moments, interact (writing into the scratch), D2H of L (and Lcorr if non-NULL), then
+ * a stream synchronise.  Afterwards the handle is in the "sources staged" state.  scratch: device, >= octo_fmm_host_scratch_bytes(cfg) bytes, borrowed for the call. */
 size_t octo_fmm_host_scratch_bytes(const octo_fmm_config *cfg);
 int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *com_off_host,
                       double *L_host, double *Lcorr_host, void *scratch, size_t scratch_bytes);

@@ -58,6 +58,7 @@ class _Library:
         lib.octo_fmm_interact.argtypes = [vp]
         lib.octo_fmm_get_expansions.argtypes = [vp, vp, vp]
         lib.octo_fmm_destroy.argtypes = [vp]
+        lib.octo_fmm_bind_outputs.argtypes = [vp, vp, vp]
         lib.octo_fmm_get_stencil.argtypes = [vp, ctypes.c_int, ip, vp]
         lib.octo_fmm_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_status.argtypes = [vp]
@@ -135,6 +136,12 @@ def octo_fmm_get_expansions(h, L, Lcorr=None):
     rc = _lib.octo_fmm_get_expansions(h, _ptr(L), _ptr(Lcorr))
     if rc != OK:
         raise OctoFmmError("octo_fmm_get_expansions", rc)
+
+
+def octo_fmm_bind_outputs(h, L, Lcorr=None):
+    rc = _lib.octo_fmm_bind_outputs(h, _ptr(L), _ptr(Lcorr))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_bind_outputs", rc)
 
 
 def octo_fmm_destroy(h):
@@ -253,6 +260,11 @@ class OctoFMM:
             Lcorr = torch.empty((3,) + self.out_shape, dtype=torch.float64, device=self.device)
         octo_fmm_get_expansions(self.handle, L, Lcorr)
         return L, Lcorr
+
+    def bind_outputs(self, L, Lcorr=None):
+        """interact() then writes straight into L / Lcorr (kept alive here); None unbinds."""
+        self._bound = (L, Lcorr)
+        octo_fmm_bind_outputs(self.handle, L, Lcorr)
 
     def solve(self, moments, com_off=None):
         self.set_moments(moments, com_off)

@@ -138,8 +138,12 @@ struct octo_fmm {
     CUtensorMap tmap;
     Params prm;
     double* src;
-    double* L;
+    double* L;             // workspace result buffers
     double* C;
+    double* outL;          // where interact() writes: the workspace, or the caller's bound buffers
+    double* outC;
+    double* resL;          // where the last interact() left its results
+    double* resC;
     double4* W;
     int* flags;
     int state;          // 0 created, 1 sources staged, 2 interacted
@@ -256,6 +260,7 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     P.tiles_z = (P.oz + TILE_Z - 1) / TILE_Z;
     P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
     P.reach = h->reach;
+    h->outL = h->L; h->outC = h->C;
     P.S = h->src; P.L = h->L; P.C = h->C; P.flags = h->flags;
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE) {
@@ -335,9 +340,10 @@ int octo_fmm_interact(octo_fmm_t* h)
     if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
     if (upload_tables(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     if (cudaMemsetAsync(h->flags, 0, sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
-    const Params& P = h->prm;
+    Params& P = h->prm;
+    P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        p2p_monopole_kernel<<<brick_blocks(P), 256, 0, h->stream>>>(P, h->src, h->W, h->L);
+        p2p_monopole_kernel<<<brick_blocks(P), 256, 0, h->stream>>>(P, h->src, h->W, h->outL);
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
@@ -348,6 +354,17 @@ int octo_fmm_interact(octo_fmm_t* h)
     }
     if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     h->state = 2;
+    h->resL = h->outL; h->resC = h->outC;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_bind_outputs(octo_fmm_t* h, double* L, double* Lcorr)
+{
+    if (!h) return OCTO_FMM_EINVAL;
+    if (!L && Lcorr) return OCTO_FMM_EINVAL;
+    if (Lcorr && h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
+    h->outL = L ? L : h->L;
+    h->outC = (L && Lcorr) ? Lcorr : h->C;
     return OCTO_FMM_OK;
 }
 
@@ -358,11 +375,14 @@ int octo_fmm_get_expansions(octo_fmm_t* h, double* L, double* Lcorr)
     const Params& P = h->prm;
     const size_t ocell = (size_t)P.ox * P.oy * P.oz;
     const size_t ncoef = h->cfg.kind == OCTO_FMM_MULTIPOLE ? 20 : 4;
-    if (cudaMemcpyAsync(L, h->L, ocell * ncoef * sizeof(double), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess)
+    // results already in place when interact() wrote into bound caller buffers
+    if (L != h->resL &&
+        cudaMemcpyAsync(L, h->resL, ocell * ncoef * sizeof(double), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
     if (Lcorr) {
         if (h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
-        if (cudaMemcpyAsync(Lcorr, h->C, ocell * 3 * sizeof(double), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess)
+        if (Lcorr != h->resC &&
+            cudaMemcpyAsync(Lcorr, h->resC, ocell * 3 * sizeof(double), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess)
             return OCTO_FMM_ECUDA;
     }
     return OCTO_FMM_OK;
@@ -426,14 +446,19 @@ int octo_fmm_run_host(octo_fmm_t* h, const double* moments_host, const double* c
     if (multi && cudaMemcpyAsync(d_c, com_off_host, ncell * 3 * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
     int rc;
+    double* const keepL = h->outL; double* const keepC = h->outC;
     if ((rc = octo_fmm_set_moments(h, d_m, d_c)) != OCTO_FMM_OK) return rc;
-    if ((rc = octo_fmm_interact(h)) != OCTO_FMM_OK) return rc;
-    if ((rc = octo_fmm_get_expansions(h, d_L, Lcorr_host ? d_C : nullptr)) != OCTO_FMM_OK) return rc;
+    h->outL = d_L; h->outC = multi ? d_C : nullptr;       // interact() writes straight into the scratch
+    rc = octo_fmm_interact(h);
+    h->outL = keepL; h->outC = keepC;
+    if (rc != OCTO_FMM_OK) return rc;
     if (cudaMemcpyAsync(L_host, d_L, ocell * (multi ? 20 : 4) * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
     if (Lcorr_host && cudaMemcpyAsync(Lcorr_host, d_C, ocell * 3 * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    h->state = 1;                       // the results went to the host; nothing is kept in the scratch
+    h->resL = h->L; h->resC = h->C;
     return OCTO_FMM_OK;
 }
 

@@ -217,6 +217,34 @@ def test_host_buffer_entry_point(env):
     f.close()
 
 
+def test_bound_outputs_match_copied_outputs(env):
+    """octo_fmm_bind_outputs: interact() writes into caller buffers; get_expansions then copies nothing
+    and the numbers are bit-identical to the default (workspace + copy) route; unbinding restores it."""
+    p, torch = env
+    w = fi.config1()
+    L, Lc, _, _ = gpu_multipole(env, w)
+    f = p.OctoFMM(w.n, w.h, w.theta, p.MULTIPOLE, True, w.out_lo, w.out_hi)
+    mom, com = torch.from_numpy(w.moments).cuda(), torch.from_numpy(w.com_off).cuda()
+    Lb = torch.full((20, 8, 8, 8), float("nan"), dtype=torch.float64, device="cuda")
+    Lcb = torch.full((3, 8, 8, 8), float("nan"), dtype=torch.float64, device="cuda")
+    f.bind_outputs(Lb, Lcb)
+    f.set_moments(mom, com)
+    f.interact()
+    torch.cuda.synchronize()
+    assert np.array_equal(Lb.cpu().numpy(), L) and np.array_equal(Lcb.cpu().numpy(), Lc)   # before any get
+    f.get_expansions(Lb, Lcb)                                  # same pointers: nothing to copy
+    L2, Lc2 = f.get_expansions()                               # other pointers: copied from the bound buffers
+    torch.cuda.synchronize()
+    assert np.array_equal(L2.cpu().numpy(), L) and np.array_equal(Lc2.cpu().numpy(), Lc)
+    f.bind_outputs(None)
+    Lb.fill_(0.0)
+    f.interact()
+    L3, _ = f.get_expansions()
+    torch.cuda.synchronize()
+    assert np.array_equal(L3.cpu().numpy(), L) and float(Lb.abs().max()) == 0.0
+    f.close()
+
+
 def test_error_paths(env):
     p, torch = env
     w = fi.config1()
