@@ -111,13 +111,18 @@ int octo_fmm_status(octo_fmm_t *h);
 
 /* Whole step with HOST buffers (pinned or pageable): H2D of moments/com_off into
  * scratch, set_moments, interact (writing into the scratch), D2H of L (and Lcorr if non-NULL), then
- * a stream synchronise.  Afterwards the handle is in the "sources staged" state.  scratch: device, >= octo_fmm_host_scratch_bytes(cfg) bytes, borrowed for the call. */
+ * a stream synchronise.  For the multipole kind the step is pipelined over slabs of z-layers on two
+ * internal copy streams, so that the copy in of slab c+1, the kernels of slab c and the copy out of
+ * slab c-1 overlap (pinned host buffers are needed for the overlap, not for correctness); every
+ * layer crosses the bus once per direction.  Returns OCTO_FMM_EMASS if the correction met a target
+ * mass <= 0.  Afterwards the handle is in the "sources staged" state.  scratch: device, >= octo_fmm_host_scratch_bytes(cfg) bytes, borrowed for the call. */
 size_t octo_fmm_host_scratch_bytes(const octo_fmm_config *cfg);
 int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *com_off_host,
                       double *L_host, double *Lcorr_host, void *scratch, size_t scratch_bytes);
 
-/* Kernel selection, for tests and profiling: "kernel" = 0 staged (TMA + shared memory, default),
- * 1 direct (global-memory loads; same pair arithmetic).  Unknown keys -> EINVAL. */
+/* Options, for tests and profiling.  "kernel" = 0 staged (TMA + shared memory, default), 1 direct
+ * (global-memory loads; same pair arithmetic).  "host_chunk" = output z-layers per pipeline slab of
+ * octo_fmm_run_host (default 24; 0 = one copy in, one launch, one copy out).  Unknown keys -> EINVAL. */
 int octo_fmm_set_option(octo_fmm_t *h, const char *key, int value);
 
 /* Launch facts of the interaction kernel the handle would run: grid, block, dynamic shared

@@ -58,7 +58,8 @@ struct Params {
     int nx, ny, nz;
     int lo[3], hi[3];        // output region
     int ox, oy, oz;          // its extents
-    int tiles_x, tiles_y, tiles_z;   // 16 x 8 x 3 bricks covering the output region
+    int kb, ke;              // z-layers [kb, ke) of the output region this launch computes (staged kernel)
+    int tiles_x, tiles_y, tiles_z;   // 16 x 8 x 3 bricks covering x, y of the output region and [kb, ke)
     long long ntiles;        // tiles_x * tiles_y * tiles_z
     int reach;
     const double* S;         // staged sources
@@ -72,11 +73,12 @@ struct Params {
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) stage_multipole_kernel(const double* __restrict__ mom,
                                                               const double* __restrict__ com, double* __restrict__ S,
-                                                              int nx, int ny, int nz)
+                                                              int nx, int ny, int nz, int z_begin, int z_count)
 {
     const long long ncell = (long long)nx * ny * nz;
-    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= ncell) return;
+    const long long local = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (local >= (long long)nx * ny * z_count) return;
+    const long long cell = local + (long long)z_begin * ny * nx;
     const int x = (int)(cell % nx);
     const long long r = cell / nx;
     const int y = (int)(r % ny), z = (int)(r / ny);
@@ -153,7 +155,7 @@ __device__ __forceinline__ void tma_load_slab(void* dst, const CUtensorMap* map,
 // columns and share their slabs through L2.
 __device__ __forceinline__ void decode_tile(const Params& p, long long t, int& x0, int& y0, int& k0)
 {
-    k0 = p.lo[2] + (int)(t % p.tiles_z) * TILE_Z;
+    k0 = p.kb + (int)(t % p.tiles_z) * TILE_Z;
     const long long c = t / p.tiles_z;
     x0 = p.lo[0] + (int)(c % p.tiles_x) * TILE_X;
     y0 = p.lo[1] + (int)(c / p.tiles_x) * TILE_Y;
@@ -247,7 +249,7 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
             for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
                 int x0, y0, k0;
                 decode_tile(p, t, x0, y0, k0);
-                const int z_lo = max(k0 - p.reach, 0), z_hi = min(k0 + TILE_Z - 1 + p.reach, p.nz - 1);
+                const int z_lo = max(k0 - p.reach, 0), z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.nz - 1);
                 for (int zz = z_lo; zz <= z_hi; ++zz) {
                     const uint32_t b = it % NSTAGE;
                     if (it >= NSTAGE) mbar_wait_backoff(&empty[b], ((it / NSTAGE) - 1) & 1);
@@ -274,10 +276,10 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
         decode_tile(p, t, x0, y0, k0);
         const int k = k0 + layer;
         const int gx = x0 + px + 2 * lx, gy = y0 + py + 2 * ly;
-        const bool layer_on = k < p.hi[2];             // warp-uniform
+        const bool layer_on = k < p.ke;                // warp-uniform
         const bool active = layer_on && gx < p.hi[0] && gy < p.hi[1];
         const int cls = cls_xy + ((k & 1) << 2);
-        const int z_hi = min(k0 + TILE_Z - 1 + p.reach, p.nz - 1);
+        const int z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.nz - 1);
 
         double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         if (active) load_target<CORR>(p, gx, gy, k, dA, tA);

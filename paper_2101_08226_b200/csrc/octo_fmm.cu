@@ -21,6 +21,7 @@ using namespace octo;
 namespace {
 
 constexpr size_t ALIGN = 256;
+constexpr int MAX_CHUNKS = 32;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Offset3 { signed char d[3]; };
@@ -150,6 +151,11 @@ struct octo_fmm {
     int kernel;         // 0 staged (TMA), 1 direct
     int sm_count;
     cudaStream_t stream;
+    // run_host pipeline (created on first use)
+    int host_chunk;        // output z-layers per pipeline slab; 0 = no pipelining
+    int host_launches;     // kernels the last run_host launched
+    cudaStream_t s_h2d, s_d2h;
+    cudaEvent_t ev_in[32], ev_out[32], ev_begin, ev_end;
 };
 
 extern "C" {
@@ -196,6 +202,9 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     h->sm_count = prop.multiProcessorCount;
     h->state = 0;
     h->kernel = 0;
+    h->host_chunk = 24;
+    h->host_launches = 0;
+    h->s_h2d = nullptr; h->s_d2h = nullptr;
     region_of(*cfg, h->lo, h->hi);
 
     // ---- a1: interaction lists (Eq. 15) ----
@@ -257,6 +266,7 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     for (int a = 0; a < 3; ++a) { P.lo[a] = h->lo[a]; P.hi[a] = h->hi[a]; }
     P.ox = h->hi[0] - h->lo[0]; P.oy = h->hi[1] - h->lo[1]; P.oz = h->hi[2] - h->lo[2];
     P.tiles_x = (P.ox + TILE_X - 1) / TILE_X; P.tiles_y = (P.oy + TILE_Y - 1) / TILE_Y;
+    P.kb = h->lo[2]; P.ke = h->hi[2];
     P.tiles_z = (P.oz + TILE_Z - 1) / TILE_Z;
     P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
     P.reach = h->reach;
@@ -308,7 +318,8 @@ int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com
     const Params& P = h->prm;
     if (h->cfg.kind == OCTO_FMM_MULTIPOLE) {
         const long long ncell = (long long)P.nx * P.ny * P.nz;
-        stage_multipole_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(moments, com_off, h->src, P.nx, P.ny, P.nz);
+        stage_multipole_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(moments, com_off, h->src, P.nx, P.ny, P.nz,
+                                                                                       0, P.nz);
     } else {
         const long long pc = (long long)(P.nx + 2 * REACH_MAX) * (P.ny + 2 * REACH_MAX) * (P.nz + 2 * REACH_MAX);
         stage_monopole_kernel<<<(unsigned)((pc + 255) / 256), 256, 0, h->stream>>>(moments, h->src, P.nx, P.ny, P.nz);
@@ -331,6 +342,20 @@ static int upload_tables(octo_fmm_t* h)
     return OCTO_FMM_OK;
 }
 
+// launch the staged interaction kernel for the z-layers [kb, ke) of the output region
+static int launch_staged(octo_fmm_t* h, int kb, int ke)
+{
+    Params P = h->prm;
+    P.L = h->outL; P.C = h->outC;
+    P.kb = kb; P.ke = ke;
+    P.tiles_z = (ke - kb + TILE_Z - 1) / TILE_Z;
+    P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
+    const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
+    if (h->cfg.am_correction) m2l_staged_kernel<true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    else                      m2l_staged_kernel<false><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    return cudaGetLastError() == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
+}
+
 static int brick_blocks(const Params& P) { return ((P.ox + 15) / 16) * ((P.oy + 7) / 8) * ((P.oz + 3) / 4); }
 
 int octo_fmm_interact(octo_fmm_t* h)
@@ -348,9 +373,7 @@ int octo_fmm_interact(octo_fmm_t* h)
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
     } else {
-        const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
-        if (h->cfg.am_correction) m2l_staged_kernel<true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-        else                      m2l_staged_kernel<false><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        if (launch_staged(h, h->lo[2], h->hi[2]) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     }
     if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     h->state = 2;
@@ -402,6 +425,13 @@ int octo_fmm_destroy(octo_fmm_t* h)
 {
     if (!h) return OCTO_FMM_EINVAL;
     cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (h->s_h2d) {
+        cudaStreamDestroy(h->s_h2d);
+        cudaStreamDestroy(h->s_d2h);
+        for (int i = 0; i < MAX_CHUNKS; ++i) { cudaEventDestroy(h->ev_in[i]); cudaEventDestroy(h->ev_out[i]); }
+        cudaEventDestroy(h->ev_begin);
+        cudaEventDestroy(h->ev_end);
+    }
     if (g_const_owner == h) g_const_owner = nullptr;
     delete h;
     return e == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
@@ -424,6 +454,78 @@ int octo_fmm_interaction_count(const octo_fmm_t* h, unsigned long long* n)
     return OCTO_FMM_OK;
 }
 
+// Whole step on host buffers, pipelined over slabs of z-layers (multipole kind, staged kernel):
+// the host->device copy of slab c+1, the staging + interaction kernels of slab c and the
+// device->host copy of slab c-1 run concurrently on three streams (PCIe is full duplex), so the
+// step costs about max(H2D, compute, D2H) instead of their sum.  Slab c's output layers
+// [a, b) need source layers [a - reach, b + reach): H2D(c) brings every layer of that range that
+// earlier slabs have not brought.  Every layer crosses PCIe exactly once in each direction.
+static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* com_h, double* L_h, double* C_h,
+                              double* d_m, double* d_c, double* d_L, double* d_C)
+{
+    const Params& P = h->prm;
+    if (!h->s_h2d) {
+        if (cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
+        for (int i = 0; i < MAX_CHUNKS; ++i)
+            if (cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming) != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->ev_end, cudaEventDisableTiming) != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    int zc = h->host_chunk;
+    while ((P.oz + zc - 1) / zc > MAX_CHUNKS) zc += TILE_Z;
+    const int nchunk = (P.oz + zc - 1) / zc;
+    const size_t plane = (size_t)P.nx * P.ny, ncell = plane * P.nz;
+    const size_t oplane = (size_t)P.ox * P.oy, ocell = oplane * P.oz;
+    cudaStream_t sm = h->stream;
+#define OCTO_TRY(call) do { if ((call) != cudaSuccess) return OCTO_FMM_ECUDA; } while (0)
+    OCTO_TRY(cudaMemsetAsync(h->flags, 0, sizeof(int), sm));
+    if (upload_tables(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    OCTO_TRY(cudaEventRecord(h->ev_begin, sm));            // the copies start after earlier work on the caller's stream
+    OCTO_TRY(cudaStreamWaitEvent(h->s_h2d, h->ev_begin, 0));
+    OCTO_TRY(cudaStreamWaitEvent(h->s_d2h, h->ev_begin, 0));
+    double* const keepL = h->outL; double* const keepC = h->outC;
+    h->outL = d_L; h->outC = d_C;
+    int brought = std::max(P.lo[2] - h->reach, 0);         // source layers [.., brought) are on the device
+    const int first_layer = brought;
+    int rc = OCTO_FMM_OK;
+    for (int c = 0; c < nchunk && rc == OCTO_FMM_OK; ++c) {
+        const int a = P.lo[2] + c * zc, b = std::min(a + zc, P.hi[2]);
+        const int need = std::min(b + h->reach, P.nz);
+        if (need > brought) {
+            const size_t off = (size_t)brought * plane, width = (size_t)(need - brought) * plane * 8;
+            OCTO_TRY(cudaMemcpy2DAsync(d_m + off, ncell * 8, mom_h + off, ncell * 8, width, 20, cudaMemcpyHostToDevice, h->s_h2d));
+            OCTO_TRY(cudaMemcpy2DAsync(d_c + off, ncell * 8, com_h + off, ncell * 8, width, 3, cudaMemcpyHostToDevice, h->s_h2d));
+        }
+        OCTO_TRY(cudaEventRecord(h->ev_in[c], h->s_h2d));
+        OCTO_TRY(cudaStreamWaitEvent(sm, h->ev_in[c], 0));
+        if (need > brought) {
+            const long long n = (long long)(need - brought) * (long long)plane;
+            stage_multipole_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(d_m, d_c, h->src, P.nx, P.ny, P.nz, brought,
+                                                                                 need - brought);
+            OCTO_TRY(cudaGetLastError());
+            brought = need;
+        }
+        rc = launch_staged(h, a, b);
+        if (rc != OCTO_FMM_OK) break;
+        OCTO_TRY(cudaEventRecord(h->ev_out[c], sm));
+        OCTO_TRY(cudaStreamWaitEvent(h->s_d2h, h->ev_out[c], 0));
+        const size_t ooff = (size_t)(a - P.lo[2]) * oplane, owidth = (size_t)(b - a) * oplane * 8;
+        OCTO_TRY(cudaMemcpy2DAsync(L_h + ooff, ocell * 8, d_L + ooff, ocell * 8, owidth, 20, cudaMemcpyDeviceToHost, h->s_d2h));
+        if (C_h)
+            OCTO_TRY(cudaMemcpy2DAsync(C_h + ooff, ocell * 8, d_C + ooff, ocell * 8, owidth, 3, cudaMemcpyDeviceToHost, h->s_d2h));
+    }
+    (void)first_layer;
+    h->outL = keepL; h->outC = keepC;
+    if (rc != OCTO_FMM_OK) return rc;
+    OCTO_TRY(cudaEventRecord(h->ev_end, h->s_d2h));
+    OCTO_TRY(cudaStreamWaitEvent(sm, h->ev_end, 0));        // the caller's stream completes when the last copy has
+#undef OCTO_TRY
+    h->host_launches = 2 * nchunk;
+    return OCTO_FMM_OK;
+}
+
 int octo_fmm_run_host(octo_fmm_t* h, const double* moments_host, const double* com_off_host, double* L_host,
                       double* Lcorr_host, void* scratch, size_t scratch_bytes)
 {
@@ -441,25 +543,32 @@ int octo_fmm_run_host(octo_fmm_t* h, const double* moments_host, const double* c
     double* d_L = (double*)w; w += align_up(ocell * (multi ? 20 : 4) * 8);
     double* d_C = multi ? (double*)w : nullptr;
     if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
-    if (cudaMemcpyAsync(d_m, moments_host, ncell * (multi ? 20 : 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
-        return OCTO_FMM_ECUDA;
-    if (multi && cudaMemcpyAsync(d_c, com_off_host, ncell * 3 * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
-        return OCTO_FMM_ECUDA;
-    int rc;
-    double* const keepL = h->outL; double* const keepC = h->outC;
-    if ((rc = octo_fmm_set_moments(h, d_m, d_c)) != OCTO_FMM_OK) return rc;
-    h->outL = d_L; h->outC = multi ? d_C : nullptr;       // interact() writes straight into the scratch
-    rc = octo_fmm_interact(h);
-    h->outL = keepL; h->outC = keepC;
-    if (rc != OCTO_FMM_OK) return rc;
-    if (cudaMemcpyAsync(L_host, d_L, ocell * (multi ? 20 : 4) * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
-        return OCTO_FMM_ECUDA;
-    if (Lcorr_host && cudaMemcpyAsync(Lcorr_host, d_C, ocell * 3 * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
-        return OCTO_FMM_ECUDA;
+    if (multi && h->kernel == 0 && h->host_chunk > 0) {
+        const int rc = run_host_pipelined(h, moments_host, com_off_host, L_host, Lcorr_host, d_m, d_c, d_L, d_C);
+        if (rc != OCTO_FMM_OK) return rc;
+    } else {
+        if (cudaMemcpyAsync(d_m, moments_host, ncell * (multi ? 20 : 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+            return OCTO_FMM_ECUDA;
+        if (multi && cudaMemcpyAsync(d_c, com_off_host, ncell * 3 * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+            return OCTO_FMM_ECUDA;
+        int rc;
+        double* const keepL = h->outL; double* const keepC = h->outC;
+        if ((rc = octo_fmm_set_moments(h, d_m, d_c)) != OCTO_FMM_OK) return rc;
+        h->outL = d_L; h->outC = multi ? d_C : nullptr;       // interact() writes straight into the scratch
+        rc = octo_fmm_interact(h);
+        h->outL = keepL; h->outC = keepC;
+        if (rc != OCTO_FMM_OK) return rc;
+        if (cudaMemcpyAsync(L_host, d_L, ocell * (multi ? 20 : 4) * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
+            return OCTO_FMM_ECUDA;
+        if (Lcorr_host && cudaMemcpyAsync(Lcorr_host, d_C, ocell * 3 * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
+            return OCTO_FMM_ECUDA;
+    }
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     h->state = 1;                       // the results went to the host; nothing is kept in the scratch
     h->resL = h->L; h->resC = h->C;
-    return OCTO_FMM_OK;
+    int f = 0;
+    if (cudaMemcpy(&f, h->flags, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
+    return (f & 1) ? OCTO_FMM_EMASS : OCTO_FMM_OK;
 }
 
 int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
@@ -468,6 +577,11 @@ int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
     if (!std::strcmp(key, "kernel")) {
         if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
         h->kernel = value;
+        return OCTO_FMM_OK;
+    }
+    if (!std::strcmp(key, "host_chunk")) {       // z-layers per run_host pipeline slab; 0 = one copy, one launch
+        if (value < 0 || value > 4096) return OCTO_FMM_EINVAL;
+        h->host_chunk = value;
         return OCTO_FMM_OK;
     }
     return OCTO_FMM_EINVAL;

@@ -217,6 +217,31 @@ def test_host_buffer_entry_point(env):
     f.close()
 
 
+@pytest.mark.parametrize("chunk", [0, 6, 8, 10, 24])
+def test_host_entry_point_pipelined_over_z_slabs(env, chunk):
+    """run_host pipelines H2D / kernels / D2H over slabs of z-layers; any slab size (ragged against the
+    3-layer bricks or not, 0 = unpipelined) must give bit-identical results to the device-pointer route,
+    on a whole grid with domain faces and on an interior output region."""
+    p, torch = env
+    w = fi.config2(ncell=32)
+    for lo, hi in (((0, 0, 0), (0, 0, 0)), ((8, 0, 8), (32, 16, 24))):
+        f = p.OctoFMM(w.n, w.h, 0.5, p.MULTIPOLE, True, lo, hi)
+        L, Lc = f.solve(torch.from_numpy(w.moments).cuda(), torch.from_numpy(w.com_off).cuda())
+        torch.cuda.synchronize()
+        f.set_option("host_chunk", chunk)
+        nb = p.octo_fmm_host_scratch_bytes(f.cfg)
+        scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        mom = torch.from_numpy(w.moments).pin_memory()
+        com = torch.from_numpy(w.com_off).pin_memory()
+        Lh = torch.full((20,) + f.out_shape, float("nan"), dtype=torch.float64).pin_memory()
+        Lch = torch.full((3,) + f.out_shape, float("nan"), dtype=torch.float64).pin_memory()
+        for _ in range(2):                                   # twice: the pipeline's streams/events are reused
+            p.octo_fmm_run_host(f.handle, mom, com, Lh, Lch, scratch, nb)
+            assert f.status() == p.OK
+            assert np.array_equal(Lh.numpy(), L.cpu().numpy()) and np.array_equal(Lch.numpy(), Lc.cpu().numpy())
+        f.close()
+
+
 def test_bound_outputs_match_copied_outputs(env):
     """octo_fmm_bind_outputs: interact() writes into caller buffers; get_expansions then copies nothing
     and the numbers are bit-identical to the default (workspace + copy) route; unbinding restores it."""
