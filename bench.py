@@ -311,6 +311,9 @@ def run_ours(args):
     peak_tflops = sm_count * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
     probe_scratch = torch.empty(8 << 20, dtype=torch.uint8, device=dev)
     probe = p.octo_fmm_fp64_peak_probe(local, stream.cuda_stream, probe_scratch, 40000)
+    issue_peak = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6
+    issue_probe = {name: p.octo_fmm_fp64_issue_probe(local, stream.cuda_stream, probe_scratch, mode) / issue_peak
+                   for mode, name in ((0, "dfma_three_fresh_registers"), (1, "dfma_operand_reuse"), (2, "dmul"))}
     achieved = flops_per * n_int / (kernel_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "m2l_staged_kernel<correction>", "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops,
@@ -320,6 +323,7 @@ def run_ours(args):
                 "frac_of_measured_dfma": achieved / (probe["flops_per_s"] / 1e12),
                 "flops_per_interaction": flops_per, "fp64_instr_per_interaction": instr_per,
                 "fp64_pipe_issue_frac": (instr_per * n_int / (kernel_ms * 1e-3)) / (sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
+                "fp64_issue_probe_frac_of_issue_peak": issue_probe,
                 "kernel_ms": kernel_ms, "interactions_per_launch": n_int,
                 "traffic": TRAFFIC_BYTES.get((args.workload, args.ncell or 256, args.theta)),
                 "algorithmic_bytes": int((23 + 23) * 8 * w.moments[0].size),

@@ -136,6 +136,12 @@ int octo_fmm_launch_info(const octo_fmm_t *h, int *grid, int *block, int *smem_b
 int octo_fmm_fp64_peak_probe(int device, void *stream, void *scratch, int iters, double *flops_per_s,
                              int *sm_count, int *clock_khz);
 
+/* FP64 issue-rate probe with REGISTER operands, 12 warps per SM: mode 0 = DFMA with three fresh register
+ * operands, 1 = DFMA repeating one operand in the same slot (operand-reuse cache), 2 = DMUL.  Returns
+ * thread-level FP64 instructions per second (issue peak = SMs x 64 x clock).  It documents why the
+ * interaction kernel's FP64 pipe is not 100 % busy.  scratch: device, >= 8 MiB. */
+int octo_fmm_fp64_issue_probe(int device, void *stream, void *scratch, int mode, int iters, double *instr_per_s);
+
 /* FP64 operations one multipole (kind 0) / monopole (kind 1) interaction executes in the kernel's
  * inner loop, counted from its operation list (DFMA = 2, DADD/DMUL = 1); see DESIGN.md. */
 int octo_fmm_flops_per_interaction(int kind, int am_correction, int *flops, int *fp64_instructions);

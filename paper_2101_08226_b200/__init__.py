@@ -66,6 +66,7 @@ class _Library:
         lib.octo_fmm_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
         lib.octo_fmm_launch_info.argtypes = [vp, ip, ip, ip, ip, ip]
         lib.octo_fmm_fp64_peak_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, dp, ip, ip]
+        lib.octo_fmm_fp64_issue_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, ctypes.c_int, dp]
         lib.octo_fmm_flops_per_interaction.argtypes = [ctypes.c_int, ctypes.c_int, ip, ip]
         lib.octo_fmm_version.restype = ctypes.c_char_p
         self._cdll = lib
@@ -203,6 +204,14 @@ def octo_fmm_fp64_peak_probe(device, stream, scratch, iters=20000):
     if rc != OK:
         raise OctoFmmError("octo_fmm_fp64_peak_probe", rc)
     return {"flops_per_s": f.value, "sm_count": sm.value, "clock_khz": clk.value}
+
+
+def octo_fmm_fp64_issue_probe(device, stream, scratch, mode, iters=2000):
+    r = ctypes.c_double(0)
+    rc = _lib.octo_fmm_fp64_issue_probe(int(device), stream or None, _ptr(scratch), int(mode), int(iters), ctypes.byref(r))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_fp64_issue_probe", rc)
+    return r.value
 
 
 def octo_fmm_flops_per_interaction(kind, am_correction):

@@ -471,4 +471,37 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, 
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
 }
 
+
+// FP64 issue-rate probe with register operands (the peak probe above uses immediates):
+//   MODE 0: a[i] = fma(b[.], c[.], a[i]) with three fresh register operands per instruction
+//   MODE 1: a[i] = fma(b[u], c[i], a[i]): 16 consecutive DFMAs repeat b[u] in the same slot (operand-reuse cache)
+//   MODE 2: a[i] = a[i] * b[.]  (DMUL, two register operands)
+template <int MODE>
+__global__ void __launch_bounds__(384) fp64_issue_probe_kernel(double* out, const double* __restrict__ in, int iters)
+{
+    constexpr int NA = 16;
+    double a[NA], b[4], c[8];
+#pragma unroll
+    for (int i = 0; i < NA; ++i) a[i] = in[threadIdx.x + i];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) b[i] = in[64 + threadIdx.x + i];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) c[i] = in[128 + threadIdx.x + i];
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int i = 0; i < NA; ++i) {
+                if (MODE == 0) a[i] = fma(b[(i + u) & 3], c[(i * 3 + u) & 7], a[i]);
+                else if (MODE == 1) a[i] = fma(b[u], c[i & 7], a[i]);
+                else a[i] = a[i] * b[(i + u) & 3];
+            }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < NA; ++i) s += a[i];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace octo

@@ -641,6 +641,38 @@ int octo_fmm_fp64_peak_probe(int device, void* stream, void* scratch, int iters,
     return OCTO_FMM_OK;
 }
 
+int octo_fmm_fp64_issue_probe(int device, void* stream, void* scratch, int mode, int iters, double* instr_per_s)
+{
+    if (!scratch || iters <= 0 || !instr_per_s || mode < 0 || mode > 2) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int blocks = prop.multiProcessorCount, threads = 384;     // 12 warps per SM, as the interaction kernel
+    double* out = (double*)scratch;
+    double* in = out + (size_t)blocks * threads;
+    if (((size_t)blocks * threads + 1024) * 8 > (size_t)8 * 1024 * 1024) return OCTO_FMM_EINVAL;
+    if (cudaMemsetAsync(in, 0, 1024 * 8, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return OCTO_FMM_ECUDA;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int n = pass ? iters : iters / 8 + 1;
+        if (pass) cudaEventRecord(e0, st);
+        if (mode == 0) fp64_issue_probe_kernel<0><<<blocks, threads, 0, st>>>(out, in, n);
+        else if (mode == 1) fp64_issue_probe_kernel<1><<<blocks, threads, 0, st>>>(out, in, n);
+        else fp64_issue_probe_kernel<2><<<blocks, threads, 0, st>>>(out, in, n);
+    }
+    cudaEventRecord(e1, st);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    *instr_per_s = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3);   // thread-level FP64 instructions
+    return OCTO_FMM_OK;
+}
+
 int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int* fp64_instructions)
 {
     // Counted from the operation list of m2l_pair<> + the separation.

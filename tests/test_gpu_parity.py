@@ -303,3 +303,15 @@ def test_fp64_probe_runs(env):
     scratch = torch.empty(8 << 20, dtype=torch.uint8, device="cuda")
     r = p.octo_fmm_fp64_peak_probe(0, torch.cuda.current_stream().cuda_stream, scratch, 4000)
     assert r["sm_count"] > 0 and r["flops_per_s"] > 1e12
+
+
+def test_fp64_issue_probe_shows_the_register_read_limit(env):
+    """a DFMA with three fresh register operands issues at about 2/3 of the rate of a
+    DMUL; repeating an operand in the same slot (operand-reuse cache) recovers most of it."""
+    p, torch = env
+    scratch = torch.empty(8 << 20, dtype=torch.uint8, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    fresh, reuse, dmul = (p.octo_fmm_fp64_issue_probe(0, st, scratch, m, 1000) for m in (0, 1, 2))
+    assert dmul > 1e12
+    assert 0.55 < fresh / dmul < 0.80
+    assert reuse > 1.15 * fresh
