@@ -397,7 +397,8 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
 // ------------------------------------------------------------------------------------------
 // a5: monopole (leaf) variant.  R = (i_A - i_B) h has no per-cell part, so -1/|R| and
 // -R/|R|^3 depend on the list entry only: they are tabulated once per (class, entry) on the
-// host in FP64 and the kernel is a 4-FMA stencil sum.  W = [class][entry]{w0,wx,wy,wz}.
+// host in FP64 and the kernel is a 4-FMA stencil sum.  W = [class][entry]{w0,wx,wy,wz}
+// (class-major with stride MAX_LIST, indexed like c_entries).
 // mass is zero-padded by REACH_MAX cells on every side: P[(nz+10)][(ny+10)][(nx+10)].
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __restrict__ mass, double* __restrict__ P,
@@ -414,42 +415,73 @@ __global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __res
     P[i] = in ? mass[((long long)z * ny + y) * nx + x] : 0.0;
 }
 
-__global__ void __launch_bounds__(256) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
-                                                           const double4* __restrict__ W, double* __restrict__ out)
+constexpr int MT_X = 16, MT_Y = 16, MT_Z = 8;           // target tile of one block
+constexpr int MS_X = MT_X + 2 * REACH_MAX, MS_Y = MT_Y + 2 * REACH_MAX, MS_Z = MT_Z + 2 * REACH_MAX;
+constexpr int MONO_SMEM = MS_X * MS_Y * MS_Z * 8;       // 97344 B: two blocks per SM
+
+// One block = a 16 x 16 x 8 target tile whose masses (tile + 5-cell halo) sit in shared memory.
+// Warp w holds xy-parity class w >> 1, rows 4 (w & 1) + {0..3} of that class; every thread owns one
+// (x, y) and all 8 layers: two passes (even z, odd z), 4 targets per pass that share the parity
+// class, hence the list and the weights -- one uniform weight load and 4 mass loads feed 16 DFMAs,
+// each of which repeats the mass operand of its predecessor (operand-reuse cache).
+__global__ void __launch_bounds__(256, 2) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
+                                                              const double4* __restrict__ W, double* __restrict__ out)
 {
+    extern __shared__ __align__(16) double tile[];
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
-    const int px = warp & 1, py = (warp >> 1) & 1, pz = warp >> 2;
-    const int bx = (p.ox + 15) / 16, by = (p.oy + 7) / 8;
+    const int px = (warp >> 1) & 1, py = warp >> 2;
+    const int bx = (p.ox + MT_X - 1) / MT_X, by = (p.oy + MT_Y - 1) / MT_Y;
     const int b = blockIdx.x;
-    const int x0 = p.lo[0] + (b % bx) * 16, y0 = p.lo[1] + ((b / bx) % by) * 8, z0 = p.lo[2] + (b / (bx * by)) * 4;
-    const int gx = x0 + px + 2 * (lane & 7), gy = y0 + py + 2 * ((lane >> 3) & 3);
-    const int X = p.nx + 2 * REACH_MAX, Y = p.ny + 2 * REACH_MAX;
-    const long long ocell = (long long)p.ox * p.oy * p.oz;
-    const int cls = warp;
-    const int s_begin = c_begin[cls][0], s_end = c_begin[cls][2 * REACH_MAX + 1];
-    // two cells per thread (k and k + 2 share the parity class, hence the list and the weights)
-    const int k0 = z0 + pz, k1 = k0 + 2;
-    const bool act0 = gx < p.hi[0] && gy < p.hi[1] && k0 < p.hi[2];
-    const bool act1 = gx < p.hi[0] && gy < p.hi[1] && k1 < p.hi[2];
-    if (!act0) return;
-    const double* c0 = P + ((long long)(k0 + REACH_MAX) * Y + (gy + REACH_MAX)) * X + (gx + REACH_MAX);
-    const double* c1 = act1 ? c0 + 2LL * Y * X : c0;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0, b0 = 0.0, b1 = 0.0, b2 = 0.0, b3 = 0.0;
-#pragma unroll 4
-    for (int s = s_begin; s < s_end; ++s) {
-        const StEntry e = c_entries[cls * MAX_LIST + s];
-        const long long off = ((long long)e.dz * Y + e.dy) * X + e.dx;
-        const double4 w = W[cls * MAX_LIST + s];
-        const double m0 = c0[off], m1 = c1[off];
-        a0 = fma(m0, w.x, a0); a1 = fma(m0, w.y, a1); a2 = fma(m0, w.z, a2); a3 = fma(m0, w.w, a3);
-        b0 = fma(m1, w.x, b0); b1 = fma(m1, w.y, b1); b2 = fma(m1, w.z, b2); b3 = fma(m1, w.w, b3);
+    const int x0 = p.lo[0] + (b % bx) * MT_X, y0 = p.lo[1] + ((b / bx) % by) * MT_Y, z0 = p.lo[2] + (b / (bx * by)) * MT_Z;
+    const int X = p.nx + 2 * REACH_MAX, Y = p.ny + 2 * REACH_MAX, Z = p.nz + 2 * REACH_MAX;
+
+    // tile (x0-5 .. x0+20, ...) = padded coordinates (x0 .. x0+25, ...); beyond the padded array -> 0
+    for (int i = threadIdx.x; i < MS_X * MS_Y * MS_Z; i += 256) {
+        const int tx = i % MS_X, r = i / MS_X, ty = r % MS_Y, tz = r / MS_Y;
+        const int gx = x0 + tx, gy = y0 + ty, gz = z0 + tz;
+        tile[i] = (gx < X && gy < Y && gz < Z) ? P[((long long)gz * Y + gy) * X + gx] : 0.0;
     }
-    long long o = ((long long)(k0 - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
-    out[o] = a0; out[ocell + o] = a1; out[2 * ocell + o] = a2; out[3 * ocell + o] = a3;
-    if (act1) {
-        o += 2LL * p.oy * p.ox;
-        out[o] = b0; out[ocell + o] = b1; out[2 * ocell + o] = b2; out[3 * ocell + o] = b3;
+    __syncthreads();
+
+    const int lx = lane & 7, ly = ((warp & 1) << 2) + (lane >> 3);
+    const int gx = x0 + px + 2 * lx, gy = y0 + py + 2 * ly;
+    const bool act_xy = gx < p.hi[0] && gy < p.hi[1];
+    const long long ocell = (long long)p.ox * p.oy * p.oz;
+    constexpr int LAYER2 = 2 * MS_Y * MS_X;
+#pragma unroll 1
+    for (int pz = 0; pz < 2; ++pz) {
+        const int cls = (px + 2 * py) + 4 * pz;
+        const double* base = tile + ((pz + REACH_MAX) * MS_Y + (py + 2 * ly + REACH_MAX)) * MS_X + (px + 2 * lx + REACH_MAX);
+        double a[4][4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) a[j][c] = 0.0;
+        const int s_begin = cls * MAX_LIST + c_begin[cls][0], s_end = cls * MAX_LIST + c_begin[cls][2 * REACH_MAX + 1];
+#pragma unroll 2
+        for (int s = s_begin; s < s_end; ++s) {
+            const StEntry e = c_entries[s];
+            const double* q = base + (e.dz * MS_Y + e.dy) * MS_X + e.dx;
+            const double4 w = W[s];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const double m = q[j * LAYER2];
+                a[j][0] = fma(m, w.x, a[j][0]);
+                a[j][1] = fma(m, w.y, a[j][1]);
+                a[j][2] = fma(m, w.z, a[j][2]);
+                a[j][3] = fma(m, w.w, a[j][3]);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int k = z0 + pz + 2 * j;
+            if (act_xy && k < p.hi[2]) {
+                const long long o = ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) out[c * ocell + o] = a[j][c];
+            }
+        }
     }
 }
 

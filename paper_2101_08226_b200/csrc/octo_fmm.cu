@@ -306,6 +306,9 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
         if (cudaMemcpyAsync(h->W, h->weights.data(), h->weights.size() * sizeof(double4), cudaMemcpyHostToDevice,
                             h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
         if (cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+        if (cudaFuncSetAttribute(p2p_monopole_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MONO_SMEM) != cudaSuccess) {
+            delete h; return OCTO_FMM_ECUDA;
+        }
     }
     *out = h;
     return OCTO_FMM_OK;
@@ -356,6 +359,11 @@ static int launch_staged(octo_fmm_t* h, int kb, int ke)
     return cudaGetLastError() == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
 
+static int mono_blocks(const Params& P)
+{
+    return ((P.ox + MT_X - 1) / MT_X) * ((P.oy + MT_Y - 1) / MT_Y) * ((P.oz + MT_Z - 1) / MT_Z);
+}
+
 static int brick_blocks(const Params& P) { return ((P.ox + 15) / 16) * ((P.oy + 7) / 8) * ((P.oz + 3) / 4); }
 
 int octo_fmm_interact(octo_fmm_t* h)
@@ -368,7 +376,7 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        p2p_monopole_kernel<<<brick_blocks(P), 256, 0, h->stream>>>(P, h->src, h->W, h->outL);
+        p2p_monopole_kernel<<<mono_blocks(P), 256, MONO_SMEM, h->stream>>>(P, h->src, h->W, h->outL);
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
@@ -596,7 +604,7 @@ int octo_fmm_launch_info(const octo_fmm_t* h, int* grid, int* block, int* smem_b
     int g, b, s;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
         e = cudaFuncGetAttributes(&fa, p2p_monopole_kernel);
-        g = brick_blocks(P); b = 256; s = 0;
+        g = mono_blocks(P); b = 256; s = MONO_SMEM;
     } else if (h->kernel == 1) {
         e = h->cfg.am_correction ? cudaFuncGetAttributes(&fa, m2l_direct_kernel<true>) : cudaFuncGetAttributes(&fa, m2l_direct_kernel<false>);
         g = brick_blocks(P); b = 256; s = 0;
