@@ -53,6 +53,7 @@ struct StEntry {
 __constant__ StEntry c_entries[8 * MAX_LIST];
 __constant__ int c_begin[8][2 * REACH_MAX + 2];   // first entry of (class, dz); [..][11] = end
 __constant__ double c_hmul[2 * REACH_MAX + 1];    // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h)
+__constant__ double2 c_mono_rad[3 * REACH_MAX * REACH_MAX + 1];   // monopole: {-1/r, -1/r^3}, r = sqrt(d2) h, by d2 = |Delta|^2
 
 struct Params {
     int nx, ny, nz;
@@ -396,9 +397,8 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
 
 // ------------------------------------------------------------------------------------------
 // a5: monopole (leaf) variant.  R = (i_A - i_B) h has no per-cell part, so -1/|R| and
-// -R/|R|^3 depend on the list entry only: they are tabulated once per (class, entry) on the
-// host in FP64 and the kernel is a 4-FMA stencil sum.  W = [class][entry]{w0,wx,wy,wz}
-// (class-major with stride MAX_LIST, indexed like c_entries).
+// -R/|R|^3 depend on the list entry only: -1/r and -1/r^3 are tabulated by |Delta|^2 on the host
+// in FP64 (constant memory) and the kernel is a 4-FMA stencil sum.
 // mass is zero-padded by REACH_MAX cells on every side: P[(nz+10)][(ny+10)][(nx+10)].
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __restrict__ mass, double* __restrict__ P,
@@ -425,7 +425,7 @@ constexpr int MONO_SMEM = MS_X * MS_Y * MS_Z * 8;       // 97344 B: two blocks p
 // class, hence the list and the weights -- one uniform weight load and 4 mass loads feed 16 DFMAs,
 // each of which repeats the mass operand of its predecessor (operand-reuse cache).
 __global__ void __launch_bounds__(256, 2) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
-                                                              const double4* __restrict__ W, double* __restrict__ out)
+                                                              double* __restrict__ out)
 {
     extern __shared__ __align__(16) double tile[];
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
@@ -463,7 +463,13 @@ __global__ void __launch_bounds__(256, 2) p2p_monopole_kernel(const Params p, co
         for (int s = s_begin; s < s_end; ++s) {
             const StEntry e = c_entries[s];
             const double* q = base + (e.dz * MS_Y + e.dy) * MS_X + e.dx;
-            const double4 w = W[s];
+            // weights of this list entry: they depend on Delta only (R = -Delta h has no per-cell part)
+            const double2 rad = c_mono_rad[e.dx * e.dx + e.dy * e.dy + e.dz * e.dz];
+            double4 w;
+            w.x = rad.x;
+            w.y = c_hmul[e.dx + REACH_MAX] * rad.y;
+            w.z = c_hmul[e.dy + REACH_MAX] * rad.y;
+            w.w = c_hmul[e.dz + REACH_MAX] * rad.y;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const double m = q[j * LAYER2];

@@ -79,7 +79,7 @@ bool config_ok(const octo_fmm_config* c)
     return true;
 }
 
-struct Sizes { size_t src, L, C, W, flags, total; };
+struct Sizes { size_t src, L, C, flags, total; };
 
 Sizes sizes_of(const octo_fmm_config& c)
 {
@@ -92,16 +92,14 @@ Sizes sizes_of(const octo_fmm_config& c)
         s.src = align_up(ncell * NPAIR * 2 * sizeof(double));
         s.L = align_up(ocell * 20 * sizeof(double));
         s.C = align_up(ocell * 3 * sizeof(double));
-        s.W = 0;
     } else {
         const size_t pc = (size_t)(c.n[0] + 2 * REACH_MAX) * (c.n[1] + 2 * REACH_MAX) * (c.n[2] + 2 * REACH_MAX);
         s.src = align_up(pc * sizeof(double));
         s.L = align_up(ocell * 4 * sizeof(double));
         s.C = 0;
-        s.W = align_up((size_t)8 * MAX_LIST * sizeof(double4));
     }
     s.flags = ALIGN;
-    s.total = s.src + s.L + s.C + s.W + s.flags;
+    s.total = s.src + s.L + s.C + s.flags;
     return s;
 }
 
@@ -134,7 +132,7 @@ struct octo_fmm {
     std::vector<StEntry> entries;          // 8 * MAX_LIST
     int begin[8][2 * REACH_MAX + 2];
     double hmul[2 * REACH_MAX + 1];
-    std::vector<double4> weights;          // monopole: 8 * MAX_LIST
+    double2 mono_rad[3 * REACH_MAX * REACH_MAX + 1];   // monopole: {-1/r, -1/r^3} by |Delta|^2
     unsigned long long n_interactions;
     CUtensorMap tmap;
     Params prm;
@@ -145,7 +143,6 @@ struct octo_fmm {
     double* outC;
     double* resL;          // where the last interact() left its results
     double* resC;
-    double4* W;
     int* flags;
     int state;          // 0 created, 1 sources staged, 2 interacted
     int kernel;         // 0 staged (TMA), 1 direct
@@ -258,7 +255,6 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     h->src = (double*)w; w += sz.src;
     h->L = (double*)w;   w += sz.L;
     h->C = (double*)w;   w += sz.C;
-    h->W = (double4*)w;  w += sz.W;
     h->flags = (int*)w;
 
     Params& P = h->prm;
@@ -292,20 +288,12 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
         cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         if (e1 != cudaSuccess || e2 != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
     } else {
-        // ---- monopole weights: -1/|R| and -R/|R|^3 with R = (i_A - i_B) h = -Delta h ----
-        h->weights.assign((size_t)8 * MAX_LIST, double4{0, 0, 0, 0});
-        for (int p = 0; p < 8; ++p)
-            for (size_t s = 0; s < h->list[p].size(); ++s) {
-                const double Rx = h->hmul[h->list[p][s].d[0] + REACH_MAX], Ry = h->hmul[h->list[p][s].d[1] + REACH_MAX],
-                             Rz = h->hmul[h->list[p][s].d[2] + REACH_MAX];
-                const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = std::sqrt(r2);
-                double4 wv;
-                wv.x = -1.0 / r; wv.y = -Rx / (r2 * r); wv.z = -Ry / (r2 * r); wv.w = -Rz / (r2 * r);
-                h->weights[(size_t)p * MAX_LIST + s] = wv;
-            }
-        if (cudaMemcpyAsync(h->W, h->weights.data(), h->weights.size() * sizeof(double4), cudaMemcpyHostToDevice,
-                            h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
-        if (cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+        // ---- monopole radial table: -1/r and -1/r^3 by d2 = |Delta|^2, r = sqrt(d2) h (FP64 sqrt and division on
+        //      the host); the kernel forms -R/r^3 = ((i_A - i_B) h) * (-1/r^3) per list entry ----
+        for (int d2 = 0; d2 <= 3 * REACH_MAX * REACH_MAX; ++d2) {
+            const double r = std::sqrt((double)d2) * cfg->h;
+            h->mono_rad[d2] = d2 ? double2{-1.0 / r, -1.0 / (r * r * r)} : double2{0.0, 0.0};
+        }
         if (cudaFuncSetAttribute(p2p_monopole_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MONO_SMEM) != cudaSuccess) {
             delete h; return OCTO_FMM_ECUDA;
         }
@@ -340,6 +328,9 @@ static int upload_tables(octo_fmm_t* h)
     if (cudaMemcpyToSymbolAsync(c_begin, h->begin, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
     if (cudaMemcpyToSymbolAsync(c_hmul, h->hmul, sizeof(h->hmul), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+        return OCTO_FMM_ECUDA;
+    if (h->cfg.kind == OCTO_FMM_MONOPOLE &&
+        cudaMemcpyToSymbolAsync(c_mono_rad, h->mono_rad, sizeof(h->mono_rad), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
     g_const_owner = h;
     return OCTO_FMM_OK;
@@ -376,7 +367,7 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        p2p_monopole_kernel<<<mono_blocks(P), 256, MONO_SMEM, h->stream>>>(P, h->src, h->W, h->outL);
+        p2p_monopole_kernel<<<mono_blocks(P), 256, MONO_SMEM, h->stream>>>(P, h->src, h->outL);
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
