@@ -45,8 +45,9 @@ constexpr int STAGED_SMEM = NSTAGE * SLAB_BYTES + 64;
 static_assert(STAGED_SMEM <= 227 * 1024, "shared memory per CTA");
 
 struct StEntry {
-    int off;                 // staged kernel: shared-memory offset (double2) relative to the thread's base
-    signed char dx, dy, dz, pad;
+    int off;                 // shared-memory offset relative to the thread's base (multipole: double2 units in
+                             // the slab; monopole: doubles in the mass tile)
+    signed char dx, dy, dz, d2;   // d2 = |Delta|^2 (monopole handles only)
 };
 
 // Stencil tables (the interaction lists of the 8 parity classes, Eq. 15) in constant memory.
@@ -417,15 +418,23 @@ __global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __res
 
 constexpr int MT_X = 16, MT_Y = 16, MT_Z = 8;           // target tile of one block
 constexpr int MS_X = MT_X + 2 * REACH_MAX, MS_Y = MT_Y + 2 * REACH_MAX, MS_Z = MT_Z + 2 * REACH_MAX;
-constexpr int MONO_SMEM = MS_X * MS_Y * MS_Z * 8;       // 97344 B: two blocks per SM
+constexpr int MS_XH = 14;                               // half-row: 13 cells of one x-parity + 1 pad
+constexpr int MS_ROW = 2 * MS_XH;                       // 28 doubles: two tile rows are 64 bytes mod 128 apart
+constexpr int MONO_SMEM = MS_ROW * MS_Y * MS_Z * 8;     // 104832 B: two blocks per SM
+constexpr int MONO_THREADS = 256;
 
-// One block = a 16 x 16 x 8 target tile whose masses (tile + 5-cell halo) sit in shared memory.
+// One block = a 16 x 16 x 8 target tile whose masses (tile + 5-cell halo) sit in shared memory,
+// every x-row de-interleaved into its even and odd cells (as the multipole slabs) and padded to 28
+// doubles, so that the 32 lanes of a warp (8 cells two apart in x, 4 rows two apart in y) read
+// 256 consecutive-bank bytes: two conflict-free wavefronts per LDS.64 instead of four.
 // Warp w holds xy-parity class w >> 1, rows 4 (w & 1) + {0..3} of that class; every thread owns one
 // (x, y) and all 8 layers: two passes (even z, odd z), 4 targets per pass that share the parity
-// class, hence the list and the weights -- one uniform weight load and 4 mass loads feed 16 DFMAs,
-// each of which repeats the mass operand of its predecessor (operand-reuse cache).
-__global__ void __launch_bounds__(256, 2) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
-                                                              double* __restrict__ out)
+// class, hence the list and the weights -- one entry decode and 4 mass loads feed 16 DFMAs.
+// Measured bound (profiles/r01_monopole.md): instruction issue -- an FP64 instruction holds the
+// dispatch port for its 2-3 cycles, so the ~30 decode/load instructions per entry are not hidden
+// under the 19 FP64 ones (72 cycles per warp and entry = 128 interactions).
+__global__ void __launch_bounds__(MONO_THREADS, 2) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
+                                                                       double* __restrict__ out)
 {
     extern __shared__ __align__(16) double tile[];
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
@@ -437,10 +446,11 @@ __global__ void __launch_bounds__(256, 2) p2p_monopole_kernel(const Params p, co
     const int X = p.nx + 2 * REACH_MAX, Y = p.ny + 2 * REACH_MAX, Z = p.nz + 2 * REACH_MAX;
 
     // tile (x0-5 .. x0+20, ...) = padded coordinates (x0 .. x0+25, ...); beyond the padded array -> 0
-    for (int i = threadIdx.x; i < MS_X * MS_Y * MS_Z; i += 256) {
+    for (int i = threadIdx.x; i < MS_X * MS_Y * MS_Z; i += MONO_THREADS) {
         const int tx = i % MS_X, r = i / MS_X, ty = r % MS_Y, tz = r / MS_Y;
-        const int gx = x0 + tx, gy = y0 + ty, gz = z0 + tz;
-        tile[i] = (gx < X && gy < Y && gz < Z) ? P[((long long)gz * Y + gy) * X + gx] : 0.0;
+        const int sx = x0 + tx, sy = y0 + ty, sz = z0 + tz;
+        tile[r * MS_ROW + (tx & 1) * MS_XH + (tx >> 1)] =
+            (sx < X && sy < Y && sz < Z) ? P[((long long)sz * Y + sy) * X + sx] : 0.0;
     }
     __syncthreads();
 
@@ -448,11 +458,12 @@ __global__ void __launch_bounds__(256, 2) p2p_monopole_kernel(const Params p, co
     const int gx = x0 + px + 2 * lx, gy = y0 + py + 2 * ly;
     const bool act_xy = gx < p.hi[0] && gy < p.hi[1];
     const long long ocell = (long long)p.ox * p.oy * p.oz;
-    constexpr int LAYER2 = 2 * MS_Y * MS_X;
+    constexpr int LAYER2 = 2 * MS_Y * MS_ROW;
 #pragma unroll 1
     for (int pz = 0; pz < 2; ++pz) {
         const int cls = (px + 2 * py) + 4 * pz;
-        const double* base = tile + ((pz + REACH_MAX) * MS_Y + (py + 2 * ly + REACH_MAX)) * MS_X + (px + 2 * lx + REACH_MAX);
+        // the entry offsets carry the x-parity part (host: e.off), the thread adds its own row and half-row index
+        const double* base = tile + ((pz + REACH_MAX) * MS_Y + (py + 2 * ly + REACH_MAX)) * MS_ROW + lx;
         double a[4][4];
 #pragma unroll
         for (int j = 0; j < 4; ++j)
@@ -462,9 +473,9 @@ __global__ void __launch_bounds__(256, 2) p2p_monopole_kernel(const Params p, co
 #pragma unroll 2
         for (int s = s_begin; s < s_end; ++s) {
             const StEntry e = c_entries[s];
-            const double* q = base + (e.dz * MS_Y + e.dy) * MS_X + e.dx;
+            const double* q = base + e.off;
             // weights of this list entry: they depend on Delta only (R = -Delta h has no per-cell part)
-            const double2 rad = c_mono_rad[e.dx * e.dx + e.dy * e.dy + e.dz * e.dz];
+            const double2 rad = c_mono_rad[e.d2];
             double4 w;
             w.x = rad.x;
             w.y = c_hmul[e.dx + REACH_MAX] * rad.y;

@@ -224,8 +224,15 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
             const int dx = h->list[p][s].d[0], dy = h->list[p][s].d[1], dz = h->list[p][s].d[2];
             StEntry e;
             // shared-memory offset of the source relative to the thread's base (see kernels.cuh)
-            e.off = (py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1);   // double2 units
-            e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz; e.pad = 0;
+            if (cfg->kind == OCTO_FMM_MULTIPOLE) {
+                e.off = (py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1);   // double2 units
+                e.d2 = 0;
+            } else {
+                // monopole: offset in the de-interleaved mass tile (doubles), see p2p_monopole_kernel
+                e.off = (dz * MS_Y + dy) * MS_ROW + (((px + dx + REACH_MAX) & 1) ? MS_XH : 0) + ((px + dx + REACH_MAX) >> 1);
+                e.d2 = (signed char)(dx * dx + dy * dy + dz * dz);    // <= 75: index of the radial table
+            }
+            e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz;
             h->entries[(size_t)p * MAX_LIST + s] = e;
         }
     }
@@ -367,7 +374,7 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        p2p_monopole_kernel<<<mono_blocks(P), 256, MONO_SMEM, h->stream>>>(P, h->src, h->outL);
+        p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(P, h->src, h->outL);
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
@@ -595,7 +602,7 @@ int octo_fmm_launch_info(const octo_fmm_t* h, int* grid, int* block, int* smem_b
     int g, b, s;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
         e = cudaFuncGetAttributes(&fa, p2p_monopole_kernel);
-        g = mono_blocks(P); b = 256; s = MONO_SMEM;
+        g = mono_blocks(P); b = MONO_THREADS; s = MONO_SMEM;
     } else if (h->kernel == 1) {
         e = h->cfg.am_correction ? cudaFuncGetAttributes(&fa, m2l_direct_kernel<true>) : cudaFuncGetAttributes(&fa, m2l_direct_kernel<false>);
         g = brick_blocks(P); b = 256; s = 0;
