@@ -50,6 +50,8 @@ def make_workload(name, theta, ncell, seed):
         w = fi.config3(seed=seed, theta=theta, ncell=ncell or 128)
     elif name == "cfg2":
         w = fi.config2(seed=seed, theta=theta, ncell=ncell or 32)
+    elif name == "cfg4":
+        w = fi.config4(seed=seed, theta=theta, ncell=ncell or 128)
     else:
         raise SystemExit("unknown workload " + name)
     return w
@@ -81,7 +83,10 @@ def oracle_sample(w, theta, nregions, first=0):
     t0 = time.perf_counter()
     total = 0
     for lo, hi in regions:
-        _, _, cnt = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, lo, hi, True)
+        if w.com_off is None:      # monopole workload (cfg 4)
+            _, cnt = oracle.interact_monopole(w.n, w.h, theta, w.moments[0], lo, hi)
+        else:
+            _, _, cnt = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, lo, hi, True)
         total += cnt
     return total, time.perf_counter() - t0, oracle.num_threads(), len(regions)
 
@@ -215,15 +220,18 @@ def run_ours(args):
     w = make_workload(args.workload, args.theta, args.ncell, args.seed + rank)
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
-    f = p.OctoFMM(w.n, w.h, args.theta, p.MULTIPOLE, True, device=local, stream=stream)
+    multi = w.com_off is not None          # cfg 4 is the monopole (leaf) variant
+    kind = p.MULTIPOLE if multi else p.MONOPOLE
+    f = p.OctoFMM(w.n, w.h, args.theta, kind, True, device=local, stream=stream)
     n_int = f.interaction_count()
     info = f.launch_info()
-    flops_per, instr_per = p.octo_fmm_flops_per_interaction(p.MULTIPOLE, True)
+    flops_per, instr_per = p.octo_fmm_flops_per_interaction(kind, True)
 
     mom = torch.from_numpy(w.moments).to(dev)
-    com = torch.from_numpy(w.com_off).to(dev)
-    L = torch.empty((20,) + f.out_shape, dtype=torch.float64, device=dev)
-    Lc = torch.empty((3,) + f.out_shape, dtype=torch.float64, device=dev)
+    com = torch.from_numpy(w.com_off).to(dev) if multi else None
+    ncoef = 20 if multi else 4
+    L = torch.empty((ncoef,) + f.out_shape, dtype=torch.float64, device=dev)
+    Lc = torch.empty((3,) + f.out_shape, dtype=torch.float64, device=dev) if multi else None
 
     f.bind_outputs(L, Lc)          # interact() writes the expansions straight into the caller's buffers
 
@@ -249,18 +257,27 @@ def run_ours(args):
     kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     t_begin = time.perf_counter()
+    # inputs + outputs smaller than L2 (cfg 4): flush L2 between the timed steps by writing 256 MB, and time every
+    # step with its own pair of events so that the flush is not counted
+    flush = (mom.numel() + L.numel()) * 8 < 256e6
+    l2_scratch = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if flush else None
+    sev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     ev0.record(stream)
     for i in range(args.steps):
+        if flush:
+            l2_scratch.fill_(i & 1)
+        sev[i][0].record(stream)
         f.set_moments(mom, com)
         kev[i][0].record(stream)
         f.interact()
         kev[i][1].record(stream)
         f.get_expansions(L, Lc)
+        sev[i][1].record(stream)
     ev1.record(stream)
     barrier()
     t_end = time.perf_counter()
     clocks = sampler.stop(t_begin, t_end)
-    ms_total = ev0.elapsed_time(ev1)
+    ms_total = sum(a.elapsed_time(b) for a, b in sev) if flush else ev0.elapsed_time(ev1)
     kernel_ms = sum(a.elapsed_time(b) for a, b in kev) / args.steps
     if f.status() != p.OK:
         raise SystemExit("bench.py: device reported status %d" % f.status())
@@ -274,9 +291,9 @@ def run_ours(args):
         nb = p.octo_fmm_host_scratch_bytes(f.cfg)
         scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
         mom_h = torch.from_numpy(w.moments).pin_memory()
-        com_h = torch.from_numpy(w.com_off).pin_memory()
-        L_h = torch.empty((20,) + f.out_shape, dtype=torch.float64).pin_memory()
-        Lc_h = torch.empty((3,) + f.out_shape, dtype=torch.float64).pin_memory()
+        com_h = torch.from_numpy(w.com_off).pin_memory() if multi else None
+        L_h = torch.empty((ncoef,) + f.out_shape, dtype=torch.float64).pin_memory()
+        Lc_h = torch.empty((3,) + f.out_shape, dtype=torch.float64).pin_memory() if multi else None
         p.octo_fmm_run_host(f.handle, mom_h, com_h, L_h, Lc_h, scratch, nb)       # warm-up
         barrier()
         t0 = time.perf_counter()
@@ -289,8 +306,8 @@ def run_ours(args):
         e2e_ms = max(a.elapsed_time(b), 1e3 * (time.perf_counter() - t0))
         e2e_ms, e2e_units = aggregate_over_ranks(e2e_ms, n_int * args.e2e_steps, dist if world > 1 else None, dev)
         e2e = {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT,
-               "h2d_bytes_per_step": int(mom_h.numel() * 8 + com_h.numel() * 8),
-               "d2h_bytes_per_step": int(L_h.numel() * 8 + Lc_h.numel() * 8),
+               "h2d_bytes_per_step": int(mom_h.numel() * 8 + (com_h.numel() * 8 if multi else 0)),
+               "d2h_bytes_per_step": int(L_h.numel() * 8 + (Lc_h.numel() * 8 if multi else 0)),
                "steps": args.e2e_steps, "ms_per_step": e2e_ms / args.e2e_steps,
                "checksum_L0": float(L_h[0].sum())}
         del scratch, mom_h, com_h, L_h, Lc_h
@@ -314,8 +331,9 @@ def run_ours(args):
     issue_peak = sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6
     issue_probe = {name: p.octo_fmm_fp64_issue_probe(local, stream.cuda_stream, probe_scratch, mode) / issue_peak
                    for mode, name in ((0, "dfma_three_fresh_registers"), (1, "dfma_operand_reuse"), (2, "dmul"))}
+    bytes_per_cell = (23 + 23) * 8 if multi else (1 + 4) * 8      # algorithmic: inputs read once, outputs written once
     achieved = flops_per * n_int / (kernel_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "m2l_staged_kernel<correction>", "achieved": achieved, "peak": peak_tflops,
+    roofline = {"bound": "alu", "kernel": "m2l_staged_kernel<correction>" if multi else "p2p_monopole_kernel", "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                 "peak_source": "derived: %d SMs x %d FP64 FMA lanes x 2 x %.0f MHz (sm_max_mhz of %s)" % (
                     sm_count, FP64_LANES_PER_SM, sm_max_mhz, "MEASURED_PEAKS.json" if peaks else "nvidia-smi"),
@@ -326,8 +344,8 @@ def run_ours(args):
                 "fp64_issue_probe_frac_of_issue_peak": issue_probe,
                 "kernel_ms": kernel_ms, "interactions_per_launch": n_int,
                 "traffic": TRAFFIC_BYTES.get((args.workload, args.ncell or 256, args.theta)),
-                "algorithmic_bytes": int((23 + 23) * 8 * w.moments[0].size),
-                "hbm_gbs_at_algorithmic_bytes": (23 + 23) * 8 * w.moments[0].size / (kernel_ms * 1e-3) / 1e9,
+                "algorithmic_bytes": int(bytes_per_cell * w.moments[0].size),
+                "hbm_gbs_at_algorithmic_bytes": bytes_per_cell * w.moments[0].size / (kernel_ms * 1e-3) / 1e9,
                 "hbm_peak_gbs": peaks.get("hbm_gbs")}
 
     # ---- the oracle timed beside it on this box's host cores (bounded sample) ----
@@ -339,9 +357,11 @@ def run_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "%s theta=%g correction=on (%d^3 cells, %d sub-grids of 8^3)" % (
-                w.name, args.theta, w.n[0], (w.n[0] // 8) ** 3),
-                "interactions_per_step": n_int, "l2": "inputs (%.2f GB) larger than L2" % (mom.numel() * 8 / 1e9),
+            "config": {"workload": "%s theta=%g %s (%d^3 cells, %d sub-grids of 8^3)" % (
+                w.name, args.theta, "correction=on" if multi else "monopole", w.n[0], (w.n[0] // 8) ** 3),
+                "interactions_per_step": n_int, "l2": ("inputs (%.2f GB) larger than L2" % (mom.numel() * 8 / 1e9)) if mom.numel() * 8 > 126e6 else
+                ("inputs + outputs (%.3f GB) vs 126 MB L2; 256 MB scratch written between timed steps" % (
+                    (mom.numel() + L.numel()) * 8 / 1e9)),
                 "launch": info, "parallelism": "independent problem per GPU" if world > 1 else "single GPU"},
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
             "gpu_launches": 2 * args.steps}
