@@ -315,3 +315,48 @@ def test_fp64_issue_probe_shows_the_register_read_limit(env):
     assert dmul > 1e12
     assert 0.55 < fresh / dmul < 0.80
     assert reuse > 1.15 * fresh
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.35, 0.7])
+def test_single_subgrid_domain(env, theta):
+    """Smallest legal grid: one 8^3 sub-grid that is the whole (isolated) domain -- most of every list falls
+    outside the grid, bricks are ragged in y-tiles and in z (8 = 3 + 3 + 2), the slab ring is clipped on both sides."""
+    w = fi.config1(seed=5, ncell=24)
+    w.moments = np.ascontiguousarray(w.moments[:, 8:16, 8:16, 8:16])
+    w.com_off = np.ascontiguousarray(w.com_off[:, 8:16, 8:16, 8:16])
+    w.n, w.out_lo, w.out_hi = (8, 8, 8), (0, 0, 0), (8, 8, 8)
+    for kernel in (0, 1):
+        L, Lc, cnt, _ = gpu_multipole(env, w, theta=theta, kernel=kernel)
+        Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off)
+        assert cnt == cntr > 0
+        check(L, Lc, Lr, Lcr)
+
+
+def test_zero_mass_sources_are_harmless(env):
+    """Cells of zero mass and zero moments as SOURCES contribute exactly nothing (Q9/Q18); as targets they are
+    only legal with the correction off."""
+    p, torch = env
+    w = fi.config1(seed=9)
+    hole = (slice(None), slice(3, 9), slice(14, 20), slice(2, 7))      # a block outside the 8..16 output region
+    w.moments[hole] = 0.0
+    w.com_off[hole] = 0.0
+    L, Lc, cnt, _ = gpu_multipole(env, w)
+    Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, w.theta, w.moments, w.com_off, w.out_lo, w.out_hi, True)
+    assert cnt == cntr and np.isfinite(L).all()
+    check(L, Lc, Lr, Lcr)
+
+
+def test_monopole_non_cubic_grid_and_sub_region(env):
+    """Monopole kernel on a 24 x 16 x 8 grid (tiles ragged in x, whole-domain faces) and on an interior region."""
+    p, torch = env
+    wm = fi.config4(ncell=24)
+    mass = np.ascontiguousarray(wm.moments[0][:8, :16, :])
+    for lo, hi in (((0, 0, 0), (0, 0, 0)), ((8, 8, 0), (24, 16, 8))):
+        g = p.OctoFMM((24, 16, 8), wm.h, 0.5, p.MONOPOLE, out_lo=lo, out_hi=hi)
+        out, _ = g.solve(torch.from_numpy(mass).cuda())
+        torch.cuda.synchronize()
+        olo, ohi = ((0, 0, 0), (24, 16, 8)) if hi == (0, 0, 0) else (lo, hi)
+        ref, cnt = oracle.interact_monopole((24, 16, 8), wm.h, 0.5, mass, olo, ohi)
+        assert g.interaction_count() == cnt
+        assert parity_error(out.cpu().numpy(), ref) < TOL
+        g.close()
