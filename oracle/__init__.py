@@ -51,6 +51,11 @@ def lib():
                                                     dp, dp, dp, dp, ullp]
         L.fmm_oracle_interact_monopole.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, dp, dp, ullp]
         L.fmm_oracle_interaction_count.argtypes = [ip, ip, ip, ctypes.c_double, ullp]
+        L.fmm_oracle_stencil_leaf.argtypes = L.fmm_oracle_stencil.argtypes
+        L.fmm_oracle_interact_monopole_leaf.argtypes = L.fmm_oracle_interact_monopole.argtypes
+        L.fmm_oracle_m2m.argtypes = [ip, ctypes.c_double, dp, dp, dp, dp]
+        L.fmm_oracle_l2l.argtypes = [ip, ctypes.c_double, dp, dp, dp, dp, dp, dp]
+        L.fmm_oracle_direct_sum.argtypes = [ip, ctypes.c_double, dp, dp]
         L.fmm_oracle_num_threads.restype = ctypes.c_int
         L.fmm_oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -151,3 +156,97 @@ def interaction_count(n, theta, out_lo=None, out_hi=None) -> int:
 
 def num_threads() -> int:
     return int(lib().fmm_oracle_num_threads())
+
+
+# ---- NEXT f1: the other passes of a complete uniform-grid solve ------------------------------------
+def stencil_leaf(theta: float, parity: int) -> np.ndarray:
+    """Leaf-level list of the complete solve: the Eq. 15 list plus the near field (every Delta != 0 whose
+    parents are not well separated), int8 [count][3], (dz,dy,dx)-lexicographic."""
+    L = lib()
+    cnt = ctypes.c_int(0)
+    _check(L.fmm_oracle_stencil_leaf(theta, parity, 0, ctypes.byref(cnt), None), "stencil_leaf")
+    out = np.zeros((cnt.value, 3), dtype=np.int8)
+    _check(L.fmm_oracle_stencil_leaf(theta, parity, cnt.value, ctypes.byref(cnt),
+                                     out.ctypes.data_as(ctypes.POINTER(ctypes.c_byte))), "stencil_leaf")
+    return out
+
+
+def interact_monopole_leaf(n, h, theta, mass):
+    """Monopole sum over the leaf-level list (Eq. 15 list + near field), whole grid.  Returns (out[4], count)."""
+    nx, ny, nz = n
+    mass = np.ascontiguousarray(mass, dtype=np.float64).reshape(nz, ny, nx)
+    out = np.zeros((4, nz, ny, nx))
+    cnt = ctypes.c_ulonglong(0)
+    _check(lib().fmm_oracle_interact_monopole_leaf(_i3(n), _i3((0, 0, 0)), _i3(n), float(h), float(theta), _dp(mass),
+                                                   _dp(out), ctypes.byref(cnt)), "interact_monopole_leaf")
+    return out, cnt.value
+
+
+def m2m(n_child, h_child, moments, com_off):
+    """Parent multipoles [20][n/2] and centre-of-mass offsets [3][n/2] from the children's (L125)."""
+    nx, ny, nz = n_child
+    moments = np.ascontiguousarray(moments, dtype=np.float64)
+    com_off = np.ascontiguousarray(com_off, dtype=np.float64)
+    assert moments.shape == (20, nz, ny, nx) and com_off.shape == (3, nz, ny, nx)
+    pm = np.zeros((20, nz // 2, ny // 2, nx // 2))
+    po = np.zeros((3, nz // 2, ny // 2, nx // 2))
+    _check(lib().fmm_oracle_m2m(_i3(n_child), float(h_child), _dp(moments), _dp(com_off), _dp(pm), _dp(po)), "m2m")
+    return pm, po
+
+
+def l2l(n_child, h_child, parent_L, parent_corr, parent_off, child_off, child_L, child_corr):
+    """child_L += parent_L shifted to the child centres, child_corr += parent_corr (in place; L125)."""
+    for a in (parent_L, parent_corr, parent_off, child_off, child_L, child_corr):
+        assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    _check(lib().fmm_oracle_l2l(_i3(n_child), float(h_child), _dp(parent_L), _dp(parent_corr), _dp(parent_off),
+                                _dp(child_off), _dp(child_L), _dp(child_corr)), "l2l")
+
+
+def direct_sum(n, h, mass):
+    """Exact point-mass sum on the cell centres, out[4][nz][ny][nx] = (phi, g).  O(N^2)."""
+    nx, ny, nz = n
+    mass = np.ascontiguousarray(mass, dtype=np.float64).reshape(nz, ny, nx)
+    out = np.zeros((4, nz, ny, nx))
+    _check(lib().fmm_oracle_direct_sum(_i3(n), float(h), _dp(mass), _dp(out)), "direct_sum")
+    return out
+
+
+def solve(n, h, theta, mass, am_correction=True, coarsest=2):
+    """Complete uniform-grid solve on an isolated cubic grid of n = 2^k leaf cells per axis (2^3-cell level is the
+    coarsest that can hold interacting cells: siblings interact there when 3 theta^2 > 1):
+    leaves are point masses at their cell centres; upward pass (M2M) to the level of `coarsest`^3 cells; at every
+    multipole level the same-level interaction step (the hot path, Eq. 15 list, correction optional) plus the
+    parent's expansion (L2L); at the leaves the expansion of the parent evaluated at the cell centre plus the
+    monopole sum over the leaf-level list (Eq. 15 list + near field).  Returns out[4][n][n][n] = (phi, g_x, g_y, g_z),
+    g = -(L1 + correction) + direct part.  A cell's own mass contributes nothing (point-mass model)."""
+    n = int(n)
+    mass = np.ascontiguousarray(mass, dtype=np.float64).reshape(n, n, n)
+    # ---- upward pass ----
+    lev_n, lev_h = [n], [float(h)]
+    mom = np.zeros((20, n, n, n))
+    mom[0] = mass
+    lev_m, lev_o = [mom], [np.zeros((3, n, n, n))]
+    while lev_n[-1] > coarsest:
+        nc, hc = lev_n[-1], lev_h[-1]
+        assert nc % 2 == 0
+        pm, po = m2m((nc, nc, nc), hc, lev_m[-1], lev_o[-1])
+        lev_n.append(nc // 2); lev_h.append(2.0 * hc); lev_m.append(pm); lev_o.append(po)
+    # ---- downward pass over the multipole levels (coarsest first) ----
+    L_par = corr_par = None
+    for lv in range(len(lev_n) - 1, 0, -1):
+        nl, hl = lev_n[lv], lev_h[lv]
+        Lf, Lc, _ = interact_multipole((nl, nl, nl), hl, theta, lev_m[lv], lev_o[lv], None, None, am_correction)
+        L = Lf.copy()
+        L[1:4] -= Lc                       # the expansion proper; the correction is carried beside it
+        corr = Lc.copy()
+        if L_par is not None:
+            l2l((nl, nl, nl), hl, L_par, corr_par, lev_o[lv + 1], lev_o[lv], L, corr)
+        L_par, corr_par = L, corr
+    # ---- leaves ----
+    out, _ = interact_monopole_leaf((n, n, n), h, theta, mass)
+    if L_par is not None:
+        Ll = np.zeros((20, n, n, n)); cl = np.zeros((3, n, n, n))
+        l2l((n, n, n), h, L_par, corr_par, lev_o[1], lev_o[0], Ll, cl)
+        out[0] += Ll[0]
+        out[1:4] -= Ll[1:4] + cl
+    return out

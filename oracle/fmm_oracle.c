@@ -76,10 +76,12 @@ static int parent_of(int i) { return (i >= 0) ? (i / 2) : -((-i + 1) / 2); }
 
 /* Is Delta a partner of a cell with parity (px,py,pz)?  Cells well separated (L135),      */
 /* parents not well separated; a parent is never well separated from itself (Delta_I = 0). */
-static int is_partner(int px, int py, int pz, int dx, int dy, int dz, double theta)
+/* leaf != 0: the leaf-level list of the complete solve (NEXT f1) -- every Delta != 0 whose parents are not */
+/* well separated, i.e. the Eq. 15 list plus the near field (cells that are not well separated, L135/L456). */
+static int is_partner_mode(int px, int py, int pz, int dx, int dy, int dz, double theta, int leaf)
 {
     long d2 = (long)dx * dx + (long)dy * dy + (long)dz * dz;
-    if (d2 == 0 || !well_separated(d2, theta)) return 0;
+    if (d2 == 0 || (!leaf && !well_separated(d2, theta))) return 0;
     int Ix = parent_of(px + dx) - parent_of(px);
     int Iy = parent_of(py + dy) - parent_of(py);
     int Iz = parent_of(pz + dz) - parent_of(pz);
@@ -93,7 +95,7 @@ static int search_reach(double theta) { return 2 * (int)floor(1.0 / theta) + 3; 
 
 /* Stencil of parity class parity = px + 2 py + 4 pz, in lexicographic (dz, dy, dx) order. */
 /* dxyz receives up to cap triples (dx,dy,dz); *count is always the full count.           */
-int fmm_oracle_stencil(double theta, int parity, int cap, int *count, signed char *dxyz)
+static int stencil_mode(double theta, int parity, int leaf, int cap, int *count, signed char *dxyz)
 {
     if (!(theta > 0.0 && theta < 1.0) || parity < 0 || parity > 7 || !count) return ORC_EINVAL;
     int px = parity & 1, py = (parity >> 1) & 1, pz = (parity >> 2) & 1;
@@ -102,7 +104,7 @@ int fmm_oracle_stencil(double theta, int parity, int cap, int *count, signed cha
     for (int dz = -S; dz <= S; ++dz)
         for (int dy = -S; dy <= S; ++dy)
             for (int dx = -S; dx <= S; ++dx)
-                if (is_partner(px, py, pz, dx, dy, dz, theta)) {
+                if (is_partner_mode(px, py, pz, dx, dy, dz, theta, leaf)) {
                     if (dxyz && c < cap) {
                         dxyz[3 * c + 0] = (signed char)dx;
                         dxyz[3 * c + 1] = (signed char)dy;
@@ -112,6 +114,15 @@ int fmm_oracle_stencil(double theta, int parity, int cap, int *count, signed cha
                 }
     *count = c;
     return ORC_OK;
+}
+int fmm_oracle_stencil(double theta, int parity, int cap, int *count, signed char *dxyz)
+{
+    return stencil_mode(theta, parity, 0, cap, count, dxyz);
+}
+/* leaf-level list of the complete solve: Eq. 15 list + near field (see is_partner_mode) */
+int fmm_oracle_stencil_leaf(double theta, int parity, int cap, int *count, signed char *dxyz)
+{
+    return stencil_mode(theta, parity, 1, cap, count, dxyz);
 }
 
 /* ---------------------------------------------------------------------------------- */
@@ -277,18 +288,19 @@ static int check_region(const int n[3], const int lo[3], const int hi[3])
 /* Build the 8 per-parity partner lists once. */
 typedef struct { int count[8]; signed char *d[8]; } stencil_set;
 
-static int build_stencils(double theta, stencil_set *S)
+static int build_stencils_mode(double theta, int leaf, stencil_set *S)
 {
     memset(S, 0, sizeof *S);
     for (int p = 0; p < 8; ++p) {
         int c = 0;
-        if (fmm_oracle_stencil(theta, p, 0, &c, NULL) != ORC_OK) return ORC_EINVAL;
+        if (stencil_mode(theta, p, leaf, 0, &c, NULL) != ORC_OK) return ORC_EINVAL;
         S->d[p] = (signed char *)malloc((size_t)3 * (c > 0 ? c : 1));
         if (!S->d[p]) return ORC_EINVAL;
-        fmm_oracle_stencil(theta, p, c, &S->count[p], S->d[p]);
+        stencil_mode(theta, p, leaf, c, &S->count[p], S->d[p]);
     }
     return ORC_OK;
 }
+static int build_stencils(double theta, stencil_set *S) { return build_stencils_mode(theta, 0, S); }
 static void free_stencils(stencil_set *S) { for (int p = 0; p < 8; ++p) free(S->d[p]); }
 
 /*
@@ -361,14 +373,14 @@ int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int
  *   phi_A = -sum_B m_B/|R| ,  g_A = -sum_B m_B R/|R|^3 ,  R = x_A - x_B = (i_A - i_B) h.
  * out = [4][oz][oy][ox] = (phi, gx, gy, gz).
  */
-int fmm_oracle_interact_monopole(const int n[3], const int out_lo[3], const int out_hi[3], double h,
-                                 double theta, const double *mass, double *out,
-                                 unsigned long long *n_interactions)
+static int interact_monopole_mode(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                  double theta, int leaf, const double *mass, double *out,
+                                  unsigned long long *n_interactions)
 {
     if (!n || !out_lo || !out_hi || !mass || !out || !(h > 0.0)) return ORC_EINVAL;
     if (!check_region(n, out_lo, out_hi)) return ORC_EINVAL;
     stencil_set S;
-    if (build_stencils(theta, &S) != ORC_OK) return ORC_EINVAL;
+    if (build_stencils_mode(theta, leaf, &S) != ORC_OK) return ORC_EINVAL;
     const size_t nx = n[0], ny = n[1], nz = n[2];
     const size_t ox = out_hi[0] - out_lo[0], oy = out_hi[1] - out_lo[1], oz = out_hi[2] - out_lo[2];
     const size_t ocell = ox * oy * oz;
@@ -397,6 +409,20 @@ int fmm_oracle_interact_monopole(const int n[3], const int out_lo[3], const int 
     free_stencils(&S);
     if (n_interactions) *n_interactions = total;
     return ORC_OK;
+}
+
+int fmm_oracle_interact_monopole(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                 double theta, const double *mass, double *out,
+                                 unsigned long long *n_interactions)
+{
+    return interact_monopole_mode(n, out_lo, out_hi, h, theta, 0, mass, out, n_interactions);
+}
+/* the same sum over the leaf-level list of the complete solve (Eq. 15 list + near field) */
+int fmm_oracle_interact_monopole_leaf(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                      double theta, const double *mass, double *out,
+                                      unsigned long long *n_interactions)
+{
+    return interact_monopole_mode(n, out_lo, out_hi, h, theta, 1, mass, out, n_interactions);
 }
 
 /* Number of ordered in-domain pairs for a region, by enumeration on the index grid. */
@@ -439,4 +465,175 @@ void fmm_oracle_set_num_threads(int t)
 #else
     (void)t;
 #endif
+}
+
+/* ====================================================================================== */
+/* NEXT f1: the other passes of a complete uniform-grid solve, plain forms.   */
+/* "the multipoles of each cell are composed of the multipoles of its child cells ... The   */
+/* expansion of each cell is composed of the expansion due to its interactions with other   */
+/* cells at the same level, and the expansion of its parent cell".          */
+/* Positions are kept RELATIVE to the parent's geometric centre (no O(1) coordinates).      */
+/* ====================================================================================== */
+
+/* unique (lexicographic) -> full tensors of one cell */
+static void unpack_moments(const double *u, size_t stride, double *M0, double M1[3], double M2[3][3], double M3[3][3][3])
+{
+    *M0 = u[0];
+    for (int i = 0; i < 3; ++i) M1[i] = u[(size_t)(1 + i) * stride];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) M2[i][j] = u[(size_t)(4 + u2(i, j)) * stride];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j)
+            for (int k = 0; k < 3; ++k) M3[i][j][k] = u[(size_t)(10 + u3(i, j, k)) * stride];
+}
+
+/*
+ * M2M: parent multipoles (order 3, about the parent's centre of mass) from its 8 children.
+ * nc = child grid (even dims), hc = child cell width; child c of parent P=(I,J,K) is (2I+a,2J+b,2K+c).
+ * Child expansion centre relative to the parent's geometric centre: rel = ((a,b,c) - 1/2) hc + delta_c.
+ * Parent centre of mass: delta_P = sum_c (M_c rel_c + M1_c) / sum_c M_c   (geometric centre if the mass is 0).
+ * Shift of raw moments from z_c to z_P, d = z_c - z_P:
+ *   M1'_i = M1_i + M d_i;  M2'_ij = M2_ij + M1_i d_j + M1_j d_i + M d_i d_j;
+ *   M3'_ijk = M3_ijk + M2_ij d_k + M2_ik d_j + M2_jk d_i + M1_i d_j d_k + M1_j d_i d_k + M1_k d_i d_j + M d_i d_j d_k.
+ * pm = [20][nz/2][ny/2][nx/2], poff = [3][...].
+ */
+int fmm_oracle_m2m(const int nc[3], double hc, const double *cm, const double *coff, double *pm, double *poff)
+{
+    if (!nc || !cm || !coff || !pm || !poff || !(hc > 0.0)) return ORC_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (nc[a] <= 0 || (nc[a] & 1)) return ORC_EINVAL;
+    const size_t cx = nc[0], cy = nc[1], cz = nc[2], ccell = cx * cy * cz;
+    const size_t px = cx / 2, py = cy / 2, pz = cz / 2, pcell = px * py * pz;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (size_t K = 0; K < pz; ++K)
+        for (size_t J = 0; J < py; ++J)
+            for (size_t I = 0; I < px; ++I) {
+                double M0[8], M1[8][3], M2[8][3][3], M3[8][3][3][3], rel[8][3];
+                long double mass = 0.0L, com[3] = {0.0L, 0.0L, 0.0L};
+                for (int c = 0; c < 8; ++c) {
+                    const int a[3] = {c & 1, (c >> 1) & 1, (c >> 2) & 1};
+                    const size_t cell = ((2 * K + a[2]) * cy + (2 * J + a[1])) * cx + (2 * I + a[0]);
+                    unpack_moments(cm + cell, ccell, &M0[c], M1[c], M2[c], M3[c]);
+                    for (int i = 0; i < 3; ++i) rel[c][i] = ((double)a[i] - 0.5) * hc + coff[(size_t)i * ccell + cell];
+                    mass += (long double)M0[c];
+                    for (int i = 0; i < 3; ++i) com[i] += (long double)(M0[c] * rel[c][i]) + (long double)M1[c][i];
+                }
+                double dP[3] = {0.0, 0.0, 0.0};
+                if (mass != 0.0L)
+                    for (int i = 0; i < 3; ++i) dP[i] = (double)(com[i] / mass);
+                long double S1[3] = {0, 0, 0}, S2[3][3], S3[3][3][3];
+                memset(S2, 0, sizeof S2);
+                memset(S3, 0, sizeof S3);
+                for (int c = 0; c < 8; ++c) {
+                    double d[3];
+                    for (int i = 0; i < 3; ++i) d[i] = rel[c][i] - dP[i];
+                    for (int i = 0; i < 3; ++i) S1[i] += (long double)(M1[c][i] + M0[c] * d[i]);
+                    for (int i = 0; i < 3; ++i)
+                        for (int j = 0; j < 3; ++j)
+                            S2[i][j] += (long double)(M2[c][i][j] + M1[c][i] * d[j] + M1[c][j] * d[i] + M0[c] * d[i] * d[j]);
+                    for (int i = 0; i < 3; ++i)
+                        for (int j = 0; j < 3; ++j)
+                            for (int k = 0; k < 3; ++k)
+                                S3[i][j][k] += (long double)(M3[c][i][j][k] + M2[c][i][j] * d[k] + M2[c][i][k] * d[j] +
+                                                             M2[c][j][k] * d[i] + M1[c][i] * d[j] * d[k] + M1[c][j] * d[i] * d[k] +
+                                                             M1[c][k] * d[i] * d[j] + M0[c] * d[i] * d[j] * d[k]);
+                }
+                const size_t P = (K * py + J) * px + I;
+                pm[P] = (double)mass;
+                for (int i = 0; i < 3; ++i) pm[(size_t)(1 + i) * pcell + P] = (double)S1[i];
+                for (int i = 0; i < 3; ++i)
+                    for (int j = i; j < 3; ++j) pm[(size_t)(4 + u2(i, j)) * pcell + P] = (double)S2[i][j];
+                for (int i = 0; i < 3; ++i)
+                    for (int j = i; j < 3; ++j)
+                        for (int k = j; k < 3; ++k) pm[(size_t)(10 + u3(i, j, k)) * pcell + P] = (double)S3[i][j][k];
+                for (int i = 0; i < 3; ++i) poff[(size_t)i * pcell + P] = dP[i];
+            }
+    return ORC_OK;
+}
+
+/*
+ * L2L: add the parent's local expansion, shifted to the child's expansion centre, to the child's (L125).
+ * e = z_c - z_P = ((a,b,c) - 1/2) hc + delta_c - delta_P  (relative to the parent's geometric centre);
+ * Taylor shift to order 3:
+ *   L0_c += L0 + L1_i e_i + 1/2 L2_ij e_i e_j + 1/6 L3_ijk e_i e_j e_k
+ *   L1_c,i += L1_i + L2_ij e_j + 1/2 L3_ijk e_j e_k ;  L2_c,ij += L2_ij + L3_ijk e_k ;  L3_c += L3.
+ * The angular-momentum correction is a uniform acceleration of the parent cell and is handed down
+ * unchanged: corr_c += corr_P  (pcorr / ccorr may be NULL).
+ * pL = [20][parent grid], poff = [3][parent grid], coff = [3][child grid], cL = [20][child grid] (in/out).
+ */
+int fmm_oracle_l2l(const int nc[3], double hc, const double *pL, const double *pcorr, const double *poff,
+                   const double *coff, double *cL, double *ccorr)
+{
+    if (!nc || !pL || !poff || !coff || !cL || !(hc > 0.0)) return ORC_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (nc[a] <= 0 || (nc[a] & 1)) return ORC_EINVAL;
+    const size_t cx = nc[0], cy = nc[1], cz = nc[2], ccell = cx * cy * cz;
+    const size_t px = cx / 2, py = cy / 2, pcell = px * py * (cz / 2);
+#pragma omp parallel for collapse(2) schedule(static)
+    for (size_t k = 0; k < cz; ++k)
+        for (size_t j = 0; j < cy; ++j)
+            for (size_t i = 0; i < cx; ++i) {
+                const size_t cell = (k * cy + j) * cx + i;
+                const size_t P = ((k / 2) * py + (j / 2)) * px + (i / 2);
+                const int a[3] = {(int)(i & 1), (int)(j & 1), (int)(k & 1)};
+                double e[3], L0, L1[3], L2[3][3], L3[3][3][3];
+                for (int c = 0; c < 3; ++c)
+                    e[c] = ((double)a[c] - 0.5) * hc + coff[(size_t)c * ccell + cell] - poff[(size_t)c * pcell + P];
+                unpack_moments(pL + P, pcell, &L0, L1, L2, L3);
+                long double s0 = (long double)L0;
+                for (int x = 0; x < 3; ++x) {
+                    s0 += (long double)(L1[x] * e[x]);
+                    for (int y = 0; y < 3; ++y) {
+                        s0 += (long double)(0.5 * L2[x][y] * e[x] * e[y]);
+                        for (int z = 0; z < 3; ++z) s0 += (long double)(L3[x][y][z] * e[x] * e[y] * e[z] / 6.0);
+                    }
+                }
+                cL[cell] += (double)s0;
+                for (int x = 0; x < 3; ++x) {
+                    long double s1 = (long double)L1[x];
+                    for (int y = 0; y < 3; ++y) {
+                        s1 += (long double)(L2[x][y] * e[y]);
+                        for (int z = 0; z < 3; ++z) s1 += (long double)(0.5 * L3[x][y][z] * e[y] * e[z]);
+                    }
+                    cL[(size_t)(1 + x) * ccell + cell] += (double)s1;
+                }
+                for (int x = 0; x < 3; ++x)
+                    for (int y = x; y < 3; ++y) {
+                        long double s2 = (long double)L2[x][y];
+                        for (int z = 0; z < 3; ++z) s2 += (long double)(L3[x][y][z] * e[z]);
+                        cL[(size_t)(4 + u2(x, y)) * ccell + cell] += (double)s2;
+                    }
+                for (int x = 0; x < 3; ++x)
+                    for (int y = x; y < 3; ++y)
+                        for (int z = y; z < 3; ++z) cL[(size_t)(10 + u3(x, y, z)) * ccell + cell] += L3[x][y][z];
+                if (pcorr && ccorr)
+                    for (int c = 0; c < 3; ++c) ccorr[(size_t)c * ccell + cell] += pcorr[(size_t)c * pcell + P];
+            }
+    return ORC_OK;
+}
+
+/*
+ * Plain direct sum over point masses on the cell centres of an n^3-type grid (the exact result the
+ * complete solve approximates): phi_A = -sum_{B != A} m_B/|R|, g_A = -sum m_B R/|R|^3, G = 1 (L363).
+ * out = [4][nz][ny][nx].  O(N^2): for the pins on small grids only.
+ */
+int fmm_oracle_direct_sum(const int n[3], double h, const double *mass, double *out)
+{
+    if (!n || !mass || !out || !(h > 0.0)) return ORC_EINVAL;
+    const long nx = n[0], ny = n[1], nz = n[2], nc = nx * ny * nz;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (long a = 0; a < nc; ++a) {
+        const long ai = a % nx, aj = (a / nx) % ny, ak = a / (nx * ny);
+        long double acc[4] = {0.0L, 0.0L, 0.0L, 0.0L};
+        for (long b = 0; b < nc; ++b) {
+            if (b == a) continue;
+            const long bi = b % nx, bj = (b / nx) % ny, bk = b / (nx * ny);
+            const double R[3] = {(double)(ai - bi) * h, (double)(aj - bj) * h, (double)(ak - bk) * h};
+            const double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2], r = sqrt(r2), m = mass[b];
+            acc[0] += (long double)(-m / r);
+            for (int c = 0; c < 3; ++c) acc[1 + c] += (long double)(-m * R[c] / (r2 * r));
+        }
+        for (int c = 0; c < 4; ++c) out[(size_t)c * nc + a] = (double)acc[c];
+    }
+    return ORC_OK;
 }

@@ -1,0 +1,163 @@
+"""Pins of the oracle's complete uniform-grid solve (NEXT f1): M2M, L2L, leaf list, the driver.
+
+Independent references: P2M of the constituents (helpers.moments_of_points), symbolic Taylor shift (sympy), the exact
+point-mass sum, momentum and angular-momentum conservation, the analytic potential of a uniform
+sphere (Eq. 42) and the residuals the paper prints for it (Table 1)."""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from helpers import IDX2, IDX3, full2, full3, load_golden, moments_of_points
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def test_leaf_list_is_the_eq15_list_plus_the_near_field():
+    for theta, far, near in ((0.5, 231, 32), (0.35, 651, 92), (0.7, 133, 18)):
+        for par in range(8):
+            a = {tuple(v) for v in oracle.stencil(theta, par)}
+            b = {tuple(v) for v in oracle.stencil_leaf(theta, par)}
+            assert a < b and len(a) == far and len(b) == far + near
+            for d in b - a:                                   # the added cells are exactly the not-well-separated ones
+                assert 0 < sum(int(c) ** 2 for c in d) * theta * theta <= 1.0
+
+
+def test_m2m_equals_p2m_of_all_constituents():
+    """Two levels of 8-point cells: the parent moments from M2M equal the moments of all 64 points about the parent's
+    centre of mass, and the parent's offset is that centre of mass."""
+    rng = np.random.default_rng(3)
+    hc = 0.25
+    n = (4, 4, 4)
+    mom = np.zeros((20,) + n)
+    off = np.zeros((3,) + n)
+    pts = {}
+    for k, j, i in itertools.product(range(4), repeat=3):
+        centre = (np.array([i, j, k]) + 0.5) * hc
+        y = centre + rng.uniform(-0.5, 0.5, (8, 3)) * hc
+        m = rng.uniform(0.1, 1.0, 8)
+        com = (m[:, None] * y).sum(0) / m.sum()
+        mom[:, k, j, i] = moments_of_points(m, y, com)
+        off[:, k, j, i] = com - centre
+        pts[(i, j, k)] = (m, y)
+    pm, po = oracle.m2m(n, hc, mom, off)
+    for K, J, I in itertools.product(range(2), repeat=3):
+        ms = np.concatenate([pts[(2 * I + a, 2 * J + b, 2 * K + c)][0] for c in range(2) for b in range(2) for a in range(2)])
+        ys = np.concatenate([pts[(2 * I + a, 2 * J + b, 2 * K + c)][1] for c in range(2) for b in range(2) for a in range(2)])
+        com = (ms[:, None] * ys).sum(0) / ms.sum()
+        ref = moments_of_points(ms, ys, com)
+        got = pm[:, K, J, I]
+        assert np.allclose(po[:, K, J, I], com - (np.array([I, J, K]) + 0.5) * 2 * hc, rtol=0, atol=1e-15)
+        scale = np.array([ms.sum()] + [ms.sum() * hc] * 3 + [ms.sum() * hc ** 2] * 6 + [ms.sum() * hc ** 3] * 10)
+        assert (np.abs(got - ref) / scale).max() < 5e-15
+        assert np.abs(got[1:4]).max() < 1e-15 * ms.sum()      # dipole about the centre of mass vanishes
+
+
+def _taylor_shift_reference(L, e):
+    """Derivatives at e of phi(a) = sum_n L^(n) a^n / n!, by symbolic differentiation."""
+    import sympy as sp
+    a = sp.symbols("a0:3", real=True)
+    L1, L2, L3 = L[1:4], full2(L[4:10]), full3(L[10:20])
+    phi = L[0] + sum(L1[i] * a[i] for i in range(3))
+    phi += sum(L2[i, j] * a[i] * a[j] for i in range(3) for j in range(3)) / 2
+    phi += sum(L3[i, j, k] * a[i] * a[j] * a[k] for i in range(3) for j in range(3) for k in range(3)) / 6
+    at = {a[c]: e[c] for c in range(3)}
+    out = [float(phi.subs(at))]
+    out += [float(sp.diff(phi, a[i]).subs(at)) for i in range(3)]
+    out += [float(sp.diff(phi, a[i], a[j]).subs(at)) for i, j in IDX2]
+    out += [float(sp.diff(phi, a[i], a[j], a[k]).subs(at)) for i, j, k in IDX3]
+    return np.array(out)
+
+
+def test_l2l_is_the_exact_taylor_shift_and_passes_the_correction_unchanged():
+    rng = np.random.default_rng(4)
+    hc = 0.125
+    nc = (2, 2, 2)
+    pL = rng.normal(size=(20, 1, 1, 1))
+    pcorr = rng.normal(size=(3, 1, 1, 1))
+    poff = rng.uniform(-0.2, 0.2, (3, 1, 1, 1)) * hc
+    coff = rng.uniform(-0.4, 0.4, (3,) + nc) * hc
+    cL0 = rng.normal(size=(20,) + nc)
+    cc0 = rng.normal(size=(3,) + nc)
+    cL, cc = cL0.copy(), cc0.copy()
+    oracle.l2l(nc, hc, pL, pcorr, poff, coff, cL, cc)
+    for k, j, i in itertools.product(range(2), repeat=3):
+        e = (np.array([i, j, k]) - 0.5) * hc + coff[:, k, j, i] - poff[:, 0, 0, 0]
+        ref = _taylor_shift_reference(pL[:, 0, 0, 0], e)
+        assert np.allclose(cL[:, k, j, i] - cL0[:, k, j, i], ref, rtol=1e-13, atol=1e-14)
+        assert np.allclose(cc[:, k, j, i] - cc0[:, k, j, i], pcorr[:, 0, 0, 0], rtol=0, atol=1e-15)
+
+
+@pytest.fixture(scope="module")
+def random16():
+    n, h = 16, 1.0 / 16
+    mass = np.random.default_rng(1).uniform(0.5, 1.5, (n, n, n)) * h ** 3
+    return n, h, mass, oracle.direct_sum((n, n, n), h, mass)
+
+
+@pytest.mark.parametrize("theta,phi_max,phi_mean,g_max", [(0.5, 6e-4, 6e-5, 8e-3), (0.35, 2e-4, 3e-5, 2e-3),
+                                                           (0.7, 1.2e-2, 8e-4, 8e-2)])
+def test_complete_solve_against_the_exact_point_sum(random16, theta, phi_max, phi_mean, g_max):
+    """Error of the order-3 solve within the truncation error, falling with theta; theta = 0.7 also needs the 2^3-cell
+    level (siblings interact there), whose omission leaves an 11 % error."""
+    n, h, mass, ref = random16
+    out = oracle.solve(n, h, theta, mass)
+    rel = np.abs(out[0] - ref[0]) / np.abs(ref[0])
+    assert rel.max() < phi_max and rel.mean() < phi_mean
+    assert rel.mean() > phi_mean / 50                          # the tolerance is not vacuous
+    assert np.abs(out[1:] - ref[1:]).max() / np.abs(ref[1:]).max() < g_max
+
+
+def _net_force_and_torque(n, h, mass, out):
+    x = (np.arange(n) + 0.5) * h
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    F = mass[None] * out[1:]
+    T = np.cross(np.stack([X, Y, Z]), F, axis=0)
+    return (np.abs(F.sum(axis=(1, 2, 3))).max() / np.abs(F).sum(), np.abs(T.sum(axis=(1, 2, 3))).max() / np.abs(T).sum())
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.35])
+def test_complete_solve_conserves_momentum_and_with_the_correction_angular_momentum(random16, theta):
+    n, h, mass, _ = random16
+    f_on, t_on = _net_force_and_torque(n, h, mass, oracle.solve(n, h, theta, mass, True))
+    f_off, t_off = _net_force_and_torque(n, h, mass, oracle.solve(n, h, theta, mass, False))
+    assert f_on < 1e-15 and f_off < 1e-15                      # L125: linear momentum to machine precision
+    assert t_on < 5e-15                                        # L127: with the correction, angular momentum too
+    assert t_off > 1e-8                                        # ... and visibly not without it (Fig. 12)
+
+
+def _uniform_sphere(n):
+    h = 1.0 / n
+    x = (np.arange(n) + 0.5) * h - 0.5
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    r = np.sqrt(X * X + Y * Y + Z * Z)
+    R, M = 0.25, 1.0
+    rho = np.where(r < R, 1.0, 1e-10)                          # cell-centre sampling, ambient 1e-10 (L452)
+    mass = rho * (M / rho.sum())                               # total mass 1
+    phi = np.where(r < R, -M * (3 * R * R - r * r) / (2 * R ** 3), -M / r)
+    return h, mass, phi, r
+
+
+GOLD = load_golden(os.path.join(HERE, "golden", "table1_sphere.txt"))
+
+
+@pytest.mark.parametrize("ncell,theta", [(64, 0.5), (64, 0.35)])
+def test_uniform_sphere_residuals_are_of_the_order_the_paper_prints(ncell, theta):
+    """Section 3.4 / Table 1.  Rasterisation and self-term are not specified in the paper, so: same order of
+    magnitude (within a factor 3 of the printed max and mean of the nearest printed row), the maximum sits outside
+    the sphere near the corners of the enclosing square and lowering theta lowers max and mean (L456, L508)."""
+    rows = {(int(r[0]), float(r[1])): (float(r[2]), float(r[3])) for r in GOLD["_multi"]["sphere"]}
+    pmax, pmean = rows[(64, 0.5)] if theta == 0.5 else rows[(128, 0.35)]
+    h, mass, phi, r = _uniform_sphere(ncell)
+    out = oracle.solve(ncell, h, theta, mass)
+    eps = np.abs(out[0] - phi) / np.abs(phi)
+    assert pmax / 3 < eps.max() < pmax * 3
+    assert pmean / 3 < eps.mean() < pmean * 3.5
+    k = np.unravel_index(np.argmax(eps), eps.shape)
+    assert r[k] > 0.25                                         # outside the sphere (L456, Fig. 4)
+    if theta == 0.35:
+        out5 = oracle.solve(ncell, h, 0.5, mass)
+        eps5 = np.abs(out5[0] - phi) / np.abs(phi)
+        assert eps.max() < 0.6 * eps5.max() and eps.mean() < 0.8 * eps5.mean()
