@@ -148,6 +148,44 @@ int octo_fmm_flops_per_interaction(int kind, int am_correction, int *flops, int 
 
 const char *octo_fmm_version(void);
 
+/* ---- complete uniform-grid solve ------------------------------------
+ * "The multipoles of each cell are composed of the multipoles of its child cells ... The expansion of
+ * each cell is composed of the expansion due to its interactions with other cells at the same level, and
+ * the expansion of its parent cell".  On an isolated (L321) cubic grid of n^3 leaf cells,
+ * n a power of two >= 16: the leaves are point masses at their cell centres; parent multipoles (order 3,
+ * about the centre of mass) come from their children (M2M) up to the level of 2^3 cells; every multipole
+ * level runs the interaction step above (Eq. 15 list, correction optional) and receives its parent's
+ * expansion (L2L); a leaf gets its parent's expansion evaluated at its centre plus the monopole sum over
+ * every other leaf whose parent is not well separated from its own (Eq. 15 list + near field).
+ * out = [4][n][n][n] = (phi, g_x, g_y, g_z), g = -(grad phi + correction); a cell's own mass contributes
+ * nothing.  Same ownership rules as above: the caller lends the workspace, everything is enqueued on
+ * cfg.stream, nothing is allocated.  Formulas: DESIGN.md section 12. */
+typedef struct octo_fmm_solver octo_fmm_solver_t;
+typedef struct {
+    int n;                  /* leaf cells per axis, a power of two, 16 <= n <= 2048                     */
+    double h;               /* leaf cell width                                                          */
+    double theta;           /* opening angle, 1/3 < theta < 1                                           */
+    int am_correction;      /* 0/1: angular-momentum correction at the multipole levels (L127)          */
+    int device;             /* CUDA device ordinal                                                      */
+    void *stream;           /* cudaStream_t, borrowed                                                   */
+    void *workspace;        /* device memory, 256-byte aligned, borrowed for the handle's lifetime      */
+    size_t workspace_bytes; /* >= octo_fmm_solver_workspace_bytes(cfg)                                  */
+} octo_fmm_solver_config;
+
+size_t octo_fmm_solver_workspace_bytes(const octo_fmm_solver_config *cfg);   /* 0 on invalid configuration */
+int octo_fmm_solver_create(const octo_fmm_solver_config *cfg, octo_fmm_solver_t **out);
+/* mass: device, [n][n][n] (x fastest); out: device, [4][n][n][n].  Asynchronous on the stream. */
+int octo_fmm_solver_solve(octo_fmm_solver_t *s, const double *mass, double *out);
+/* Synchronises the stream; OCTO_FMM_EMASS if the correction met a cell of mass <= 0 at some level. */
+int octo_fmm_solver_status(octo_fmm_solver_t *s);
+int octo_fmm_solver_destroy(octo_fmm_solver_t *s);
+/* Ordered in-domain pairs one solve evaluates, all levels. */
+int octo_fmm_solver_interaction_count(const octo_fmm_solver_t *s, unsigned long long *n);
+/* The leaf-level list (Eq. 15 list + near field) of a parity class, as octo_fmm_get_stencil. */
+int octo_fmm_solver_get_leaf_stencil(const octo_fmm_solver_t *s, int parity, int *count, signed char (*dxyz)[3]);
+/* Number of multipole levels (n/2 ... 2) and of kernels one solve launches. */
+int octo_fmm_solver_num_levels(const octo_fmm_solver_t *s, int *multipole_levels, int *launches_per_solve);
+
 #ifdef __cplusplus
 }
 #endif

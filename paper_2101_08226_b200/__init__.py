@@ -34,6 +34,12 @@ class octo_fmm_config(ctypes.Structure):
                 ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
 
 
+class octo_fmm_solver_config(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int), ("h", ctypes.c_double), ("theta", ctypes.c_double), ("am_correction", ctypes.c_int),
+                ("device", ctypes.c_int), ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p),
+                ("workspace_bytes", ctypes.c_size_t)]
+
+
 class _Library:
     """Loads libocto_fmm.so on first use and fails loudly when it is missing (no CPU fallback).
 
@@ -69,6 +75,16 @@ class _Library:
         lib.octo_fmm_fp64_issue_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, ctypes.c_int, dp]
         lib.octo_fmm_flops_per_interaction.argtypes = [ctypes.c_int, ctypes.c_int, ip, ip]
         lib.octo_fmm_version.restype = ctypes.c_char_p
+        scfgp = ctypes.POINTER(octo_fmm_solver_config)
+        lib.octo_fmm_solver_workspace_bytes.restype = ctypes.c_size_t
+        lib.octo_fmm_solver_workspace_bytes.argtypes = [scfgp]
+        lib.octo_fmm_solver_create.argtypes = [scfgp, ctypes.POINTER(vp)]
+        lib.octo_fmm_solver_solve.argtypes = [vp, vp, vp]
+        lib.octo_fmm_solver_status.argtypes = [vp]
+        lib.octo_fmm_solver_destroy.argtypes = [vp]
+        lib.octo_fmm_solver_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
+        lib.octo_fmm_solver_get_leaf_stencil.argtypes = [vp, ctypes.c_int, ip, vp]
+        lib.octo_fmm_solver_num_levels.argtypes = [vp, ip, ip]
         self._cdll = lib
 
     def __getattr__(self, name):
@@ -220,6 +236,121 @@ def octo_fmm_flops_per_interaction(kind, am_correction):
     if rc != OK:
         raise OctoFmmError("octo_fmm_flops_per_interaction", rc)
     return f.value, i.value
+
+
+# ---- complete uniform-grid solve (octo_fmm_solver_*) ------------------------------------------
+def make_solver_config(n, h, theta, am_correction=True, device=0, stream=0, workspace=0, workspace_bytes=0):
+    c = octo_fmm_solver_config()
+    c.n, c.h, c.theta, c.am_correction = int(n), float(h), float(theta), int(bool(am_correction))
+    c.device, c.stream, c.workspace, c.workspace_bytes = int(device), stream or None, workspace or None, int(workspace_bytes)
+    return c
+
+
+def octo_fmm_solver_workspace_bytes(cfg):
+    return int(_lib.octo_fmm_solver_workspace_bytes(ctypes.byref(cfg)))
+
+
+def octo_fmm_solver_create(cfg):
+    h = _vp()
+    rc = _lib.octo_fmm_solver_create(ctypes.byref(cfg), ctypes.byref(h))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_create", rc)
+    return h
+
+
+def octo_fmm_solver_solve(s, mass, out):
+    rc = _lib.octo_fmm_solver_solve(s, _ptr(mass), _ptr(out))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_solve", rc)
+
+
+def octo_fmm_solver_status(s):
+    return int(_lib.octo_fmm_solver_status(s))
+
+
+def octo_fmm_solver_destroy(s):
+    rc = _lib.octo_fmm_solver_destroy(s)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_destroy", rc)
+
+
+def octo_fmm_solver_interaction_count(s):
+    n = ctypes.c_ulonglong(0)
+    rc = _lib.octo_fmm_solver_interaction_count(s, ctypes.byref(n))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_interaction_count", rc)
+    return int(n.value)
+
+
+def octo_fmm_solver_get_leaf_stencil(s, parity):
+    import numpy as np
+    cnt = ctypes.c_int(0)
+    rc = _lib.octo_fmm_solver_get_leaf_stencil(s, int(parity), ctypes.byref(cnt), None)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_get_leaf_stencil", rc)
+    out = np.zeros((cnt.value, 3), dtype=np.int8)
+    rc = _lib.octo_fmm_solver_get_leaf_stencil(s, int(parity), ctypes.byref(cnt), out.ctypes.data)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_get_leaf_stencil", rc)
+    return out
+
+
+def octo_fmm_solver_num_levels(s):
+    a, b = ctypes.c_int(0), ctypes.c_int(0)
+    rc = _lib.octo_fmm_solver_num_levels(s, ctypes.byref(a), ctypes.byref(b))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_num_levels", rc)
+    return a.value, b.value
+
+
+class OctoFMMSolver:
+    """Owns the workspace tensor and the handle of a complete uniform-grid solve."""
+
+    def __init__(self, n, h, theta, am_correction=True, device=0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("octo_fmm needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.torch = torch
+        self.n = int(n)
+        self.device = torch.device("cuda", device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        cfg = make_solver_config(n, h, theta, am_correction, device=device, stream=self.stream.cuda_stream)
+        nbytes = octo_fmm_solver_workspace_bytes(cfg)
+        if nbytes == 0:
+            raise OctoFmmError("octo_fmm_solver_workspace_bytes", EINVAL)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        cfg.workspace, cfg.workspace_bytes = self.workspace.data_ptr(), nbytes
+        self.cfg = cfg
+        self.handle = octo_fmm_solver_create(cfg)
+
+    def solve(self, mass, out=None):
+        if out is None:
+            out = self.torch.empty((4, self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
+        octo_fmm_solver_solve(self.handle, mass, out)
+        return out
+
+    def status(self):
+        return octo_fmm_solver_status(self.handle)
+
+    def interaction_count(self):
+        return octo_fmm_solver_interaction_count(self.handle)
+
+    def leaf_stencil(self, parity):
+        return octo_fmm_solver_get_leaf_stencil(self.handle, parity)
+
+    def num_levels(self):
+        return octo_fmm_solver_num_levels(self.handle)
+
+    def close(self):
+        if getattr(self, "handle", None) is not None:
+            octo_fmm_solver_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 # ---- convenience wrapper ---------------------------------------------------------------------

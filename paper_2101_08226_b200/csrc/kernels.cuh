@@ -26,7 +26,7 @@
 namespace octo {
 
 constexpr int REACH_MAX = 5;            // theta_min = 0.34 for 8^3 sub-grids
-constexpr int MAX_LIST = 651;           // |S_p| for 1/3 < theta (7 * 93)
+constexpr int MAX_LIST = 744;           // |S_p| <= 651 for 1/3 < theta (7 * 93); + 92 near-field cells in the leaf list
 constexpr int TILE_X = 16;              // target brick of one CTA pass: 16 x 8 x 3 cells = 12 warps
 constexpr int TILE_Y = 8;
 constexpr int TILE_Z = 3;

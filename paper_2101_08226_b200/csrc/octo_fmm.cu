@@ -15,6 +15,7 @@
 
 #include "../../include/octo_fmm.h"
 #include "kernels.cuh"
+#include "solver.cuh"
 
 using namespace octo;
 
@@ -31,7 +32,9 @@ inline bool well_separated(long long d2, double theta) { return (double)d2 * the
 inline int floor_div2(int v) { return v >> 1; }   // arithmetic shift: floor for negatives too
 
 // partner list of parity class (px,py,pz): cells well separated, parents not (L135)
-std::vector<Offset3> build_list(int px, int py, int pz, double theta, int* reach_out)
+// leaf: the leaf-level list of the complete solve -- every Delta != 0 whose parents are not well separated
+// (the Eq. 15 list plus the near field)
+std::vector<Offset3> build_list(int px, int py, int pz, double theta, int* reach_out, bool leaf = false)
 {
     std::vector<Offset3> out;
     const int S = 2 * (int)std::floor(1.0 / theta) + 3;
@@ -40,7 +43,7 @@ std::vector<Offset3> build_list(int px, int py, int pz, double theta, int* reach
         for (int dy = -S; dy <= S; ++dy)
             for (int dx = -S; dx <= S; ++dx) {
                 const long long c2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
-                if (c2 == 0 || !well_separated(c2, theta)) continue;
+                if (c2 == 0 || (!leaf && !well_separated(c2, theta))) continue;
                 const int Ix = floor_div2(px + dx), Iy = floor_div2(py + dy), Iz = floor_div2(pz + dz);
                 const long long p2 = (long long)Ix * Ix + (long long)Iy * Iy + (long long)Iz * Iz;
                 if (p2 != 0 && well_separated(p2, theta)) continue;
@@ -54,25 +57,30 @@ std::vector<Offset3> build_list(int px, int py, int pz, double theta, int* reach
     return out;
 }
 
-bool region_of(const octo_fmm_config& c, int lo[3], int hi[3])
+// creation flags of internal handles (the levels of the complete solve)
+constexpr int CF_ANY_SIZE = 1;    // any even grid size >= 2 (whole-grid output); sizes that are not multiples of 8 use the direct kernel
+constexpr int CF_LEAF_LIST = 2;   // monopole kind with the leaf-level list (Eq. 15 list + near field)
+
+bool region_of(const octo_fmm_config& c, int lo[3], int hi[3], int flags = 0)
 {
     bool whole = true;
     for (int a = 0; a < 3; ++a) whole = whole && c.out_lo[a] == 0 && c.out_hi[a] == 0;
     for (int a = 0; a < 3; ++a) {
         lo[a] = whole ? 0 : c.out_lo[a];
         hi[a] = whole ? c.n[a] : c.out_hi[a];
-        if (lo[a] < 0 || hi[a] > c.n[a] || lo[a] >= hi[a] || lo[a] % 8 || hi[a] % 8) return false;
+        if (lo[a] < 0 || hi[a] > c.n[a] || lo[a] >= hi[a]) return false;
+        if (!(flags & CF_ANY_SIZE) && (lo[a] % 8 || hi[a] % 8)) return false;
     }
     return true;
 }
 
-bool config_ok(const octo_fmm_config* c)
+bool config_ok(const octo_fmm_config* c, int flags = 0)
 {
     if (!c) return false;
     for (int a = 0; a < 3; ++a)
-        if (c->n[a] <= 0 || c->n[a] % 8 || c->n[a] > 4096) return false;
+        if (c->n[a] <= 0 || c->n[a] % ((flags & CF_ANY_SIZE) ? 2 : 8) || c->n[a] > 4096) return false;
     int lo[3], hi[3];
-    if (!region_of(*c, lo, hi)) return false;
+    if (!region_of(*c, lo, hi, flags)) return false;
     if (!(c->h > 0.0) || !std::isfinite(c->h)) return false;
     if (!(c->theta > 1.0 / 3.0 && c->theta < 1.0)) return false;   // reach <= 5 (theta_min, L137)
     if (c->kind != OCTO_FMM_MULTIPOLE && c->kind != OCTO_FMM_MONOPOLE) return false;
@@ -81,10 +89,10 @@ bool config_ok(const octo_fmm_config* c)
 
 struct Sizes { size_t src, L, C, flags, total; };
 
-Sizes sizes_of(const octo_fmm_config& c)
+Sizes sizes_of(const octo_fmm_config& c, int flags = 0)
 {
     int lo[3], hi[3];
-    region_of(c, lo, hi);
+    region_of(c, lo, hi, flags);
     const size_t ncell = (size_t)c.n[0] * c.n[1] * c.n[2];
     const size_t ocell = (size_t)(hi[0] - lo[0]) * (hi[1] - lo[1]) * (hi[2] - lo[2]);
     Sizes s{};
@@ -177,12 +185,12 @@ size_t octo_fmm_host_scratch_bytes(const octo_fmm_config* cfg)
     return align_up(ncell * 8) + align_up(ocell * 4 * 8);
 }
 
-int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
+static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** out)
 {
     if (!out) return OCTO_FMM_EINVAL;
     *out = nullptr;
-    if (!config_ok(cfg)) return OCTO_FMM_EINVAL;
-    const Sizes sz = sizes_of(*cfg);
+    if (!config_ok(cfg, flags)) return OCTO_FMM_EINVAL;
+    const Sizes sz = sizes_of(*cfg, flags);
     if (!cfg->workspace || cfg->workspace_bytes < sz.total || ((uintptr_t)cfg->workspace % ALIGN)) return OCTO_FMM_EINVAL;
 
     int ndev = 0;
@@ -202,11 +210,14 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     h->host_chunk = 24;
     h->host_launches = 0;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
-    region_of(*cfg, h->lo, h->hi);
+    region_of(*cfg, h->lo, h->hi, flags);
+    const bool small = cfg->n[0] % 8 || cfg->n[1] % 8 || cfg->n[2] % 8;    // only with CF_ANY_SIZE
+    if (small) h->kernel = 1;
 
     // ---- a1: interaction lists (Eq. 15) ----
     h->reach = 0;
-    for (int p = 0; p < 8; ++p) h->list[p] = build_list(p & 1, (p >> 1) & 1, (p >> 2) & 1, cfg->theta, &h->reach);
+    for (int p = 0; p < 8; ++p)
+        h->list[p] = build_list(p & 1, (p >> 1) & 1, (p >> 2) & 1, cfg->theta, &h->reach, (flags & CF_LEAF_LIST) != 0);
     if (h->reach > REACH_MAX) { delete h; return OCTO_FMM_EINVAL; }
     for (int p = 0; p < 8; ++p)
         if ((int)h->list[p].size() > MAX_LIST) { delete h; return OCTO_FMM_EINVAL; }
@@ -276,7 +287,7 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     h->outL = h->L; h->outC = h->C;
     P.S = h->src; P.L = h->L; P.C = h->C; P.flags = h->flags;
 
-    if (cfg->kind == OCTO_FMM_MULTIPOLE) {
+    if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
         // ---- TMA descriptor of S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
         //      {2 (pair), nx/2 (xh), 2 ny (y*2 + xpar), 10 (cp), nz}
         EncodeTiledFn enc = encode_tiled_fn();
@@ -294,7 +305,7 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
         cudaError_t e1 = cudaFuncSetAttribute(m2l_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         if (e1 != cudaSuccess || e2 != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
-    } else {
+    } else if (cfg->kind == OCTO_FMM_MONOPOLE) {
         // ---- monopole radial table: -1/r and -1/r^3 by d2 = |Delta|^2, r = sqrt(d2) h (FP64 sqrt and division on
         //      the host); the kernel forms -R/r^3 = ((i_A - i_B) h) * (-1/r^3) per list entry ----
         for (int d2 = 0; d2 <= 3 * REACH_MAX * REACH_MAX; ++d2) {
@@ -308,6 +319,8 @@ int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out)
     *out = h;
     return OCTO_FMM_OK;
 }
+
+int octo_fmm_create(const octo_fmm_config* cfg, octo_fmm_t** out) { return create_internal(cfg, 0, out); }
 
 int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com_off)
 {
@@ -582,6 +595,7 @@ int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
     if (!h || !key) return OCTO_FMM_EINVAL;
     if (!std::strcmp(key, "kernel")) {
         if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
+        if (value == 0 && (h->cfg.n[0] % 8 || h->cfg.n[1] % 8 || h->cfg.n[2] % 8)) return OCTO_FMM_EINVAL;
         h->kernel = value;
         return OCTO_FMM_OK;
     }
@@ -694,3 +708,5 @@ int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int*
 }
 
 }  // extern "C"
+
+#include "solver.inl"

@@ -1,0 +1,219 @@
+// solver.cuh -- the other passes of a complete uniform-grid solve, sm_100a.
+//
+// "The multipoles of each cell are composed of the multipoles of its child cells ... The expansion of each
+// cell is composed of the expansion due to its interactions with other cells at the same level, and the
+// expansion of its parent cell".  The same-level interactions are the hot path
+// (kernels.cuh); here are the upward pass (M2M), the downward pass (L2L) and the leaf evaluation.
+// All three are HBM-bound, one thread per cell, SoA arrays [comp][z][y][x], positions kept relative
+// to the parent's geometric centre.  Formulas: DESIGN.md section 12.
+#pragma once
+
+#include <cuda_runtime.h>
+
+namespace octo {
+
+// unique-component index of a symmetric rank-2 / rank-3 tensor, lexicographic order
+__host__ __device__ constexpr int u2(int i, int j)
+{
+    return i > j ? u2(j, i) : (i == 0 ? j : (i == 1 ? 2 + j : 5));
+}
+__host__ __device__ constexpr int u3s(int i, int j, int k)   // i <= j <= k
+{
+    return i == 0 ? (j == 0 ? k : (j == 1 ? 2 + k : 5)) : (i == 1 ? (j == 1 ? 5 + k : 8) : 9);
+}
+__host__ __device__ constexpr int u3(int i, int j, int k)
+{
+    return i > j ? u3(j, i, k) : (j > k ? u3(i, k, j) : u3s(i, j, k));
+}
+static_assert(u2(0, 0) == 0 && u2(1, 0) == 1 && u2(0, 2) == 2 && u2(1, 1) == 3 && u2(2, 1) == 4 && u2(2, 2) == 5, "u2");
+static_assert(u3(0, 0, 0) == 0 && u3(0, 1, 0) == 1 && u3(2, 0, 0) == 2 && u3(1, 0, 1) == 3 && u3(2, 1, 0) == 4 &&
+              u3(0, 2, 2) == 5 && u3(1, 1, 1) == 6 && u3(1, 2, 1) == 7 && u3(2, 1, 2) == 8 && u3(2, 2, 2) == 9, "u3");
+
+// ------------------------------------------------------------------------------------------
+// M2M: parent multipoles (order 3, raw moments about the parent's centre of mass) from its 8
+// children.  LEAF: the children are point masses at their cell centres (cm = mass [nz][ny][nx],
+// coff unused); otherwise cm = [20][child grid], coff = [3][child grid].
+//   rel_c = ((a,b,c) - 1/2) hc + delta_c;   delta_P = sum_c (M_c rel_c + M1_c) / sum_c M_c  (0 if the mass is 0)
+//   d = rel_c - delta_P;  M1' = M1 + M d;  M2'_ij = M2_ij + M1_i d_j + M1_j d_i + M d_i d_j;
+//   M3'_ijk = M3_ijk + (M2_ij d_k + M2_ik d_j + M2_jk d_i) + (M1_i d_j d_k + M1_j d_i d_k + M1_k d_i d_j) + M d_i d_j d_k
+// ------------------------------------------------------------------------------------------
+template <bool LEAF>
+__global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm, const double* __restrict__ coff,
+                                                  double* __restrict__ pm, double* __restrict__ poff, int pnx, int pny, int pnz,
+                                                  double hc)
+{
+    const long long pcell = (long long)pnx * pny * pnz, ccell = 8 * pcell;
+    const long long P = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (P >= pcell) return;
+    const int I = (int)(P % pnx), J = (int)((P / pnx) % pny), K = (int)(P / ((long long)pnx * pny));
+    const int cnx = 2 * pnx, cny = 2 * pny;
+    long long cell[8];
+    double rel[8][3];
+    double mass = 0.0, com[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        const int a[3] = {c & 1, (c >> 1) & 1, (c >> 2) & 1};
+        cell[c] = ((long long)(2 * K + a[2]) * cny + (2 * J + a[1])) * cnx + (2 * I + a[0]);
+        const double m0 = cm[cell[c]];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            rel[c][i] = ((double)a[i] - 0.5) * hc + (LEAF ? 0.0 : coff[i * ccell + cell[c]]);
+            com[i] += m0 * rel[c][i] + (LEAF ? 0.0 : cm[(1 + i) * ccell + cell[c]]);
+        }
+        mass += m0;
+    }
+    double dP[3] = {0.0, 0.0, 0.0};
+    if (mass != 0.0) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) dP[i] = com[i] / mass;
+    }
+    double S[20];
+#pragma unroll
+    for (int t = 0; t < 20; ++t) S[t] = 0.0;
+    S[0] = mass;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        double M[20];
+        M[0] = cm[cell[c]];
+#pragma unroll
+        for (int t = 1; t < 20; ++t) M[t] = LEAF ? 0.0 : cm[t * ccell + cell[c]];
+        double d[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) d[i] = rel[c][i] - dP[i];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) S[1 + i] += M[1 + i] + M[0] * d[i];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = i; j < 3; ++j)
+                S[4 + u2(i, j)] += M[4 + u2(i, j)] + M[1 + i] * d[j] + M[1 + j] * d[i] + M[0] * d[i] * d[j];
+#pragma unroll
+        for (int i = 0; i < 3; ++i)
+#pragma unroll
+            for (int j = i; j < 3; ++j)
+#pragma unroll
+                for (int k = j; k < 3; ++k)
+                    S[10 + u3(i, j, k)] += M[10 + u3(i, j, k)] + M[4 + u2(i, j)] * d[k] + M[4 + u2(i, k)] * d[j] +
+                                           M[4 + u2(j, k)] * d[i] + M[1 + i] * d[j] * d[k] + M[1 + j] * d[i] * d[k] +
+                                           M[1 + k] * d[i] * d[j] + M[0] * d[i] * d[j] * d[k];
+    }
+#pragma unroll
+    for (int t = 0; t < 20; ++t) pm[t * pcell + P] = S[t];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) poff[i * pcell + P] = dP[i];
+}
+
+// Taylor shift of a parent expansion pL (20 unique components in registers) by e, orders 0..NORD
+//   out0 = L0 + L1_i e_i + 1/2 L2_ij e_i e_j + 1/6 L3_ijk e_i e_j e_k
+//   out1_i = L1_i + L2_ij e_j + 1/2 L3_ijk e_j e_k;  out2_ij = L2_ij + L3_ijk e_k;  out3 = L3
+template <int NORD>
+__device__ __forceinline__ void taylor_shift(const double (&L)[20], const double (&e)[3], double (&out)[20])
+{
+    double s0 = L[0];
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+        s0 += L[1 + x] * e[x];
+#pragma unroll
+        for (int y = 0; y < 3; ++y) {
+            s0 += 0.5 * L[4 + u2(x, y)] * e[x] * e[y];
+#pragma unroll
+            for (int z = 0; z < 3; ++z) s0 += L[10 + u3(x, y, z)] * e[x] * e[y] * e[z] / 6.0;
+        }
+    }
+    out[0] = s0;
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+        double s1 = L[1 + x];
+#pragma unroll
+        for (int y = 0; y < 3; ++y) {
+            s1 += L[4 + u2(x, y)] * e[y];
+#pragma unroll
+            for (int z = 0; z < 3; ++z) s1 += 0.5 * L[10 + u3(x, y, z)] * e[y] * e[z];
+        }
+        out[1 + x] = s1;
+    }
+    if (NORD >= 2) {
+#pragma unroll
+        for (int x = 0; x < 3; ++x)
+#pragma unroll
+            for (int y = x; y < 3; ++y) {
+                double s2 = L[4 + u2(x, y)];
+#pragma unroll
+                for (int z = 0; z < 3; ++z) s2 += L[10 + u3(x, y, z)] * e[z];
+                out[4 + u2(x, y)] = s2;
+            }
+#pragma unroll
+        for (int t = 10; t < 20; ++t) out[t] = L[t];
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// L2L: cL = (cL with the correction taken out of L1) + parent expansion shifted to the child's
+// centre; cC += parent correction (a uniform acceleration, handed down unchanged).
+// HAS_PARENT = false (coarsest level): only the un-folding  L1 -= C.
+//   e = ((a,b,c) - 1/2) hc + delta_c - delta_P
+// ------------------------------------------------------------------------------------------
+template <bool HAS_PARENT>
+__global__ void __launch_bounds__(128) l2l_kernel(double* __restrict__ cL, double* __restrict__ cC, const double* __restrict__ coff,
+                                                  const double* __restrict__ pL, const double* __restrict__ pC,
+                                                  const double* __restrict__ poff, int cnx, int cny, int cnz, double hc)
+{
+    const long long ccell = (long long)cnx * cny * cnz;
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= ccell) return;
+    double C[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) C[i] = cC[i * ccell + cell];
+    if (!HAS_PARENT) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) cL[(1 + i) * ccell + cell] -= C[i];
+        return;
+    }
+    const int i = (int)(cell % cnx), j = (int)((cell / cnx) % cny), k = (int)(cell / ((long long)cnx * cny));
+    const int pnx = cnx / 2, pny = cny / 2;
+    const long long pcell = ccell / 8;
+    const long long P = ((long long)(k / 2) * pny + (j / 2)) * pnx + (i / 2);
+    const int a[3] = {i & 1, j & 1, k & 1};
+    double e[3], L[20], sh[20];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) e[c] = ((double)a[c] - 0.5) * hc + coff[c * ccell + cell] - poff[c * pcell + P];
+#pragma unroll
+    for (int t = 0; t < 20; ++t) L[t] = pL[t * pcell + P];
+    taylor_shift<3>(L, e, sh);
+#pragma unroll
+    for (int t = 0; t < 20; ++t) {
+        double v = cL[t * ccell + cell];
+        if (t >= 1 && t <= 3) v -= C[t - 1];
+        cL[t * ccell + cell] = v + sh[t];
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) cC[c * ccell + cell] = C[c] + pC[c * pcell + P];
+}
+
+// ------------------------------------------------------------------------------------------
+// Leaf evaluation: out = (phi, g) of the leaf-level monopole sum; add the parent's expansion
+// evaluated at the leaf's cell centre:  phi += L0(e),  g -= L1(e) + correction,  e = ((a,b,c) - 1/2) h - delta_P.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) leaf_eval_kernel(double* __restrict__ out, const double* __restrict__ pL,
+                                                        const double* __restrict__ pC, const double* __restrict__ poff, int nx,
+                                                        int ny, int nz, double h)
+{
+    const long long ncell = (long long)nx * ny * nz;
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= ncell) return;
+    const int i = (int)(cell % nx), j = (int)((cell / nx) % ny), k = (int)(cell / ((long long)nx * ny));
+    const long long pcell = ncell / 8;
+    const long long P = ((long long)(k / 2) * (ny / 2) + (j / 2)) * (nx / 2) + (i / 2);
+    const int a[3] = {i & 1, j & 1, k & 1};
+    double e[3], L[20], sh[20];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) e[c] = ((double)a[c] - 0.5) * h - poff[c * pcell + P];
+#pragma unroll
+    for (int t = 0; t < 20; ++t) L[t] = pL[t * pcell + P];
+    taylor_shift<1>(L, e, sh);
+    out[cell] += sh[0];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) out[(1 + c) * ncell + cell] -= sh[1 + c] + pC[c * pcell + P];
+}
+
+}  // namespace octo

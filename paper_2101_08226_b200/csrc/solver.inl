@@ -1,0 +1,207 @@
+// solver.inl -- host logic and C ABI of the complete uniform-grid solve (octo_fmm_solver_*), included by
+// octo_fmm.cu (it drives the per-level octo_fmm handles through their internals).
+//
+// Levels: the leaves (n^3 point masses, monopole kind with the leaf-level list = Eq. 15 list + near field) and
+// the multipole levels n/2, n/4, ..., 2 (the 2^3-cell level is the coarsest that can hold interacting cells:
+// siblings interact there when 3 theta^2 > 1).  Levels whose size is not a multiple of 8 (4^3, 2^3) run the
+// direct interaction kernel.  solve() = stage leaves -> M2M up -> per level, coarsest first: stage, interact,
+// L2L -> leaf interaction + leaf evaluation.
+
+namespace {
+
+struct SolverLevel {
+    int n;                // cells per axis
+    double h;
+    octo_fmm* fmm;        // multipole handle of this level
+    double* raw;          // [20][n^3] raw moments (M2M output, set_moments input)
+    double* off;          // [3][n^3] centre-of-mass offsets
+    size_t ws_bytes;      // handle workspace
+};
+
+octo_fmm_config level_config(const octo_fmm_solver_config& sc, int n, double h, int kind)
+{
+    octo_fmm_config c;
+    std::memset(&c, 0, sizeof c);
+    for (int a = 0; a < 3; ++a) c.n[a] = n;
+    c.h = h;
+    c.theta = sc.theta;
+    c.kind = kind;
+    c.am_correction = sc.am_correction;
+    c.device = sc.device;
+    c.stream = sc.stream;
+    return c;
+}
+
+bool solver_config_ok(const octo_fmm_solver_config* c)
+{
+    if (!c) return false;
+    if (c->n < 16 || c->n > 2048 || (c->n & (c->n - 1))) return false;        // a power of two >= 16
+    if (!(c->h > 0.0) || !std::isfinite(c->h)) return false;
+    if (!(c->theta > 1.0 / 3.0 && c->theta < 1.0)) return false;
+    return true;
+}
+
+}  // namespace
+
+struct octo_fmm_solver {
+    octo_fmm_solver_config cfg;
+    octo_fmm* leaf;
+    std::vector<SolverLevel> lev;     // lev[0] = n/2, ..., lev.back() = 2
+    cudaStream_t stream;
+    unsigned long long n_interactions;
+};
+
+extern "C" {
+
+size_t octo_fmm_solver_workspace_bytes(const octo_fmm_solver_config* cfg)
+{
+    if (!solver_config_ok(cfg)) return 0;
+    octo_fmm_config lc = level_config(*cfg, cfg->n, cfg->h, OCTO_FMM_MONOPOLE);
+    size_t total = sizes_of(lc, CF_LEAF_LIST).total;
+    double h = cfg->h;
+    for (int n = cfg->n / 2; n >= 2; n /= 2) {
+        h *= 2.0;
+        octo_fmm_config mc = level_config(*cfg, n, h, OCTO_FMM_MULTIPOLE);
+        const size_t nc = (size_t)n * n * n;
+        total += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
+    }
+    return total;
+}
+
+int octo_fmm_solver_destroy(octo_fmm_solver_t* s)
+{
+    if (!s) return OCTO_FMM_EINVAL;
+    int rc = OCTO_FMM_OK;
+    if (s->leaf && octo_fmm_destroy(s->leaf) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+    for (SolverLevel& l : s->lev)
+        if (l.fmm && octo_fmm_destroy(l.fmm) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+    delete s;
+    return rc;
+}
+
+int octo_fmm_solver_create(const octo_fmm_solver_config* cfg, octo_fmm_solver_t** out)
+{
+    if (!out) return OCTO_FMM_EINVAL;
+    *out = nullptr;
+    if (!solver_config_ok(cfg)) return OCTO_FMM_EINVAL;
+    const size_t need = octo_fmm_solver_workspace_bytes(cfg);
+    if (!cfg->workspace || cfg->workspace_bytes < need || ((uintptr_t)cfg->workspace % ALIGN)) return OCTO_FMM_EINVAL;
+    octo_fmm_solver* s = new (std::nothrow) octo_fmm_solver();
+    if (!s) return OCTO_FMM_ENOMEM;
+    s->cfg = *cfg;
+    s->leaf = nullptr;
+    s->stream = (cudaStream_t)cfg->stream;
+    s->n_interactions = 0;
+    char* w = (char*)cfg->workspace;
+    {
+        octo_fmm_config lc = level_config(*cfg, cfg->n, cfg->h, OCTO_FMM_MONOPOLE);
+        lc.workspace = w;
+        lc.workspace_bytes = sizes_of(lc, CF_LEAF_LIST).total;
+        w += lc.workspace_bytes;
+        const int rc = create_internal(&lc, CF_LEAF_LIST, &s->leaf);
+        if (rc != OCTO_FMM_OK) { octo_fmm_solver_destroy(s); return rc; }
+        s->n_interactions += s->leaf->n_interactions;
+    }
+    double h = cfg->h;
+    for (int n = cfg->n / 2; n >= 2; n /= 2) {
+        h *= 2.0;
+        SolverLevel l;
+        l.n = n; l.h = h; l.fmm = nullptr;
+        octo_fmm_config mc = level_config(*cfg, n, h, OCTO_FMM_MULTIPOLE);
+        const size_t nc = (size_t)n * n * n;
+        l.ws_bytes = sizes_of(mc, CF_ANY_SIZE).total;
+        mc.workspace = w; mc.workspace_bytes = l.ws_bytes; w += l.ws_bytes;
+        l.raw = (double*)w; w += align_up(nc * 20 * 8);
+        l.off = (double*)w; w += align_up(nc * 3 * 8);
+        const int rc = create_internal(&mc, CF_ANY_SIZE, &l.fmm);
+        s->lev.push_back(l);
+        if (rc != OCTO_FMM_OK) { octo_fmm_solver_destroy(s); return rc; }
+        s->n_interactions += l.fmm->n_interactions;
+    }
+    *out = s;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
+{
+    if (!s || !mass || !out) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(s->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaStream_t st = s->stream;
+    int rc;
+    // ---- leaves: stage the masses; upward pass ----
+    if ((rc = octo_fmm_set_moments(s->leaf, mass, nullptr)) != OCTO_FMM_OK) return rc;
+    for (size_t lv = 0; lv < s->lev.size(); ++lv) {
+        SolverLevel& l = s->lev[lv];
+        const long long nc = (long long)l.n * l.n * l.n;
+        const unsigned blocks = (unsigned)((nc + 127) / 128);
+        if (lv == 0) m2m_kernel<true><<<blocks, 128, 0, st>>>(mass, nullptr, l.raw, l.off, l.n, l.n, l.n, s->cfg.h);
+        else         m2m_kernel<false><<<blocks, 128, 0, st>>>(s->lev[lv - 1].raw, s->lev[lv - 1].off, l.raw, l.off, l.n, l.n, l.n,
+                                                              s->lev[lv - 1].h);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    // ---- downward pass over the multipole levels, coarsest first ----
+    for (int lv = (int)s->lev.size() - 1; lv >= 0; --lv) {
+        SolverLevel& l = s->lev[lv];
+        if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
+        if ((rc = octo_fmm_interact(l.fmm)) != OCTO_FMM_OK) return rc;
+        const long long nc = (long long)l.n * l.n * l.n;
+        const unsigned blocks = (unsigned)((nc + 127) / 128);
+        if (lv == (int)s->lev.size() - 1)
+            l2l_kernel<false><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, nullptr, nullptr, nullptr, l.n, l.n, l.n, l.h);
+        else {
+            SolverLevel& p = s->lev[lv + 1];
+            l2l_kernel<true><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, p.fmm->L, p.fmm->C, p.off, l.n, l.n, l.n, l.h);
+        }
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    // ---- leaves: monopole sum over the leaf-level list straight into `out`, then the parent's expansion ----
+    double* const keep = s->leaf->outL;
+    s->leaf->outL = out;
+    rc = octo_fmm_interact(s->leaf);
+    s->leaf->outL = keep;
+    if (rc != OCTO_FMM_OK) return rc;
+    {
+        const int n = s->cfg.n;
+        const long long nc = (long long)n * n * n;
+        SolverLevel& p = s->lev[0];
+        leaf_eval_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_solver_status(octo_fmm_solver_t* s)
+{
+    if (!s) return OCTO_FMM_EINVAL;
+    int rc = octo_fmm_status(s->leaf);
+    for (SolverLevel& l : s->lev) {
+        const int r = octo_fmm_status(l.fmm);
+        if (rc == OCTO_FMM_OK) rc = r;
+    }
+    return rc;
+}
+
+int octo_fmm_solver_interaction_count(const octo_fmm_solver_t* s, unsigned long long* n)
+{
+    if (!s || !n) return OCTO_FMM_EINVAL;
+    *n = s->n_interactions;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_solver_get_leaf_stencil(const octo_fmm_solver_t* s, int parity, int* count, signed char (*dxyz)[3])
+{
+    if (!s) return OCTO_FMM_EINVAL;
+    return octo_fmm_get_stencil(s->leaf, parity, count, dxyz);
+}
+
+int octo_fmm_solver_num_levels(const octo_fmm_solver_t* s, int* multipole_levels, int* launches_per_solve)
+{
+    if (!s) return OCTO_FMM_EINVAL;
+    const int nl = (int)s->lev.size();
+    if (multipole_levels) *multipole_levels = nl;
+    // leaf: stage + interact + leaf_eval; per multipole level: m2m + stage + interact + l2l
+    if (launches_per_solve) *launches_per_solve = 3 + 4 * nl;
+    return OCTO_FMM_OK;
+}
+
+}  // extern "C"
