@@ -103,45 +103,44 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
     for (int i = 0; i < 3; ++i) poff[i * pcell + P] = dP[i];
 }
 
-// Taylor shift of a parent expansion pL (20 unique components in registers) by e, orders 0..NORD
+// Taylor shift of a parent expansion L (20 unique components in registers) by e, orders 0..NORD:
+//   out3 = L3;  out2_ij = L2_ij + L3_ijk e_k;  out1_i = L1_i + L2_ij e_j + 1/2 L3_ijk e_j e_k;
 //   out0 = L0 + L1_i e_i + 1/2 L2_ij e_i e_j + 1/6 L3_ijk e_i e_j e_k
-//   out1_i = L1_i + L2_ij e_j + 1/2 L3_ijk e_j e_k;  out2_ij = L2_ij + L3_ijk e_k;  out3 = L3
+// evaluated through the contractions w_ij = L3_ijk e_k, v_i = L2_ij e_j, u_i = w_ij e_j (about 50 FMAs).
 template <int NORD>
 __device__ __forceinline__ void taylor_shift(const double (&L)[20], const double (&e)[3], double (&out)[20])
 {
+    double w[6], v[3], u[3];
+#pragma unroll
+    for (int x = 0; x < 3; ++x)
+#pragma unroll
+        for (int y = x; y < 3; ++y) {
+            double t = 0.0;
+#pragma unroll
+            for (int z = 0; z < 3; ++z) t = fma(L[10 + u3(x, y, z)], e[z], t);
+            w[u2(x, y)] = t;
+        }
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+        double tv = 0.0, tu = 0.0;
+#pragma unroll
+        for (int y = 0; y < 3; ++y) {
+            tv = fma(L[4 + u2(x, y)], e[y], tv);
+            tu = fma(w[u2(x, y)], e[y], tu);
+        }
+        v[x] = tv;
+        u[x] = tu;
+    }
     double s0 = L[0];
 #pragma unroll
     for (int x = 0; x < 3; ++x) {
-        s0 += L[1 + x] * e[x];
-#pragma unroll
-        for (int y = 0; y < 3; ++y) {
-            s0 += 0.5 * L[4 + u2(x, y)] * e[x] * e[y];
-#pragma unroll
-            for (int z = 0; z < 3; ++z) s0 += L[10 + u3(x, y, z)] * e[x] * e[y] * e[z] / 6.0;
-        }
+        out[1 + x] = L[1 + x] + v[x] + 0.5 * u[x];
+        s0 = fma(e[x], L[1 + x] + 0.5 * v[x] + (1.0 / 6.0) * u[x], s0);
     }
     out[0] = s0;
-#pragma unroll
-    for (int x = 0; x < 3; ++x) {
-        double s1 = L[1 + x];
-#pragma unroll
-        for (int y = 0; y < 3; ++y) {
-            s1 += L[4 + u2(x, y)] * e[y];
-#pragma unroll
-            for (int z = 0; z < 3; ++z) s1 += 0.5 * L[10 + u3(x, y, z)] * e[y] * e[z];
-        }
-        out[1 + x] = s1;
-    }
     if (NORD >= 2) {
 #pragma unroll
-        for (int x = 0; x < 3; ++x)
-#pragma unroll
-            for (int y = x; y < 3; ++y) {
-                double s2 = L[4 + u2(x, y)];
-#pragma unroll
-                for (int z = 0; z < 3; ++z) s2 += L[10 + u3(x, y, z)] * e[z];
-                out[4 + u2(x, y)] = s2;
-            }
+        for (int t = 0; t < 6; ++t) out[4 + t] = L[4 + t] + w[t];
 #pragma unroll
         for (int t = 10; t < 20; ++t) out[t] = L[t];
     }
