@@ -195,6 +195,95 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_solve(args):
+    """--workload solve: the complete uniform-grid solve (octo_fmm_solver_*, NEXT f1) on the paper's uniform-sphere
+    problem (section 3.4); a step = one solve (all levels); interactions = ordered pairs over all levels."""
+    import numpy as np
+    import torch
+    import fmm_inputs as fi
+    import oracle
+    import paper_2101_08226_b200 as p
+    from paper_2101_08226_b200 import build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    local = env_int("LOCAL_RANK", 0)
+    if env_int("WORLD_SIZE", 1) > 1:
+        raise SystemExit("bench.py --workload solve is a single-GPU line")
+    torch.cuda.set_device(local)
+    build.build()
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream(dev)
+    n = args.ncell or 256
+    h, mass, phi, r = fi.uniform_sphere(n)
+    s = p.OctoFMMSolver(n, h, args.theta, True, device=local, stream=stream)
+    n_int = s.interaction_count()
+    levels, launches = s.num_levels()
+    m_d = torch.from_numpy(mass).to(dev)
+    out = torch.empty((4, n, n, n), dtype=torch.float64, device=dev)
+    for _ in range(max(args.warmup, 3)):
+        s.solve(m_d, out)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        s.solve(m_d, out)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop(t0, time.perf_counter())
+    ms = ev0.elapsed_time(ev1) / args.steps
+    if s.status() != p.OK:
+        raise SystemExit("bench.py: device reported status %d" % s.status())
+    eps = np.abs(out[0].cpu().numpy() - phi) / np.abs(phi)
+    # end to end through the host-buffer entry point
+    nb = p.octo_fmm_solver_host_scratch_bytes(s.cfg)
+    scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
+    m_h = torch.from_numpy(mass).pin_memory()
+    o_h = torch.empty((4, n, n, n), dtype=torch.float64).pin_memory()
+    p.octo_fmm_solver_solve_host(s.handle, m_h, o_h, scratch, nb)
+    t0 = time.perf_counter()
+    for _ in range(max(args.e2e_steps, 1)):
+        p.octo_fmm_solver_solve_host(s.handle, m_h, o_h, scratch, nb)
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / max(args.e2e_steps, 1)
+    # the oracle's complete solve on the host cores, on the 64^3 version of the same problem
+    nref = 64
+    hr, mr, _, _ = fi.uniform_sphere(nref)
+    oracle.lib()
+    t0 = time.perf_counter()
+    oracle.solve(nref, hr, args.theta, mr, True)
+    t_ref = time.perf_counter() - t0
+    cnt_ref = oracle.interact_monopole_leaf((nref, nref, nref), hr, args.theta, mr)[1]
+    m = nref // 2
+    while m >= 2:
+        cnt_ref += oracle.interaction_count((m, m, m), args.theta)
+        m //= 2
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak = sm_count * FP64_LANES_PER_SM * 2 * 1965.0e6 / 1e12
+    leaf_int = n_int - sum(oracle.interaction_count((n >> k,) * 3, args.theta) for k in range(1, n.bit_length()) if (n >> k) >= 2)
+    flops = 301.0 * (n_int - leaf_int) + 8.0 * leaf_int
+    line = {"metric": METRIC, "value": n_int / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "complete solve, uniform sphere (paper 3.4), %d^3 leaf cells, theta=%g, correction on" % (n, args.theta),
+                       "interactions_per_step": n_int, "leaf_interactions": leaf_int, "multipole_levels": levels,
+                       "cells_per_s": n ** 3 / (ms * 1e-3), "l2": "arrays of the fine levels larger than L2",
+                       "residual_vs_analytic": {"max": float(eps.max()), "mean": float(eps.mean())}},
+            "roofline": {"bound": "alu", "kernel": "whole solve (m2l_staged_kernel at the n/2 level dominates)",
+                         "achieved": flops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                         "frac": flops / (ms * 1e-3) / 1e12 / peak, "traffic": None},
+            "cpu_baseline": {"value": cnt_ref / t_ref, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": "oracle.solve of the same problem at %d^3 (%d interactions) in %.1f s" % (nref, cnt_ref, t_ref)},
+            "e2e": {"value": n_int / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(mass.nbytes),
+                    "d2h_bytes_per_step": int(o_h.numel() * 8), "ms_per_step": e2e_ms},
+            "clocks": clocks, "gpu_launches": launches * args.steps}
+    print(json.dumps(line))
+    s.close()
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -395,6 +484,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "solve":
+        run_solve(args)
     else:
         run_ours(args)
 

@@ -302,3 +302,18 @@ def config5(seed: int = DEFAULT_SEED, theta: float = 0.5, ncell: int = 256, keep
 
 
 CONFIGS = {"cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5}
+
+
+def uniform_sphere(ncell: int = 64, radius: float = 0.25, total_mass: float = 1.0, ambient: float = 1.0e-10):
+    """Paper section 3.4 (L448-456): a uniform sphere of radius 0.25 and mass 1 at the centre of the unit box, ambient
+    density 1e-10 of the sphere's, uniform grid.  The paper does not say how the sphere is rasterised: cells are
+    sampled at their centres and the masses scaled to the total mass.  Returns (h, mass[n][n][n], phi_analytic, r):
+    phi_analytic = -M (3 R^2 - r^2) / (2 R^3) inside, -M / r outside (the potential Eq. 42 compares with)."""
+    h = 1.0 / ncell
+    x = (np.arange(ncell) + 0.5) * h - 0.5
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    r = np.sqrt(X * X + Y * Y + Z * Z)
+    rho = np.where(r < radius, 1.0, ambient)
+    mass = rho * (total_mass / rho.sum())
+    phi = np.where(r < radius, -total_mass * (3.0 * radius ** 2 - r * r) / (2.0 * radius ** 3), -total_mass / r)
+    return h, mass, phi, r

@@ -176,6 +176,11 @@ size_t octo_fmm_solver_workspace_bytes(const octo_fmm_solver_config *cfg);   /* 
 int octo_fmm_solver_create(const octo_fmm_solver_config *cfg, octo_fmm_solver_t **out);
 /* mass: device, [n][n][n] (x fastest); out: device, [4][n][n][n].  Asynchronous on the stream. */
 int octo_fmm_solver_solve(octo_fmm_solver_t *s, const double *mass, double *out);
+/* The same with HOST buffers: H2D of the masses into scratch, solve, D2H of out, stream synchronise.
+ * scratch: device, >= octo_fmm_solver_host_scratch_bytes(cfg), borrowed for the call. */
+size_t octo_fmm_solver_host_scratch_bytes(const octo_fmm_solver_config *cfg);
+int octo_fmm_solver_solve_host(octo_fmm_solver_t *s, const double *mass_host, double *out_host, void *scratch,
+                               size_t scratch_bytes);
 /* Synchronises the stream; OCTO_FMM_EMASS if the correction met a cell of mass <= 0 at some level. */
 int octo_fmm_solver_status(octo_fmm_solver_t *s);
 int octo_fmm_solver_destroy(octo_fmm_solver_t *s);

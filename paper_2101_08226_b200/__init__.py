@@ -81,6 +81,9 @@ class _Library:
         lib.octo_fmm_solver_create.argtypes = [scfgp, ctypes.POINTER(vp)]
         lib.octo_fmm_solver_solve.argtypes = [vp, vp, vp]
         lib.octo_fmm_solver_status.argtypes = [vp]
+        lib.octo_fmm_solver_host_scratch_bytes.restype = ctypes.c_size_t
+        lib.octo_fmm_solver_host_scratch_bytes.argtypes = [scfgp]
+        lib.octo_fmm_solver_solve_host.argtypes = [vp, vp, vp, vp, ctypes.c_size_t]
         lib.octo_fmm_solver_destroy.argtypes = [vp]
         lib.octo_fmm_solver_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_solver_get_leaf_stencil.argtypes = [vp, ctypes.c_int, ip, vp]
@@ -262,6 +265,16 @@ def octo_fmm_solver_solve(s, mass, out):
     rc = _lib.octo_fmm_solver_solve(s, _ptr(mass), _ptr(out))
     if rc != OK:
         raise OctoFmmError("octo_fmm_solver_solve", rc)
+
+
+def octo_fmm_solver_host_scratch_bytes(cfg):
+    return int(_lib.octo_fmm_solver_host_scratch_bytes(ctypes.byref(cfg)))
+
+
+def octo_fmm_solver_solve_host(s, mass_host, out_host, scratch, scratch_bytes):
+    rc = _lib.octo_fmm_solver_solve_host(s, _ptr(mass_host), _ptr(out_host), _ptr(scratch), int(scratch_bytes))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_solve_host", rc)
 
 
 def octo_fmm_solver_status(s):

@@ -170,6 +170,29 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
     return OCTO_FMM_OK;
 }
 
+size_t octo_fmm_solver_host_scratch_bytes(const octo_fmm_solver_config* cfg)
+{
+    if (!solver_config_ok(cfg)) return 0;
+    const size_t nc = (size_t)cfg->n * cfg->n * cfg->n;
+    return align_up(nc * 8) + align_up(nc * 4 * 8);
+}
+
+int octo_fmm_solver_solve_host(octo_fmm_solver_t* s, const double* mass_host, double* out_host, void* scratch, size_t scratch_bytes)
+{
+    if (!s || !mass_host || !out_host || !scratch) return OCTO_FMM_EINVAL;
+    if (scratch_bytes < octo_fmm_solver_host_scratch_bytes(&s->cfg) || ((uintptr_t)scratch % ALIGN)) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(s->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    const size_t nc = (size_t)s->cfg.n * s->cfg.n * s->cfg.n;
+    double* d_m = (double*)scratch;
+    double* d_o = (double*)((char*)scratch + align_up(nc * 8));
+    if (cudaMemcpyAsync(d_m, mass_host, nc * 8, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    const int rc = octo_fmm_solver_solve(s, d_m, d_o);
+    if (rc != OCTO_FMM_OK) return rc;
+    if (cudaMemcpyAsync(out_host, d_o, nc * 4 * 8, cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    return OCTO_FMM_OK;
+}
+
 int octo_fmm_solver_status(octo_fmm_solver_t* s)
 {
     if (!s) return OCTO_FMM_EINVAL;
