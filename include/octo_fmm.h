@@ -122,7 +122,7 @@ int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *c
 
 /* Options, for tests and profiling.  "kernel" = 0 staged (TMA + shared memory, default), 1 direct
  * (global-memory loads; same pair arithmetic).  "host_chunk" = output z-layers per pipeline slab of
- * octo_fmm_run_host (default 24; 0 = one copy in, one launch, one copy out).  Unknown keys -> EINVAL. */
+ * octo_fmm_run_host (default 12; 0 = one copy in, one launch, one copy out).  Unknown keys -> EINVAL. */
 int octo_fmm_set_option(octo_fmm_t *h, const char *key, int value);
 
 /* Launch facts of the interaction kernel the handle would run: grid, block, dynamic shared

@@ -207,7 +207,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->sm_count = prop.multiProcessorCount;
     h->state = 0;
     h->kernel = 0;
-    h->host_chunk = 24;
+    h->host_chunk = 12;
     h->host_launches = 0;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
     region_of(*cfg, h->lo, h->hi, flags);
