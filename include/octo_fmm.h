@@ -174,7 +174,8 @@ typedef struct {
 
 size_t octo_fmm_solver_workspace_bytes(const octo_fmm_solver_config *cfg);   /* 0 on invalid configuration */
 int octo_fmm_solver_create(const octo_fmm_solver_config *cfg, octo_fmm_solver_t **out);
-/* mass: device, [n][n][n] (x fastest); out: device, [4][n][n][n].  Asynchronous on the stream. */
+/* mass: device, [n][n][n] (x fastest); out: device, [4][n][n][n]; both 16-byte aligned (else EINVAL).
+ * Asynchronous on the stream. */
 int octo_fmm_solver_solve(octo_fmm_solver_t *s, const double *mass, double *out);
 /* The same with HOST buffers: H2D of the masses into scratch, solve, D2H of out, stream synchronise.
  * scratch: device, >= octo_fmm_solver_host_scratch_bytes(cfg), borrowed for the call. */

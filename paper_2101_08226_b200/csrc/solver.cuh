@@ -42,19 +42,27 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
                                                   double* __restrict__ pm, double* __restrict__ poff, int pnx, int pny, int pnz,
                                                   double hc)
 {
+    // grid = (ceil(pnx / blockDim.x), pny, pnz): no integer divisions
     const long long pcell = (long long)pnx * pny * pnz, ccell = 8 * pcell;
-    const long long P = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (P >= pcell) return;
-    const int I = (int)(P % pnx), J = (int)((P / pnx) % pny), K = (int)(P / ((long long)pnx * pny));
+    const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y, K = blockIdx.z;
+    if (I >= pnx) return;
+    const long long P = ((long long)K * pny + J) * pnx + I;
     const int cnx = 2 * pnx, cny = 2 * pny;
     long long cell[8];
-    double rel[8][3];
+    double rel[8][3], m0s[8];
     double mass = 0.0, com[3] = {0.0, 0.0, 0.0};
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         const int a[3] = {c & 1, (c >> 1) & 1, (c >> 2) & 1};
         cell[c] = ((long long)(2 * K + a[2]) * cny + (2 * J + a[1])) * cnx + (2 * I + a[0]);
-        const double m0 = cm[cell[c]];
+        double m0;
+        if (LEAF) {          // the two x-children are one aligned double2 (cm is 16-byte aligned, cnx is even)
+            const double2 pair = *reinterpret_cast<const double2*>(cm + (cell[c] - a[0]));
+            m0 = a[0] ? pair.y : pair.x;
+        } else {
+            m0 = cm[cell[c]];
+        }
+        m0s[c] = m0;
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             rel[c][i] = ((double)a[i] - 0.5) * hc + (LEAF ? 0.0 : coff[i * ccell + cell[c]]);
@@ -74,7 +82,7 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         double M[20];
-        M[0] = cm[cell[c]];
+        M[0] = m0s[c];
 #pragma unroll
         for (int t = 1; t < 20; ++t) M[t] = LEAF ? 0.0 : cm[t * ccell + cell[c]];
         double d[3];
@@ -157,18 +165,19 @@ __global__ void __launch_bounds__(128) l2l_kernel(double* __restrict__ cL, doubl
                                                   const double* __restrict__ pL, const double* __restrict__ pC,
                                                   const double* __restrict__ poff, int cnx, int cny, int cnz, double hc)
 {
+    // grid = (ceil(cnx / blockDim.x), cny, cnz)
     const long long ccell = (long long)cnx * cny * cnz;
-    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= ccell) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= cnx) return;
+    const long long cell = ((long long)k * cny + j) * cnx + i;
     double C[3];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) C[i] = cC[i * ccell + cell];
+    for (int c = 0; c < 3; ++c) C[c] = cC[c * ccell + cell];
     if (!HAS_PARENT) {
 #pragma unroll
-        for (int i = 0; i < 3; ++i) cL[(1 + i) * ccell + cell] -= C[i];
+        for (int c = 0; c < 3; ++c) cL[(1 + c) * ccell + cell] -= C[c];
         return;
     }
-    const int i = (int)(cell % cnx), j = (int)((cell / cnx) % cny), k = (int)(cell / ((long long)cnx * cny));
     const int pnx = cnx / 2, pny = cny / 2;
     const long long pcell = ccell / 8;
     const long long P = ((long long)(k / 2) * pny + (j / 2)) * pnx + (i / 2);
@@ -192,27 +201,46 @@ __global__ void __launch_bounds__(128) l2l_kernel(double* __restrict__ cL, doubl
 // ------------------------------------------------------------------------------------------
 // Leaf evaluation: out = (phi, g) of the leaf-level monopole sum; add the parent's expansion
 // evaluated at the leaf's cell centre:  phi += L0(e),  g -= L1(e) + correction,  e = ((a,b,c) - 1/2) h - delta_P.
+// One thread per PARENT (grid = (ceil(pnx / blockDim.x), pny, pnz)): the parent's 26 numbers are read once
+// and its 8 leaves are updated as four double2 (x-pairs), so every access of a warp is contiguous.
+// out must be 16-byte aligned.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) leaf_eval_kernel(double* __restrict__ out, const double* __restrict__ pL,
                                                         const double* __restrict__ pC, const double* __restrict__ poff, int nx,
                                                         int ny, int nz, double h)
 {
-    const long long ncell = (long long)nx * ny * nz;
-    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= ncell) return;
-    const int i = (int)(cell % nx), j = (int)((cell / nx) % ny), k = (int)(cell / ((long long)nx * ny));
-    const long long pcell = ncell / 8;
-    const long long P = ((long long)(k / 2) * (ny / 2) + (j / 2)) * (nx / 2) + (i / 2);
-    const int a[3] = {i & 1, j & 1, k & 1};
-    double e[3], L[20], sh[20];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) e[c] = ((double)a[c] - 0.5) * h - poff[c * pcell + P];
+    const int pnx = nx / 2, pny = ny / 2;
+    const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y, K = blockIdx.z;
+    if (I >= pnx) return;
+    const long long ncell = (long long)nx * ny * nz, pcell = ncell / 8;
+    const long long P = ((long long)K * pny + J) * pnx + I;
+    double L[20], C[3], dP[3];
 #pragma unroll
     for (int t = 0; t < 20; ++t) L[t] = pL[t * pcell + P];
-    taylor_shift<1>(L, e, sh);
-    out[cell] += sh[0];
 #pragma unroll
-    for (int c = 0; c < 3; ++c) out[(1 + c) * ncell + cell] -= sh[1 + c] + pC[c * pcell + P];
+    for (int c = 0; c < 3; ++c) { C[c] = pC[c * pcell + P]; dP[c] = poff[c * pcell + P]; }
+#pragma unroll
+    for (int cz = 0; cz < 2; ++cz)
+#pragma unroll
+        for (int cy = 0; cy < 2; ++cy) {
+            const long long row = ((long long)(2 * K + cz) * ny + (2 * J + cy)) * nx + 2 * I;     // even: 16-byte aligned
+            double sh0[20], sh1[20];
+            const double e0[3] = {-0.5 * h - dP[0], ((double)cy - 0.5) * h - dP[1], ((double)cz - 0.5) * h - dP[2]};
+            const double e1[3] = {0.5 * h - dP[0], e0[1], e0[2]};
+            taylor_shift<1>(L, e0, sh0);
+            taylor_shift<1>(L, e1, sh1);
+            double2* o = reinterpret_cast<double2*>(out + row);
+            double2 v = *o;
+            v.x += sh0[0]; v.y += sh1[0];
+            *o = v;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                double2* g = reinterpret_cast<double2*>(out + (1 + c) * ncell + row);
+                double2 w = *g;
+                w.x -= sh0[1 + c] + C[c]; w.y -= sh1[1 + c] + C[c];
+                *g = w;
+            }
+        }
 }
 
 }  // namespace octo

@@ -125,6 +125,7 @@ int octo_fmm_solver_create(const octo_fmm_solver_config* cfg, octo_fmm_solver_t*
 int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
 {
     if (!s || !mass || !out) return OCTO_FMM_EINVAL;
+    if (((uintptr_t)mass % 16) || ((uintptr_t)out % 16)) return OCTO_FMM_EINVAL;     // double2 accesses
     if (cudaSetDevice(s->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
     cudaStream_t st = s->stream;
     int rc;
@@ -132,8 +133,7 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
     if ((rc = octo_fmm_set_moments(s->leaf, mass, nullptr)) != OCTO_FMM_OK) return rc;
     for (size_t lv = 0; lv < s->lev.size(); ++lv) {
         SolverLevel& l = s->lev[lv];
-        const long long nc = (long long)l.n * l.n * l.n;
-        const unsigned blocks = (unsigned)((nc + 127) / 128);
+        const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
         if (lv == 0) m2m_kernel<true><<<blocks, 128, 0, st>>>(mass, nullptr, l.raw, l.off, l.n, l.n, l.n, s->cfg.h);
         else         m2m_kernel<false><<<blocks, 128, 0, st>>>(s->lev[lv - 1].raw, s->lev[lv - 1].off, l.raw, l.off, l.n, l.n, l.n,
                                                               s->lev[lv - 1].h);
@@ -144,8 +144,7 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
         SolverLevel& l = s->lev[lv];
         if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
         if ((rc = octo_fmm_interact(l.fmm)) != OCTO_FMM_OK) return rc;
-        const long long nc = (long long)l.n * l.n * l.n;
-        const unsigned blocks = (unsigned)((nc + 127) / 128);
+        const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
         if (lv == (int)s->lev.size() - 1)
             l2l_kernel<false><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, nullptr, nullptr, nullptr, l.n, l.n, l.n, l.h);
         else {
@@ -162,9 +161,8 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
     if (rc != OCTO_FMM_OK) return rc;
     {
         const int n = s->cfg.n;
-        const long long nc = (long long)n * n * n;
         SolverLevel& p = s->lev[0];
-        leaf_eval_kernel<<<(unsigned)((nc + 127) / 128), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
+        leaf_eval_kernel<<<dim3((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2)), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     return OCTO_FMM_OK;

@@ -113,3 +113,21 @@ def test_solver_rejects_bad_configurations(env):
             p.octo_fmm_solver_create(p.make_solver_config(n, 1.0 / n, theta))
     with pytest.raises(p.OctoFmmError):          # no workspace
         p.octo_fmm_solver_create(p.make_solver_config(32, 1.0 / 32, 0.5))
+
+
+def test_solve_host_entry_point(env):
+    """octo_fmm_solver_solve_host (H2D + solve + D2H) gives the device-pointer route's numbers bit for bit."""
+    p, torch = env
+    n = 32
+    h, mass, _, _ = fi.uniform_sphere(n)
+    s = p.OctoFMMSolver(n, h, 0.5, True)
+    dev_out = s.solve(torch.from_numpy(mass).cuda()).cpu().numpy()
+    nb = p.octo_fmm_solver_host_scratch_bytes(s.cfg)
+    scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    m_h = torch.from_numpy(mass).pin_memory()
+    o_h = torch.full((4, n, n, n), float("nan"), dtype=torch.float64).pin_memory()
+    p.octo_fmm_solver_solve_host(s.handle, m_h, o_h, scratch, nb)
+    assert np.array_equal(o_h.numpy(), dev_out)
+    with pytest.raises(p.OctoFmmError):
+        p.octo_fmm_solver_solve_host(s.handle, m_h, o_h, scratch, nb - 1)
+    s.close()

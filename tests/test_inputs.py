@@ -59,3 +59,17 @@ def test_binary_mass_ratio_and_noise():
     assert np.abs(ratio - 1).max() <= 1.0001e-8 and np.abs(ratio - 1).max() > 1e-9
     w4 = fi.config4(ncell=32)
     assert w4.kind == "monopole" and w4.moments.shape == (1, 32, 32, 32) and w4.com_off is None
+
+
+def test_uniform_sphere_of_section_3_4():
+    """Radius 0.25, total mass 1, ambient 1e-10 of the sphere's density (L452); the analytic potential is continuous at
+    the surface and -M/r outside."""
+    h, mass, phi, r = fi.uniform_sphere(32)
+    assert h == 1.0 / 32 and mass.shape == (32, 32, 32)
+    assert abs(mass.sum() - 1.0) < 1e-14
+    inside = r < 0.25
+    assert np.isclose(mass[~inside].max() / mass[inside].min(), 1e-10, rtol=1e-12)
+    assert abs(inside.sum() * h ** 3 / (4.0 / 3.0 * np.pi * 0.25 ** 3) - 1.0) < 0.03      # rasterised volume
+    assert np.allclose(phi[~inside], -1.0 / r[~inside])
+    assert np.isclose(-(3 * 0.0625 - 0.25 ** 2) / (2 * 0.25 ** 3), -1.0 / 0.25)           # continuity at r = R
+    assert phi.min() > -1.5 / 0.25 - 1e-12                                                # centre value -3M/2R
