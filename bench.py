@@ -323,6 +323,11 @@ def run_ours(args):
     Lc = torch.empty((3,) + f.out_shape, dtype=torch.float64, device=dev) if multi else None
 
     f.bind_outputs(L, Lc)          # interact() writes the expansions straight into the caller's buffers
+    if multi:
+        # The headline is the GENERAL path (all 27 dipole terms evaluated, 301 flop per interaction) although these
+        # centre-of-mass inputs would let the library leave them out; its default path is measured after the timed
+        # region and reported beside it as "com_fast_path".
+        f.set_option("dipole_terms", 1)
 
     def step():
         f.set_moments(mom, com)
@@ -401,6 +406,29 @@ def run_ours(args):
                "checksum_L0": float(L_h[0].sum())}
         del scratch, mom_h, com_h, L_h, Lc_h
 
+    # ---- the library's default path on these inputs (dipole terms left out after the device-side check) ----
+    fast = None
+    if multi:
+        f.set_option("dipole_terms", 0)
+        f.set_moments(mom, com)
+        used = f.dipole_terms_used()
+        for _ in range(2):
+            f.interact()
+        fa, fb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        fa.record(stream)
+        for _ in range(3):
+            f.interact()
+        fb.record(stream)
+        torch.cuda.synchronize()
+        fast_ms = fa.elapsed_time(fb) / 3
+        ff, fi_ = p.octo_fmm_flops_per_interaction_path(kind, True, used)
+        fast = {"dipole_terms_evaluated": bool(used), "kernel_ms": fast_ms, "interactions_per_s": n_int / (fast_ms * 1e-3),
+                "flops_per_interaction": ff, "fp64_instr_per_interaction": fi_,
+                "achieved_tflops": ff * n_int / (fast_ms * 1e-3) / 1e12,
+                "note": "every |M1_i| <= 4e-16 |M| h (checked on the device at staging): the 27 dipole terms contribute "
+                        "nothing and are not evaluated; results agree with the general path to round-off"}
+        f.set_option("dipole_terms", 1)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -454,6 +482,9 @@ def run_ours(args):
                 "launch": info, "parallelism": "independent problem per GPU" if world > 1 else "single GPU"},
             "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
             "gpu_launches": 2 * args.steps}
+    if fast is not None:
+        fast["frac_of_peak"] = fast["achieved_tflops"] / peak_tflops
+        line["com_fast_path"] = fast
     print(json.dumps(line))
     f.close()
     if world > 1:

@@ -120,8 +120,16 @@ size_t octo_fmm_host_scratch_bytes(const octo_fmm_config *cfg);
 int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *com_off_host,
                       double *L_host, double *Lcorr_host, void *scratch, size_t scratch_bytes);
 
+/* The dipole terms.  Sources expanded about their centre of mass have M^(1) = 0 up to round-off, and the 27
+ * terms that contain M^(1) then contribute nothing.  set_moments() checks on the device whether every cell
+ * has |M^(1)_i| <= 4e-16 |M| h; if so interact() leaves those terms out (245 instead of 301 flop per
+ * interaction), otherwise it evaluates them -- results agree with the general formula to round-off either
+ * way.  octo_fmm_set_option(h, "dipole_terms", 1) forces the general path.  After set_moments(),
+ * octo_fmm_dipole_terms_used() synchronises the stream and tells which path interact() takes. */
+int octo_fmm_dipole_terms_used(octo_fmm_t *h, int *used);
+
 /* Options, for tests and profiling.  "kernel" = 0 staged (TMA + shared memory, default), 1 direct
- * (global-memory loads; same pair arithmetic).  "host_chunk" = output z-layers per pipeline slab of
+ * (global-memory loads; same pair arithmetic).  "dipole_terms" = 0 decided on the device (default), 1 always evaluated.  "host_chunk" = output z-layers per pipeline slab of
  * octo_fmm_run_host (default 12; 0 = one copy in, one launch, one copy out).  Unknown keys -> EINVAL. */
 int octo_fmm_set_option(octo_fmm_t *h, const char *key, int value);
 
@@ -145,6 +153,8 @@ int octo_fmm_fp64_issue_probe(int device, void *stream, void *scratch, int mode,
 /* FP64 operations one multipole (kind 0) / monopole (kind 1) interaction executes in the kernel's
  * inner loop, counted from its operation list (DFMA = 2, DADD/DMUL = 1); see DESIGN.md. */
 int octo_fmm_flops_per_interaction(int kind, int am_correction, int *flops, int *fp64_instructions);
+/* The same for a given path: dipole_terms = 0 is the path without the 27 dipole terms (multipole kind only). */
+int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int *flops, int *fp64_instructions);
 
 const char *octo_fmm_version(void);
 

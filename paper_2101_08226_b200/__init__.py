@@ -74,6 +74,8 @@ class _Library:
         lib.octo_fmm_fp64_peak_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, dp, ip, ip]
         lib.octo_fmm_fp64_issue_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, ctypes.c_int, dp]
         lib.octo_fmm_flops_per_interaction.argtypes = [ctypes.c_int, ctypes.c_int, ip, ip]
+        lib.octo_fmm_flops_per_interaction_path.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, ip]
+        lib.octo_fmm_dipole_terms_used.argtypes = [vp, ip]
         lib.octo_fmm_version.restype = ctypes.c_char_p
         scfgp = ctypes.POINTER(octo_fmm_solver_config)
         lib.octo_fmm_solver_workspace_bytes.restype = ctypes.c_size_t
@@ -239,6 +241,23 @@ def octo_fmm_flops_per_interaction(kind, am_correction):
     if rc != OK:
         raise OctoFmmError("octo_fmm_flops_per_interaction", rc)
     return f.value, i.value
+
+
+def octo_fmm_flops_per_interaction_path(kind, am_correction, dipole_terms):
+    f, i = ctypes.c_int(0), ctypes.c_int(0)
+    rc = _lib.octo_fmm_flops_per_interaction_path(int(kind), int(bool(am_correction)), int(bool(dipole_terms)),
+                                                  ctypes.byref(f), ctypes.byref(i))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_flops_per_interaction_path", rc)
+    return f.value, i.value
+
+
+def octo_fmm_dipole_terms_used(h):
+    u = ctypes.c_int(0)
+    rc = _lib.octo_fmm_dipole_terms_used(h, ctypes.byref(u))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_dipole_terms_used", rc)
+    return bool(u.value)
 
 
 # ---- complete uniform-grid solve (octo_fmm_solver_*) ------------------------------------------
@@ -435,6 +454,9 @@ class OctoFMM:
 
     def launch_info(self):
         return octo_fmm_launch_info(self.handle)
+
+    def dipole_terms_used(self):
+        return octo_fmm_dipole_terms_used(self.handle)
 
     def set_option(self, key, value):
         octo_fmm_set_option(self.handle, key, value)

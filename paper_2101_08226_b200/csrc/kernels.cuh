@@ -67,15 +67,20 @@ struct Params {
     const double* S;         // staged sources
     double* L;               // [20][oz][oy][ox]
     double* C;               // [3][oz][oy][ox]
-    int* flags;              // bit 0: target mass <= 0 with correction
+    int* flags;              // flags[0] bit 0: target mass <= 0 with correction; flags[1] bit 1: some source cell has a
+                             // dipole moment (raised by the staging kernel, cleared by set_moments)
+    int force_dipole;        // 1: evaluate the dipole terms whatever bit 1 says
 };
 
 // ------------------------------------------------------------------------------------------
 // a2: stage the sources
 // ------------------------------------------------------------------------------------------
+constexpr double DIPOLE_TOL = 4.0e-16;   // |M1_i| <= DIPOLE_TOL |M| h counts as "no dipole" (round-off of a P2M / M2M about the centre of mass)
+
 __global__ void __launch_bounds__(256) stage_multipole_kernel(const double* __restrict__ mom,
                                                               const double* __restrict__ com, double* __restrict__ S,
-                                                              int nx, int ny, int nz, int z_begin, int z_count)
+                                                              int nx, int ny, int nz, int z_begin, int z_count, double h,
+                                                              int* __restrict__ flags)
 {
     const long long ncell = (long long)nx * ny * nz;
     const long long local = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -88,6 +93,10 @@ __global__ void __launch_bounds__(256) stage_multipole_kernel(const double* __re
 #pragma unroll
     for (int c = 0; c < 20; ++c) M[c] = mom[(long long)c * ncell + cell];
     reduce_moments(M, s);
+    {
+        const double lim = DIPOLE_TOL * fabs(M[0]) * h;
+        if (fabs(M[1]) > lim || fabs(M[2]) > lim || fabs(M[3]) > lim) atomicOr(flags + 1, 2);
+    }
 #pragma unroll
     for (int c = 0; c < 3; ++c) s[C_DX + c] = com ? com[(long long)c * ncell + cell] : 0.0;
     s[19] = 0.0;
@@ -222,48 +231,11 @@ __device__ __forceinline__ void store_target(const Params& p, const Acc& acc, in
     for (int c = 0; c < 3; ++c) p.C[(long long)c * ocell + o] = C[c];
 }
 
-template <bool CORR>
-__global__ void __launch_bounds__(STAGED_THREADS, 1)
-m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
+// The consumer warps' loop over the bricks of this CTA.  DIPOLE = false is the fast path for sources
+// expanded about their centre of mass (no dipole terms), see m2l_staged_kernel.
+template <bool CORR, bool DIPOLE>
+__device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, uint64_t* full, uint64_t* empty, int warp, int lane)
 {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    double2* slab0 = reinterpret_cast<double2*>(smem_raw);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + NSTAGE * SLAB_BYTES);
-    uint64_t* empty = full + NSTAGE;
-
-    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
-    const int lane = threadIdx.x & 31;
-
-    if (threadIdx.x == 0) {
-        for (int b = 0; b < NSTAGE; ++b) {
-            mbar_init(&full[b], 1);
-            mbar_init(&empty[b], CONSUMER_WARPS);
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();
-
-    if (warp == CONSUMER_WARPS) {
-        // ------------------------------ producer ------------------------------
-        if (lane == 0) {
-            uint32_t it = 0;
-            for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
-                int x0, y0, k0;
-                decode_tile(p, t, x0, y0, k0);
-                const int z_lo = max(k0 - p.reach, 0), z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.nz - 1);
-                for (int zz = z_lo; zz <= z_hi; ++zz) {
-                    const uint32_t b = it % NSTAGE;
-                    if (it >= NSTAGE) mbar_wait_backoff(&empty[b], ((it / NSTAGE) - 1) & 1);
-                    mbar_arrive_expect_tx(&full[b], SLAB_BYTES);
-                    tma_load_slab(slab0 + (size_t)b * SLAB_ELEMS, &tmap, &full[b], (x0 >> 1) - 3, 2 * (y0 - REACH_MAX), zz);
-                    ++it;
-                }
-            }
-        }
-        return;
-    }
-
     // ------------------------------ consumers ------------------------------
     const int cls_xy = warp & 3;                       // px + 2 py
     const int layer = warp >> 2;                       // 0..2
@@ -340,17 +312,68 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
             for (;;) {
                 if (!ensure()) break;
                 OCTO_FETCH(B);
-                m2l_pair<CORR>(acc, A.x, A.y, A.z, A.w, A.src, tA);
+                m2l_pair<CORR, DIPOLE>(acc, A.x, A.y, A.z, A.w, A.src, tA);
                 if (!ensure()) { A = B; break; }
                 OCTO_FETCH(A);
-                m2l_pair<CORR>(acc, B.x, B.y, B.z, B.w, B.src, tA);
+                m2l_pair<CORR, DIPOLE>(acc, B.x, B.y, B.z, B.w, B.src, tA);
             }
-            m2l_pair<CORR>(acc, A.x, A.y, A.z, A.w, A.src, tA);
+            m2l_pair<CORR, DIPOLE>(acc, A.x, A.y, A.z, A.w, A.src, tA);
         }
 #undef OCTO_FETCH
 
         if (active) store_target<CORR>(p, acc, gx, gy, k);
     }
+}
+
+template <bool CORR>
+__global__ void __launch_bounds__(STAGED_THREADS, 1)
+m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double2* slab0 = reinterpret_cast<double2*>(smem_raw);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + NSTAGE * SLAB_BYTES);
+    uint64_t* empty = full + NSTAGE;
+
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < NSTAGE; ++b) {
+            mbar_init(&full[b], 1);
+            mbar_init(&empty[b], CONSUMER_WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == CONSUMER_WARPS) {
+        // ------------------------------ producer ------------------------------
+        if (lane == 0) {
+            uint32_t it = 0;
+            for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
+                int x0, y0, k0;
+                decode_tile(p, t, x0, y0, k0);
+                const int z_lo = max(k0 - p.reach, 0), z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.nz - 1);
+                for (int zz = z_lo; zz <= z_hi; ++zz) {
+                    const uint32_t b = it % NSTAGE;
+                    if (it >= NSTAGE) mbar_wait_backoff(&empty[b], ((it / NSTAGE) - 1) & 1);
+                    mbar_arrive_expect_tx(&full[b], SLAB_BYTES);
+                    tma_load_slab(slab0 + (size_t)b * SLAB_ELEMS, &tmap, &full[b], (x0 >> 1) - 3, 2 * (y0 - REACH_MAX), zz);
+                    ++it;
+                }
+            }
+        }
+        return;
+    }
+
+    // ------------------------------ consumers ------------------------------
+    // Sources expanded about their centre of mass have no dipole moment: the staging kernel raises bit 1 of
+    // the flags if any cell has |M1_i| > DIPOLE_TOL |M| h, and only then (or when the caller forces it) the
+    // 27 dipole terms are evaluated.  The branch is uniform over the grid.
+    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
+    if (dipole) staged_consume<CORR, true>(p, slab0, full, empty, warp, lane);
+    else        staged_consume<CORR, false>(p, slab0, full, empty, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -371,6 +394,7 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
     const long long plane = (long long)p.ny * p.nx;
     const double2* S2 = reinterpret_cast<const double2*>(p.S);
     const int cls = warp;
+    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
     for (int pass = 0; pass < 2; ++pass) {
         const int k = z0 + pz + 2 * pass;
         if (!(gx < p.hi[0] && gy < p.hi[1] && k < p.hi[2])) continue;
@@ -390,7 +414,8 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
             const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
             const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by_);
             const double z = c_hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
-            m2l_pair<CORR>(acc, x, y, z, pair_head(x, y, z), src, tA);
+            if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
+            else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
         }
         store_target<CORR>(p, acc, gx, gy, k);
     }

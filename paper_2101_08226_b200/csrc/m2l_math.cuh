@@ -92,7 +92,9 @@ __device__ __forceinline__ double pair_head(const double x, const double y, cons
 
 // Body of one ordered pair A <- B.  (x,y,z) = R = z_A - z_B, w = 1/|R|; s[0..15] staged source
 // components; tA[0..6] = staged third moments of the target divided by its mass (correction only).
-template <bool CORR>
+// DIPOLE = false leaves out the 27 terms with the source's dipole moment (and D2_zz, which only they need):
+// the fast path for sources expanded about their centre of mass, chosen on the device (kernels.cuh).
+template <bool CORR, bool DIPOLE>
 __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y, const double z, const double w,
                                          const double (&s)[16], const double (&tA)[7])
 {
@@ -120,23 +122,23 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
     // ---- D0, D1 ----
     a.l0 = fma(m0, -w, a.l0);
     const double D1x = d1 * x, D1y = d1 * y, D1z = d1 * z;
-    a.l1[0] = fma(m0, D1x, a.l1[0]);  a.l0b = fma(m1x, D1x, a.l0b);
-    a.l1[1] = fma(m0, D1y, a.l1[1]);  a.l0 = fma(m1y, D1y, a.l0);
-    a.l1[2] = fma(m0, D1z, a.l1[2]);  a.l0b = fma(m1z, D1z, a.l0b);
+    a.l1[0] = fma(m0, D1x, a.l1[0]);  if (DIPOLE) a.l0b = fma(m1x, D1x, a.l0b);
+    a.l1[1] = fma(m0, D1y, a.l1[1]);  if (DIPOLE) a.l0 = fma(m1y, D1y, a.l0);
+    a.l1[2] = fma(m0, D1z, a.l1[2]);  if (DIPOLE) a.l0b = fma(m1z, D1z, a.l0b);
 
     // ---- D2 (6 components; zz is needed by the dipole term of L1_z) ----
     const double ax = d2 * x, ay = d2 * y, az = d2 * z;
     const double Dxx = fma(ax, x, d1), Dyy = fma(ay, y, d1), Dzz = fma(az, z, d1);
     const double Dxy = ax * y, Dxz = ax * z, Dyz = ay * z;
-    a.l2[0] = fma(m0, Dxx, a.l2[0]);  a.l1[0] = fma(m1x, Dxx, a.l1[0]);  a.l0 = fma(qxx, Dxx, a.l0);
-    a.l2[1] = fma(m0, Dxy, a.l2[1]);  a.l1[1] = fma(m1x, Dxy, a.l1[1]);  a.l1[0] = fma(m1y, Dxy, a.l1[0]);
+    a.l2[0] = fma(m0, Dxx, a.l2[0]);  if (DIPOLE) a.l1[0] = fma(m1x, Dxx, a.l1[0]);  a.l0 = fma(qxx, Dxx, a.l0);
+    a.l2[1] = fma(m0, Dxy, a.l2[1]);  if (DIPOLE) a.l1[1] = fma(m1x, Dxy, a.l1[1]);  if (DIPOLE) a.l1[0] = fma(m1y, Dxy, a.l1[0]);
     a.l0b = fma(qxy, Dxy, a.l0b);
-    a.l2[2] = fma(m0, Dxz, a.l2[2]);  a.l1[2] = fma(m1x, Dxz, a.l1[2]);  a.l1[0] = fma(m1z, Dxz, a.l1[0]);
+    a.l2[2] = fma(m0, Dxz, a.l2[2]);  if (DIPOLE) a.l1[2] = fma(m1x, Dxz, a.l1[2]);  if (DIPOLE) a.l1[0] = fma(m1z, Dxz, a.l1[0]);
     a.l0 = fma(qxz, Dxz, a.l0);
-    a.l2[3] = fma(m0, Dyy, a.l2[3]);  a.l1[1] = fma(m1y, Dyy, a.l1[1]);  a.l0b = fma(qyy, Dyy, a.l0b);
-    a.l2[4] = fma(m0, Dyz, a.l2[4]);  a.l1[2] = fma(m1y, Dyz, a.l1[2]);  a.l1[1] = fma(m1z, Dyz, a.l1[1]);
+    a.l2[3] = fma(m0, Dyy, a.l2[3]);  if (DIPOLE) a.l1[1] = fma(m1y, Dyy, a.l1[1]);  a.l0b = fma(qyy, Dyy, a.l0b);
+    a.l2[4] = fma(m0, Dyz, a.l2[4]);  if (DIPOLE) a.l1[2] = fma(m1y, Dyz, a.l1[2]);  if (DIPOLE) a.l1[1] = fma(m1z, Dyz, a.l1[1]);
     a.l0 = fma(qyz, Dyz, a.l0);
-    a.l1[2] = fma(m1z, Dzz, a.l1[2]);
+    if (DIPOLE) a.l1[2] = fma(m1z, Dzz, a.l1[2]);
 
     // ---- D3: 7 independent + xzz, yzz ----
     const double bx = d3 * x, by = d3 * y;
@@ -145,29 +147,29 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
     const double Dxxx = fma(bxx, x, ax3);
     const double Dxxy = fma(bxx, y, ay);
     const double Dxxz = fma(bxx, z, az);
-    a.l3[0] = fma(m0, Dxxx, a.l3[0]);  a.l2[0] = fma(m1x, Dxxx, a.l2[0]);  a.l1[0] = fma(qxx, Dxxx, a.l1[0]);
+    a.l3[0] = fma(m0, Dxxx, a.l3[0]);  if (DIPOLE) a.l2[0] = fma(m1x, Dxxx, a.l2[0]);  a.l1[0] = fma(qxx, Dxxx, a.l1[0]);
     a.l0b = fma(oxxx, Dxxx, a.l0b);
-    a.l3[1] = fma(m0, Dxxy, a.l3[1]);  a.l2[1] = fma(m1x, Dxxy, a.l2[1]);  a.l2[0] = fma(m1y, Dxxy, a.l2[0]);
+    a.l3[1] = fma(m0, Dxxy, a.l3[1]);  if (DIPOLE) a.l2[1] = fma(m1x, Dxxy, a.l2[1]);  if (DIPOLE) a.l2[0] = fma(m1y, Dxxy, a.l2[0]);
     a.l1[1] = fma(qxx, Dxxy, a.l1[1]);  a.l1[0] = fma(qxy, Dxxy, a.l1[0]);  a.l0 = fma(oxxy, Dxxy, a.l0);
-    a.l3[2] = fma(m0, Dxxz, a.l3[2]);  a.l2[2] = fma(m1x, Dxxz, a.l2[2]);  a.l2[0] = fma(m1z, Dxxz, a.l2[0]);
+    a.l3[2] = fma(m0, Dxxz, a.l3[2]);  if (DIPOLE) a.l2[2] = fma(m1x, Dxxz, a.l2[2]);  if (DIPOLE) a.l2[0] = fma(m1z, Dxxz, a.l2[0]);
     a.l1[2] = fma(qxx, Dxxz, a.l1[2]);  a.l1[0] = fma(qxz, Dxxz, a.l1[0]);  a.l0b = fma(oxxz, Dxxz, a.l0b);
     const double Dxyy = fma(bxy, y, ax);
     const double Dxyz = bxy * z;
-    a.l3[3] = fma(m0, Dxyy, a.l3[3]);  a.l2[3] = fma(m1x, Dxyy, a.l2[3]);  a.l2[1] = fma(m1y, Dxyy, a.l2[1]);
+    a.l3[3] = fma(m0, Dxyy, a.l3[3]);  if (DIPOLE) a.l2[3] = fma(m1x, Dxyy, a.l2[3]);  if (DIPOLE) a.l2[1] = fma(m1y, Dxyy, a.l2[1]);
     a.l1[0] = fma(qyy, Dxyy, a.l1[0]);  a.l1[1] = fma(qxy, Dxyy, a.l1[1]);  a.l0 = fma(oxyy, Dxyy, a.l0);
-    a.l3[4] = fma(m0, Dxyz, a.l3[4]);  a.l2[4] = fma(m1x, Dxyz, a.l2[4]);  a.l2[2] = fma(m1y, Dxyz, a.l2[2]);
-    a.l2[1] = fma(m1z, Dxyz, a.l2[1]);  a.l1[0] = fma(qyz, Dxyz, a.l1[0]);  a.l1[1] = fma(qxz, Dxyz, a.l1[1]);
+    a.l3[4] = fma(m0, Dxyz, a.l3[4]);  if (DIPOLE) a.l2[4] = fma(m1x, Dxyz, a.l2[4]);  if (DIPOLE) a.l2[2] = fma(m1y, Dxyz, a.l2[2]);
+    if (DIPOLE) a.l2[1] = fma(m1z, Dxyz, a.l2[1]);  a.l1[0] = fma(qyz, Dxyz, a.l1[0]);  a.l1[1] = fma(qxz, Dxyz, a.l1[1]);
     a.l1[2] = fma(qxy, Dxyz, a.l1[2]);  a.l0b = fma(oxyz, Dxyz, a.l0b);
     const double Dyyy = fma(byy, y, ay3);
     const double Dyyz = fma(byy, z, az);
-    a.l3[5] = fma(m0, Dyyy, a.l3[5]);  a.l2[3] = fma(m1y, Dyyy, a.l2[3]);  a.l1[1] = fma(qyy, Dyyy, a.l1[1]);
+    a.l3[5] = fma(m0, Dyyy, a.l3[5]);  if (DIPOLE) a.l2[3] = fma(m1y, Dyyy, a.l2[3]);  a.l1[1] = fma(qyy, Dyyy, a.l1[1]);
     a.l0 = fma(oyyy, Dyyy, a.l0);
-    a.l3[6] = fma(m0, Dyyz, a.l3[6]);  a.l2[4] = fma(m1y, Dyyz, a.l2[4]);  a.l2[3] = fma(m1z, Dyyz, a.l2[3]);
+    a.l3[6] = fma(m0, Dyyz, a.l3[6]);  if (DIPOLE) a.l2[4] = fma(m1y, Dyyz, a.l2[4]);  if (DIPOLE) a.l2[3] = fma(m1z, Dyyz, a.l2[3]);
     a.l1[2] = fma(qyy, Dyyz, a.l1[2]);  a.l1[1] = fma(qyz, Dyyz, a.l1[1]);  a.l0b = fma(oyyz, Dyyz, a.l0b);
     const double Dxzz = -(Dxxx + Dxyy);
     const double Dyzz = -(Dxxy + Dyyy);
-    a.l2[2] = fma(m1z, Dxzz, a.l2[2]);  a.l1[2] = fma(qxz, Dxzz, a.l1[2]);
-    a.l2[4] = fma(m1z, Dyzz, a.l2[4]);  a.l1[2] = fma(qyz, Dyzz, a.l1[2]);
+    if (DIPOLE) a.l2[2] = fma(m1z, Dxzz, a.l2[2]);  a.l1[2] = fma(qxz, Dxzz, a.l1[2]);
+    if (DIPOLE) a.l2[4] = fma(m1z, Dyzz, a.l2[4]);  a.l1[2] = fma(qyz, Dyzz, a.l1[2]);
 
     double n0 = 0.0, n1 = 0.0, n2 = 0.0, n3 = 0.0, n4 = 0.0, n5 = 0.0, n6 = 0.0;
     if (CORR) {

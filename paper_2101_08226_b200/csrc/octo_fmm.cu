@@ -286,6 +286,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.reach = h->reach;
     h->outL = h->L; h->outC = h->C;
     P.S = h->src; P.L = h->L; P.C = h->C; P.flags = h->flags;
+    P.force_dipole = 0;
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
         // ---- TMA descriptor of S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
@@ -329,8 +330,9 @@ int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com
     const Params& P = h->prm;
     if (h->cfg.kind == OCTO_FMM_MULTIPOLE) {
         const long long ncell = (long long)P.nx * P.ny * P.nz;
+        if (cudaMemsetAsync(h->flags + 1, 0, sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
         stage_multipole_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(moments, com_off, h->src, P.nx, P.ny, P.nz,
-                                                                                       0, P.nz);
+                                                                                       0, P.nz, h->cfg.h, h->flags);
     } else {
         const long long pc = (long long)(P.nx + 2 * REACH_MAX) * (P.ny + 2 * REACH_MAX) * (P.nz + 2 * REACH_MAX);
         stage_monopole_kernel<<<(unsigned)((pc + 255) / 256), 256, 0, h->stream>>>(moments, h->src, P.nx, P.ny, P.nz);
@@ -440,6 +442,18 @@ int octo_fmm_status(octo_fmm_t* h)
     return (f & 1) ? OCTO_FMM_EMASS : OCTO_FMM_OK;
 }
 
+int octo_fmm_dipole_terms_used(octo_fmm_t* h, int* used)
+{
+    if (!h || !used) return OCTO_FMM_EINVAL;
+    if (h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
+    if (h->state < 1) return OCTO_FMM_ESTATE;
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    int f = 0;
+    if (cudaMemcpy(&f, h->flags + 1, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
+    *used = (h->prm.force_dipole || (f & 2)) ? 1 : 0;
+    return OCTO_FMM_OK;
+}
+
 int octo_fmm_destroy(octo_fmm_t* h)
 {
     if (!h) return OCTO_FMM_EINVAL;
@@ -499,7 +513,7 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
     const size_t oplane = (size_t)P.ox * P.oy, ocell = oplane * P.oz;
     cudaStream_t sm = h->stream;
 #define OCTO_TRY(call) do { if ((call) != cudaSuccess) return OCTO_FMM_ECUDA; } while (0)
-    OCTO_TRY(cudaMemsetAsync(h->flags, 0, sizeof(int), sm));
+    OCTO_TRY(cudaMemsetAsync(h->flags, 0, 2 * sizeof(int), sm));
     if (upload_tables(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     OCTO_TRY(cudaEventRecord(h->ev_begin, sm));            // the copies start after earlier work on the caller's stream
     OCTO_TRY(cudaStreamWaitEvent(h->s_h2d, h->ev_begin, 0));
@@ -522,7 +536,7 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
         if (need > brought) {
             const long long n = (long long)(need - brought) * (long long)plane;
             stage_multipole_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(d_m, d_c, h->src, P.nx, P.ny, P.nz, brought,
-                                                                                 need - brought);
+                                                                                 need - brought, h->cfg.h, h->flags);
             OCTO_TRY(cudaGetLastError());
             brought = need;
         }
@@ -597,6 +611,11 @@ int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
         if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
         if (value == 0 && (h->cfg.n[0] % 8 || h->cfg.n[1] % 8 || h->cfg.n[2] % 8)) return OCTO_FMM_EINVAL;
         h->kernel = value;
+        return OCTO_FMM_OK;
+    }
+    if (!std::strcmp(key, "dipole_terms")) {     // 0 = decided on the device from the staged sources (default), 1 = always
+        if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
+        h->prm.force_dipole = value;
         return OCTO_FMM_OK;
     }
     if (!std::strcmp(key, "host_chunk")) {       // z-layers per run_host pipeline slab; 0 = one copy, one launch
@@ -693,7 +712,7 @@ int octo_fmm_fp64_issue_probe(int device, void* stream, void* scratch, int mode,
     return OCTO_FMM_OK;
 }
 
-int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int* fp64_instructions)
+int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int* flops, int* fp64_instructions)
 {
     // Counted from the operation list of m2l_pair<> + the separation.
     int f, i;
@@ -701,10 +720,16 @@ int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int*
     else if (kind == OCTO_FMM_MULTIPOLE) {
         if (am_correction) { f = 301; i = 178; }   // 123 DFMA + 43 DMUL + 12 DADD
         else               { f = 201; i = 117; }   //  84 DFMA + 26 DMUL +  7 DADD
+        if (!dipole_terms) { f -= 56; i -= 28; }   // 27 dipole FMAs and the FMA of D2_zz
     } else return OCTO_FMM_EINVAL;
     if (flops) *flops = f;
     if (fp64_instructions) *fp64_instructions = i;
     return OCTO_FMM_OK;
+}
+
+int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int* fp64_instructions)
+{
+    return octo_fmm_flops_per_interaction_path(kind, am_correction, 1, flops, fp64_instructions);
 }
 
 }  // extern "C"

@@ -27,16 +27,20 @@ def env():
     return p, torch
 
 
-def gpu_multipole(env, w, theta=None, correction=True, kernel=0, out_lo=None, out_hi=None):
+def gpu_multipole(env, w, theta=None, correction=True, kernel=0, out_lo=None, out_hi=None, dipole_terms=0,
+                  expect_dipole_path=None):
     p, torch = env
     theta = w.theta if theta is None else theta
     out_lo = w.out_lo if out_lo is None else out_lo
     out_hi = w.out_hi if out_hi is None else out_hi
     f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, correction, out_lo, out_hi)
     f.set_option("kernel", kernel)
+    f.set_option("dipole_terms", dipole_terms)
     mom = torch.from_numpy(w.moments).cuda()
     com = torch.from_numpy(w.com_off).cuda()
     L, Lc = f.solve(mom, com)
+    if expect_dipole_path is not None:
+        assert f.dipole_terms_used() == expect_dipole_path
     torch.cuda.synchronize()
     assert f.status() == p.OK
     cnt = f.interaction_count()
@@ -360,3 +364,33 @@ def test_monopole_non_cubic_grid_and_sub_region(env):
         assert g.interaction_count() == cnt
         assert parity_error(out.cpu().numpy(), ref) < TOL
         g.close()
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_dipole_terms_are_left_out_only_when_every_cell_has_none(env, kernel):
+    """The device decides at staging: centre-of-mass expansions (|M1| ~ 1e-19 m h here) take the path without the
+    27 dipole terms, forcing the general path changes the result by round-off only, and sources with real dipole
+    moments (expansion centres moved off the centres of mass) make the kernel evaluate them -- all three agree
+    with the oracle, which always keeps the terms."""
+    w = fi.config1()
+    assert np.abs(w.moments[1:4]).max() < 1e-17 * np.abs(w.moments[0]).max() * w.h * 10
+    Lr, Lcr, _ = oracle.interact_multipole(w.n, w.h, w.theta, w.moments, w.com_off, w.out_lo, w.out_hi, True)
+    L0, Lc0, _, _ = gpu_multipole(env, w, kernel=kernel, expect_dipole_path=False)
+    L1, Lc1, _, _ = gpu_multipole(env, w, kernel=kernel, dipole_terms=1, expect_dipole_path=True)
+    check(L0, Lc0, Lr, Lcr)
+    check(L1, Lc1, Lr, Lcr)
+    assert parity_error(L0, L1) < 1e-14
+    # one single cell with a dipole moment far from the output region is enough to switch the whole launch
+    w2 = fi.config1()
+    w2.moments[1, 2, 21, 3] = 1e-6 * w2.moments[0, 2, 21, 3] * w2.h
+    Lr2, Lcr2, _ = oracle.interact_multipole(w2.n, w2.h, w2.theta, w2.moments, w2.com_off, w2.out_lo, w2.out_hi, True)
+    L2, Lc2, _, _ = gpu_multipole(env, w2, kernel=kernel, expect_dipole_path=True)
+    check(L2, Lc2, Lr2, Lcr2)
+    # dipoles everywhere, of the size an expansion about the geometric centre would have
+    w3 = fi.config1()
+    rng = np.random.default_rng(3)
+    w3.moments[1:4] = rng.uniform(-0.1, 0.1, w3.moments[1:4].shape) * w3.moments[0] * w3.h
+    Lr3, Lcr3, _ = oracle.interact_multipole(w3.n, w3.h, w3.theta, w3.moments, w3.com_off, w3.out_lo, w3.out_hi, True)
+    L3, Lc3, _, _ = gpu_multipole(env, w3, kernel=kernel, expect_dipole_path=True)
+    check(L3, Lc3, Lr3, Lcr3)
+    assert parity_error(L3, Lr) > 1e-6                         # the dipoles matter: the test is sensitive
