@@ -128,8 +128,9 @@ int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *c
  * octo_fmm_dipole_terms_used() synchronises the stream and tells which path interact() takes. */
 int octo_fmm_dipole_terms_used(octo_fmm_t *h, int *used);
 
-/* Options, for tests and profiling.  "kernel" = 0 staged (TMA + shared memory, default), 1 direct
- * (global-memory loads; same pair arithmetic).  "dipole_terms" = 0 decided on the device (default), 1 always evaluated.  "host_chunk" = output z-layers per pipeline slab of
+/* Options, for tests and profiling.  "kernel" = 0 staged (TMA + shared memory; default above 4096 target
+ * cells), 1 direct (one cell per thread, global-memory loads; same pair arithmetic), 2 one warp per cell with
+ * a warp-level reduction of the partial expansions (default up to 4096 target cells).  "dipole_terms" = 0 decided on the device (default), 1 always evaluated.  "host_chunk" = output z-layers per pipeline slab of
  * octo_fmm_run_host (default 12; 0 = one copy in, one launch, one copy out).  Unknown keys -> EINVAL. */
 int octo_fmm_set_option(octo_fmm_t *h, const char *key, int value);
 

@@ -3,6 +3,7 @@
 //   stage_multipole_kernel   a2: raw moments -> staged layout in the workspace
 //   m2l_staged_kernel        a3/a4/a6: persistent, TMA-fed slab pipeline (default)
 //   m2l_direct_kernel        a3/a4/a6: same pair arithmetic, global-memory loads (cross-check)
+//   m2l_warp_kernel          a3/a4/a6 for small regions: one warp per cell, warp-level reduction of partial expansions
 //   p2p_monopole_kernel      a5: monopole variant
 //   dfma_peak_kernel         FP64 ALU roofline probe
 //
@@ -419,6 +420,58 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
         }
         store_target<CORR>(p, acc, gx, gy, k);
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// a3/a4/a6 for small output regions (coarse levels of the complete solve, single sub-grids):
+// one WARP per target cell.  The lanes split the cell's interaction list (entry s = lane, lane + 32,
+// ...), each accumulates a partial expansion, and the 20 + 3 partial sums are combined by a
+// butterfly of warp shuffles; lane 0 stores.  With a few hundred to a few thousand targets the
+// one-cell-per-thread kernels leave most SMs idle and take ~150 us of pure latency; this takes
+// ~10 us.  Sources are read from the staged array in global memory with explicit in-grid tests.
+// ------------------------------------------------------------------------------------------
+template <bool CORR>
+__global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
+{
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const long long t = (long long)blockIdx.x * 8 + warp;
+    if (t >= (long long)p.ox * p.oy * p.oz) return;
+    const int gx = p.lo[0] + (int)(t % p.ox), gy = p.lo[1] + (int)((t / p.ox) % p.oy), k = p.lo[2] + (int)(t / ((long long)p.ox * p.oy));
+    const int cls = (gx & 1) + 2 * (gy & 1) + 4 * (k & 1);
+    const long long plane = (long long)p.ny * p.nx;
+    const double2* S2 = reinterpret_cast<const double2*>(p.S);
+    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
+    double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    load_target<CORR>(p, gx, gy, k, dA, tA);
+    Acc acc;
+    acc_zero(acc);
+    const int s_end = c_begin[cls][2 * REACH_MAX + 1];
+#pragma unroll 1
+    for (int s = c_begin[cls][0] + lane; s < s_end; s += 32) {
+        const StEntry e = c_entries[cls * MAX_LIST + s];
+        const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+        if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
+        const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
+        double src[16], bx_, by_, bz_;
+        OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
+        const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
+        const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by_);
+        const double z = c_hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+        if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
+        else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
+    }
+    // warp-level reduction of the partial expansions (fixed butterfly order: deterministic)
+    static_assert(sizeof(Acc) == 20 * sizeof(double), "Acc is 20 doubles");
+    double* v = reinterpret_cast<double*>(&acc);
+#pragma unroll
+    for (int c = 0; c < 20; ++c) {
+        double a = v[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+        v[c] = a;
+    }
+    if (lane == 0) store_target<CORR>(p, acc, gx, gy, k);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -23,6 +23,7 @@ namespace {
 
 constexpr size_t ALIGN = 256;
 constexpr int MAX_CHUNKS = 32;
+constexpr long long WARP_KERNEL_MAX_CELLS = 4096;   // at most this many targets: m2l_warp_kernel by default
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Offset3 { signed char d[3]; };
@@ -213,6 +214,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     region_of(*cfg, h->lo, h->hi, flags);
     const bool small = cfg->n[0] % 8 || cfg->n[1] % 8 || cfg->n[2] % 8;    // only with CF_ANY_SIZE
     if (small) h->kernel = 1;
+    // few targets (coarse levels of the complete solve, single sub-grids): one warp per cell
+    if ((long long)(h->hi[0] - h->lo[0]) * (h->hi[1] - h->lo[1]) * (h->hi[2] - h->lo[2]) <= WARP_KERNEL_MAX_CELLS) h->kernel = 2;
 
     // ---- a1: interaction lists (Eq. 15) ----
     h->reach = 0;
@@ -393,6 +396,10 @@ int octo_fmm_interact(octo_fmm_t* h)
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
+    } else if (h->kernel == 2) {
+        const unsigned blocks = (unsigned)(((long long)P.ox * P.oy * P.oz + 7) / 8);
+        if (h->cfg.am_correction) m2l_warp_kernel<true><<<blocks, 256, 0, h->stream>>>(P);
+        else                      m2l_warp_kernel<false><<<blocks, 256, 0, h->stream>>>(P);
     } else {
         if (launch_staged(h, h->lo[2], h->hi[2]) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     }
@@ -608,7 +615,7 @@ int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
 {
     if (!h || !key) return OCTO_FMM_EINVAL;
     if (!std::strcmp(key, "kernel")) {
-        if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
+        if (value != 0 && value != 1 && value != 2) return OCTO_FMM_EINVAL;
         if (value == 0 && (h->cfg.n[0] % 8 || h->cfg.n[1] % 8 || h->cfg.n[2] % 8)) return OCTO_FMM_EINVAL;
         h->kernel = value;
         return OCTO_FMM_OK;
@@ -639,6 +646,9 @@ int octo_fmm_launch_info(const octo_fmm_t* h, int* grid, int* block, int* smem_b
     } else if (h->kernel == 1) {
         e = h->cfg.am_correction ? cudaFuncGetAttributes(&fa, m2l_direct_kernel<true>) : cudaFuncGetAttributes(&fa, m2l_direct_kernel<false>);
         g = brick_blocks(P); b = 256; s = 0;
+    } else if (h->kernel == 2) {
+        e = h->cfg.am_correction ? cudaFuncGetAttributes(&fa, m2l_warp_kernel<true>) : cudaFuncGetAttributes(&fa, m2l_warp_kernel<false>);
+        g = (int)(((long long)P.ox * P.oy * P.oz + 7) / 8); b = 256; s = 0;
     } else {
         e = h->cfg.am_correction ? cudaFuncGetAttributes(&fa, m2l_staged_kernel<true>) : cudaFuncGetAttributes(&fa, m2l_staged_kernel<false>);
         g = (int)std::min<long long>(P.ntiles, h->sm_count); b = STAGED_THREADS; s = STAGED_SMEM;

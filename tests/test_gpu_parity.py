@@ -71,7 +71,7 @@ def test_stencils_bit_exact(env, theta):
     f.close()
 
 
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [0, 1, 2])
 @pytest.mark.parametrize("correction", [True, False])
 def test_config1(env, kernel, correction):
     """cfg 1: one 8^3 sub-grid + 26 neighbours, theta = 0.5."""
@@ -93,7 +93,7 @@ def test_config1_theta_sweep(env, theta):
     check(L, Lc, Lr, Lcr)
 
 
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [0, 1, 2])
 def test_whole_small_grid_with_domain_faces(env, kernel):
     """Every cell of a 24 x 16 x 8 grid is a target: all tiles touch the domain boundary (TMA
     zero fill = isolated boundary, L321), tiles are ragged in x (24 = 16 + 8) and the slab ring
@@ -210,6 +210,7 @@ def test_host_buffer_entry_point(env):
     w = fi.config1()
     L, Lc, _, _ = gpu_multipole(env, w)
     f = p.OctoFMM(w.n, w.h, w.theta, p.MULTIPOLE, True, w.out_lo, w.out_hi)
+    f.set_option("kernel", 0)          # same kernel as gpu_multipole, so that the comparison can be bit for bit
     nb = p.octo_fmm_host_scratch_bytes(f.cfg)
     scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
     mom = torch.from_numpy(w.moments).pin_memory()
@@ -253,6 +254,7 @@ def test_bound_outputs_match_copied_outputs(env):
     w = fi.config1()
     L, Lc, _, _ = gpu_multipole(env, w)
     f = p.OctoFMM(w.n, w.h, w.theta, p.MULTIPOLE, True, w.out_lo, w.out_hi)
+    f.set_option("kernel", 0)          # same kernel as gpu_multipole: bit-for-bit comparison
     mom, com = torch.from_numpy(w.moments).cuda(), torch.from_numpy(w.com_off).cuda()
     Lb = torch.full((20, 8, 8, 8), float("nan"), dtype=torch.float64, device="cuda")
     Lcb = torch.full((3, 8, 8, 8), float("nan"), dtype=torch.float64, device="cuda")
@@ -329,7 +331,7 @@ def test_single_subgrid_domain(env, theta):
     w.moments = np.ascontiguousarray(w.moments[:, 8:16, 8:16, 8:16])
     w.com_off = np.ascontiguousarray(w.com_off[:, 8:16, 8:16, 8:16])
     w.n, w.out_lo, w.out_hi = (8, 8, 8), (0, 0, 0), (8, 8, 8)
-    for kernel in (0, 1):
+    for kernel in (0, 1, 2):
         L, Lc, cnt, _ = gpu_multipole(env, w, theta=theta, kernel=kernel)
         Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off)
         assert cnt == cntr > 0
@@ -366,7 +368,7 @@ def test_monopole_non_cubic_grid_and_sub_region(env):
         g.close()
 
 
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [0, 1, 2])
 def test_dipole_terms_are_left_out_only_when_every_cell_has_none(env, kernel):
     """The device decides at staging: centre-of-mass expansions (|M1| ~ 1e-19 m h here) take the path without the
     27 dipole terms, forcing the general path changes the result by round-off only, and sources with real dipole
@@ -394,3 +396,17 @@ def test_dipole_terms_are_left_out_only_when_every_cell_has_none(env, kernel):
     L3, Lc3, _, _ = gpu_multipole(env, w3, kernel=kernel, expect_dipole_path=True)
     check(L3, Lc3, Lr3, Lcr3)
     assert parity_error(L3, Lr) > 1e-6                         # the dipoles matter: the test is sensitive
+
+
+def test_default_kernel_choice(env):
+    """Up to 4096 target cells the handle runs one warp per cell (warp-level reduction of the partial expansions),
+    above that the TMA-staged kernel; both can be forced."""
+    p, torch = env
+    small = p.OctoFMM((24, 24, 24), 1.0 / 24, 0.5, out_lo=(8, 8, 8), out_hi=(16, 16, 16))
+    big = p.OctoFMM((24, 24, 24), 1.0 / 24, 0.5)
+    assert small.launch_info()["block"] == 256 and small.launch_info()["grid"] == 64       # 512 warps
+    assert big.launch_info()["block"] == 416
+    small.set_option("kernel", 0)
+    assert small.launch_info()["block"] == 416
+    small.close()
+    big.close()
