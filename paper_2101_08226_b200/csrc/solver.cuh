@@ -12,18 +12,19 @@
 
 namespace octo {
 
-// unique-component index of a symmetric rank-2 / rank-3 tensor, lexicographic order
-__host__ __device__ constexpr int u2(int i, int j)
+// unique-component index of a symmetric rank-2 / rank-3 tensor, lexicographic order.  Non-recursive on
+// purpose: in fully unrolled loops the compiler folds them to constants (a recursive constexpr is called at run
+// time in device code and turns every tensor into a local-memory array).
+__host__ __device__ __forceinline__ constexpr int u2(int i, int j)
 {
-    return i > j ? u2(j, i) : (i == 0 ? j : (i == 1 ? 2 + j : 5));
+    return (i < j ? i : j) * 3 - ((i < j ? i : j) * ((i < j ? i : j) - 1)) / 2 + ((i < j ? j : i) - (i < j ? i : j));
 }
-__host__ __device__ constexpr int u3s(int i, int j, int k)   // i <= j <= k
+__host__ __device__ __forceinline__ constexpr int u3(int i, int j, int k)
 {
-    return i == 0 ? (j == 0 ? k : (j == 1 ? 2 + k : 5)) : (i == 1 ? (j == 1 ? 5 + k : 8) : 9);
-}
-__host__ __device__ constexpr int u3(int i, int j, int k)
-{
-    return i > j ? u3(j, i, k) : (j > k ? u3(i, k, j) : u3s(i, j, k));
+    // a <= b <= c the sorted indices
+    return u2((i + j + k) - (i < j ? (i < k ? i : k) : (j < k ? j : k)) - (i > j ? (i > k ? i : k) : (j > k ? j : k)),
+              (i > j ? (i > k ? i : k) : (j > k ? j : k))) +
+           ((i < j ? (i < k ? i : k) : (j < k ? j : k)) == 0 ? 0 : ((i < j ? (i < k ? i : k) : (j < k ? j : k)) == 1 ? 3 : 4));
 }
 static_assert(u2(0, 0) == 0 && u2(1, 0) == 1 && u2(0, 2) == 2 && u2(1, 1) == 3 && u2(2, 1) == 4 && u2(2, 2) == 5, "u2");
 static_assert(u3(0, 0, 0) == 0 && u3(0, 1, 0) == 1 && u3(2, 0, 0) == 2 && u3(1, 0, 1) == 3 && u3(2, 1, 0) == 4 &&
