@@ -528,7 +528,6 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
     double* const keepL = h->outL; double* const keepC = h->outC;
     h->outL = d_L; h->outC = d_C;
     int brought = std::max(P.lo[2] - h->reach, 0);         // source layers [.., brought) are on the device
-    const int first_layer = brought;
     int rc = OCTO_FMM_OK;
     for (int c = 0; c < nchunk && rc == OCTO_FMM_OK; ++c) {
         const int a = P.lo[2] + c * zc, b = std::min(a + zc, P.hi[2]);
@@ -556,7 +555,6 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
         if (C_h)
             OCTO_TRY(cudaMemcpy2DAsync(C_h + ooff, ocell * 8, d_C + ooff, ocell * 8, owidth, 3, cudaMemcpyDeviceToHost, h->s_d2h));
     }
-    (void)first_layer;
     h->outL = keepL; h->outC = keepC;
     if (rc != OCTO_FMM_OK) return rc;
     OCTO_TRY(cudaEventRecord(h->ev_end, h->s_d2h));

@@ -410,3 +410,47 @@ def test_default_kernel_choice(env):
     assert small.launch_info()["block"] == 416
     small.close()
     big.close()
+
+
+def test_large_grid_400_sampled(env):
+    """A grid larger than any BASELINE configuration (400^3 = 64 M cells, about 46 GB on the device; 400 is not a
+    power of two and leaves ragged bricks in z): sources are generated on the device, and sampled 16^3 regions are
+    recomputed by the oracle from their 28^3 neighbourhoods (6 >= reach cells of halo, even-aligned so that the
+    parities agree; clipped at the domain faces)."""
+    p, torch = env
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9:
+        pytest.skip("needs 60 GB of free device memory")
+    n, h = 400, 1.0 / 400
+    g = torch.Generator(device="cuda").manual_seed(400)
+    mom = torch.rand((20, n, n, n), dtype=torch.float64, device="cuda", generator=g)
+    mom[1:] -= 0.5
+    mom[0] += 0.5
+    mom[1:4] *= 1e-3 * h                       # real dipoles: the general path runs
+    mom[4:10] *= 0.1 * h * h
+    mom[10:20] *= 0.05 * h ** 3
+    mom *= h ** 3
+    com = (torch.rand((3, n, n, n), dtype=torch.float64, device="cuda", generator=g) - 0.5) * (0.2 * h)
+    f = p.OctoFMM((n, n, n), h, 0.5, p.MULTIPOLE, True)
+    L = torch.empty((20, n, n, n), dtype=torch.float64, device="cuda")
+    Lc = torch.empty((3, n, n, n), dtype=torch.float64, device="cuda")
+    f.bind_outputs(L, Lc)
+    f.set_moments(mom, com)
+    f.interact()
+    assert f.status() == p.OK and f.dipole_terms_used()
+    assert f.interaction_count() == oracle.interaction_count((n, n, n), 0.5)
+    for lo in ((0, 0, 0), (384, 384, 384), (192, 0, 384), (208, 176, 96), (384, 192, 192)):
+        blo = [max(v - 6, 0) for v in lo]
+        bhi = [min(v + 22, n) for v in lo]
+        sl = (slice(None), slice(blo[2], bhi[2]), slice(blo[1], bhi[1]), slice(blo[0], bhi[0]))
+        bm, bc = mom[sl].cpu().numpy().copy(), com[sl].cpu().numpy().copy()
+        bn = tuple(bhi[a] - blo[a] for a in range(3))
+        olo = tuple(lo[a] - blo[a] for a in range(3))
+        ohi = tuple(olo[a] + 16 for a in range(3))
+        Lr, Lcr, _ = oracle.interact_multipole(bn, h, 0.5, bm, bc, olo, ohi, True)
+        osl = (slice(None), slice(lo[2], lo[2] + 16), slice(lo[1], lo[1] + 16), slice(lo[0], lo[0] + 16))
+        check(L[osl].cpu().numpy(), Lc[osl].cpu().numpy(), Lr, Lcr)
+    f.close()
+    del mom, com, L, Lc
+    torch.cuda.empty_cache()
