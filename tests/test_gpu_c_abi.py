@@ -1,0 +1,46 @@
+"""The boundary really is a C ABI: a plain C client (tests/c_abi_client.c: include/octo_fmm.h + the CUDA runtime, no
+Python, no torch) runs cfg 1 through the shared library and its output is compared with the oracle."""
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+
+import fmm_inputs as fi
+import oracle
+from helpers import parity_error
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_plain_c_client(tmp_path):
+    import torch
+    assert torch.cuda.is_available()
+    if shutil.which("nvcc") is None:
+        pytest.skip("nvcc not on PATH")
+    from paper_2101_08226_b200 import build
+    build.build()
+    libdir = os.path.join(ROOT, "paper_2101_08226_b200")
+    exe = str(tmp_path / "c_abi_client")
+    subprocess.run(["nvcc", "-O1", "-x", "cu", "-I", os.path.join(ROOT, "include"), os.path.join(ROOT, "tests", "c_abi_client.c"),
+                    "-o", exe, "-L", libdir, "-locto_fmm", "-Xlinker", "-rpath", "-Xlinker", libdir], check=True)
+    w = fi.config1()
+    inp, outp = str(tmp_path / "in.bin"), str(tmp_path / "out.bin")
+    with open(inp, "wb") as f:
+        np.array(list(w.n) + list(w.out_lo) + list(w.out_hi) + [1], dtype=np.int32).tofile(f)
+        np.array([w.h, w.theta], dtype=np.float64).tofile(f)
+        w.moments.astype(np.float64).tofile(f)
+        w.com_off.astype(np.float64).tofile(f)
+    r = subprocess.run([exe, inp, outp], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+    raw = np.fromfile(outp, dtype=np.uint8)
+    ocell = 8 * 8 * 8
+    vals = raw[:ocell * 23 * 8].view(np.float64)
+    count = int(raw[ocell * 23 * 8:ocell * 23 * 8 + 8].view(np.uint64)[0])
+    nst = int(raw[ocell * 23 * 8 + 8:ocell * 23 * 8 + 12].view(np.int32)[0])
+    L, Lc = vals[:ocell * 20].reshape(20, 8, 8, 8), vals[ocell * 20:].reshape(3, 8, 8, 8)
+    Lr, Lcr, cnt = oracle.interact_multipole(w.n, w.h, w.theta, w.moments, w.com_off, w.out_lo, w.out_hi, True)
+    assert count == cnt == 118272 and nst == 231
+    assert parity_error(L, Lr) < 1e-12 and parity_error(Lc, Lcr) < 1e-11
