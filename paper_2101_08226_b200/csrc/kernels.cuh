@@ -55,7 +55,6 @@ struct StEntry {
 __constant__ StEntry c_entries[8 * MAX_LIST];
 __constant__ int c_begin[8][2 * REACH_MAX + 2];   // first entry of (class, dz); [..][11] = end
 __constant__ double c_hmul[2 * REACH_MAX + 1];    // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h)
-__constant__ double2 c_mono_rad[3 * REACH_MAX * REACH_MAX + 1];   // monopole: {-1/r, -1/r^3}, r = sqrt(d2) h, by d2 = |Delta|^2
 
 struct Params {
     int nx, ny, nz;
@@ -476,8 +475,8 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
 
 // ------------------------------------------------------------------------------------------
 // a5: monopole (leaf) variant.  R = (i_A - i_B) h has no per-cell part, so -1/|R| and
-// -R/|R|^3 depend on the list entry only: -1/r and -1/r^3 are tabulated by |Delta|^2 on the host
-// in FP64 (constant memory) and the kernel is a 4-FMA stencil sum.
+// -R/|R|^3 depend on the offset Delta only: they are tabulated for the 11^3 offsets on the host
+// in FP64 and the kernel is a 4-FMA stencil sum.
 // mass is zero-padded by REACH_MAX cells on every side: P[(nz+10)][(ny+10)][(nx+10)].
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __restrict__ mass, double* __restrict__ P,
@@ -494,36 +493,42 @@ __global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __res
     P[i] = in ? mass[((long long)z * ny + y) * nx + x] : 0.0;
 }
 
-constexpr int MT_X = 16, MT_Y = 16, MT_Z = 8;           // target tile of one block
+constexpr int MT_X = 16, MT_Y = 16, MT_Z = 16;          // target tile of one block
 constexpr int MS_X = MT_X + 2 * REACH_MAX, MS_Y = MT_Y + 2 * REACH_MAX, MS_Z = MT_Z + 2 * REACH_MAX;
 constexpr int MS_XH = 14;                               // half-row: 13 cells of one x-parity + 1 pad
 constexpr int MS_ROW = 2 * MS_XH;                       // 28 doubles: two tile rows are 64 bytes mod 128 apart
-constexpr int MONO_SMEM = MS_ROW * MS_Y * MS_Z * 8;     // 104832 B: two blocks per SM
-constexpr int MONO_THREADS = 256;
+constexpr int MONO_TILE_BYTES = MS_ROW * MS_Y * MS_Z * 8;                    // 151424 B
+constexpr int MONO_NW = (2 * REACH_MAX + 1) * (2 * REACH_MAX + 1) * (2 * REACH_MAX + 1);   // 1331 offsets Delta
+constexpr int MONO_SMEM = MONO_TILE_BYTES + MONO_NW * 32;                    // + 42592 B of weights = 194016 B
+constexpr int MONO_THREADS = 512;
+static_assert(MONO_SMEM <= 227 * 1024, "shared memory per CTA");
 
-// One block = a 16 x 16 x 8 target tile whose masses (tile + 5-cell halo) sit in shared memory,
-// every x-row de-interleaved into its even and odd cells (as the multipole slabs) and padded to 28
-// doubles, so that the 32 lanes of a warp (8 cells two apart in x, 4 rows two apart in y) read
-// 256 consecutive-bank bytes: two conflict-free wavefronts per LDS.64 instead of four.
-// Warp w holds xy-parity class w >> 1, rows 4 (w & 1) + {0..3} of that class; every thread owns one
-// (x, y) and all 8 layers: two passes (even z, odd z), 4 targets per pass that share the parity
-// class, hence the list and the weights -- one entry decode and 4 mass loads feed 16 DFMAs.
-// Measured bound (profiles/r01_monopole.md): instruction issue -- an FP64 instruction holds the
-// dispatch port for its 2-3 cycles, so the ~30 decode/load instructions per entry are not hidden
-// under the 19 FP64 ones (72 cycles per warp and entry = 128 interactions).
-__global__ void __launch_bounds__(MONO_THREADS, 2) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
-                                                                       double* __restrict__ out)
+// One block (16 warps, one per SM) = a 16 x 16 x 16 target tile.  Shared memory holds the masses of the tile + 5-cell
+// halo (every x-row de-interleaved into its even and odd cells and padded to 28 doubles: the 32 lanes of a warp --
+// 8 cells two apart in x, 4 rows two apart in y -- read 256 consecutive-bank bytes, two conflict-free wavefronts per
+// LDS.64) and the table of the weights (-1/|R|, -R/|R|^3) of all 11^3 offsets Delta (R = -Delta h has no per-cell
+// part; built on the host in FP64).  Warp w: xy-parity class (w >> 1) & 3, rows 4 (w & 1) + {0..3} of that class,
+// layers 8 (w >> 3) + {0..7}; a thread owns one (x, y) and 8 layers: two passes (even z, odd z) of 4 targets that
+// share the parity class, hence the list entry, its tile offset and its weights.  Per entry and warp: one constant
+// load (tile offset and weight index, packed on the host), two broadcast LDS.128 of the weights, four LDS.64 of the
+// masses, 16 DFMAs.
+__global__ void __launch_bounds__(MONO_THREADS, 1) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
+                                                                       const double4* __restrict__ Wg, double* __restrict__ out)
 {
-    extern __shared__ __align__(16) double tile[];
+    extern __shared__ __align__(16) unsigned char mono_smem[];
+    double* tile = reinterpret_cast<double*>(mono_smem);
+    double4* W = reinterpret_cast<double4*>(mono_smem + MONO_TILE_BYTES);
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
-    const int px = (warp >> 1) & 1, py = warp >> 2;
+    const int px = (warp >> 1) & 1, py = (warp >> 2) & 1, zg = warp >> 3;
     const int bx = (p.ox + MT_X - 1) / MT_X, by = (p.oy + MT_Y - 1) / MT_Y;
     const int b = blockIdx.x;
     const int x0 = p.lo[0] + (b % bx) * MT_X, y0 = p.lo[1] + ((b / bx) % by) * MT_Y, z0 = p.lo[2] + (b / (bx * by)) * MT_Z;
     const int X = p.nx + 2 * REACH_MAX, Y = p.ny + 2 * REACH_MAX, Z = p.nz + 2 * REACH_MAX;
 
+    for (int i = threadIdx.x; i < MONO_NW; i += MONO_THREADS) W[i] = Wg[i];
     // tile (x0-5 .. x0+20, ...) = padded coordinates (x0 .. x0+25, ...); beyond the padded array -> 0
+#pragma unroll 4
     for (int i = threadIdx.x; i < MS_X * MS_Y * MS_Z; i += MONO_THREADS) {
         const int tx = i % MS_X, r = i / MS_X, ty = r % MS_Y, tz = r / MS_Y;
         const int sx = x0 + tx, sy = y0 + ty, sz = z0 + tz;
@@ -540,8 +545,8 @@ __global__ void __launch_bounds__(MONO_THREADS, 2) p2p_monopole_kernel(const Par
 #pragma unroll 1
     for (int pz = 0; pz < 2; ++pz) {
         const int cls = (px + 2 * py) + 4 * pz;
-        // the entry offsets carry the x-parity part (host: e.off), the thread adds its own row and half-row index
-        const double* base = tile + ((pz + REACH_MAX) * MS_Y + (py + 2 * ly + REACH_MAX)) * MS_ROW + lx;
+        // the entry offsets carry the x-parity part (host: e.off), the thread adds its own layer, row and half-row index
+        const double* base = tile + ((8 * zg + pz + REACH_MAX) * MS_Y + (py + 2 * ly + REACH_MAX)) * MS_ROW + lx;
         double a[4][4];
 #pragma unroll
         for (int j = 0; j < 4; ++j)
@@ -550,15 +555,9 @@ __global__ void __launch_bounds__(MONO_THREADS, 2) p2p_monopole_kernel(const Par
         const int s_begin = cls * MAX_LIST + c_begin[cls][0], s_end = cls * MAX_LIST + c_begin[cls][2 * REACH_MAX + 1];
 #pragma unroll 2
         for (int s = s_begin; s < s_end; ++s) {
-            const StEntry e = c_entries[s];
-            const double* q = base + e.off;
-            // weights of this list entry: they depend on Delta only (R = -Delta h has no per-cell part)
-            const double2 rad = c_mono_rad[e.d2];
-            double4 w;
-            w.x = rad.x;
-            w.y = c_hmul[e.dx + REACH_MAX] * rad.y;
-            w.z = c_hmul[e.dy + REACH_MAX] * rad.y;
-            w.w = c_hmul[e.dz + REACH_MAX] * rad.y;
+            const int packed = c_entries[s].off;                 // low 16 bits: tile offset (signed), high 16: weight index
+            const double* q = base + (short)(packed & 0xffff);
+            const double4 w = W[packed >> 16];
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const double m = q[j * LAYER2];
@@ -570,7 +569,7 @@ __global__ void __launch_bounds__(MONO_THREADS, 2) p2p_monopole_kernel(const Par
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const int k = z0 + pz + 2 * j;
+            const int k = z0 + 8 * zg + pz + 2 * j;
             if (act_xy && k < p.hi[2]) {
                 const long long o = ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
 #pragma unroll

@@ -88,7 +88,7 @@ bool config_ok(const octo_fmm_config* c, int flags = 0)
     return true;
 }
 
-struct Sizes { size_t src, L, C, flags, total; };
+struct Sizes { size_t src, L, C, W, flags, total; };
 
 Sizes sizes_of(const octo_fmm_config& c, int flags = 0)
 {
@@ -106,9 +106,10 @@ Sizes sizes_of(const octo_fmm_config& c, int flags = 0)
         s.src = align_up(pc * sizeof(double));
         s.L = align_up(ocell * 4 * sizeof(double));
         s.C = 0;
+        s.W = align_up((size_t)MONO_NW * sizeof(double4));
     }
     s.flags = ALIGN;
-    s.total = s.src + s.L + s.C + s.flags;
+    s.total = s.src + s.L + s.C + s.W + s.flags;
     return s;
 }
 
@@ -141,7 +142,7 @@ struct octo_fmm {
     std::vector<StEntry> entries;          // 8 * MAX_LIST
     int begin[8][2 * REACH_MAX + 2];
     double hmul[2 * REACH_MAX + 1];
-    double2 mono_rad[3 * REACH_MAX * REACH_MAX + 1];   // monopole: {-1/r, -1/r^3} by |Delta|^2
+    double4* W;            // monopole: device table of the weights of the 11^3 offsets
     unsigned long long n_interactions;
     CUtensorMap tmap;
     Params prm;
@@ -242,9 +243,12 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
                 e.off = (py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1);   // double2 units
                 e.d2 = 0;
             } else {
-                // monopole: offset in the de-interleaved mass tile (doubles), see p2p_monopole_kernel
-                e.off = (dz * MS_Y + dy) * MS_ROW + (((px + dx + REACH_MAX) & 1) ? MS_XH : 0) + ((px + dx + REACH_MAX) >> 1);
-                e.d2 = (signed char)(dx * dx + dy * dy + dz * dz);    // <= 75: index of the radial table
+                // monopole: offset in the de-interleaved mass tile (doubles, low 16 bits) and index of the offset's
+                // weights (high 16 bits), see p2p_monopole_kernel
+                const int toff = (dz * MS_Y + dy) * MS_ROW + (((px + dx + REACH_MAX) & 1) ? MS_XH : 0) + ((px + dx + REACH_MAX) >> 1);
+                const int widx = ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
+                e.off = (toff & 0xffff) | (widx << 16);
+                e.d2 = (signed char)(dx * dx + dy * dy + dz * dz);
             }
             e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz;
             h->entries[(size_t)p * MAX_LIST + s] = e;
@@ -276,6 +280,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->src = (double*)w; w += sz.src;
     h->L = (double*)w;   w += sz.L;
     h->C = (double*)w;   w += sz.C;
+    h->W = (double4*)w;  w += sz.W;
     h->flags = (int*)w;
 
     Params& P = h->prm;
@@ -310,12 +315,20 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         if (e1 != cudaSuccess || e2 != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
     } else if (cfg->kind == OCTO_FMM_MONOPOLE) {
-        // ---- monopole radial table: -1/r and -1/r^3 by d2 = |Delta|^2, r = sqrt(d2) h (FP64 sqrt and division on
-        //      the host); the kernel forms -R/r^3 = ((i_A - i_B) h) * (-1/r^3) per list entry ----
-        for (int d2 = 0; d2 <= 3 * REACH_MAX * REACH_MAX; ++d2) {
-            const double r = std::sqrt((double)d2) * cfg->h;
-            h->mono_rad[d2] = d2 ? double2{-1.0 / r, -1.0 / (r * r * r)} : double2{0.0, 0.0};
-        }
+        // ---- monopole weights of the 11^3 offsets: (-1/|R|, -R/|R|^3) with R = (i_A - i_B) h = -Delta h, in FP64
+        //      on the host (sqrt, division); Delta = 0 gets zero weights ----
+        std::vector<double4> wt((size_t)MONO_NW, double4{0.0, 0.0, 0.0, 0.0});
+        for (int dz = -REACH_MAX; dz <= REACH_MAX; ++dz)
+            for (int dy = -REACH_MAX; dy <= REACH_MAX; ++dy)
+                for (int dx = -REACH_MAX; dx <= REACH_MAX; ++dx) {
+                    if (!dx && !dy && !dz) continue;
+                    const double Rx = h->hmul[dx + REACH_MAX], Ry = h->hmul[dy + REACH_MAX], Rz = h->hmul[dz + REACH_MAX];
+                    const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = std::sqrt(r2), ir3 = -1.0 / (r2 * r);
+                    const int widx = ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
+                    wt[widx] = double4{-1.0 / r, Rx * ir3, Ry * ir3, Rz * ir3};
+                }
+        if (cudaMemcpyAsync(h->W, wt.data(), wt.size() * sizeof(double4), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
+            cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
         if (cudaFuncSetAttribute(p2p_monopole_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MONO_SMEM) != cudaSuccess) {
             delete h; return OCTO_FMM_ECUDA;
         }
@@ -354,9 +367,6 @@ static int upload_tables(octo_fmm_t* h)
         return OCTO_FMM_ECUDA;
     if (cudaMemcpyToSymbolAsync(c_hmul, h->hmul, sizeof(h->hmul), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
-    if (h->cfg.kind == OCTO_FMM_MONOPOLE &&
-        cudaMemcpyToSymbolAsync(c_mono_rad, h->mono_rad, sizeof(h->mono_rad), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
-        return OCTO_FMM_ECUDA;
     g_const_owner = h;
     return OCTO_FMM_OK;
 }
@@ -392,7 +402,7 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(P, h->src, h->outL);
+        p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(P, h->src, h->W, h->outL);
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
