@@ -3,8 +3,8 @@
 //
 // Levels: the leaves (n^3 point masses, monopole kind with the leaf-level list = Eq. 15 list + near field) and
 // the multipole levels n/2, n/4, ..., 2 (the 2^3-cell level is the coarsest that can hold interacting cells:
-// siblings interact there when 3 theta^2 > 1).  Levels whose size is not a multiple of 8 (4^3, 2^3) run the
-// direct interaction kernel.  solve() = stage leaves -> M2M up -> per level, coarsest first: stage, interact,
+// siblings interact there when 3 theta^2 > 1).  Levels of at most 4096 cells (16^3 ... 2^3) run the one-warp-per-cell
+// interaction kernel, the finer ones the TMA-staged kernel.  solve() = stage leaves -> M2M up -> per level, coarsest first: stage, interact,
 // L2L -> leaf interaction + leaf evaluation.
 
 namespace {
