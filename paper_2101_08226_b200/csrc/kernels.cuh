@@ -477,20 +477,24 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
 // a5: monopole (leaf) variant.  R = (i_A - i_B) h has no per-cell part, so -1/|R| and
 // -R/|R|^3 depend on the offset Delta only: they are tabulated for the 11^3 offsets on the host
 // in FP64 and the kernel is a 4-FMA stencil sum.
-// mass is zero-padded by REACH_MAX cells on every side: P[(nz+10)][(ny+10)][(nx+10)].
+// The mass is staged zero-padded by REACH_MAX cells (x: 5 on the left, 7 on the right, so that a half-row is a
+// multiple of 16 bytes) and with every x-row de-interleaved into its even and odd cells:
+//   P[z + 5][y + 5][xpar][xh],  padded x = x + 5, xpar = padded x & 1, xh = padded x >> 1,  MONO_PADX = nx + 12
+// -- the layout the interaction kernel wants in shared memory, so that one TMA box brings a whole tile.
 // ------------------------------------------------------------------------------------------
+constexpr int MONO_PAD_RIGHT = REACH_MAX + 2;
 __global__ void __launch_bounds__(256) stage_monopole_kernel(const double* __restrict__ mass, double* __restrict__ P,
                                                              int nx, int ny, int nz)
 {
-    const int X = nx + 2 * REACH_MAX, Y = ny + 2 * REACH_MAX, Z = nz + 2 * REACH_MAX;
+    const int X = nx + REACH_MAX + MONO_PAD_RIGHT, Y = ny + 2 * REACH_MAX, Z = nz + 2 * REACH_MAX;
     const long long n = (long long)X * Y * Z;
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;     // padded cell index, x fastest
     if (i >= n) return;
-    const int x = (int)(i % X) - REACH_MAX;
+    const int xp = (int)(i % X);
     const long long r = i / X;
-    const int y = (int)(r % Y) - REACH_MAX, z = (int)(r / Y) - REACH_MAX;
+    const int x = xp - REACH_MAX, y = (int)(r % Y) - REACH_MAX, z = (int)(r / Y) - REACH_MAX;
     const bool in = x >= 0 && y >= 0 && z >= 0 && x < nx && y < ny && z < nz;
-    P[i] = in ? mass[((long long)z * ny + y) * nx + x] : 0.0;
+    P[r * X + (xp & 1) * (X >> 1) + (xp >> 1)] = in ? mass[((long long)z * ny + y) * nx + x] : 0.0;
 }
 
 constexpr int MT_X = 16, MT_Y = 16, MT_Z = 16;          // target tile of one block
@@ -499,7 +503,7 @@ constexpr int MS_XH = 14;                               // half-row: 13 cells of
 constexpr int MS_ROW = 2 * MS_XH;                       // 28 doubles: two tile rows are 64 bytes mod 128 apart
 constexpr int MONO_TILE_BYTES = MS_ROW * MS_Y * MS_Z * 8;                    // 151424 B
 constexpr int MONO_NW = (2 * REACH_MAX + 1) * (2 * REACH_MAX + 1) * (2 * REACH_MAX + 1);   // 1331 offsets Delta
-constexpr int MONO_SMEM = MONO_TILE_BYTES + MONO_NW * 32;                    // + 42592 B of weights = 194016 B
+constexpr int MONO_SMEM = MONO_TILE_BYTES + MONO_NW * 32 + 64;               // + 42592 B of weights + mbarrier = 194080 B
 constexpr int MONO_THREADS = 512;
 static_assert(MONO_SMEM <= 227 * 1024, "shared memory per CTA");
 
@@ -512,10 +516,18 @@ static_assert(MONO_SMEM <= 227 * 1024, "shared memory per CTA");
 // share the parity class, hence the list entry, its tile offset and its weights.  Per entry and warp: one constant
 // load (tile offset and weight index, packed on the host), two broadcast LDS.128 of the weights, four LDS.64 of the
 // masses, 16 DFMAs.
-__global__ void __launch_bounds__(MONO_THREADS, 1) p2p_monopole_kernel(const Params p, const double* __restrict__ P,
+__device__ __forceinline__ void tma_load_tile3(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"((uint64_t)map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+
+__global__ void __launch_bounds__(MONO_THREADS, 1) p2p_monopole_kernel(const __grid_constant__ CUtensorMap tmap, const Params p,
                                                                        const double4* __restrict__ Wg, double* __restrict__ out)
 {
-    extern __shared__ __align__(16) unsigned char mono_smem[];
+    extern __shared__ __align__(128) unsigned char mono_smem[];
     double* tile = reinterpret_cast<double*>(mono_smem);
     double4* W = reinterpret_cast<double4*>(mono_smem + MONO_TILE_BYTES);
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
@@ -524,18 +536,20 @@ __global__ void __launch_bounds__(MONO_THREADS, 1) p2p_monopole_kernel(const Par
     const int bx = (p.ox + MT_X - 1) / MT_X, by = (p.oy + MT_Y - 1) / MT_Y;
     const int b = blockIdx.x;
     const int x0 = p.lo[0] + (b % bx) * MT_X, y0 = p.lo[1] + ((b / bx) % by) * MT_Y, z0 = p.lo[2] + (b / (bx * by)) * MT_Z;
-    const int X = p.nx + 2 * REACH_MAX, Y = p.ny + 2 * REACH_MAX, Z = p.nz + 2 * REACH_MAX;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(mono_smem + MONO_TILE_BYTES + MONO_NW * 32);
 
-    for (int i = threadIdx.x; i < MONO_NW; i += MONO_THREADS) W[i] = Wg[i];
-    // tile (x0-5 .. x0+20, ...) = padded coordinates (x0 .. x0+25, ...); beyond the padded array -> 0
-#pragma unroll 4
-    for (int i = threadIdx.x; i < MS_X * MS_Y * MS_Z; i += MONO_THREADS) {
-        const int tx = i % MS_X, r = i / MS_X, ty = r % MS_Y, tz = r / MS_Y;
-        const int sx = x0 + tx, sy = y0 + ty, sz = z0 + tz;
-        tile[r * MS_ROW + (tx & 1) * MS_XH + (tx >> 1)] =
-            (sx < X && sy < Y && sz < Z) ? P[((long long)sz * Y + sy) * X + sx] : 0.0;
+    // the tile (x0-5 .. x0+22, y0-5 .. y0+20, z0-5 .. z0+20 = staged coordinates x0.., y0.., z0..) is ONE TMA box
+    // {14, 52, 26} of the staged array [z][y * 2 + xpar][xh]; parts beyond the array are zero-filled
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_arrive_expect_tx(bar, MONO_TILE_BYTES);
+        tma_load_tile3(tile, &tmap, bar, x0 >> 1, 2 * y0, z0);
     }
-    __syncthreads();
+    for (int i = threadIdx.x; i < MONO_NW; i += MONO_THREADS) W[i] = Wg[i];
+    __syncthreads();                 // weights in place, barrier initialised
+    mbar_wait(bar, 0);               // tile in place
 
     const int lx = lane & 7, ly = ((warp & 1) << 2) + (lane >> 3);
     const int gx = x0 + px + 2 * lx, gy = y0 + py + 2 * ly;

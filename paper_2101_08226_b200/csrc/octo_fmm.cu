@@ -102,7 +102,7 @@ Sizes sizes_of(const octo_fmm_config& c, int flags = 0)
         s.L = align_up(ocell * 20 * sizeof(double));
         s.C = align_up(ocell * 3 * sizeof(double));
     } else {
-        const size_t pc = (size_t)(c.n[0] + 2 * REACH_MAX) * (c.n[1] + 2 * REACH_MAX) * (c.n[2] + 2 * REACH_MAX);
+        const size_t pc = (size_t)(c.n[0] + REACH_MAX + MONO_PAD_RIGHT) * (c.n[1] + 2 * REACH_MAX) * (c.n[2] + 2 * REACH_MAX);
         s.src = align_up(pc * sizeof(double));
         s.L = align_up(ocell * 4 * sizeof(double));
         s.C = 0;
@@ -329,6 +329,20 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
                 }
         if (cudaMemcpyAsync(h->W, wt.data(), wt.size() * sizeof(double4), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
             cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+        // ---- TMA descriptor of the staged masses P[z][y * 2 + xpar][xh] (see stage_monopole_kernel) ----
+        EncodeTiledFn enc = encode_tiled_fn();
+        if (!enc) { delete h; return OCTO_FMM_ECUDA; }
+        const cuuint64_t X = (cuuint64_t)cfg->n[0] + REACH_MAX + MONO_PAD_RIGHT, Y = (cuuint64_t)cfg->n[1] + 2 * REACH_MAX,
+                         Z = (cuuint64_t)cfg->n[2] + 2 * REACH_MAX;
+        cuuint64_t mdims[3] = {X / 2, 2 * Y, Z};
+        cuuint64_t mstrides[2] = {X / 2 * 8, X * Y * 8};
+        cuuint32_t mbox[3] = {MS_XH, 2 * MS_Y, MS_Z};
+        cuuint32_t mestr[3] = {1, 1, 1};
+        std::memset(&h->tmap, 0, sizeof(h->tmap));
+        if (enc(&h->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)h->src, mdims, mstrides, mbox, mestr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+            delete h; return OCTO_FMM_ECUDA;
+        }
         if (cudaFuncSetAttribute(p2p_monopole_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MONO_SMEM) != cudaSuccess) {
             delete h; return OCTO_FMM_ECUDA;
         }
@@ -350,7 +364,7 @@ int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com
         stage_multipole_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(moments, com_off, h->src, P.nx, P.ny, P.nz,
                                                                                        0, P.nz, h->cfg.h, h->flags);
     } else {
-        const long long pc = (long long)(P.nx + 2 * REACH_MAX) * (P.ny + 2 * REACH_MAX) * (P.nz + 2 * REACH_MAX);
+        const long long pc = (long long)(P.nx + REACH_MAX + MONO_PAD_RIGHT) * (P.ny + 2 * REACH_MAX) * (P.nz + 2 * REACH_MAX);
         stage_monopole_kernel<<<(unsigned)((pc + 255) / 256), 256, 0, h->stream>>>(moments, h->src, P.nx, P.ny, P.nz);
     }
     if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
@@ -402,7 +416,7 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(P, h->src, h->W, h->outL);
+        p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(h->tmap, P, h->W, h->outL);
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
