@@ -115,7 +115,8 @@ int octo_fmm_status(octo_fmm_t *h);
  * internal copy streams, so that the copy in of slab c+1, the kernels of slab c and the copy out of
  * slab c-1 overlap (pinned host buffers are needed for the overlap, not for correctness); every
  * layer crosses the bus once per direction.  Returns OCTO_FMM_EMASS if the correction met a target
- * mass <= 0.  Afterwards the handle is in the "sources staged" state.  scratch: device, >= octo_fmm_host_scratch_bytes(cfg) bytes, borrowed for the call. */
+ * mass <= 0.  Afterwards the handle is in the "sources staged" state.
+ * scratch: device, >= octo_fmm_host_scratch_bytes(cfg) bytes, borrowed for the call. */
 size_t octo_fmm_host_scratch_bytes(const octo_fmm_config *cfg);
 int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *com_off_host,
                       double *L_host, double *Lcorr_host, void *scratch, size_t scratch_bytes);
@@ -130,8 +131,10 @@ int octo_fmm_dipole_terms_used(octo_fmm_t *h, int *used);
 
 /* Options, for tests and profiling.  "kernel" = 0 staged (TMA + shared memory; default above 4096 target
  * cells), 1 direct (one cell per thread, global-memory loads; same pair arithmetic), 2 one warp per cell with
- * a warp-level reduction of the partial expansions (default up to 4096 target cells).  "dipole_terms" = 0 decided on the device (default), 1 always evaluated.  "host_chunk" = output z-layers per pipeline slab of
- * octo_fmm_run_host (default 12; 0 = one copy in, one launch, one copy out).  Unknown keys -> EINVAL. */
+ * a warp-level reduction of the partial expansions (default up to 4096 target cells).
+ * "dipole_terms" = 0 decided on the device (default), 1 always evaluated.
+ * "host_chunk" = output z-layers per pipeline slab of octo_fmm_run_host (default 12; 0 = one copy in, one
+ * launch, one copy out).  Unknown keys -> EINVAL. */
 int octo_fmm_set_option(octo_fmm_t *h, const char *key, int value);
 
 /* Launch facts of the interaction kernel the handle would run: grid, block, dynamic shared
