@@ -46,7 +46,9 @@ def test_workspace_sizing_and_validation(pkg):
     assert pkg.octo_fmm_host_scratch_bytes(ok) >= ncell * 8 * 46
     mono = pkg.make_config((128, 128, 128), 1.0 / 128, 0.5, kind=pkg.MONOPOLE)
     assert pkg.octo_fmm_workspace_bytes(mono) >= (138 ** 3 + 4 * 128 ** 3) * 8
-    for bad in (pkg.make_config((250, 256, 256), 1.0 / 256, 0.5),          # not a multiple of 8
+    for bad in (pkg.make_config((0, 256, 256), 1.0 / 256, 0.5),            # empty grid
+                pkg.make_config((-8, 8, 8), 1.0 / 8, 0.5),
+                pkg.make_config((250, 256, 256), 1.0 / 256, 0.5),          # not a multiple of 8
                 pkg.make_config((256, 256, 256), 1.0 / 256, 1.0 / 3.0),    # theta <= theta_min reach (L137)
                 pkg.make_config((256, 256, 256), 1.0 / 256, 1.0),
                 pkg.make_config((256, 256, 256), 0.0, 0.5),

@@ -60,7 +60,7 @@ def check(L, Lc, Lr, Lcr, tol=TOL):
     return e
 
 
-@pytest.mark.parametrize("theta", [0.5, 0.35, 0.34, 0.7, 0.4])
+@pytest.mark.parametrize("theta", [0.5, 0.35, 0.34, 0.334, 0.7, 0.4, 0.58, 0.9, 0.99])
 def test_stencils_bit_exact(env, theta):
     p, torch = env
     f = p.OctoFMM((24, 24, 24), 1.0 / 24, theta, out_lo=(8, 8, 8), out_hi=(16, 16, 16))
@@ -454,3 +454,14 @@ def test_large_grid_400_sampled(env):
     f.close()
     del mom, com, L, Lc
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("theta", [0.334, 0.9])
+def test_extreme_opening_angles(env, theta):
+    """Just above theta_min (largest lists, 651 cells, reach 5) and close to 1 (short lists in which siblings interact)."""
+    w = fi.config1(seed=13)
+    for kernel in (0, 2):
+        L, Lc, cnt, _ = gpu_multipole(env, w, theta=theta, kernel=kernel)
+        Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, w.out_lo, w.out_hi, True)
+        assert cnt == cntr
+        check(L, Lc, Lr, Lcr)
