@@ -131,6 +131,7 @@ EncodeTiledFn encode_tiled_fn()
 }
 
 const void* g_const_owner = nullptr;   // handle whose tables are in constant memory
+unsigned long long g_list_sig = 0;     // signature (theta, kind, list flavour, device) of the lists in constant memory
 
 }  // namespace
 
@@ -159,6 +160,7 @@ struct octo_fmm {
     int sm_count;
     cudaStream_t stream;
     // run_host pipeline (created on first use)
+    unsigned long long list_sig;   // identifies the contents of entries/begin (see upload_tables)
     int host_chunk;        // output z-layers per pipeline slab; 0 = no pipelining
     int host_launches;     // kernels the last run_host launched
     cudaStream_t s_h2d, s_d2h;
@@ -255,6 +257,13 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         }
     }
     for (int d = -REACH_MAX; d <= REACH_MAX; ++d) h->hmul[d + REACH_MAX] = (double)(-d) * cfg->h;
+    {
+        unsigned long long tb;
+        std::memcpy(&tb, &cfg->theta, sizeof tb);
+        h->list_sig = (tb * 0x9E3779B97F4A7C15ull) ^ ((unsigned long long)(cfg->kind + 1) << 8) ^ ((unsigned long long)((flags & CF_LEAF_LIST) ? 2 : 1) << 4) ^
+                      (unsigned long long)(cfg->device + 1);
+        if (h->list_sig == 0) h->list_sig = 1;
+    }
 
     // ---- interaction count: per-axis closed form over the lists (out-of-grid partners skipped) ----
     {
@@ -375,10 +384,14 @@ int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com
 static int upload_tables(octo_fmm_t* h)
 {
     if (g_const_owner == h) return OCTO_FMM_OK;
-    if (cudaMemcpyToSymbolAsync(c_entries, h->entries.data(), h->entries.size() * sizeof(StEntry), 0,
-                                cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
-    if (cudaMemcpyToSymbolAsync(c_begin, h->begin, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
-        return OCTO_FMM_ECUDA;
+    // the lists depend on (theta, kind, list flavour) only: the levels of a complete solve share them and differ in h
+    if (g_list_sig != h->list_sig) {
+        if (cudaMemcpyToSymbolAsync(c_entries, h->entries.data(), h->entries.size() * sizeof(StEntry), 0,
+                                    cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (cudaMemcpyToSymbolAsync(c_begin, h->begin, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+            return OCTO_FMM_ECUDA;
+        g_list_sig = h->list_sig;
+    }
     if (cudaMemcpyToSymbolAsync(c_hmul, h->hmul, sizeof(h->hmul), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
     g_const_owner = h;
@@ -496,7 +509,7 @@ int octo_fmm_destroy(octo_fmm_t* h)
         cudaEventDestroy(h->ev_begin);
         cudaEventDestroy(h->ev_end);
     }
-    if (g_const_owner == h) g_const_owner = nullptr;
+    if (g_const_owner == h) { g_const_owner = nullptr; g_list_sig = 0; }
     delete h;
     return e == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
