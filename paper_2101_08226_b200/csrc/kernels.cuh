@@ -80,7 +80,7 @@ constexpr double DIPOLE_TOL = 4.0e-16;   // |M1_i| <= DIPOLE_TOL |M| h counts as
 __global__ void __launch_bounds__(256) stage_multipole_kernel(const double* __restrict__ mom,
                                                               const double* __restrict__ com, double* __restrict__ S,
                                                               int nx, int ny, int nz, int z_begin, int z_count, double h,
-                                                              int* __restrict__ flags)
+                                                              int* __restrict__ flags, int corr)
 {
     const long long ncell = (long long)nx * ny * nz;
     const long long local = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(256) stage_multipole_kernel(const double* __re
     double M[20], s[20];
 #pragma unroll
     for (int c = 0; c < 20; ++c) M[c] = mom[(long long)c * ncell + cell];
-    reduce_moments(M, s);
+    reduce_moments(M, s, corr != 0);
     {
         const double lim = DIPOLE_TOL * fabs(M[0]) * h;
         if (fabs(M[1]) > lim || fabs(M[2]) > lim || fabs(M[3]) > lim) atomicOr(flags + 1, 2);
@@ -219,10 +219,10 @@ __device__ __forceinline__ void load_target(const Params& p, int gx, int gy, int
 }
 
 template <bool CORR>
-__device__ __forceinline__ void store_target(const Params& p, const Acc& acc, int gx, int gy, int k)
+__device__ __forceinline__ void store_target(const Params& p, const Acc& acc, const double (&tA)[7], int gx, int gy, int k)
 {
     double L[20], C[3];
-    acc_finish<CORR>(acc, L, C);
+    acc_finish<CORR>(acc, tA, L, C);
     const long long ocell = (long long)p.ox * p.oy * p.oz;
     const long long o = ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
 #pragma unroll
@@ -321,7 +321,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         }
 #undef OCTO_FETCH
 
-        if (active) store_target<CORR>(p, acc, gx, gy, k);
+        if (active) store_target<CORR>(p, acc, tA, gx, gy, k);
     }
 }
 
@@ -417,7 +417,7 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
             if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
             else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
         }
-        store_target<CORR>(p, acc, gx, gy, k);
+        store_target<CORR>(p, acc, tA, gx, gy, k);
     }
 }
 
@@ -470,7 +470,7 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
         for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
         v[c] = a;
     }
-    if (lane == 0) store_target<CORR>(p, acc, gx, gy, k);
+    if (lane == 0) store_target<CORR>(p, acc, tA, gx, gy, k);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -59,7 +59,10 @@ __device__ __forceinline__ double rsqrt_fast(double x)
 }
 
 // Reduce the 20 raw moments of a cell to the 16 staged source components (once per cell).
-__device__ __forceinline__ void reduce_moments(const double M[20], double* s)
+// The seven octupole slots hold, with the correction OFF, the reduced -1/6 M3 that contracts with the 7
+// independent components of D3; with the correction ON, N' = -1/6 x (trace-free part of M3), components
+// xxx xxy xxz xyy xyz yyy yyz -- the form the cubic-form evaluation of m2l_pair<true> needs.
+__device__ __forceinline__ void reduce_moments(const double M[20], double* s, const bool corr)
 {
     s[C_M0] = M[0];
     s[C_M1X] = -M[1];
@@ -80,6 +83,18 @@ __device__ __forceinline__ void reduce_moments(const double M[20], double* s)
     s[C_OXYZ] = -M[14];
     s[C_OYYY] = -(M[16] - 3.0 * M[18]) * (1.0 / 6.0);
     s[C_OYYZ] = -(3.0 * M[17] - M[19]) * (1.0 / 6.0);
+    if (corr) {
+        // trace-free part: N_ijk = M_ijk - (d_ij t_k + d_ik t_j + d_jk t_i) / 5,  t_k = M_jjk
+        const double tx = (M[10] + M[13]) + M[15], ty = (M[11] + M[16]) + M[18], tz = (M[12] + M[17]) + M[19];
+        const double k = -1.0 / 6.0;
+        s[C_OXXX] = k * (M[10] - 0.6 * tx);
+        s[C_OXXY] = k * (M[11] - 0.2 * ty);
+        s[C_OXXZ] = k * (M[12] - 0.2 * tz);
+        s[C_OXYY] = k * (M[13] - 0.2 * tx);
+        s[C_OXYZ] = k * M[14];
+        s[C_OYYY] = k * (M[16] - 0.6 * ty);
+        s[C_OYYZ] = k * (M[17] - 0.2 * tz);
+    }
 }
 
 // Head of one ordered pair: 1/|R|.  Kept apart from the body so that the kernels can run the
@@ -148,77 +163,77 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
     const double Dxxy = fma(bxx, y, ay);
     const double Dxxz = fma(bxx, z, az);
     a.l3[0] = fma(m0, Dxxx, a.l3[0]);  if (DIPOLE) a.l2[0] = fma(m1x, Dxxx, a.l2[0]);  a.l1[0] = fma(qxx, Dxxx, a.l1[0]);
-    a.l0b = fma(oxxx, Dxxx, a.l0b);
+    if (!CORR) a.l0b = fma(oxxx, Dxxx, a.l0b);
     a.l3[1] = fma(m0, Dxxy, a.l3[1]);  if (DIPOLE) a.l2[1] = fma(m1x, Dxxy, a.l2[1]);  if (DIPOLE) a.l2[0] = fma(m1y, Dxxy, a.l2[0]);
-    a.l1[1] = fma(qxx, Dxxy, a.l1[1]);  a.l1[0] = fma(qxy, Dxxy, a.l1[0]);  a.l0 = fma(oxxy, Dxxy, a.l0);
+    a.l1[1] = fma(qxx, Dxxy, a.l1[1]);  a.l1[0] = fma(qxy, Dxxy, a.l1[0]);  if (!CORR) a.l0 = fma(oxxy, Dxxy, a.l0);
     a.l3[2] = fma(m0, Dxxz, a.l3[2]);  if (DIPOLE) a.l2[2] = fma(m1x, Dxxz, a.l2[2]);  if (DIPOLE) a.l2[0] = fma(m1z, Dxxz, a.l2[0]);
-    a.l1[2] = fma(qxx, Dxxz, a.l1[2]);  a.l1[0] = fma(qxz, Dxxz, a.l1[0]);  a.l0b = fma(oxxz, Dxxz, a.l0b);
+    a.l1[2] = fma(qxx, Dxxz, a.l1[2]);  a.l1[0] = fma(qxz, Dxxz, a.l1[0]);  if (!CORR) a.l0b = fma(oxxz, Dxxz, a.l0b);
     const double Dxyy = fma(bxy, y, ax);
     const double Dxyz = bxy * z;
     a.l3[3] = fma(m0, Dxyy, a.l3[3]);  if (DIPOLE) a.l2[3] = fma(m1x, Dxyy, a.l2[3]);  if (DIPOLE) a.l2[1] = fma(m1y, Dxyy, a.l2[1]);
-    a.l1[0] = fma(qyy, Dxyy, a.l1[0]);  a.l1[1] = fma(qxy, Dxyy, a.l1[1]);  a.l0 = fma(oxyy, Dxyy, a.l0);
+    a.l1[0] = fma(qyy, Dxyy, a.l1[0]);  a.l1[1] = fma(qxy, Dxyy, a.l1[1]);  if (!CORR) a.l0 = fma(oxyy, Dxyy, a.l0);
     a.l3[4] = fma(m0, Dxyz, a.l3[4]);  if (DIPOLE) a.l2[4] = fma(m1x, Dxyz, a.l2[4]);  if (DIPOLE) a.l2[2] = fma(m1y, Dxyz, a.l2[2]);
     if (DIPOLE) a.l2[1] = fma(m1z, Dxyz, a.l2[1]);  a.l1[0] = fma(qyz, Dxyz, a.l1[0]);  a.l1[1] = fma(qxz, Dxyz, a.l1[1]);
-    a.l1[2] = fma(qxy, Dxyz, a.l1[2]);  a.l0b = fma(oxyz, Dxyz, a.l0b);
+    a.l1[2] = fma(qxy, Dxyz, a.l1[2]);  if (!CORR) a.l0b = fma(oxyz, Dxyz, a.l0b);
     const double Dyyy = fma(byy, y, ay3);
     const double Dyyz = fma(byy, z, az);
     a.l3[5] = fma(m0, Dyyy, a.l3[5]);  if (DIPOLE) a.l2[3] = fma(m1y, Dyyy, a.l2[3]);  a.l1[1] = fma(qyy, Dyyy, a.l1[1]);
-    a.l0 = fma(oyyy, Dyyy, a.l0);
+    if (!CORR) a.l0 = fma(oyyy, Dyyy, a.l0);
     a.l3[6] = fma(m0, Dyyz, a.l3[6]);  if (DIPOLE) a.l2[4] = fma(m1y, Dyyz, a.l2[4]);  if (DIPOLE) a.l2[3] = fma(m1z, Dyyz, a.l2[3]);
-    a.l1[2] = fma(qyy, Dyyz, a.l1[2]);  a.l1[1] = fma(qyz, Dyyz, a.l1[1]);  a.l0b = fma(oyyz, Dyyz, a.l0b);
+    a.l1[2] = fma(qyy, Dyyz, a.l1[2]);  a.l1[1] = fma(qyz, Dyyz, a.l1[1]);  if (!CORR) a.l0b = fma(oyyz, Dyyz, a.l0b);
     const double Dxzz = -(Dxxx + Dxyy);
     const double Dyzz = -(Dxxy + Dyyy);
     if (DIPOLE) a.l2[2] = fma(m1z, Dxzz, a.l2[2]);  a.l1[2] = fma(qxz, Dxzz, a.l1[2]);
     if (DIPOLE) a.l2[4] = fma(m1z, Dyzz, a.l2[4]);  a.l1[2] = fma(qyz, Dyzz, a.l1[2]);
 
-    double n0 = 0.0, n1 = 0.0, n2 = 0.0, n3 = 0.0, n4 = 0.0, n5 = 0.0, n6 = 0.0;
     if (CORR) {
-        // n3 = O_B - M_B (O_A / M_A), L127
-        n0 = fma(-m0, tA[0], oxxx);   // xxx
-        n1 = fma(-m0, tA[1], oxxy);   // xxy
-        n2 = fma(-m0, tA[2], oxxz);   // xxz
-        n3 = fma(-m0, tA[3], oxyy);   // xyy
-        n4 = fma(-m0, tA[4], oxyz);   // xyz
-        n5 = fma(-m0, tA[5], oyyy);   // yyy
-        n6 = fma(-m0, tA[6], oyyz);   // yyz
-    }
-
-    if (CORR) {
-        // ---- correction (L127): dL1_i += n3_t D4_{i,t}, runs over t ----
-        const double d4 = d3 * (-7.0 * w2);    // -105/r^9
-        const double cx = d4 * x, cy = d4 * y;
-        const double cxx = cx * x, cxy = cx * y, cyy = cy * y;
-        const double cxxx = cxx * x, cxxy = cxx * y, cxyy = cxy * y, cyyy = cyy * y;
-        const double bxz = bx * z, byz = by * z;
-        const double d2_3 = 3.0 * d2, bxy3 = 3.0 * bxy;
-        const double Exxxx = fma(cxxx, x, fma(6.0, bxx, d2_3));
-        const double Exxxy = fma(cxxx, y, bxy3);
-        const double Exxxz = fma(cxxx, z, 3.0 * bxz);
-        const double Exxyy = fma(cxxy, y, (bxx + byy) + d2);
-        const double Exxyz = fma(cxxy, z, byz);
-        const double Exyyy = fma(cxyy, y, bxy3);
-        const double Exyyz = fma(cxyy, z, bxz);
-        const double Eyyyy = fma(cyyy, y, fma(6.0, byy, d2_3));
-        const double Eyyyz = fma(cyyy, z, 3.0 * byz);
-        const double Exxzz = -(Exxxx + Exxyy);
-        const double Exyzz = -(Exxxy + Exyyy);
-        const double Eyyzz = -(Exxyy + Eyyyy);
-
-        a.c[0] = fma(n0, Exxxx, a.c[0]); a.c[1] = fma(n0, Exxxy, a.c[1]); a.c[2] = fma(n0, Exxxz, a.c[2]);
-        a.c[0] = fma(n1, Exxxy, a.c[0]); a.c[1] = fma(n1, Exxyy, a.c[1]); a.c[2] = fma(n1, Exxyz, a.c[2]);
-        a.c[0] = fma(n2, Exxxz, a.c[0]); a.c[1] = fma(n2, Exxyz, a.c[1]); a.c[2] = fma(n2, Exxzz, a.c[2]);
-        a.c[0] = fma(n3, Exxyy, a.c[0]); a.c[1] = fma(n3, Exyyy, a.c[1]); a.c[2] = fma(n3, Exyyz, a.c[2]);
-        a.c[0] = fma(n4, Exxyz, a.c[0]); a.c[1] = fma(n4, Exyyz, a.c[1]); a.c[2] = fma(n4, Exyzz, a.c[2]);
-        a.c[0] = fma(n5, Exyyy, a.c[0]); a.c[1] = fma(n5, Eyyyy, a.c[1]); a.c[2] = fma(n5, Eyyyz, a.c[2]);
-        a.c[0] = fma(n6, Exyyz, a.c[0]); a.c[1] = fma(n6, Eyyyz, a.c[1]); a.c[2] = fma(n6, Eyyzz, a.c[2]);
+        // ---- octupole term of L0 and the correction (L127) through the cubic form of n3 ----
+        // n = N'_B - M_B (N'_A / M_A): -1/6 x trace-free part of n3 = M3_B - (M_B / M_A) M3_A.  D3 and D4 are
+        // trace-free, so only this part of n3 matters, and with Q_i = n_ijk R_j R_k, C = Q.R:
+        //   -1/6 n3 :. D3          = d3 C                      (-> L0; the part M_B N'_A/M_A of the source's own
+        //                                                          octupole is added per cell in acc_finish)
+        //   -1/6 n3_jkl D4_ijkl    = d4 C R_i + 3 d3 Q_i       (-> dL1_i; D4_ijkl = d/dR_i D3_jkl, d(d3)/dR_i = d4 R_i)
+        // 48 instead of the 68 FP64 instructions of generating D4 and contracting it component by component.
+        const double nxxx = fma(-m0, tA[0], oxxx), nxxy = fma(-m0, tA[1], oxxy), nxxz = fma(-m0, tA[2], oxxz);
+        const double nxyy = fma(-m0, tA[3], oxyy), nxyz = fma(-m0, tA[4], oxyz);
+        const double nyyy = fma(-m0, tA[5], oyyy), nyyz = fma(-m0, tA[6], oyyz);
+        const double nxzz = -(nxxx + nxyy), nyzz = -(nxxy + nyyy);          // trace-free: n_izz = -n_ixx - n_iyy
+        const double zz = z * z;
+        const double pa = fma(x, x, -zz), pb = fma(y, y, -zz);              // x^2 - z^2, y^2 - z^2
+        const double x2 = x + x;
+        const double pxy = x2 * y, pxz = x2 * z, pyz = (y + y) * z;         // 2xy, 2xz, 2yz
+        const double Qx = fma(nxyz, pyz, fma(nxxz, pxz, fma(nxxy, pxy, fma(nxyy, pb, nxxx * pa))));
+        const double Qy = fma(nyyz, pyz, fma(nxyz, pxz, fma(nxyy, pxy, fma(nyyy, pb, nxxy * pa))));
+        const double Qz = fma(nyzz, pyz, fma(nxzz, pxz, fma(nxyz, pxy, fma(nyyz, pb, nxxz * pa))));
+        const double C = fma(z, Qz, fma(y, Qy, x * Qx));
+        a.l0 = fma(d3, C, a.l0);
+        const double t4 = (d3 * (-7.0 * w2)) * C;                           // d4 C,  d4 = -105/r^9
+        const double t3 = 3.0 * d3;
+        a.c[0] = fma(t3, Qx, fma(t4, x, a.c[0]));
+        a.c[1] = fma(t3, Qy, fma(t4, y, a.c[1]));
+        a.c[2] = fma(t3, Qz, fma(t4, z, a.c[2]));
     }
 }
 
 // Rebuild the 20 + 3 output coefficients from the independent accumulators.
+// With the correction, the sources' octupoles entered L0 only through n = N'_B - M_B tA (m2l_pair); the rest,
+// sum_B M_B (tA :. D3(R_B)) = tA :. L3, is added here, with tA taken to the reduced form that contracts with the
+// 7 independent components of the trace-free L3.
 template <bool CORR>
-__device__ __forceinline__ void acc_finish(const Acc& a, double L[20], double C[3])
+__device__ __forceinline__ void acc_finish(const Acc& a, const double (&tA)[7], double L[20], double C[3])
 {
     L[0] = a.l0 + a.l0b;
+    if (CORR) {
+        double t = 0.0;
+        t = fma(fma(4.0, tA[0], 3.0 * tA[3]), a.l3[0], t);     // xxx
+        t = fma(fma(6.0, tA[1], 3.0 * tA[5]), a.l3[1], t);     // xxy
+        t = fma(fma(4.0, tA[2], tA[6]), a.l3[2], t);           // xxz
+        t = fma(fma(6.0, tA[3], 3.0 * tA[0]), a.l3[3], t);     // xyy
+        t = fma(6.0 * tA[4], a.l3[4], t);                      // xyz
+        t = fma(fma(4.0, tA[5], 3.0 * tA[1]), a.l3[5], t);     // yyy
+        t = fma(fma(4.0, tA[6], tA[2]), a.l3[6], t);           // yyz
+        L[0] += t;
+    }
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         C[i] = CORR ? a.c[i] : 0.0;

@@ -371,7 +371,7 @@ int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com
         const long long ncell = (long long)P.nx * P.ny * P.nz;
         if (cudaMemsetAsync(h->flags + 1, 0, sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
         stage_multipole_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(moments, com_off, h->src, P.nx, P.ny, P.nz,
-                                                                                       0, P.nz, h->cfg.h, h->flags);
+                                                                                       0, P.nz, h->cfg.h, h->flags, h->cfg.am_correction);
     } else {
         const long long pc = (long long)(P.nx + REACH_MAX + MONO_PAD_RIGHT) * (P.ny + 2 * REACH_MAX) * (P.nz + 2 * REACH_MAX);
         stage_monopole_kernel<<<(unsigned)((pc + 255) / 256), 256, 0, h->stream>>>(moments, h->src, P.nx, P.ny, P.nz);
@@ -579,7 +579,7 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
         if (need > brought) {
             const long long n = (long long)(need - brought) * (long long)plane;
             stage_multipole_kernel<<<(unsigned)((n + 255) / 256), 256, 0, sm>>>(d_m, d_c, h->src, P.nx, P.ny, P.nz, brought,
-                                                                                 need - brought, h->cfg.h, h->flags);
+                                                                                 need - brought, h->cfg.h, h->flags, h->cfg.am_correction);
             OCTO_TRY(cudaGetLastError());
             brought = need;
         }
@@ -763,7 +763,7 @@ int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_
     int f, i;
     if (kind == OCTO_FMM_MONOPOLE) { f = 8; i = 4; }
     else if (kind == OCTO_FMM_MULTIPOLE) {
-        if (am_correction) { f = 301; i = 178; }   // 123 DFMA + 43 DMUL + 12 DADD
+        if (am_correction) { f = 263; i = 158; }   // 105 DFMA + 40 DMUL + 13 DADD
         else               { f = 201; i = 117; }   //  84 DFMA + 26 DMUL +  7 DADD
         if (!dipole_terms) { f -= 56; i -= 28; }   // 27 dipole FMAs and the FMA of D2_zz
     } else return OCTO_FMM_EINVAL;
