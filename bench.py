@@ -495,8 +495,8 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum of the interaction kernel, one `ncu --set full` capture
 # per entry (profiles/); None until captured for that workload.
 TRAFFIC_BYTES = {
-    # profiles/r01_final.md: 7.111 GB read + 3.099 GB written per launch
-    ("cfg5", 256, 0.5): 10209414000,
+    # profiles/r01_final.md: 7.072 GB read + 3.061 GB written per launch
+    ("cfg5", 256, 0.5): 10132895000,
 }
 
 

@@ -763,8 +763,9 @@ int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_
     int f, i;
     if (kind == OCTO_FMM_MONOPOLE) { f = 8; i = 4; }
     else if (kind == OCTO_FMM_MULTIPOLE) {
-        if (am_correction) { f = 263; i = 158; }   // 105 DFMA + 40 DMUL + 13 DADD
-        else               { f = 201; i = 117; }   //  84 DFMA + 26 DMUL +  7 DADD
+        // counted in the SASS of the hot loops (cuobjdump), per pair
+        if (am_correction) { f = 264; i = 157; }   // 107 DFMA + 38 DMUL + 12 DADD
+        else               { f = 202; i = 118; }   //  84 DFMA + 26 DMUL +  8 DADD
         if (!dipole_terms) { f -= 56; i -= 28; }   // 27 dipole FMAs and the FMA of D2_zz
     } else return OCTO_FMM_EINVAL;
     if (flops) *flops = f;
