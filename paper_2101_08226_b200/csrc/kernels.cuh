@@ -572,14 +572,13 @@ __global__ void __launch_bounds__(MONO_THREADS, 1) p2p_monopole_kernel(const __g
             const int packed = c_entries[s].off;                 // low 16 bits: tile offset (signed), high 16: weight index
             const double* q = base + (short)(packed & 0xffff);
             const double4 w = W[packed >> 16];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const double m = q[j * LAYER2];
-                a[j][0] = fma(m, w.x, a[j][0]);
-                a[j][1] = fma(m, w.y, a[j][1]);
-                a[j][2] = fma(m, w.z, a[j][2]);
-                a[j][3] = fma(m, w.w, a[j][3]);
-            }
+            const double m0 = q[0], m1 = q[LAYER2], m2 = q[2 * LAYER2], m3 = q[3 * LAYER2];
+            // boustrophedon order: consecutive DFMAs share the mass or the weight, so that one operand always
+            // comes from the operand-reuse cache (a DFMA with three fresh register operands takes 3 cycles, not 2)
+            a[0][0] = fma(m0, w.x, a[0][0]); a[0][1] = fma(m0, w.y, a[0][1]); a[0][2] = fma(m0, w.z, a[0][2]); a[0][3] = fma(m0, w.w, a[0][3]);
+            a[1][3] = fma(m1, w.w, a[1][3]); a[1][2] = fma(m1, w.z, a[1][2]); a[1][1] = fma(m1, w.y, a[1][1]); a[1][0] = fma(m1, w.x, a[1][0]);
+            a[2][0] = fma(m2, w.x, a[2][0]); a[2][1] = fma(m2, w.y, a[2][1]); a[2][2] = fma(m2, w.z, a[2][2]); a[2][3] = fma(m2, w.w, a[2][3]);
+            a[3][3] = fma(m3, w.w, a[3][3]); a[3][2] = fma(m3, w.z, a[3][2]); a[3][1] = fma(m3, w.y, a[3][1]); a[3][0] = fma(m3, w.x, a[3][0]);
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
