@@ -285,6 +285,66 @@ def run_solve(args):
     s.close()
 
 
+def run_coupled(args):
+    """--coupled: ONE problem sharded over the ranks (z-slabs of a grid of ncell x ncell x (ncell * N) cells, rank r owns
+    slab r) with one halo exchange of boundary layers per step (paper_2101_08226_b200/sharded.py).
+    Opt-in: the default N > 1 arm runs independent problems.  A step = halo exchange + staging + interaction."""
+    import torch
+    import torch.distributed as dist
+    world, rank, local = env_int("WORLD_SIZE", 1), env_int("RANK", 0), env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2101_08226_b200 import build
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2101_08226_b200 as p
+    from paper_2101_08226_b200.sharded import HALO, ShardedLevel
+    w = make_workload(args.workload, args.theta, args.ncell, args.seed + rank)     # rank r's slab of the tall domain
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream(dev)
+    lvl = ShardedLevel(w.n, w.h, args.theta, True, rank=rank, world=world, device=local, stream=stream)
+    lvl.fmm.set_option("dipole_terms", 1)
+    mom, com = torch.from_numpy(w.moments).to(dev), torch.from_numpy(w.com_off).to(dev)
+    L = torch.empty((20,) + lvl.fmm.out_shape, dtype=torch.float64, device=dev)
+    Lc = torch.empty((3,) + lvl.fmm.out_shape, dtype=torch.float64, device=dev)
+    lvl.fmm.bind_outputs(L, Lc)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        lvl.step(mom, com, L, Lc)
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        lvl.step(mom, com, L, Lc)
+    ev1.record(stream)
+    barrier()
+    if lvl.fmm.status() != p.OK:
+        raise SystemExit("bench.py: device reported status %d" % lvl.fmm.status())
+    ms, units = aggregate_over_ranks(ev0.elapsed_time(ev1), lvl.interaction_count() * args.steps, dist if world > 1 else None, dev)
+    if rank == 0:
+        halo_bytes = (2 if world > 2 else (1 if world == 2 else 0)) * 23 * HALO * w.n[0] * w.n[1] * 8
+        print(json.dumps({"metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": "%s stacked in z: %d x %d x %d cells, theta=%g, correction on" % (
+                              w.name, w.n[0], w.n[1], w.n[2] * world, args.theta),
+                              "parallelism": "z-slabs, one halo exchange per step (%d bytes sent per interior rank)" % halo_bytes},
+                          "gpu_launches": 2 * args.steps}))
+    lvl.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -513,6 +573,8 @@ def main():
     ap.add_argument("--ncell", type=int, default=0)
     ap.add_argument("--seed", type=int, default=20210108)
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--coupled", action="store_true",
+                    help="N > 1: ONE problem in z-slabs with a halo exchange per step instead of independent problems")
     ap.add_argument("--ref-seconds", type=float, default=12.0,
                     help="CPU seconds of oracle work per cpu_baseline sample / per --impl reference step")
     args = ap.parse_args()
@@ -520,6 +582,8 @@ def main():
         run_reference(args)
     elif args.workload == "solve":
         run_solve(args)
+    elif args.coupled:
+        run_coupled(args)
     else:
         run_ours(args)
 
