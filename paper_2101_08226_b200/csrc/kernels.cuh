@@ -461,10 +461,9 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
         else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
     }
     // warp-level reduction of the partial expansions (fixed butterfly order: deterministic)
-    static_assert(sizeof(Acc) == 20 * sizeof(double), "Acc is 20 doubles");
     double* v = reinterpret_cast<double*>(&acc);
 #pragma unroll
-    for (int c = 0; c < 20; ++c) {
+    for (int c = 0; c < ACC_DOUBLES; ++c) {
         double a = v[c];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);

@@ -26,6 +26,7 @@ enum {
     NCOMP = 19
 };
 
+// Accumulators of one target cell: the independent components of the trace-free L2 / L3, two partial sums of L0.
 struct Acc {
     double l0, l0b; // two partial sums of L0
     double l1[3];
@@ -33,6 +34,8 @@ struct Acc {
     double l3[7];   // xxx xxy xxz xyy xyz yyy yyz
     double c[3];    // correction to L1
 };
+constexpr int ACC_DOUBLES = 20;
+static_assert(sizeof(Acc) == ACC_DOUBLES * sizeof(double), "Acc is a plain array of doubles");
 
 __device__ __forceinline__ void acc_zero(Acc& a)
 {
@@ -59,6 +62,8 @@ __device__ __forceinline__ double rsqrt_fast(double x)
 }
 
 // Reduce the 20 raw moments of a cell to the 16 staged source components (once per cell).
+// With the correction ON the five quadrupole slots hold q~ = 1/2 x (trace-free part of M2) (for the evaluation
+// through R-contractions in m2l_pair<true>) instead of the reduced 1/2 M2.
 // The seven octupole slots hold, with the correction OFF, the reduced -1/6 M3 that contracts with the 7
 // independent components of D3; with the correction ON, N' = -1/6 x (trace-free part of M3), components
 // xxx xxy xxz xyy xyz yyy yyz -- the form the cubic-form evaluation of m2l_pair<true> needs.
@@ -84,6 +89,13 @@ __device__ __forceinline__ void reduce_moments(const double M[20], double* s, co
     s[C_OYYY] = -(M[16] - 3.0 * M[18]) * (1.0 / 6.0);
     s[C_OYYZ] = -(3.0 * M[17] - M[19]) * (1.0 / 6.0);
     if (corr) {
+        // quadrupole slots: q~ = 1/2 x (trace-free part of M2), components xx xy xz yy yz
+        const double tr3 = ((M[4] + M[7]) + M[9]) * (1.0 / 3.0);
+        s[C_QXX] = 0.5 * (M[4] - tr3);
+        s[C_QXY] = 0.5 * M[5];
+        s[C_QXZ] = 0.5 * M[6];
+        s[C_QYY] = 0.5 * (M[7] - tr3);
+        s[C_QYZ] = 0.5 * M[8];
         // trace-free part: N_ijk = M_ijk - (d_ij t_k + d_ik t_j + d_jk t_i) / 5,  t_k = M_jjk
         const double tx = (M[10] + M[13]) + M[15], ty = (M[11] + M[16]) + M[18], tz = (M[12] + M[17]) + M[19];
         const double k = -1.0 / 6.0;
@@ -105,6 +117,113 @@ __device__ __forceinline__ double pair_head(const double x, const double y, cons
     return rsqrt_fast(r2);
 }
 
+// Body of one ordered pair with the correction ON.  Instead of generating the components of D2, D3, D4 and
+// multiplying each by every source component, everything a source contributes is written as a radial factor times
+// products of components of R, with the source's mass folded into the radial factors:
+//   L0   += -M w + d1 (m1.R) + d2 S + d3 C                 S = q~_jk R_j R_k,  C = n_jkl R_j R_k R_l  (see below)
+//   L1_i += (M d1 + d2 (m1.R) + d3 S) R_i + d1 m1_i + 2 d2 V_i        V_i = q~_ij R_j
+//   L2_ij += c1 d_ij + c2 R_i R_j + h_i R_j + h_j R_i      c1 = M d1 + d2 (m1.R),  c2 = M d2 + d3 (m1.R),  h = d2 m1
+//   L3_ijk += M d2 (d_ij R_k + d_ik R_j + d_jk R_i) + M d3 R_i R_j R_k
+//   dL1_i += d4 C R_i + 3 d3 Q_i,  L0 += d3 C              n = N'_B - M_B (N'_A / M_A),  Q_i = n_ijk R_j R_k  (L127)
+// with m1 = -M1 (staged), q~ = 1/2 trace-free M2, N' = -1/6 trace-free M3.  These are the sums of the header of
+// this file with D2_ij = d1 d_ij + d2 R_i R_j etc. multiplied out (the quadrupole and dipole parts use that D2 and
+// D3 are trace-free); the independent components of L2 and L3 are accumulated as in the component form, each
+// completed per pair.  120 FP64 instructions per pair without the dipole terms and 141 with them, against 129 / 157
+// for the component-by-component contraction; the oracle keeps the component form.
+template <bool DIPOLE>
+__device__ __forceinline__ void m2l_pair_monomial(Acc& a, const double x, const double y, const double z, const double w,
+                                                  const double (&s)[16], const double (&tA)[7])
+{
+    const double w2 = w * w;                  // 1/r^2
+    const double d1 = w * w2;                 // 1/r^3
+    const double d2 = d1 * (-3.0 * w2);       // -3/r^5
+    const double d3 = d2 * (-5.0 * w2);       // 15/r^7
+    const double m0 = s[C_M0];
+    const double qxx = s[C_QXX], qxy = s[C_QXY], qxz = s[C_QXZ], qyy = s[C_QYY], qyz = s[C_QYZ];
+    const double e1 = m0 * d1, e2 = m0 * d2, e3 = m0 * d3;
+    a.l0 = fma(m0, -w, a.l0);
+
+    // products of R shared by the quadrupole and octupole parts
+    const double zz = z * z;
+    const double pa = fma(x, x, -zz), pb = fma(y, y, -zz);              // x^2 - z^2, y^2 - z^2
+    const double x2 = x + x, y2 = y + y;
+    const double pxy = x2 * y, pxz = x2 * z, pyz = y2 * z;              // 2xy, 2xz, 2yz
+
+    // ---- quadrupole: S = q~ : R R (q~ trace-free),  V = q~ R ----
+    const double S = fma(qyz, pyz, fma(qxz, pxz, fma(qxy, pxy, fma(qyy, pb, qxx * pa))));
+    a.l0b = fma(d2, S, a.l0b);
+    const double qzz = -(qxx + qyy);
+    const double Vx = fma(qxz, z, fma(qxy, y, qxx * x));
+    const double Vy = fma(qyz, z, fma(qyy, y, qxy * x));
+    const double Vz = fma(qzz, z, fma(qyz, y, qxz * x));
+    const double u2 = d2 + d2;
+
+    // ---- monopole and dipole coefficients of the R-monomials ----
+    double c1 = e1, c2 = e2;
+    if (DIPOLE) {
+        const double m1x = s[C_M1X], m1y = s[C_M1Y], m1z = s[C_M1Z];
+        const double ar = fma(m1z, z, fma(m1y, y, m1x * x));            // m1 . R
+        a.l0 = fma(d1, ar, a.l0);
+        c1 = fma(d2, ar, e1);
+        c2 = fma(d3, ar, e2);
+        a.l1[0] = fma(d1, m1x, a.l1[0]);
+        a.l1[1] = fma(d1, m1y, a.l1[1]);
+        a.l1[2] = fma(d1, m1z, a.l1[2]);
+        const double hx = d2 * m1x, hy = d2 * m1y, hz = d2 * m1z;
+        a.l2[0] = fma(hx, x2, a.l2[0]);
+        a.l2[1] = fma(hy, x, fma(hx, y, a.l2[1]));
+        a.l2[2] = fma(hz, x, fma(hx, z, a.l2[2]));
+        a.l2[3] = fma(hy, y2, a.l2[3]);
+        a.l2[4] = fma(hz, y, fma(hy, z, a.l2[4]));
+    }
+    // ---- L1 ----
+    const double k1 = fma(d3, S, c1);
+    a.l1[0] = fma(u2, Vx, fma(k1, x, a.l1[0]));
+    a.l1[1] = fma(u2, Vy, fma(k1, y, a.l1[1]));
+    a.l1[2] = fma(u2, Vz, fma(k1, z, a.l1[2]));
+    // ---- L2_ij += c1 d_ij + c2 R_i R_j: the diagonal is completed per pair (c1 and c2 x^2 cancel to a large extent;
+    //      summing them separately over the list would lose those digits) ----
+    const double c2x = c2 * x, c2y = c2 * y;
+    a.l2[0] += fma(c2x, x, c1);
+    a.l2[1] = fma(c2x, y, a.l2[1]);
+    a.l2[2] = fma(c2x, z, a.l2[2]);
+    a.l2[3] += fma(c2y, y, c1);
+    a.l2[4] = fma(c2y, z, a.l2[4]);
+    // ---- L3_ijk += M d2 (d_ij R_k + d_ik R_j + d_jk R_i) + M d3 R_i R_j R_k, again completed per pair ----
+    const double e3x = e3 * x, e3y = e3 * y, e2t = 3.0 * e2;
+    const double fxx3 = fma(e3x, x, e2t), fxx1 = fma(e3x, x, e2);      // M (d3 x^2 + 3 d2), M (d3 x^2 + d2)
+    const double fyy3 = fma(e3y, y, e2t), fyy1 = fma(e3y, y, e2);
+    const double e3xy = e3x * y;
+    a.l3[0] = fma(fxx3, x, a.l3[0]);      // xxx
+    a.l3[1] = fma(fxx1, y, a.l3[1]);      // xxy
+    a.l3[2] = fma(fxx1, z, a.l3[2]);      // xxz
+    a.l3[3] = fma(fyy1, x, a.l3[3]);      // xyy
+    a.l3[4] = fma(e3xy, z, a.l3[4]);      // xyz
+    a.l3[5] = fma(fyy3, y, a.l3[5]);      // yyy
+    a.l3[6] = fma(fyy1, z, a.l3[6]);      // yyz
+
+    // ---- octupole term of L0 and the correction (L127) through the cubic form of n3 ----
+    // n = N'_B - M_B (N'_A / M_A): -1/6 x trace-free part of n3 = M3_B - (M_B / M_A) M3_A.  D3 and D4 are
+    // trace-free, so only this part of n3 matters, and with Q_i = n_ijk R_j R_k, C = Q.R:
+    //   -1/6 n3 :. D3          = d3 C                      (-> L0; the part M_B N'_A/M_A of the source's own
+    //                                                          octupole is added per cell in acc_finish)
+    //   -1/6 n3_jkl D4_ijkl    = d4 C R_i + 3 d3 Q_i       (-> dL1_i; D4_ijkl = d/dR_i D3_jkl, d(d3)/dR_i = d4 R_i)
+    const double nxxx = fma(-m0, tA[0], s[C_OXXX]), nxxy = fma(-m0, tA[1], s[C_OXXY]), nxxz = fma(-m0, tA[2], s[C_OXXZ]);
+    const double nxyy = fma(-m0, tA[3], s[C_OXYY]), nxyz = fma(-m0, tA[4], s[C_OXYZ]);
+    const double nyyy = fma(-m0, tA[5], s[C_OYYY]), nyyz = fma(-m0, tA[6], s[C_OYYZ]);
+    const double nxzz = -(nxxx + nxyy), nyzz = -(nxxy + nyyy);          // trace-free: n_izz = -n_ixx - n_iyy
+    const double Qx = fma(nxyz, pyz, fma(nxxz, pxz, fma(nxxy, pxy, fma(nxyy, pb, nxxx * pa))));
+    const double Qy = fma(nyyz, pyz, fma(nxyz, pxz, fma(nxyy, pxy, fma(nyyy, pb, nxxy * pa))));
+    const double Qz = fma(nyzz, pyz, fma(nxzz, pxz, fma(nxyz, pxy, fma(nyyz, pb, nxxz * pa))));
+    const double C = fma(z, Qz, fma(y, Qy, x * Qx));
+    a.l0 = fma(d3, C, a.l0);
+    const double t4 = (d3 * (-7.0 * w2)) * C;                           // d4 C,  d4 = -105/r^9
+    const double t3 = 3.0 * d3;
+    a.c[0] = fma(t3, Qx, fma(t4, x, a.c[0]));
+    a.c[1] = fma(t3, Qy, fma(t4, y, a.c[1]));
+    a.c[2] = fma(t3, Qz, fma(t4, z, a.c[2]));
+}
+
 // Body of one ordered pair A <- B.  (x,y,z) = R = z_A - z_B, w = 1/|R|; s[0..15] staged source
 // components; tA[0..6] = staged third moments of the target divided by its mass (correction only).
 // DIPOLE = false leaves out the 27 terms with the source's dipole moment (and D2_zz, which only they need):
@@ -113,6 +232,10 @@ template <bool CORR, bool DIPOLE>
 __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y, const double z, const double w,
                                          const double (&s)[16], const double (&tA)[7])
 {
+    if constexpr (CORR) {
+        m2l_pair_monomial<DIPOLE>(a, x, y, z, w, s, tA);
+        return;
+    }
     const double w2 = w * w;                  // 1/r^2
     const double d1 = w * w2;                 // 1/r^3
     const double d2 = d1 * (-3.0 * w2);       // -3/r^5
@@ -186,66 +309,44 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
     if (DIPOLE) a.l2[2] = fma(m1z, Dxzz, a.l2[2]);  a.l1[2] = fma(qxz, Dxzz, a.l1[2]);
     if (DIPOLE) a.l2[4] = fma(m1z, Dyzz, a.l2[4]);  a.l1[2] = fma(qyz, Dyzz, a.l1[2]);
 
-    if (CORR) {
-        // ---- octupole term of L0 and the correction (L127) through the cubic form of n3 ----
-        // n = N'_B - M_B (N'_A / M_A): -1/6 x trace-free part of n3 = M3_B - (M_B / M_A) M3_A.  D3 and D4 are
-        // trace-free, so only this part of n3 matters, and with Q_i = n_ijk R_j R_k, C = Q.R:
-        //   -1/6 n3 :. D3          = d3 C                      (-> L0; the part M_B N'_A/M_A of the source's own
-        //                                                          octupole is added per cell in acc_finish)
-        //   -1/6 n3_jkl D4_ijkl    = d4 C R_i + 3 d3 Q_i       (-> dL1_i; D4_ijkl = d/dR_i D3_jkl, d(d3)/dR_i = d4 R_i)
-        // 48 instead of the 68 FP64 instructions of generating D4 and contracting it component by component.
-        const double nxxx = fma(-m0, tA[0], oxxx), nxxy = fma(-m0, tA[1], oxxy), nxxz = fma(-m0, tA[2], oxxz);
-        const double nxyy = fma(-m0, tA[3], oxyy), nxyz = fma(-m0, tA[4], oxyz);
-        const double nyyy = fma(-m0, tA[5], oyyy), nyyz = fma(-m0, tA[6], oyyz);
-        const double nxzz = -(nxxx + nxyy), nyzz = -(nxxy + nyyy);          // trace-free: n_izz = -n_ixx - n_iyy
-        const double zz = z * z;
-        const double pa = fma(x, x, -zz), pb = fma(y, y, -zz);              // x^2 - z^2, y^2 - z^2
-        const double x2 = x + x;
-        const double pxy = x2 * y, pxz = x2 * z, pyz = (y + y) * z;         // 2xy, 2xz, 2yz
-        const double Qx = fma(nxyz, pyz, fma(nxxz, pxz, fma(nxxy, pxy, fma(nxyy, pb, nxxx * pa))));
-        const double Qy = fma(nyyz, pyz, fma(nxyz, pxz, fma(nxyy, pxy, fma(nyyy, pb, nxxy * pa))));
-        const double Qz = fma(nyzz, pyz, fma(nxzz, pxz, fma(nxyz, pxy, fma(nyyz, pb, nxxz * pa))));
-        const double C = fma(z, Qz, fma(y, Qy, x * Qx));
-        a.l0 = fma(d3, C, a.l0);
-        const double t4 = (d3 * (-7.0 * w2)) * C;                           // d4 C,  d4 = -105/r^9
-        const double t3 = 3.0 * d3;
-        a.c[0] = fma(t3, Qx, fma(t4, x, a.c[0]));
-        a.c[1] = fma(t3, Qy, fma(t4, y, a.c[1]));
-        a.c[2] = fma(t3, Qz, fma(t4, z, a.c[2]));
-    }
 }
 
-// Rebuild the 20 + 3 output coefficients from the independent accumulators.
-// With the correction, the sources' octupoles entered L0 only through n = N'_B - M_B tA (m2l_pair); the rest,
-// sum_B M_B (tA :. D3(R_B)) = tA :. L3, is added here, with tA taken to the reduced form that contracts with the
-// 7 independent components of the trace-free L3.
+// Rebuild the 20 + 3 output coefficients from the accumulators.
 template <bool CORR>
 __device__ __forceinline__ void acc_finish(const Acc& a, const double (&tA)[7], double L[20], double C[3])
 {
     L[0] = a.l0 + a.l0b;
-    if (CORR) {
-        double t = 0.0;
-        t = fma(fma(4.0, tA[0], 3.0 * tA[3]), a.l3[0], t);     // xxx
-        t = fma(fma(6.0, tA[1], 3.0 * tA[5]), a.l3[1], t);     // xxy
-        t = fma(fma(4.0, tA[2], tA[6]), a.l3[2], t);           // xxz
-        t = fma(fma(6.0, tA[3], 3.0 * tA[0]), a.l3[3], t);     // xyy
-        t = fma(6.0 * tA[4], a.l3[4], t);                      // xyz
-        t = fma(fma(4.0, tA[5], 3.0 * tA[1]), a.l3[5], t);     // yyy
-        t = fma(fma(4.0, tA[6], tA[2]), a.l3[6], t);           // yyz
-        L[0] += t;
-    }
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
         C[i] = CORR ? a.c[i] : 0.0;
         L[1 + i] = CORR ? a.l1[i] + a.c[i] : a.l1[i];
     }
-    L[4] = a.l2[0]; L[5] = a.l2[1]; L[6] = a.l2[2]; L[7] = a.l2[3]; L[8] = a.l2[4];
-    L[9] = -(a.l2[0] + a.l2[3]);                       // zz = -(xx + yy)
-    L[10] = a.l3[0]; L[11] = a.l3[1]; L[12] = a.l3[2]; L[13] = a.l3[3]; L[14] = a.l3[4];
-    L[15] = -(a.l3[0] + a.l3[3]);                      // xzz = -(xxx + xyy)
-    L[16] = a.l3[5]; L[17] = a.l3[6];
-    L[18] = -(a.l3[1] + a.l3[5]);                      // yzz = -(xxy + yyy)
-    L[19] = -(a.l3[2] + a.l3[6]);                      // zzz = -(xxz + yyz)
+    double l2[5], l3[7];
+#pragma unroll
+    for (int i = 0; i < 5; ++i) l2[i] = a.l2[i];
+#pragma unroll
+    for (int i = 0; i < 7; ++i) l3[i] = a.l3[i];
+    if (CORR) {
+        // the sources' octupoles entered L0 only through n = N'_B - M_B tA; the rest, sum_B M_B (tA :. D3(R_B)) =
+        // tA :. L3, is added here, with tA taken to the reduced form that contracts with the 7 independent
+        // components of the trace-free L3
+        double t = 0.0;
+        t = fma(fma(4.0, tA[0], 3.0 * tA[3]), l3[0], t);       // xxx
+        t = fma(fma(6.0, tA[1], 3.0 * tA[5]), l3[1], t);       // xxy
+        t = fma(fma(4.0, tA[2], tA[6]), l3[2], t);             // xxz
+        t = fma(fma(6.0, tA[3], 3.0 * tA[0]), l3[3], t);       // xyy
+        t = fma(6.0 * tA[4], l3[4], t);                        // xyz
+        t = fma(fma(4.0, tA[5], 3.0 * tA[1]), l3[5], t);       // yyy
+        t = fma(fma(4.0, tA[6], tA[2]), l3[6], t);             // yyz
+        L[0] += t;
+    }
+    L[4] = l2[0]; L[5] = l2[1]; L[6] = l2[2]; L[7] = l2[3]; L[8] = l2[4];
+    L[9] = -(l2[0] + l2[3]);                           // zz = -(xx + yy)
+    L[10] = l3[0]; L[11] = l3[1]; L[12] = l3[2]; L[13] = l3[3]; L[14] = l3[4];
+    L[15] = -(l3[0] + l3[3]);                          // xzz = -(xxx + xyy)
+    L[16] = l3[5]; L[17] = l3[6];
+    L[18] = -(l3[1] + l3[5]);                          // yzz = -(xxy + yyy)
+    L[19] = -(l3[2] + l3[6]);                          // zzz = -(xxz + yyz)
 }
 
 }  // namespace octo

@@ -764,9 +764,13 @@ int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_
     if (kind == OCTO_FMM_MONOPOLE) { f = 8; i = 4; }
     else if (kind == OCTO_FMM_MULTIPOLE) {
         // counted in the SASS of the hot loops (cuobjdump), per pair
-        if (am_correction) { f = 264; i = 157; }   // 107 DFMA + 38 DMUL + 12 DADD
-        else               { f = 202; i = 118; }   //  84 DFMA + 26 DMUL +  8 DADD
-        if (!dipole_terms) { f -= 56; i -= 28; }   // 27 dipole FMAs and the FMA of D2_zz
+        if (am_correction) {
+            if (dipole_terms) { f = 224; i = 138; }   // 86 DFMA + 38 DMUL + 14 DADD
+            else              { f = 188; i = 118; }   // 70 DFMA + 34 DMUL + 14 DADD
+        } else {
+            if (dipole_terms) { f = 202; i = 118; }   // 84 DFMA + 26 DMUL +  8 DADD
+            else              { f = 146; i = 90; }    // 56 DFMA + 26 DMUL +  8 DADD
+        }
     } else return OCTO_FMM_EINVAL;
     if (flops) *flops = f;
     if (fp64_instructions) *fp64_instructions = i;

@@ -65,8 +65,8 @@ def test_create_without_workspace_or_device_fails_cleanly(pkg):
     with pytest.raises(pkg.OctoFmmError) as ei:      # NULL workspace
         pkg.octo_fmm_create(cfg)
     assert ei.value.status == pkg.EINVAL
-    assert pkg.octo_fmm_flops_per_interaction(pkg.MULTIPOLE, True) == (264, 157)
-    assert pkg.octo_fmm_flops_per_interaction_path(pkg.MULTIPOLE, True, False) == (208, 129)
+    assert pkg.octo_fmm_flops_per_interaction(pkg.MULTIPOLE, True) == (224, 138)
+    assert pkg.octo_fmm_flops_per_interaction_path(pkg.MULTIPOLE, True, False) == (188, 118)
     assert pkg.octo_fmm_flops_per_interaction(pkg.MULTIPOLE, False) == (202, 118)
     assert pkg.octo_fmm_flops_per_interaction(pkg.MONOPOLE, False) == (8, 4)
 
