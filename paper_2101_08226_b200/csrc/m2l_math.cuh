@@ -131,7 +131,7 @@ __device__ __forceinline__ double pair_head(const double x, const double y, cons
 // completed per pair.  120 FP64 instructions per pair without the dipole terms and 141 with them, against 129 / 157
 // for the component-by-component contraction; the oracle keeps the component form.
 template <bool DIPOLE>
-__device__ __forceinline__ void m2l_pair_monomial(Acc& a, const double x, const double y, const double z, const double w,
+__device__ __forceinline__ void m2l_pair_folded(Acc& a, const double x, const double y, const double z, const double w,
                                                   const double (&s)[16], const double (&tA)[7])
 {
     const double w2 = w * w;                  // 1/r^2
@@ -233,7 +233,7 @@ __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y,
                                          const double (&s)[16], const double (&tA)[7])
 {
     if constexpr (CORR) {
-        m2l_pair_monomial<DIPOLE>(a, x, y, z, w, s, tA);
+        m2l_pair_folded<DIPOLE>(a, x, y, z, w, s, tA);
         return;
     }
     const double w2 = w * w;                  // 1/r^2
