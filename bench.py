@@ -557,8 +557,8 @@ def run_ours(args):
 # dram__bytes_read.sum + dram__bytes_write.sum of the interaction kernel, one `ncu --set full` capture
 # per entry (profiles/); None until captured for that workload.
 TRAFFIC_BYTES = {
-    # profiles/r01_final.md: 7.072 GB read + 3.061 GB written per launch
-    ("cfg5", 256, 0.5): 10132895000,
+    # profiles/r01_final.md: 8.198 GB read + 3.063 GB written per launch
+    ("cfg5", 256, 0.5): 11260626000,
 }
 
 
