@@ -4,10 +4,15 @@
 // How it computes it differs from the definition on purpose (this is the GPU formulation; the
 // CPU oracle uses full tensors):
 //   * The Green's-function derivative tensors D^(n) of -1/r are symmetric and TRACE-FREE, so only
-//     2n+1 components of each are independent.  We generate the components with at most one z
-//     index (5 of D2, 7 of D3, 9 of D4) plus the few z-heavy ones the contractions touch, and we
-//     contract them with source moments that were reduced once per cell at staging time
-//     (trace removed, multiplicity and (-1)^m/m! folded in).  98 FMAs per pair instead of 125.
+//     2n+1 components of each are independent, and each is a radial factor d_n(r) times products
+//     of R_i plus delta terms.  Source moments are reduced once per cell at staging time (trace
+//     removed, multiplicity and (-1)^m/m! folded in).
+//   * Correction on (m2l_pair_folded): no component of D2..D4 is formed; what a
+//     source contributes is written as radial factors (with the source's mass folded in) times the
+//     R-contractions S = q_jk R_j R_k, V_i = q_ij R_j, a = m1.R, and the correction goes through the
+//     cubic form C = n_ijk R_i R_j R_k (c_i = d4 C R_i + 3 d3 Q_i).  86 DFMA + 38 DMUL + 14 DADD per pair.
+//   * Correction off (m2l_pair component form): the components of D1..D3 with at most one z index
+//     contracted with the reduced moments, grouped so that consecutive FMAs share an operand.
 //   * Accumulators are the independent components of L (1 + 3 + 5 + 7) and the correction (3);
 //     the dependent components (L2_zz, L3_xzz, L3_yzz, L3_zzz) are rebuilt once per cell.
 //   * 1/r comes from MUFU.RSQ64H (rsqrt.approx.ftz.f64, ~2^-21) and ONE cubically convergent
