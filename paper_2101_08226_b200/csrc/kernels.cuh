@@ -592,6 +592,120 @@ __global__ void __launch_bounds__(MONO_THREADS, 1) p2p_monopole_kernel(const __g
 }
 
 // ------------------------------------------------------------------------------------------
+// a5 on the FP64 tensor-core instruction (DMMA m8n8k4), the default monopole kernel.
+//
+// The monopole sum is a convolution, out[c][t] = sum_s W[c][s] m[t + s] with weights that depend on the offset only,
+// i.e. a dense contraction, and `mma.sync.m8n8k4.f64` runs on the FP64 pipe at 8 FMAs per lane for FOUR register
+// operands -- measured 37.2 TFLOP/s on this B200 (100 % of the FP64 peak), where a DFMA with three fresh register
+// operands reaches 65 % (register-file read bandwidth).  One DMMA, D(8x8) += A(8x4) B(4x8):
+//   columns j : 8 targets two apart in x (the x-even cells of a 16-cell row segment)
+//   k         : 4 source offsets s_k;  B[k][j] = m[t_j + s_k]
+//   rows i    : component c = i & 3 of (phi, gx, gy, gz) for variant v = i >> 2; v = 0 is the target t_j itself,
+//               v = 1 its x-odd sibling t_j + e_x, for which the SAME source cell sits at offset s_k - e_x:
+//               A[i][k] = W[c][s_k] (v = 0, if s_k is in the list of the even class), W[c][s_k - e_x] (v = 1, if that
+//               is in the list of the odd class), else 0.
+// Siblings share their parent, hence (Eq. 15) almost all of their source cells: the union U of the two lists, in
+// source-cell coordinates, is 0.1 % .. 8 % longer than either list, so 92 - 99.9 % of the multiplications are useful.
+// The host lays U out in chunks of 4 offsets as a table of ready-made A fragments (one double + one tile offset per
+// lane and chunk, identical for every block: read through L1), per (y, z)-parity pair.
+// Block = 8 warps = a 16 x 16 x 8 target tile (two blocks per SM, so that one block's tile load hides behind the
+// other's arithmetic); the masses of tile + halo arrive as one TMA box like in p2p_monopole_kernel.  A warp owns the
+// 16 x-rows of one (y, z)-parity pair in two layers: per chunk it loads one A fragment and 16 B fragments (LDS.64 at
+// compile-time offsets from one address) and issues 16 independent DMMAs.
+// ------------------------------------------------------------------------------------------
+constexpr int DT_Z = 8;
+constexpr int DS_Z = DT_Z + 2 * REACH_MAX;                                   // 18 layers
+constexpr int DMMA_TILE_BYTES = MS_ROW * MS_Y * DS_Z * 8;                    // 104832 B
+constexpr int DMMA_SMEM = DMMA_TILE_BYTES + 64;
+constexpr int DMMA_THREADS = 256;
+constexpr int DMMA_MAX_CHUNKS = (2 * REACH_MAX + 2) * (2 * REACH_MAX + 1) * (2 * REACH_MAX + 1) / 4;   // |U| <= 12 * 11 * 11
+static_assert(2 * DMMA_SMEM <= 227 * 1024, "two blocks per SM");
+
+struct DmmaEntry {
+    double a;      // this lane's element of the A fragment: A[lane >> 2][lane & 3]
+    int off;       // tile offset (doubles) of source offset k = lane & 3, relative to the target row's base
+    int pad;
+};
+struct DmmaLists {
+    int nchunk[4];   // chunks of (py, pz) pair cp = py + 2 pz; its table starts at tab + cp * DMMA_MAX_CHUNKS * 32
+};
+
+__device__ __forceinline__ void dmma_8x8x4(double& d0, double& d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(DMMA_THREADS, 2)
+p2p_monopole_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params p, const DmmaEntry* __restrict__ tab,
+                         const DmmaLists dl, double* __restrict__ out)
+{
+    extern __shared__ __align__(128) unsigned char mono_smem[];
+    double* tile = reinterpret_cast<double*>(mono_smem);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(mono_smem + DMMA_TILE_BYTES);
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const int bx = (p.ox + MT_X - 1) / MT_X, by = (p.oy + MT_Y - 1) / MT_Y;
+    const int b = blockIdx.x;
+    const int x0 = p.lo[0] + (b % bx) * MT_X, y0 = p.lo[1] + ((b / bx) % by) * MT_Y, z0 = p.lo[2] + (b / (bx * by)) * DT_Z;
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_arrive_expect_tx(bar, DMMA_TILE_BYTES);
+        tma_load_tile3(tile, &tmap, bar, x0 >> 1, 2 * y0, z0);
+    }
+    __syncthreads();                 // barrier initialised
+
+    const int cp = warp & 3, py = cp & 1, pz = cp >> 1, half = warp >> 2;
+    // rows of this warp: y = y0 + py + 2 r (r = 0..7), z = z0 + pz + 4 half + 2 zz (zz = 0, 1)
+    const double* base = tile + ((pz + 4 * half + REACH_MAX) * MS_Y + (py + REACH_MAX)) * MS_ROW + (lane >> 2);
+    const int nch = cp == 0 ? dl.nchunk[0] : cp == 1 ? dl.nchunk[1] : cp == 2 ? dl.nchunk[2] : dl.nchunk[3];
+    const int4* t = reinterpret_cast<const int4*>(tab + (size_t)cp * DMMA_MAX_CHUNKS * 32 + lane);
+    double acc[16][2];
+#pragma unroll
+    for (int g = 0; g < 16; ++g) acc[g][0] = acc[g][1] = 0.0;
+    int4 e = __ldg(t);
+    mbar_wait(bar, 0);               // tile in place
+#pragma unroll 1
+    for (int c = 0; c < nch; ++c) {
+        const int4 en = __ldg(t + (size_t)min(c + 1, nch - 1) * 32);       // next chunk's fragment
+        const double a = __hiloint2double(e.y, e.x);
+        const double* q = base + e.z;
+        double m[16];
+#pragma unroll
+        for (int g = 0; g < 16; ++g) m[g] = q[((g >> 3) * 2 * MS_Y + (g & 7) * 2) * MS_ROW];
+#pragma unroll
+        for (int g = 0; g < 16; ++g) dmma_8x8x4(acc[g][0], acc[g][1], a, m[g]);
+        e = en;
+    }
+
+    // D fragment: row = lane >> 2 -> component (lane >> 2) & 3, variant v = lane >> 4; columns 2 (lane & 3) + {0, 1}
+    // -> cells x0 + 4 (lane & 3) + v (d0) and + 2 (d1).  One exchange with lane ^ 16 gives every lane two
+    // x-consecutive cells, so that a warp stores four 128-byte row segments (one per component).
+    const int v = lane >> 4, comp = (lane >> 2) & 3;
+    const int gx = x0 + 4 * (lane & 3) + 2 * v;
+    const long long ocell = (long long)p.ox * p.oy * p.oz;
+#pragma unroll
+    for (int g = 0; g < 16; ++g) {
+        const double send = v ? acc[g][0] : acc[g][1];
+        const double recv = __shfl_xor_sync(0xffffffffu, send, 16);
+        const double lo = v ? recv : acc[g][0], hi = v ? acc[g][1] : recv;
+        const int gy = y0 + py + 2 * (g & 7), k = z0 + pz + 4 * half + 2 * (g >> 3);
+        if (gy < p.hi[1] && k < p.hi[2] && gx < p.hi[0]) {
+            double* dst = out + comp * ocell + ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+            if (gx + 1 < p.hi[0] && (reinterpret_cast<uintptr_t>(dst) & 15) == 0) {
+                *reinterpret_cast<double2*>(dst) = make_double2(lo, hi);
+            } else {
+                dst[0] = lo;
+                if (gx + 1 < p.hi[0]) dst[1] = hi;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // FP64 ALU roofline probe: 8 independent DFMA chains per thread.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double seed)

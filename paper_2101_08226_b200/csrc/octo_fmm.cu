@@ -88,7 +88,7 @@ bool config_ok(const octo_fmm_config* c, int flags = 0)
     return true;
 }
 
-struct Sizes { size_t src, L, C, W, flags, total; };
+struct Sizes { size_t src, L, C, W, T, flags, total; };
 
 Sizes sizes_of(const octo_fmm_config& c, int flags = 0)
 {
@@ -107,9 +107,10 @@ Sizes sizes_of(const octo_fmm_config& c, int flags = 0)
         s.L = align_up(ocell * 4 * sizeof(double));
         s.C = 0;
         s.W = align_up((size_t)MONO_NW * sizeof(double4));
+        s.T = align_up((size_t)4 * DMMA_MAX_CHUNKS * 32 * sizeof(DmmaEntry));
     }
     s.flags = ALIGN;
-    s.total = s.src + s.L + s.C + s.W + s.flags;
+    s.total = s.src + s.L + s.C + s.W + s.T + s.flags;
     return s;
 }
 
@@ -144,6 +145,10 @@ struct octo_fmm {
     int begin[8][2 * REACH_MAX + 2];
     double hmul[2 * REACH_MAX + 1];
     double4* W;            // monopole: device table of the weights of the 11^3 offsets
+    DmmaEntry* T;          // monopole: device table of the A fragments of p2p_monopole_dmma_kernel
+    DmmaLists dl;
+    CUtensorMap tmap2;     // monopole: the 16 x 16 x 8 tile box of p2p_monopole_dmma_kernel
+    int mono_kernel;       // 0 tensor-core instruction (default), 1 DFMA
     unsigned long long n_interactions;
     CUtensorMap tmap;
     Params prm;
@@ -211,6 +216,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->sm_count = prop.multiProcessorCount;
     h->state = 0;
     h->kernel = 0;
+    h->mono_kernel = 0;
     h->host_chunk = 12;
     h->host_launches = 0;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
@@ -290,6 +296,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->L = (double*)w;   w += sz.L;
     h->C = (double*)w;   w += sz.C;
     h->W = (double4*)w;  w += sz.W;
+    h->T = (DmmaEntry*)w; w += sz.T;
     h->flags = (int*)w;
 
     Params& P = h->prm;
@@ -355,6 +362,55 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         if (cudaFuncSetAttribute(p2p_monopole_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MONO_SMEM) != cudaSuccess) {
             delete h; return OCTO_FMM_ECUDA;
         }
+        // ---- p2p_monopole_dmma_kernel: A fragments of the chunks of U = S_even + (S_odd + e_x), per (py, pz) ----
+        {
+            std::vector<DmmaEntry> tab((size_t)4 * DMMA_MAX_CHUNKS * 32, DmmaEntry{0.0, 0, 0});
+            auto widx_of = [](int dx, int dy, int dz) {
+                return ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
+            };
+            for (int cp = 0; cp < 4; ++cp) {
+                const std::vector<Offset3>& Se = h->list[2 * (cp & 1) + 4 * (cp >> 1)];
+                const std::vector<Offset3>& So = h->list[1 + 2 * (cp & 1) + 4 * (cp >> 1)];
+                // membership of a source position (relative to the even target) in the two lists
+                constexpr int NX = 2 * REACH_MAX + 2, NY = 2 * REACH_MAX + 1;
+                std::vector<unsigned char> in_e((size_t)NX * NY * NY, 0), in_o((size_t)NX * NY * NY, 0);
+                auto pos = [&](int sx, int sy, int sz) { return ((size_t)(sz + REACH_MAX) * NY + (sy + REACH_MAX)) * NX + (sx + REACH_MAX); };
+                for (const Offset3& o : Se) in_e[pos(o.d[0], o.d[1], o.d[2])] = 1;
+                for (const Offset3& o : So) in_o[pos(o.d[0] + 1, o.d[1], o.d[2])] = 1;
+                int n = 0;
+                DmmaEntry* tb = tab.data() + (size_t)cp * DMMA_MAX_CHUNKS * 32;
+                for (int sz = -REACH_MAX; sz <= REACH_MAX; ++sz)
+                    for (int sy = -REACH_MAX; sy <= REACH_MAX; ++sy)
+                        for (int sx = -REACH_MAX; sx <= REACH_MAX + 1; ++sx) {
+                            const bool e = in_e[pos(sx, sy, sz)], o = in_o[pos(sx, sy, sz)];
+                            if (!e && !o) continue;
+                            const int chunk = n >> 2, k = n & 3;
+                            const int off = (sz * MS_Y + sy) * MS_ROW + (((sx + REACH_MAX) & 1) ? MS_XH : 0) + ((sx + REACH_MAX) >> 1);
+                            for (int i = 0; i < 8; ++i) {
+                                DmmaEntry& t = tb[(size_t)chunk * 32 + 4 * i + k];
+                                t.off = off;
+                                const int c = i & 3;
+                                double w = 0.0;
+                                if (i < 4 && e) { const double4& q = wt[widx_of(sx, sy, sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
+                                if (i >= 4 && o) { const double4& q = wt[widx_of(sx - 1, sy, sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
+                                t.a = w;
+                            }
+                            ++n;
+                        }
+                h->dl.nchunk[cp] = (n + 3) / 4;     // the padding slots keep a = 0, off = 0 (a valid tile address)
+            }
+            if (cudaMemcpyAsync(h->T, tab.data(), tab.size() * sizeof(DmmaEntry), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
+                cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+            cuuint32_t mbox2[3] = {MS_XH, 2 * MS_Y, DS_Z};
+            std::memset(&h->tmap2, 0, sizeof(h->tmap2));
+            if (enc(&h->tmap2, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void*)h->src, mdims, mstrides, mbox2, mestr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
+                delete h; return OCTO_FMM_ECUDA;
+            }
+            if (cudaFuncSetAttribute(p2p_monopole_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess) {
+                delete h; return OCTO_FMM_ECUDA;
+            }
+        }
     }
     *out = h;
     return OCTO_FMM_OK;
@@ -416,6 +472,10 @@ static int mono_blocks(const Params& P)
 {
     return ((P.ox + MT_X - 1) / MT_X) * ((P.oy + MT_Y - 1) / MT_Y) * ((P.oz + MT_Z - 1) / MT_Z);
 }
+static int dmma_blocks(const Params& P)
+{
+    return ((P.ox + MT_X - 1) / MT_X) * ((P.oy + MT_Y - 1) / MT_Y) * ((P.oz + DT_Z - 1) / DT_Z);
+}
 
 static int brick_blocks(const Params& P) { return ((P.ox + 15) / 16) * ((P.oy + 7) / 8) * ((P.oz + 3) / 4); }
 
@@ -429,7 +489,10 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(h->tmap, P, h->W, h->outL);
+        if (h->mono_kernel == 0)
+            p2p_monopole_dmma_kernel<<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
+        else
+            p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(h->tmap, P, h->W, h->outL);
     } else if (h->kernel == 1) {
         if (h->cfg.am_correction) m2l_direct_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P);
         else                      m2l_direct_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P);
@@ -655,6 +718,11 @@ int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
         h->kernel = value;
         return OCTO_FMM_OK;
     }
+    if (!std::strcmp(key, "mono_kernel")) {      // monopole handles: 0 = FP64 tensor-core instruction (default), 1 = DFMA
+        if (h->cfg.kind != OCTO_FMM_MONOPOLE || (value != 0 && value != 1)) return OCTO_FMM_EINVAL;
+        h->mono_kernel = value;
+        return OCTO_FMM_OK;
+    }
     if (!std::strcmp(key, "dipole_terms")) {     // 0 = decided on the device from the staged sources (default), 1 = always
         if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
         h->prm.force_dipole = value;
@@ -675,7 +743,10 @@ int octo_fmm_launch_info(const octo_fmm_t* h, int* grid, int* block, int* smem_b
     cudaFuncAttributes fa;
     cudaError_t e;
     int g, b, s;
-    if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
+    if (h->cfg.kind == OCTO_FMM_MONOPOLE && h->mono_kernel == 0) {
+        e = cudaFuncGetAttributes(&fa, p2p_monopole_dmma_kernel);
+        g = dmma_blocks(P); b = DMMA_THREADS; s = DMMA_SMEM;
+    } else if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
         e = cudaFuncGetAttributes(&fa, p2p_monopole_kernel);
         g = mono_blocks(P); b = MONO_THREADS; s = MONO_SMEM;
     } else if (h->kernel == 1) {
