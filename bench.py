@@ -513,7 +513,7 @@ def run_ours(args):
                    for mode, name in ((0, "dfma_three_fresh_registers"), (1, "dfma_operand_reuse"), (2, "dmul"))}
     bytes_per_cell = (23 + 23) * 8 if multi else (1 + 4) * 8      # algorithmic: inputs read once, outputs written once
     achieved = flops_per * n_int / (kernel_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "m2l_staged_kernel<correction>" if multi else "p2p_monopole_kernel", "achieved": achieved, "peak": peak_tflops,
+    roofline = {"bound": "alu", "kernel": "m2l_staged_kernel<correction>" if multi else "p2p_monopole_dmma_kernel", "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                 "peak_source": "derived: %d SMs x %d FP64 FMA lanes x 2 x %.0f MHz (sm_max_mhz of %s)" % (
                     sm_count, FP64_LANES_PER_SM, sm_max_mhz, "MEASURED_PEAKS.json" if peaks else "nvidia-smi"),
@@ -523,7 +523,7 @@ def run_ours(args):
                 "fp64_pipe_issue_frac": (instr_per * n_int / (kernel_ms * 1e-3)) / (sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
                 "fp64_issue_probe_frac_of_issue_peak": issue_probe,
                 "kernel_ms": kernel_ms, "interactions_per_launch": n_int,
-                "traffic": TRAFFIC_BYTES.get((args.workload, args.ncell or 256, args.theta)),
+                "traffic": TRAFFIC_BYTES.get((args.workload, int(w.n[0]), args.theta)),
                 "algorithmic_bytes": int(bytes_per_cell * w.moments[0].size),
                 "hbm_gbs_at_algorithmic_bytes": bytes_per_cell * w.moments[0].size / (kernel_ms * 1e-3) / 1e9,
                 "hbm_peak_gbs": peaks.get("hbm_gbs")}
@@ -559,6 +559,8 @@ def run_ours(args):
 TRAFFIC_BYTES = {
     # profiles/r01_final.md: 8.198 GB read + 3.063 GB written per launch
     ("cfg5", 256, 0.5): 11260626000,
+    # profiles/r01_monopole.md (DMMA kernel, 256^3): 151.9 MB read + 478.7 MB written per launch
+    ("cfg4", 256, 0.5): 630586368,
 }
 
 

@@ -377,27 +377,60 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
                 auto pos = [&](int sx, int sy, int sz) { return ((size_t)(sz + REACH_MAX) * NY + (sy + REACH_MAX)) * NX + (sx + REACH_MAX); };
                 for (const Offset3& o : Se) in_e[pos(o.d[0], o.d[1], o.d[2])] = 1;
                 for (const Offset3& o : So) in_o[pos(o.d[0] + 1, o.d[1], o.d[2])] = 1;
-                int n = 0;
-                DmmaEntry* tb = tab.data() + (size_t)cp * DMMA_MAX_CHUNKS * 32;
+                // the offsets of U in (sz, sy, sx) order
+                struct Src { int sx, sy, sz, off; bool e, o; };
+                std::vector<Src> U;
                 for (int sz = -REACH_MAX; sz <= REACH_MAX; ++sz)
                     for (int sy = -REACH_MAX; sy <= REACH_MAX; ++sy)
                         for (int sx = -REACH_MAX; sx <= REACH_MAX + 1; ++sx) {
                             const bool e = in_e[pos(sx, sy, sz)], o = in_o[pos(sx, sy, sz)];
                             if (!e && !o) continue;
-                            const int chunk = n >> 2, k = n & 3;
                             const int off = (sz * MS_Y + sy) * MS_ROW + (((sx + REACH_MAX) & 1) ? MS_XH : 0) + ((sx + REACH_MAX) >> 1);
-                            for (int i = 0; i < 8; ++i) {
-                                DmmaEntry& t = tb[(size_t)chunk * 32 + 4 * i + k];
-                                t.off = off;
-                                const int c = i & 3;
-                                double w = 0.0;
-                                if (i < 4 && e) { const double4& q = wt[widx_of(sx, sy, sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
-                                if (i >= 4 && o) { const double4& q = wt[widx_of(sx - 1, sy, sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
-                                t.a = w;
-                            }
-                            ++n;
+                            U.push_back(Src{sx, sy, sz, off, e, o});
                         }
-                h->dl.nchunk[cp] = (n + 3) / 4;     // the padding slots keep a = 0, off = 0 (a valid tile address)
+                // Chunks of 4 offsets whose B-fragment load has no shared-memory bank conflict.  An LDS.64 is served
+                // per half-warp = 4 targets (j) x 4 offsets (k), addresses off_k + j: two offsets are compatible if
+                // their 4-double segments overlap in ADDRESS (|difference| <= 3: broadcast) or are at least 4 banks
+                // (of 8 bytes, 16 per 128-byte wavefront) apart.  Greedy in list order; the few slots left empty
+                // repeat the chunk's first offset with zero weights.
+                auto compatible = [](int a, int b) {
+                    const int d = b - a;
+                    if (d >= -3 && d <= 3) return true;
+                    const int D = ((d % 16) + 16) % 16;
+                    return D >= 4 && D <= 12;
+                };
+                std::vector<char> used(U.size(), 0);
+                DmmaEntry* tb = tab.data() + (size_t)cp * DMMA_MAX_CHUNKS * 32;
+                int nchunk = 0;
+                bool overflow = false;
+                for (size_t first = 0; first < U.size(); ++first) {
+                    if (used[first]) continue;
+                    if (nchunk == DMMA_MAX_CHUNKS) { overflow = true; break; }
+                    size_t member[4];
+                    int nm = 0;
+                    member[nm++] = first; used[first] = 1;
+                    for (size_t j = first + 1; j < U.size() && nm < 4; ++j) {
+                        if (used[j]) continue;
+                        bool ok = true;
+                        for (int k = 0; k < nm; ++k) ok = ok && compatible(U[member[k]].off, U[j].off);
+                        if (ok) { member[nm++] = j; used[j] = 1; }
+                    }
+                    for (int k = 0; k < 4; ++k) {
+                        const Src* u = k < nm ? &U[member[k]] : nullptr;
+                        for (int i = 0; i < 8; ++i) {
+                            DmmaEntry& t = tb[(size_t)nchunk * 32 + 4 * i + k];
+                            t.off = u ? u->off : U[first].off;
+                            const int c = i & 3;
+                            double w = 0.0;
+                            if (u && i < 4 && u->e) { const double4& q = wt[widx_of(u->sx, u->sy, u->sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
+                            if (u && i >= 4 && u->o) { const double4& q = wt[widx_of(u->sx - 1, u->sy, u->sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
+                            t.a = w;
+                        }
+                    }
+                    ++nchunk;
+                }
+                if (overflow) { delete h; return OCTO_FMM_EINVAL; }
+                h->dl.nchunk[cp] = nchunk;
             }
             if (cudaMemcpyAsync(h->T, tab.data(), tab.size() * sizeof(DmmaEntry), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
                 cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
