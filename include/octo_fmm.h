@@ -123,7 +123,7 @@ int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *c
 
 /* The dipole terms.  Sources expanded about their centre of mass have M^(1) = 0 up to round-off, and the 27
  * terms that contain M^(1) then contribute nothing.  set_moments() checks on the device whether every cell
- * has |M^(1)_i| <= 4e-16 |M| h; if so interact() leaves those terms out (245 instead of 301 flop per
+ * has |M^(1)_i| <= 4e-16 |M| h; if so interact() leaves those terms out (188 instead of 224 flop per
  * interaction), otherwise it evaluates them -- results agree with the general formula to round-off either
  * way.  octo_fmm_set_option(h, "dipole_terms", 1) forces the general path.  After set_moments(),
  * octo_fmm_dipole_terms_used() synchronises the stream and tells which path interact() takes. */
@@ -134,7 +134,10 @@ int octo_fmm_dipole_terms_used(octo_fmm_t *h, int *used);
  * a warp-level reduction of the partial expansions (default up to 4096 target cells).
  * "dipole_terms" = 0 decided on the device (default), 1 always evaluated.
  * "host_chunk" = output z-layers per pipeline slab of octo_fmm_run_host (default 12; 0 = one copy in, one
- * launch, one copy out).  Unknown keys -> EINVAL. */
+ * launch, one copy out).
+ * "mono_kernel" (MONOPOLE handles) = 0 the sum as 8x8x4 FP64 tensor-core contractions (mma.sync m8n8k4.f64:
+ * 16-cell row segments x 4 offsets per instruction; default), 1 the same sum with DFMAs.  Both follow the list
+ * of Eq. 15 and agree to round-off (the summation order differs).  Unknown keys -> EINVAL. */
 int octo_fmm_set_option(octo_fmm_t *h, const char *key, int value);
 
 /* Launch facts of the interaction kernel the handle would run: grid, block, dynamic shared

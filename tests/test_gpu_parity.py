@@ -368,6 +368,48 @@ def test_monopole_non_cubic_grid_and_sub_region(env):
         g.close()
 
 
+@pytest.mark.parametrize("theta", [0.5, 0.35, 0.7])
+@pytest.mark.parametrize("mono_kernel", [0, 1])
+def test_monopole_tensor_core_and_dfma_kernels(env, theta, mono_kernel):
+    """a5 by both kernels (0: the sum as 8x8x4 FP64 tensor-core contractions over even/odd sibling pairs, the default;
+    1: DFMA) against the oracle: a 40 x 24 x 16 grid (tiles ragged in y and z, every domain face) and an interior region
+    that starts and ends inside 16-cell row segments."""
+    p, torch = env
+    n = (40, 24, 16)
+    w = fi.config4(ncell=40)
+    mass = np.ascontiguousarray(w.moments[0][:n[2], :n[1], :n[0]])
+    for lo, hi in (((0, 0, 0), (0, 0, 0)), ((8, 8, 0), (32, 24, 8))):
+        g = p.OctoFMM(n, w.h, theta, p.MONOPOLE, out_lo=lo, out_hi=hi)
+        g.set_option("mono_kernel", mono_kernel)
+        assert g.launch_info()["block"] == (256 if mono_kernel == 0 else 512)
+        out, _ = g.solve(torch.from_numpy(mass).cuda())
+        torch.cuda.synchronize()
+        olo, ohi = ((0, 0, 0), n) if hi == (0, 0, 0) else (lo, hi)
+        ref, cnt = oracle.interact_monopole(n, w.h, theta, mass, olo, ohi)
+        assert g.interaction_count() == cnt
+        assert parity_error(out.cpu().numpy(), ref) < TOL
+        g.close()
+
+
+def test_monopole_tensor_core_kernel_unaligned_bound_output(env):
+    """The tensor-core kernel stores pairs of x-neighbours with 16-byte stores; a bound output buffer that is only
+    8-byte aligned must take the scalar path and give the same numbers."""
+    p, torch = env
+    w = fi.config4(ncell=32)
+    m = torch.from_numpy(w.moments).cuda()
+    f = p.OctoFMM(w.n, w.h, 0.5, p.MONOPOLE)
+    ref, _ = f.solve(m)
+    buf = torch.zeros(4 * 32 ** 3 + 1, dtype=torch.float64, device="cuda")
+    view = buf[1:].view(4, 32, 32, 32)
+    assert view.data_ptr() % 16 == 8
+    f.bind_outputs(view)
+    f.set_moments(m)
+    f.interact()
+    torch.cuda.synchronize()
+    assert torch.equal(view, ref)
+    f.close()
+
+
 @pytest.mark.parametrize("kernel", [0, 1, 2])
 def test_dipole_terms_are_left_out_only_when_every_cell_has_none(env, kernel):
     """The device decides at staging: centre-of-mass expansions (|M1| ~ 1e-19 m h here) take the path without the
