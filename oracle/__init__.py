@@ -54,6 +54,7 @@ def lib():
         L.fmm_oracle_stencil_leaf.argtypes = L.fmm_oracle_stencil.argtypes
         L.fmm_oracle_interact_monopole_leaf.argtypes = L.fmm_oracle_interact_monopole.argtypes
         L.fmm_oracle_m2m.argtypes = [ip, ctypes.c_double, dp, dp, dp, dp]
+        L.fmm_oracle_m2m_about.argtypes = [ip, ctypes.c_double, dp, dp, dp, dp]
         L.fmm_oracle_l2l.argtypes = [ip, ctypes.c_double, dp, dp, dp, dp, dp, dp]
         L.fmm_oracle_direct_sum.argtypes = [ip, ctypes.c_double, dp, dp]
         L.fmm_oracle_num_threads.restype = ctypes.c_int
@@ -194,6 +195,20 @@ def m2m(n_child, h_child, moments, com_off):
     return pm, po
 
 
+def m2m_about(n_child, h_child, moments, com_off, parent_off):
+    """Parent multipoles [20][n/2] about PRESCRIBED parent centres parent_off [3][n/2] (second right-hand side, L81-83)."""
+    nx, ny, nz = n_child
+    moments = np.ascontiguousarray(moments, dtype=np.float64)
+    com_off = np.ascontiguousarray(com_off, dtype=np.float64)
+    parent_off = np.ascontiguousarray(parent_off, dtype=np.float64)
+    assert moments.shape == (20, nz, ny, nx) and com_off.shape == (3, nz, ny, nx)
+    assert parent_off.shape == (3, nz // 2, ny // 2, nx // 2)
+    pm = np.zeros((20, nz // 2, ny // 2, nx // 2))
+    _check(lib().fmm_oracle_m2m_about(_i3(n_child), float(h_child), _dp(moments), _dp(com_off), _dp(parent_off), _dp(pm)),
+           "m2m_about")
+    return pm
+
+
 def l2l(n_child, h_child, parent_L, parent_corr, parent_off, child_off, child_L, child_corr):
     """child_L += parent_L shifted to the child centres, child_corr += parent_corr (in place; L125)."""
     for a in (parent_L, parent_corr, parent_off, child_off, child_L, child_corr):
@@ -208,6 +223,44 @@ def direct_sum(n, h, mass):
     mass = np.ascontiguousarray(mass, dtype=np.float64).reshape(nz, ny, nx)
     out = np.zeros((4, nz, ny, nx))
     _check(lib().fmm_oracle_direct_sum(_i3(n), float(h), _dp(mass), _dp(out)), "direct_sum")
+    return out
+
+
+def solve_rhs2(n, h, theta, mass, dmass, coarsest=2):
+    """Second right-hand side (Alg. 1: "Compute g, phi, and d(phi)/dt using the FMM ... with
+    the numerically computed value of d(rho)/dt as the source term"): the same tree, lists and EXPANSION CENTRES as
+    solve(n, h, theta, mass) -- the centres of mass of `mass` -- but the sources are the signed point sources
+    `dmass` at the leaf centres, and no angular-momentum correction (it belongs to the force, L127).
+    Returns out[4][n][n][n] = (d(phi)/dt, -grad of it)."""
+    n = int(n)
+    mass = np.ascontiguousarray(mass, dtype=np.float64).reshape(n, n, n)
+    dmass = np.ascontiguousarray(dmass, dtype=np.float64).reshape(n, n, n)
+    # ---- centres: upward pass of the density ----
+    lev_n, lev_h = [n], [float(h)]
+    mom = np.zeros((20, n, n, n)); mom[0] = mass
+    mom2 = np.zeros((20, n, n, n)); mom2[0] = dmass
+    lev_m, lev_o, lev_m2 = [mom], [np.zeros((3, n, n, n))], [mom2]
+    while lev_n[-1] > coarsest:
+        nc, hc = lev_n[-1], lev_h[-1]
+        pm, po = m2m((nc, nc, nc), hc, lev_m[-1], lev_o[-1])
+        pm2 = m2m_about((nc, nc, nc), hc, lev_m2[-1], lev_o[-1], po)
+        lev_n.append(nc // 2); lev_h.append(2.0 * hc); lev_m.append(pm); lev_o.append(po); lev_m2.append(pm2)
+    # ---- downward pass of the second right-hand side ----
+    L_par = None
+    for lv in range(len(lev_n) - 1, 0, -1):
+        nl, hl = lev_n[lv], lev_h[lv]
+        L, Lc, _ = interact_multipole((nl, nl, nl), hl, theta, lev_m2[lv], lev_o[lv], None, None, False)
+        L = L.copy()
+        zero_c = np.zeros_like(Lc)
+        if L_par is not None:
+            l2l((nl, nl, nl), hl, L_par, np.zeros((3,) + L_par.shape[1:]), lev_o[lv + 1], lev_o[lv], L, zero_c)
+        L_par = L
+    out, _ = interact_monopole_leaf((n, n, n), h, theta, dmass)
+    if L_par is not None:
+        Ll = np.zeros((20, n, n, n)); cl = np.zeros((3, n, n, n))
+        l2l((n, n, n), h, L_par, np.zeros((3,) + L_par.shape[1:]), lev_o[1], lev_o[0], Ll, cl)
+        out[0] += Ll[0]
+        out[1:4] -= Ll[1:4]
     return out
 
 

@@ -496,8 +496,10 @@ static void unpack_moments(const double *u, size_t stride, double *M0, double M1
  *   M1'_i = M1_i + M d_i;  M2'_ij = M2_ij + M1_i d_j + M1_j d_i + M d_i d_j;
  *   M3'_ijk = M3_ijk + M2_ij d_k + M2_ik d_j + M2_jk d_i + M1_i d_j d_k + M1_j d_i d_k + M1_k d_i d_j + M d_i d_j d_k.
  * pm = [20][nz/2][ny/2][nx/2], poff = [3][...].
+ * given != 0 (second right-hand side, L81-83: the time derivative of the density expanded about the centres
+ * of the density itself): delta_P is READ from poff instead of being computed; the shift is the same.
  */
-int fmm_oracle_m2m(const int nc[3], double hc, const double *cm, const double *coff, double *pm, double *poff)
+static int m2m_impl(const int nc[3], double hc, const double *cm, const double *coff, double *pm, double *poff, int given)
 {
     if (!nc || !cm || !coff || !pm || !poff || !(hc > 0.0)) return ORC_EINVAL;
     for (int a = 0; a < 3; ++a)
@@ -519,7 +521,10 @@ int fmm_oracle_m2m(const int nc[3], double hc, const double *cm, const double *c
                     for (int i = 0; i < 3; ++i) com[i] += (long double)(M0[c] * rel[c][i]) + (long double)M1[c][i];
                 }
                 double dP[3] = {0.0, 0.0, 0.0};
-                if (mass != 0.0L)
+                const size_t P = (K * py + J) * px + I;
+                if (given)
+                    for (int i = 0; i < 3; ++i) dP[i] = poff[(size_t)i * pcell + P];
+                else if (mass != 0.0L)
                     for (int i = 0; i < 3; ++i) dP[i] = (double)(com[i] / mass);
                 long double S1[3] = {0, 0, 0}, S2[3][3], S3[3][3][3];
                 memset(S2, 0, sizeof S2);
@@ -538,7 +543,6 @@ int fmm_oracle_m2m(const int nc[3], double hc, const double *cm, const double *c
                                                              M2[c][j][k] * d[i] + M1[c][i] * d[j] * d[k] + M1[c][j] * d[i] * d[k] +
                                                              M1[c][k] * d[i] * d[j] + M0[c] * d[i] * d[j] * d[k]);
                 }
-                const size_t P = (K * py + J) * px + I;
                 pm[P] = (double)mass;
                 for (int i = 0; i < 3; ++i) pm[(size_t)(1 + i) * pcell + P] = (double)S1[i];
                 for (int i = 0; i < 3; ++i)
@@ -546,9 +550,21 @@ int fmm_oracle_m2m(const int nc[3], double hc, const double *cm, const double *c
                 for (int i = 0; i < 3; ++i)
                     for (int j = i; j < 3; ++j)
                         for (int k = j; k < 3; ++k) pm[(size_t)(10 + u3(i, j, k)) * pcell + P] = (double)S3[i][j][k];
-                for (int i = 0; i < 3; ++i) poff[(size_t)i * pcell + P] = dP[i];
+                if (!given)
+                    for (int i = 0; i < 3; ++i) poff[(size_t)i * pcell + P] = dP[i];
             }
     return ORC_OK;
+}
+
+int fmm_oracle_m2m(const int nc[3], double hc, const double *cm, const double *coff, double *pm, double *poff)
+{
+    return m2m_impl(nc, hc, cm, coff, pm, poff, 0);
+}
+
+/* M2M about PRESCRIBED parent centres: poff (in) = delta_P of every parent cell; pm (out). */
+int fmm_oracle_m2m_about(const int nc[3], double hc, const double *cm, const double *coff, const double *poff, double *pm)
+{
+    return m2m_impl(nc, hc, cm, coff, pm, (double *)poff, 1);
 }
 
 /*

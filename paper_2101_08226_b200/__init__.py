@@ -82,6 +82,7 @@ class _Library:
         lib.octo_fmm_solver_workspace_bytes.argtypes = [scfgp]
         lib.octo_fmm_solver_create.argtypes = [scfgp, ctypes.POINTER(vp)]
         lib.octo_fmm_solver_solve.argtypes = [vp, vp, vp]
+        lib.octo_fmm_solver_solve_rhs2.argtypes = [vp, vp, vp]
         lib.octo_fmm_solver_status.argtypes = [vp]
         lib.octo_fmm_solver_host_scratch_bytes.restype = ctypes.c_size_t
         lib.octo_fmm_solver_host_scratch_bytes.argtypes = [scfgp]
@@ -286,6 +287,12 @@ def octo_fmm_solver_solve(s, mass, out):
         raise OctoFmmError("octo_fmm_solver_solve", rc)
 
 
+def octo_fmm_solver_solve_rhs2(s, dmass, out):
+    rc = _lib.octo_fmm_solver_solve_rhs2(s, _ptr(dmass), _ptr(out))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_solve_rhs2", rc)
+
+
 def octo_fmm_solver_host_scratch_bytes(cfg):
     return int(_lib.octo_fmm_solver_host_scratch_bytes(ctypes.byref(cfg)))
 
@@ -359,6 +366,13 @@ class OctoFMMSolver:
         if out is None:
             out = self.torch.empty((4, self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
         octo_fmm_solver_solve(self.handle, mass, out)
+        return out
+
+    def solve_rhs2(self, dmass, out=None):
+        """(d(phi)/dt, -grad) of the sources dmass on the tree and centres of the last solve()."""
+        if out is None:
+            out = self.torch.empty((4, self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
+        octo_fmm_solver_solve_rhs2(self.handle, dmass, out)
         return out
 
     def status(self):

@@ -37,8 +37,10 @@ static_assert(u3(0, 0, 0) == 0 && u3(0, 1, 0) == 1 && u3(2, 0, 0) == 2 && u3(1, 
 //   rel_c = ((a,b,c) - 1/2) hc + delta_c;   delta_P = sum_c (M_c rel_c + M1_c) / sum_c M_c  (0 if the mass is 0)
 //   d = rel_c - delta_P;  M1' = M1 + M d;  M2'_ij = M2_ij + M1_i d_j + M1_j d_i + M d_i d_j;
 //   M3'_ijk = M3_ijk + (M2_ij d_k + M2_ik d_j + M2_jk d_i) + (M1_i d_j d_k + M1_j d_i d_k + M1_k d_i d_j) + M d_i d_j d_k
+// GIVEN (second right-hand side, L81-83: d(rho)/dt expanded about the centres of rho): delta_P is read from poff
+// instead of being computed and written; coff are then the children's centres from the first right-hand side.
 // ------------------------------------------------------------------------------------------
-template <bool LEAF>
+template <bool LEAF, bool GIVEN = false>
 __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm, const double* __restrict__ coff,
                                                   double* __restrict__ pm, double* __restrict__ poff, int pnx, int pny, int pnz,
                                                   double hc)
@@ -72,7 +74,10 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
         mass += m0;
     }
     double dP[3] = {0.0, 0.0, 0.0};
-    if (mass != 0.0) {
+    if (GIVEN) {
+#pragma unroll
+        for (int i = 0; i < 3; ++i) dP[i] = poff[i * pcell + P];
+    } else if (mass != 0.0) {
 #pragma unroll
         for (int i = 0; i < 3; ++i) dP[i] = com[i] / mass;
     }
@@ -108,8 +113,10 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
     }
 #pragma unroll
     for (int t = 0; t < 20; ++t) pm[t * pcell + P] = S[t];
+    if (!GIVEN) {
 #pragma unroll
-    for (int i = 0; i < 3; ++i) poff[i * pcell + P] = dP[i];
+        for (int i = 0; i < 3; ++i) poff[i * pcell + P] = dP[i];
+    }
 }
 
 // Taylor shift of a parent expansion L (20 unique components in registers) by e, orders 0..NORD:

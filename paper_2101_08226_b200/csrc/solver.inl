@@ -49,6 +49,7 @@ struct octo_fmm_solver {
     std::vector<SolverLevel> lev;     // lev[0] = n/2, ..., lev.back() = 2
     cudaStream_t stream;
     unsigned long long n_interactions;
+    bool have_centres;    // solve() has run: lev[].off hold the expansion centres of the density
 };
 
 extern "C" {
@@ -92,6 +93,7 @@ int octo_fmm_solver_create(const octo_fmm_solver_config* cfg, octo_fmm_solver_t*
     s->leaf = nullptr;
     s->stream = (cudaStream_t)cfg->stream;
     s->n_interactions = 0;
+    s->have_centres = false;
     char* w = (char*)cfg->workspace;
     {
         octo_fmm_config lc = level_config(*cfg, cfg->n, cfg->h, OCTO_FMM_MONOPOLE);
@@ -154,6 +156,55 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     // ---- leaves: monopole sum over the leaf-level list straight into `out`, then the parent's expansion ----
+    double* const keep = s->leaf->outL;
+    s->leaf->outL = out;
+    rc = octo_fmm_interact(s->leaf);
+    s->leaf->outL = keep;
+    if (rc != OCTO_FMM_OK) return rc;
+    {
+        const int n = s->cfg.n;
+        SolverLevel& p = s->lev[0];
+        leaf_eval_kernel<<<dim3((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2)), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    s->have_centres = true;
+    return OCTO_FMM_OK;
+}
+
+// Second right-hand side (L81-83): the same passes with the sources d(mass)/dt, about the centres the last solve()
+// left in lev[].off, without the angular-momentum correction (the level handles are switched for the duration).
+int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t* s, const double* dmass, double* out)
+{
+    if (!s || !dmass || !out) return OCTO_FMM_EINVAL;
+    if (((uintptr_t)dmass % 16) || ((uintptr_t)out % 16)) return OCTO_FMM_EINVAL;
+    if (!s->have_centres) return OCTO_FMM_ESTATE;
+    if (cudaSetDevice(s->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaStream_t st = s->stream;
+    int rc;
+    if ((rc = octo_fmm_set_moments(s->leaf, dmass, nullptr)) != OCTO_FMM_OK) return rc;
+    for (size_t lv = 0; lv < s->lev.size(); ++lv) {
+        SolverLevel& l = s->lev[lv];
+        const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
+        if (lv == 0) m2m_kernel<true, true><<<blocks, 128, 0, st>>>(dmass, nullptr, l.raw, l.off, l.n, l.n, l.n, s->cfg.h);
+        else         m2m_kernel<false, true><<<blocks, 128, 0, st>>>(s->lev[lv - 1].raw, s->lev[lv - 1].off, l.raw, l.off, l.n, l.n,
+                                                                    l.n, s->lev[lv - 1].h);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    for (int lv = (int)s->lev.size() - 1; lv >= 0; --lv) {
+        SolverLevel& l = s->lev[lv];
+        const int keep_corr = l.fmm->cfg.am_correction;
+        l.fmm->cfg.am_correction = 0;
+        rc = octo_fmm_set_moments(l.fmm, l.raw, l.off);
+        if (rc == OCTO_FMM_OK) rc = octo_fmm_interact(l.fmm);       // writes C = 0
+        l.fmm->cfg.am_correction = keep_corr;
+        if (rc != OCTO_FMM_OK) return rc;
+        if (lv < (int)s->lev.size() - 1) {
+            SolverLevel& p = s->lev[lv + 1];
+            const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
+            l2l_kernel<true><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, p.fmm->L, p.fmm->C, p.off, l.n, l.n, l.n, l.h);
+            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        }
+    }
     double* const keep = s->leaf->outL;
     s->leaf->outL = out;
     rc = octo_fmm_interact(s->leaf);

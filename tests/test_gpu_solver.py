@@ -131,3 +131,33 @@ def test_solve_host_entry_point(env):
     with pytest.raises(p.OctoFmmError):
         p.octo_fmm_solver_solve_host(s.handle, m_h, o_h, scratch, nb - 1)
     s.close()
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.35])
+def test_second_right_hand_side_32(env, theta):
+    """f2 (L81-83): d(phi)/dt from d(mass)/dt on the tree and the expansion centres of the density's solve, no
+    correction, against the oracle's solve_rhs2; signed sources with zero net change."""
+    p, torch = env
+    n, h = 32, 1.0 / 32
+    rng = np.random.default_rng(12)
+    mass = rng.uniform(0.5, 1.5, (n, n, n)) * h ** 3
+    dm = rng.uniform(-1.0, 1.0, (n, n, n)) * h ** 3
+    dm -= dm.mean()
+    s = p.OctoFMMSolver(n, h, theta, True)
+    with pytest.raises(p.OctoFmmError):                       # no centres before the first solve
+        s.solve_rhs2(torch.from_numpy(dm).cuda())
+    out = s.solve(torch.from_numpy(mass).cuda()).clone()
+    out2 = s.solve_rhs2(torch.from_numpy(dm).cuda())
+    torch.cuda.synchronize()
+    assert s.status() == p.OK
+    ref2 = oracle.solve_rhs2(n, h, theta, mass, dm)
+    e_phi, e_g = _errors(out2.cpu().numpy(), ref2)
+    assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+    # the density's solve is unchanged by the second right-hand side having run on the same handles
+    again = s.solve(torch.from_numpy(mass).cuda())
+    torch.cuda.synchronize()
+    assert torch.equal(again, out)
+    ref = oracle.solve(n, h, theta, mass, True)
+    e_phi, e_g = _errors(out.cpu().numpy(), ref)
+    assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+    s.close()

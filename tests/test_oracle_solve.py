@@ -161,3 +161,67 @@ def test_uniform_sphere_residuals_are_of_the_order_the_paper_prints(ncell, theta
         out5 = oracle.solve(ncell, h, 0.5, mass)
         eps5 = np.abs(out5[0] - phi) / np.abs(phi)
         assert eps.max() < 0.6 * eps5.max() and eps.mean() < 0.8 * eps5.mean()
+
+
+# ---- second right-hand side (Alg. 1) ----
+
+def test_m2m_about_prescribed_centres_equals_p2m_of_all_constituents():
+    """Signed point sources (a time derivative of a density) in two levels of cells: the parent moments about a
+    PRESCRIBED centre (the density's, here random) equal the moments of all 64 points about that centre."""
+    rng = np.random.default_rng(8)
+    hc = 0.25
+    n = (4, 4, 4)
+    mom = np.zeros((20,) + n)
+    off = rng.uniform(-0.3, 0.3, (3,) + n) * hc                      # the children's centres: not the sources' own
+    poff = rng.uniform(-0.3, 0.3, (3, 2, 2, 2)) * 2 * hc
+    pts = {}
+    for k, j, i in itertools.product(range(4), repeat=3):
+        centre = (np.array([i, j, k]) + 0.5) * hc
+        y = centre + rng.uniform(-0.5, 0.5, (8, 3)) * hc
+        m = rng.uniform(-1.0, 1.0, 8)
+        mom[:, k, j, i] = moments_of_points(m, y, centre + off[:, k, j, i])
+        pts[(i, j, k)] = (m, y)
+    pm = oracle.m2m_about(n, hc, mom, off, poff)
+    for K, J, I in itertools.product(range(2), repeat=3):
+        ms = np.concatenate([pts[(2 * I + a, 2 * J + b, 2 * K + c)][0] for c in range(2) for b in range(2) for a in range(2)])
+        ys = np.concatenate([pts[(2 * I + a, 2 * J + b, 2 * K + c)][1] for c in range(2) for b in range(2) for a in range(2)])
+        ref = moments_of_points(ms, ys, (np.array([I, J, K]) + 0.5) * 2 * hc + poff[:, K, J, I])
+        tot = np.abs(ms).sum()
+        scale = np.array([tot] + [tot * hc] * 3 + [tot * hc ** 2] * 6 + [tot * hc ** 3] * 10)
+        assert (np.abs(pm[:, K, J, I] - ref) / scale).max() < 5e-15
+    # with the centres M2M itself computes, the two routines agree
+    mom_pos = np.abs(mom); mom_pos[1:] = mom[1:]
+    pm1, po1 = oracle.m2m(n, hc, mom_pos, off)
+    assert np.array_equal(oracle.m2m_about(n, hc, mom_pos, off, po1), pm1)
+
+
+def test_second_right_hand_side_is_linear_and_uses_the_centres_of_the_density(random16):
+    """d(mass)/dt proportional to the mass has the density's own centres, so the second right-hand side must be that
+    multiple of the solve without the correction -- to round-off, at every cell."""
+    n, h, mass, _ = random16
+    base = oracle.solve(n, h, 0.5, mass, am_correction=False)
+    got = oracle.solve_rhs2(n, h, 0.5, mass, -0.37 * mass)
+    assert np.abs(got + 0.37 * base).max() / np.abs(base).max() < 1e-15
+    # linear in the sources
+    rng = np.random.default_rng(5)
+    d1, d2 = (rng.uniform(-1, 1, (n, n, n)) * h ** 3 for _ in range(2))
+    s12 = oracle.solve_rhs2(n, h, 0.5, mass, d1 + 2.0 * d2)
+    s1, s2 = oracle.solve_rhs2(n, h, 0.5, mass, d1), oracle.solve_rhs2(n, h, 0.5, mass, d2)
+    assert np.abs(s12 - (s1 + 2.0 * s2)).max() / np.abs(s12).max() < 1e-13
+
+
+@pytest.mark.parametrize("theta,tol", [(0.5, 4e-3), (0.35, 1e-3)])
+def test_second_right_hand_side_against_the_exact_point_sum(random16, theta, tol):
+    """A smooth signed source (mass flowing from one half of the box to the other, zero net change): the potential
+    rate agrees with the exact sum over the point sources within the truncation error, falling with theta."""
+    n, h, mass, _ = random16
+    x = (np.arange(n) + 0.5) * h
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    dm = mass * np.sin(2 * np.pi * X) * np.cos(np.pi * Y)
+    dm -= dm.mean()
+    ref = oracle.direct_sum((n, n, n), h, dm)
+    got = oracle.solve_rhs2(n, h, theta, mass, dm)
+    e_phi = np.abs(got[0] - ref[0]).max() / np.abs(ref[0]).max()
+    e_g = np.abs(got[1:] - ref[1:]).max() / np.abs(ref[1:]).max()
+    assert e_phi < tol and e_g < 10 * tol, (e_phi, e_g)
+    assert e_phi > tol / 100
