@@ -239,6 +239,21 @@ def run_solve(args):
     if s.status() != p.OK:
         raise SystemExit("bench.py: device reported status %d" % s.status())
     eps = np.abs(out[0].cpu().numpy() - phi) / np.abs(phi)
+    # the second right-hand side (f2, L81-83) on the same tree and centres, timed beside the solve (not part of `value`):
+    # d(mass)/dt of a rigid drift of the sphere along x, u . grad(rho) by central differences
+    dm_d = (torch.roll(m_d, 1, 2) - torch.roll(m_d, -1, 2)) * (0.5 / h)
+    out2 = torch.empty((n, n, n), dtype=torch.float64, device=dev)
+    s.solve_rhs2(dm_d, out2)
+    torch.cuda.synchronize()
+    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev2.record(stream)
+    for _ in range(args.steps):
+        s.solve_rhs2(dm_d, out2)
+    ev3.record(stream)
+    torch.cuda.synchronize()
+    rhs2_ms = ev2.elapsed_time(ev3) / args.steps
+    s.solve(m_d, out)
+    torch.cuda.synchronize()
     # end to end through the host-buffer entry point
     nb = p.octo_fmm_solver_host_scratch_bytes(s.cfg)
     scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
@@ -280,6 +295,9 @@ def run_solve(args):
                              "sample": "oracle.solve of the same problem at %d^3 (%d interactions) in %.1f s" % (nref, cnt_ref, t_ref)},
             "e2e": {"value": n_int / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(mass.nbytes),
                     "d2h_bytes_per_step": int(o_h.numel() * 8), "ms_per_step": e2e_ms},
+            "second_rhs": {"ms_per_solve": rhs2_ms, "value": n_int / (rhs2_ms * 1e-3), "unit": UNIT,
+                           "note": "octo_fmm_solver_solve_rhs2: d(phi)/dt from d(mass)/dt on the same tree and centres, "
+                                   "correction off, dipole terms on; timed beside the solve, not part of value"},
             "clocks": clocks, "gpu_launches": launches * args.steps}
     print(json.dumps(line))
     s.close()

@@ -196,13 +196,15 @@ int octo_fmm_solver_create(const octo_fmm_solver_config *cfg, octo_fmm_solver_t 
 int octo_fmm_solver_solve(octo_fmm_solver_t *s, const double *mass, double *out);
 /* Second right-hand side (Alg. 1: "Compute g, phi, and d(phi)/dt using the
  * FMM ... with the numerically computed value of d(rho)/dt as the source term").  dmass: device, [n][n][n], the
- * time derivative of the cell masses (any sign); out: device, [4][n][n][n] = (d(phi)/dt, minus its gradient).
+ * time derivative of the cell masses (any sign); dphi_dt: device, [n][n][n] (only the potential of this solve is
+ * used, Eq. 3; both 16-byte aligned).
  * Same tree, lists, kernels and EXPANSION CENTRES as the last octo_fmm_solver_solve() on this handle (the centres
  * of mass of the density, kept in the workspace; ESTATE if there was none), no angular-momentum correction (it
  * belongs to the force, L127), all dipole terms evaluated (the sources are not expanded about their own centres).
- * Asynchronous on the stream; overwrites the per-level results of solve().  The two right-hand sides share the
- * geometry, not the pair arithmetic: DESIGN.md section 10a says why a fused kernel was not built. */
-int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t *s, const double *dmass, double *out);
+ * Asynchronous on the stream; overwrites the per-level results of solve().  At the multipole levels the two
+ * right-hand sides share the geometry, not the pair arithmetic (DESIGN.md section 10a says why a fused kernel was
+ * not built); the leaf sum is a potential-only tensor-core contraction over the 8 children of a parent. */
+int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t *s, const double *dmass, double *dphi_dt);
 /* The same with HOST buffers: H2D of the masses into scratch, solve, D2H of out, stream synchronise.
  * scratch: device, >= octo_fmm_solver_host_scratch_bytes(cfg), borrowed for the call. */
 size_t octo_fmm_solver_host_scratch_bytes(const octo_fmm_solver_config *cfg);

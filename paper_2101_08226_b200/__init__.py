@@ -369,9 +369,9 @@ class OctoFMMSolver:
         return out
 
     def solve_rhs2(self, dmass, out=None):
-        """(d(phi)/dt, -grad) of the sources dmass on the tree and centres of the last solve()."""
+        """d(phi)/dt [n][n][n] of the sources dmass on the tree and centres of the last solve()."""
         if out is None:
-            out = self.torch.empty((4, self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
+            out = self.torch.empty((self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
         octo_fmm_solver_solve_rhs2(self.handle, dmass, out)
         return out
 

@@ -706,6 +706,86 @@ p2p_monopole_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params 
 }
 
 // ------------------------------------------------------------------------------------------
+// Potential-only monopole sum for the second right-hand side of the complete solve (d(phi)/dt from d(mass)/dt,
+// only the potential of that solve is used, Eq. 3), on the same tensor-core instruction.
+// With one output per target the 8 rows of a DMMA are the 8 CHILDREN of one parent cell (they share the parent,
+// hence -- Eq. 15 -- all source cells of the leaf list: 264 positions for 263 partners each), the 8 columns are 8
+// parents next to each other in x, k runs over 4 source positions s_k relative to the parent's (even, even, even)
+// child:  A[v][k] = W_phi[s_k - c_v] (0 if that offset is not in child v's list),  B[k][j] = m[t_j + s_k].
+// One DMMA = 8 parents x 8 children x 4 sources, a quarter of the instructions of the four-output kernel.
+// Block = 8 warps = a 16 x 16 x 8 target tile = 32 parent rows of 8 parents; a warp owns 4 of them.
+// ------------------------------------------------------------------------------------------
+constexpr int DMMA_MAX_CHUNKS_POT = (2 * REACH_MAX + 2) * (2 * REACH_MAX + 2) * (2 * REACH_MAX + 2) / 4;   // |U| <= 12^3
+
+__global__ void __launch_bounds__(DMMA_THREADS, 2)
+p2p_potential_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params p, const DmmaEntry* __restrict__ tab,
+                          const int nch, double* __restrict__ out)
+{
+    extern __shared__ __align__(128) unsigned char mono_smem[];
+    double* tile = reinterpret_cast<double*>(mono_smem);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(mono_smem + DMMA_TILE_BYTES);
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const int bx = (p.ox + MT_X - 1) / MT_X, by = (p.oy + MT_Y - 1) / MT_Y;
+    const int b = blockIdx.x;
+    const int x0 = p.lo[0] + (b % bx) * MT_X, y0 = p.lo[1] + ((b / bx) % by) * MT_Y, z0 = p.lo[2] + (b / (bx * by)) * DT_Z;
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_arrive_expect_tx(bar, DMMA_TILE_BYTES);
+        tma_load_tile3(tile, &tmap, bar, x0 >> 1, 2 * y0, z0);
+    }
+    __syncthreads();
+
+    // parent rows of this warp: y = y0 + 8 (warp & 1) + 2 i (i = 0..3), z = z0 + 2 (warp >> 1)
+    const int yb = 8 * (warp & 1), zb = 2 * (warp >> 1);
+    const double* base = tile + ((zb + REACH_MAX) * MS_Y + (yb + REACH_MAX)) * MS_ROW + (lane >> 2);
+    const int4* t = reinterpret_cast<const int4*>(tab + lane);
+    double acc[4][2];
+#pragma unroll
+    for (int g = 0; g < 4; ++g) acc[g][0] = acc[g][1] = 0.0;
+    int4 e = __ldg(t);
+    mbar_wait(bar, 0);
+#pragma unroll 1
+    for (int c = 0; c < nch; ++c) {
+        const int4 en = __ldg(t + (size_t)min(c + 1, nch - 1) * 32);
+        const double a = __hiloint2double(e.y, e.x);
+        const double* q = base + e.z;
+        double m[4];
+#pragma unroll
+        for (int g = 0; g < 4; ++g) m[g] = q[g * 2 * MS_ROW];
+#pragma unroll
+        for (int g = 0; g < 4; ++g) dmma_8x8x4(acc[g][0], acc[g][1], a, m[g]);
+        e = en;
+    }
+
+    // D fragment: row = lane >> 2 = child v = vx + 2 vy + 4 vz; columns 2 (lane & 3) + {0, 1} = parents.
+    // d0 -> cell x0 + 4 (lane & 3) + vx, d1 -> + 2.  One exchange with lane ^ 4 (the other vx) gives every lane two
+    // x-consecutive cells.
+    const int v = lane >> 2, vx = v & 1, vy = (v >> 1) & 1, vz = v >> 2;
+    const int gx = x0 + 4 * (lane & 3) + 2 * vx;
+    const int k = z0 + zb + vz;
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+        const double send = vx ? acc[g][0] : acc[g][1];
+        const double recv = __shfl_xor_sync(0xffffffffu, send, 4);
+        const double lo = vx ? recv : acc[g][0], hi = vx ? acc[g][1] : recv;
+        const int gy = y0 + yb + 2 * g + vy;
+        if (gy < p.hi[1] && k < p.hi[2] && gx < p.hi[0]) {
+            double* dst = out + ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+            if (gx + 1 < p.hi[0] && (reinterpret_cast<uintptr_t>(dst) & 15) == 0) {
+                *reinterpret_cast<double2*>(dst) = make_double2(lo, hi);
+            } else {
+                dst[0] = lo;
+                if (gx + 1 < p.hi[0]) dst[1] = hi;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // FP64 ALU roofline probe: 8 independent DFMA chains per thread.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double seed)

@@ -107,7 +107,7 @@ Sizes sizes_of(const octo_fmm_config& c, int flags = 0)
         s.L = align_up(ocell * 4 * sizeof(double));
         s.C = 0;
         s.W = align_up((size_t)MONO_NW * sizeof(double4));
-        s.T = align_up((size_t)4 * DMMA_MAX_CHUNKS * 32 * sizeof(DmmaEntry));
+        s.T = align_up(((size_t)4 * DMMA_MAX_CHUNKS + DMMA_MAX_CHUNKS_POT) * 32 * sizeof(DmmaEntry));
     }
     s.flags = ALIGN;
     s.total = s.src + s.L + s.C + s.W + s.T + s.flags;
@@ -131,6 +131,76 @@ EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
+// One row of the 8 x 4 A fragment of the tensor-core monopole kernels: the outputs of this row belong to the target
+// shifted by (cx, cy, cz) from the base target, whose interaction list is *list, and are component comp of the weights.
+struct DmmaRow { const std::vector<Offset3>* list; int cx, cy, cz, comp; };
+
+// Table of A fragments, one chunk = 4 source positions relative to the base target.  U = the union over the rows of
+// (list + shift), in (sz, sy, sx) order.  A[i][k] = weight comp_i of offset (s_k - shift_i) if that offset is in row i's
+// list, else 0.  The 4 positions of a chunk are chosen so that the B-fragment load (kernels.cuh) has no shared-memory
+// bank conflict: an LDS.64 is served per half-warp = 4 targets (j) x 4 positions (k) at addresses off_k + j; two
+// positions are compatible if their 4-double segments overlap in ADDRESS (|difference| <= 3: broadcast) or lie at least
+// 4 banks (of 8 bytes, 16 per 128-byte wavefront) apart.  Greedy in list order; a slot left empty repeats the chunk's
+// first position with zero weights.  Returns the number of chunks, -1 if they exceed max_chunks.
+int build_dmma_table(const DmmaRow (&rows)[8], const std::vector<double4>& wt, DmmaEntry* tb, int max_chunks)
+{
+    constexpr int NP = 2 * REACH_MAX + 2;     // positions -5 .. 6 per axis
+    auto pos = [&](int sx, int sy, int sz) { return ((size_t)(sz + REACH_MAX) * NP + (sy + REACH_MAX)) * NP + (sx + REACH_MAX); };
+    auto widx_of = [](int dx, int dy, int dz) {
+        return ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
+    };
+    std::vector<unsigned char> in((size_t)NP * NP * NP, 0);      // bit i: position is in row i's shifted list
+    for (int i = 0; i < 8; ++i)
+        for (const Offset3& o : *rows[i].list) in[pos(o.d[0] + rows[i].cx, o.d[1] + rows[i].cy, o.d[2] + rows[i].cz)] |= (unsigned char)(1u << i);
+    struct Src { int sx, sy, sz, off; unsigned char rows; };
+    std::vector<Src> U;
+    for (int sz = -REACH_MAX; sz <= REACH_MAX + 1; ++sz)
+        for (int sy = -REACH_MAX; sy <= REACH_MAX + 1; ++sy)
+            for (int sx = -REACH_MAX; sx <= REACH_MAX + 1; ++sx) {
+                const unsigned char r = in[pos(sx, sy, sz)];
+                if (!r) continue;
+                const int off = (sz * MS_Y + sy) * MS_ROW + (((sx + REACH_MAX) & 1) ? MS_XH : 0) + ((sx + REACH_MAX) >> 1);
+                U.push_back(Src{sx, sy, sz, off, r});
+            }
+    auto compatible = [](int a, int b) {
+        const int d = b - a;
+        if (d >= -3 && d <= 3) return true;
+        const int D = ((d % 16) + 16) % 16;
+        return D >= 4 && D <= 12;
+    };
+    std::vector<char> used(U.size(), 0);
+    int nchunk = 0;
+    for (size_t first = 0; first < U.size(); ++first) {
+        if (used[first]) continue;
+        if (nchunk == max_chunks) return -1;
+        size_t member[4];
+        int nm = 0;
+        member[nm++] = first; used[first] = 1;
+        for (size_t j = first + 1; j < U.size() && nm < 4; ++j) {
+            if (used[j]) continue;
+            bool ok = true;
+            for (int k = 0; k < nm; ++k) ok = ok && compatible(U[member[k]].off, U[j].off);
+            if (ok) { member[nm++] = j; used[j] = 1; }
+        }
+        for (int k = 0; k < 4; ++k) {
+            const Src* u = k < nm ? &U[member[k]] : nullptr;
+            for (int i = 0; i < 8; ++i) {
+                DmmaEntry& t = tb[(size_t)nchunk * 32 + 4 * i + k];
+                t.off = u ? u->off : U[first].off;
+                double w = 0.0;
+                if (u && ((u->rows >> i) & 1)) {
+                    const double4& q = wt[widx_of(u->sx - rows[i].cx, u->sy - rows[i].cy, u->sz - rows[i].cz)];
+                    const int c = rows[i].comp;
+                    w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w;
+                }
+                t.a = w;
+            }
+        }
+        ++nchunk;
+    }
+    return nchunk;
+}
+
 const void* g_const_owner = nullptr;   // handle whose tables are in constant memory
 unsigned long long g_list_sig = 0;     // signature (theta, kind, list flavour, device) of the lists in constant memory
 
@@ -147,6 +217,7 @@ struct octo_fmm {
     double4* W;            // monopole: device table of the weights of the 11^3 offsets
     DmmaEntry* T;          // monopole: device table of the A fragments of p2p_monopole_dmma_kernel
     DmmaLists dl;
+    int nchunk_pot;        // chunks of the potential-only table (after the four tables of dl in T)
     CUtensorMap tmap2;     // monopole: the 16 x 16 x 8 tile box of p2p_monopole_dmma_kernel
     int mono_kernel;       // 0 tensor-core instruction (default), 1 DFMA
     unsigned long long n_interactions;
@@ -362,75 +433,25 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         if (cudaFuncSetAttribute(p2p_monopole_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, MONO_SMEM) != cudaSuccess) {
             delete h; return OCTO_FMM_ECUDA;
         }
-        // ---- p2p_monopole_dmma_kernel: A fragments of the chunks of U = S_even + (S_odd + e_x), per (py, pz) ----
+        // ---- tensor-core kernels: tables of A fragments (build_dmma_table) ----
         {
-            std::vector<DmmaEntry> tab((size_t)4 * DMMA_MAX_CHUNKS * 32, DmmaEntry{0.0, 0, 0});
-            auto widx_of = [](int dx, int dy, int dz) {
-                return ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
-            };
+            std::vector<DmmaEntry> tab((size_t)4 * DMMA_MAX_CHUNKS * 32 + (size_t)DMMA_MAX_CHUNKS_POT * 32, DmmaEntry{0.0, 0, 0});
+            // p2p_monopole_dmma_kernel, per (py, pz): rows 0-3 = (phi, g) of the x-even target, rows 4-7 of its x-odd sibling
             for (int cp = 0; cp < 4; ++cp) {
-                const std::vector<Offset3>& Se = h->list[2 * (cp & 1) + 4 * (cp >> 1)];
-                const std::vector<Offset3>& So = h->list[1 + 2 * (cp & 1) + 4 * (cp >> 1)];
-                // membership of a source position (relative to the even target) in the two lists
-                constexpr int NX = 2 * REACH_MAX + 2, NY = 2 * REACH_MAX + 1;
-                std::vector<unsigned char> in_e((size_t)NX * NY * NY, 0), in_o((size_t)NX * NY * NY, 0);
-                auto pos = [&](int sx, int sy, int sz) { return ((size_t)(sz + REACH_MAX) * NY + (sy + REACH_MAX)) * NX + (sx + REACH_MAX); };
-                for (const Offset3& o : Se) in_e[pos(o.d[0], o.d[1], o.d[2])] = 1;
-                for (const Offset3& o : So) in_o[pos(o.d[0] + 1, o.d[1], o.d[2])] = 1;
-                // the offsets of U in (sz, sy, sx) order
-                struct Src { int sx, sy, sz, off; bool e, o; };
-                std::vector<Src> U;
-                for (int sz = -REACH_MAX; sz <= REACH_MAX; ++sz)
-                    for (int sy = -REACH_MAX; sy <= REACH_MAX; ++sy)
-                        for (int sx = -REACH_MAX; sx <= REACH_MAX + 1; ++sx) {
-                            const bool e = in_e[pos(sx, sy, sz)], o = in_o[pos(sx, sy, sz)];
-                            if (!e && !o) continue;
-                            const int off = (sz * MS_Y + sy) * MS_ROW + (((sx + REACH_MAX) & 1) ? MS_XH : 0) + ((sx + REACH_MAX) >> 1);
-                            U.push_back(Src{sx, sy, sz, off, e, o});
-                        }
-                // Chunks of 4 offsets whose B-fragment load has no shared-memory bank conflict.  An LDS.64 is served
-                // per half-warp = 4 targets (j) x 4 offsets (k), addresses off_k + j: two offsets are compatible if
-                // their 4-double segments overlap in ADDRESS (|difference| <= 3: broadcast) or are at least 4 banks
-                // (of 8 bytes, 16 per 128-byte wavefront) apart.  Greedy in list order; the few slots left empty
-                // repeat the chunk's first offset with zero weights.
-                auto compatible = [](int a, int b) {
-                    const int d = b - a;
-                    if (d >= -3 && d <= 3) return true;
-                    const int D = ((d % 16) + 16) % 16;
-                    return D >= 4 && D <= 12;
-                };
-                std::vector<char> used(U.size(), 0);
-                DmmaEntry* tb = tab.data() + (size_t)cp * DMMA_MAX_CHUNKS * 32;
-                int nchunk = 0;
-                bool overflow = false;
-                for (size_t first = 0; first < U.size(); ++first) {
-                    if (used[first]) continue;
-                    if (nchunk == DMMA_MAX_CHUNKS) { overflow = true; break; }
-                    size_t member[4];
-                    int nm = 0;
-                    member[nm++] = first; used[first] = 1;
-                    for (size_t j = first + 1; j < U.size() && nm < 4; ++j) {
-                        if (used[j]) continue;
-                        bool ok = true;
-                        for (int k = 0; k < nm; ++k) ok = ok && compatible(U[member[k]].off, U[j].off);
-                        if (ok) { member[nm++] = j; used[j] = 1; }
-                    }
-                    for (int k = 0; k < 4; ++k) {
-                        const Src* u = k < nm ? &U[member[k]] : nullptr;
-                        for (int i = 0; i < 8; ++i) {
-                            DmmaEntry& t = tb[(size_t)nchunk * 32 + 4 * i + k];
-                            t.off = u ? u->off : U[first].off;
-                            const int c = i & 3;
-                            double w = 0.0;
-                            if (u && i < 4 && u->e) { const double4& q = wt[widx_of(u->sx, u->sy, u->sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
-                            if (u && i >= 4 && u->o) { const double4& q = wt[widx_of(u->sx - 1, u->sy, u->sz)]; w = c == 0 ? q.x : c == 1 ? q.y : c == 2 ? q.z : q.w; }
-                            t.a = w;
-                        }
-                    }
-                    ++nchunk;
-                }
-                if (overflow) { delete h; return OCTO_FMM_EINVAL; }
-                h->dl.nchunk[cp] = nchunk;
+                DmmaRow rows[8];
+                for (int i = 0; i < 8; ++i)
+                    rows[i] = DmmaRow{&h->list[(i >> 2) + 2 * (cp & 1) + 4 * (cp >> 1)], i >> 2, 0, 0, i & 3};
+                const int n = build_dmma_table(rows, wt, tab.data() + (size_t)cp * DMMA_MAX_CHUNKS * 32, DMMA_MAX_CHUNKS);
+                if (n < 0) { delete h; return OCTO_FMM_EINVAL; }
+                h->dl.nchunk[cp] = n;
+            }
+            // p2p_potential_dmma_kernel: row v = the potential of child v = vx + 2 vy + 4 vz of one parent
+            {
+                DmmaRow rows[8];
+                for (int v = 0; v < 8; ++v) rows[v] = DmmaRow{&h->list[v], v & 1, (v >> 1) & 1, v >> 2, 0};
+                const int n = build_dmma_table(rows, wt, tab.data() + (size_t)4 * DMMA_MAX_CHUNKS * 32, DMMA_MAX_CHUNKS_POT);
+                if (n < 0) { delete h; return OCTO_FMM_EINVAL; }
+                h->nchunk_pot = n;
             }
             if (cudaMemcpyAsync(h->T, tab.data(), tab.size() * sizeof(DmmaEntry), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
                 cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
@@ -440,7 +461,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
                 delete h; return OCTO_FMM_ECUDA;
             }
-            if (cudaFuncSetAttribute(p2p_monopole_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess) {
+            if (cudaFuncSetAttribute(p2p_monopole_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess ||
+                cudaFuncSetAttribute(p2p_potential_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess) {
                 delete h; return OCTO_FMM_ECUDA;
             }
         }
@@ -540,6 +562,18 @@ int octo_fmm_interact(octo_fmm_t* h)
     h->state = 2;
     h->resL = h->outL; h->resC = h->outC;
     return OCTO_FMM_OK;
+}
+
+// Monopole handles: the potential row only, out = [oz][oy][ox] (second right-hand side of the complete solve).
+static int interact_potential(octo_fmm_t* h, double* out)
+{
+    if (!h || !out || h->cfg.kind != OCTO_FMM_MONOPOLE) return OCTO_FMM_EINVAL;
+    if (h->state < 1) return OCTO_FMM_ESTATE;
+    if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    const Params& P = h->prm;
+    p2p_potential_dmma_kernel<<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(
+        h->tmap2, P, h->T + (size_t)4 * DMMA_MAX_CHUNKS * 32, h->nchunk_pot, out);
+    return cudaGetLastError() == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
 
 int octo_fmm_bind_outputs(octo_fmm_t* h, double* L, double* Lcorr)

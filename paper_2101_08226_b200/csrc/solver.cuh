@@ -211,8 +211,9 @@ __global__ void __launch_bounds__(128) l2l_kernel(double* __restrict__ cL, doubl
 // evaluated at the leaf's cell centre:  phi += L0(e),  g -= L1(e) + correction,  e = ((a,b,c) - 1/2) h - delta_P.
 // One thread per PARENT (grid = (ceil(pnx / blockDim.x), pny, pnz)): the parent's 26 numbers are read once
 // and its 8 leaves are updated as four double2 (x-pairs), so every access of a warp is contiguous.
-// out must be 16-byte aligned.
+// out must be 16-byte aligned.  PHI_ONLY (second right-hand side): out = [nz][ny][nx], only the potential row.
 // ------------------------------------------------------------------------------------------
+template <bool PHI_ONLY = false>
 __global__ void __launch_bounds__(128) leaf_eval_kernel(double* __restrict__ out, const double* __restrict__ pL,
                                                         const double* __restrict__ pC, const double* __restrict__ poff, int nx,
                                                         int ny, int nz, double h)
@@ -241,12 +242,14 @@ __global__ void __launch_bounds__(128) leaf_eval_kernel(double* __restrict__ out
             double2 v = *o;
             v.x += sh0[0]; v.y += sh1[0];
             *o = v;
+            if constexpr (!PHI_ONLY) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                double2* g = reinterpret_cast<double2*>(out + (1 + c) * ncell + row);
-                double2 w = *g;
-                w.x -= sh0[1 + c] + C[c]; w.y -= sh1[1 + c] + C[c];
-                *g = w;
+                for (int c = 0; c < 3; ++c) {
+                    double2* g = reinterpret_cast<double2*>(out + (1 + c) * ncell + row);
+                    double2 w = *g;
+                    w.x -= sh0[1 + c] + C[c]; w.y -= sh1[1 + c] + C[c];
+                    *g = w;
+                }
             }
         }
 }

@@ -164,7 +164,7 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
     {
         const int n = s->cfg.n;
         SolverLevel& p = s->lev[0];
-        leaf_eval_kernel<<<dim3((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2)), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
+        leaf_eval_kernel<false><<<dim3((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2)), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     s->have_centres = true;
@@ -205,15 +205,12 @@ int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t* s, const double* dmass, double
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
         }
     }
-    double* const keep = s->leaf->outL;
-    s->leaf->outL = out;
-    rc = octo_fmm_interact(s->leaf);
-    s->leaf->outL = keep;
-    if (rc != OCTO_FMM_OK) return rc;
+    // leaves: only the potential of this solve is used (Eq. 3): potential-only leaf sum and evaluation
+    if ((rc = interact_potential(s->leaf, out)) != OCTO_FMM_OK) return rc;
     {
         const int n = s->cfg.n;
         SolverLevel& p = s->lev[0];
-        leaf_eval_kernel<<<dim3((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2)), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
+        leaf_eval_kernel<true><<<dim3((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2)), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     return OCTO_FMM_OK;

@@ -136,7 +136,8 @@ def test_solve_host_entry_point(env):
 @pytest.mark.parametrize("theta", [0.5, 0.35])
 def test_second_right_hand_side_32(env, theta):
     """f2 (L81-83): d(phi)/dt from d(mass)/dt on the tree and the expansion centres of the density's solve, no
-    correction, against the oracle's solve_rhs2; signed sources with zero net change."""
+    correction, against the oracle's solve_rhs2; signed sources with zero net change.  The leaf sum of this pass is
+    the potential-only tensor-core kernel (rows = the 8 children of a parent)."""
     p, torch = env
     n, h = 32, 1.0 / 32
     rng = np.random.default_rng(12)
@@ -150,9 +151,9 @@ def test_second_right_hand_side_32(env, theta):
     out2 = s.solve_rhs2(torch.from_numpy(dm).cuda())
     torch.cuda.synchronize()
     assert s.status() == p.OK
-    ref2 = oracle.solve_rhs2(n, h, theta, mass, dm)
-    e_phi, e_g = _errors(out2.cpu().numpy(), ref2)
-    assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+    ref2 = oracle.solve_rhs2(n, h, theta, mass, dm)[0]
+    e_phi = np.abs(out2.cpu().numpy() - ref2).max() / np.abs(ref2).max()
+    assert e_phi < TOL, e_phi
     # the density's solve is unchanged by the second right-hand side having run on the same handles
     again = s.solve(torch.from_numpy(mass).cuda())
     torch.cuda.synchronize()
