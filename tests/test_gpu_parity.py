@@ -352,6 +352,37 @@ def test_zero_mass_sources_are_harmless(env):
     check(L, Lc, Lr, Lcr)
 
 
+@pytest.mark.parametrize("kernel", [0, 1, 2])
+def test_mixed_monopole_and_multipole_cells(env, kernel):
+    """Mixed pairs (the same-level part): a level on which whole 8^3 sub-grids are leaves -- point
+    masses at the cell centres, i.e. zero offset and zero moments above M0 -- next to refined sub-grids that carry full
+    multipoles.  Multipole <-> monopole pairs in both directions are the general pair formula with those zeros; targets
+    and sources of both kinds against the oracle, correction on."""
+    p, torch = env
+    w = fi.config1(seed=21, ncell=32)
+    sub = np.random.default_rng(4).random((4, 4, 4)) < 0.5               # which sub-grids are leaves
+    leaf = np.repeat(np.repeat(np.repeat(sub, 8, 0), 8, 1), 8, 2)
+    assert 0.2 < leaf.mean() < 0.8
+    w.moments[1:, leaf] = 0.0
+    w.com_off[:, leaf] = 0.0
+    L, Lc, cnt, _ = gpu_multipole(env, w, kernel=kernel, out_lo=(0, 0, 0), out_hi=(32, 32, 32))
+    Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, w.theta, w.moments, w.com_off, (0, 0, 0), (32, 32, 32), True)
+    assert cnt == cntr
+    check(L, Lc, Lr, Lcr)
+    # a leaf target among leaf sources only sees masses at lattice points: the monopole kernel gives its (phi, g)
+    f = p.OctoFMM(w.n, w.h, 0.5, p.MONOPOLE)
+    out, _ = f.solve(torch.from_numpy(np.ascontiguousarray(w.moments[:1])).cuda())
+    torch.cuda.synchronize()
+    f.close()
+    all_leaf = fi.config1(seed=21, ncell=32)
+    all_leaf.moments[1:] = 0.0
+    all_leaf.com_off[:] = 0.0
+    L2, _, _, _ = gpu_multipole(env, all_leaf, kernel=kernel, correction=False, out_lo=(0, 0, 0), out_hi=(32, 32, 32))
+    out = out.cpu().numpy()
+    assert np.abs(L2[0] - out[0]).max() / np.abs(out[0]).max() < 1e-13
+    assert np.abs(L2[1:4] + out[1:4]).max() / np.abs(out[1:4]).max() < 1e-13      # g = -L1
+
+
 def test_monopole_non_cubic_grid_and_sub_region(env):
     """Monopole kernel on a 24 x 16 x 8 grid (tiles ragged in x, whole-domain faces) and on an interior region."""
     p, torch = env
