@@ -278,7 +278,7 @@ def run_solve(args):
         m //= 2
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     peak = sm_count * FP64_LANES_PER_SM * 2 * 1965.0e6 / 1e12
-    leaf_int = n_int - sum(oracle.interaction_count((n >> k,) * 3, args.theta) for k in range(1, n.bit_length()) if (n >> k) >= 2)
+    leaf_int = s.leaf_interaction_count()
     f_multi = p.octo_fmm_flops_per_interaction_path(p.MULTIPOLE, True, False)[0]   # the solver's levels have no dipoles
     flops = float(f_multi) * (n_int - leaf_int) + 8.0 * leaf_int
     line = {"metric": METRIC, "value": n_int / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,

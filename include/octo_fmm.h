@@ -215,6 +215,8 @@ int octo_fmm_solver_status(octo_fmm_solver_t *s);
 int octo_fmm_solver_destroy(octo_fmm_solver_t *s);
 /* Ordered in-domain pairs one solve evaluates, all levels. */
 int octo_fmm_solver_interaction_count(const octo_fmm_solver_t *s, unsigned long long *n);
+/* ... of which at the leaf level (monopole pairs, 8 flop each; the rest are multipole pairs). */
+int octo_fmm_solver_leaf_interaction_count(const octo_fmm_solver_t *s, unsigned long long *n);
 /* The leaf-level list (Eq. 15 list + near field) of a parity class, as octo_fmm_get_stencil. */
 int octo_fmm_solver_get_leaf_stencil(const octo_fmm_solver_t *s, int parity, int *count, signed char (*dxyz)[3]);
 /* Number of multipole levels (n/2 ... 2) and of kernels one solve launches. */

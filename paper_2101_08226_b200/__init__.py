@@ -89,6 +89,7 @@ class _Library:
         lib.octo_fmm_solver_solve_host.argtypes = [vp, vp, vp, vp, ctypes.c_size_t]
         lib.octo_fmm_solver_destroy.argtypes = [vp]
         lib.octo_fmm_solver_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
+        lib.octo_fmm_solver_leaf_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_solver_get_leaf_stencil.argtypes = [vp, ctypes.c_int, ip, vp]
         lib.octo_fmm_solver_num_levels.argtypes = [vp, ip, ip]
         self._cdll = lib
@@ -321,6 +322,14 @@ def octo_fmm_solver_interaction_count(s):
     return int(n.value)
 
 
+def octo_fmm_solver_leaf_interaction_count(s):
+    n = ctypes.c_ulonglong(0)
+    rc = _lib.octo_fmm_solver_leaf_interaction_count(s, ctypes.byref(n))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_leaf_interaction_count", rc)
+    return int(n.value)
+
+
 def octo_fmm_solver_get_leaf_stencil(s, parity):
     import numpy as np
     cnt = ctypes.c_int(0)
@@ -380,6 +389,9 @@ class OctoFMMSolver:
 
     def interaction_count(self):
         return octo_fmm_solver_interaction_count(self.handle)
+
+    def leaf_interaction_count(self):
+        return octo_fmm_solver_leaf_interaction_count(self.handle)
 
     def leaf_stencil(self, parity):
         return octo_fmm_solver_get_leaf_stencil(self.handle, parity)

@@ -257,6 +257,13 @@ int octo_fmm_solver_interaction_count(const octo_fmm_solver_t* s, unsigned long 
     return OCTO_FMM_OK;
 }
 
+int octo_fmm_solver_leaf_interaction_count(const octo_fmm_solver_t* s, unsigned long long* n)
+{
+    if (!s || !n) return OCTO_FMM_EINVAL;
+    *n = s->leaf->n_interactions;
+    return OCTO_FMM_OK;
+}
+
 int octo_fmm_solver_get_leaf_stencil(const octo_fmm_solver_t* s, int parity, int* count, signed char (*dxyz)[3])
 {
     if (!s) return OCTO_FMM_EINVAL;
