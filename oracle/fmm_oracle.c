@@ -47,7 +47,11 @@
  * (L137), worked example W1, symbolic derivatives of -1/r (sympy), order-of-convergence
  * against direct summation over point masses, Newton's third law (L125), angular-momentum
  * conservation with the correction on and its violation with it off (L127), point-mass
- * and uniform-sphere closed forms.  No function here is "parity unpinned".
+ * and uniform-sphere closed forms; for the passes of the complete solve (M2M, M2M about prescribed
+ * centres, L2L, leaf list, direct sum; tests/test_oracle_solve.py): P2M of all constituents, the symbolic
+ * Taylor shift, the exact point sum, conservation, the uniform-sphere residuals of Table 1, and for the
+ * second right-hand side (L81-83) proportionality to the density's solve and linearity.
+ * No function here is "parity unpinned".
  *
  * Layouts: moments [20][nz][ny][nx] (monopole: [1][nz][ny][nx]), com_off [3][nz][ny][nx],
  * outputs SoA over the output region: L [20][oz][oy][ox], Lcorr [3][oz][oy][ox],
