@@ -681,8 +681,23 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
             cudaEventCreateWithFlags(&h->ev_end, cudaEventDisableTiming) != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     int zc = h->host_chunk;
-    while ((P.oz + zc - 1) / zc > MAX_CHUNKS) zc += TILE_Z;
-    const int nchunk = (P.oz + zc - 1) / zc;
+    while ((P.oz + zc - 1) / zc + 4 > MAX_CHUNKS) zc += TILE_Z;
+    // Slab boundaries.  The bus is the bottleneck, so what the pipeline adds to the pure copy time is its fill (the
+    // input of the first slab + halo before the first launch) and its drain (the last launch and its copy out): the
+    // first and the last two slabs are short (3 and 6 layers), the others zc.
+    int bound[MAX_CHUNKS + 1];
+    int nchunk = 0;
+    {
+        int z = P.lo[2];
+        bound[0] = z;
+        const bool ramp = P.oz >= 4 * zc && zc > 2 * TILE_Z;
+        auto push = [&](int len) { z = std::min(z + len, P.hi[2]); bound[++nchunk] = z; };
+        if (ramp) { push(TILE_Z); push(2 * TILE_Z); }
+        const int tail = ramp ? 3 * TILE_Z : 0;
+        while (P.hi[2] - z > tail + zc) push(zc);
+        if (P.hi[2] - z > tail) push(P.hi[2] - z - tail);
+        if (ramp) { push(2 * TILE_Z); push(TILE_Z); }
+    }
     const size_t plane = (size_t)P.nx * P.ny, ncell = plane * P.nz;
     const size_t oplane = (size_t)P.ox * P.oy, ocell = oplane * P.oz;
     cudaStream_t sm = h->stream;
@@ -697,7 +712,7 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
     int brought = std::max(P.lo[2] - h->reach, 0);         // source layers [.., brought) are on the device
     int rc = OCTO_FMM_OK;
     for (int c = 0; c < nchunk && rc == OCTO_FMM_OK; ++c) {
-        const int a = P.lo[2] + c * zc, b = std::min(a + zc, P.hi[2]);
+        const int a = bound[c], b = bound[c + 1];
         const int need = std::min(b + h->reach, P.nz);
         if (need > brought) {
             const size_t off = (size_t)brought * plane, width = (size_t)(need - brought) * plane * 8;
