@@ -101,6 +101,16 @@ int octo_fmm_destroy(octo_fmm_t *h);
  * *count receives the list length; dxyz (may be NULL) must hold that many (dx,dy,dz) triples. */
 int octo_fmm_get_stencil(const octo_fmm_t *h, int parity, int *count, signed char (*dxyz)[3]);
 
+/* Host-only view (no device, no handle) of the operand tables of the tensor-core monopole kernels, for tests: the
+ * table for opening angle theta, cell width h, list flavour leaf (0 = the list of Eq. 15, 1 = + the near field of
+ * the complete solve) and which = 0..3 (the (y, z)-parity pair py + 2 pz of the four-output kernel: rows 0-3 =
+ * (phi, gx, gy, gz) of the x-even target, rows 4-7 of its x-odd sibling) or 4 (potential-only kernel: row v = child
+ * vx + 2 vy + 4 vz of one parent).  *nchunk chunks of 4 source positions; for chunk c, row i, slot k:
+ * a[32 c + 4 i + k] = the weight (0 where the position is not in row i's list), off[32 c + 4 i + k] = the position's
+ * offset in the mass tile, (sz * 26 + sy) * 28 + ((sx + 5) & 1) * 14 + ((sx + 5) >> 1) doubles, position (sx, sy, sz)
+ * relative to the base target.  a, off: host, cap_chunks * 32 elements (NULL: only *nchunk). */
+int octo_fmm_dmma_table(double theta, double h, int leaf, int which, int cap_chunks, int *nchunk, double *a, int *off);
+
 /* Number of ordered in-domain (A,B) pairs one interact() evaluates (out-of-grid partners are
  * skipped: isolated boundary, L321). */
 int octo_fmm_interaction_count(const octo_fmm_t *h, unsigned long long *n);

@@ -66,6 +66,7 @@ class _Library:
         lib.octo_fmm_destroy.argtypes = [vp]
         lib.octo_fmm_bind_outputs.argtypes = [vp, vp, vp]
         lib.octo_fmm_get_stencil.argtypes = [vp, ctypes.c_int, ip, vp]
+        lib.octo_fmm_dmma_table.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, vp, vp]
         lib.octo_fmm_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_status.argtypes = [vp]
         lib.octo_fmm_run_host.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_size_t]
@@ -189,6 +190,22 @@ def octo_fmm_get_stencil(h, parity):
     if rc != OK:
         raise OctoFmmError("octo_fmm_get_stencil", rc)
     return out
+
+
+def octo_fmm_dmma_table(theta, h, leaf, which):
+    """Host-only: (a[nchunk][8][4], off[nchunk][8][4]) of the operand table of the tensor-core monopole kernels."""
+    import numpy as np
+    n = ctypes.c_int(0)
+    rc = _lib.octo_fmm_dmma_table(float(theta), float(h), int(leaf), int(which), 0, ctypes.byref(n), None, None)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_dmma_table", rc)
+    a = np.zeros((n.value, 8, 4))
+    off = np.zeros((n.value, 8, 4), dtype=np.int32)
+    rc = _lib.octo_fmm_dmma_table(float(theta), float(h), int(leaf), int(which), n.value, ctypes.byref(n), a.ctypes.data,
+                                  off.ctypes.data)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_dmma_table", rc)
+    return a, off
 
 
 def octo_fmm_interaction_count(h):

@@ -201,6 +201,34 @@ int build_dmma_table(const DmmaRow (&rows)[8], const std::vector<double4>& wt, D
     return nchunk;
 }
 
+// Monopole weights of the 11^3 offsets: (-1/|R|, -R/|R|^3) with R = (i_A - i_B) h = -Delta h (hmul[d + 5] = -d h), in
+// FP64 on the host (sqrt, division); Delta = 0 gets zero weights.
+std::vector<double4> monopole_weights(const double (&hmul)[2 * REACH_MAX + 1])
+{
+    std::vector<double4> wt((size_t)MONO_NW, double4{0.0, 0.0, 0.0, 0.0});
+    for (int dz = -REACH_MAX; dz <= REACH_MAX; ++dz)
+        for (int dy = -REACH_MAX; dy <= REACH_MAX; ++dy)
+            for (int dx = -REACH_MAX; dx <= REACH_MAX; ++dx) {
+                if (!dx && !dy && !dz) continue;
+                const double Rx = hmul[dx + REACH_MAX], Ry = hmul[dy + REACH_MAX], Rz = hmul[dz + REACH_MAX];
+                const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = std::sqrt(r2), ir3 = -1.0 / (r2 * r);
+                const int widx = ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
+                wt[widx] = double4{-1.0 / r, Rx * ir3, Ry * ir3, Rz * ir3};
+            }
+    return wt;
+}
+
+// The rows of the two tensor-core tables: which = 0..3 -> p2p_monopole_dmma_kernel for (py, pz) = (which & 1, which >> 1):
+// rows 0-3 = (phi, g) of the x-even target, rows 4-7 of its x-odd sibling; which = 4 -> p2p_potential_dmma_kernel: row v =
+// the potential of child v = vx + 2 vy + 4 vz of one parent.
+void dmma_rows(const std::vector<Offset3> (&list)[8], int which, DmmaRow (&rows)[8])
+{
+    for (int i = 0; i < 8; ++i) {
+        if (which < 4) rows[i] = DmmaRow{&list[(i >> 2) + 2 * (which & 1) + 4 * (which >> 1)], i >> 2, 0, 0, i & 3};
+        else           rows[i] = DmmaRow{&list[i], i & 1, (i >> 1) & 1, i >> 2, 0};
+    }
+}
+
 const void* g_const_owner = nullptr;   // handle whose tables are in constant memory
 unsigned long long g_list_sig = 0;     // signature (theta, kind, list flavour, device) of the lists in constant memory
 
@@ -404,16 +432,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     } else if (cfg->kind == OCTO_FMM_MONOPOLE) {
         // ---- monopole weights of the 11^3 offsets: (-1/|R|, -R/|R|^3) with R = (i_A - i_B) h = -Delta h, in FP64
         //      on the host (sqrt, division); Delta = 0 gets zero weights ----
-        std::vector<double4> wt((size_t)MONO_NW, double4{0.0, 0.0, 0.0, 0.0});
-        for (int dz = -REACH_MAX; dz <= REACH_MAX; ++dz)
-            for (int dy = -REACH_MAX; dy <= REACH_MAX; ++dy)
-                for (int dx = -REACH_MAX; dx <= REACH_MAX; ++dx) {
-                    if (!dx && !dy && !dz) continue;
-                    const double Rx = h->hmul[dx + REACH_MAX], Ry = h->hmul[dy + REACH_MAX], Rz = h->hmul[dz + REACH_MAX];
-                    const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = std::sqrt(r2), ir3 = -1.0 / (r2 * r);
-                    const int widx = ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
-                    wt[widx] = double4{-1.0 / r, Rx * ir3, Ry * ir3, Rz * ir3};
-                }
+        const std::vector<double4> wt = monopole_weights(h->hmul);
         if (cudaMemcpyAsync(h->W, wt.data(), wt.size() * sizeof(double4), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
             cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
         // ---- TMA descriptor of the staged masses P[z][y * 2 + xpar][xh] (see stage_monopole_kernel) ----
@@ -436,22 +455,13 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         // ---- tensor-core kernels: tables of A fragments (build_dmma_table) ----
         {
             std::vector<DmmaEntry> tab((size_t)4 * DMMA_MAX_CHUNKS * 32 + (size_t)DMMA_MAX_CHUNKS_POT * 32, DmmaEntry{0.0, 0, 0});
-            // p2p_monopole_dmma_kernel, per (py, pz): rows 0-3 = (phi, g) of the x-even target, rows 4-7 of its x-odd sibling
-            for (int cp = 0; cp < 4; ++cp) {
+            for (int which = 0; which < 5; ++which) {
                 DmmaRow rows[8];
-                for (int i = 0; i < 8; ++i)
-                    rows[i] = DmmaRow{&h->list[(i >> 2) + 2 * (cp & 1) + 4 * (cp >> 1)], i >> 2, 0, 0, i & 3};
-                const int n = build_dmma_table(rows, wt, tab.data() + (size_t)cp * DMMA_MAX_CHUNKS * 32, DMMA_MAX_CHUNKS);
+                dmma_rows(h->list, which, rows);
+                const int n = build_dmma_table(rows, wt, tab.data() + (size_t)which * DMMA_MAX_CHUNKS * 32,
+                                               which < 4 ? DMMA_MAX_CHUNKS : DMMA_MAX_CHUNKS_POT);
                 if (n < 0) { delete h; return OCTO_FMM_EINVAL; }
-                h->dl.nchunk[cp] = n;
-            }
-            // p2p_potential_dmma_kernel: row v = the potential of child v = vx + 2 vy + 4 vz of one parent
-            {
-                DmmaRow rows[8];
-                for (int v = 0; v < 8; ++v) rows[v] = DmmaRow{&h->list[v], v & 1, (v >> 1) & 1, v >> 2, 0};
-                const int n = build_dmma_table(rows, wt, tab.data() + (size_t)4 * DMMA_MAX_CHUNKS * 32, DMMA_MAX_CHUNKS_POT);
-                if (n < 0) { delete h; return OCTO_FMM_EINVAL; }
-                h->nchunk_pot = n;
+                if (which < 4) h->dl.nchunk[which] = n; else h->nchunk_pot = n;
             }
             if (cudaMemcpyAsync(h->T, tab.data(), tab.size() * sizeof(DmmaEntry), cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
                 cudaStreamSynchronize(h->stream) != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
@@ -651,6 +661,30 @@ int octo_fmm_get_stencil(const octo_fmm_t* h, int parity, int* count, signed cha
     if (dxyz)
         for (size_t s = 0; s < h->list[parity].size(); ++s)
             for (int a = 0; a < 3; ++a) dxyz[s][a] = h->list[parity][s].d[a];
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_dmma_table(double theta, double h, int leaf, int which, int cap_chunks, int* nchunk, double* a, int* off)
+{
+    if (!(theta > 1.0 / 3.0 && theta < 1.0) || !(h > 0.0) || which < 0 || which > 4 || !nchunk || cap_chunks < 0) return OCTO_FMM_EINVAL;
+    std::vector<Offset3> list[8];
+    int reach = 0;
+    for (int p = 0; p < 8; ++p) list[p] = build_list(p & 1, (p >> 1) & 1, (p >> 2) & 1, theta, &reach, leaf != 0);
+    if (reach > REACH_MAX) return OCTO_FMM_EINVAL;
+    double hmul[2 * REACH_MAX + 1];
+    for (int d = -REACH_MAX; d <= REACH_MAX; ++d) hmul[d + REACH_MAX] = (double)(-d) * h;
+    const std::vector<double4> wt = monopole_weights(hmul);
+    DmmaRow rows[8];
+    dmma_rows(list, which, rows);
+    const int maxc = which < 4 ? DMMA_MAX_CHUNKS : DMMA_MAX_CHUNKS_POT;
+    std::vector<DmmaEntry> tab((size_t)maxc * 32, DmmaEntry{0.0, 0, 0});
+    const int n = build_dmma_table(rows, wt, tab.data(), maxc);
+    if (n < 0) return OCTO_FMM_EINVAL;
+    *nchunk = n;
+    if (a && off) {
+        if (cap_chunks < n) return OCTO_FMM_EINVAL;
+        for (size_t i = 0; i < (size_t)n * 32; ++i) { a[i] = tab[i].a; off[i] = tab[i].off; }
+    }
     return OCTO_FMM_OK;
 }
 
