@@ -746,19 +746,29 @@ p2p_potential_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params
     double acc[4][2];
 #pragma unroll
     for (int g = 0; g < 4; ++g) acc[g][0] = acc[g][1] = 0.0;
-    int4 e = __ldg(t);
+    // the A fragments come from global memory (L1 / L2): with 4 contractions per chunk a warp has only ~64 cycles of
+    // work per fragment, so the loads run POT_PREFETCH chunks ahead in a register ring
+    constexpr int POT_PREFETCH = 8;
+    int4 e[POT_PREFETCH];
+#pragma unroll
+    for (int u = 0; u < POT_PREFETCH; ++u) e[u] = __ldg(t + (size_t)min(u, nch - 1) * 32);
     mbar_wait(bar, 0);
 #pragma unroll 1
-    for (int c = 0; c < nch; ++c) {
-        const int4 en = __ldg(t + (size_t)min(c + 1, nch - 1) * 32);
-        const double a = __hiloint2double(e.y, e.x);
-        const double* q = base + e.z;
-        double m[4];
+    for (int c = 0; c < nch; c += POT_PREFETCH) {
 #pragma unroll
-        for (int g = 0; g < 4; ++g) m[g] = q[g * 2 * MS_ROW];
+        for (int u = 0; u < POT_PREFETCH; ++u) {
+            if (c + u < nch) {                                  // warp-uniform
+                const int4 cur = e[u];
+                e[u] = __ldg(t + (size_t)min(c + u + POT_PREFETCH, nch - 1) * 32);
+                const double a = __hiloint2double(cur.y, cur.x);
+                const double* q = base + cur.z;
+                double m[4];
 #pragma unroll
-        for (int g = 0; g < 4; ++g) dmma_8x8x4(acc[g][0], acc[g][1], a, m[g]);
-        e = en;
+                for (int g = 0; g < 4; ++g) m[g] = q[g * 2 * MS_ROW];
+#pragma unroll
+                for (int g = 0; g < 4; ++g) dmma_8x8x4(acc[g][0], acc[g][1], a, m[g]);
+            }
+        }
     }
 
     // D fragment: row = lane >> 2 = child v = vx + 2 vy + 4 vz; columns 2 (lane & 3) + {0, 1} = parents.
