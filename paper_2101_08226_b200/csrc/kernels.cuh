@@ -23,6 +23,7 @@
 #include <stdint.h>
 
 #include "m2l_math.cuh"
+#include "taylor.cuh"
 
 namespace octo {
 
@@ -70,6 +71,11 @@ struct Params {
     int* flags;              // flags[0] bit 0: target mass <= 0 with correction; flags[1] bit 1: some source cell has a
                              // dipole moment (raised by the staging kernel, cleared by set_moments)
     int force_dipole;        // 1: evaluate the dipole terms whatever bit 1 says
+    // fused L2L epilogue of the complete solve (m2l_staged_kernel<CORR, true>): the parent level's finished expansions
+    const double* pL;        // [20][nz/2][ny/2][nx/2]
+    const double* pC;        // [3][...]   corrections carried beside the expansions
+    const double* poff;      // [3][...]   expansion-centre offsets of the parent cells
+    double hc;               // width of this level's cells
 };
 
 // ------------------------------------------------------------------------------------------
@@ -218,13 +224,37 @@ __device__ __forceinline__ void load_target(const Params& p, int gx, int gy, int
     }
 }
 
-template <bool CORR>
-__device__ __forceinline__ void store_target(const Params& p, const Acc& acc, const double (&tA)[7], int gx, int gy, int k)
+// FUSE_L2L (complete solve, whole-grid output): what l2l_kernel would do in a second pass over the level is done
+// here -- the correction is NOT folded into L1 but carried beside it, and the parent's expansion, Taylor-shifted to
+// this cell's expansion centre, and the parent's correction are added before the one store.
+template <bool CORR, bool FUSE_L2L = false>
+__device__ __forceinline__ void store_target(const Params& p, const Acc& acc, const double (&tA)[7], const double (&dA)[3],
+                                             int gx, int gy, int k)
 {
     double L[20], C[3];
     acc_finish<CORR>(acc, tA, L, C);
     const long long ocell = (long long)p.ox * p.oy * p.oz;
     const long long o = ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+    if constexpr (FUSE_L2L) {
+        const int pnx = p.nx >> 1, pny = p.ny >> 1;
+        const long long pcell = (long long)pnx * pny * (p.nz >> 1);
+        const long long P = ((long long)(k >> 1) * pny + (gy >> 1)) * pnx + (gx >> 1);
+        double pL[20], sh[20], e[3];
+        e[0] = ((double)(gx & 1) - 0.5) * p.hc + dA[0] - p.poff[P];
+        e[1] = ((double)(gy & 1) - 0.5) * p.hc + dA[1] - p.poff[pcell + P];
+        e[2] = ((double)(k & 1) - 0.5) * p.hc + dA[2] - p.poff[2 * pcell + P];
+#pragma unroll
+        for (int t = 0; t < 20; ++t) pL[t] = p.pL[t * pcell + P];
+        taylor_shift<3>(pL, e, sh);
+#pragma unroll
+        for (int t = 0; t < 20; ++t) {
+            double v = L[t];
+            if (t >= 1 && t <= 3) v -= C[t - 1];
+            L[t] = v + sh[t];
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) C[c] += p.pC[c * pcell + P];
+    }
 #pragma unroll
     for (int c = 0; c < 20; ++c) p.L[(long long)c * ocell + o] = L[c];
 #pragma unroll
@@ -233,7 +263,7 @@ __device__ __forceinline__ void store_target(const Params& p, const Acc& acc, co
 
 // The consumer warps' loop over the bricks of this CTA.  DIPOLE = false is the fast path for sources
 // expanded about their centre of mass (no dipole terms), see m2l_staged_kernel.
-template <bool CORR, bool DIPOLE>
+template <bool CORR, bool DIPOLE, bool FUSE_L2L>
 __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, uint64_t* full, uint64_t* empty, int warp, int lane)
 {
     // ------------------------------ consumers ------------------------------
@@ -321,11 +351,11 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         }
 #undef OCTO_FETCH
 
-        if (active) store_target<CORR>(p, acc, tA, gx, gy, k);
+        if (active) store_target<CORR, FUSE_L2L>(p, acc, tA, dA, gx, gy, k);
     }
 }
 
-template <bool CORR>
+template <bool CORR, bool FUSE_L2L = false>
 __global__ void __launch_bounds__(STAGED_THREADS, 1)
 m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
 {
@@ -372,8 +402,8 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
     // the flags if any cell has |M1_i| > DIPOLE_TOL |M| h, and only then (or when the caller forces it) the
     // 27 dipole terms are evaluated.  The branch is uniform over the grid.
     const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
-    if (dipole) staged_consume<CORR, true>(p, slab0, full, empty, warp, lane);
-    else        staged_consume<CORR, false>(p, slab0, full, empty, warp, lane);
+    if (dipole) staged_consume<CORR, true, FUSE_L2L>(p, slab0, full, empty, warp, lane);
+    else        staged_consume<CORR, false, FUSE_L2L>(p, slab0, full, empty, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -417,7 +447,7 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
             if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
             else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
         }
-        store_target<CORR>(p, acc, tA, gx, gy, k);
+        store_target<CORR>(p, acc, tA, dA, gx, gy, k);
     }
 }
 
@@ -469,7 +499,7 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
         for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
         v[c] = a;
     }
-    if (lane == 0) store_target<CORR>(p, acc, tA, gx, gy, k);
+    if (lane == 0) store_target<CORR>(p, acc, tA, dA, gx, gy, k);
 }
 
 // ------------------------------------------------------------------------------------------

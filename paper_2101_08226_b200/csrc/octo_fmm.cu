@@ -410,6 +410,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->outL = h->L; h->outC = h->C;
     P.S = h->src; P.L = h->L; P.C = h->C; P.flags = h->flags;
     P.force_dipole = 0;
+    P.pL = nullptr; P.pC = nullptr; P.poff = nullptr; P.hc = cfg->h;
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
         // ---- TMA descriptor of S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
@@ -428,7 +429,9 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         if (r != CUDA_SUCCESS) { delete h; return OCTO_FMM_ECUDA; }
         cudaError_t e1 = cudaFuncSetAttribute(m2l_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
-        if (e1 != cudaSuccess || e2 != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+        cudaError_t e3 = cudaFuncSetAttribute(m2l_staged_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        cudaError_t e4 = cudaFuncSetAttribute(m2l_staged_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
     } else if (cfg->kind == OCTO_FMM_MONOPOLE) {
         // ---- monopole weights of the 11^3 offsets: (-1/|R|, -R/|R|^3) with R = (i_A - i_B) h = -Delta h, in FP64
         //      on the host (sqrt, division); Delta = 0 gets zero weights ----
@@ -528,8 +531,13 @@ static int launch_staged(octo_fmm_t* h, int kb, int ke)
     P.tiles_z = (ke - kb + TILE_Z - 1) / TILE_Z;
     P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
     const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
-    if (h->cfg.am_correction) m2l_staged_kernel<true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-    else                      m2l_staged_kernel<false><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    if (P.pL) {            // complete solve: L2L fused into the epilogue (solver.inl sets the parent arrays)
+        if (h->cfg.am_correction) m2l_staged_kernel<true, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        else                      m2l_staged_kernel<false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    } else {
+        if (h->cfg.am_correction) m2l_staged_kernel<true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        else                      m2l_staged_kernel<false><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    }
     return cudaGetLastError() == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
 

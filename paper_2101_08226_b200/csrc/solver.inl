@@ -32,6 +32,13 @@ octo_fmm_config level_config(const octo_fmm_solver_config& sc, int n, double h, 
     return c;
 }
 
+// the parent level's finished expansions, for the fused L2L epilogue of the staged interaction kernel
+void set_parent(octo_fmm* h, const SolverLevel& p)
+{
+    h->prm.pL = p.fmm->L; h->prm.pC = p.fmm->C; h->prm.poff = p.off;
+}
+void clear_parent(octo_fmm* h) { h->prm.pL = nullptr; h->prm.pC = nullptr; h->prm.poff = nullptr; }
+
 bool solver_config_ok(const octo_fmm_solver_config* c)
 {
     if (!c) return false;
@@ -145,11 +152,17 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
     for (int lv = (int)s->lev.size() - 1; lv >= 0; --lv) {
         SolverLevel& l = s->lev[lv];
         if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
-        if ((rc = octo_fmm_interact(l.fmm)) != OCTO_FMM_OK) return rc;
+        const bool has_parent = lv < (int)s->lev.size() - 1;
+        // levels that run the TMA-staged kernel add the parent's expansion in its epilogue (no second pass over the level)
+        const bool fused = has_parent && l.fmm->kernel == 0;
+        if (fused) set_parent(l.fmm, s->lev[lv + 1]);
+        rc = octo_fmm_interact(l.fmm);
+        if (fused) clear_parent(l.fmm);
+        if (rc != OCTO_FMM_OK) return rc;
         const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
-        if (lv == (int)s->lev.size() - 1)
+        if (!has_parent)
             l2l_kernel<false><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, nullptr, nullptr, nullptr, l.n, l.n, l.n, l.h);
-        else {
+        else if (!fused) {
             SolverLevel& p = s->lev[lv + 1];
             l2l_kernel<true><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, p.fmm->L, p.fmm->C, p.off, l.n, l.n, l.n, l.h);
         }
@@ -194,11 +207,15 @@ int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t* s, const double* dmass, double
         SolverLevel& l = s->lev[lv];
         const int keep_corr = l.fmm->cfg.am_correction;
         l.fmm->cfg.am_correction = 0;
+        const bool has_parent = lv < (int)s->lev.size() - 1;
+        const bool fused = has_parent && l.fmm->kernel == 0;
         rc = octo_fmm_set_moments(l.fmm, l.raw, l.off);
+        if (fused) set_parent(l.fmm, s->lev[lv + 1]);
         if (rc == OCTO_FMM_OK) rc = octo_fmm_interact(l.fmm);       // writes C = 0
+        if (fused) clear_parent(l.fmm);
         l.fmm->cfg.am_correction = keep_corr;
         if (rc != OCTO_FMM_OK) return rc;
-        if (lv < (int)s->lev.size() - 1) {
+        if (has_parent && !fused) {
             SolverLevel& p = s->lev[lv + 1];
             const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
             l2l_kernel<true><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, p.fmm->L, p.fmm->C, p.off, l.n, l.n, l.n, l.h);
@@ -276,7 +293,13 @@ int octo_fmm_solver_num_levels(const octo_fmm_solver_t* s, int* multipole_levels
     const int nl = (int)s->lev.size();
     if (multipole_levels) *multipole_levels = nl;
     // leaf: stage + interact + leaf_eval; per multipole level: m2m + stage + interact + l2l
-    if (launches_per_solve) *launches_per_solve = 3 + 4 * nl;
+    // (the levels on the staged kernel, all but the coarsest, do their L2L in its epilogue)
+    if (launches_per_solve) {
+        int n = 3 + 4 * nl;
+        for (size_t lv = 0; lv + 1 < s->lev.size(); ++lv)
+            if (s->lev[lv].fmm->kernel == 0) --n;
+        *launches_per_solve = n;
+    }
     return OCTO_FMM_OK;
 }
 
