@@ -666,6 +666,54 @@ __device__ __forceinline__ void dmma_8x8x4(double& d0, double& d1, double a, dou
                  : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+// Complete solve: the leaf evaluation fused into the tensor-core leaf kernels (FUSE_EVAL).  When the sums of a block
+// are done its mass tile is dead, so the block parks them there, res = [NCOMP][8][16][16], and thread t takes parent cell
+// (t & 7, (t >> 3) & 7, t >> 6) of the tile: it loads the parent's finished expansion once, evaluates it at the centres of
+// its 8 leaves (phi += L0(e), g -= L1(e) + correction, e = ((a,b,c) - 1/2) h - delta_P) and stores every output exactly
+// once as x-pairs -- what leaf_eval_kernel does in a second pass over the leaves (read + write of all outputs).
+// Whole-grid output with even extents (the solver's leaves); out 16-byte aligned.
+template <int NCOMP>
+__device__ __forceinline__ void fused_leaf_eval(const Params& p, const double* __restrict__ res, double* __restrict__ out,
+                                                int x0, int y0, int z0)
+{
+    const int t = threadIdx.x;
+    const int I = t & 7, J = (t >> 3) & 7, K = t >> 6;
+    const int gx = x0 + 2 * I, gy = y0 + 2 * J, gz = z0 + 2 * K;
+    if (gx >= p.hi[0] || gy >= p.hi[1] || gz >= p.hi[2]) return;
+    const int pnx = p.nx >> 1, pny = p.ny >> 1;
+    const long long pcell = (long long)pnx * pny * (p.nz >> 1), ocell = (long long)p.ox * p.oy * p.oz;
+    const long long P = ((long long)(gz >> 1) * pny + (gy >> 1)) * pnx + (gx >> 1);
+    double L[20], C[3], dP[3];
+#pragma unroll
+    for (int c = 0; c < 20; ++c) L[c] = p.pL[c * pcell + P];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { C[c] = p.pC[c * pcell + P]; dP[c] = p.poff[c * pcell + P]; }
+    const double h = p.hc;
+#pragma unroll
+    for (int cz = 0; cz < 2; ++cz)
+#pragma unroll
+        for (int cy = 0; cy < 2; ++cy) {
+            const int r = ((2 * K + cz) * MT_Y + (2 * J + cy)) * MT_X + 2 * I;
+            const long long o = ((long long)(gz + cz - p.lo[2]) * p.oy + (gy + cy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+            double sh0[20], sh1[20];
+            const double e0[3] = {-0.5 * h - dP[0], ((double)cy - 0.5) * h - dP[1], ((double)cz - 0.5) * h - dP[2]};
+            const double e1[3] = {0.5 * h - dP[0], e0[1], e0[2]};
+            taylor_shift<1>(L, e0, sh0);
+            taylor_shift<1>(L, e1, sh1);
+            const double2 s = *reinterpret_cast<const double2*>(res + r);
+            *reinterpret_cast<double2*>(out + o) = make_double2(s.x + sh0[0], s.y + sh1[0]);
+            if constexpr (NCOMP == 4) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double2 g = *reinterpret_cast<const double2*>(res + (1 + c) * (MT_X * MT_Y * DT_Z) + r);
+                    *reinterpret_cast<double2*>(out + (1 + c) * ocell + o) =
+                        make_double2(g.x - (sh0[1 + c] + C[c]), g.y - (sh1[1 + c] + C[c]));
+                }
+            }
+        }
+}
+
+template <bool FUSE_EVAL = false>
 __global__ void __launch_bounds__(DMMA_THREADS, 2)
 p2p_monopole_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params p, const DmmaEntry* __restrict__ tab,
                          const DmmaLists dl, double* __restrict__ out)
@@ -717,13 +765,17 @@ p2p_monopole_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params 
     const int v = lane >> 4, comp = (lane >> 2) & 3;
     const int gx = x0 + 4 * (lane & 3) + 2 * v;
     const long long ocell = (long long)p.ox * p.oy * p.oz;
+    if constexpr (FUSE_EVAL) __syncthreads();          // every warp has finished reading the mass tile
 #pragma unroll
     for (int g = 0; g < 16; ++g) {
         const double send = v ? acc[g][0] : acc[g][1];
         const double recv = __shfl_xor_sync(0xffffffffu, send, 16);
         const double lo = v ? recv : acc[g][0], hi = v ? acc[g][1] : recv;
         const int gy = y0 + py + 2 * (g & 7), k = z0 + pz + 4 * half + 2 * (g >> 3);
-        if (gy < p.hi[1] && k < p.hi[2] && gx < p.hi[0]) {
+        if constexpr (FUSE_EVAL) {
+            *reinterpret_cast<double2*>(tile + comp * (MT_X * MT_Y * DT_Z) + ((k - z0) * MT_Y + (gy - y0)) * MT_X + (gx - x0)) =
+                make_double2(lo, hi);
+        } else if (gy < p.hi[1] && k < p.hi[2] && gx < p.hi[0]) {
             double* dst = out + comp * ocell + ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
             if (gx + 1 < p.hi[0] && (reinterpret_cast<uintptr_t>(dst) & 15) == 0) {
                 *reinterpret_cast<double2*>(dst) = make_double2(lo, hi);
@@ -732,6 +784,10 @@ p2p_monopole_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params 
                 if (gx + 1 < p.hi[0]) dst[1] = hi;
             }
         }
+    }
+    if constexpr (FUSE_EVAL) {
+        __syncthreads();
+        fused_leaf_eval<4>(p, tile, out, x0, y0, z0);
     }
 }
 

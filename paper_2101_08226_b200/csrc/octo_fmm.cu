@@ -474,7 +474,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) {
                 delete h; return OCTO_FMM_ECUDA;
             }
-            if (cudaFuncSetAttribute(p2p_monopole_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess ||
+            if (cudaFuncSetAttribute(p2p_monopole_dmma_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess ||
+                cudaFuncSetAttribute(p2p_monopole_dmma_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess ||
                 cudaFuncSetAttribute(p2p_potential_dmma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, DMMA_SMEM) != cudaSuccess) {
                 delete h; return OCTO_FMM_ECUDA;
             }
@@ -562,8 +563,10 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        if (h->mono_kernel == 0)
-            p2p_monopole_dmma_kernel<<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
+        if (h->mono_kernel == 0 && P.pL)        // complete solve: leaf evaluation fused into the epilogue (solver.inl)
+            p2p_monopole_dmma_kernel<true><<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
+        else if (h->mono_kernel == 0)
+            p2p_monopole_dmma_kernel<false><<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
         else
             p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(h->tmap, P, h->W, h->outL);
     } else if (h->kernel == 1) {
@@ -868,7 +871,7 @@ int octo_fmm_launch_info(const octo_fmm_t* h, int* grid, int* block, int* smem_b
     cudaError_t e;
     int g, b, s;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE && h->mono_kernel == 0) {
-        e = cudaFuncGetAttributes(&fa, p2p_monopole_dmma_kernel);
+        e = cudaFuncGetAttributes(&fa, p2p_monopole_dmma_kernel<false>);
         g = dmma_blocks(P); b = DMMA_THREADS; s = DMMA_SMEM;
     } else if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
         e = cudaFuncGetAttributes(&fa, p2p_monopole_kernel);

@@ -169,12 +169,16 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     // ---- leaves: monopole sum over the leaf-level list straight into `out`, then the parent's expansion ----
+    // (the tensor-core leaf kernel evaluates the parent's expansion in its epilogue; the DFMA kernel needs the extra pass)
     double* const keep = s->leaf->outL;
+    const bool fused_eval = s->leaf->mono_kernel == 0;
     s->leaf->outL = out;
+    if (fused_eval) set_parent(s->leaf, s->lev[0]);
     rc = octo_fmm_interact(s->leaf);
+    if (fused_eval) clear_parent(s->leaf);
     s->leaf->outL = keep;
     if (rc != OCTO_FMM_OK) return rc;
-    {
+    if (!fused_eval) {
         const int n = s->cfg.n;
         SolverLevel& p = s->lev[0];
         leaf_eval_kernel<false><<<dim3((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2)), 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
@@ -223,6 +227,8 @@ int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t* s, const double* dmass, double
         }
     }
     // leaves: only the potential of this solve is used (Eq. 3): potential-only leaf sum and evaluation
+    // (fusing the evaluation into this kernel's epilogue as in solve() was measured slower: with a quarter of the
+    //  contractions per tile the epilogue is not hidden)
     if ((rc = interact_potential(s->leaf, out)) != OCTO_FMM_OK) return rc;
     {
         const int n = s->cfg.n;
@@ -295,7 +301,7 @@ int octo_fmm_solver_num_levels(const octo_fmm_solver_t* s, int* multipole_levels
     // leaf: stage + interact + leaf_eval; per multipole level: m2m + stage + interact + l2l
     // (the levels on the staged kernel, all but the coarsest, do their L2L in its epilogue)
     if (launches_per_solve) {
-        int n = 3 + 4 * nl;
+        int n = 3 + 4 * nl - (s->leaf->mono_kernel == 0 ? 1 : 0);     // tensor-core leaf kernel: no leaf_eval launch
         for (size_t lv = 0; lv + 1 < s->lev.size(); ++lv)
             if (s->lev[lv].fmm->kernel == 0) --n;
         *launches_per_solve = n;

@@ -58,7 +58,7 @@ def test_random_masses_32(env, theta, correction):
     leaf_cnt = oracle.interact_monopole_leaf((n, n, n), h, theta, mass)[1]
     assert s.interaction_count() == leaf_cnt + _oracle_count(n, theta)
     assert s.leaf_interaction_count() == leaf_cnt
-    assert s.num_levels() == (4, 19)
+    assert s.num_levels() == (4, 18)       # the tensor-core leaf kernel evaluates the parent expansion itself
     e_phi, e_g = _errors(out.cpu().numpy(), ref)
     assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
     s.close()
