@@ -547,3 +547,52 @@ def test_extreme_opening_angles(env, theta):
         Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, w.out_lo, w.out_hi, True)
         assert cnt == cntr
         check(L, Lc, Lr, Lcr)
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_random_configurations(env, seed):
+    """Seeded random configurations against the oracle: non-cubic grids of 1..5 sub-grids per axis, theta anywhere in
+    (0.34, 0.95), cell widths over two decades, whole-grid and sub-grid-aligned output regions, both kinds, correction
+    on and off, sources with and without dipole moments, every interaction kernel (staged / direct / one warp per cell;
+    tensor-core / DFMA monopole)."""
+    p, torch = env
+    rng = np.random.default_rng(seed)
+    for _ in range(8):
+        n = tuple(int(8 * rng.integers(1, 6)) for _ in range(3))
+        theta = float(rng.uniform(0.34, 0.95))
+        h = float(rng.uniform(0.01, 2.0))
+        if rng.random() < 0.5:
+            lo = tuple(int(8 * rng.integers(0, n[a] // 8)) for a in range(3))
+            hi = tuple(int(lo[a] + 8 * rng.integers(1, (n[a] - lo[a]) // 8 + 1)) for a in range(3))
+        else:
+            lo, hi = (0, 0, 0), n
+        region = dict(out_lo=lo, out_hi=hi) if (lo, hi) != ((0, 0, 0), n) else {}
+        if rng.integers(0, 2):
+            mass = rng.random(n[::-1]) * h ** 3
+            ref, cnt = oracle.interact_monopole(n, h, theta, mass, lo, hi)
+            for mono_kernel in (0, 1):
+                f = p.OctoFMM(n, h, theta, p.MONOPOLE, **region)
+                f.set_option("mono_kernel", mono_kernel)
+                out, _ = f.solve(torch.from_numpy(mass[None].copy()).cuda())
+                torch.cuda.synchronize()
+                assert f.interaction_count() == cnt
+                if cnt:
+                    assert parity_error(out.cpu().numpy(), ref) < TOL, (mono_kernel, n, theta, lo, hi)
+                f.close()
+        else:
+            corr = bool(rng.integers(0, 2))
+            mom = rng.normal(size=(20,) + n[::-1]) * 1e-3 * h ** 3
+            mom[0] = (0.5 + rng.random(n[::-1])) * h ** 3
+            mom[1:4] *= h * (0.0 if rng.random() < 0.5 else 1.0)
+            mom[4:10] *= 30 * h * h
+            mom[10:20] *= 30 * h ** 3
+            com = (rng.random((3,) + n[::-1]) - 0.5) * 0.4 * h
+            Lr, Lcr, cnt = oracle.interact_multipole(n, h, theta, mom, com, lo, hi, corr)
+            for kernel in (0, 1, 2):
+                f = p.OctoFMM(n, h, theta, p.MULTIPOLE, corr, **region)
+                f.set_option("kernel", kernel)
+                L, Lc = f.solve(torch.from_numpy(mom).cuda(), torch.from_numpy(com).cuda())
+                torch.cuda.synchronize()
+                assert f.status() == p.OK and f.interaction_count() == cnt
+                assert parity_error(L.cpu().numpy(), Lr) < TOL, (kernel, corr, n, theta, lo, hi)
+                f.close()
