@@ -494,18 +494,19 @@ def test_default_kernel_choice(env):
     big.close()
 
 
-def test_large_grid_400_sampled(env):
-    """A grid larger than any BASELINE configuration (400^3 = 64 M cells, about 46 GB on the device; 400 is not a
-    power of two and leaves ragged bricks in z): sources are generated on the device, and sampled 16^3 regions are
-    recomputed by the oracle from their 28^3 neighbourhoods (6 >= reach cells of halo, even-aligned so that the
-    parities agree; clipped at the domain faces)."""
+@pytest.mark.parametrize("n,need_gb", [(400, 60), (512, 110)])
+def test_large_grid_sampled(env, n, need_gb):
+    """Grids larger than any BASELINE configuration: 400^3 = 64 M cells (about 46 GB on the device; 400 is not a power
+    of two and leaves ragged bricks in z) and 512^3 = 134 M cells (about 96 GB; 2.7e9 moments, i.e. element indices
+    beyond 2^31).  Sources are generated on the device, and sampled 16^3 regions are recomputed by the oracle from their
+    28^3 neighbourhoods (6 >= reach cells of halo, even-aligned so that the parities agree; clipped at the domain faces)."""
     p, torch = env
     torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
-    if free < 60e9:
-        pytest.skip("needs 60 GB of free device memory")
-    n, h = 400, 1.0 / 400
-    g = torch.Generator(device="cuda").manual_seed(400)
+    if free < need_gb * 1e9:
+        pytest.skip("needs %d GB of free device memory" % need_gb)
+    h = 1.0 / n
+    g = torch.Generator(device="cuda").manual_seed(n)
     mom = torch.rand((20, n, n, n), dtype=torch.float64, device="cuda", generator=g)
     mom[1:] -= 0.5
     mom[0] += 0.5
@@ -522,7 +523,8 @@ def test_large_grid_400_sampled(env):
     f.interact()
     assert f.status() == p.OK and f.dipole_terms_used()
     assert f.interaction_count() == oracle.interaction_count((n, n, n), 0.5)
-    for lo in ((0, 0, 0), (384, 384, 384), (192, 0, 384), (208, 176, 96), (384, 192, 192)):
+    m = n - 16
+    for lo in ((0, 0, 0), (m, m, m), (n // 2 - 8, 0, m), (208, 176, 96), (m, n // 2 - 8, n // 2 - 8)):
         blo = [max(v - 6, 0) for v in lo]
         bhi = [min(v + 22, n) for v in lo]
         sl = (slice(None), slice(blo[2], bhi[2]), slice(blo[1], bhi[1]), slice(blo[0], bhi[0]))
