@@ -88,7 +88,7 @@ def test_binary_field_64_and_conservation(env):
     s.close()
 
 
-@pytest.mark.parametrize("n,theta", [(128, 0.5), (256, 0.5), (512, 0.5), (256, 0.35)])
+@pytest.mark.parametrize("n,theta", [(128, 0.5), (256, 0.5), (512, 0.5), (128, 0.35), (256, 0.35)])
 def test_uniform_sphere_residuals_table1(env, n, theta):
     """Section 3.4 on the GPU at the grids of Table 1 (tests/golden/table1_sphere.txt): residuals against the
     analytic potential within a factor 3 of the printed max and mean (the paper does not state its rasterisation nor
