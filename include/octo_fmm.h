@@ -143,6 +143,9 @@ int octo_fmm_dipole_terms_used(octo_fmm_t *h, int *used);
  * cells), 1 direct (one cell per thread, global-memory loads; same pair arithmetic), 2 one warp per cell with
  * a warp-level reduction of the partial expansions (default up to 4096 target cells).
  * "dipole_terms" = 0 decided on the device (default), 1 always evaluated.
+ * "am_correction" = 0 / 1 (MULTIPOLE handles): switches the correction of cfg.am_correction for the following
+ * set_moments() + interact() (the handle goes back to the "created" state) -- one handle and one workspace can
+ * so serve a second right-hand side on the same centres (d(rho)/dt, L81-83: no correction) after the first.
  * "host_chunk" = output z-layers per pipeline slab of octo_fmm_run_host (default 12; 0 = one copy in, one
  * launch, one copy out).
  * "mono_kernel" (MONOPOLE handles) = 0 the sum as 8x8x4 FP64 tensor-core contractions (mma.sync m8n8k4.f64:

@@ -850,6 +850,12 @@ int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
         h->mono_kernel = value;
         return OCTO_FMM_OK;
     }
+    if (!std::strcmp(key, "am_correction")) {    // multipole handles: switch the correction for the next set_moments() + interact()
+        if (h->cfg.kind != OCTO_FMM_MULTIPOLE || (value != 0 && value != 1)) return OCTO_FMM_EINVAL;
+        h->cfg.am_correction = value;
+        h->state = 0;                            // the staged sources depend on it: set_moments() again
+        return OCTO_FMM_OK;
+    }
     if (!std::strcmp(key, "dipole_terms")) {     // 0 = decided on the device from the staged sources (default), 1 = always
         if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
         h->prm.force_dipole = value;

@@ -598,3 +598,35 @@ def test_random_configurations(env, seed):
                 assert f.status() == p.OK and f.interaction_count() == cnt
                 assert parity_error(L.cpu().numpy(), Lr) < TOL, (kernel, corr, n, theta, lo, hi)
                 f.close()
+
+
+def test_second_right_hand_side_on_one_handle(env):
+    """f2 at the kernel level (L81-83): after the density's step, the same handle and workspace take the moments of
+    d(rho)/dt about the SAME centres -- signed, with dipoles -- with the correction switched off."""
+    p, torch = env
+    w = fi.config1(seed=31, ncell=32)
+    rng = np.random.default_rng(31)
+    mom2 = w.moments * rng.uniform(-1.0, 1.0, w.moments.shape)          # signed masses, dipoles, everything
+    mom2[1:4] = rng.normal(size=mom2[1:4].shape) * np.abs(w.moments[0]) * w.h * 0.1
+    f = p.OctoFMM(w.n, w.h, w.theta, p.MULTIPOLE, True)
+    com = torch.from_numpy(w.com_off).cuda()
+    L1, Lc1 = f.solve(torch.from_numpy(w.moments).cuda(), com)
+    f.set_option("am_correction", 0)
+    with pytest.raises(p.OctoFmmError):
+        f.interact()                                                      # the sources must be staged again
+    L2, Lc2 = f.solve(torch.from_numpy(mom2).cuda(), com)
+    torch.cuda.synchronize()
+    assert f.status() == p.OK and f.dipole_terms_used()
+    r1 = oracle.interact_multipole(w.n, w.h, w.theta, w.moments, w.com_off, None, None, True)
+    r2 = oracle.interact_multipole(w.n, w.h, w.theta, mom2, w.com_off, None, None, False)
+    check(L1.cpu().numpy(), Lc1.cpu().numpy(), r1[0], r1[1])
+    # signed sources: a cell's own L0 can cancel to nothing, so the orders are normalised over the grid, not per cell
+    g2 = L2.cpu().numpy()
+    assert parity_error(g2, r2[0]) < TOL
+    for lo, hi in ((0, 1), (1, 4), (4, 10), (10, 20)):
+        assert np.abs(g2[lo:hi] - r2[0][lo:hi]).max() / np.abs(r2[0][lo:hi]).max() < TOL
+    assert float(Lc2.abs().max()) == 0.0
+    f.set_option("am_correction", 1)
+    L3, _ = f.solve(torch.from_numpy(w.moments).cuda(), com)
+    assert torch.equal(L3, L1)
+    f.close()
