@@ -50,6 +50,8 @@ def lib():
         L.fmm_oracle_interact_multipole.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                                     dp, dp, dp, dp, ullp]
         L.fmm_oracle_interact_monopole.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, dp, dp, ullp]
+        L.fmm_oracle_interact_multipole_mixed.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                                          dp, dp, ctypes.POINTER(ctypes.c_ubyte), dp, dp, ullp]
         L.fmm_oracle_interaction_count.argtypes = [ip, ip, ip, ctypes.c_double, ullp]
         L.fmm_oracle_stencil_leaf.argtypes = L.fmm_oracle_stencil.argtypes
         L.fmm_oracle_interact_monopole_leaf.argtypes = L.fmm_oracle_interact_monopole.argtypes
@@ -126,6 +128,29 @@ def interact_multipole(n, h, theta, moments, com_off, out_lo=None, out_hi=None, 
                                          int(bool(am_correction)), _dp(moments), _dp(com_off), _dp(Lout), _dp(Lc),
                                          ctypes.byref(cnt))
     _check(rc, "interact_multipole")
+    return Lout, Lc, cnt.value
+
+
+def interact_multipole_mixed(n, h, theta, moments, com_off, leaf, out_lo=None, out_hi=None, am_correction=True):
+    """One level of an adaptive mesh: leaf[nz][ny][nx] = 1 where the cell belongs to a leaf sub-grid.
+    Partners of A = the Eq. 15 list + the near-field cells B with leaf[A] or leaf[B].  Returns (L, Lcorr, n_interactions)."""
+    L = lib()
+    out_lo = (0, 0, 0) if out_lo is None else out_lo
+    out_hi = tuple(n) if out_hi is None else out_hi
+    moments = np.ascontiguousarray(moments, dtype=np.float64)
+    com_off = np.ascontiguousarray(com_off, dtype=np.float64)
+    leaf = np.ascontiguousarray(leaf, dtype=np.uint8)
+    nx, ny, nz = n
+    assert moments.shape == (20, nz, ny, nx) and com_off.shape == (3, nz, ny, nx) and leaf.shape == (nz, ny, nx)
+    o = tuple(out_hi[a] - out_lo[a] for a in range(3))
+    Lout = np.zeros((20, o[2], o[1], o[0]))
+    Lc = np.zeros((3, o[2], o[1], o[0]))
+    cnt = ctypes.c_ulonglong(0)
+    rc = L.fmm_oracle_interact_multipole_mixed(_i3(n), _i3(out_lo), _i3(out_hi), float(h), float(theta),
+                                               int(bool(am_correction)), _dp(moments), _dp(com_off),
+                                               leaf.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte)), _dp(Lout), _dp(Lc),
+                                               ctypes.byref(cnt))
+    _check(rc, "interact_multipole_mixed")
     return Lout, Lc, cnt.value
 
 

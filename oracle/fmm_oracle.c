@@ -315,15 +315,17 @@ static void free_stencils(stencil_set *S) { for (int p = 0; p < 8; ++p) free(S->
  * L gets the correction folded into L1 when enabled; Lcorr (may be NULL) gets it alone.
  * n_interactions (may be NULL) receives the number of ordered in-domain pairs.
  */
-int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int out_hi[3], double h,
-                                  double theta, int am_correction, const double *moments,
-                                  const double *com_off, double *L, double *Lcorr,
-                                  unsigned long long *n_interactions)
+static int interact_multipole_impl(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                   double theta, int am_correction, const double *moments,
+                                   const double *com_off, const unsigned char *leaf, double *L, double *Lcorr,
+                                   unsigned long long *n_interactions)
 {
     if (!n || !out_lo || !out_hi || !moments || !com_off || !L || !(h > 0.0)) return ORC_EINVAL;
     if (!check_region(n, out_lo, out_hi)) return ORC_EINVAL;
     stencil_set S;
-    if (build_stencils(theta, &S) != ORC_OK) return ORC_EINVAL;
+    /* leaf != NULL (a level of an adaptive mesh, see fmm_oracle_interact_multipole_mixed): candidates are the Eq. 15
+     * list plus the near field; a near-field pair counts only if A or B is a leaf cell */
+    if (build_stencils_mode(theta, leaf != NULL, &S) != ORC_OK) return ORC_EINVAL;
 
     const size_t nx = n[0], ny = n[1], nz = n[2], ncell = nx * ny * nz;
     const size_t ox = out_hi[0] - out_lo[0], oy = out_hi[1] - out_lo[1], oz = out_hi[2] - out_lo[2];
@@ -349,6 +351,7 @@ int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int
                     const int bi = i + dx, bj = j + dy, bk = k + dz;
                     if (bi < 0 || bj < 0 || bk < 0 || bi >= (int)nx || bj >= (int)ny || bk >= (int)nz) continue;
                     const size_t b = ((size_t)bk * ny + bj) * nx + bi;
+                    if (leaf && !leaf[a] && !leaf[b] && !is_partner_mode(i & 1, j & 1, k & 1, dx, dy, dz, theta, 0)) continue;
                     double MB[20], R[3], term[20], cterm[3];
                     for (int c = 0; c < 20; ++c) MB[c] = moments[(size_t)c * ncell + b];
                     R[0] = (double)(i - bi) * h + (dA[0] - com_off[0 * ncell + b]);
@@ -369,6 +372,32 @@ int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int
     free_stencils(&S);
     if (n_interactions) *n_interactions = total;
     return bad_mass ? ORC_EMASS : ORC_OK;
+}
+
+int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                  double theta, int am_correction, const double *moments,
+                                  const double *com_off, double *L, double *Lcorr,
+                                  unsigned long long *n_interactions)
+{
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, L, Lcorr, n_interactions);
+}
+
+/*
+ * One level of an ADAPTIVE mesh (a node "is either fully refined with eight child
+ * nodes (an interior node) or not refined at all (a leaf node)"; the paper does not describe the gravity side of a
+ * refinement boundary -- DESIGN.md reading R8).  leaf[cell] = 1: the cell belongs to a leaf sub-grid (it has no
+ * children), 0: to a refined one.  Well-separated pairs (Eq. 15 list) interact here whatever their kind.  A pair that is
+ * NOT well separated is normally left to the children (L135); when A or B has none, nobody below will take it, so it is
+ * taken here, with the same pair formula (a leaf is the special case M1 = M2 = M3 = 0, delta = 0 of its moments).
+ * Hence: partners of A = Eq. 15 list + those near-field cells B for which leaf[A] or leaf[B].
+ */
+int fmm_oracle_interact_multipole_mixed(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                        double theta, int am_correction, const double *moments,
+                                        const double *com_off, const unsigned char *leaf, double *L, double *Lcorr,
+                                        unsigned long long *n_interactions)
+{
+    if (!leaf) return ORC_EINVAL;
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, leaf, L, Lcorr, n_interactions);
 }
 
 /*
