@@ -139,6 +139,18 @@ int octo_fmm_run_host(octo_fmm_t *h, const double *moments_host, const double *c
  * octo_fmm_dipole_terms_used() synchronises the stream and tells which path interact() takes. */
 int octo_fmm_dipole_terms_used(octo_fmm_t *h, int *used);
 
+/* One level of an ADAPTIVE mesh (a node "is either fully refined with eight child nodes
+ * (an interior node) or not refined at all (a leaf node)"; the paper does not describe the gravity side of a
+ * refinement boundary: DESIGN.md reading R8).  leaf: device, [nz][ny][nx] bytes, 1 = the cell belongs to a leaf
+ * sub-grid (it has no children; hand it over as a point mass: M1 = M2 = M3 = 0, offset 0), 0 = to a refined one.
+ * octo_fmm_interact_mixed() = octo_fmm_interact() (the list of Eq. 15, whatever the cells' kind) + the near-field
+ * pairs nobody below this level will take: a cell B that is NOT well separated from A (and whose parent is not well
+ * separated from A's) interacts with A here if A or B is a leaf.  Same pair formula, same outputs (get_expansions).
+ * MULTIPOLE handles; asynchronous on the stream.  octo_fmm_mixed_interaction_count() synchronises the stream and
+ * returns the number of ordered pairs the last octo_fmm_interact_mixed() evaluated (it depends on leaf). */
+int octo_fmm_interact_mixed(octo_fmm_t *h, const unsigned char *leaf);
+int octo_fmm_mixed_interaction_count(octo_fmm_t *h, unsigned long long *n);
+
 /* Options, for tests and profiling.  "kernel" = 0 staged (TMA + shared memory; default above 4096 target
  * cells), 1 direct (one cell per thread, global-memory loads; same pair arithmetic), 2 one warp per cell with
  * a warp-level reduction of the partial expansions (default up to 4096 target cells).

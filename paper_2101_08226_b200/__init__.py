@@ -66,6 +66,8 @@ class _Library:
         lib.octo_fmm_destroy.argtypes = [vp]
         lib.octo_fmm_bind_outputs.argtypes = [vp, vp, vp]
         lib.octo_fmm_get_stencil.argtypes = [vp, ctypes.c_int, ip, vp]
+        lib.octo_fmm_interact_mixed.argtypes = [vp, vp]
+        lib.octo_fmm_mixed_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_dmma_table.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, vp, vp]
         lib.octo_fmm_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_status.argtypes = [vp]
@@ -190,6 +192,20 @@ def octo_fmm_get_stencil(h, parity):
     if rc != OK:
         raise OctoFmmError("octo_fmm_get_stencil", rc)
     return out
+
+
+def octo_fmm_interact_mixed(h, leaf):
+    rc = _lib.octo_fmm_interact_mixed(h, _ptr(leaf))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_interact_mixed", rc)
+
+
+def octo_fmm_mixed_interaction_count(h):
+    n = ctypes.c_ulonglong(0)
+    rc = _lib.octo_fmm_mixed_interaction_count(h, ctypes.byref(n))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_mixed_interaction_count", rc)
+    return int(n.value)
 
 
 def octo_fmm_dmma_table(theta, h, leaf, which):
@@ -465,6 +481,13 @@ class OctoFMM:
 
     def interact(self):
         octo_fmm_interact(self.handle)
+
+    def interact_mixed(self, leaf):
+        """One level of an adaptive mesh: leaf = uint8 [nz][ny][nx] on the device, 1 where the cell is a leaf."""
+        octo_fmm_interact_mixed(self.handle, leaf)
+
+    def mixed_interaction_count(self):
+        return octo_fmm_mixed_interaction_count(self.handle)
 
     def get_expansions(self, L=None, Lcorr=None, want_corr=True):
         torch = self.torch

@@ -56,6 +56,9 @@ struct StEntry {
 __constant__ StEntry c_entries[8 * MAX_LIST];
 __constant__ int c_begin[8][2 * REACH_MAX + 2];   // first entry of (class, dz); [..][11] = end
 __constant__ double c_hmul[2 * REACH_MAX + 1];    // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h)
+constexpr int MAX_NEAR = 96;                      // near field (cells that are NOT well separated): <= 92 for 1/3 < theta
+__constant__ char4 c_near[8][MAX_NEAR];           // (dx, dy, dz, 0) of the near-field cells of each parity class
+__constant__ int c_near_count[8];
 
 struct Params {
     int nx, ny, nz;
@@ -448,6 +451,73 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
             else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
         }
         store_target<CORR>(p, acc, tA, dA, gx, gy, k);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// One level of an adaptive mesh (reading R8): the near-field pairs.  leaf[cell] = 1: the cell
+// belongs to a leaf sub-grid (no children).  A pair that is not well separated is normally left to the children; when A or
+// B has none it is taken at this level with the same pair formula.  Runs AFTER an interaction kernel has written the
+// Eq. 15 part: one thread per target cell (warps = parity classes as in m2l_direct_kernel), the near-field cells B with
+// leaf[A] | leaf[B] are accumulated and the finished coefficients are ADDED to L and Lcorr (acc_finish is linear).
+// count (may be null): number of pairs taken, for the bit-exact check of the pair set.
+// ------------------------------------------------------------------------------------------
+template <bool CORR>
+__global__ void __launch_bounds__(256) m2l_near_kernel(const Params p, const unsigned char* __restrict__ leaf,
+                                                       unsigned long long* __restrict__ count)
+{
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const int px = warp & 1, py = (warp >> 1) & 1, pz = warp >> 2;
+    const int bx = (p.ox + 15) / 16, by = (p.oy + 7) / 8;
+    const int b = blockIdx.x;
+    const int x0 = p.lo[0] + (b % bx) * 16, y0 = p.lo[1] + ((b / bx) % by) * 8, z0 = p.lo[2] + (b / (bx * by)) * 4;
+    const int gx = x0 + px + 2 * (lane & 7), gy = y0 + py + 2 * (lane >> 3);
+    const long long plane = (long long)p.ny * p.nx;
+    const double2* S2 = reinterpret_cast<const double2*>(p.S);
+    const int cls = warp;
+    const long long ocell = (long long)p.ox * p.oy * p.oz;
+    unsigned long long taken = 0;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int k = z0 + pz + 2 * pass;
+        if (!(gx < p.hi[0] && gy < p.hi[1] && k < p.hi[2])) continue;
+        const bool leafA = leaf[(long long)k * plane + (long long)gy * p.nx + gx] != 0;
+        double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        load_target<CORR>(p, gx, gy, k, dA, tA);
+        Acc acc;
+        acc_zero(acc);
+        const int n_near = c_near_count[cls];
+        bool any = false;
+#pragma unroll 1
+        for (int s = 0; s < n_near; ++s) {
+            const char4 e = c_near[cls][s];
+            const int sx = gx + e.x, sy = gy + e.y, sz = k + e.z;
+            if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
+            if (!leafA && leaf[(long long)sz * plane + (long long)sy * p.nx + sx] == 0) continue;
+            const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
+            double src[16], bx_, by_, bz_;
+            OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
+            const double x = c_hmul[e.x + REACH_MAX] + (dA[0] - bx_);
+            const double y = c_hmul[e.y + REACH_MAX] + (dA[1] - by_);
+            const double z = c_hmul[e.z + REACH_MAX] + (dA[2] - bz_);
+            m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
+            any = true;
+            ++taken;
+        }
+        if (any) {
+            double L[20], C[3];
+            acc_finish<CORR>(acc, tA, L, C);
+            const long long o = ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
+#pragma unroll
+            for (int c = 0; c < 20; ++c) p.L[(long long)c * ocell + o] += L[c];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) p.C[(long long)c * ocell + o] += C[c];
+        }
+    }
+    if (count) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) taken += __shfl_xor_sync(0xffffffffu, taken, o);
+        if (lane == 0 && taken) atomicAdd(count, taken);
     }
 }
 

@@ -240,6 +240,8 @@ struct octo_fmm {
     int reach;
     std::vector<Offset3> list[8];
     std::vector<StEntry> entries;          // 8 * MAX_LIST
+    std::vector<char4> near_list;          // 8 * MAX_NEAR: the near field of each parity class (mixed levels, f3)
+    int near_count[8];
     int begin[8][2 * REACH_MAX + 2];
     double hmul[2 * REACH_MAX + 1];
     double4* W;            // monopole: device table of the weights of the 11^3 offsets
@@ -248,6 +250,7 @@ struct octo_fmm {
     int nchunk_pot;        // chunks of the potential-only table (after the four tables of dl in T)
     CUtensorMap tmap2;     // monopole: the 16 x 16 x 8 tile box of p2p_monopole_dmma_kernel
     int mono_kernel;       // 0 tensor-core instruction (default), 1 DFMA
+    bool mixed;            // the last interaction was octo_fmm_interact_mixed
     unsigned long long n_interactions;
     CUtensorMap tmap;
     Params prm;
@@ -316,6 +319,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->state = 0;
     h->kernel = 0;
     h->mono_kernel = 0;
+    h->mixed = false;
     h->host_chunk = 12;
     h->host_launches = 0;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
@@ -332,6 +336,21 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     if (h->reach > REACH_MAX) { delete h; return OCTO_FMM_EINVAL; }
     for (int p = 0; p < 8; ++p)
         if ((int)h->list[p].size() > MAX_LIST) { delete h; return OCTO_FMM_EINVAL; }
+
+    // near field = the leaf-level list minus the Eq. 15 list (cells that are not well separated whose parents are not either)
+    h->near_list.assign((size_t)8 * MAX_NEAR, char4{0, 0, 0, 0});
+    for (int p = 0; p < 8; ++p) {
+        int r = 0;
+        const std::vector<Offset3> full = build_list(p & 1, (p >> 1) & 1, (p >> 2) & 1, cfg->theta, &r, true);
+        int n = 0;
+        for (const Offset3& o : full) {
+            const long long c2 = (long long)o.d[0] * o.d[0] + (long long)o.d[1] * o.d[1] + (long long)o.d[2] * o.d[2];
+            if (well_separated(c2, cfg->theta)) continue;
+            if (n == MAX_NEAR) { delete h; return OCTO_FMM_EINVAL; }
+            h->near_list[(size_t)p * MAX_NEAR + n++] = char4{o.d[0], o.d[1], o.d[2], 0};
+        }
+        h->near_count[p] = n;
+    }
 
     h->entries.assign((size_t)8 * MAX_LIST, StEntry{0, 0, 0, 0, 0});
     for (int p = 0; p < 8; ++p) {
@@ -515,6 +534,11 @@ static int upload_tables(octo_fmm_t* h)
                                     cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
         if (cudaMemcpyToSymbolAsync(c_begin, h->begin, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
             return OCTO_FMM_ECUDA;
+        if (cudaMemcpyToSymbolAsync(c_near, h->near_list.data(), h->near_list.size() * sizeof(char4), 0, cudaMemcpyHostToDevice,
+                                    h->stream) != cudaSuccess ||
+            cudaMemcpyToSymbolAsync(c_near_count, h->near_count, sizeof(h->near_count), 0, cudaMemcpyHostToDevice, h->stream) !=
+                cudaSuccess)
+            return OCTO_FMM_ECUDA;
         g_list_sig = h->list_sig;
     }
     if (cudaMemcpyToSymbolAsync(c_hmul, h->hmul, sizeof(h->hmul), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
@@ -581,7 +605,35 @@ int octo_fmm_interact(octo_fmm_t* h)
     }
     if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     h->state = 2;
+    h->mixed = false;
     h->resL = h->outL; h->resC = h->outC;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_interact_mixed(octo_fmm_t* h, const unsigned char* leaf)
+{
+    if (!h || !leaf || h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
+    const int rc = octo_fmm_interact(h);                       // the Eq. 15 part, whatever the cells' kind
+    if (rc != OCTO_FMM_OK) return rc;
+    unsigned long long* cnt = reinterpret_cast<unsigned long long*>(h->flags + 2);
+    if (cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    Params P = h->prm;
+    P.L = h->outL; P.C = h->outC;
+    if (h->cfg.am_correction) m2l_near_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, cnt);
+    else                      m2l_near_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, cnt);
+    if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    h->mixed = true;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_mixed_interaction_count(octo_fmm_t* h, unsigned long long* n)
+{
+    if (!h || !n) return OCTO_FMM_EINVAL;
+    if (h->state < 2 || !h->mixed) return OCTO_FMM_ESTATE;
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    unsigned long long near = 0;
+    if (cudaMemcpy(&near, h->flags + 2, sizeof near, cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
+    *n = h->n_interactions + near;
     return OCTO_FMM_OK;
 }
 

@@ -630,3 +630,50 @@ def test_second_right_hand_side_on_one_handle(env):
     L3, _ = f.solve(torch.from_numpy(w.moments).cuda(), com)
     assert torch.equal(L3, L1)
     f.close()
+
+
+def _mixed_level(seed, n, frac=0.5):
+    w = fi.config1(seed=seed, ncell=n)
+    sub = np.random.default_rng(seed).random((n // 8,) * 3) < frac
+    leaf = np.repeat(np.repeat(np.repeat(sub, 8, 0), 8, 1), 8, 2).astype(np.uint8)
+    w.moments[1:, leaf == 1] = 0.0                  # leaves are point masses at their cell centres
+    w.com_off[:, leaf == 1] = 0.0
+    return w, leaf
+
+
+@pytest.mark.parametrize("theta,correction,kernel", [(0.5, True, 0), (0.5, False, 1), (0.35, True, 2), (0.7, True, 0)])
+def test_mixed_level_of_an_adaptive_mesh(env, theta, correction, kernel):
+    """f3 (reading R8): a level whose sub-grids are leaves or refined; octo_fmm_interact_mixed adds the near-field
+    pairs in which A or B is a leaf to the Eq. 15 step.  Coefficients and the NUMBER of pairs against the oracle,
+    whole grid and a sub-region; the two uniform limits."""
+    p, torch = env
+    w, leaf = _mixed_level(41, 32)
+    mom, com = torch.from_numpy(w.moments).cuda(), torch.from_numpy(w.com_off).cuda()
+    lf = torch.from_numpy(leaf).cuda()
+    for lo, hi in (((0, 0, 0), (32, 32, 32)), ((8, 0, 16), (24, 16, 32))):
+        f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, correction, lo, hi if (lo, hi) != ((0, 0, 0), (32, 32, 32)) else (0, 0, 0))
+        f.set_option("kernel", kernel)
+        f.set_moments(mom, com)
+        f.interact_mixed(lf)
+        L, Lc = f.get_expansions()
+        torch.cuda.synchronize()
+        assert f.status() == p.OK
+        Lr, Lcr, cnt = oracle.interact_multipole_mixed(w.n, w.h, theta, w.moments, w.com_off, leaf, lo, hi, correction)
+        assert f.mixed_interaction_count() == cnt
+        check(L.cpu().numpy(), Lc.cpu().numpy(), Lr, Lcr if correction else None)
+        f.close()
+    # no leaf: the plain step, bit for bit; every cell a leaf: the near field is taken everywhere
+    f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, correction)
+    f.set_option("kernel", kernel)
+    plain, _ = f.solve(mom, com)
+    plain = plain.clone()
+    f.interact_mixed(torch.zeros_like(lf))
+    L, _ = f.get_expansions()
+    assert torch.equal(L, plain) and f.mixed_interaction_count() == f.interaction_count()
+    f.interact_mixed(torch.ones_like(lf))
+    torch.cuda.synchronize()
+    near = sum(len(oracle.stencil_leaf(theta, q)) - len(oracle.stencil(theta, q)) for q in range(8))
+    assert f.mixed_interaction_count() > f.interaction_count() and near > 0
+    with pytest.raises(p.OctoFmmError):
+        p.OctoFMM(w.n, w.h, theta, p.MONOPOLE).interact_mixed(lf)
+    f.close()
