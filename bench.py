@@ -510,6 +510,35 @@ def run_ours(args):
                         "nothing and are not evaluated; results agree with the general path to round-off"}
         f.set_option("dipole_terms", 1)
 
+    # ---- one level of an adaptive mesh (f3): half of the sub-grids are leaves (point masses), seeded; the near-field
+    #      pairs with a leaf on either side are taken at this level.  Measured beside the step, not part of `value`. ----
+    mixed = None
+    if multi and rank == 0 and w.n[0] % 8 == 0:
+        g = torch.Generator(device="cpu").manual_seed(args.seed)
+        sub = (torch.rand(tuple(v // 8 for v in w.n[::-1]), generator=g) < 0.5).to(dev)
+        leaf = sub.repeat_interleave(8, 0).repeat_interleave(8, 1).repeat_interleave(8, 2).to(torch.uint8).contiguous()
+        keep = (leaf == 0).to(torch.float64)
+        mom_m = mom.clone()
+        mom_m[1:] *= keep
+        com_m = com * keep
+        f.set_moments(mom_m, com_m)
+        f.interact_mixed(leaf)
+        torch.cuda.synchronize()
+        ma, mb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ma.record(stream)
+        for _ in range(3):
+            f.interact_mixed(leaf)
+        mb.record(stream)
+        torch.cuda.synchronize()
+        mixed_ms = ma.elapsed_time(mb) / 3
+        pairs = f.mixed_interaction_count()
+        mixed = {"leaf_fraction_of_subgrids": float(sub.double().mean()), "kernel_ms": mixed_ms, "interactions": pairs,
+                 "near_field_interactions": pairs - n_int, "interactions_per_s": pairs / (mixed_ms * 1e-3),
+                 "note": "octo_fmm_interact_mixed: Eq. 15 step + m2l_near_kernel (pairs that are not well separated and "
+                         "have a leaf on either side); timed beside the step, not part of value"}
+        del mom_m, com_m, leaf, keep
+        f.set_moments(mom, com)
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -566,6 +595,8 @@ def run_ours(args):
     if fast is not None:
         fast["frac_of_peak"] = fast["achieved_tflops"] / peak_tflops
         line["com_fast_path"] = fast
+    if mixed is not None:
+        line["mixed_level"] = mixed
     print(json.dumps(line))
     f.close()
     if world > 1:
