@@ -522,8 +522,10 @@ def run_ours(args):
         mom_m[1:] *= keep
         com_m = com * keep
         f.set_moments(mom_m, com_m)
+        f.set_option("mixed_count", 1)
         f.interact_mixed(leaf)
-        torch.cuda.synchronize()
+        pairs = f.mixed_interaction_count()
+        f.set_option("mixed_count", 0)
         ma, mb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ma.record(stream)
         for _ in range(3):
@@ -531,11 +533,11 @@ def run_ours(args):
         mb.record(stream)
         torch.cuda.synchronize()
         mixed_ms = ma.elapsed_time(mb) / 3
-        pairs = f.mixed_interaction_count()
         mixed = {"leaf_fraction_of_subgrids": float(sub.double().mean()), "kernel_ms": mixed_ms, "interactions": pairs,
                  "near_field_interactions": pairs - n_int, "interactions_per_s": pairs / (mixed_ms * 1e-3),
-                 "note": "octo_fmm_interact_mixed: Eq. 15 step + m2l_near_kernel (pairs that are not well separated and "
-                         "have a leaf on either side); timed beside the step, not part of value"}
+                 "note": "octo_fmm_interact_mixed: one pass of the slab-fed kernel over the Eq. 15 list + the near field (a pair "
+                         "that is not well separated counts if it has a leaf on either side); timed beside the step, not part "
+                         "of value"}
         del mom_m, com_m, leaf, keep
         f.set_moments(mom, com)
 

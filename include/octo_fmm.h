@@ -146,8 +146,9 @@ int octo_fmm_dipole_terms_used(octo_fmm_t *h, int *used);
  * octo_fmm_interact_mixed() = octo_fmm_interact() (the list of Eq. 15, whatever the cells' kind) + the near-field
  * pairs nobody below this level will take: a cell B that is NOT well separated from A (and whose parent is not well
  * separated from A's) interacts with A here if A or B is a leaf.  Same pair formula, same outputs (get_expansions).
- * MULTIPOLE handles; asynchronous on the stream.  octo_fmm_mixed_interaction_count() synchronises the stream and
- * returns the number of ordered pairs the last octo_fmm_interact_mixed() evaluated (it depends on leaf). */
+ * MULTIPOLE handles; asynchronous on the stream.  With octo_fmm_set_option(h, "mixed_count", 1) the call also counts
+ * the ordered pairs it evaluates (they depend on leaf); octo_fmm_mixed_interaction_count() then synchronises the stream
+ * and returns the number (ESTATE if the last octo_fmm_interact_mixed() did not count). */
 int octo_fmm_interact_mixed(octo_fmm_t *h, const unsigned char *leaf);
 int octo_fmm_mixed_interaction_count(octo_fmm_t *h, unsigned long long *n);
 
@@ -155,6 +156,7 @@ int octo_fmm_mixed_interaction_count(octo_fmm_t *h, unsigned long long *n);
  * cells), 1 direct (one cell per thread, global-memory loads; same pair arithmetic), 2 one warp per cell with
  * a warp-level reduction of the partial expansions (default up to 4096 target cells).
  * "dipole_terms" = 0 decided on the device (default), 1 always evaluated.
+ * "mixed_count" = 1: octo_fmm_interact_mixed also counts its pairs (default 0).
  * "am_correction" = 0 / 1 (MULTIPOLE handles): switches the correction of cfg.am_correction for the following
  * set_moments() + interact() (the handle goes back to the "created" state) -- one handle and one workspace can
  * so serve a second right-hand side on the same centres (d(rho)/dt, L81-83: no correction) after the first.

@@ -49,7 +49,7 @@ static_assert(STAGED_SMEM <= 227 * 1024, "shared memory per CTA");
 struct StEntry {
     int off;                 // shared-memory offset relative to the thread's base (multipole: double2 units in
                              // the slab; monopole: doubles in the mass tile)
-    signed char dx, dy, dz, d2;   // d2 = |Delta|^2 (monopole handles only)
+    signed char dx, dy, dz, d2;   // d2: monopole handles |Delta|^2; mixed-level lists 1 = near-field entry (not well separated)
 };
 
 // Stencil tables (the interaction lists of the 8 parity classes, Eq. 15) in constant memory.
@@ -79,6 +79,7 @@ struct Params {
     const double* pC;        // [3][...]   corrections carried beside the expansions
     const double* poff;      // [3][...]   expansion-centre offsets of the parent cells
     double hc;               // width of this level's cells
+    const unsigned char* leaf;   // mixed level (m2l_staged_kernel<., ., true>): [nz][ny][nx], 1 = leaf cell
 };
 
 // ------------------------------------------------------------------------------------------
@@ -113,6 +114,21 @@ __global__ void __launch_bounds__(256) stage_multipole_kernel(const double* __re
     double2* dst = reinterpret_cast<double2*>(S) + (long long)z * NPAIR * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1);
 #pragma unroll
     for (int c = 0; c < NPAIR; ++c) dst[(long long)c * plane] = make_double2(s[2 * c], s[2 * c + 1]);
+}
+
+// Mixed level (f3): the leaf flag of every cell into the padding slot (component 19) of its staged record, so that the
+// slab-fed kernel finds the flag of a partner next to its moments.
+__global__ void __launch_bounds__(256) stage_leaf_flags_kernel(const unsigned char* __restrict__ leaf, double* __restrict__ S,
+                                                               int nx, int ny, int nz)
+{
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= (long long)nx * ny * nz) return;
+    const int x = (int)(cell % nx);
+    const long long r = cell / nx;
+    const int y = (int)(r % ny), z = (int)(r / ny);
+    const long long plane = (long long)ny * nx;
+    double2* dst = reinterpret_cast<double2*>(S) + ((long long)z * NPAIR + (NPAIR - 1)) * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1);
+    dst->y = leaf[cell] ? 1.0 : 0.0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -203,6 +219,15 @@ __device__ __forceinline__ void decode_tile(const Params& p, long long t, int& x
         bx_ = v_[8].x; by_ = v_[8].y; bz_ = v_[9].x;                                       \
     }
 
+// the same, plus the record's padding slot (the partner's leaf flag on a mixed level)
+#define OCTO_LOAD_SOURCE_F(q, stride, src, bx_, by_, bz_, fl_)                            \
+    {                                                                                     \
+        double2 v_[NPAIR];                                                                \
+        _Pragma("unroll") for (int c_ = 0; c_ < NPAIR; ++c_) v_[c_] = (q)[(long long)c_ * (stride)]; \
+        _Pragma("unroll") for (int c_ = 0; c_ < 8; ++c_) { src[2 * c_] = v_[c_].x; src[2 * c_ + 1] = v_[c_].y; } \
+        bx_ = v_[8].x; by_ = v_[8].y; bz_ = v_[9].x; fl_ = v_[9].y;                       \
+    }
+
 // the target's own expansion centre and (for the correction) M3_A / M_A in staged form
 template <bool CORR>
 __device__ __forceinline__ void load_target(const Params& p, int gx, int gy, int k, double (&dA)[3], double (&tA)[7])
@@ -266,7 +291,10 @@ __device__ __forceinline__ void store_target(const Params& p, const Acc& acc, co
 
 // The consumer warps' loop over the bricks of this CTA.  DIPOLE = false is the fast path for sources
 // expanded about their centre of mass (no dipole terms), see m2l_staged_kernel.
-template <bool CORR, bool DIPOLE, bool FUSE_L2L>
+// MIXED (one level of an adaptive mesh, f3): the lists are the leaf-level lists (Eq. 15 + near field); a near-field entry
+// counts only if the target or the partner is a leaf cell -- otherwise the pair's 1/r is set to 0, and since every term of
+// the pair carries a power of 1/r it contributes exactly nothing.
+template <bool CORR, bool DIPOLE, bool FUSE_L2L, bool MIXED>
 __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, uint64_t* full, uint64_t* empty, int warp, int lane)
 {
     // ------------------------------ consumers ------------------------------
@@ -290,6 +318,8 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
 
         double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         if (active) load_target<CORR>(p, gx, gy, k, dA, tA);
+        bool leafA = false;
+        if (MIXED && active) leafA = p.leaf[((long long)k * p.ny + gy) * p.nx + gx] != 0;
 
         Acc acc;
         acc_zero(acc);
@@ -332,12 +362,14 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         {                                                                                   \
             const StEntry e_ = c_entries[s];                                                \
             ++s;                                                                            \
-            double bx_, by_, bz_;                                                           \
-            OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_);                \
+            double bx_, by_, bz_, fl_ = 0.0;                                                \
+            if (MIXED) { OCTO_LOAD_SOURCE_F(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
+            else       { OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_); }  \
             P.x = c_hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                                \
             P.y = c_hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                                \
             P.z = Rz0 - bz_;                                                                \
             P.w = pair_head(P.x, P.y, P.z);                                                 \
+            if (MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;                          \
         }
         struct Fetched { double src[16]; double x, y, z, w; } A, B;
         if (ensure()) {
@@ -358,7 +390,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
     }
 }
 
-template <bool CORR, bool FUSE_L2L = false>
+template <bool CORR, bool FUSE_L2L = false, bool MIXED = false>
 __global__ void __launch_bounds__(STAGED_THREADS, 1)
 m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
 {
@@ -405,8 +437,8 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
     // the flags if any cell has |M1_i| > DIPOLE_TOL |M| h, and only then (or when the caller forces it) the
     // 27 dipole terms are evaluated.  The branch is uniform over the grid.
     const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
-    if (dipole) staged_consume<CORR, true, FUSE_L2L>(p, slab0, full, empty, warp, lane);
-    else        staged_consume<CORR, false, FUSE_L2L>(p, slab0, full, empty, warp, lane);
+    if (dipole) staged_consume<CORR, true, FUSE_L2L, MIXED>(p, slab0, full, empty, warp, lane);
+    else        staged_consume<CORR, false, FUSE_L2L, MIXED>(p, slab0, full, empty, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------

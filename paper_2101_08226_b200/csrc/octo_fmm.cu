@@ -241,6 +241,11 @@ struct octo_fmm {
     std::vector<Offset3> list[8];
     std::vector<StEntry> entries;          // 8 * MAX_LIST
     std::vector<char4> near_list;          // 8 * MAX_NEAR: the near field of each parity class (mixed levels, f3)
+    std::vector<StEntry> entries_mixed;    // 8 * MAX_LIST: Eq. 15 list + near field (d2 = 1 marks a near-field entry), staged kernel
+    int begin_mixed[8][2 * REACH_MAX + 2];
+    unsigned long long list_sig_mixed;
+    int mixed_count;       // 1: interact_mixed also counts its pairs (option "mixed_count")
+    bool mixed_counted;    // the last interact_mixed did
     int near_count[8];
     int begin[8][2 * REACH_MAX + 2];
     double hmul[2 * REACH_MAX + 1];
@@ -320,6 +325,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->kernel = 0;
     h->mono_kernel = 0;
     h->mixed = false;
+    h->mixed_count = 0;
+    h->mixed_counted = false;
     h->host_chunk = 12;
     h->host_launches = 0;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
@@ -350,6 +357,25 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
             h->near_list[(size_t)p * MAX_NEAR + n++] = char4{o.d[0], o.d[1], o.d[2], 0};
         }
         h->near_count[p] = n;
+        // the same list for the slab-fed kernel: (dz, dy, dx) order, shared-memory offsets, near-field entries marked
+        if (cfg->kind == OCTO_FMM_MULTIPOLE) {
+            if (p == 0) h->entries_mixed.assign((size_t)8 * MAX_LIST, StEntry{0, 0, 0, 0, 0});
+            if ((int)full.size() > MAX_LIST || r > REACH_MAX) { delete h; return OCTO_FMM_EINVAL; }
+            const int px = p & 1, py = (p >> 1) & 1;
+            int cur = 0;
+            for (int dz = -REACH_MAX; dz <= REACH_MAX + 1; ++dz) {
+                while (cur < (int)full.size() && full[cur].d[2] < dz) ++cur;
+                h->begin_mixed[p][dz + REACH_MAX] = cur;
+            }
+            for (size_t s2 = 0; s2 < full.size(); ++s2) {
+                const int dx = full[s2].d[0], dy = full[s2].d[1], dz = full[s2].d[2];
+                StEntry e;
+                e.off = (py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1);
+                e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz;
+                e.d2 = well_separated((long long)dx * dx + (long long)dy * dy + (long long)dz * dz, cfg->theta) ? 0 : 1;
+                h->entries_mixed[(size_t)p * MAX_LIST + s2] = e;
+            }
+        }
     }
 
     h->entries.assign((size_t)8 * MAX_LIST, StEntry{0, 0, 0, 0, 0});
@@ -387,6 +413,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         h->list_sig = (tb * 0x9E3779B97F4A7C15ull) ^ ((unsigned long long)(cfg->kind + 1) << 8) ^ ((unsigned long long)((flags & CF_LEAF_LIST) ? 2 : 1) << 4) ^
                       (unsigned long long)(cfg->device + 1);
         if (h->list_sig == 0) h->list_sig = 1;
+        h->list_sig_mixed = h->list_sig ^ 0x5bd1e995ull;
+        if (h->list_sig_mixed == 0) h->list_sig_mixed = 2;
     }
 
     // ---- interaction count: per-axis closed form over the lists (out-of-grid partners skipped) ----
@@ -430,6 +458,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.S = h->src; P.L = h->L; P.C = h->C; P.flags = h->flags;
     P.force_dipole = 0;
     P.pL = nullptr; P.pC = nullptr; P.poff = nullptr; P.hc = cfg->h;
+    P.leaf = nullptr;
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
         // ---- TMA descriptor of S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
@@ -450,7 +479,11 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e3 = cudaFuncSetAttribute(m2l_staged_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e4 = cudaFuncSetAttribute(m2l_staged_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
-        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) { delete h; return OCTO_FMM_ECUDA; }
+        cudaError_t e5 = cudaFuncSetAttribute(m2l_staged_kernel<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        cudaError_t e6 = cudaFuncSetAttribute(m2l_staged_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess || e5 != cudaSuccess || e6 != cudaSuccess) {
+            delete h; return OCTO_FMM_ECUDA;
+        }
     } else if (cfg->kind == OCTO_FMM_MONOPOLE) {
         // ---- monopole weights of the 11^3 offsets: (-1/|R|, -R/|R|^3) with R = (i_A - i_B) h = -Delta h, in FP64
         //      on the host (sqrt, division); Delta = 0 gets zero weights ----
@@ -525,21 +558,24 @@ int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com
     return OCTO_FMM_OK;
 }
 
-static int upload_tables(octo_fmm_t* h)
+static int upload_tables(octo_fmm_t* h, bool mixed = false)
 {
-    if (g_const_owner == h) return OCTO_FMM_OK;
+    const unsigned long long sig = mixed ? h->list_sig_mixed : h->list_sig;
+    if (g_const_owner == h && g_list_sig == sig) return OCTO_FMM_OK;
     // the lists depend on (theta, kind, list flavour) only: the levels of a complete solve share them and differ in h
-    if (g_list_sig != h->list_sig) {
-        if (cudaMemcpyToSymbolAsync(c_entries, h->entries.data(), h->entries.size() * sizeof(StEntry), 0,
+    if (g_list_sig != sig) {
+        const StEntry* ent = mixed ? h->entries_mixed.data() : h->entries.data();
+        const void* beg = mixed ? (const void*)h->begin_mixed : (const void*)h->begin;
+        if (cudaMemcpyToSymbolAsync(c_entries, ent, (size_t)8 * MAX_LIST * sizeof(StEntry), 0,
                                     cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
-        if (cudaMemcpyToSymbolAsync(c_begin, h->begin, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+        if (cudaMemcpyToSymbolAsync(c_begin, beg, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
             return OCTO_FMM_ECUDA;
         if (cudaMemcpyToSymbolAsync(c_near, h->near_list.data(), h->near_list.size() * sizeof(char4), 0, cudaMemcpyHostToDevice,
                                     h->stream) != cudaSuccess ||
             cudaMemcpyToSymbolAsync(c_near_count, h->near_count, sizeof(h->near_count), 0, cudaMemcpyHostToDevice, h->stream) !=
                 cudaSuccess)
             return OCTO_FMM_ECUDA;
-        g_list_sig = h->list_sig;
+        g_list_sig = sig;
     }
     if (cudaMemcpyToSymbolAsync(c_hmul, h->hmul, sizeof(h->hmul), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
@@ -548,7 +584,7 @@ static int upload_tables(octo_fmm_t* h)
 }
 
 // launch the staged interaction kernel for the z-layers [kb, ke) of the output region
-static int launch_staged(octo_fmm_t* h, int kb, int ke)
+static int launch_staged(octo_fmm_t* h, int kb, int ke, bool mixed = false)
 {
     Params P = h->prm;
     P.L = h->outL; P.C = h->outC;
@@ -556,7 +592,10 @@ static int launch_staged(octo_fmm_t* h, int kb, int ke)
     P.tiles_z = (ke - kb + TILE_Z - 1) / TILE_Z;
     P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
     const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
-    if (P.pL) {            // complete solve: L2L fused into the epilogue (solver.inl sets the parent arrays)
+    if (mixed) {           // one level of an adaptive mesh: leaf-level lists, near-field entries conditional on the leaf flags
+        if (h->cfg.am_correction) m2l_staged_kernel<true, false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        else                      m2l_staged_kernel<false, false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    } else if (P.pL) {     // complete solve: L2L fused into the epilogue (solver.inl sets the parent arrays)
         if (h->cfg.am_correction) m2l_staged_kernel<true, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
         else                      m2l_staged_kernel<false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
     } else {
@@ -610,26 +649,74 @@ int octo_fmm_interact(octo_fmm_t* h)
     return OCTO_FMM_OK;
 }
 
+// number of near-field pairs with a leaf on either side (for the bit-exact check of the pair set)
+__global__ void __launch_bounds__(256) count_near_kernel(const Params p, const unsigned char* __restrict__ leaf,
+                                                         unsigned long long* __restrict__ count)
+{
+    const long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long taken = 0;
+    if (o < (long long)p.ox * p.oy * p.oz) {
+        const int gx = p.lo[0] + (int)(o % p.ox), gy = p.lo[1] + (int)((o / p.ox) % p.oy), k = p.lo[2] + (int)(o / ((long long)p.ox * p.oy));
+        const int cls = (gx & 1) + 2 * (gy & 1) + 4 * (k & 1);
+        const long long plane = (long long)p.ny * p.nx;
+        const bool leafA = leaf[(long long)k * plane + (long long)gy * p.nx + gx] != 0;
+        for (int s = 0; s < c_near_count[cls]; ++s) {
+            const char4 e = c_near[cls][s];
+            const int sx = gx + e.x, sy = gy + e.y, sz = k + e.z;
+            if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
+            if (leafA || leaf[(long long)sz * plane + (long long)sy * p.nx + sx] != 0) ++taken;
+        }
+    }
+    for (int d = 16; d > 0; d >>= 1) taken += __shfl_xor_sync(0xffffffffu, taken, d);
+    if ((threadIdx.x & 31) == 0 && taken) atomicAdd(count, taken);
+}
+
 int octo_fmm_interact_mixed(octo_fmm_t* h, const unsigned char* leaf)
 {
     if (!h || !leaf || h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
-    const int rc = octo_fmm_interact(h);                       // the Eq. 15 part, whatever the cells' kind
-    if (rc != OCTO_FMM_OK) return rc;
-    unsigned long long* cnt = reinterpret_cast<unsigned long long*>(h->flags + 2);
-    if (cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
-    Params P = h->prm;
-    P.L = h->outL; P.C = h->outC;
-    if (h->cfg.am_correction) m2l_near_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, cnt);
-    else                      m2l_near_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, cnt);
-    if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (h->state < 1) return OCTO_FMM_ESTATE;
+    if (h->kernel == 0) {
+        // slab-fed kernel: one pass over the leaf-level lists; the partner's leaf flag travels in the padding slot of its record
+        if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (upload_tables(h, true) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+        if (cudaMemsetAsync(h->flags, 0, sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+        Params& P = h->prm;
+        const long long ncell = (long long)P.nx * P.ny * P.nz;
+        stage_leaf_flags_kernel<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(leaf, h->src, P.nx, P.ny, P.nz);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        P.leaf = leaf;
+        const int rc = launch_staged(h, h->lo[2], h->hi[2], true);
+        P.leaf = nullptr;
+        if (rc != OCTO_FMM_OK) return rc;
+        h->state = 2;
+        h->resL = h->outL; h->resC = h->outC;
+    } else {
+        const int rc = octo_fmm_interact(h);                   // the Eq. 15 part, whatever the cells' kind
+        if (rc != OCTO_FMM_OK) return rc;
+        Params P = h->prm;
+        P.L = h->outL; P.C = h->outC;
+        if (h->cfg.am_correction) m2l_near_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, nullptr);
+        else                      m2l_near_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, nullptr);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
     h->mixed = true;
+    h->mixed_counted = false;
+    if (h->mixed_count) {
+        unsigned long long* cnt = reinterpret_cast<unsigned long long*>(h->flags + 2);
+        if (cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+        const Params& P = h->prm;
+        const long long ocell = (long long)P.ox * P.oy * P.oz;
+        count_near_kernel<<<(unsigned)((ocell + 255) / 256), 256, 0, h->stream>>>(P, leaf, cnt);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        h->mixed_counted = true;
+    }
     return OCTO_FMM_OK;
 }
 
 int octo_fmm_mixed_interaction_count(octo_fmm_t* h, unsigned long long* n)
 {
     if (!h || !n) return OCTO_FMM_EINVAL;
-    if (h->state < 2 || !h->mixed) return OCTO_FMM_ESTATE;
+    if (h->state < 2 || !h->mixed || !h->mixed_counted) return OCTO_FMM_ESTATE;
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     unsigned long long near = 0;
     if (cudaMemcpy(&near, h->flags + 2, sizeof near, cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
@@ -900,6 +987,11 @@ int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)
     if (!std::strcmp(key, "mono_kernel")) {      // monopole handles: 0 = FP64 tensor-core instruction (default), 1 = DFMA
         if (h->cfg.kind != OCTO_FMM_MONOPOLE || (value != 0 && value != 1)) return OCTO_FMM_EINVAL;
         h->mono_kernel = value;
+        return OCTO_FMM_OK;
+    }
+    if (!std::strcmp(key, "mixed_count")) {      // 1: octo_fmm_interact_mixed also counts the pairs it evaluates
+        if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
+        h->mixed_count = value;
         return OCTO_FMM_OK;
     }
     if (!std::strcmp(key, "am_correction")) {    // multipole handles: switch the correction for the next set_moments() + interact()

@@ -653,6 +653,7 @@ def test_mixed_level_of_an_adaptive_mesh(env, theta, correction, kernel):
     for lo, hi in (((0, 0, 0), (32, 32, 32)), ((8, 0, 16), (24, 16, 32))):
         f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, correction, lo, hi if (lo, hi) != ((0, 0, 0), (32, 32, 32)) else (0, 0, 0))
         f.set_option("kernel", kernel)
+        f.set_option("mixed_count", 1)
         f.set_moments(mom, com)
         f.interact_mixed(lf)
         L, Lc = f.get_expansions()
@@ -665,6 +666,7 @@ def test_mixed_level_of_an_adaptive_mesh(env, theta, correction, kernel):
     # no leaf: the plain step, bit for bit; every cell a leaf: the near field is taken everywhere
     f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, correction)
     f.set_option("kernel", kernel)
+    f.set_option("mixed_count", 1)
     plain, _ = f.solve(mom, com)
     plain = plain.clone()
     f.interact_mixed(torch.zeros_like(lf))
