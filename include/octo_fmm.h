@@ -30,8 +30,13 @@
  * workspace) and never synchronises the stream except in octo_fmm_destroy and
  * octo_fmm_status.  All work is enqueued on cfg.stream (a cudaStream_t).  Inputs may be reused
  * by the caller once the stream has passed set_moments; outputs are complete once the stream
- * has passed get_expansions.  A handle is not thread-safe.  Handles that share a device share
- * the stencil table in constant memory: use them on one stream (or serialise them).
+ * has passed get_expansions.  One handle is not thread-safe; DIFFERENT handles may be driven from
+ * different streams and host threads at the same time.  Everything that depends on a handle's cell
+ * width travels with its launches; the interaction lists (a function of theta and kind only) are
+ * kept in one constant-memory bank per device, and the library orders an upload of other lists
+ * against the kernels of other streams that still read the previous ones (events, no host
+ * synchronisation): handles with the same theta and kind share the bank and run concurrently,
+ * handles with different lists are serialised on the device.
  *
  * Errors: every call returns an OCTO_FMM_* status; nothing throws or aborts.
  * There is no CPU fallback: without a usable CUDA device create() fails with OCTO_FMM_ECUDA.

@@ -108,12 +108,37 @@ _vp = ctypes.c_void_p
 
 
 def _ptr(t):
-    """Device/host address of a torch tensor or numpy array (or None)."""
+    """Device/host address of a torch tensor or numpy array (or None).  The C ABI takes plain pointers to dense
+    arrays, so anything that is not contiguous is refused here instead of being read out of bounds there."""
     if t is None:
         return None
     if hasattr(t, "data_ptr"):
+        if not t.is_contiguous():
+            raise ValueError("octo_fmm: tensors must be contiguous")
         return t.data_ptr()
+    if not t.flags["C_CONTIGUOUS"]:
+        raise ValueError("octo_fmm: arrays must be C-contiguous")
     return t.ctypes.data
+
+
+def _check_device_tensor(t, name, dtype, numel, device, stream=None):
+    """Argument check of the convenience classes: a CUDA tensor of the handle's device, of the exact dtype and element
+    count the C ABI will read or write.  `stream`: the handle's stream; a tensor allocated on another stream is tied to
+    it (record_stream) so that the caching allocator does not hand its memory out while the library still uses it."""
+    if t is None:
+        return
+    if not hasattr(t, "is_cuda") or not t.is_cuda:
+        raise ValueError("octo_fmm: %s must be a CUDA tensor (there is no CPU path)" % name)
+    if t.device != device:
+        raise ValueError("octo_fmm: %s is on %s, the handle on %s" % (name, t.device, device))
+    if t.dtype != dtype:
+        raise ValueError("octo_fmm: %s must be %s, got %s" % (name, dtype, t.dtype))
+    if not t.is_contiguous():
+        raise ValueError("octo_fmm: %s must be contiguous" % name)
+    if t.numel() != numel:
+        raise ValueError("octo_fmm: %s has %d elements, expected %d" % (name, t.numel(), numel))
+    if stream is not None:
+        t.record_stream(stream)
 
 
 def make_config(n, h, theta, kind=MULTIPOLE, am_correction=True, out_lo=(0, 0, 0), out_hi=(0, 0, 0),
@@ -404,9 +429,14 @@ class OctoFMMSolver:
         self.cfg = cfg
         self.handle = octo_fmm_solver_create(cfg)
 
+    def _check(self, t, name, numel):
+        _check_device_tensor(t, name, self.torch.float64, numel, self.device, self.stream)
+
     def solve(self, mass, out=None):
         if out is None:
             out = self.torch.empty((4, self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
+        self._check(mass, "mass", self.n ** 3)
+        self._check(out, "out", 4 * self.n ** 3)
         octo_fmm_solver_solve(self.handle, mass, out)
         return out
 
@@ -414,6 +444,8 @@ class OctoFMMSolver:
         """d(phi)/dt [n][n][n] of the sources dmass on the tree and centres of the last solve()."""
         if out is None:
             out = self.torch.empty((self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
+        self._check(dmass, "dmass", self.n ** 3)
+        self._check(out, "out", self.n ** 3)
         octo_fmm_solver_solve_rhs2(self.handle, dmass, out)
         return out
 
@@ -476,7 +508,20 @@ class OctoFMM:
         o = [self.out_hi[a] - self.out_lo[a] for a in range(3)]
         return (o[2], o[1], o[0])
 
+    def _ncell(self):
+        return self.n[0] * self.n[1] * self.n[2]
+
+    def _ocell(self):
+        o = self.out_shape
+        return o[0] * o[1] * o[2]
+
+    def _check(self, t, name, numel, dtype=None):
+        _check_device_tensor(t, name, dtype or self.torch.float64, numel, self.device, self.stream)
+
     def set_moments(self, moments, com_off=None):
+        self._check(moments, "moments", (20 if self.kind == MULTIPOLE else 1) * self._ncell())
+        if self.kind == MULTIPOLE:
+            self._check(com_off, "com_off", 3 * self._ncell())
         octo_fmm_set_moments(self.handle, moments, com_off)
 
     def interact(self):
@@ -484,6 +529,7 @@ class OctoFMM:
 
     def interact_mixed(self, leaf):
         """One level of an adaptive mesh: leaf = uint8 [nz][ny][nx] on the device, 1 where the cell is a leaf."""
+        self._check(leaf, "leaf", self._ncell(), self.torch.uint8)
         octo_fmm_interact_mixed(self.handle, leaf)
 
     def mixed_interaction_count(self):
@@ -496,11 +542,15 @@ class OctoFMM:
             L = torch.empty((ncoef,) + self.out_shape, dtype=torch.float64, device=self.device)
         if Lcorr is None and want_corr and self.kind == MULTIPOLE:
             Lcorr = torch.empty((3,) + self.out_shape, dtype=torch.float64, device=self.device)
+        self._check(L, "L", ncoef * self._ocell())
+        self._check(Lcorr, "Lcorr", 3 * self._ocell())
         octo_fmm_get_expansions(self.handle, L, Lcorr)
         return L, Lcorr
 
     def bind_outputs(self, L, Lcorr=None):
         """interact() then writes straight into L / Lcorr (kept alive here); None unbinds."""
+        self._check(L, "L", (20 if self.kind == MULTIPOLE else 4) * self._ocell())
+        self._check(Lcorr, "Lcorr", 3 * self._ocell())
         self._bound = (L, Lcorr)
         octo_fmm_bind_outputs(self.handle, L, Lcorr)
 

@@ -52,10 +52,12 @@ struct StEntry {
     signed char dx, dy, dz, d2;   // d2: monopole handles |Delta|^2; mixed-level lists 1 = near-field entry (not well separated)
 };
 
-// Stencil tables (the interaction lists of the 8 parity classes, Eq. 15) in constant memory.
+// Stencil tables (the interaction lists of the 8 parity classes, Eq. 15) in constant memory.  They depend on
+// (theta, kind, list flavour) only and are shared by every handle of a device that uses the same lists; octo_fmm.cu
+// (ConstBank) orders uploads against the kernels of other streams that still read the previous contents.  Everything
+// that depends on a handle's cell width h travels in Params (kernel-parameter space), not here.
 __constant__ StEntry c_entries[8 * MAX_LIST];
 __constant__ int c_begin[8][2 * REACH_MAX + 2];   // first entry of (class, dz); [..][11] = end
-__constant__ double c_hmul[2 * REACH_MAX + 1];    // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h)
 constexpr int MAX_NEAR = 96;                      // near field (cells that are NOT well separated): <= 92 for 1/3 < theta
 __constant__ char4 c_near[8][MAX_NEAR];           // (dx, dy, dz, 0) of the near-field cells of each parity class
 __constant__ int c_near_count[8];
@@ -80,6 +82,7 @@ struct Params {
     const double* poff;      // [3][...]   expansion-centre offsets of the parent cells
     double hc;               // width of this level's cells
     const unsigned char* leaf;   // mixed level (m2l_staged_kernel<., ., true>): [nz][ny][nx], 1 = leaf cell
+    double hmul[2 * REACH_MAX + 1];   // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h), per handle
 };
 
 // ------------------------------------------------------------------------------------------
@@ -351,7 +354,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
                 const int dz = zz - k;
                 if (layer_on && dz >= -p.reach && dz <= p.reach) {
                     sl = slab0 + (size_t)b * SLAB_ELEMS + tbase;
-                    Rz0 = c_hmul[dz + REACH_MAX] + dA[2];
+                    Rz0 = p.hmul[dz + REACH_MAX] + dA[2];
                     s = cls * MAX_LIST + c_begin[cls][dz + REACH_MAX];
                     s_end = cls * MAX_LIST + c_begin[cls][dz + REACH_MAX + 1];
                 }
@@ -365,8 +368,8 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
             double bx_, by_, bz_, fl_ = 0.0;                                                \
             if (MIXED) { OCTO_LOAD_SOURCE_F(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
             else       { OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_); }  \
-            P.x = c_hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                                \
-            P.y = c_hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                                \
+            P.x = p.hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                                \
+            P.y = p.hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                                \
             P.z = Rz0 - bz_;                                                                \
             P.w = pair_head(P.x, P.y, P.z);                                                 \
             if (MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;                          \
@@ -392,7 +395,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
 
 template <bool CORR, bool FUSE_L2L = false, bool MIXED = false>
 __global__ void __launch_bounds__(STAGED_THREADS, 1)
-m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
+m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ Params p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* slab0 = reinterpret_cast<double2*>(smem_raw);
@@ -447,7 +450,7 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const Params p)
 // Block = 256 threads = the 8 parity classes x 32 cells of a 16 x 8 x 2 brick, two passes in z.
 // ------------------------------------------------------------------------------------------
 template <bool CORR>
-__global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
+__global__ void __launch_bounds__(256) m2l_direct_kernel(const __grid_constant__ Params p)
 {
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
@@ -476,9 +479,9 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
             const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
             double src[16], bx_, by_, bz_;
             OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
-            const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
-            const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by_);
-            const double z = c_hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+            const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
+            const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
+            const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
             if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
             else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
         }
@@ -495,7 +498,7 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const Params p)
 // count (may be null): number of pairs taken, for the bit-exact check of the pair set.
 // ------------------------------------------------------------------------------------------
 template <bool CORR>
-__global__ void __launch_bounds__(256) m2l_near_kernel(const Params p, const unsigned char* __restrict__ leaf,
+__global__ void __launch_bounds__(256) m2l_near_kernel(const __grid_constant__ Params p, const unsigned char* __restrict__ leaf,
                                                        unsigned long long* __restrict__ count)
 {
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
@@ -509,6 +512,7 @@ __global__ void __launch_bounds__(256) m2l_near_kernel(const Params p, const uns
     const double2* S2 = reinterpret_cast<const double2*>(p.S);
     const int cls = warp;
     const long long ocell = (long long)p.ox * p.oy * p.oz;
+    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);   // as the interaction kernels
     unsigned long long taken = 0;
     for (int pass = 0; pass < 2; ++pass) {
         const int k = z0 + pz + 2 * pass;
@@ -529,10 +533,11 @@ __global__ void __launch_bounds__(256) m2l_near_kernel(const Params p, const uns
             const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
             double src[16], bx_, by_, bz_;
             OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
-            const double x = c_hmul[e.x + REACH_MAX] + (dA[0] - bx_);
-            const double y = c_hmul[e.y + REACH_MAX] + (dA[1] - by_);
-            const double z = c_hmul[e.z + REACH_MAX] + (dA[2] - bz_);
-            m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
+            const double x = p.hmul[e.x + REACH_MAX] + (dA[0] - bx_);
+            const double y = p.hmul[e.y + REACH_MAX] + (dA[1] - by_);
+            const double z = p.hmul[e.z + REACH_MAX] + (dA[2] - bz_);
+            if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
+            else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
             any = true;
             ++taken;
         }
@@ -562,7 +567,7 @@ __global__ void __launch_bounds__(256) m2l_near_kernel(const Params p, const uns
 // ~10 us.  Sources are read from the staged array in global memory with explicit in-grid tests.
 // ------------------------------------------------------------------------------------------
 template <bool CORR>
-__global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
+__global__ void __launch_bounds__(256) m2l_warp_kernel(const __grid_constant__ Params p)
 {
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
@@ -586,9 +591,9 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const Params p)
         const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
         double src[16], bx_, by_, bz_;
         OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
-        const double x = c_hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
-        const double y = c_hmul[e.dy + REACH_MAX] + (dA[1] - by_);
-        const double z = c_hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+        const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
+        const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
+        const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
         if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
         else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
     }

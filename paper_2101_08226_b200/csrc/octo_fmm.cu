@@ -10,7 +10,9 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "../../include/octo_fmm.h"
@@ -229,8 +231,22 @@ void dmma_rows(const std::vector<Offset3> (&list)[8], int which, DmmaRow (&rows)
     }
 }
 
-const void* g_const_owner = nullptr;   // handle whose tables are in constant memory
-unsigned long long g_list_sig = 0;     // signature (theta, kind, list flavour, device) of the lists in constant memory
+// The interaction lists live in ONE __constant__ bank per device (kernels.cuh: c_entries, c_begin, c_near): they depend
+// on (theta, kind, list flavour) only, so the levels of a complete solve and every handle with the same theta share them
+// and nothing is uploaded in the steady state.  Handles with DIFFERENT lists may be driven from different streams and
+// host threads; the bank serialises them: a host mutex guards the book-keeping, every kernel that reads the bank leaves
+// an event on its stream, and an upload first makes its stream wait for the readers of the previous contents on other
+// streams (and a reader on another stream waits for the upload).  Everything that depends on a handle's h is in Params.
+constexpr int MAX_DEVICES = 64;
+struct ConstBank {
+    std::mutex mu;
+    unsigned long long sig = 0;                               // lists in (or on their way into) the bank
+    cudaStream_t up_stream = nullptr;                         // stream the current contents were uploaded on
+    cudaEvent_t uploaded = nullptr;                           // recorded after that upload
+    std::vector<std::pair<cudaStream_t, cudaEvent_t>> readers;   // last reading kernel of every stream since the upload
+    std::vector<cudaEvent_t> pool;                            // spare events
+};
+ConstBank g_bank[MAX_DEVICES];
 
 }  // namespace
 
@@ -272,9 +288,10 @@ struct octo_fmm {
     int sm_count;
     cudaStream_t stream;
     // run_host pipeline (created on first use)
-    unsigned long long list_sig;   // identifies the contents of entries/begin (see upload_tables)
+    unsigned long long list_sig;   // identifies the contents of entries/begin (see bank_acquire)
     int host_chunk;        // output z-layers per pipeline slab; 0 = no pipelining
     int host_launches;     // kernels the last run_host launched
+    bool pipeline_ready;   // the side streams and events below all exist
     cudaStream_t s_h2d, s_d2h;
     cudaEvent_t ev_in[32], ev_out[32], ev_begin, ev_end;
 };
@@ -310,7 +327,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     if (!cfg->workspace || cfg->workspace_bytes < sz.total || ((uintptr_t)cfg->workspace % ALIGN)) return OCTO_FMM_EINVAL;
 
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) return OCTO_FMM_ECUDA;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev || cfg->device >= MAX_DEVICES) return OCTO_FMM_ECUDA;
     if (cudaSetDevice(cfg->device) != cudaSuccess) return OCTO_FMM_ECUDA;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cfg->device) != cudaSuccess) return OCTO_FMM_ECUDA;
@@ -329,7 +346,10 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->mixed_counted = false;
     h->host_chunk = 12;
     h->host_launches = 0;
+    h->pipeline_ready = false;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
+    for (int i = 0; i < MAX_CHUNKS; ++i) { h->ev_in[i] = nullptr; h->ev_out[i] = nullptr; }
+    h->ev_begin = nullptr; h->ev_end = nullptr;
     region_of(*cfg, h->lo, h->hi, flags);
     const bool small = cfg->n[0] % 8 || cfg->n[1] % 8 || cfg->n[2] % 8;    // only with CF_ANY_SIZE
     if (small) h->kernel = 1;
@@ -459,6 +479,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.force_dipole = 0;
     P.pL = nullptr; P.pC = nullptr; P.poff = nullptr; P.hc = cfg->h;
     P.leaf = nullptr;
+    for (int d = 0; d <= 2 * REACH_MAX; ++d) P.hmul[d] = h->hmul[d];
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
         // ---- TMA descriptor of S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
@@ -558,30 +579,63 @@ int octo_fmm_set_moments(octo_fmm_t* h, const double* moments, const double* com
     return OCTO_FMM_OK;
 }
 
-static int upload_tables(octo_fmm_t* h, bool mixed = false)
+// Make the lists of h current in the device's constant bank for a kernel about to be launched on h->stream, then
+// (bank_reader_done) note that kernel as a reader.  The caller holds BankLock from before bank_acquire until after
+// bank_reader_done, so that no other host thread can slip an upload between the two.
+struct BankLock {
+    std::unique_lock<std::mutex> lk;
+    explicit BankLock(const octo_fmm_t* h);
+};
+
+static int bank_acquire(octo_fmm_t* h, bool mixed = false)
 {
+    ConstBank& b = g_bank[h->cfg.device];
     const unsigned long long sig = mixed ? h->list_sig_mixed : h->list_sig;
-    if (g_const_owner == h && g_list_sig == sig) return OCTO_FMM_OK;
-    // the lists depend on (theta, kind, list flavour) only: the levels of a complete solve share them and differ in h
-    if (g_list_sig != sig) {
-        const StEntry* ent = mixed ? h->entries_mixed.data() : h->entries.data();
-        const void* beg = mixed ? (const void*)h->begin_mixed : (const void*)h->begin;
-        if (cudaMemcpyToSymbolAsync(c_entries, ent, (size_t)8 * MAX_LIST * sizeof(StEntry), 0,
-                                    cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
-        if (cudaMemcpyToSymbolAsync(c_begin, beg, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
-            return OCTO_FMM_ECUDA;
-        if (cudaMemcpyToSymbolAsync(c_near, h->near_list.data(), h->near_list.size() * sizeof(char4), 0, cudaMemcpyHostToDevice,
-                                    h->stream) != cudaSuccess ||
-            cudaMemcpyToSymbolAsync(c_near_count, h->near_count, sizeof(h->near_count), 0, cudaMemcpyHostToDevice, h->stream) !=
-                cudaSuccess)
-            return OCTO_FMM_ECUDA;
-        g_list_sig = sig;
+    if (b.sig == sig) {
+        // same lists; if they were uploaded on another stream, this stream has to see the upload complete
+        if (b.up_stream != h->stream && b.uploaded && cudaStreamWaitEvent(h->stream, b.uploaded, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+        return OCTO_FMM_OK;
     }
-    if (cudaMemcpyToSymbolAsync(c_hmul, h->hmul, sizeof(h->hmul), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
+    // other lists: wait for every kernel on OTHER streams that still reads the old contents (same-stream readers are
+    // ordered before the upload by the stream itself)
+    for (auto& r : b.readers) {
+        if (r.first != h->stream && cudaStreamWaitEvent(h->stream, r.second, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+        b.pool.push_back(r.second);
+    }
+    b.readers.clear();
+    const StEntry* ent = mixed ? h->entries_mixed.data() : h->entries.data();
+    const void* beg = mixed ? (const void*)h->begin_mixed : (const void*)h->begin;
+    b.sig = 0;                                        // nothing valid until every piece is on its way
+    if (cudaMemcpyToSymbolAsync(c_entries, ent, (size_t)8 * MAX_LIST * sizeof(StEntry), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
+        cudaMemcpyToSymbolAsync(c_begin, beg, sizeof(h->begin), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
+        cudaMemcpyToSymbolAsync(c_near, h->near_list.data(), h->near_list.size() * sizeof(char4), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess ||
+        cudaMemcpyToSymbolAsync(c_near_count, h->near_count, sizeof(h->near_count), 0, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
         return OCTO_FMM_ECUDA;
-    g_const_owner = h;
+    if (!b.uploaded && cudaEventCreateWithFlags(&b.uploaded, cudaEventDisableTiming) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (cudaEventRecord(b.uploaded, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    b.up_stream = h->stream;
+    b.sig = sig;
     return OCTO_FMM_OK;
 }
+
+static int bank_reader_done(octo_fmm_t* h)
+{
+    ConstBank& b = g_bank[h->cfg.device];
+    for (auto& r : b.readers)
+        if (r.first == h->stream) return cudaEventRecord(r.second, h->stream) == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
+    cudaEvent_t ev = nullptr;
+    if (!b.pool.empty()) { ev = b.pool.back(); b.pool.pop_back(); }
+    else if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (cudaEventRecord(ev, h->stream) != cudaSuccess) { b.pool.push_back(ev); return OCTO_FMM_ECUDA; }
+    b.readers.emplace_back(h->stream, ev);
+    return OCTO_FMM_OK;
+}
+
+BankLock::BankLock(const octo_fmm_t* h) : lk(g_bank[h->cfg.device].mu) {}
+
+// true if the kernel interact() launches for this handle reads the constant bank (the tensor-core monopole kernels read
+// only their own tables in the workspace)
+static bool reads_bank(const octo_fmm_t* h) { return h->cfg.kind == OCTO_FMM_MULTIPOLE || h->mono_kernel != 0; }
 
 // launch the staged interaction kernel for the z-layers [kb, ke) of the output region
 static int launch_staged(octo_fmm_t* h, int kb, int ke, bool mixed = false)
@@ -621,7 +675,10 @@ int octo_fmm_interact(octo_fmm_t* h)
     if (!h) return OCTO_FMM_EINVAL;
     if (h->state < 1) return OCTO_FMM_ESTATE;
     if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
-    if (upload_tables(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    const bool bank = reads_bank(h);
+    BankLock guard(h);
+    if (!bank) guard.lk.unlock();
+    else if (bank_acquire(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     if (cudaMemsetAsync(h->flags, 0, sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
@@ -643,6 +700,7 @@ int octo_fmm_interact(octo_fmm_t* h)
         if (launch_staged(h, h->lo[2], h->hi[2]) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     }
     if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (bank && bank_reader_done(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     h->state = 2;
     h->mixed = false;
     h->resL = h->outL; h->resC = h->outC;
@@ -675,10 +733,11 @@ int octo_fmm_interact_mixed(octo_fmm_t* h, const unsigned char* leaf)
 {
     if (!h || !leaf || h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
     if (h->state < 1) return OCTO_FMM_ESTATE;
+    if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
     if (h->kernel == 0) {
         // slab-fed kernel: one pass over the leaf-level lists; the partner's leaf flag travels in the padding slot of its record
-        if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
-        if (upload_tables(h, true) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+        BankLock guard(h);
+        if (bank_acquire(h, true) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
         if (cudaMemsetAsync(h->flags, 0, sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
         Params& P = h->prm;
         const long long ncell = (long long)P.nx * P.ny * P.nz;
@@ -688,16 +747,21 @@ int octo_fmm_interact_mixed(octo_fmm_t* h, const unsigned char* leaf)
         const int rc = launch_staged(h, h->lo[2], h->hi[2], true);
         P.leaf = nullptr;
         if (rc != OCTO_FMM_OK) return rc;
+        if (bank_reader_done(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
         h->state = 2;
         h->resL = h->outL; h->resC = h->outC;
     } else {
         const int rc = octo_fmm_interact(h);                   // the Eq. 15 part, whatever the cells' kind
         if (rc != OCTO_FMM_OK) return rc;
+        BankLock guard(h);
+        if (bank_acquire(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;      // the near-field table travels with the lists
         Params P = h->prm;
         P.L = h->outL; P.C = h->outC;
+        // the same dipole decision as the interaction kernels (flags[1] or "dipole_terms"), read on the device
         if (h->cfg.am_correction) m2l_near_kernel<true><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, nullptr);
         else                      m2l_near_kernel<false><<<brick_blocks(P), 256, 0, h->stream>>>(P, leaf, nullptr);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (bank_reader_done(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     }
     h->mixed = true;
     h->mixed_counted = false;
@@ -706,8 +770,11 @@ int octo_fmm_interact_mixed(octo_fmm_t* h, const unsigned char* leaf)
         if (cudaMemsetAsync(cnt, 0, sizeof(unsigned long long), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
         const Params& P = h->prm;
         const long long ocell = (long long)P.ox * P.oy * P.oz;
+        BankLock guard(h);
+        if (bank_acquire(h, h->kernel == 0) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;   // c_near is the same in both flavours: no re-upload
         count_near_kernel<<<(unsigned)((ocell + 255) / 256), 256, 0, h->stream>>>(P, leaf, cnt);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (bank_reader_done(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
         h->mixed_counted = true;
     }
     return OCTO_FMM_OK;
@@ -792,14 +859,14 @@ int octo_fmm_destroy(octo_fmm_t* h)
 {
     if (!h) return OCTO_FMM_EINVAL;
     cudaError_t e = cudaStreamSynchronize(h->stream);
-    if (h->s_h2d) {
-        cudaStreamDestroy(h->s_h2d);
-        cudaStreamDestroy(h->s_d2h);
-        for (int i = 0; i < MAX_CHUNKS; ++i) { cudaEventDestroy(h->ev_in[i]); cudaEventDestroy(h->ev_out[i]); }
-        cudaEventDestroy(h->ev_begin);
-        cudaEventDestroy(h->ev_end);
+    if (h->s_h2d) cudaStreamDestroy(h->s_h2d);
+    if (h->s_d2h) cudaStreamDestroy(h->s_d2h);
+    for (int i = 0; i < MAX_CHUNKS; ++i) {
+        if (h->ev_in[i]) cudaEventDestroy(h->ev_in[i]);
+        if (h->ev_out[i]) cudaEventDestroy(h->ev_out[i]);
     }
-    if (g_const_owner == h) { g_const_owner = nullptr; g_list_sig = 0; }
+    if (h->ev_begin) cudaEventDestroy(h->ev_begin);
+    if (h->ev_end) cudaEventDestroy(h->ev_end);
     delete h;
     return e == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
@@ -855,14 +922,16 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
                               double* d_m, double* d_c, double* d_L, double* d_C)
 {
     const Params& P = h->prm;
-    if (!h->s_h2d) {
-        if (cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
-        if (cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (!h->pipeline_ready) {
+        // created piece by piece; whatever exists is destroyed by octo_fmm_destroy (the handle is zero-initialised)
+        if (!h->s_h2d && cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (!h->s_d2h && cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
         for (int i = 0; i < MAX_CHUNKS; ++i)
-            if (cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming) != cudaSuccess ||
-                cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming) != cudaSuccess) return OCTO_FMM_ECUDA;
-        if (cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&h->ev_end, cudaEventDisableTiming) != cudaSuccess) return OCTO_FMM_ECUDA;
+            if ((!h->ev_in[i] && cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming) != cudaSuccess) ||
+                (!h->ev_out[i] && cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming) != cudaSuccess)) return OCTO_FMM_ECUDA;
+        if ((!h->ev_begin && cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming) != cudaSuccess) ||
+            (!h->ev_end && cudaEventCreateWithFlags(&h->ev_end, cudaEventDisableTiming) != cudaSuccess)) return OCTO_FMM_ECUDA;
+        h->pipeline_ready = true;
     }
     int zc = h->host_chunk;
     while ((P.oz + zc - 1) / zc + 4 > MAX_CHUNKS) zc += TILE_Z;
@@ -885,14 +954,20 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
     const size_t plane = (size_t)P.nx * P.ny, ncell = plane * P.nz;
     const size_t oplane = (size_t)P.ox * P.oy, ocell = oplane * P.oz;
     cudaStream_t sm = h->stream;
+    BankLock guard(h);                                     // held over all launches of this step
+    // interact() is redirected into the caller's scratch for the duration of this call only: restored on EVERY exit
+    struct Redirect {
+        octo_fmm_t* h; double* L; double* C;
+        Redirect(octo_fmm_t* h_, double* nl, double* nc) : h(h_), L(h_->outL), C(h_->outC) { h->outL = nl; h->outC = nc; }
+        ~Redirect() { h->outL = L; h->outC = C; }
+    } redirect(h, d_L, d_C);
 #define OCTO_TRY(call) do { if ((call) != cudaSuccess) return OCTO_FMM_ECUDA; } while (0)
+    auto body = [&]() -> int {
     OCTO_TRY(cudaMemsetAsync(h->flags, 0, 2 * sizeof(int), sm));
-    if (upload_tables(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    if (bank_acquire(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     OCTO_TRY(cudaEventRecord(h->ev_begin, sm));            // the copies start after earlier work on the caller's stream
     OCTO_TRY(cudaStreamWaitEvent(h->s_h2d, h->ev_begin, 0));
     OCTO_TRY(cudaStreamWaitEvent(h->s_d2h, h->ev_begin, 0));
-    double* const keepL = h->outL; double* const keepC = h->outC;
-    h->outL = d_L; h->outC = d_C;
     int brought = std::max(P.lo[2] - h->reach, 0);         // source layers [.., brought) are on the device
     int rc = OCTO_FMM_OK;
     for (int c = 0; c < nchunk && rc == OCTO_FMM_OK; ++c) {
@@ -921,11 +996,20 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
         if (C_h)
             OCTO_TRY(cudaMemcpy2DAsync(C_h + ooff, ocell * 8, d_C + ooff, ocell * 8, owidth, 3, cudaMemcpyDeviceToHost, h->s_d2h));
     }
-    h->outL = keepL; h->outC = keepC;
     if (rc != OCTO_FMM_OK) return rc;
+    if (bank_reader_done(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     OCTO_TRY(cudaEventRecord(h->ev_end, h->s_d2h));
     OCTO_TRY(cudaStreamWaitEvent(sm, h->ev_end, 0));        // the caller's stream completes when the last copy has
+    return OCTO_FMM_OK;
+    };
 #undef OCTO_TRY
+    const int rc = body();
+    if (rc != OCTO_FMM_OK) {
+        // join the side streams so that nothing of this call is still in flight when the caller frees its buffers
+        cudaStreamSynchronize(h->s_h2d);
+        cudaStreamSynchronize(h->s_d2h);
+        return rc;
+    }
     h->host_launches = 2 * nchunk;
     return OCTO_FMM_OK;
 }

@@ -118,6 +118,54 @@ def cell_forces_and_torques(moments, com_off, L, h, lo=(0, 0, 0)):
     return F, T
 
 
+def invariants_on_device(torch, mom, com, L, h):
+    """Sum of the forces and of the torques over a whole closed level (the formulas of
+    helpers.cell_forces_and_torques, component by component on device tensors so that 256^3 cells fit and take
+    seconds).  Returns (max_i |sum F_i| / sum |F|, max_i |sum T_i| / sum |T|)."""
+    i2 = {}
+    for t, (a, b) in enumerate([(0, 0), (0, 1), (0, 2), (1, 1), (1, 2), (2, 2)]):
+        i2[(a, b)] = i2[(b, a)] = 4 + t
+    i3 = {}
+    import itertools
+    for t, idx in enumerate([(0, 0, 0), (0, 0, 1), (0, 0, 2), (0, 1, 1), (0, 1, 2), (0, 2, 2), (1, 1, 1), (1, 1, 2), (1, 2, 2), (2, 2, 2)]):
+        for q in set(itertools.permutations(idx)):
+            i3[q] = 10 + t
+    nz, ny, nx = mom.shape[1:]
+    F = []
+    for i in range(3):
+        g = mom[0] * L[1 + i]
+        for j in range(3):
+            g = g + mom[1 + j] * L[i2[(i, j)]]
+            for k in range(3):
+                g = g + 0.5 * mom[i2[(j, k)]] * L[i3[(i, j, k)]]
+        F.append(-g)
+    ar = lambda m: (torch.arange(m, dtype=torch.float64, device=mom.device) + 0.5) * h
+    z = [ar(nx)[None, None, :] + com[0], ar(ny)[None, :, None] + com[1], ar(nz)[:, None, None] + com[2]]
+    inner = {}
+    for b in range(3):
+        for c in range(3):
+            if b == c:
+                continue
+            v = mom[1 + b] * L[1 + c]
+            for j in range(3):
+                v = v + mom[i2[(b, j)]] * L[i2[(c, j)]]
+                for k in range(3):
+                    v = v + 0.5 * mom[i3[(b, j, k)]] * L[i3[(c, j, k)]]
+            inner[(b, c)] = v
+    T = []
+    for a in range(3):
+        b, c = (a + 1) % 3, (a + 2) % 3
+        T.append(z[b] * F[c] - z[c] * F[b] - (inner[(b, c)] - inner[(c, b)]))
+
+    def ratio(V):
+        # plane sums on the device, the few hundred plane values summed exactly on the host
+        import math
+        tot = max(abs(math.fsum(v.sum(dim=(1, 2)).cpu().tolist())) for v in V)
+        den = math.fsum(sum(v.abs().sum(dim=(1, 2)) for v in V).cpu().tolist())
+        return tot / den
+    return ratio(F), ratio(T)
+
+
 def parity_error(got, ref):
     """north_star metric: per-cell max-norm error normalised by the cell's largest |coefficient|.
 

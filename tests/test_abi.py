@@ -79,3 +79,18 @@ def test_product_path_does_not_touch_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(base, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text and "fmm_oracle" not in text, f
+
+
+def test_marshalling_refuses_strided_arrays_and_cpu_tensors():
+    """_ptr() hands plain addresses to the C ABI: a strided array or tensor would be read as if it were dense."""
+    import numpy as np
+    import torch
+    import paper_2101_08226_b200 as p
+    a = np.zeros((4, 6))
+    assert p._ptr(a) == a.ctypes.data and p._ptr(None) is None
+    with pytest.raises(ValueError):
+        p._ptr(a[:, ::2])
+    with pytest.raises(ValueError):
+        p._ptr(torch.zeros((4, 6))[:, ::2])
+    with pytest.raises(ValueError):
+        p._check_device_tensor(torch.zeros(8, dtype=torch.float64), "moments", torch.float64, 8, torch.device("cuda", 0))

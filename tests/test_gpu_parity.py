@@ -9,12 +9,12 @@ import pytest
 
 import fmm_inputs as fi
 import oracle
-from helpers import cell_forces_and_torques, parity_error, per_order_error
+from helpers import cell_forces_and_torques, invariants_on_device, parity_error, per_order_error
 
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-12          # the contract
-TOL_ORDER = 2e-12    # per-order (L1 cancels heavily in smooth fields; still far below the contract's spirit)
+TOL_ORDER = 1e-12    # per order, each normalised by its own largest coefficient in the cell: the same bar
 
 
 @pytest.fixture(scope="module")
@@ -56,7 +56,7 @@ def check(L, Lc, Lr, Lcr, tol=TOL):
     assert max(eo) < TOL_ORDER, ("per order", eo)
     if Lcr is not None and np.abs(Lcr).max() > 0:
         ec = parity_error(Lc, Lcr)
-        assert ec < 1e-11, ("correction", ec)   # a small difference of large terms; folded value is held to TOL above
+        assert ec < TOL, ("correction", ec)
     return e
 
 
@@ -130,26 +130,43 @@ def cached_workload(name):
     return _CACHE[name]
 
 
-def _sampled_subgrids(n):
-    """8^3 sub-grids to compare at full size: corners, a face, an edge, interior, both stars."""
+def _stratified_subgrids(n, per_axis, seed):
+    """per_axis^3 seeded sub-grids, one from every stratum of the lattice of 8^3 sub-grids ("a seeded
+    sample of 512 sub-grids (stratified: corners, faces, interior)"), the eight corner sub-grids always among them."""
     s = n // 8
-    picks = {(0, 0, 0), (s - 1, s - 1, s - 1), (0, s // 2, s - 1), (s // 2, s // 2, s // 2),
-             (int(0.3 * s), s // 2, s // 2), (int(0.7 * s), s // 2, s // 2), (s // 2 + 1, 0, s // 3), (1, 2, 3)}
+    w = s // per_axis
+    rng = np.random.default_rng(seed)
+    picks = set()
+    for cz in range(per_axis):
+        for cy in range(per_axis):
+            for cx in range(per_axis):
+                o = rng.integers(0, w, 3)
+                picks.add((cx * w + int(o[0]), cy * w + int(o[1]), cz * w + int(o[2])))
+    for c in range(8):          # the corner strata contribute the corner sub-grid itself
+        corner = tuple((s - 1) if (c >> a) & 1 else 0 for a in range(3))
+        stratum = tuple(v // w for v in corner)
+        picks = {q for q in picks if tuple(v // w for v in q) != stratum} | {corner}
     return sorted(picks)
 
 
-def test_config3_full_size_sampled(env):
-    """cfg 3: 128^3 binary in the launch configuration bench.py uses; the oracle recomputes sampled
-    sub-grids; Newton's third law and the torque balance are checked on the whole GPU result."""
-    w = fi.config3()
+def _octant_face_regions(n):
+    """Every sub-grid of the octant [0, n/2)^3 that touches a domain face, as three disjoint slabs of cells."""
+    m = n // 2
+    return [((0, 0, 0), (8, m, m)), ((8, 0, 0), (m, 8, m)), ((8, 8, 0), (m, m, 8))]
+
+
+def _region_slices(lo, hi):
+    return (slice(None), slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+
+
+def test_config3_whole_grid(env):
+    """cfg 3: 128^3 binary in the launch configuration bench.py uses, EVERY cell against the oracle (full
+    runs for cfg 1-4); Newton's third law and the torque balance on the whole GPU result."""
+    w = cached_workload("cfg3")
     L, Lc, cnt, info = gpu_multipole(env, w)
-    assert cnt == 468364296
-    worst = 0.0
-    for (sx, sy, sz) in _sampled_subgrids(128):
-        lo, hi = (8 * sx, 8 * sy, 8 * sz), (8 * sx + 8, 8 * sy + 8, 8 * sz + 8)
-        Lr, Lcr, _ = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off, lo, hi, True)
-        sl = (slice(None), slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
-        worst = max(worst, check(L[sl], Lc[sl], Lr, Lcr))
+    Lr, Lcr, cntr = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off, None, None, True)
+    assert cnt == cntr == 468364296
+    check(L, Lc, Lr, Lcr)
     F, T = cell_forces_and_torques(w.moments, w.com_off, L, w.h)
     assert np.abs(F.sum(axis=(1, 2, 3))).max() / np.abs(F).sum() < 1e-14
     assert np.abs(T.sum(axis=(1, 2, 3))).max() / np.abs(T).sum() < 1e-12
@@ -157,9 +174,10 @@ def test_config3_full_size_sampled(env):
 
 @pytest.mark.parametrize("theta", [0.5, 0.35, 0.7])
 def test_config5_full_size_sampled(env, theta):
-    """cfg 5: 256^3, theta sweep, sampled sub-grids against the oracle -- in the configuration `bench.py` times (one
-    whole-grid launch of the staged kernel with all dipole terms, "dipole_terms" = 1) and on the library's default path
-    for these centre-of-mass inputs (dipole terms left out after the device-side check)."""
+    """cfg 5: 256^3, theta sweep, against the oracle on the sample SURVEY 8(d) prescribes -- 512 seeded, stratified
+    sub-grids plus every sub-grid of one octant that touches a domain face (721 more) -- in the configuration `bench.py`
+    times (one whole-grid launch of the staged kernel with all dipole terms, "dipole_terms" = 1) and on the library's
+    default path for these centre-of-mass inputs (dipole terms left out after the device-side check)."""
     p, torch = env
     w = cached_workload("cfg5")
     f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, True)
@@ -167,7 +185,12 @@ def test_config5_full_size_sampled(env, theta):
     com = torch.from_numpy(w.com_off).cuda()
     expect = {0.5: 3810941448, 0.35: 10646746680, 0.7: 2201973760}[theta]
     assert f.interaction_count() == expect
-    refs = {}
+    regions = _octant_face_regions(256)
+    subs = _stratified_subgrids(256, 8, seed=20210108)
+    assert len(subs) == 512
+    regions += [((8 * sx, 8 * sy, 8 * sz), (8 * sx + 8, 8 * sy + 8, 8 * sz + 8)) for (sx, sy, sz) in subs]
+    refs = [oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, lo, hi, True) for lo, hi in regions]
+    worst = 0.0
     for dipole_terms in (1, 0):
         f.set_option("dipole_terms", dipole_terms)
         L, Lc = f.solve(mom, com)
@@ -175,19 +198,50 @@ def test_config5_full_size_sampled(env, theta):
         assert f.status() == p.OK
         assert f.dipole_terms_used() == bool(dipole_terms)
         assert f.launch_info()["grid"] == torch.cuda.get_device_properties(0).multi_processor_count
-        for (sx, sy, sz) in _sampled_subgrids(256)[:6]:
-            lo, hi = (8 * sx, 8 * sy, 8 * sz), (8 * sx + 8, 8 * sy + 8, 8 * sz + 8)
-            if (lo, hi) not in refs:
-                refs[(lo, hi)] = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, lo, hi, True)
-            Lr, Lcr, _ = refs[(lo, hi)]
-            g = L[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
-            gc = Lc[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]].cpu().numpy()
-            check(g, gc, Lr, Lcr)
+        Lh, Lch = L.cpu().numpy(), Lc.cpu().numpy()
+        for (lo, hi), (Lr, Lcr, _) in zip(regions, refs):
+            sl = _region_slices(lo, hi)
+            worst = max(worst, check(Lh[sl], Lch[sl], Lr, Lcr))
+        del L, Lc, Lh, Lch
     f.close()
 
 
+def test_config5_whole_grid_invariants_and_cross_checks(env):
+    """cfg 5, theta = 0.5, over 100 % of the 256^3 cells, on the device: (i) the slab-fed kernel run twice gives
+    bit-identical results (a hazard in the slab ring of the persistent 148-CTA launch would not); (ii) it agrees with the
+    ring-free m2l_direct_kernel (global-memory loads, explicit in-grid tests) within 1e-13 per cell; (iii) Newton's third
+    law and, with the correction, the torque balance hold on the whole GPU result."""
+    p, torch = env
+    w = cached_workload("cfg5")
+    mom = torch.from_numpy(w.moments).cuda()
+    com = torch.from_numpy(w.com_off).cuda()
+    f = p.OctoFMM(w.n, w.h, 0.5, p.MULTIPOLE, True)
+    f.set_option("dipole_terms", 1)
+    L1, C1 = (t.clone() for t in f.solve(mom, com))
+    L2, C2 = f.solve(mom, com)
+    torch.cuda.synchronize()
+    assert f.status() == p.OK
+    assert torch.equal(L1, L2) and torch.equal(C1, C2)
+    del L2, C2
+    f.set_option("kernel", 1)
+    Ld, Cd = f.solve(mom, com)
+    torch.cuda.synchronize()
+    assert f.status() == p.OK
+    scale = L1.abs().amax(dim=0)
+    err = float(((L1 - Ld).abs().amax(dim=0) / scale).max())
+    assert err < 1e-13, err
+    errc = float(((C1 - Cd).abs().amax(dim=0) / C1.abs().amax(dim=0)).max())
+    assert errc < 1e-12, errc
+    del Ld, Cd, scale
+    f.close()
+    eF, eT = invariants_on_device(torch, mom, com, L1, w.h)
+    assert eF < 1e-14, eF
+    assert eT < 1e-12, eT
+
+
 def test_monopole_config4(env):
-    """cfg 4: monopole variant; small full-grid parity, full-size sampled parity, zero net force."""
+    """cfg 4: monopole variant; small full-grid parity, then the full 128^3 grid, every cell against the oracle, and
+    zero net force."""
     p, torch = env
     w = fi.config4(ncell=32)
     f = p.OctoFMM(w.n, w.h, 0.5, p.MONOPOLE)
@@ -202,12 +256,10 @@ def test_monopole_config4(env):
     f = p.OctoFMM(w.n, w.h, 0.5, p.MONOPOLE)
     out, _ = f.solve(torch.from_numpy(w.moments).cuda())
     torch.cuda.synchronize()
-    assert f.interaction_count() == 468364296
     out = out.cpu().numpy()
-    for (sx, sy, sz) in _sampled_subgrids(128):
-        lo, hi = (8 * sx, 8 * sy, 8 * sz), (8 * sx + 8, 8 * sy + 8, 8 * sz + 8)
-        ref, _ = oracle.interact_monopole(w.n, w.h, 0.5, w.moments[0], lo, hi)
-        assert parity_error(out[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]], ref) < TOL
+    ref, cnt = oracle.interact_monopole(w.n, w.h, 0.5, w.moments[0])
+    assert f.interaction_count() == cnt == 468364296
+    assert parity_error(out, ref) < TOL
     mg = w.moments[0][None] * out[1:4]
     assert np.abs(mg.sum(axis=(1, 2, 3))).max() / np.abs(mg).sum() < 1e-14
     f.close()
@@ -679,3 +731,81 @@ def test_mixed_level_of_an_adaptive_mesh(env, theta, correction, kernel):
     with pytest.raises(p.OctoFmmError):
         p.OctoFMM(w.n, w.h, theta, p.MONOPOLE).interact_mixed(lf)
     f.close()
+
+
+def test_two_handles_on_two_streams_with_different_lists_and_cell_widths(env):
+    """Handles of one device share one constant-memory bank of interaction lists (a function of theta and kind);
+    everything that depends on h travels with the launch.  Two handles with different theta AND different h, each on its
+    own stream, interleaved for many rounds without any host synchronisation in between, must both match the oracle:
+    the library orders every upload against the other stream's kernels that still read the previous lists.  A third
+    handle shares theta with the first (same lists, other h, other stream: no upload, concurrent)."""
+    p, torch = env
+    wa = fi.config2(ncell=32)                      # polytrope, theta 0.5, h = 1/32
+    wb = fi.config1(seed=17, ncell=32, theta=0.35)
+    wb.h = 0.37                                    # another cell width: the moments below are rescaled to it
+    scale = wb.h / (1.0 / 32)
+    for sl, power in ((slice(1, 4), 1), (slice(4, 10), 2), (slice(10, 20), 3)):
+        wb.moments[sl] *= scale ** power
+    wb.com_off *= scale
+    wc = fi.config1(seed=23, ncell=32)             # theta 0.5 as wa, h = 1/32 * 3
+    wc.h = 3.0 / 32
+    for sl, power in ((slice(1, 4), 1), (slice(4, 10), 2), (slice(10, 20), 3)):
+        wc.moments[sl] *= 3.0 ** power
+    wc.com_off *= 3.0
+    whole = ((0, 0, 0), (32, 32, 32))
+    cases = [(wa, 0.5, True), (wb, 0.35, True), (wc, 0.5, False)]
+    streams = [torch.cuda.Stream() for _ in cases]
+    handles, data, outs = [], [], []
+    for (w, theta, corr), st in zip(cases, streams):
+        f = p.OctoFMM(w.n, w.h, theta, p.MULTIPOLE, corr, stream=st)
+        f.set_option("kernel", 0)
+        handles.append(f)
+        with torch.cuda.stream(st):
+            data.append((torch.from_numpy(w.moments).cuda(), torch.from_numpy(w.com_off).cuda()))
+            L = torch.empty((20, 32, 32, 32), dtype=torch.float64, device="cuda")
+            C = torch.empty((3, 32, 32, 32), dtype=torch.float64, device="cuda")
+            f.bind_outputs(L, C)
+            outs.append((L, C))
+    torch.cuda.synchronize()
+    for rnd in range(12):
+        order = [0, 1, 2] if rnd % 2 == 0 else [1, 2, 0]
+        for i in order:
+            handles[i].set_moments(*data[i])
+            handles[i].interact()                   # asynchronous on its own stream
+    torch.cuda.synchronize()
+    for (w, theta, corr), f, (L, C) in zip(cases, handles, outs):
+        assert f.status() == p.OK
+        Lr, Lcr, cnt = oracle.interact_multipole(w.n, w.h, theta, w.moments, w.com_off, whole[0], whole[1], corr)
+        assert f.interaction_count() == cnt
+        check(L.cpu().numpy(), C.cpu().numpy(), Lr, Lcr if corr else None)
+        f.close()
+
+
+def test_binding_refuses_tensors_the_c_abi_would_misread(env):
+    """The C ABI takes plain pointers; the convenience classes check what they marshal: device, dtype, contiguity and
+    element count (a float32 or strided tensor would otherwise be read out of bounds without any error)."""
+    p, torch = env
+    w = fi.config1()
+    f = p.OctoFMM(w.n, w.h, 0.5, p.MULTIPOLE, True, w.out_lo, w.out_hi)
+    mom, com = torch.from_numpy(w.moments).cuda(), torch.from_numpy(w.com_off).cuda()
+    for bad_m, bad_c in ((mom.float(), com), (mom, com.cpu()), (mom[:, :, :, ::2], com), (mom[:19], com),
+                         (mom.transpose(1, 3), com), (mom, None)):
+        with pytest.raises(ValueError):
+            f.set_moments(bad_m, bad_c)
+    f.set_moments(mom, com)
+    f.interact()
+    with pytest.raises(ValueError):
+        f.get_expansions(torch.empty((20, 8, 8, 4), dtype=torch.float64, device="cuda"))
+    with pytest.raises(ValueError):
+        f.bind_outputs(torch.empty((20, 8, 8, 8), dtype=torch.float32, device="cuda"))
+    with pytest.raises(ValueError):
+        f.interact_mixed(torch.zeros((24, 24, 24), dtype=torch.float64, device="cuda"))
+    L, _ = f.get_expansions()
+    assert f.status() == p.OK and bool(torch.isfinite(L).all())
+    f.close()
+    s = p.OctoFMMSolver(16, 1.0 / 16, 0.5)
+    with pytest.raises(ValueError):
+        s.solve(torch.ones((16, 16, 16), dtype=torch.float32, device="cuda"))
+    with pytest.raises(ValueError):
+        s.solve(torch.ones((16, 16, 8), dtype=torch.float64, device="cuda"))
+    s.close()

@@ -163,3 +163,21 @@ def test_linearity_and_component_order():
         L, _ = oracle.pair(R, e)
         np.testing.assert_allclose(L[0], -mult[t] * D3[idx] / 6.0, rtol=1e-13)
         assert np.all(L[1:] == 0.0)
+
+
+def test_device_invariant_helper_matches_the_numpy_one():
+    """helpers.invariants_on_device (torch, used on 256^3 GPU results) against helpers.cell_forces_and_torques (numpy)
+    on a small random level: same force and torque sums."""
+    import torch
+    from helpers import cell_forces_and_torques, invariants_on_device
+    rng = np.random.default_rng(5)
+    n, h = 6, 0.37
+    mom = rng.normal(size=(20, n, n, n))
+    com = rng.normal(size=(3, n, n, n)) * 0.1 * h
+    L = rng.normal(size=(20, n, n, n))
+    F, T = cell_forces_and_torques(mom, com, L, h)
+    eF = np.abs(F.sum(axis=(1, 2, 3))).max() / np.abs(F).sum()
+    eT = np.abs(T.sum(axis=(1, 2, 3))).max() / np.abs(T).sum()
+    gF, gT = invariants_on_device(torch, torch.from_numpy(mom), torch.from_numpy(com), torch.from_numpy(L), h)
+    assert abs(gF - eF) < 1e-12 * max(eF, 1.0) and abs(gT - eT) < 1e-12 * max(eT, 1.0)
+    assert eF > 1e-3 and eT > 1e-3          # random L: nothing cancels, so the comparison is not 0 == 0
