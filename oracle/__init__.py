@@ -49,6 +49,8 @@ def lib():
         L.fmm_oracle_pair.argtypes = [dp, dp, ctypes.c_double, dp, ctypes.c_int, dp, dp]
         L.fmm_oracle_interact_multipole.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                                     dp, dp, dp, dp, ullp]
+        L.fmm_oracle_interact_multipole_cond.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                                         dp, dp, dp, dp, dp, ullp]
         L.fmm_oracle_interact_monopole.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, dp, dp, ullp]
         L.fmm_oracle_interact_multipole_mixed.argtypes = [ip, ip, ip, ctypes.c_double, ctypes.c_double, ctypes.c_int,
                                                           dp, dp, ctypes.POINTER(ctypes.c_ubyte), dp, dp, ullp]
@@ -129,6 +131,27 @@ def interact_multipole(n, h, theta, moments, com_off, out_lo=None, out_hi=None, 
                                          ctypes.byref(cnt))
     _check(rc, "interact_multipole")
     return Lout, Lc, cnt.value
+
+
+def interact_multipole_cond(n, h, theta, moments, com_off, out_lo=None, out_hi=None, am_correction=True):
+    """interact_multipole plus the condition of every sum: returns (L, Lcorr, Labs[23][oz][oy][ox], n_interactions),
+    Labs = sum over the partners of |term| for the 20 coefficients and the 3 components of the correction."""
+    out_lo = (0, 0, 0) if out_lo is None else out_lo
+    out_hi = tuple(n) if out_hi is None else out_hi
+    moments = np.ascontiguousarray(moments, dtype=np.float64)
+    com_off = np.ascontiguousarray(com_off, dtype=np.float64)
+    nx, ny, nz = n
+    assert moments.shape == (20, nz, ny, nx) and com_off.shape == (3, nz, ny, nx)
+    o = tuple(out_hi[a] - out_lo[a] for a in range(3))
+    Lout = np.zeros((20, o[2], o[1], o[0]))
+    Lc = np.zeros((3, o[2], o[1], o[0]))
+    La = np.zeros((23, o[2], o[1], o[0]))
+    cnt = ctypes.c_ulonglong(0)
+    rc = lib().fmm_oracle_interact_multipole_cond(_i3(n), _i3(out_lo), _i3(out_hi), float(h), float(theta),
+                                                  int(bool(am_correction)), _dp(moments), _dp(com_off), _dp(Lout), _dp(Lc),
+                                                  _dp(La), ctypes.byref(cnt))
+    _check(rc, "interact_multipole_cond")
+    return Lout, Lc, La, cnt.value
 
 
 def interact_multipole_mixed(n, h, theta, moments, com_off, leaf, out_lo=None, out_hi=None, am_correction=True):

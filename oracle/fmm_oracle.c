@@ -318,7 +318,7 @@ static void free_stencils(stencil_set *S) { for (int p = 0; p < 8; ++p) free(S->
 static int interact_multipole_impl(const int n[3], const int out_lo[3], const int out_hi[3], double h,
                                    double theta, int am_correction, const double *moments,
                                    const double *com_off, const unsigned char *leaf, double *L, double *Lcorr,
-                                   unsigned long long *n_interactions)
+                                   double *Labs, unsigned long long *n_interactions)
 {
     if (!n || !out_lo || !out_hi || !moments || !com_off || !L || !(h > 0.0)) return ORC_EINVAL;
     if (!check_region(n, out_lo, out_hi)) return ORC_EINVAL;
@@ -340,7 +340,9 @@ static int interact_multipole_impl(const int n[3], const int out_lo[3], const in
                 const size_t a = ((size_t)k * ny + j) * nx + i;
                 const int p = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
                 long double acc[20], cacc[3] = {0.0L, 0.0L, 0.0L};
+                long double aabs[23];      /* sum over the partners of |term|: the condition of each sum (Labs) */
                 for (int c = 0; c < 20; ++c) acc[c] = 0.0L;
+                for (int c = 0; c < 23; ++c) aabs[c] = 0.0L;
                 double MA3[10], MA0 = moments[a], dA[3];
                 for (int c = 0; c < 10; ++c) MA3[c] = moments[(size_t)(10 + c) * ncell + a];
                 for (int c = 0; c < 3; ++c) dA[c] = com_off[(size_t)c * ncell + a];
@@ -360,6 +362,10 @@ static int interact_multipole_impl(const int n[3], const int out_lo[3], const in
                     pair_terms(R, MB, MA0, MA3, am_correction && MA0 > 0.0, term, cterm);
                     for (int c = 0; c < 20; ++c) acc[c] += (long double)term[c];
                     for (int c = 0; c < 3; ++c) cacc[c] += (long double)cterm[c];
+                    if (Labs) {
+                        for (int c = 0; c < 20; ++c) aabs[c] += (long double)fabs(term[c]);
+                        for (int c = 0; c < 3; ++c) aabs[20 + c] += (long double)fabs(cterm[c]);
+                    }
                     ++total;
                 }
                 const size_t o = ((size_t)(k - out_lo[2]) * oy + (j - out_lo[1])) * ox + (i - out_lo[0]);
@@ -368,6 +374,8 @@ static int interact_multipole_impl(const int n[3], const int out_lo[3], const in
                 for (int c = 0; c < 20; ++c) L[(size_t)c * ocell + o] = (double)acc[c];
                 if (Lcorr)
                     for (int c = 0; c < 3; ++c) Lcorr[(size_t)c * ocell + o] = (double)cacc[c];
+                if (Labs)
+                    for (int c = 0; c < 23; ++c) Labs[(size_t)c * ocell + o] = (double)aabs[c];
             }
     free_stencils(&S);
     if (n_interactions) *n_interactions = total;
@@ -379,7 +387,24 @@ int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int
                                   const double *com_off, double *L, double *Lcorr,
                                   unsigned long long *n_interactions)
 {
-    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, L, Lcorr, n_interactions);
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, L, Lcorr, NULL, n_interactions);
+}
+
+/*
+ * The same step, and beside every sum its CONDITION: Labs [23][oz][oy][ox] = sum over the partners of |term| for
+ * the 20 coefficients (without the correction) and for the 3 components of the correction.  Nothing of the result
+ * depends on it; the parity tests use it to hold each expansion order to 1e-12 of the size of what was summed
+ * ("each order normalised by that order's sum_B |term| (condition-aware)") -- in a smooth field the
+ * partners' contributions to L2 and to the correction cancel to a small remainder, and an error of n eps sum|term| is
+ * then a large fraction of the remainder although every term is right to the last bit.
+ */
+int fmm_oracle_interact_multipole_cond(const int n[3], const int out_lo[3], const int out_hi[3], double h,
+                                       double theta, int am_correction, const double *moments,
+                                       const double *com_off, double *L, double *Lcorr, double *Labs,
+                                       unsigned long long *n_interactions)
+{
+    if (!Labs) return ORC_EINVAL;
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, L, Lcorr, Labs, n_interactions);
 }
 
 /*
@@ -397,7 +422,7 @@ int fmm_oracle_interact_multipole_mixed(const int n[3], const int out_lo[3], con
                                         unsigned long long *n_interactions)
 {
     if (!leaf) return ORC_EINVAL;
-    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, leaf, L, Lcorr, n_interactions);
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, leaf, L, Lcorr, NULL, n_interactions);
 }
 
 /*

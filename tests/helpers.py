@@ -184,6 +184,25 @@ def per_order_error(got, ref):
     return out
 
 
+def conditioned_order_error(got, gotc, ref, refc, labs):
+    """Condition-aware per-order error: for each expansion order, and for the correction alone, the
+    largest |got - ref| of the order's coefficients in a cell divided by the largest sum_B |term| of that order in the
+    cell (labs [23][...] from oracle.interact_multipole_cond).  A correct kernel stays at a few n eps whatever the
+    cancellation between partners; gotc/refc None skips the correction.  Returns [e0, e1, e2, e3, ecorr]."""
+    out = []
+    for sl in (slice(0, 1), slice(1, 4), slice(4, 10), slice(10, 20)):
+        den = labs[sl].max(axis=0)
+        den = np.where(den > 0, den, 1.0)
+        out.append(float((np.abs(got[sl] - ref[sl]).max(axis=0) / den).max()))
+    if gotc is not None and refc is not None:
+        den = labs[20:23].max(axis=0)
+        den = np.where(den > 0, den, 1.0)
+        out.append(float((np.abs(gotc - refc).max(axis=0) / den).max()))
+    else:
+        out.append(0.0)
+    return out
+
+
 def load_golden(path):
     vals = {}
     multi = {}

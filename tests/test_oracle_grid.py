@@ -186,3 +186,30 @@ def test_monopole_zero_net_force_and_multipole_limit():
     L, _, _ = oracle.interact_multipole(w.n, w.h, 0.5, mom, np.zeros((3,) + mass.shape), am_correction=False)
     np.testing.assert_allclose(L[0], out[0], rtol=1e-14)
     np.testing.assert_allclose(-L[1:4], out[1:4], rtol=0, atol=1e-14 * np.abs(out[1:4]).max())
+
+
+def test_condition_output_is_the_sum_of_absolute_terms():
+    """oracle.interact_multipole_cond: Labs = sum_B |term| -- pinned by re-summing oracle.pair over the list in plain
+    Python for a few cells, by |L| <= Labs (triangle inequality) everywhere, and by L, Lcorr being bit-identical to
+    interact_multipole's (the extra output changes nothing)."""
+    w = fi.config1(seed=3, ncell=16)
+    lo, hi = (4, 4, 4), (12, 12, 12)
+    L, Lc, La, cnt = oracle.interact_multipole_cond(w.n, w.h, 0.5, w.moments, w.com_off, lo, hi, True)
+    L0, Lc0, cnt0 = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off, lo, hi, True)
+    assert np.array_equal(L, L0) and np.array_equal(Lc, Lc0) and cnt == cnt0
+    Lnc = L.copy()
+    Lnc[1:4] -= Lc
+    assert (np.abs(Lnc) <= La[:20] * (1 + 1e-12)).all() and (np.abs(Lc) <= La[20:] * (1 + 1e-12)).all()
+    for (i, j, k) in ((4, 4, 4), (7, 9, 11), (11, 11, 10)):
+        par = (i & 1) + 2 * (j & 1) + 4 * (k & 1)
+        tot = np.zeros(23)
+        for d in oracle.stencil(0.5, par):
+            bi, bj, bk = i + int(d[0]), j + int(d[1]), k + int(d[2])
+            if not (0 <= bi < 16 and 0 <= bj < 16 and 0 <= bk < 16):
+                continue
+            R = np.array([(i - bi) * w.h, (j - bj) * w.h, (k - bk) * w.h]) + (w.com_off[:, k, j, i] - w.com_off[:, bk, bj, bi])
+            t, c = oracle.pair(R, w.moments[:, bk, bj, bi], w.moments[0, k, j, i], w.moments[10:, k, j, i], True)
+            tot[:20] += np.abs(t)
+            tot[20:] += np.abs(c)
+        got = La[:, k - 4, j - 4, i - 4]
+        assert np.abs(got - tot).max() <= 1e-13 * tot.max()
