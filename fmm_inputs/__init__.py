@@ -317,3 +317,146 @@ def uniform_sphere(ncell: int = 64, radius: float = 0.25, total_mass: float = 1.
     mass = rho * (total_mass / rho.sum())
     phi = np.where(r < radius, -total_mass * (3.0 * radius ** 2 - r * r) / (2.0 * radius ** 3), -total_mass / r)
     return h, mass, phi, r
+
+
+# ---------------------------------------------------------------------------------------------
+# Adaptive oct-trees of 8^3 sub-grids.  Inputs only: topology and leaf masses.
+# ---------------------------------------------------------------------------------------------
+TREE_ABSENT, TREE_LEAF, TREE_REFINED = 0, 1, 2
+
+
+class Tree:
+    """An oct-tree of 8^3 sub-grids over a cube of width n0 * h0.  Level l is a dense
+    [n_l][n_l][n_l] lattice, n_l = n0 2^l, h_l = h0 / 2^l, with kind[l] (uint8: 0 absent, 1 leaf, 2 refined; constant
+    over every aligned 8^3 sub-grid) and mass[l] (float64; the point mass of every leaf cell, 0 elsewhere).
+    "A node is either fully refined with eight child nodes (an interior node) or not refined at all (a leaf node)"
+    (L287): a cell exists on level l+1 iff its parent cell is refined; the tree is properly nested (2:1 over the 26
+    neighbours of a sub-grid), so a refinement boundary involves exactly two levels (L287-291)."""
+
+    def __init__(self, n0, h0, kind, mass):
+        self.n0, self.h0, self.kind, self.mass = int(n0), float(h0), kind, mass
+
+    @property
+    def depth(self):
+        return len(self.kind)
+
+    def n(self, l):
+        return self.n0 << l
+
+    def h(self, l):
+        return self.h0 / (1 << l)
+
+    def leaf_points(self):
+        """(pos[np][3], mass[np], level[np], index[np][3]) of all leaf cells, levels in order, C order inside a level."""
+        pos, ms, lv, idx = [], [], [], []
+        for l in range(self.depth):
+            k, j, i = np.nonzero(self.kind[l] == TREE_LEAF)
+            h = self.h(l)
+            pos.append(np.stack([(i + 0.5) * h, (j + 0.5) * h, (k + 0.5) * h], axis=1))
+            ms.append(self.mass[l][k, j, i])
+            lv.append(np.full(len(i), l))
+            idx.append(np.stack([i, j, k], axis=1))
+        return np.concatenate(pos), np.concatenate(ms), np.concatenate(lv), np.concatenate(idx)
+
+
+def _expand8(a):
+    return np.repeat(np.repeat(np.repeat(a, 8, 0), 8, 1), 8, 2)
+
+
+def _dilate26(a):
+    """True where a sub-grid or any of its 26 neighbours is True (sub-grid lattice, isolated domain)."""
+    p = np.pad(a, 1)
+    out = np.zeros_like(a)
+    s = a.shape[0]
+    for dz in range(3):
+        for dy in range(3):
+            for dx in range(3):
+                out |= p[dz:dz + s, dy:dy + s, dx:dx + s]
+    return out
+
+
+def make_tree(n0, depth, want_refined, density, box=1.0):
+    """Build a properly nested tree.  n0: cells per axis of level 0 (a multiple of 8, every cell exists); depth: number
+    of levels; want_refined(l, cx, cy, cz) -> bool array over the sub-grid lattice of level l (centres of the sub-grids
+    as arrays): the sub-grids the caller wants refined on level l < depth - 1; density(x, y, z) -> rho at leaf centres
+    (mass = rho h_l^3).  Proper nesting is enforced bottom-up: a sub-grid is refined as well if any of the 26 neighbours
+    of one of its child sub-grids is refined (then no leaf touches a leaf two levels finer)."""
+    assert n0 % 8 == 0 and depth >= 1
+    h0 = box / n0
+    ref = []                                   # refined flags over the sub-grid lattice of each level
+    exists = [np.ones((n0 // 8,) * 3, dtype=bool)]
+    for l in range(depth - 1):
+        s = (n0 // 8) << l
+        c = (np.arange(s) + 0.5) * (box / s)
+        CZ, CY, CX = np.meshgrid(c, c, c, indexing="ij")
+        r = np.asarray(want_refined(l, CX, CY, CZ), dtype=bool) & exists[l]
+        ref.append(r)
+        exists.append(np.repeat(np.repeat(np.repeat(r, 2, 0), 2, 1), 2, 2))
+    ref.append(np.zeros_like(exists[-1]))
+    # 2:1 over the 26 neighbours, bottom-up: the parent of every neighbour of a refined sub-grid must be refined
+    for l in range(depth - 2, 0, -1):
+        need = _dilate26(ref[l])                       # sub-grids of level l that must EXIST
+        s = need.shape[0] // 2
+        need_parent = need.reshape(s, 2, s, 2, s, 2).any(axis=(1, 3, 5))
+        ref[l - 1] |= need_parent
+    # top-down again: existence follows the (grown) refinement
+    exists = [np.ones((n0 // 8,) * 3, dtype=bool)]
+    for l in range(depth - 1):
+        ref[l] &= exists[l]
+        exists.append(np.repeat(np.repeat(np.repeat(ref[l], 2, 0), 2, 1), 2, 2))
+    ref[depth - 1] &= False
+    kind, mass = [], []
+    for l in range(depth):
+        k = np.where(exists[l], np.where(ref[l], TREE_REFINED, TREE_LEAF), TREE_ABSENT).astype(np.uint8)
+        k = _expand8(k)
+        n = n0 << l
+        h = h0 / (1 << l)
+        x = (np.arange(n) + 0.5) * h
+        Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+        m = np.where(k == TREE_LEAF, np.asarray(density(X, Y, Z), dtype=np.float64) * h ** 3, 0.0)
+        kind.append(np.ascontiguousarray(k))
+        mass.append(np.ascontiguousarray(m))
+    return Tree(n0, h0, kind, mass)
+
+
+def tree_is_properly_nested(tree) -> bool:
+    """Every refined cell's children exist; no leaf sub-grid has a neighbour (26) two levels finer."""
+    for l in range(tree.depth - 1):
+        k, kf = tree.kind[l], tree.kind[l + 1]
+        par = np.repeat(np.repeat(np.repeat(k, 2, 0), 2, 1), 2, 2)
+        if ((kf != TREE_ABSENT) != (par == TREE_REFINED)).any():
+            return False
+        # sub-grid lattice of level l+1: refined sub-grids need all 26 neighbours to exist (inside the domain)
+        sub = kf[::8, ::8, ::8]
+        need = _dilate26(sub == TREE_REFINED)
+        if (need & (sub == TREE_ABSENT)).any():
+            return False
+    return not (tree.kind[-1] == TREE_REFINED).any()
+
+
+def seeded_tree(seed: int, n0: int = 16, depth: int = 3, frac: float = 0.4):
+    """A seeded random tree for the pins and the parity tests: level 0 is refined everywhere, on every deeper level each
+    existing sub-grid is refined with probability `frac` (proper nesting then refines some more); leaf densities
+    ~ U(0.5, 1.5) (SplitMix64 stream per level, C order)."""
+    def want(l, cx, cy, cz):
+        u = uniform01(seed + 1000 * (l + 1), cx.size).reshape(cx.shape)
+        return (u < frac) | (l == 0)
+
+    def rho(X, Y, Z):
+        return 0.5 + uniform01(seed + 77 + X.shape[0], X.size).reshape(X.shape)
+    return make_tree(n0, depth, want, rho)
+
+
+def star_tree(n0: int = 16, depth: int = 3, stars=None, radius_factor: float = 1.3):
+    """The paper's refinement pattern in miniature (density-based refinement, Eq. 34-35: finer where the
+    density is higher): level l refines the sub-grids within radius_factor * R_star / 2^l... of a star centre; density
+    = the n = 1.5 polytropes of `stars` (default: the two-star binary of cfg 3) over the 1e-10 floor."""
+    stars = BINARY if stars is None else stars
+
+    def want(l, cx, cy, cz):
+        w = np.zeros(cx.shape, dtype=bool)
+        for s in stars:
+            rr = np.sqrt((cx - s.centre[0]) ** 2 + (cy - s.centre[1]) ** 2 + (cz - s.centre[2]) ** 2)
+            w |= rr < radius_factor * s.radius / (1.5 ** l)
+        return w
+    return make_tree(n0, depth, want, lambda X, Y, Z: field_density(stars, X, Y, Z))

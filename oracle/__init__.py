@@ -61,6 +61,12 @@ def lib():
         L.fmm_oracle_m2m_about.argtypes = [ip, ctypes.c_double, dp, dp, dp, dp]
         L.fmm_oracle_l2l.argtypes = [ip, ctypes.c_double, dp, dp, dp, dp, dp, dp]
         L.fmm_oracle_direct_sum.argtypes = [ip, ctypes.c_double, dp, dp]
+        ubp = ctypes.POINTER(ctypes.c_ubyte)
+        L.fmm_oracle_tree_interact_multipole.argtypes = [ip, ctypes.c_double, ctypes.c_double, ctypes.c_int, dp, dp, ubp,
+                                                         dp, dp, ullp]
+        L.fmm_oracle_tree_leaf_p2p.argtypes = [ip, ctypes.c_double, ctypes.c_double, ubp, dp, dp, ullp]
+        L.fmm_oracle_tree_cross_level.argtypes = [ip, ctypes.c_double, ctypes.c_double, ubp, dp, ubp, dp, dp, dp, ullp]
+        L.fmm_oracle_direct_sum_points.argtypes = [ctypes.c_long, dp, dp, dp]
         L.fmm_oracle_num_threads.restype = ctypes.c_int
         L.fmm_oracle_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -351,3 +357,139 @@ def solve(n, h, theta, mass, am_correction=True, coarsest=2):
         out[0] += Ll[0]
         out[1:4] -= Ll[1:4] + cl
     return out
+
+
+# ---- adaptive oct-tree of 8^3 sub-grids (reading R9) ------------------------------------
+def _ub(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte))
+
+
+def tree_interact_multipole(n, h, theta, moments, com_off, kind, am_correction=True):
+    """Same-level multipole step on one level of a tree (kind: 0 absent, 1 leaf, 2 refined): every existing cell takes
+    the existing cells of its Eq. 15 list, except that two leaves do not meet here.  Returns (L, Lcorr, count)."""
+    n = int(n)
+    moments = np.ascontiguousarray(moments, dtype=np.float64)
+    com_off = np.ascontiguousarray(com_off, dtype=np.float64)
+    kind = np.ascontiguousarray(kind, dtype=np.uint8)
+    assert moments.shape == (20, n, n, n) and com_off.shape == (3, n, n, n) and kind.shape == (n, n, n)
+    Lout, Lc = np.zeros((20, n, n, n)), np.zeros((3, n, n, n))
+    cnt = ctypes.c_ulonglong(0)
+    _check(lib().fmm_oracle_tree_interact_multipole(_i3((n, n, n)), float(h), float(theta), int(bool(am_correction)),
+                                                    _dp(moments), _dp(com_off), _ub(kind), _dp(Lout), _dp(Lc),
+                                                    ctypes.byref(cnt)), "tree_interact_multipole")
+    return Lout, Lc, cnt.value
+
+
+def tree_leaf_p2p(n, h, theta, kind, mass):
+    """Point-mass sum of the leaf cells of one level over the leaf-level list.  Returns (out[4][n][n][n], count)."""
+    n = int(n)
+    kind = np.ascontiguousarray(kind, dtype=np.uint8)
+    mass = np.ascontiguousarray(mass, dtype=np.float64)
+    assert kind.shape == (n, n, n) and mass.shape == (n, n, n)
+    out = np.zeros((4, n, n, n))
+    cnt = ctypes.c_ulonglong(0)
+    _check(lib().fmm_oracle_tree_leaf_p2p(_i3((n, n, n)), float(h), float(theta), _ub(kind), _dp(mass), _dp(out),
+                                          ctypes.byref(cnt)), "tree_leaf_p2p")
+    return out, cnt.value
+
+
+def tree_cross_level(nc, hc, theta, kind_c, mass_c, kind_f, mass_f, out_c, out_f):
+    """Point-mass pairs across a refinement boundary: a coarse leaf and the 8 children of every refined cell of its
+    near field, both directions; ADDED to out_c [4][nc]^3 and out_f [4][2 nc]^3.  Returns the number of ordered pairs."""
+    nc = int(nc)
+    for a in (kind_c, kind_f):
+        assert a.dtype == np.uint8 and a.flags["C_CONTIGUOUS"]
+    for a in (mass_c, mass_f, out_c, out_f):
+        assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    assert kind_c.shape == (nc,) * 3 and kind_f.shape == (2 * nc,) * 3 and out_c.shape == (4,) + (nc,) * 3
+    cnt = ctypes.c_ulonglong(0)
+    _check(lib().fmm_oracle_tree_cross_level(_i3((nc, nc, nc)), float(hc), float(theta), _ub(kind_c), _dp(mass_c), _ub(kind_f),
+                                             _dp(mass_f), _dp(out_c), _dp(out_f), ctypes.byref(cnt)), "tree_cross_level")
+    return cnt.value
+
+
+def direct_sum_points(pos, mass):
+    """Exact (phi, g) of point masses at arbitrary positions; pos [np][3], returns out [np][4].  O(N^2)."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    mass = np.ascontiguousarray(mass, dtype=np.float64)
+    out = np.zeros((len(mass), 4))
+    _check(lib().fmm_oracle_direct_sum_points(len(mass), _dp(pos), _dp(mass), _dp(out)), "direct_sum_points")
+    return out
+
+
+def solve_tree(n0, h0, theta, kind, mass, am_correction=True, coarsest=2):
+    """The gravity solve on an adaptive oct-tree of 8^3 sub-grids ("The FMM adapts naturally to an
+    oct-tree based adaptive mesh refinement"; L287-291; reading R9).  Level l = 0 .. len(kind)-1 is a dense
+    [n_l]^3 lattice, n_l = n0 2^l, h_l = h0 / 2^l, with kind[l] (0 absent, 1 leaf, 2 refined) and mass[l] (leaf masses);
+    above level 0 the uniform levels n0/2 .. `coarsest` as in solve().  Steps, in the paper's order (L125):
+      upward    leaf = point mass at its geometric centre; refined cell = M2M of its 8 children (leaf or refined);
+      downward  every existing cell: same-level step over its Eq. 15 list (two leaves excepted) + its parent's
+                expansion (L2L), the correction carried beside it;
+      leaves    phi = L0 + point-mass sums, g = -(L1 + correction) + point-mass sums, the sums being (a) the leaves of
+                its own level on the leaf-level list, (b) the children of the refined cells of its near field, (c) the
+                coarser leaves in the near field of its parent.
+    Returns (out, counts): out[l] = [4][n_l]^3 = (phi, g) at the leaf cells of level l (0 elsewhere);
+    counts = {"m2l": .., "p2p": .., "cross": .., and per tree level "m2l_levels", "p2p_levels", "cross_levels"} ordered pairs
+    ("m2l" includes the uniform levels above level 0)."""
+    D = len(kind)
+    n0 = int(n0)
+    kind = [np.ascontiguousarray(k, dtype=np.uint8) for k in kind]
+    mass = [np.ascontiguousarray(np.where(k == 1, m, 0.0), dtype=np.float64) for k, m in zip(kind, mass)]
+    ns = [n0 << l for l in range(D)]
+    hs = [float(h0) / (1 << l) for l in range(D)]
+    # ---- upward pass over the tree levels ----
+    mom, off = [None] * D, [None] * D
+    for l in range(D - 1, -1, -1):
+        n = ns[l]
+        m = np.zeros((20, n, n, n)); m[0] = mass[l]
+        o = np.zeros((3, n, n, n))
+        if l < D - 1:
+            pm, po = m2m((2 * n,) * 3, hs[l + 1], mom[l + 1], off[l + 1])
+            ref = kind[l] == 2
+            m = np.where(ref[None], pm, m)
+            o = np.where(ref[None], po, o)
+        mom[l], off[l] = np.ascontiguousarray(m), np.ascontiguousarray(o)
+    # ---- the uniform levels above level 0 ----
+    up_n, up_h, up_m, up_o = [n0], [hs[0]], [mom[0]], [off[0]]
+    while up_n[-1] > coarsest:
+        nc, hc = up_n[-1], up_h[-1]
+        pm, po = m2m((nc, nc, nc), hc, up_m[-1], up_o[-1])
+        up_n.append(nc // 2); up_h.append(2.0 * hc); up_m.append(pm); up_o.append(po)
+    counts = {"m2l": 0, "p2p": 0, "cross": 0, "m2l_levels": [], "p2p_levels": [], "cross_levels": []}
+    L_par = corr_par = off_par = None
+    for lv in range(len(up_n) - 1, 0, -1):
+        nl, hl = up_n[lv], up_h[lv]
+        Lf, Lc, c = interact_multipole((nl, nl, nl), hl, theta, up_m[lv], up_o[lv], None, None, am_correction)
+        counts["m2l"] += c
+        L = Lf.copy(); L[1:4] -= Lc
+        corr = Lc.copy()
+        if L_par is not None:
+            l2l((nl, nl, nl), hl, L_par, corr_par, off_par, up_o[lv], L, corr)
+        L_par, corr_par, off_par = L, corr, up_o[lv]
+    # ---- downward pass over the tree levels, leaves evaluated on the way ----
+    out = [None] * D
+    for l in range(D):
+        n, h = ns[l], hs[l]
+        Lf, Lc, c = tree_interact_multipole(n, h, theta, mom[l], off[l], kind[l], am_correction)
+        counts["m2l"] += c
+        counts["m2l_levels"].append(c)
+        L = Lf.copy(); L[1:4] -= Lc
+        corr = Lc.copy()
+        if L_par is not None:
+            l2l((n, n, n), h, L_par, corr_par, off_par, off[l], L, corr)
+        o, c = tree_leaf_p2p(n, h, theta, kind[l], mass[l])
+        counts["p2p"] += c
+        counts["p2p_levels"].append(c)
+        out[l] = o
+        L_par, corr_par, off_par = L, corr, off[l]
+        mom[l] = (L, corr)                         # kept for the leaf evaluation below
+    for l in range(D - 1):
+        c = tree_cross_level(ns[l], hs[l], theta, kind[l], mass[l], kind[l + 1], mass[l + 1], out[l], out[l + 1])
+        counts["cross"] += c
+        counts["cross_levels"].append(c)
+    for l in range(D):
+        L, corr = mom[l]
+        leaf = kind[l] == 1
+        out[l][0] += np.where(leaf, L[0], 0.0)
+        out[l][1:4] -= np.where(leaf[None], L[1:4] + corr, 0.0)
+    return out, counts

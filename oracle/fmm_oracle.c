@@ -315,9 +315,12 @@ static void free_stencils(stencil_set *S) { for (int p = 0; p < 8; ++p) free(S->
  * L gets the correction folded into L1 when enabled; Lcorr (may be NULL) gets it alone.
  * n_interactions (may be NULL) receives the number of ordered in-domain pairs.
  */
+enum { TREE_ABSENT = 0, TREE_LEAF = 1, TREE_REFINED = 2 };   /* kind of a cell on one level of an adaptive tree */
+
 static int interact_multipole_impl(const int n[3], const int out_lo[3], const int out_hi[3], double h,
                                    double theta, int am_correction, const double *moments,
-                                   const double *com_off, const unsigned char *leaf, double *L, double *Lcorr,
+                                   const double *com_off, const unsigned char *leaf, const unsigned char *kind,
+                                   double *L, double *Lcorr,
                                    double *Labs, unsigned long long *n_interactions)
 {
     if (!n || !out_lo || !out_hi || !moments || !com_off || !L || !(h > 0.0)) return ORC_EINVAL;
@@ -346,14 +349,18 @@ static int interact_multipole_impl(const int n[3], const int out_lo[3], const in
                 double MA3[10], MA0 = moments[a], dA[3];
                 for (int c = 0; c < 10; ++c) MA3[c] = moments[(size_t)(10 + c) * ncell + a];
                 for (int c = 0; c < 3; ++c) dA[c] = com_off[(size_t)c * ncell + a];
-                if (am_correction && !(MA0 > 0.0)) bad_mass |= 1;
+                const int absent = kind && kind[a] == TREE_ABSENT;     /* adaptive tree: no such cell on this level */
+                if (am_correction && !(MA0 > 0.0) && !absent) bad_mass |= 1;
 
-                for (int s = 0; s < S.count[p]; ++s) {
+                for (int s = 0; s < S.count[p] && !absent; ++s) {
                     const int dx = S.d[p][3 * s], dy = S.d[p][3 * s + 1], dz = S.d[p][3 * s + 2];
                     const int bi = i + dx, bj = j + dy, bk = k + dz;
                     if (bi < 0 || bj < 0 || bk < 0 || bi >= (int)nx || bj >= (int)ny || bk >= (int)nz) continue;
                     const size_t b = ((size_t)bk * ny + bj) * nx + bi;
                     if (leaf && !leaf[a] && !leaf[b] && !is_partner_mode(i & 1, j & 1, k & 1, dx, dy, dz, theta, 0)) continue;
+                    /* adaptive tree (fmm_oracle_tree_interact_multipole): B must exist, and two leaf cells meet as point
+                     * masses in fmm_oracle_tree_leaf_p2p instead */
+                    if (kind && (kind[b] == TREE_ABSENT || (kind[a] == TREE_LEAF && kind[b] == TREE_LEAF))) continue;
                     double MB[20], R[3], term[20], cterm[3];
                     for (int c = 0; c < 20; ++c) MB[c] = moments[(size_t)c * ncell + b];
                     R[0] = (double)(i - bi) * h + (dA[0] - com_off[0 * ncell + b]);
@@ -387,7 +394,7 @@ int fmm_oracle_interact_multipole(const int n[3], const int out_lo[3], const int
                                   const double *com_off, double *L, double *Lcorr,
                                   unsigned long long *n_interactions)
 {
-    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, L, Lcorr, NULL, n_interactions);
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, NULL, L, Lcorr, NULL, n_interactions);
 }
 
 /*
@@ -404,7 +411,7 @@ int fmm_oracle_interact_multipole_cond(const int n[3], const int out_lo[3], cons
                                        unsigned long long *n_interactions)
 {
     if (!Labs) return ORC_EINVAL;
-    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, L, Lcorr, Labs, n_interactions);
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, NULL, NULL, L, Lcorr, Labs, n_interactions);
 }
 
 /*
@@ -422,7 +429,7 @@ int fmm_oracle_interact_multipole_mixed(const int n[3], const int out_lo[3], con
                                         unsigned long long *n_interactions)
 {
     if (!leaf) return ORC_EINVAL;
-    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, leaf, L, Lcorr, NULL, n_interactions);
+    return interact_multipole_impl(n, out_lo, out_hi, h, theta, am_correction, moments, com_off, leaf, NULL, L, Lcorr, NULL, n_interactions);
 }
 
 /*
@@ -432,7 +439,7 @@ int fmm_oracle_interact_multipole_mixed(const int n[3], const int out_lo[3], con
  * out = [4][oz][oy][ox] = (phi, gx, gy, gz).
  */
 static int interact_monopole_mode(const int n[3], const int out_lo[3], const int out_hi[3], double h,
-                                  double theta, int leaf, const double *mass, double *out,
+                                  double theta, int leaf, const unsigned char *kind, const double *mass, double *out,
                                   unsigned long long *n_interactions)
 {
     if (!n || !out_lo || !out_hi || !mass || !out || !(h > 0.0)) return ORC_EINVAL;
@@ -450,9 +457,12 @@ static int interact_monopole_mode(const int n[3], const int out_lo[3], const int
             for (int i = out_lo[0]; i < out_hi[0]; ++i) {
                 const int p = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
                 long double acc[4] = {0.0L, 0.0L, 0.0L, 0.0L};
-                for (int s = 0; s < S.count[p]; ++s) {
+                /* adaptive tree (fmm_oracle_tree_leaf_p2p): only leaf cells are point masses, as targets and as sources */
+                const int skip = kind && kind[((size_t)k * ny + j) * nx + i] != TREE_LEAF;
+                for (int s = 0; s < S.count[p] && !skip; ++s) {
                     const int bi = i + S.d[p][3 * s], bj = j + S.d[p][3 * s + 1], bk = k + S.d[p][3 * s + 2];
                     if (bi < 0 || bj < 0 || bk < 0 || bi >= (int)nx || bj >= (int)ny || bk >= (int)nz) continue;
+                    if (kind && kind[((size_t)bk * ny + bj) * nx + bi] != TREE_LEAF) continue;
                     const double m = mass[((size_t)bk * ny + bj) * nx + bi];
                     double R[3] = {(double)(i - bi) * h, (double)(j - bj) * h, (double)(k - bk) * h};
                     double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2];
@@ -473,14 +483,14 @@ int fmm_oracle_interact_monopole(const int n[3], const int out_lo[3], const int 
                                  double theta, const double *mass, double *out,
                                  unsigned long long *n_interactions)
 {
-    return interact_monopole_mode(n, out_lo, out_hi, h, theta, 0, mass, out, n_interactions);
+    return interact_monopole_mode(n, out_lo, out_hi, h, theta, 0, NULL, mass, out, n_interactions);
 }
 /* the same sum over the leaf-level list of the complete solve (Eq. 15 list + near field) */
 int fmm_oracle_interact_monopole_leaf(const int n[3], const int out_lo[3], const int out_hi[3], double h,
                                       double theta, const double *mass, double *out,
                                       unsigned long long *n_interactions)
 {
-    return interact_monopole_mode(n, out_lo, out_hi, h, theta, 1, mass, out, n_interactions);
+    return interact_monopole_mode(n, out_lo, out_hi, h, theta, 1, NULL, mass, out, n_interactions);
 }
 
 /* Number of ordered in-domain pairs for a region, by enumeration on the index grid. */
@@ -708,6 +718,160 @@ int fmm_oracle_direct_sum(const int n[3], double h, const double *mass, double *
             for (int c = 0; c < 3; ++c) acc[1 + c] += (long double)(-m * R[c] / (r2 * r));
         }
         for (int c = 0; c < 4; ++c) out[(size_t)c * nc + a] = (double)acc[c];
+    }
+    return ORC_OK;
+}
+
+
+/* ====================================================================================== */
+/* NEXT f3: the gravity solve on an ADAPTIVE oct-tree of 8^3 sub-grids.       */
+/* PAPER.md L125 ("The FMM adapts naturally to an oct-tree based adaptive mesh refinement"),*/
+/* L287-291 (a node "is either fully refined with eight child nodes (an interior node) or   */
+/* not refined at all (a leaf node)"; the mesh is properly nested, so a refinement boundary */
+/* involves exactly two levels).  The paper does not describe the gravity side of such a    */
+/* boundary; reading R9 takes the rule the paper does give (L135: well-separated  */
+/* cells interact at the level where their parents are not well separated; what is not well */
+/* separated is left to the children, L456) and applies it as a symmetric dual descent:      */
+/*   pair (A, B) of one level whose parents are not well separated --                        */
+/*     well separated            : they interact here, with the general pair formula; a leaf */
+/*                                 is the point mass M0 = m, M1 = M2 = M3 = 0, delta = 0     */
+/*                                 (two leaves: that formula IS the point-mass sum, and it   */
+/*                                 is taken as such in fmm_oracle_tree_leaf_p2p);            */
+/*     not, both refined         : left to their children;                                   */
+/*     not, both leaves          : point masses, directly (fmm_oracle_tree_leaf_p2p);        */
+/*     not, A leaf and B refined : A meets the eight CHILDREN of B, which proper nesting     */
+/*                                 makes leaves one level down: point masses, directly, in   */
+/*                                 both directions (fmm_oracle_tree_cross_level).            */
+/* Every pair is taken exactly once in each direction with antisymmetric forces, so linear   */
+/* momentum -- and with the correction angular momentum -- is conserved as on a uniform grid */
+/* (L125, L127), and a fully refined tree is the uniform solve, term by term.                */
+/* A level is a dense n^3 array with kind[cell] = TREE_ABSENT / TREE_LEAF / TREE_REFINED.    */
+/* ====================================================================================== */
+
+/* the same-level multipole step on one level of the tree: targets = cells that exist; partners = cells of the Eq. 15
+ * list that exist, except that two leaves do not meet here.  L (correction folded in) and Lcorr as in
+ * fmm_oracle_interact_multipole; absent targets get zeros. */
+int fmm_oracle_tree_interact_multipole(const int n[3], double h, double theta, int am_correction,
+                                       const double *moments, const double *com_off, const unsigned char *kind,
+                                       double *L, double *Lcorr, unsigned long long *n_interactions)
+{
+    if (!kind) return ORC_EINVAL;
+    const int lo[3] = {0, 0, 0};
+    return interact_multipole_impl(n, lo, n, h, theta, am_correction, moments, com_off, NULL, kind, L, Lcorr, NULL, n_interactions);
+}
+
+/* point-mass sum of the leaf cells of one level over the leaf-level list (Eq. 15 list + near field): targets and sources
+ * are the cells with kind == TREE_LEAF.  out = [4][nz][ny][nx] = (phi, g); other targets get zeros. */
+int fmm_oracle_tree_leaf_p2p(const int n[3], double h, double theta, const unsigned char *kind, const double *mass,
+                             double *out, unsigned long long *n_interactions)
+{
+    if (!kind) return ORC_EINVAL;
+    const int lo[3] = {0, 0, 0};
+    return interact_monopole_mode(n, lo, n, h, theta, 1, kind, mass, out, n_interactions);
+}
+
+/*
+ * The pairs across a refinement boundary.  Coarse level: nc^3-type grid of width hc with kind_c, mass_c; fine level:
+ * (2 nc)-type grid of width hc / 2 with kind_f, mass_f.  For every coarse LEAF A and every cell B of its near field (the
+ * leaf-level list minus the Eq. 15 list: not well separated, parents not well separated either) that is REFINED, A and
+ * each of the 8 children b of B are point masses at their geometric centres:
+ *   x_A - x_b = ((double)(2 i_A - i_b) + 0.5) * (hc / 2)      per axis, in this operation order,
+ *   out_c[A] += (-m_b / r, -m_b R / r^3),    out_f[b] += (-m_A / r, +m_A R / r^3)   (R = x_A - x_b).
+ * A child that is not a leaf means the tree is not properly nested: ORC_EINVAL.  Both outputs are ADDED to
+ * ([4][...], long double sums per target in list order, then child order).  n_pairs counts ordered pairs.
+ */
+int fmm_oracle_tree_cross_level(const int nc[3], double hc, double theta, const unsigned char *kind_c, const double *mass_c,
+                                const unsigned char *kind_f, const double *mass_f, double *out_c, double *out_f,
+                                unsigned long long *n_pairs)
+{
+    if (!nc || !kind_c || !mass_c || !kind_f || !mass_f || !out_c || !out_f || !(hc > 0.0)) return ORC_EINVAL;
+    stencil_set S;
+    if (build_stencils_mode(theta, 1, &S) != ORC_OK) return ORC_EINVAL;
+    const long cx = nc[0], cy = nc[1], cz = nc[2], ccell = cx * cy * cz;
+    const long fx = 2 * cx, fy = 2 * cy, fz = 2 * cz, fcell = fx * fy * fz;
+    const double hf = 0.5 * hc;
+    unsigned long long total = 0;
+    int bad = 0;
+    /* coarse leaf targets */
+#pragma omp parallel for collapse(2) schedule(dynamic, 1) reduction(+ : total) reduction(| : bad)
+    for (long k = 0; k < cz; ++k)
+        for (long j = 0; j < cy; ++j)
+            for (long i = 0; i < cx; ++i) {
+                const long a = (k * cy + j) * cx + i;
+                if (kind_c[a] != TREE_LEAF) continue;
+                const int p = (int)((i & 1) + 2 * (j & 1) + 4 * (k & 1));
+                long double acc[4] = {0.0L, 0.0L, 0.0L, 0.0L};
+                for (int s = 0; s < S.count[p]; ++s) {
+                    const int dx = S.d[p][3 * s], dy = S.d[p][3 * s + 1], dz = S.d[p][3 * s + 2];
+                    if (well_separated((long)dx * dx + (long)dy * dy + (long)dz * dz, theta)) continue;   /* Eq. 15 list: same level */
+                    const long bi = i + dx, bj = j + dy, bk = k + dz;
+                    if (bi < 0 || bj < 0 || bk < 0 || bi >= cx || bj >= cy || bk >= cz) continue;
+                    if (kind_c[(bk * cy + bj) * cx + bi] != TREE_REFINED) continue;
+                    for (int c = 0; c < 8; ++c) {
+                        const long ci = 2 * bi + (c & 1), cj = 2 * bj + ((c >> 1) & 1), ck = 2 * bk + (c >> 2);
+                        const long b = (ck * fy + cj) * fx + ci;
+                        if (kind_f[b] != TREE_LEAF) { bad |= 1; continue; }
+                        const double R[3] = {((double)(2 * i - ci) + 0.5) * hf, ((double)(2 * j - cj) + 0.5) * hf,
+                                             ((double)(2 * k - ck) + 0.5) * hf};
+                        const double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2], r = sqrt(r2), m = mass_f[b];
+                        acc[0] += (long double)(-m / r);
+                        for (int x = 0; x < 3; ++x) acc[1 + x] += (long double)(-m * R[x] / (r2 * r));
+                        ++total;
+                    }
+                }
+                for (int x = 0; x < 4; ++x) out_c[(long)x * ccell + a] += (double)acc[x];
+            }
+    /* fine leaf targets: the coarse leaves in the near field of their (refined) parent */
+#pragma omp parallel for collapse(2) schedule(dynamic, 1) reduction(+ : total)
+    for (long k = 0; k < fz; ++k)
+        for (long j = 0; j < fy; ++j)
+            for (long i = 0; i < fx; ++i) {
+                const long b = (k * fy + j) * fx + i;
+                if (kind_f[b] != TREE_LEAF) continue;
+                const long pi = i / 2, pj = j / 2, pk = k / 2;
+                const int p = (int)((pi & 1) + 2 * (pj & 1) + 4 * (pk & 1));
+                long double acc[4] = {0.0L, 0.0L, 0.0L, 0.0L};
+                for (int s = 0; s < S.count[p]; ++s) {
+                    const int dx = S.d[p][3 * s], dy = S.d[p][3 * s + 1], dz = S.d[p][3 * s + 2];
+                    if (well_separated((long)dx * dx + (long)dy * dy + (long)dz * dz, theta)) continue;
+                    const long ai = pi + dx, aj = pj + dy, ak = pk + dz;
+                    if (ai < 0 || aj < 0 || ak < 0 || ai >= cx || aj >= cy || ak >= cz) continue;
+                    const long a = (ak * cy + aj) * cx + ai;
+                    if (kind_c[a] != TREE_LEAF) continue;
+                    /* R = x_b - x_A = -(x_A - x_b), the latter formed as above */
+                    const double R[3] = {-(((double)(2 * ai - i) + 0.5) * hf), -(((double)(2 * aj - j) + 0.5) * hf),
+                                         -(((double)(2 * ak - k) + 0.5) * hf)};
+                    const double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2], r = sqrt(r2), m = mass_c[a];
+                    acc[0] += (long double)(-m / r);
+                    for (int x = 0; x < 3; ++x) acc[1 + x] += (long double)(-m * R[x] / (r2 * r));
+                    ++total;
+                }
+                for (int x = 0; x < 4; ++x) out_f[(long)x * fcell + b] += (double)acc[x];
+            }
+    free_stencils(&S);
+    if (n_pairs) *n_pairs = total;
+    return bad ? ORC_EINVAL : ORC_OK;
+}
+
+/*
+ * Exact sum over point masses at arbitrary positions (the leaves of a tree, whatever their level):
+ * phi_a = -sum_{b != a} m_b / |x_a - x_b|,  g_a = -sum m_b (x_a - x_b) / |x_a - x_b|^3.  pos = [np][3], out = [np][4].
+ * O(N^2): the exact result the tree solve approximates, for the pins.
+ */
+int fmm_oracle_direct_sum_points(long np, const double *pos, const double *mass, double *out)
+{
+    if (np < 0 || !pos || !mass || !out) return ORC_EINVAL;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (long a = 0; a < np; ++a) {
+        long double acc[4] = {0.0L, 0.0L, 0.0L, 0.0L};
+        for (long b = 0; b < np; ++b) {
+            if (b == a) continue;
+            const double R[3] = {pos[3 * a] - pos[3 * b], pos[3 * a + 1] - pos[3 * b + 1], pos[3 * a + 2] - pos[3 * b + 2]};
+            const double r2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2], r = sqrt(r2);
+            acc[0] += (long double)(-mass[b] / r);
+            for (int x = 0; x < 3; ++x) acc[1 + x] += (long double)(-mass[b] * R[x] / (r2 * r));
+        }
+        for (int x = 0; x < 4; ++x) out[4 * a + x] = (double)acc[x];
     }
     return ORC_OK;
 }
