@@ -254,6 +254,58 @@ int octo_fmm_solver_get_leaf_stencil(const octo_fmm_solver_t *s, int parity, int
 /* Number of multipole levels (n/2 ... 2) and of kernels one solve launches. */
 int octo_fmm_solver_num_levels(const octo_fmm_solver_t *s, int *multipole_levels, int *launches_per_solve);
 
+/* ---- the solve on an ADAPTIVE oct-tree of 8^3 sub-grids -------------------------
+ * "The FMM adapts naturally to an oct-tree based adaptive mesh refinement"; a node "is either
+ * fully refined with eight child nodes (an interior node) or not refined at all (a leaf node)" and the mesh is
+ * properly nested, so that a refinement boundary involves exactly two levels (L287-291).  The paper does not
+ * describe the gravity side of such a boundary; the reading taken (R9) applies the rule of
+ * L135 as a symmetric dual descent: a pair of one level whose parents are not well separated
+ *   - is well separated (Eq. 15): interacts on that level with the general pair formula, whatever the kinds of
+ *     the two cells (a leaf is the point mass M0 = m, M1 = M2 = M3 = 0, delta = 0; two leaves: the point-mass sum);
+ *   - is not, both refined: left to the children;  both leaves: point masses, directly;
+ *   - is not, A leaf and B refined: A meets the eight CHILDREN of B -- leaves one level down by proper nesting --
+ *     as point masses, in both directions:  x_A - x_b = ((double)(2 i_A - i_b) + 0.5) * (h_A / 2) per axis.
+ * Every pair is taken once in each direction with antisymmetric forces: linear momentum, and with the correction
+ * angular momentum, are conserved as on a uniform grid (L125, L127); a fully refined tree IS the uniform solve.
+ *
+ * Layout: tree level l = 0 .. depth-1 is a dense lattice [n_l][n_l][n_l], n_l = n0 2^l, h_l = h0 / 2^l, x fastest.
+ * kind[l] (uint8, HOST memory, read at create() only): 0 the cell does not exist on this level, 1 leaf, 2 refined;
+ * constant over every aligned 8^3 sub-grid; every cell of level 0 exists; a cell exists on level l+1 iff its parent
+ * is refined; no refined cell on the last level (else EINVAL).  Proper nesting over the 26 neighbours of a sub-grid
+ * is the caller's duty (a leaf next to a sub-grid two levels finer is not detected).  Above level 0 the uniform
+ * levels n0/2 .. 2 are built by the library.
+ * mass[l]: DEVICE [n_l^3], read at the leaf cells only; out[l]: DEVICE [4][n_l^3] = (phi, g_x, g_y, g_z) at the
+ * leaf cells, zeros elsewhere.  mass and out are HOST arrays of `depth` device pointers, all 16-byte aligned.
+ * The caller lends the workspace; everything is enqueued on cfg.stream; create() synchronises the stream once (it
+ * uploads the topology from pageable memory).  One handle is not thread-safe. */
+typedef struct octo_fmm_tree octo_fmm_tree_t;
+typedef struct {
+    int n0;                 /* cells per axis of level 0: a power of two, 8 <= n0, n0 2^(depth-1) <= 2048      */
+    int depth;              /* number of tree levels, 1..10                                                    */
+    double h0;              /* cell width of level 0                                                           */
+    double theta;           /* opening angle, 1/3 < theta < 1                                                  */
+    int am_correction;      /* 0/1 (L127)                                                                      */
+    int device;
+    void *stream;           /* cudaStream_t, borrowed                                                          */
+    void *workspace;        /* device memory, 256-byte aligned, borrowed for the handle's lifetime             */
+    size_t workspace_bytes; /* >= octo_fmm_tree_workspace_bytes(cfg, kind_host)                                */
+} octo_fmm_tree_config;
+
+size_t octo_fmm_tree_workspace_bytes(const octo_fmm_tree_config *cfg, const unsigned char *const *kind_host); /* 0 if invalid */
+int octo_fmm_tree_create(const octo_fmm_tree_config *cfg, const unsigned char *const *kind_host, octo_fmm_tree_t **out);
+/* Asynchronous on the stream. */
+int octo_fmm_tree_solve(octo_fmm_tree_t *t, const double *const *mass, double *const *out);
+/* The same solve, and the ordered pairs it evaluates, counted on the device for the bit-exact check of the pair set:
+ * counts[0] multipole pairs of all levels (uniform levels included), counts[1] leaf-leaf point-mass pairs of one
+ * level, counts[2] point-mass pairs across a refinement boundary.  Synchronises the stream. */
+int octo_fmm_tree_interaction_counts(octo_fmm_tree_t *t, const double *const *mass, double *const *out,
+                                     unsigned long long counts[3]);
+/* Synchronises the stream; OCTO_FMM_EMASS if the correction met an existing cell of mass <= 0. */
+int octo_fmm_tree_status(octo_fmm_tree_t *t);
+/* Kernels one solve launches. */
+int octo_fmm_tree_launches(const octo_fmm_tree_t *t, int *launches);
+int octo_fmm_tree_destroy(octo_fmm_tree_t *t);
+
 #ifdef __cplusplus
 }
 #endif

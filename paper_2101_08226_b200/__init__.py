@@ -34,6 +34,12 @@ class octo_fmm_config(ctypes.Structure):
                 ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
 
 
+class octo_fmm_tree_config(ctypes.Structure):
+    _fields_ = [("n0", ctypes.c_int), ("depth", ctypes.c_int), ("h0", ctypes.c_double), ("theta", ctypes.c_double),
+                ("am_correction", ctypes.c_int), ("device", ctypes.c_int), ("stream", ctypes.c_void_p),
+                ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
+
+
 class octo_fmm_solver_config(ctypes.Structure):
     _fields_ = [("n", ctypes.c_int), ("h", ctypes.c_double), ("theta", ctypes.c_double), ("am_correction", ctypes.c_int),
                 ("device", ctypes.c_int), ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p),
@@ -80,6 +86,16 @@ class _Library:
         lib.octo_fmm_flops_per_interaction_path.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, ip]
         lib.octo_fmm_dipole_terms_used.argtypes = [vp, ip]
         lib.octo_fmm_version.restype = ctypes.c_char_p
+        tcfgp = ctypes.POINTER(octo_fmm_tree_config)
+        vpp = ctypes.POINTER(ctypes.c_void_p)
+        lib.octo_fmm_tree_workspace_bytes.restype = ctypes.c_size_t
+        lib.octo_fmm_tree_workspace_bytes.argtypes = [tcfgp, vpp]
+        lib.octo_fmm_tree_create.argtypes = [tcfgp, vpp, ctypes.POINTER(vp)]
+        lib.octo_fmm_tree_solve.argtypes = [vp, vpp, vpp]
+        lib.octo_fmm_tree_interaction_counts.argtypes = [vp, vpp, vpp, ctypes.POINTER(ctypes.c_ulonglong)]
+        lib.octo_fmm_tree_status.argtypes = [vp]
+        lib.octo_fmm_tree_launches.argtypes = [vp, ip]
+        lib.octo_fmm_tree_destroy.argtypes = [vp]
         scfgp = ctypes.POINTER(octo_fmm_solver_config)
         lib.octo_fmm_solver_workspace_bytes.restype = ctypes.c_size_t
         lib.octo_fmm_solver_workspace_bytes.argtypes = [scfgp]
@@ -467,6 +483,134 @@ class OctoFMMSolver:
     def close(self):
         if getattr(self, "handle", None) is not None:
             octo_fmm_solver_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+# ---- the solve on an adaptive oct-tree of 8^3 sub-grids (octo_fmm_tree_*) ----------------------
+def make_tree_config(n0, depth, h0, theta, am_correction=True, device=0, stream=0, workspace=0, workspace_bytes=0):
+    c = octo_fmm_tree_config()
+    c.n0, c.depth, c.h0, c.theta, c.am_correction = int(n0), int(depth), float(h0), float(theta), int(bool(am_correction))
+    c.device, c.stream, c.workspace, c.workspace_bytes = int(device), stream or None, workspace or None, int(workspace_bytes)
+    return c
+
+
+def _ptr_array(items):
+    """A C array of void* from tensors / arrays / raw addresses (the per-level pointer tables of the tree calls)."""
+    arr = (ctypes.c_void_p * len(items))()
+    for i, t in enumerate(items):
+        arr[i] = t if isinstance(t, int) else _ptr(t)
+    return arr
+
+
+def octo_fmm_tree_workspace_bytes(cfg, kind_host):
+    return int(_lib.octo_fmm_tree_workspace_bytes(ctypes.byref(cfg), _ptr_array(kind_host)))
+
+
+def octo_fmm_tree_create(cfg, kind_host):
+    h = _vp()
+    rc = _lib.octo_fmm_tree_create(ctypes.byref(cfg), _ptr_array(kind_host), ctypes.byref(h))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_tree_create", rc)
+    return h
+
+
+def octo_fmm_tree_solve(t, mass, out):
+    rc = _lib.octo_fmm_tree_solve(t, _ptr_array(mass), _ptr_array(out))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_tree_solve", rc)
+
+
+def octo_fmm_tree_interaction_counts(t, mass, out):
+    c = (ctypes.c_ulonglong * 3)()
+    rc = _lib.octo_fmm_tree_interaction_counts(t, _ptr_array(mass), _ptr_array(out), c)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_tree_interaction_counts", rc)
+    return {"m2l": int(c[0]), "p2p": int(c[1]), "cross": int(c[2])}
+
+
+def octo_fmm_tree_status(t):
+    return int(_lib.octo_fmm_tree_status(t))
+
+
+def octo_fmm_tree_launches(t):
+    n = ctypes.c_int(0)
+    rc = _lib.octo_fmm_tree_launches(t, ctypes.byref(n))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_tree_launches", rc)
+    return n.value
+
+
+def octo_fmm_tree_destroy(t):
+    rc = _lib.octo_fmm_tree_destroy(t)
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_tree_destroy", rc)
+
+
+class OctoFMMTree:
+    """Owns the workspace tensor and the handle of a solve on an adaptive tree.  kind: list of numpy uint8 arrays
+    [n_l]^3 (host; 0 absent, 1 leaf, 2 refined), one per level."""
+
+    def __init__(self, n0, h0, theta, kind, am_correction=True, device=0, stream=None):
+        import numpy as np
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("octo_fmm needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.torch = torch
+        self.n0, self.depth = int(n0), len(kind)
+        self.device = torch.device("cuda", device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.kind = [np.ascontiguousarray(k, dtype=np.uint8) for k in kind]
+        for l, k in enumerate(self.kind):
+            if k.shape != (self.n0 << l,) * 3:
+                raise ValueError("octo_fmm: kind[%d] must have shape %s" % (l, ((self.n0 << l,) * 3,)))
+        cfg = make_tree_config(n0, self.depth, h0, theta, am_correction, device=device, stream=self.stream.cuda_stream)
+        nbytes = octo_fmm_tree_workspace_bytes(cfg, self.kind)
+        if nbytes == 0:
+            raise OctoFmmError("octo_fmm_tree_workspace_bytes", EINVAL)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        cfg.workspace, cfg.workspace_bytes = self.workspace.data_ptr(), nbytes
+        self.cfg = cfg
+        self.handle = octo_fmm_tree_create(cfg, self.kind)
+
+    def n(self, l):
+        return self.n0 << l
+
+    def _check(self, mass, out):
+        if len(mass) != self.depth or len(out) != self.depth:
+            raise ValueError("octo_fmm: one mass and one out tensor per level")
+        for l in range(self.depth):
+            _check_device_tensor(mass[l], "mass[%d]" % l, self.torch.float64, self.n(l) ** 3, self.device, self.stream)
+            _check_device_tensor(out[l], "out[%d]" % l, self.torch.float64, 4 * self.n(l) ** 3, self.device, self.stream)
+
+    def empty_out(self):
+        return [self.torch.empty((4,) + (self.n(l),) * 3, dtype=self.torch.float64, device=self.device) for l in range(self.depth)]
+
+    def solve(self, mass, out=None):
+        out = self.empty_out() if out is None else out
+        self._check(mass, out)
+        octo_fmm_tree_solve(self.handle, mass, out)
+        return out
+
+    def interaction_counts(self, mass, out=None):
+        out = self.empty_out() if out is None else out
+        self._check(mass, out)
+        return octo_fmm_tree_interaction_counts(self.handle, mass, out), out
+
+    def status(self):
+        return octo_fmm_tree_status(self.handle)
+
+    def launches(self):
+        return octo_fmm_tree_launches(self.handle)
+
+    def close(self):
+        if getattr(self, "handle", None) is not None:
+            octo_fmm_tree_destroy(self.handle)
             self.handle = None
 
     def __del__(self):

@@ -83,6 +83,8 @@ struct Params {
     double hc;               // width of this level's cells
     const unsigned char* leaf;   // mixed level (m2l_staged_kernel<., ., true>): [nz][ny][nx], 1 = leaf cell
     double hmul[2 * REACH_MAX + 1];   // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h), per handle
+    const int* tile_list;        // levels of an adaptive tree: the bricks (ids in the dense enumeration) that have work;
+                                 // nullptr = all ntiles bricks.  With a list, ntiles is its length.
 };
 
 // ------------------------------------------------------------------------------------------
@@ -131,7 +133,7 @@ __global__ void __launch_bounds__(256) stage_leaf_flags_kernel(const unsigned ch
     const int y = (int)(r % ny), z = (int)(r / ny);
     const long long plane = (long long)ny * nx;
     double2* dst = reinterpret_cast<double2*>(S) + ((long long)z * NPAIR + (NPAIR - 1)) * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1);
-    dst->y = leaf[cell] ? 1.0 : 0.0;
+    dst->y = leaf[cell] == 1 ? 1.0 : 0.0;       // mixed level: 0 / 1; tree level: the cell's kind, 1 = leaf
 }
 
 // ------------------------------------------------------------------------------------------
@@ -194,6 +196,7 @@ __device__ __forceinline__ void tma_load_slab(void* dst, const CUtensorMap* map,
 // columns and share their slabs through L2.
 __device__ __forceinline__ void decode_tile(const Params& p, long long t, int& x0, int& y0, int& k0)
 {
+    if (p.tile_list) t = p.tile_list[t];
     k0 = p.kb + (int)(t % p.tiles_z) * TILE_Z;
     const long long c = t / p.tiles_z;
     x0 = p.lo[0] + (int)(c % p.tiles_x) * TILE_X;
@@ -294,10 +297,14 @@ __device__ __forceinline__ void store_target(const Params& p, const Acc& acc, co
 
 // The consumer warps' loop over the bricks of this CTA.  DIPOLE = false is the fast path for sources
 // expanded about their centre of mass (no dipole terms), see m2l_staged_kernel.
-// MIXED (one level of an adaptive mesh, f3): the lists are the leaf-level lists (Eq. 15 + near field); a near-field entry
-// counts only if the target or the partner is a leaf cell -- otherwise the pair's 1/r is set to 0, and since every term of
-// the pair carries a power of 1/r it contributes exactly nothing.
-template <bool CORR, bool DIPOLE, bool FUSE_L2L, bool MIXED>
+// MODE_MIXED (one level of an adaptive mesh, f3 reading R8): the lists are the leaf-level lists (Eq. 15 + near field); a
+// near-field entry counts only if the target or the partner is a leaf cell -- otherwise the pair's 1/r is set to 0, and
+// since every term of the pair carries a power of 1/r it contributes exactly nothing.
+// MODE_TREE (a level of the adaptive tree solve, f3 reading R9): p.leaf holds the KIND of every cell (0 absent, 1 leaf,
+// 2 refined); absent cells are no targets (as sources their staged record is all zeros), and two leaves do not meet here
+// (they are point masses: the tensor-core leaf kernel takes them), again through 1/r = 0.
+constexpr int MODE_PLAIN = 0, MODE_MIXED = 1, MODE_TREE = 2;
+template <bool CORR, bool DIPOLE, bool FUSE_L2L, int MODE>
 __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, uint64_t* full, uint64_t* empty, int warp, int lane)
 {
     // ------------------------------ consumers ------------------------------
@@ -320,9 +327,15 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         const int z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.nz - 1);
 
         double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-        if (active) load_target<CORR>(p, gx, gy, k, dA, tA);
         bool leafA = false;
-        if (MIXED && active) leafA = p.leaf[((long long)k * p.ny + gy) * p.nx + gx] != 0;
+        bool present = active;                             // MODE_TREE: the cell exists on this level
+        if (MODE == MODE_MIXED && active) leafA = p.leaf[((long long)k * p.ny + gy) * p.nx + gx] != 0;
+        if (MODE == MODE_TREE && active) {
+            const unsigned char kd = p.leaf[((long long)k * p.ny + gy) * p.nx + gx];
+            leafA = kd == 1;
+            present = kd != 0;
+        }
+        if (present) load_target<CORR>(p, gx, gy, k, dA, tA);
 
         Acc acc;
         acc_zero(acc);
@@ -366,13 +379,14 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
             const StEntry e_ = c_entries[s];                                                \
             ++s;                                                                            \
             double bx_, by_, bz_, fl_ = 0.0;                                                \
-            if (MIXED) { OCTO_LOAD_SOURCE_F(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
+            if (MODE != MODE_PLAIN) { OCTO_LOAD_SOURCE_F(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
             else       { OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_); }  \
             P.x = p.hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                                \
             P.y = p.hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                                \
             P.z = Rz0 - bz_;                                                                \
             P.w = pair_head(P.x, P.y, P.z);                                                 \
-            if (MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;                          \
+            if (MODE == MODE_MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;             \
+            if (MODE == MODE_TREE && leafA && fl_ != 0.0) P.w = 0.0;                        \
         }
         struct Fetched { double src[16]; double x, y, z, w; } A, B;
         if (ensure()) {
@@ -389,11 +403,11 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         }
 #undef OCTO_FETCH
 
-        if (active) store_target<CORR, FUSE_L2L>(p, acc, tA, dA, gx, gy, k);
+        if (present) store_target<CORR, FUSE_L2L>(p, acc, tA, dA, gx, gy, k);
     }
 }
 
-template <bool CORR, bool FUSE_L2L = false, bool MIXED = false>
+template <bool CORR, bool FUSE_L2L = false, int MODE = MODE_PLAIN>
 __global__ void __launch_bounds__(STAGED_THREADS, 1)
 m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ Params p)
 {
@@ -440,8 +454,8 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     // the flags if any cell has |M1_i| > DIPOLE_TOL |M| h, and only then (or when the caller forces it) the
     // 27 dipole terms are evaluated.  The branch is uniform over the grid.
     const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
-    if (dipole) staged_consume<CORR, true, FUSE_L2L, MIXED>(p, slab0, full, empty, warp, lane);
-    else        staged_consume<CORR, false, FUSE_L2L, MIXED>(p, slab0, full, empty, warp, lane);
+    if (dipole) staged_consume<CORR, true, FUSE_L2L, MODE>(p, slab0, full, empty, warp, lane);
+    else        staged_consume<CORR, false, FUSE_L2L, MODE>(p, slab0, full, empty, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -831,7 +845,7 @@ p2p_monopole_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params 
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
     const int bx = (p.ox + MT_X - 1) / MT_X, by = (p.oy + MT_Y - 1) / MT_Y;
-    const int b = blockIdx.x;
+    const int b = p.tile_list ? p.tile_list[blockIdx.x] : blockIdx.x;       // tree levels: only the tiles that hold leaf cells
     const int x0 = p.lo[0] + (b % bx) * MT_X, y0 = p.lo[1] + ((b / bx) % by) * MT_Y, z0 = p.lo[2] + (b / (bx * by)) * DT_Z;
 
     if (threadIdx.x == 0) {

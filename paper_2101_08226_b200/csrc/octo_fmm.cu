@@ -18,6 +18,7 @@
 #include "../../include/octo_fmm.h"
 #include "kernels.cuh"
 #include "solver.cuh"
+#include "tree.cuh"
 
 using namespace octo;
 
@@ -291,6 +292,10 @@ struct octo_fmm {
     unsigned long long list_sig;   // identifies the contents of entries/begin (see bank_acquire)
     int host_chunk;        // output z-layers per pipeline slab; 0 = no pipelining
     int host_launches;     // kernels the last run_host launched
+    // a level of the adaptive tree solve (tree.inl): the kinds of its cells, and the bricks / tiles that have work
+    const unsigned char* tree_kind;   // device [n^3]; non-null: the slab-fed kernel runs in MODE_TREE
+    const int* tile_list;             // device; null = every brick (multipole) / tile (monopole)
+    int tile_count;
     bool pipeline_ready;   // the side streams and events below all exist
     cudaStream_t s_h2d, s_d2h;
     cudaEvent_t ev_in[32], ev_out[32], ev_begin, ev_end;
@@ -346,6 +351,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->mixed_counted = false;
     h->host_chunk = 12;
     h->host_launches = 0;
+    h->tree_kind = nullptr; h->tile_list = nullptr; h->tile_count = 0;
     h->pipeline_ready = false;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
     for (int i = 0; i < MAX_CHUNKS; ++i) { h->ev_in[i] = nullptr; h->ev_out[i] = nullptr; }
@@ -479,6 +485,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.force_dipole = 0;
     P.pL = nullptr; P.pC = nullptr; P.poff = nullptr; P.hc = cfg->h;
     P.leaf = nullptr;
+    P.tile_list = nullptr;
     for (int d = 0; d <= 2 * REACH_MAX; ++d) P.hmul[d] = h->hmul[d];
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
@@ -500,9 +507,12 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e3 = cudaFuncSetAttribute(m2l_staged_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e4 = cudaFuncSetAttribute(m2l_staged_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
-        cudaError_t e5 = cudaFuncSetAttribute(m2l_staged_kernel<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
-        cudaError_t e6 = cudaFuncSetAttribute(m2l_staged_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
-        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess || e5 != cudaSuccess || e6 != cudaSuccess) {
+        cudaError_t e5 = cudaFuncSetAttribute(m2l_staged_kernel<true, false, MODE_MIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        cudaError_t e6 = cudaFuncSetAttribute(m2l_staged_kernel<false, false, MODE_MIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        cudaError_t e7 = cudaFuncSetAttribute(m2l_staged_kernel<true, true, MODE_TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        cudaError_t e8 = cudaFuncSetAttribute(m2l_staged_kernel<false, true, MODE_TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess || e5 != cudaSuccess || e6 != cudaSuccess ||
+            e7 != cudaSuccess || e8 != cudaSuccess) {
             delete h; return OCTO_FMM_ECUDA;
         }
     } else if (cfg->kind == OCTO_FMM_MONOPOLE) {
@@ -645,10 +655,17 @@ static int launch_staged(octo_fmm_t* h, int kb, int ke, bool mixed = false)
     P.kb = kb; P.ke = ke;
     P.tiles_z = (ke - kb + TILE_Z - 1) / TILE_Z;
     P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
+    if (h->tile_list) { P.tile_list = h->tile_list; P.ntiles = h->tile_count; }     // whole-grid launches only (tree levels)
     const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
-    if (mixed) {           // one level of an adaptive mesh: leaf-level lists, near-field entries conditional on the leaf flags
-        if (h->cfg.am_correction) m2l_staged_kernel<true, false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-        else                      m2l_staged_kernel<false, false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    if (grid == 0) return OCTO_FMM_OK;
+    if (h->tree_kind) {    // a level of the adaptive tree: absent cells, leaf-leaf pairs left to the leaf kernel, parent's expansion fused in
+        if (!P.pL) return OCTO_FMM_ESTATE;
+        P.leaf = h->tree_kind;
+        if (h->cfg.am_correction) m2l_staged_kernel<true, true, MODE_TREE><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        else                      m2l_staged_kernel<false, true, MODE_TREE><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+    } else if (mixed) {    // one level of an adaptive mesh: leaf-level lists, near-field entries conditional on the leaf flags
+        if (h->cfg.am_correction) m2l_staged_kernel<true, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        else                      m2l_staged_kernel<false, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
     } else if (P.pL) {     // complete solve: L2L fused into the epilogue (solver.inl sets the parent arrays)
         if (h->cfg.am_correction) m2l_staged_kernel<true, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
         else                      m2l_staged_kernel<false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
@@ -683,7 +700,13 @@ int octo_fmm_interact(octo_fmm_t* h)
     Params& P = h->prm;
     P.L = h->outL; P.C = h->outC;
     if (h->cfg.kind == OCTO_FMM_MONOPOLE) {
-        if (h->mono_kernel == 0 && P.pL)        // complete solve: leaf evaluation fused into the epilogue (solver.inl)
+        if (h->tile_list) {                     // a level of the adaptive tree: only the tiles that hold leaves
+            if (h->mono_kernel != 0) return OCTO_FMM_ESTATE;
+            Params Q = P;
+            Q.tile_list = h->tile_list;
+            if (h->tile_count > 0)
+                p2p_monopole_dmma_kernel<false><<<h->tile_count, DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, Q, h->T, h->dl, h->outL);
+        } else if (h->mono_kernel == 0 && P.pL) // complete solve: leaf evaluation fused into the epilogue (solver.inl)
             p2p_monopole_dmma_kernel<true><<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
         else if (h->mono_kernel == 0)
             p2p_monopole_dmma_kernel<false><<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
@@ -1217,3 +1240,4 @@ int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int*
 }  // extern "C"
 
 #include "solver.inl"
+#include "tree.inl"

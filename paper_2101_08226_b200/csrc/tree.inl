@@ -1,0 +1,454 @@
+// tree.inl -- host logic and C ABI of the gravity solve on an adaptive oct-tree of 8^3 sub-grids (octo_fmm_tree_*,
+// SURVEY 8(f) f3), included by octo_fmm.cu after solver.inl (it drives per-level octo_fmm handles
+// through their internals, like the uniform solve).
+//
+// Levels: tree levels l = 0 .. depth-1 (dense [n_l]^3 lattices, n_l = n0 2^l, with kind[cell]); above level 0 the uniform
+// multipole levels n0/2 .. 2 exactly as in the uniform solve.  Per tree level: a multipole handle (slab-fed kernel in
+// MODE_TREE over the bricks that have work) if the level has refined cells, a monopole handle with the leaf-level list
+// (tensor-core kernel over the tiles that hold leaves) if it has leaves.
+// solve(): leaf moments + M2M bottom-up -> uniform levels up and down -> per tree level, coarsest first: stage, multipole
+// step with the parent's expansion fused in, leaf-leaf sums, leaf finish (expansion at the centre + cross-level pairs).
+
+namespace {
+
+struct TreeLevel {
+    int n;
+    double h;
+    bool has_refined, has_leaf;
+    unsigned char* kind;        // device [n^3]
+    unsigned char* nodeflag;    // device [(n/8)^3]
+    double* lm;                 // device [n^3] masked masses (leaf: m, else 0)
+    double* raw;                // device [20][n^3] (null on a level without refined cells)
+    double* off;                // device [3][n^3]
+    octo_fmm* fmm;              // multipole handle (null without refined cells)
+    octo_fmm* leaf;             // monopole handle, leaf-level list (null without leaves)
+    int* m2l_tiles;  int n_m2l_tiles;     // bricks of the slab-fed kernel that have work
+    int* p2p_tiles;  int n_p2p_tiles;     // 16 x 16 x 8 tiles of the tensor-core kernel that hold leaves
+    std::vector<int> h_m2l_tiles, h_p2p_tiles;
+    std::vector<unsigned char> h_nodeflag;
+};
+
+struct TreePlan {
+    std::vector<TreeLevel> lev;
+    size_t bytes;
+    bool ok;
+};
+
+inline bool tree_config_ok(const octo_fmm_tree_config* c)
+{
+    if (!c) return false;
+    if (c->n0 < 8 || c->n0 > 2048 || (c->n0 & (c->n0 - 1))) return false;       // a power of two >= 8
+    if (c->depth < 1 || c->depth > 10) return false;
+    if (((long long)c->n0 << (c->depth - 1)) > 2048) return false;
+    if (!(c->h0 > 0.0) || !std::isfinite(c->h0)) return false;
+    if (!(c->theta > 1.0 / 3.0 && c->theta < 1.0)) return false;
+    return true;
+}
+
+octo_fmm_solver_config as_solver_config(const octo_fmm_tree_config& t)
+{
+    octo_fmm_solver_config s;
+    std::memset(&s, 0, sizeof s);
+    s.n = t.n0; s.h = t.h0; s.theta = t.theta; s.am_correction = t.am_correction; s.device = t.device; s.stream = t.stream;
+    return s;
+}
+
+// Topology checks, per-sub-grid flags, tile lists and the workspace size.  kind_host[l] = [n_l^3] on the HOST.
+TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* kind_host)
+{
+    TreePlan P;
+    P.ok = false;
+    P.bytes = 0;
+    const int D = cfg.depth;
+    P.lev.resize(D);
+    const octo_fmm_solver_config sc = as_solver_config(cfg);
+    for (int l = 0; l < D; ++l) {
+        TreeLevel& L = P.lev[l];
+        L.n = cfg.n0 << l;
+        L.h = cfg.h0 / (double)(1 << l);
+        L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
+        L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
+        const unsigned char* k = kind_host[l];
+        if (!k) return P;
+        const int n = L.n, nn = n / 8;
+        L.has_refined = L.has_leaf = false;
+        // kinds are constant over sub-grids, children exist iff the parent is refined, the last level has no refined cell
+        for (int K = 0; K < nn; ++K)
+            for (int J = 0; J < nn; ++J)
+                for (int I = 0; I < nn; ++I) {
+                    const unsigned char v = k[((size_t)(8 * K) * n + 8 * J) * n + 8 * I];
+                    if (v > 2) return P;
+                    for (int c = 0; c < 8; ++c)
+                        for (int b = 0; b < 8; ++b)
+                            for (int a = 0; a < 8; ++a)
+                                if (k[((size_t)(8 * K + c) * n + 8 * J + b) * n + 8 * I + a] != v) return P;
+                    if (l == 0 && v == KIND_ABSENT) return P;
+                    if (l == D - 1 && v == KIND_REFINED) return P;
+                    if (l > 0) {
+                        const unsigned char* kp = kind_host[l - 1];
+                        const int pn = n / 2;
+                        const unsigned char pv = kp[((size_t)(4 * K) * pn + 4 * J) * pn + 4 * I];
+                        if ((v != KIND_ABSENT) != (pv == KIND_REFINED)) return P;
+                    }
+                    L.has_refined |= v == KIND_REFINED;
+                    L.has_leaf |= v == KIND_LEAF;
+                }
+    }
+    // flags: NODE_OWN_L = leaf sub-grid with a refined 26-neighbour; NODE_COARSE_NBR = the parent sub-grid has a leaf 26-neighbour
+    for (int l = 0; l < D; ++l) {
+        TreeLevel& L = P.lev[l];
+        const int n = L.n, nn = n / 8;
+        const unsigned char* k = kind_host[l];
+        auto node_kind = [&](const unsigned char* kk, int m, int I, int J, int K) { return kk[((size_t)(8 * K) * m + 8 * J) * m + 8 * I]; };
+        L.h_nodeflag.assign((size_t)nn * nn * nn, 0);
+        for (int K = 0; K < nn; ++K)
+            for (int J = 0; J < nn; ++J)
+                for (int I = 0; I < nn; ++I) {
+                    if (node_kind(k, n, I, J, K) != KIND_LEAF) continue;
+                    unsigned char f = 0;
+                    for (int c = -1; c <= 1; ++c)
+                        for (int b = -1; b <= 1; ++b)
+                            for (int a = -1; a <= 1; ++a) {
+                                const int i2 = I + a, j2 = J + b, k2 = K + c;
+                                if (i2 >= 0 && j2 >= 0 && k2 >= 0 && i2 < nn && j2 < nn && k2 < nn && node_kind(k, n, i2, j2, k2) == KIND_REFINED)
+                                    f |= NODE_OWN_L;
+                                if (l > 0) {
+                                    const int pnn = nn / 2, pi = I / 2 + a, pj = J / 2 + b, pk = K / 2 + c;
+                                    if (pi >= 0 && pj >= 0 && pk >= 0 && pi < pnn && pj < pnn && pk < pnn &&
+                                        node_kind(kind_host[l - 1], n / 2, pi, pj, pk) == KIND_LEAF)
+                                        f |= NODE_COARSE_NBR;
+                                }
+                            }
+                    L.h_nodeflag[((size_t)K * nn + J) * nn + I] = f;
+                }
+        auto node_works = [&](int I, int J, int K) {   // its cells take part in the multipole step of this level
+            const unsigned char v = node_kind(k, n, I, J, K);
+            return v == KIND_REFINED || (v == KIND_LEAF && (L.h_nodeflag[((size_t)K * nn + J) * nn + I] & NODE_OWN_L));
+        };
+        // bricks of the slab-fed kernel: 16 x 8 x 3 cells, dense enumeration t = (ty * tiles_x + tx) * tiles_z + tz
+        if (L.has_refined) {
+            const int tx_n = (n + TILE_X - 1) / TILE_X, ty_n = (n + TILE_Y - 1) / TILE_Y, tz_n = (n + TILE_Z - 1) / TILE_Z;
+            for (int ty = 0; ty < ty_n; ++ty)
+                for (int tx = 0; tx < tx_n; ++tx)
+                    for (int tz = 0; tz < tz_n; ++tz) {
+                        bool work = false;
+                        const int z0 = tz * TILE_Z, z1 = std::min(z0 + TILE_Z, n) - 1;
+                        for (int K = z0 / 8; K <= z1 / 8 && !work; ++K)
+                            for (int I = (tx * TILE_X) / 8; I <= std::min(tx * TILE_X + TILE_X - 1, n - 1) / 8 && !work; ++I)
+                                work = node_works(I, (ty * TILE_Y) / 8, K);
+                        if (work) L.h_m2l_tiles.push_back((ty * tx_n + tx) * tz_n + tz);
+                    }
+        }
+        // tiles of the tensor-core leaf kernel: 16 x 16 x 8 cells, b = (tz * by + ty) * bx + tx
+        if (L.has_leaf) {
+            const int bx = (n + MT_X - 1) / MT_X, by = (n + MT_Y - 1) / MT_Y, bz = (n + DT_Z - 1) / DT_Z;
+            for (int tz = 0; tz < bz; ++tz)
+                for (int ty = 0; ty < by; ++ty)
+                    for (int tx = 0; tx < bx; ++tx) {
+                        bool work = false;
+                        for (int J = 2 * ty; J <= std::min(2 * ty + 1, nn - 1) && !work; ++J)
+                            for (int I = 2 * tx; I <= std::min(2 * tx + 1, nn - 1) && !work; ++I)
+                                work = node_kind(k, n, I, J, tz) == KIND_LEAF;
+                        if (work) L.h_p2p_tiles.push_back((tz * by + ty) * bx + tx);
+                    }
+        }
+        L.n_m2l_tiles = (int)L.h_m2l_tiles.size();
+        L.n_p2p_tiles = (int)L.h_p2p_tiles.size();
+        // workspace of this level
+        const size_t nc = (size_t)n * n * n;
+        P.bytes += align_up(nc) + align_up((size_t)nn * nn * nn) + align_up(nc * 8);           // kind, nodeflag, lm
+        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4);
+        if (L.has_refined) {
+            octo_fmm_config mc = level_config(sc, n, L.h, OCTO_FMM_MULTIPOLE);
+            P.bytes += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
+        }
+        if (L.has_leaf) {
+            octo_fmm_config lc = level_config(sc, n, L.h, OCTO_FMM_MONOPOLE);
+            P.bytes += sizes_of(lc, CF_LEAF_LIST).total;
+        }
+    }
+    // the uniform levels above level 0
+    double h = cfg.h0;
+    for (int n = cfg.n0 / 2; n >= 2; n /= 2) {
+        h *= 2.0;
+        octo_fmm_config mc = level_config(sc, n, h, OCTO_FMM_MULTIPOLE);
+        const size_t nc = (size_t)n * n * n;
+        P.bytes += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
+    }
+    P.bytes += ALIGN;      // pair counters
+    P.ok = true;
+    return P;
+}
+
+}  // namespace
+
+struct octo_fmm_tree {
+    octo_fmm_tree_config cfg;
+    std::vector<TreeLevel> lev;        // tree levels, coarsest first
+    std::vector<SolverLevel> up;       // uniform levels n0/2, ..., 2
+    unsigned long long* counts;        // device [3]: m2l, p2p, cross
+    cudaStream_t stream;
+    bool solved;
+};
+
+extern "C" {
+
+size_t octo_fmm_tree_workspace_bytes(const octo_fmm_tree_config* cfg, const unsigned char* const* kind_host)
+{
+    if (!tree_config_ok(cfg) || !kind_host) return 0;
+    const TreePlan P = tree_plan(*cfg, kind_host);
+    return P.ok ? P.bytes : 0;
+}
+
+int octo_fmm_tree_destroy(octo_fmm_tree_t* t)
+{
+    if (!t) return OCTO_FMM_EINVAL;
+    int rc = OCTO_FMM_OK;
+    for (TreeLevel& l : t->lev) {
+        if (l.fmm && octo_fmm_destroy(l.fmm) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+        if (l.leaf && octo_fmm_destroy(l.leaf) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+    }
+    for (SolverLevel& l : t->up)
+        if (l.fmm && octo_fmm_destroy(l.fmm) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+    delete t;
+    return rc;
+}
+
+int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* const* kind_host, octo_fmm_tree_t** out)
+{
+    if (!out) return OCTO_FMM_EINVAL;
+    *out = nullptr;
+    if (!tree_config_ok(cfg) || !kind_host) return OCTO_FMM_EINVAL;
+    TreePlan P = tree_plan(*cfg, kind_host);
+    if (!P.ok) return OCTO_FMM_EINVAL;
+    if (!cfg->workspace || cfg->workspace_bytes < P.bytes || ((uintptr_t)cfg->workspace % ALIGN)) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(cfg->device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    octo_fmm_tree* t = new (std::nothrow) octo_fmm_tree();
+    if (!t) return OCTO_FMM_ENOMEM;
+    t->cfg = *cfg;
+    t->stream = (cudaStream_t)cfg->stream;
+    t->solved = false;
+    t->lev = std::move(P.lev);
+    const octo_fmm_solver_config sc = as_solver_config(*cfg);
+    char* w = (char*)cfg->workspace;
+    cudaStream_t st = t->stream;
+    int rc = OCTO_FMM_OK;
+    for (size_t l = 0; l < t->lev.size() && rc == OCTO_FMM_OK; ++l) {
+        TreeLevel& L = t->lev[l];
+        const size_t nc = (size_t)L.n * L.n * L.n, nn = (size_t)(L.n / 8) * (L.n / 8) * (L.n / 8);
+        L.kind = (unsigned char*)w; w += align_up(nc);
+        L.nodeflag = (unsigned char*)w; w += align_up(nn);
+        L.lm = (double*)w; w += align_up(nc * 8);
+        L.m2l_tiles = (int*)w; w += align_up((size_t)L.n_m2l_tiles * 4 + 4);
+        L.p2p_tiles = (int*)w; w += align_up((size_t)L.n_p2p_tiles * 4 + 4);
+        if (cudaMemcpyAsync(L.kind, kind_host[l], nc, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+            cudaMemcpyAsync(L.nodeflag, L.h_nodeflag.data(), nn, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+            (L.n_m2l_tiles && cudaMemcpyAsync(L.m2l_tiles, L.h_m2l_tiles.data(), (size_t)L.n_m2l_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
+            (L.n_p2p_tiles && cudaMemcpyAsync(L.p2p_tiles, L.h_p2p_tiles.data(), (size_t)L.n_p2p_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)) {
+            rc = OCTO_FMM_ECUDA;
+            break;
+        }
+        if (L.has_refined) {
+            octo_fmm_config mc = level_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
+            mc.workspace = w; mc.workspace_bytes = sizes_of(mc, CF_ANY_SIZE).total; w += mc.workspace_bytes;
+            L.raw = (double*)w; w += align_up(nc * 20 * 8);
+            L.off = (double*)w; w += align_up(nc * 3 * 8);
+            rc = create_internal(&mc, CF_ANY_SIZE, &L.fmm);
+            if (rc != OCTO_FMM_OK) break;
+            L.fmm->kernel = 0;                 // the slab-fed kernel (MODE_TREE), whatever the size of the level
+            L.fmm->tree_kind = L.kind;
+            L.fmm->tile_list = L.m2l_tiles;
+            L.fmm->tile_count = L.n_m2l_tiles;
+        }
+        if (L.has_leaf) {
+            octo_fmm_config lc = level_config(sc, L.n, L.h, OCTO_FMM_MONOPOLE);
+            lc.workspace = w; lc.workspace_bytes = sizes_of(lc, CF_LEAF_LIST).total; w += lc.workspace_bytes;
+            rc = create_internal(&lc, CF_LEAF_LIST, &L.leaf);
+            if (rc != OCTO_FMM_OK) break;
+            L.leaf->tile_list = L.p2p_tiles;
+            L.leaf->tile_count = L.n_p2p_tiles;
+        }
+    }
+    double h = cfg->h0;
+    for (int n = cfg->n0 / 2; n >= 2 && rc == OCTO_FMM_OK; n /= 2) {
+        h *= 2.0;
+        SolverLevel l;
+        l.n = n; l.h = h; l.fmm = nullptr;
+        octo_fmm_config mc = level_config(sc, n, h, OCTO_FMM_MULTIPOLE);
+        const size_t nc = (size_t)n * n * n;
+        l.ws_bytes = sizes_of(mc, CF_ANY_SIZE).total;
+        mc.workspace = w; mc.workspace_bytes = l.ws_bytes; w += l.ws_bytes;
+        l.raw = (double*)w; w += align_up(nc * 20 * 8);
+        l.off = (double*)w; w += align_up(nc * 3 * 8);
+        rc = create_internal(&mc, CF_ANY_SIZE, &l.fmm);
+        t->up.push_back(l);
+    }
+    t->counts = (unsigned long long*)w;
+    // the topology arrays were copied from pageable host memory: make sure they have left it before returning
+    if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
+    if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
+    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); }
+    *out = t;
+    return OCTO_FMM_OK;
+}
+
+static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double* const* out, bool count)
+{
+    const int D = (int)t->lev.size();
+    cudaStream_t st = t->stream;
+    int rc;
+    // ---- upward pass: finest level first ----
+    for (int l = D - 1; l >= 0; --l) {
+        TreeLevel& L = t->lev[l];
+        const long long nc = (long long)L.n * L.n * L.n;
+        if (L.has_refined) {
+            TreeLevel& F = t->lev[l + 1];
+            const dim3 blocks((unsigned)((L.n + 127) / 128), (unsigned)L.n, (unsigned)L.n);
+            if (F.raw) m2m_kernel<false><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n, L.n, L.n, F.h);
+            else       m2m_kernel<true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n, L.n, L.n, F.h);
+        }
+        tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    // ---- the uniform levels above level 0: up ... ----
+    for (size_t lv = 0; lv < t->up.size(); ++lv) {
+        SolverLevel& l = t->up[lv];
+        const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
+        if (lv == 0) {
+            TreeLevel& B = t->lev[0];
+            if (B.raw) m2m_kernel<false><<<blocks, 128, 0, st>>>(B.raw, B.off, l.raw, l.off, l.n, l.n, l.n, B.h);
+            else       m2m_kernel<true><<<blocks, 128, 0, st>>>(B.lm, nullptr, l.raw, l.off, l.n, l.n, l.n, B.h);
+        } else {
+            m2m_kernel<false><<<blocks, 128, 0, st>>>(t->up[lv - 1].raw, t->up[lv - 1].off, l.raw, l.off, l.n, l.n, l.n, t->up[lv - 1].h);
+        }
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    // ---- ... and down, as in the uniform solve ----
+    for (int lv = (int)t->up.size() - 1; lv >= 0; --lv) {
+        SolverLevel& l = t->up[lv];
+        if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
+        const bool has_parent = lv < (int)t->up.size() - 1;
+        const bool fused = has_parent && l.fmm->kernel == 0;
+        if (fused) set_parent(l.fmm, t->up[lv + 1]);
+        rc = octo_fmm_interact(l.fmm);
+        if (fused) clear_parent(l.fmm);
+        if (rc != OCTO_FMM_OK) return rc;
+        const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
+        if (!has_parent)
+            l2l_kernel<false><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, nullptr, nullptr, nullptr, l.n, l.n, l.n, l.h);
+        else if (!fused) {
+            SolverLevel& p = t->up[lv + 1];
+            l2l_kernel<true><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, p.fmm->L, p.fmm->C, p.off, l.n, l.n, l.n, l.h);
+        }
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    if (count && cudaMemsetAsync(t->counts, 0, 3 * sizeof(unsigned long long), st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    // ---- tree levels, coarsest first ----
+    for (int l = 0; l < D; ++l) {
+        TreeLevel& L = t->lev[l];
+        // parent arrays of this level: the tree level above, or the finest uniform level
+        const double *pL, *pC, *poff;
+        if (l > 0) { pL = t->lev[l - 1].fmm->L; pC = t->lev[l - 1].fmm->C; poff = t->lev[l - 1].off; }
+        else       { pL = t->up[0].fmm->L; pC = t->up[0].fmm->C; poff = t->up[0].off; }
+        if (L.fmm && L.n_m2l_tiles > 0) {
+            if ((rc = octo_fmm_set_moments(L.fmm, L.raw, L.off)) != OCTO_FMM_OK) return rc;
+            const long long nc = (long long)L.n * L.n * L.n;
+            stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, L.fmm->src, L.n, L.n, L.n);
+            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+            L.fmm->prm.pL = pL; L.fmm->prm.pC = pC; L.fmm->prm.poff = poff;
+            rc = octo_fmm_interact(L.fmm);
+            clear_parent(L.fmm);
+            if (rc != OCTO_FMM_OK) return rc;
+        }
+        if (L.leaf) {
+            if ((rc = octo_fmm_set_moments(L.leaf, L.lm, nullptr)) != OCTO_FMM_OK) return rc;
+            double* const keep = L.leaf->outL;
+            L.leaf->outL = out[l];
+            rc = octo_fmm_interact(L.leaf);
+            L.leaf->outL = keep;
+            if (rc != OCTO_FMM_OK) return rc;
+        }
+        // leaf finish (also zeroes the cells of out[l] that are not leaves); reads the near field from the constant bank
+        {
+            octo_fmm* hb = L.fmm ? L.fmm : (L.leaf ? L.leaf : t->up[0].fmm);
+            BankLock guard(hb);
+            if (bank_acquire(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+            TreeFinishArgs a;
+            a.n = L.n; a.h = L.h; a.kind = L.kind; a.nodeflag = L.nodeflag; a.lm = L.lm; a.out = out[l];
+            a.L = L.fmm ? L.fmm->L : nullptr; a.C = L.fmm ? L.fmm->C : nullptr;
+            a.pL = pL; a.pC = pC; a.poff = poff;
+            a.kind_f = l + 1 < D ? t->lev[l + 1].kind : nullptr; a.mass_f = l + 1 < D ? t->lev[l + 1].lm : nullptr;
+            a.kind_c = l > 0 ? t->lev[l - 1].kind : nullptr;     a.mass_c = l > 0 ? t->lev[l - 1].lm : nullptr;
+            a.count = count ? t->counts : nullptr;
+            const dim3 blocks((unsigned)((L.n + 127) / 128), (unsigned)L.n, (unsigned)L.n);
+            tree_leaf_finish_kernel<<<blocks, 128, 0, st>>>(a);
+            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+            if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+        }
+        if (count) {
+            // the Eq. 15 list with its (dx, dy, dz) is the multipole flavour of the bank: any multipole handle brings it
+            octo_fmm* hb = L.fmm ? L.fmm : t->up[0].fmm;
+            BankLock guard(hb);
+            if (bank_acquire(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+            const dim3 blocks((unsigned)((L.n + 127) / 128), (unsigned)L.n, (unsigned)L.n);
+            tree_count_kernel<<<blocks, 128, 0, st>>>(L.kind, L.n, t->counts);
+            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+            if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+        }
+    }
+    t->solved = true;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_tree_solve(octo_fmm_tree_t* t, const double* const* mass, double* const* out)
+{
+    if (!t || !mass || !out) return OCTO_FMM_EINVAL;
+    for (size_t l = 0; l < t->lev.size(); ++l)
+        if (!mass[l] || !out[l] || ((uintptr_t)mass[l] % 16) || ((uintptr_t)out[l] % 16)) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(t->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    return tree_solve_impl(t, mass, out, false);
+}
+
+int octo_fmm_tree_interaction_counts(octo_fmm_tree_t* t, const double* const* mass, double* const* out, unsigned long long counts[3])
+{
+    if (!t || !mass || !out || !counts) return OCTO_FMM_EINVAL;
+    for (size_t l = 0; l < t->lev.size(); ++l)
+        if (!mass[l] || !out[l] || ((uintptr_t)mass[l] % 16) || ((uintptr_t)out[l] % 16)) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(t->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    const int rc = tree_solve_impl(t, mass, out, true);
+    if (rc != OCTO_FMM_OK) return rc;
+    if (cudaStreamSynchronize(t->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (cudaMemcpy(counts, t->counts, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
+    for (const SolverLevel& l : t->up) counts[0] += l.fmm->n_interactions;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_tree_status(octo_fmm_tree_t* t)
+{
+    if (!t) return OCTO_FMM_EINVAL;
+    if (cudaStreamSynchronize(t->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    int worst = OCTO_FMM_OK;
+    for (TreeLevel& l : t->lev) {
+        if (l.fmm) { const int rc = octo_fmm_status(l.fmm); if (rc != OCTO_FMM_OK) worst = rc; }
+        if (l.leaf) { const int rc = octo_fmm_status(l.leaf); if (rc != OCTO_FMM_OK) worst = rc; }
+    }
+    for (SolverLevel& l : t->up) { const int rc = octo_fmm_status(l.fmm); if (rc != OCTO_FMM_OK) worst = rc; }
+    return worst;
+}
+
+int octo_fmm_tree_launches(const octo_fmm_tree_t* t, int* launches)
+{
+    if (!t || !launches) return OCTO_FMM_EINVAL;
+    int n = 0;
+    for (const TreeLevel& l : t->lev) {
+        n += 1 + (l.has_refined ? 1 : 0);                                  // leaf moments, M2M
+        if (l.fmm && l.n_m2l_tiles > 0) n += 3;                            // stage, flags, multipole step
+        if (l.leaf) n += 2;                                                // stage, leaf-leaf sums
+        n += 1;                                                            // leaf finish
+    }
+    n += 4 * (int)t->up.size();
+    *launches = n;
+    return OCTO_FMM_OK;
+}
+
+}  // extern "C"

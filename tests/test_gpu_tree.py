@@ -1,0 +1,129 @@
+"""Parity of the solve on an adaptive oct-tree of 8^3 sub-grids (octo_fmm_tree_*, reading R9) against
+oracle.solve_tree, through the C ABI (-m gpu).
+
+Bar: the pair set bit-exact (ordered pairs per kind: multipole, leaf-leaf, across a refinement boundary); phi within 1e-12
+cell by cell at every leaf of every level (the potential of positive masses never vanishes), g within 1e-12 of the
+largest |g| of the tree (it passes through zero)."""
+import numpy as np
+import pytest
+
+import fmm_inputs as fi
+import oracle
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from paper_2101_08226_b200 import build
+    build.build()
+    import paper_2101_08226_b200 as p
+    assert torch.cuda.is_available()
+    return p, torch
+
+
+def _run(env, tree, theta, correction, counts=True):
+    p, torch = env
+    t = p.OctoFMMTree(tree.n0, tree.h0, theta, tree.kind, correction)
+    mass = [torch.from_numpy(m).cuda() for m in tree.mass]
+    if counts:
+        cnt, out = t.interaction_counts(mass)
+    else:
+        cnt, out = None, t.solve(mass)
+    torch.cuda.synchronize()
+    assert t.status() == p.OK
+    res = [o.cpu().numpy() for o in out]
+    t.close()
+    return res, cnt
+
+
+def _compare(tree, got, ref):
+    gmax = max(np.abs(r[1:]).max() for r in ref)
+    worst_phi = worst_g = 0.0
+    for l in range(tree.depth):
+        leaf = tree.kind[l] == fi.TREE_LEAF
+        assert np.all(got[l][:, ~leaf] == 0.0)
+        if not leaf.any():
+            continue
+        worst_phi = max(worst_phi, float((np.abs(got[l][0] - ref[l][0])[leaf] / np.abs(ref[l][0])[leaf]).max()))
+        worst_g = max(worst_g, float(np.abs(got[l][1:] - ref[l][1:])[:, leaf].max() / gmax))
+    return worst_phi, worst_g
+
+
+@pytest.mark.parametrize("seed,theta,correction", [(1, 0.5, True), (2, 0.35, True), (3, 0.7, True), (4, 0.5, False)])
+def test_seeded_trees(env, seed, theta, correction):
+    """Seeded random trees of depth 3 on a 16^3 base (leaves on two levels, refinement boundaries everywhere)."""
+    tree = fi.seeded_tree(seed)
+    assert fi.tree_is_properly_nested(tree)
+    ref, cref = oracle.solve_tree(tree.n0, tree.h0, theta, tree.kind, tree.mass, correction)
+    got, cnt = _run(env, tree, theta, correction)
+    assert cnt == {k: cref[k] for k in ("m2l", "p2p", "cross")}
+    e_phi, e_g = _compare(tree, got, ref)
+    assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+
+
+def test_deep_tree_and_the_paper_like_refinement_pattern(env):
+    """Four levels (leaves on three of them), and the two-star field refined around the stars (density-based refinement,
+    Eq. 34-35), dynamic range 1e-10."""
+    for tree, theta in ((fi.seeded_tree(1, depth=4, frac=0.3), 0.5), (fi.star_tree(16, 3), 0.5)):
+        assert fi.tree_is_properly_nested(tree)
+        ref, cref = oracle.solve_tree(tree.n0, tree.h0, theta, tree.kind, tree.mass, True)
+        got, cnt = _run(env, tree, theta, True)
+        assert cnt == {k: cref[k] for k in ("m2l", "p2p", "cross")}
+        e_phi, e_g = _compare(tree, got, ref)
+        assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+
+
+def test_fully_refined_tree_equals_the_uniform_solver(env):
+    """No refinement boundary: the tree path must reproduce the uniform solve (oracle) and agree with the uniform GPU
+    solver to round-off; a single-level tree (everything a leaf on level 0) as well."""
+    p, torch = env
+    n, h = 32, 1.0 / 32
+    m = np.random.default_rng(3).uniform(0.5, 1.5, (n, n, n)) * h ** 3
+    kind = [np.full((8,) * 3, 2, np.uint8), np.full((16,) * 3, 2, np.uint8), np.full((32,) * 3, 1, np.uint8)]
+    mass = [np.zeros((8,) * 3), np.zeros((16,) * 3), m]
+    tree = fi.Tree(8, 1.0 / 8, kind, mass)
+    ref = oracle.solve(n, h, 0.5, m, True)
+    got, cnt = _run(env, tree, 0.5, True)
+    assert cnt["cross"] == 0
+    assert (np.abs(got[2][0] - ref[0]) / np.abs(ref[0])).max() < TOL
+    assert np.abs(got[2][1:] - ref[1:]).max() / np.abs(ref[1:]).max() < TOL
+    s = p.OctoFMMSolver(n, h, 0.5, True)
+    uni = s.solve(torch.from_numpy(m).cuda()).cpu().numpy()
+    s.close()
+    assert np.abs(got[2] - uni).max() / np.abs(uni).max() < 1e-13
+    one = fi.Tree(32, h, [np.full((32,) * 3, 1, np.uint8)], [m])
+    got1, _ = _run(env, one, 0.5, True)
+    assert (np.abs(got1[0][0] - ref[0]) / np.abs(ref[0])).max() < TOL
+
+
+def test_conservation_on_the_gpu_result(env):
+    """Newton's third law over the leaves of all levels and, with the correction, the torque balance (L125, L127)."""
+    tree = fi.seeded_tree(2)
+    pos, ms, lv, idx = tree.leaf_points()
+    for corr in (True, False):
+        got, _ = _run(env, tree, 0.5, corr, counts=False)
+        res = np.concatenate([got[l][:, tree.kind[l] == fi.TREE_LEAF].T for l in range(tree.depth)])
+        F = ms[:, None] * res[:, 1:4]
+        T = np.cross(pos, F)
+        assert np.abs(F.sum(0)).max() / np.abs(F).sum() < 1e-14
+        t = np.abs(T.sum(0)).max() / np.abs(T).sum()
+        assert (t < 1e-13) if corr else (t > 1e-8)
+
+
+def test_bad_topologies_are_refused(env):
+    p, torch = env
+    tree = fi.seeded_tree(1)
+    bad = [k.copy() for k in tree.kind]
+    bad[2][0, 0, 0] = 2 if bad[2][0, 0, 0] != 2 else 1            # not constant over a sub-grid
+    with pytest.raises(p.OctoFmmError):
+        p.OctoFMMTree(tree.n0, tree.h0, 0.5, bad)
+    bad = [k.copy() for k in tree.kind]
+    bad[1][:8, :8, :8] = 1                                          # children of a leaf exist (level 2 was built for it)
+    if (tree.kind[1][:8, :8, :8] == 2).all():
+        with pytest.raises(p.OctoFmmError):
+            p.OctoFMMTree(tree.n0, tree.h0, 0.5, bad)
+    with pytest.raises(ValueError):
+        p.OctoFMMTree(tree.n0, tree.h0, 0.5, [k[:4] for k in tree.kind])
