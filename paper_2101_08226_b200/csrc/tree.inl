@@ -347,9 +347,11 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
     for (int l = 0; l < D; ++l) {
         TreeLevel& L = t->lev[l];
         // parent arrays of this level: the tree level above, or the finest uniform level
-        const double *pL, *pC, *poff;
-        if (l > 0) { pL = t->lev[l - 1].fmm->L; pC = t->lev[l - 1].fmm->C; poff = t->lev[l - 1].off; }
-        else       { pL = t->up[0].fmm->L; pC = t->up[0].fmm->C; poff = t->up[0].off; }
+        // (a level above without refined cells means that this level is empty: nothing reads the parent arrays then)
+        const double *pL = nullptr, *pC = nullptr, *poff = nullptr;
+        if (l > 0 && t->lev[l - 1].fmm) { pL = t->lev[l - 1].fmm->L; pC = t->lev[l - 1].fmm->C; poff = t->lev[l - 1].off; }
+        else if (l == 0)                { pL = t->up[0].fmm->L; pC = t->up[0].fmm->C; poff = t->up[0].off; }
+        if (!pL && (L.has_refined || L.has_leaf)) return OCTO_FMM_ESTATE;
         if (L.fmm && L.n_m2l_tiles > 0) {
             if ((rc = octo_fmm_set_moments(L.fmm, L.raw, L.off)) != OCTO_FMM_OK) return rc;
             const long long nc = (long long)L.n * L.n * L.n;
