@@ -303,10 +303,115 @@ def run_solve(args):
     s.close()
 
 
+def run_tree(args):
+    """--workload tree: the solve on an ADAPTIVE oct-tree of 8^3 sub-grids (octo_fmm_tree_*, NEXT f3) on the two-star
+    field of cfg 3/5 refined around the stars (the paper's density-based refinement, Eq. 34-35): 64^3 base
+    cells, 3 levels, 256^3-equivalent inside the stars.  A step = one solve over all levels; interactions = ordered
+    pairs of all kinds (multipole pairs, leaf-leaf point-mass pairs, point-mass pairs across refinement boundaries)."""
+    import numpy as np
+    import torch
+    import fmm_inputs as fi
+    import oracle
+    import paper_2101_08226_b200 as p
+    from paper_2101_08226_b200 import build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    local = env_int("LOCAL_RANK", 0)
+    if env_int("WORLD_SIZE", 1) > 1:
+        raise SystemExit("bench.py --workload tree is a single-GPU line")
+    torch.cuda.set_device(local)
+    build.build()
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream(dev)
+    n0 = args.ncell or 64
+    depth = 3
+    tree = fi.star_tree(n0, depth)
+    t = p.OctoFMMTree(tree.n0, tree.h0, args.theta, tree.kind, True, device=local, stream=stream)
+    mass = [torch.from_numpy(m).to(dev) for m in tree.mass]
+    out = t.empty_out()
+    cnt, _ = t.interaction_counts(mass, out)
+    n_int = cnt["m2l"] + cnt["p2p"] + cnt["cross"]
+    launches = t.launches()
+    leaves = [int((k == fi.TREE_LEAF).sum()) for k in tree.kind]
+    for _ in range(max(args.warmup, 3)):
+        t.solve(mass, out)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        t.solve(mass, out)
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop(t0, time.perf_counter())
+    ms = ev0.elapsed_time(ev1) / args.steps
+    if t.status() != p.OK:
+        raise SystemExit("bench.py: device reported status %d" % t.status())
+    # conservation on the timed result (L125, L127): sum of m g and of x x m g over the leaves of all levels
+    F = torch.zeros(3, dtype=torch.float64, device=dev)
+    Fa = torch.zeros((), dtype=torch.float64, device=dev)
+    for l in range(depth):
+        mg = mass[l][None] * out[l][1:4] * torch.from_numpy(tree.kind[l] == fi.TREE_LEAF).to(dev)[None]
+        F += mg.sum(dim=(1, 2, 3))
+        Fa += mg.abs().sum()
+    net_force = float(F.abs().max() / Fa)
+    # end to end through the host-buffer entry point (pinned host arrays, every level)
+    nb = p.octo_fmm_tree_host_scratch_bytes(t.cfg)
+    scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
+    m_h = [torch.from_numpy(m).pin_memory() for m in tree.mass]
+    o_h = [torch.empty((4,) + (tree.n(l),) * 3, dtype=torch.float64).pin_memory() for l in range(depth)]
+    p.octo_fmm_tree_solve_host(t.handle, m_h, o_h, scratch, nb)
+    t0 = time.perf_counter()
+    for _ in range(max(args.e2e_steps, 1)):
+        p.octo_fmm_tree_solve_host(t.handle, m_h, o_h, scratch, nb)
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / max(args.e2e_steps, 1)
+    h2d = sum(int(m.numel() * 8) for m, k in zip(m_h, tree.kind) if (k == fi.TREE_LEAF).any())
+    d2h = sum(int(o.numel() * 8) for o in o_h)
+    same = all(bool(torch.equal(o_h[l], out[l].cpu())) for l in range(depth))
+    # the oracle's tree solve on the host cores, on the same refinement pattern one octave down (n0 / 2)
+    small = fi.star_tree(max(n0 // 2, 16), depth)
+    oracle.lib()
+    t0 = time.perf_counter()
+    _, cref = oracle.solve_tree(small.n0, small.h0, args.theta, small.kind, small.mass, True)
+    t_ref = time.perf_counter() - t0
+    cnt_ref = cref["m2l"] + cref["p2p"] + cref["cross"]
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak = sm_count * FP64_LANES_PER_SM * 2 * 1965.0e6 / 1e12
+    f_multi = p.octo_fmm_flops_per_interaction_path(p.MULTIPOLE, True, False)[0]   # centre-of-mass expansions: no dipoles
+    flops = float(f_multi) * cnt["m2l"] + 8.0 * (cnt["p2p"] + cnt["cross"])
+    line = {"metric": METRIC, "value": n_int / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "adaptive-tree solve, two-star field refined around the stars, %d^3 base cells, %d levels "
+                                   "(%d^3-equivalent), theta=%g, correction on" % (n0, depth, n0 << (depth - 1), args.theta),
+                       "interactions_per_step": n_int, "pairs": cnt, "leaf_cells_per_level": leaves,
+                       "leaf_cells_per_s": sum(leaves) / (ms * 1e-3),
+                       "l2": "arrays of the fine levels larger than L2", "net_force_over_sum_abs_force": net_force,
+                       "host_entry_bit_identical": same},
+            "roofline": {"bound": "alu", "kernel": "whole solve (m2l_staged_kernel<.,L2L,TREE> and p2p_monopole_dmma_kernel over tile lists)",
+                         "achieved": flops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                         "frac": flops / (ms * 1e-3) / 1e12 / peak, "traffic": None,
+                         "note": "useful flops only: %d per multipole pair, 8 per point-mass pair; pairs the kernels mask "
+                                 "(two leaves in a brick of the multipole step) are executed but not counted" % f_multi},
+            "cpu_baseline": {"value": cnt_ref / t_ref, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": "oracle.solve_tree of the same pattern at %d^3 base cells (%d interactions) in %.1f s" % (
+                                 small.n0, cnt_ref, t_ref)},
+            "e2e": {"value": n_int / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_ms},
+            "clocks": clocks, "gpu_launches": launches * args.steps}
+    print(json.dumps(line))
+    t.close()
+
+
 def run_coupled(args):
     """--coupled: ONE problem sharded over the ranks (z-slabs of a grid of ncell x ncell x (ncell * N) cells, rank r owns
     slab r) with one halo exchange of boundary layers per step (paper_2101_08226_b200/sharded.py).
-    Opt-in: the default N > 1 arm runs independent problems.  A step = halo exchange + staging + interaction."""
+    Opt-in: the default N > 1 arm runs independent problems.  A step = halo exchange (in place, straight into the
+    persistent extended arrays) + staging + interaction."""
     import torch
     import torch.distributed as dist
     world, rank, local = env_int("WORLD_SIZE", 1), env_int("RANK", 0), env_int("LOCAL_RANK", 0)
@@ -314,6 +419,7 @@ def run_coupled(args):
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # the communicator log lets the driver count ranks
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     from paper_2101_08226_b200 import build
     if rank == 0:
@@ -327,7 +433,8 @@ def run_coupled(args):
     stream = torch.cuda.current_stream(dev)
     lvl = ShardedLevel(w.n, w.h, args.theta, True, rank=rank, world=world, device=local, stream=stream)
     lvl.fmm.set_option("dipole_terms", 1)
-    mom, com = torch.from_numpy(w.moments).to(dev), torch.from_numpy(w.com_off).to(dev)
+    lvl.moments.copy_(torch.from_numpy(w.moments))             # the producer writes into the owned views, once
+    lvl.com_off.copy_(torch.from_numpy(w.com_off))
     L = torch.empty((20,) + lvl.fmm.out_shape, dtype=torch.float64, device=dev)
     Lc = torch.empty((3,) + lvl.fmm.out_shape, dtype=torch.float64, device=dev)
     lvl.fmm.bind_outputs(L, Lc)
@@ -338,26 +445,62 @@ def run_coupled(args):
         torch.cuda.synchronize()
 
     for _ in range(max(args.warmup, 3)):
-        lvl.step(mom, com, L, Lc)
+        lvl.step(None, None, L, Lc)
     barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
     ev0.record(stream)
     for _ in range(args.steps):
-        lvl.step(mom, com, L, Lc)
+        lvl.step(None, None, L, Lc)
     ev1.record(stream)
     barrier()
+    clocks = sampler.stop(t0, time.perf_counter()) if rank == 0 else None
     if lvl.fmm.status() != p.OK:
         raise SystemExit("bench.py: device reported status %d" % lvl.fmm.status())
-    ms, units = aggregate_over_ranks(ev0.elapsed_time(ev1), lvl.interaction_count() * args.steps, dist if world > 1 else None, dev)
+    n_int = lvl.interaction_count()
+    ms, units = aggregate_over_ranks(ev0.elapsed_time(ev1), n_int * args.steps, dist if world > 1 else None, dev)
+    # end to end: the rank's slab from pinned host memory into the owned views, the step, the expansions back
+    m_h, c_h = torch.from_numpy(w.moments).pin_memory(), torch.from_numpy(w.com_off).pin_memory()
+    L_h = torch.empty(L.shape, dtype=torch.float64).pin_memory()
+    e2e_steps = max(args.e2e_steps, 1)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        lvl.moments.copy_(m_h, non_blocking=True)
+        lvl.com_off.copy_(c_h, non_blocking=True)
+        lvl.step(None, None, L, Lc)
+        L_h.copy_(L, non_blocking=True)
+        torch.cuda.synchronize()
+    barrier()
+    e2e_ms_local = 1e3 * (time.perf_counter() - t0)
+    e2e_ms, e2e_units = aggregate_over_ranks(e2e_ms_local, n_int * e2e_steps, dist if world > 1 else None, dev)
     if rank == 0:
-        halo_bytes = (2 if world > 2 else (1 if world == 2 else 0)) * 23 * HALO * w.n[0] * w.n[1] * 8
+        flops_per, instr_per = p.octo_fmm_flops_per_interaction(p.MULTIPOLE, True)
+        sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak = world * sm_count * FP64_LANES_PER_SM * 2 * 1965.0e6 / 1e12
+        achieved = flops_per * units / (ms * 1e-3) / 1e12
+        c, s, threads, nr = oracle_sample_bounded(w, args.theta, args.ref_seconds)
         print(json.dumps({"metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                           "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
                           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                           "config": {"workload": "%s stacked in z: %d x %d x %d cells, theta=%g, correction on" % (
                               w.name, w.n[0], w.n[1], w.n[2] * world, args.theta),
-                              "parallelism": "z-slabs, one halo exchange per step (%d bytes sent per interior rank)" % halo_bytes},
-                          "gpu_launches": 2 * args.steps}))
+                              "parallelism": "z-slabs, one in-place halo exchange per step (%d bytes sent by this rank, "
+                                             "%d layers of 23 doubles per cell per neighbour)" % (lvl.halo_bytes_sent, HALO),
+                              "l2": "inputs larger than L2" if w.moments.nbytes > 126e6 else "inputs smaller than L2"},
+                          "roofline": {"bound": "alu", "kernel": "m2l_staged_kernel<correction> on every rank (step incl. exchange and staging)",
+                                       "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None},
+                          "cpu_baseline": {"value": c / s, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                           "sample": "%d regions of 16^3 cells (%d interactions) of rank 0's slab in %.1f s" % (nr, c, s)},
+                          "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT,
+                                  "h2d_bytes_per_step": int(world * (m_h.numel() + c_h.numel()) * 8),
+                                  "d2h_bytes_per_step": int(world * L_h.numel() * 8), "ms_per_step": e2e_ms / e2e_steps},
+                          "clocks": clocks, "gpu_launches": 2 * args.steps * world}))
     lvl.close()
     if world > 1:
         dist.destroy_process_group()
@@ -572,7 +715,8 @@ def run_ours(args):
                 "fp64_pipe_issue_frac": (instr_per * n_int / (kernel_ms * 1e-3)) / (sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
                 "fp64_issue_probe_frac_of_issue_peak": issue_probe,
                 "kernel_ms": kernel_ms, "interactions_per_launch": n_int,
-                "traffic": TRAFFIC_BYTES.get((args.workload, int(w.n[0]), args.theta)),
+                "traffic": traffic_bytes(args.workload, int(w.n[0]), args.theta, p.octo_fmm_version()),
+                "kernel_version": p.octo_fmm_version(),
                 "algorithmic_bytes": int(bytes_per_cell * w.moments[0].size),
                 "hbm_gbs_at_algorithmic_bytes": bytes_per_cell * w.moments[0].size / (kernel_ms * 1e-3) / 1e9,
                 "hbm_peak_gbs": peaks.get("hbm_gbs")}
@@ -582,6 +726,15 @@ def run_ours(args):
     cpu_baseline = {"value": c / s, "unit": UNIT, "cores": threads, "kind": "oracle",
                     "sample": "%d regions of 16^3 cells (%d sub-grids, %d interactions) of %s in %.1f s" % (
                         nr, 8 * nr, c, w.name, s)}
+    # "(i) single thread, (ii) OpenMP over sub-grids on all cores": the same oracle on ONE thread, on the
+    # first regions of the same stratified sample (about a quarter of the time budget)
+    import oracle
+    oracle.lib().fmm_oracle_set_num_threads(1)
+    n1 = max(1, int(nr * (args.ref_seconds / 4.0) / max(s, 1e-9) / max(threads, 1)))
+    c1, s1, _, _ = oracle_sample(w, args.theta, min(n1, nr))
+    oracle.lib().fmm_oracle_set_num_threads(threads)
+    cpu_baseline["single_thread"] = {"value": c1 / s1, "unit": UNIT, "cores": 1,
+                                     "sample": "%d regions of 16^3 cells (%d interactions) in %.1f s" % (min(n1, nr), c1, s1)}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -605,14 +758,22 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the interaction kernel, one `ncu --set full` capture
-# per entry (profiles/); None until captured for that workload.
-TRAFFIC_BYTES = {
-    # profiles/r01_final.md: 8.198 GB read + 3.063 GB written per launch
-    ("cfg5", 256, 0.5): 11260626000,
-    # profiles/r01_monopole.md (DMMA kernel, 256^3): 151.9 MB read + 478.7 MB written per launch
-    ("cfg4", 256, 0.5): 630586368,
-}
+def traffic_bytes(workload, ncell, theta, version):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the tracked table
+    profiles/traffic.csv (one row per `ncu --set full` capture; the raw export each row comes from is named in it).
+    A row counts only if it was captured with THIS build of the kernels (version string of octo_fmm_version()):
+    a stale capture yields None, not a wrong number."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        with open(path, newline="") as fh:
+            for row in csv.DictReader(r for r in fh if not r.startswith("#")):
+                if (row["version"] == version and row["workload"] == workload and int(row["ncell"]) == int(ncell)
+                        and abs(float(row["theta"]) - float(theta)) < 1e-12):
+                    return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+    except (OSError, KeyError, ValueError):
+        return None
+    return None
 
 
 def main():
@@ -635,6 +796,8 @@ def main():
         run_reference(args)
     elif args.workload == "solve":
         run_solve(args)
+    elif args.workload == "tree":
+        run_tree(args)
     elif args.coupled:
         run_coupled(args)
     else:

@@ -300,6 +300,12 @@ int octo_fmm_tree_solve(octo_fmm_tree_t *t, const double *const *mass, double *c
  * level, counts[2] point-mass pairs across a refinement boundary.  Synchronises the stream. */
 int octo_fmm_tree_interaction_counts(octo_fmm_tree_t *t, const double *const *mass, double *const *out,
                                      unsigned long long counts[3]);
+/* The same with HOST buffers (mass_host[l], out_host[l]: host arrays of the layouts above; pinned memory makes the
+ * copies asynchronous): H2D of the masses of every level that has leaves, solve, D2H of every out[l], stream
+ * synchronise.  scratch: device, >= octo_fmm_tree_host_scratch_bytes(cfg), 256-byte aligned, borrowed for the call. */
+size_t octo_fmm_tree_host_scratch_bytes(const octo_fmm_tree_config *cfg);
+int octo_fmm_tree_solve_host(octo_fmm_tree_t *t, const double *const *mass_host, double *const *out_host, void *scratch,
+                             size_t scratch_bytes);
 /* Synchronises the stream; OCTO_FMM_EMASS if the correction met an existing cell of mass <= 0. */
 int octo_fmm_tree_status(octo_fmm_tree_t *t);
 /* Kernels one solve launches. */

@@ -93,6 +93,9 @@ class _Library:
         lib.octo_fmm_tree_create.argtypes = [tcfgp, vpp, ctypes.POINTER(vp)]
         lib.octo_fmm_tree_solve.argtypes = [vp, vpp, vpp]
         lib.octo_fmm_tree_interaction_counts.argtypes = [vp, vpp, vpp, ctypes.POINTER(ctypes.c_ulonglong)]
+        lib.octo_fmm_tree_host_scratch_bytes.restype = ctypes.c_size_t
+        lib.octo_fmm_tree_host_scratch_bytes.argtypes = [tcfgp]
+        lib.octo_fmm_tree_solve_host.argtypes = [vp, vpp, vpp, vp, ctypes.c_size_t]
         lib.octo_fmm_tree_status.argtypes = [vp]
         lib.octo_fmm_tree_launches.argtypes = [vp, ip]
         lib.octo_fmm_tree_destroy.argtypes = [vp]
@@ -532,6 +535,16 @@ def octo_fmm_tree_interaction_counts(t, mass, out):
     if rc != OK:
         raise OctoFmmError("octo_fmm_tree_interaction_counts", rc)
     return {"m2l": int(c[0]), "p2p": int(c[1]), "cross": int(c[2])}
+
+
+def octo_fmm_tree_host_scratch_bytes(cfg):
+    return int(_lib.octo_fmm_tree_host_scratch_bytes(ctypes.byref(cfg)))
+
+
+def octo_fmm_tree_solve_host(t, mass_host, out_host, scratch, scratch_bytes):
+    rc = _lib.octo_fmm_tree_solve_host(t, _ptr_array(mass_host), _ptr_array(out_host), _ptr(scratch), int(scratch_bytes))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_tree_solve_host", rc)
 
 
 def octo_fmm_tree_status(t):

@@ -425,6 +425,47 @@ int octo_fmm_tree_interaction_counts(octo_fmm_tree_t* t, const double* const* ma
     return OCTO_FMM_OK;
 }
 
+size_t octo_fmm_tree_host_scratch_bytes(const octo_fmm_tree_config* cfg)
+{
+    if (!tree_config_ok(cfg)) return 0;
+    size_t total = 0;
+    for (int l = 0; l < cfg->depth; ++l) {
+        const size_t n = (size_t)cfg->n0 << l, nc = n * n * n;
+        total += align_up(nc * 8) + align_up(nc * 4 * 8);
+    }
+    return total;
+}
+
+int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host, double* const* out_host, void* scratch,
+                             size_t scratch_bytes)
+{
+    if (!t || !mass_host || !out_host || !scratch) return OCTO_FMM_EINVAL;
+    if (scratch_bytes < octo_fmm_tree_host_scratch_bytes(&t->cfg) || ((uintptr_t)scratch % ALIGN)) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(t->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    const int D = (int)t->lev.size();
+    std::vector<const double*> m(D);
+    std::vector<double*> o(D);
+    char* w = (char*)scratch;
+    cudaStream_t st = t->stream;
+    for (int l = 0; l < D; ++l) {
+        if (!mass_host[l] || !out_host[l]) return OCTO_FMM_EINVAL;
+        const size_t nc = (size_t)t->lev[l].n * t->lev[l].n * t->lev[l].n;
+        double* dm = (double*)w; w += align_up(nc * 8);
+        o[l] = (double*)w; w += align_up(nc * 4 * 8);
+        m[l] = dm;
+        // a level without leaves has nothing to bring (its masses are never read) and nothing to take back but zeros
+        if (t->lev[l].has_leaf && cudaMemcpyAsync(dm, mass_host[l], nc * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    const int rc = tree_solve_impl(t, m.data(), o.data(), false);
+    if (rc != OCTO_FMM_OK) return rc;
+    for (int l = 0; l < D; ++l) {
+        const size_t nc = (size_t)t->lev[l].n * t->lev[l].n * t->lev[l].n;
+        if (cudaMemcpyAsync(out_host[l], o[l], nc * 4 * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    if (cudaStreamSynchronize(st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    return OCTO_FMM_OK;
+}
+
 int octo_fmm_tree_status(octo_fmm_tree_t* t)
 {
     if (!t) return OCTO_FMM_EINVAL;

@@ -4,10 +4,16 @@ The interaction step shards naturally: sub-grids are independent given the momen
 stencil's reach (5 cells) -- the paper's "boundary data from sibling sub-grids" (L388).  Rank r of a
 torch.distributed group owns the z-layers [r * nz_local, (r + 1) * nz_local) of a grid of nz_local * world layers.
 Before the step it receives HALO = 8 layers of raw moments and centre-of-mass offsets from each z-neighbour (5 are
-needed; 8 keeps the output region aligned to the 8^3 sub-grids) -- ONE exchange of point-to-point messages (NCCL over
+needed; 8 keeps the output region aligned to the 8^3 sub-grids) -- ONE batch of point-to-point messages (NCCL over
 NVLink on GPUs), no collective afterwards: outputs are disjoint.  Everything of the method still runs in the library's
 kernels; this module only moves boundary layers and calls the C ABI on the extended slab with the owned layers as the
 output region.  The lowest and highest rank see the isolated domain boundary (L321) on their outer side.
+
+Data movement: the rank keeps ONE persistent extended array per input, [20][nz_ext][ny][nx] and [3][nz_ext][ny][nx].
+The owned layers are views into it (`ShardedLevel.moments`, `.com_off`: the producer of the moments writes there), the
+neighbours' layers are received straight into its outer layers and sent straight out of its owned layers: for a fixed
+component a z-range of layers is one contiguous block, so the exchange is 23 sends and 23 receives per neighbour in one
+batch with no packing, no concatenation and no transient memory (97 MB per neighbour at 256^2 against a 3 GB slab).
 """
 from __future__ import annotations
 
@@ -21,58 +27,69 @@ def slab_layout(rank: int, world: int, nz_local: int):
     return lo, hi, lo + nz_local + hi
 
 
+def exchange_into(moments_ext, com_ext, rank: int, world: int, group=None):
+    """Halo exchange IN PLACE on the extended arrays [20][nz_ext][ny][nx] / [3][nz_ext][ny][nx] whose owned layers
+    [lo, lo + nz_local) are filled: sends the HALO outermost owned layers of every component to each z-neighbour and
+    receives theirs into the outer layers.  One batch of point-to-point operations (works on CPU tensors with the gloo
+    backend and on CUDA tensors with NCCL); blocks until the layers have arrived.  Returns the number of bytes sent."""
+    import torch.distributed as dist
+    nz_ext = moments_ext.shape[1]
+    lo = HALO if rank > 0 else 0
+    hi = HALO if rank < world - 1 else 0
+    nzl = nz_ext - lo - hi
+    if nzl < HALO:
+        raise ValueError("a slab must have at least %d layers" % HALO)
+    if com_ext.shape[1] != nz_ext or not moments_ext.is_contiguous() or not com_ext.is_contiguous():
+        raise ValueError("extended arrays must be contiguous and of equal z-extent")
+    ops, sent = [], 0
+    for arr in (moments_ext, com_ext):
+        for c in range(arr.shape[0]):
+            if lo:
+                ops.append(dist.P2POp(dist.isend, arr[c, lo:lo + HALO], rank - 1, group))
+                ops.append(dist.P2POp(dist.irecv, arr[c, 0:lo], rank - 1, group))
+                sent += arr[c, lo:lo + HALO].numel() * arr.element_size()
+            if hi:
+                ops.append(dist.P2POp(dist.isend, arr[c, lo + nzl - HALO:lo + nzl], rank + 1, group))
+                ops.append(dist.P2POp(dist.irecv, arr[c, lo + nzl:nz_ext], rank + 1, group))
+                sent += arr[c, lo + nzl - HALO:lo + nzl].numel() * arr.element_size()
+    if ops:
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+    return sent
+
+
 def pack_boundary(moments, com_off, top: bool):
-    """The HALO outermost owned layers (top or bottom) of the 23 per-cell arrays as one contiguous buffer [23][HALO][ny][nx]."""
+    """The HALO outermost owned layers (top or bottom) of the 23 per-cell arrays as one buffer [23][HALO][ny][nx] (what a
+    neighbour receives; used by the single-GPU geometry test to play the neighbour's part)."""
     import torch
     sl = slice(-HALO, None) if top else slice(0, HALO)
     return torch.cat([moments[:, sl], com_off[:, sl]], dim=0).contiguous()
 
 
 def exchange_halos(moments, com_off, rank: int, world: int, group=None):
-    """Returns (moments_ext [20][nz_ext][ny][nx], com_ext [3][nz_ext][ny][nx]): the rank's slab with the neighbours'
-    boundary layers attached.  moments [20][nz_local][ny][nx], com_off [3][...] on the rank's device (CPU tensors with
-    the gloo backend in the tests).  One batch of point-to-point operations; blocks until the layers have arrived."""
+    """Convenience for callers that hold only their owned slab: allocates the extended arrays, copies the slab in and
+    exchanges.  Returns (moments_ext, com_ext).  ShardedLevel does NOT use this (it owns persistent extended arrays)."""
     import torch
-    import torch.distributed as dist
-    nz_local = moments.shape[1]
-    if nz_local < HALO:
-        raise ValueError("a slab must have at least %d layers" % HALO)
-    lo, hi, nz_ext = slab_layout(rank, world, nz_local)
-    shape = (23, HALO) + tuple(moments.shape[2:])
-    ops, recv_lo, recv_hi, keep = [], None, None, []
-    if lo:
-        send = pack_boundary(moments, com_off, top=False)
-        recv_lo = torch.empty(shape, dtype=moments.dtype, device=moments.device)
-        keep.append(send)
-        ops += [dist.P2POp(dist.isend, send, rank - 1, group), dist.P2POp(dist.irecv, recv_lo, rank - 1, group)]
-    if hi:
-        send = pack_boundary(moments, com_off, top=True)
-        recv_hi = torch.empty(shape, dtype=moments.dtype, device=moments.device)
-        keep.append(send)
-        ops += [dist.P2POp(dist.isend, send, rank + 1, group), dist.P2POp(dist.irecv, recv_hi, rank + 1, group)]
-    if ops:
-        for req in dist.batch_isend_irecv(ops):
-            req.wait()
-    return assemble(moments, com_off, recv_lo, recv_hi)
-
-
-def assemble(moments, com_off, below=None, above=None):
-    """Extended slab from the owned layers and the received boundary buffers ([23][HALO][ny][nx] or None)."""
-    import torch
-    mparts, cparts = [], []
-    if below is not None:
-        mparts.append(below[:20]); cparts.append(below[20:])
-    mparts.append(moments); cparts.append(com_off)
-    if above is not None:
-        mparts.append(above[:20]); cparts.append(above[20:])
-    return torch.cat(mparts, dim=1).contiguous(), torch.cat(cparts, dim=1).contiguous()
+    nzl = moments.shape[1]
+    lo, hi, nz_ext = slab_layout(rank, world, nzl)
+    mext = torch.empty((20, nz_ext) + tuple(moments.shape[2:]), dtype=moments.dtype, device=moments.device)
+    cext = torch.empty((3, nz_ext) + tuple(moments.shape[2:]), dtype=moments.dtype, device=moments.device)
+    mext[:, lo:lo + nzl].copy_(moments)
+    cext[:, lo:lo + nzl].copy_(com_off)
+    exchange_into(mext, cext, rank, world, group)
+    return mext, cext
 
 
 class ShardedLevel:
-    """The interaction step of one rank's slab.  `step(moments, com_off)` = halo exchange + set_moments + interact on
-    the extended slab with the owned layers as the output region; returns (L [20][nz_local][ny][nx], Lcorr [3][...])."""
+    """The interaction step of one rank's slab.
+
+    `moments` / `com_off` are the rank's OWNED layers as views into the persistent extended arrays: fill them (e.g.
+    `lvl.moments.copy_(...)`, or let the producer write there) and call `step()` = halo exchange in place + set_moments
+    + interact on the extended slab with the owned layers as the output region.
+    Returns (L [20][nz_local][ny][nx], Lcorr [3][...])."""
 
     def __init__(self, n_local, h, theta, am_correction=True, rank=0, world=1, group=None, device=0, stream=None):
+        import torch
         from . import MULTIPOLE, OctoFMM
         nx, ny, nzl = (int(v) for v in n_local)
         if nzl % 8 or nzl < HALO:
@@ -82,13 +99,23 @@ class ShardedLevel:
         self.n_local = (nx, ny, nzl)
         self.fmm = OctoFMM((nx, ny, self.nz_ext), h, theta, MULTIPOLE, am_correction, out_lo=(0, 0, self.lo),
                            out_hi=(nx, ny, self.lo + nzl), device=device, stream=stream)
+        dev = self.fmm.device
+        self.moments_ext = torch.zeros((20, self.nz_ext, ny, nx), dtype=torch.float64, device=dev)
+        self.com_ext = torch.zeros((3, self.nz_ext, ny, nx), dtype=torch.float64, device=dev)
+        self.moments = self.moments_ext[:, self.lo:self.lo + nzl]
+        self.com_off = self.com_ext[:, self.lo:self.lo + nzl]
+        self.halo_bytes_sent = 0
 
-    def step(self, moments, com_off, L=None, Lcorr=None):
+    def step(self, moments=None, com_off=None, L=None, Lcorr=None):
+        """moments / com_off given: copied into the owned views first (one device copy; callers on the hot path write
+        into `self.moments` / `self.com_off` themselves and pass nothing)."""
+        if moments is not None:
+            self.moments.copy_(moments)
+        if com_off is not None:
+            self.com_off.copy_(com_off)
         if self.world > 1:
-            mext, cext = exchange_halos(moments, com_off, self.rank, self.world, self.group)
-        else:
-            mext, cext = moments, com_off
-        return self.step_extended(mext, cext, L, Lcorr)
+            self.halo_bytes_sent = exchange_into(self.moments_ext, self.com_ext, self.rank, self.world, self.group)
+        return self.step_extended(self.moments_ext, self.com_ext, L, Lcorr)
 
     def step_extended(self, moments_ext, com_ext, L=None, Lcorr=None):
         """The step on an already assembled extended slab ([..][nz_ext][ny][nx])."""

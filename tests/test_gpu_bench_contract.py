@@ -22,7 +22,7 @@ def run_bench(*args):
     return json.loads(lines[0])
 
 
-@pytest.mark.parametrize("workload", ["cfg2", "cfg4", "solve"])
+@pytest.mark.parametrize("workload", ["cfg2", "cfg4", "solve", "tree"])
 def test_bench_line(workload):
     extra = ["--ncell", "32"] if workload != "solve" else ["--ncell", "32"]
     d = run_bench("--workload", workload, "--steps", "2", "--warmup", "1", "--e2e-steps", "1", "--ref-seconds", "0.2", *extra)
@@ -35,6 +35,11 @@ def test_bench_line(workload):
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     c = d["cpu_baseline"]
     assert {"value", "unit", "cores", "kind", "sample"} <= set(c) and c["kind"] == "oracle" and c["cores"] >= 1
+    if workload in ("cfg2", "cfg4"):
+        assert c["single_thread"]["cores"] == 1 and c["single_thread"]["value"] > 0
+        assert "kernel_version" in r
+    if workload == "tree":
+        assert d["config"]["host_entry_bit_identical"] is True and d["config"]["net_force_over_sum_abs_force"] < 1e-13
     e = d["e2e"]
     assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
     assert e["value"] < d["value"] * 1.5                       # copies are inside the e2e region

@@ -23,7 +23,7 @@ def test_slab_layout():
 def _worker(rank, world, port, out):
     import torch
     import torch.distributed as dist
-    from paper_2101_08226_b200.sharded import exchange_halos, slab_layout
+    from paper_2101_08226_b200.sharded import exchange_halos, exchange_into, slab_layout
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -35,7 +35,16 @@ def _worker(rank, world, port, out):
     mext, cext = exchange_halos(gm[:, mine].contiguous(), gc[:, mine].contiguous(), rank, world)
     lo, hi, nz_ext = slab_layout(rank, world, nzl)
     ref = slice(rank * nzl - lo, (rank + 1) * nzl + hi)
-    out[rank] = bool(mext.shape[1] == nz_ext and torch.equal(mext, gm[:, ref]) and torch.equal(cext, gc[:, ref]))
+    ok = bool(mext.shape[1] == nz_ext and torch.equal(mext, gm[:, ref]) and torch.equal(cext, gc[:, ref]))
+    # the in-place route on persistent extended arrays: owned layers filled, outer layers poisoned, exchanged in place
+    pm = torch.full((20, nz_ext, ny, nx), float("nan"), dtype=torch.float64)
+    pc = torch.full((3, nz_ext, ny, nx), float("nan"), dtype=torch.float64)
+    pm[:, lo:lo + nzl] = gm[:, mine]
+    pc[:, lo:lo + nzl] = gc[:, mine]
+    sent = exchange_into(pm, pc, rank, world)
+    ok = ok and torch.equal(pm, gm[:, ref]) and torch.equal(pc, gc[:, ref])
+    ok = ok and sent == ((lo > 0) + (hi > 0)) * 23 * 8 * ny * nx * 8
+    out[rank] = ok
     dist.destroy_process_group()
 
 
