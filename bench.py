@@ -215,7 +215,7 @@ def run_solve(args):
     stream = torch.cuda.current_stream(dev)
     n = args.ncell or 256
     h, mass, phi, r = fi.uniform_sphere(n)
-    s = p.OctoFMMSolver(n, h, args.theta, True, device=local, stream=stream)
+    s = p.OctoFMMSolver(n, h, args.theta, True, device=local, stream=stream, two_rhs=True)
     n_int = s.interaction_count()
     levels, launches = s.num_levels()
     m_d = torch.from_numpy(mass).to(dev)
@@ -252,6 +252,34 @@ def run_solve(args):
     ev3.record(stream)
     torch.cuda.synchronize()
     rhs2_ms = ev2.elapsed_time(ev3) / args.steps
+    # both right-hand sides in one call (octo_fmm_solver_solve2): default, and with the fused kernel on every level
+    both_ms = {}
+    for fused in (0, 1):
+        s.set_option("f2_fused", fused)
+        s.solve2(m_d, dm_d, out, out2)
+        torch.cuda.synchronize()
+        ev4, ev5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev4.record(stream)
+        for _ in range(args.steps):
+            s.solve2(m_d, dm_d, out, out2)
+        ev5.record(stream)
+        torch.cuda.synchronize()
+        both_ms[fused] = ev4.elapsed_time(ev5) / args.steps
+    # like for like: the same two variants with the DIRECT kernel on every level (two launches vs one fused launch)
+    s.set_option("kernel", 1)
+    for fused in (0, 1):
+        s.set_option("f2_fused", fused)
+        s.solve2(m_d, dm_d, out, out2)
+        torch.cuda.synchronize()
+        ev4, ev5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev4.record(stream)
+        for _ in range(args.steps):
+            s.solve2(m_d, dm_d, out, out2)
+        ev5.record(stream)
+        torch.cuda.synchronize()
+        both_ms[2 + fused] = ev4.elapsed_time(ev5) / args.steps
+    s.set_option("kernel", 0)
+    s.set_option("f2_fused", 0)
     s.solve(m_d, out)
     torch.cuda.synchronize()
     # end to end through the host-buffer entry point
@@ -298,6 +326,14 @@ def run_solve(args):
             "second_rhs": {"ms_per_solve": rhs2_ms, "value": n_int / (rhs2_ms * 1e-3), "unit": UNIT,
                            "note": "octo_fmm_solver_solve_rhs2: d(phi)/dt from d(mass)/dt on the same tree and centres, "
                                    "correction off, dipole terms on; timed beside the solve, not part of value"},
+            "two_rhs_one_call": {"ms_solve_plus_rhs2_separately": ms + rhs2_ms, "ms_solve2": both_ms[0],
+                                 "ms_solve2_fused_on_every_level": both_ms[1],
+                                 "ms_solve2_direct_kernels_two_launches_per_level": both_ms[2],
+                                 "ms_solve2_direct_kernels_fused": both_ms[3],
+                                 "note": "octo_fmm_solver_solve2: one upward and one downward pass for both right-hand sides; the "
+                                         "fused kernel (shared list walk, separation, 1/r, radial factors) runs on the "
+                                         "one-warp-per-cell levels by default and, for this measurement, on every level "
+                                         "(m2l_direct2_kernel instead of two launches of the slab-fed kernel)"},
             "clocks": clocks, "gpu_launches": launches * args.steps}
     print(json.dumps(line))
     s.close()

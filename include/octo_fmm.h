@@ -219,6 +219,8 @@ typedef struct {
     void *stream;           /* cudaStream_t, borrowed                                                   */
     void *workspace;        /* device memory, 256-byte aligned, borrowed for the handle's lifetime      */
     size_t workspace_bytes; /* >= octo_fmm_solver_workspace_bytes(cfg)                                  */
+    int two_rhs;            /* 1: also hold the per-level buffers of the second right-hand side, for
+                               octo_fmm_solver_solve2 (about 1.6x the workspace); 0 otherwise              */
 } octo_fmm_solver_config;
 
 size_t octo_fmm_solver_workspace_bytes(const octo_fmm_solver_config *cfg);   /* 0 on invalid configuration */
@@ -237,6 +239,17 @@ int octo_fmm_solver_solve(octo_fmm_solver_t *s, const double *mass, double *out)
  * right-hand sides share the geometry, not the pair arithmetic (DESIGN.md section 10a says why a fused kernel was
  * not built); the leaf sum is a potential-only tensor-core contraction over the 8 children of a parent. */
 int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t *s, const double *dmass, double *dphi_dt);
+/* Both right-hand sides in ONE call (Alg. 1: "Compute g, phi, and d(phi)/dt using the FMM"): out as
+ * octo_fmm_solver_solve, dphi_dt as octo_fmm_solver_solve_rhs2 (same readings: the centres of the density, no correction
+ * for the second).  One upward pass builds both sets of multipoles, one downward pass stages both at every level; on the
+ * levels that run one warp per cell the two share ONE launch (list walk, separation, 1/r, radial factors); on the finer
+ * levels each runs the slab-fed kernel on its own sources (a fused kernel there is selectable with
+ * octo_fmm_solver_set_option(s, "f2_fused", 1); measured slower).  Needs cfg.two_rhs = 1 (ESTATE
+ * otherwise).  All four arrays device, 16-byte aligned.  Asynchronous on the stream. */
+int octo_fmm_solver_solve2(octo_fmm_solver_t *s, const double *mass, const double *dmass, double *out, double *dphi_dt);
+/* "f2_fused": 0 (default) | 1, see above.  "kernel": 0 (default) | 1 -- the slab-fed or the direct interaction kernel on
+ * the levels that do not run one warp per cell (cross-check and measurement; same numbers to round-off). */
+int octo_fmm_solver_set_option(octo_fmm_solver_t *s, const char *key, int value);
 /* The same with HOST buffers: H2D of the masses into scratch, solve, D2H of out, stream synchronise.
  * scratch: device, >= octo_fmm_solver_host_scratch_bytes(cfg), borrowed for the call. */
 size_t octo_fmm_solver_host_scratch_bytes(const octo_fmm_solver_config *cfg);

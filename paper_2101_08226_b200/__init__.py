@@ -43,7 +43,7 @@ class octo_fmm_tree_config(ctypes.Structure):
 class octo_fmm_solver_config(ctypes.Structure):
     _fields_ = [("n", ctypes.c_int), ("h", ctypes.c_double), ("theta", ctypes.c_double), ("am_correction", ctypes.c_int),
                 ("device", ctypes.c_int), ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p),
-                ("workspace_bytes", ctypes.c_size_t)]
+                ("workspace_bytes", ctypes.c_size_t), ("two_rhs", ctypes.c_int)]
 
 
 class _Library:
@@ -105,6 +105,8 @@ class _Library:
         lib.octo_fmm_solver_create.argtypes = [scfgp, ctypes.POINTER(vp)]
         lib.octo_fmm_solver_solve.argtypes = [vp, vp, vp]
         lib.octo_fmm_solver_solve_rhs2.argtypes = [vp, vp, vp]
+        lib.octo_fmm_solver_solve2.argtypes = [vp, vp, vp, vp, vp]
+        lib.octo_fmm_solver_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
         lib.octo_fmm_solver_status.argtypes = [vp]
         lib.octo_fmm_solver_host_scratch_bytes.restype = ctypes.c_size_t
         lib.octo_fmm_solver_host_scratch_bytes.argtypes = [scfgp]
@@ -340,10 +342,11 @@ def octo_fmm_dipole_terms_used(h):
 
 
 # ---- complete uniform-grid solve (octo_fmm_solver_*) ------------------------------------------
-def make_solver_config(n, h, theta, am_correction=True, device=0, stream=0, workspace=0, workspace_bytes=0):
+def make_solver_config(n, h, theta, am_correction=True, device=0, stream=0, workspace=0, workspace_bytes=0, two_rhs=False):
     c = octo_fmm_solver_config()
     c.n, c.h, c.theta, c.am_correction = int(n), float(h), float(theta), int(bool(am_correction))
     c.device, c.stream, c.workspace, c.workspace_bytes = int(device), stream or None, workspace or None, int(workspace_bytes)
+    c.two_rhs = int(bool(two_rhs))
     return c
 
 
@@ -369,6 +372,18 @@ def octo_fmm_solver_solve_rhs2(s, dmass, out):
     rc = _lib.octo_fmm_solver_solve_rhs2(s, _ptr(dmass), _ptr(out))
     if rc != OK:
         raise OctoFmmError("octo_fmm_solver_solve_rhs2", rc)
+
+
+def octo_fmm_solver_solve2(s, mass, dmass, out, dphi_dt):
+    rc = _lib.octo_fmm_solver_solve2(s, _ptr(mass), _ptr(dmass), _ptr(out), _ptr(dphi_dt))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_solve2", rc)
+
+
+def octo_fmm_solver_set_option(s, key, value):
+    rc = _lib.octo_fmm_solver_set_option(s, key.encode(), int(value))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_solver_set_option", rc)
 
 
 def octo_fmm_solver_host_scratch_bytes(cfg):
@@ -431,7 +446,7 @@ def octo_fmm_solver_num_levels(s):
 class OctoFMMSolver:
     """Owns the workspace tensor and the handle of a complete uniform-grid solve."""
 
-    def __init__(self, n, h, theta, am_correction=True, device=0, stream=None):
+    def __init__(self, n, h, theta, am_correction=True, device=0, stream=None, two_rhs=False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("octo_fmm needs a CUDA device (sm_100a); there is no CPU fallback")
@@ -439,7 +454,7 @@ class OctoFMMSolver:
         self.n = int(n)
         self.device = torch.device("cuda", device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        cfg = make_solver_config(n, h, theta, am_correction, device=device, stream=self.stream.cuda_stream)
+        cfg = make_solver_config(n, h, theta, am_correction, device=device, stream=self.stream.cuda_stream, two_rhs=two_rhs)
         nbytes = octo_fmm_solver_workspace_bytes(cfg)
         if nbytes == 0:
             raise OctoFmmError("octo_fmm_solver_workspace_bytes", EINVAL)
@@ -467,6 +482,22 @@ class OctoFMMSolver:
         self._check(out, "out", self.n ** 3)
         octo_fmm_solver_solve_rhs2(self.handle, dmass, out)
         return out
+
+    def solve2(self, mass, dmass, out=None, dphi_dt=None):
+        """Both right-hand sides in one call (needs two_rhs=True): returns (out [4][n][n][n], dphi_dt [n][n][n])."""
+        if out is None:
+            out = self.torch.empty((4, self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
+        if dphi_dt is None:
+            dphi_dt = self.torch.empty((self.n, self.n, self.n), dtype=self.torch.float64, device=self.device)
+        self._check(mass, "mass", self.n ** 3)
+        self._check(dmass, "dmass", self.n ** 3)
+        self._check(out, "out", 4 * self.n ** 3)
+        self._check(dphi_dt, "dphi_dt", self.n ** 3)
+        octo_fmm_solver_solve2(self.handle, mass, dmass, out, dphi_dt)
+        return out, dphi_dt
+
+    def set_option(self, key, value):
+        octo_fmm_solver_set_option(self.handle, key, value)
 
     def status(self):
         return octo_fmm_solver_status(self.handle)

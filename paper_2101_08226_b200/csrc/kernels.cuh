@@ -624,6 +624,125 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const __grid_constant__ P
 }
 
 // ------------------------------------------------------------------------------------------
+// Two right-hand sides in ONE pass (Alg. 1: "Compute g, phi, and d(phi)/dt using
+// the FMM"): the density (sources p.S, correction as configured) and its time derivative (sources S2: the moments of
+// d(rho)/dt about the SAME centres, staged with the correction off; no correction, dipole terms always) share the
+// interaction list, the separation R, 1/|R| and the radial factors of every pair; each keeps its own accumulators and
+// its own pair body.  Outputs: p.L / p.C for the density, q.L / q.C for the second right-hand side (q.C gets zeros).
+// m2l_warp2_kernel: one warp per target cell (coarse levels); m2l_direct2_kernel: one thread per target cell, sources
+// from global memory (the measured variant for the fine levels).
+// ------------------------------------------------------------------------------------------
+#define OCTO_LOAD_SOURCE2(q, stride, src)                                                  \
+    {                                                                                     \
+        double2 v_[8];                                                                    \
+        _Pragma("unroll") for (int c_ = 0; c_ < 8; ++c_) v_[c_] = (q)[(long long)c_ * (stride)]; \
+        _Pragma("unroll") for (int c_ = 0; c_ < 8; ++c_) { src[2 * c_] = v_[c_].x; src[2 * c_ + 1] = v_[c_].y; } \
+    }
+
+template <bool CORR>
+__global__ void __launch_bounds__(256) m2l_warp2_kernel(const __grid_constant__ Params p, const __grid_constant__ Params q)
+{
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const long long t = (long long)blockIdx.x * 8 + warp;
+    if (t >= (long long)p.ox * p.oy * p.oz) return;
+    const int gx = p.lo[0] + (int)(t % p.ox), gy = p.lo[1] + (int)((t / p.ox) % p.oy), k = p.lo[2] + (int)(t / ((long long)p.ox * p.oy));
+    const int cls = (gx & 1) + 2 * (gy & 1) + 4 * (k & 1);
+    const long long plane = (long long)p.ny * p.nx;
+    const double2* S1 = reinterpret_cast<const double2*>(p.S);
+    const double2* S2 = reinterpret_cast<const double2*>(q.S);
+    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
+    double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    const double t0[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    load_target<CORR>(p, gx, gy, k, dA, tA);
+    Acc acc, acc2;
+    acc_zero(acc);
+    acc_zero(acc2);
+    const int s_end = c_begin[cls][2 * REACH_MAX + 1];
+#pragma unroll 1
+    for (int s = c_begin[cls][0] + lane; s < s_end; s += 32) {
+        const StEntry e = c_entries[cls * MAX_LIST + s];
+        const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+        if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
+        const long long o = (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
+        double src[16], src2[16], bx_, by_, bz_;
+        OCTO_LOAD_SOURCE(S1 + o, plane, src, bx_, by_, bz_);
+        OCTO_LOAD_SOURCE2(S2 + o, plane, src2);
+        const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
+        const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
+        const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+        const double w = pair_head(x, y, z);
+        if (dipole) m2l_pair<CORR, true>(acc, x, y, z, w, src, tA);
+        else        m2l_pair<CORR, false>(acc, x, y, z, w, src, tA);
+        m2l_pair<false, true>(acc2, x, y, z, w, src2, t0);
+    }
+    double* v = reinterpret_cast<double*>(&acc);
+    double* v2 = reinterpret_cast<double*>(&acc2);
+#pragma unroll
+    for (int c = 0; c < ACC_DOUBLES; ++c) {
+        double a = v[c], b = v2[c];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a += __shfl_xor_sync(0xffffffffu, a, o);
+            b += __shfl_xor_sync(0xffffffffu, b, o);
+        }
+        v[c] = a;
+        v2[c] = b;
+    }
+    if (lane == 0) {
+        store_target<CORR>(p, acc, tA, dA, gx, gy, k);
+        store_target<false>(q, acc2, t0, dA, gx, gy, k);
+    }
+}
+
+template <bool CORR>
+__global__ void __launch_bounds__(256) m2l_direct2_kernel(const __grid_constant__ Params p, const __grid_constant__ Params q)
+{
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31;
+    const int px = warp & 1, py = (warp >> 1) & 1, pz = warp >> 2;
+    const int bx = (p.ox + 15) / 16, by = (p.oy + 7) / 8;
+    const int b = blockIdx.x;
+    const int x0 = p.lo[0] + (b % bx) * 16, y0 = p.lo[1] + ((b / bx) % by) * 8, z0 = p.lo[2] + (b / (bx * by)) * 4;
+    const int gx = x0 + px + 2 * (lane & 7), gy = y0 + py + 2 * (lane >> 3);
+    const long long plane = (long long)p.ny * p.nx;
+    const double2* S1 = reinterpret_cast<const double2*>(p.S);
+    const double2* S2 = reinterpret_cast<const double2*>(q.S);
+    const int cls = warp;
+    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
+    const double t0[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int pass = 0; pass < 2; ++pass) {
+        const int k = z0 + pz + 2 * pass;
+        if (!(gx < p.hi[0] && gy < p.hi[1] && k < p.hi[2])) continue;
+        double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+        load_target<CORR>(p, gx, gy, k, dA, tA);
+        Acc acc, acc2;
+        acc_zero(acc);
+        acc_zero(acc2);
+        const int s_end = c_begin[cls][2 * REACH_MAX + 1];
+#pragma unroll 1
+        for (int s = c_begin[cls][0]; s < s_end; ++s) {
+            const StEntry e = c_entries[cls * MAX_LIST + s];
+            const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+            if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
+            const long long o = (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
+            double src[16], src2[16], bx_, by_, bz_;
+            OCTO_LOAD_SOURCE(S1 + o, plane, src, bx_, by_, bz_);
+            OCTO_LOAD_SOURCE2(S2 + o, plane, src2);
+            const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
+            const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
+            const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+            const double w = pair_head(x, y, z);
+            if (dipole) m2l_pair<CORR, true>(acc, x, y, z, w, src, tA);
+            else        m2l_pair<CORR, false>(acc, x, y, z, w, src, tA);
+            m2l_pair<false, true>(acc2, x, y, z, w, src2, t0);
+        }
+        store_target<CORR>(p, acc, tA, dA, gx, gy, k);
+        store_target<false>(q, acc2, t0, dA, gx, gy, k);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
 // a5: monopole (leaf) variant.  R = (i_A - i_B) h has no per-cell part, so -1/|R| and
 // -R/|R|^3 depend on the offset Delta only: they are tabulated for the 11^3 offsets on the host
 // in FP64 and the kernel is a 4-FMA stencil sum.

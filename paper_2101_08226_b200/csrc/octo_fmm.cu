@@ -730,6 +730,41 @@ int octo_fmm_interact(octo_fmm_t* h)
     return OCTO_FMM_OK;
 }
 
+// Two right-hand sides in one pass (solver.inl, octo_fmm_solver_solve2): h1 = the density's handle (sources staged,
+// correction as configured), h2 = the handle of d(rho)/dt on the same grid (sources staged with the correction off).
+// fused_kind: 2 = one warp per cell (m2l_warp2_kernel), 1 = one thread per cell from global memory (m2l_direct2_kernel).
+static int interact2(octo_fmm_t* h1, octo_fmm_t* h2, int fused_kind)
+{
+    if (!h1 || !h2 || h1->cfg.kind != OCTO_FMM_MULTIPOLE || h2->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
+    if (h1->state < 1 || h2->state < 1) return OCTO_FMM_ESTATE;
+    for (int a = 0; a < 3; ++a)
+        if (h1->cfg.n[a] != h2->cfg.n[a] || h1->lo[a] != h2->lo[a] || h1->hi[a] != h2->hi[a]) return OCTO_FMM_EINVAL;
+    if (h2->cfg.am_correction || h1->stream != h2->stream) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(h1->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    BankLock guard(h1);
+    if (bank_acquire(h1) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    if (cudaMemsetAsync(h1->flags, 0, sizeof(int), h1->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    Params P = h1->prm, Q = h2->prm;
+    P.L = h1->outL; P.C = h1->outC; P.pL = nullptr;
+    Q.L = h2->outL; Q.C = h2->outC; Q.pL = nullptr;
+    if (fused_kind == 2) {
+        const unsigned blocks = (unsigned)(((long long)P.ox * P.oy * P.oz + 7) / 8);
+        if (h1->cfg.am_correction) m2l_warp2_kernel<true><<<blocks, 256, 0, h1->stream>>>(P, Q);
+        else                       m2l_warp2_kernel<false><<<blocks, 256, 0, h1->stream>>>(P, Q);
+    } else {
+        if (h1->cfg.am_correction) m2l_direct2_kernel<true><<<brick_blocks(P), 256, 0, h1->stream>>>(P, Q);
+        else                       m2l_direct2_kernel<false><<<brick_blocks(P), 256, 0, h1->stream>>>(P, Q);
+    }
+    if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (bank_reader_done(h1) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    for (octo_fmm_t* h : {h1, h2}) {
+        h->state = 2;
+        h->mixed = false;
+        h->resL = h->outL; h->resC = h->outC;
+    }
+    return OCTO_FMM_OK;
+}
+
 // number of near-field pairs with a leaf on either side (for the bit-exact check of the pair set)
 __global__ void __launch_bounds__(256) count_near_kernel(const Params p, const unsigned char* __restrict__ leaf,
                                                          unsigned long long* __restrict__ count)

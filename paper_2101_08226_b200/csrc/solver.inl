@@ -16,6 +16,8 @@ struct SolverLevel {
     double* raw;          // [20][n^3] raw moments (M2M output, set_moments input)
     double* off;          // [3][n^3] centre-of-mass offsets
     size_t ws_bytes;      // handle workspace
+    octo_fmm* fmm2;       // two_rhs: the handle of the second right-hand side (correction off), its own sources and results
+    double* raw2;         // two_rhs: [20][n^3] raw moments of d(rho)/dt about the density's centres
 };
 
 octo_fmm_config level_config(const octo_fmm_solver_config& sc, int n, double h, int kind)
@@ -57,6 +59,8 @@ struct octo_fmm_solver {
     cudaStream_t stream;
     unsigned long long n_interactions;
     bool have_centres;    // solve() has run: lev[].off hold the expansion centres of the density
+    int f2_fused;         // solve2(): 0 = fused kernel on the one-warp-per-cell levels only (default), 1 = also on the
+                          // finer levels (m2l_direct2_kernel instead of two launches of the slab-fed kernel)
 };
 
 extern "C" {
@@ -72,6 +76,7 @@ size_t octo_fmm_solver_workspace_bytes(const octo_fmm_solver_config* cfg)
         octo_fmm_config mc = level_config(*cfg, n, h, OCTO_FMM_MULTIPOLE);
         const size_t nc = (size_t)n * n * n;
         total += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
+        if (cfg->two_rhs) total += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8);
     }
     return total;
 }
@@ -81,8 +86,10 @@ int octo_fmm_solver_destroy(octo_fmm_solver_t* s)
     if (!s) return OCTO_FMM_EINVAL;
     int rc = OCTO_FMM_OK;
     if (s->leaf && octo_fmm_destroy(s->leaf) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
-    for (SolverLevel& l : s->lev)
+    for (SolverLevel& l : s->lev) {
         if (l.fmm && octo_fmm_destroy(l.fmm) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+        if (l.fmm2 && octo_fmm_destroy(l.fmm2) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+    }
     delete s;
     return rc;
 }
@@ -101,6 +108,7 @@ int octo_fmm_solver_create(const octo_fmm_solver_config* cfg, octo_fmm_solver_t*
     s->stream = (cudaStream_t)cfg->stream;
     s->n_interactions = 0;
     s->have_centres = false;
+    s->f2_fused = 0;
     char* w = (char*)cfg->workspace;
     {
         octo_fmm_config lc = level_config(*cfg, cfg->n, cfg->h, OCTO_FMM_MONOPOLE);
@@ -115,14 +123,21 @@ int octo_fmm_solver_create(const octo_fmm_solver_config* cfg, octo_fmm_solver_t*
     for (int n = cfg->n / 2; n >= 2; n /= 2) {
         h *= 2.0;
         SolverLevel l;
-        l.n = n; l.h = h; l.fmm = nullptr;
+        l.n = n; l.h = h; l.fmm = nullptr; l.fmm2 = nullptr; l.raw2 = nullptr;
         octo_fmm_config mc = level_config(*cfg, n, h, OCTO_FMM_MULTIPOLE);
         const size_t nc = (size_t)n * n * n;
         l.ws_bytes = sizes_of(mc, CF_ANY_SIZE).total;
         mc.workspace = w; mc.workspace_bytes = l.ws_bytes; w += l.ws_bytes;
         l.raw = (double*)w; w += align_up(nc * 20 * 8);
         l.off = (double*)w; w += align_up(nc * 3 * 8);
-        const int rc = create_internal(&mc, CF_ANY_SIZE, &l.fmm);
+        int rc = create_internal(&mc, CF_ANY_SIZE, &l.fmm);
+        if (rc == OCTO_FMM_OK && cfg->two_rhs) {
+            octo_fmm_config m2 = mc;
+            m2.am_correction = 0;                     // the correction belongs to the force (L127)
+            m2.workspace = w; m2.workspace_bytes = l.ws_bytes; w += l.ws_bytes;
+            l.raw2 = (double*)w; w += align_up(nc * 20 * 8);
+            rc = create_internal(&m2, CF_ANY_SIZE, &l.fmm2);
+        }
         s->lev.push_back(l);
         if (rc != OCTO_FMM_OK) { octo_fmm_solver_destroy(s); return rc; }
         s->n_interactions += l.fmm->n_interactions;
@@ -237,6 +252,108 @@ int octo_fmm_solver_solve_rhs2(octo_fmm_solver_t* s, const double* dmass, double
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     return OCTO_FMM_OK;
+}
+
+// Both right-hand sides in ONE call (L81-83, Alg. 1 "Compute g, phi, and d(phi)/dt using the FMM"):
+// one upward pass that builds the density's multipoles and centres and, about those centres, the multipoles of
+// d(rho)/dt; one downward pass in which every level stages both source sets and
+//   - on the levels that run one warp per cell: ONE fused launch (m2l_warp2_kernel: list walk, separation, 1/r and
+//     radial factors shared by the two right-hand sides);
+//   - on the finer levels: two launches of the slab-fed kernel (default; the fused m2l_direct2_kernel is selectable,
+//     "f2_fused" = 1 -- measured slower);
+// then the two leaf sums.  Needs a solver created with cfg.two_rhs = 1 (second set of per-level buffers).
+int octo_fmm_solver_solve2(octo_fmm_solver_t* s, const double* mass, const double* dmass, double* out, double* dphi_dt)
+{
+    if (!s || !mass || !dmass || !out || !dphi_dt) return OCTO_FMM_EINVAL;
+    if (((uintptr_t)mass % 16) || ((uintptr_t)dmass % 16) || ((uintptr_t)out % 16) || ((uintptr_t)dphi_dt % 16)) return OCTO_FMM_EINVAL;
+    if (!s->cfg.two_rhs) return OCTO_FMM_ESTATE;
+    if (cudaSetDevice(s->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    cudaStream_t st = s->stream;
+    int rc;
+    // ---- upward pass: density first (it fixes the centres), then d(rho)/dt about them ----
+    for (size_t lv = 0; lv < s->lev.size(); ++lv) {
+        SolverLevel& l = s->lev[lv];
+        const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
+        if (lv == 0) {
+            m2m_kernel<true><<<blocks, 128, 0, st>>>(mass, nullptr, l.raw, l.off, l.n, l.n, l.n, s->cfg.h);
+            m2m_kernel<true, true><<<blocks, 128, 0, st>>>(dmass, nullptr, l.raw2, l.off, l.n, l.n, l.n, s->cfg.h);
+        } else {
+            SolverLevel& c = s->lev[lv - 1];
+            m2m_kernel<false><<<blocks, 128, 0, st>>>(c.raw, c.off, l.raw, l.off, l.n, l.n, l.n, c.h);
+            m2m_kernel<false, true><<<blocks, 128, 0, st>>>(c.raw2, c.off, l.raw2, l.off, l.n, l.n, l.n, c.h);
+        }
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    // ---- downward pass, coarsest first ----
+    for (int lv = (int)s->lev.size() - 1; lv >= 0; --lv) {
+        SolverLevel& l = s->lev[lv];
+        if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
+        if ((rc = octo_fmm_set_moments(l.fmm2, l.raw2, l.off)) != OCTO_FMM_OK) return rc;
+        const bool has_parent = lv < (int)s->lev.size() - 1;
+        const int fused_kind = l.fmm->kernel == 2 ? 2 : (s->f2_fused && l.fmm->kernel != 2 ? 1 : 0);
+        bool l2l_fused = false;
+        if (fused_kind) {
+            if ((rc = interact2(l.fmm, l.fmm2, fused_kind)) != OCTO_FMM_OK) return rc;
+        } else {
+            l2l_fused = has_parent && l.fmm->kernel == 0;
+            if (l2l_fused) { set_parent(l.fmm, s->lev[lv + 1]); l.fmm2->prm.pL = s->lev[lv + 1].fmm2->L; l.fmm2->prm.pC = s->lev[lv + 1].fmm2->C; l.fmm2->prm.poff = s->lev[lv + 1].off; }
+            rc = octo_fmm_interact(l.fmm);
+            if (rc == OCTO_FMM_OK) rc = octo_fmm_interact(l.fmm2);
+            if (l2l_fused) { clear_parent(l.fmm); clear_parent(l.fmm2); }
+            if (rc != OCTO_FMM_OK) return rc;
+        }
+        const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
+        if (!has_parent) {
+            l2l_kernel<false><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, nullptr, nullptr, nullptr, l.n, l.n, l.n, l.h);
+        } else if (!l2l_fused) {
+            SolverLevel& p = s->lev[lv + 1];
+            l2l_kernel<true><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, p.fmm->L, p.fmm->C, p.off, l.n, l.n, l.n, l.h);
+            l2l_kernel<true><<<blocks, 128, 0, st>>>(l.fmm2->L, l.fmm2->C, l.off, p.fmm2->L, p.fmm2->C, p.off, l.n, l.n, l.n, l.h);
+        }
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    // ---- leaves: the density's (phi, g) with the fused evaluation, then the potential of the second right-hand side ----
+    if ((rc = octo_fmm_set_moments(s->leaf, mass, nullptr)) != OCTO_FMM_OK) return rc;
+    {
+        double* const keep = s->leaf->outL;
+        const bool fused_eval = s->leaf->mono_kernel == 0;
+        s->leaf->outL = out;
+        if (fused_eval) set_parent(s->leaf, s->lev[0]);
+        rc = octo_fmm_interact(s->leaf);
+        if (fused_eval) clear_parent(s->leaf);
+        s->leaf->outL = keep;
+        if (rc != OCTO_FMM_OK) return rc;
+        const int n = s->cfg.n;
+        const dim3 pb((unsigned)((n / 2 + 127) / 128), (unsigned)(n / 2), (unsigned)(n / 2));
+        SolverLevel& p = s->lev[0];
+        if (!fused_eval) leaf_eval_kernel<false><<<pb, 128, 0, st>>>(out, p.fmm->L, p.fmm->C, p.off, n, n, n, s->cfg.h);
+        if ((rc = octo_fmm_set_moments(s->leaf, dmass, nullptr)) != OCTO_FMM_OK) return rc;
+        if ((rc = interact_potential(s->leaf, dphi_dt)) != OCTO_FMM_OK) return rc;
+        leaf_eval_kernel<true><<<pb, 128, 0, st>>>(dphi_dt, p.fmm2->L, p.fmm2->C, p.off, n, n, n, s->cfg.h);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    s->have_centres = true;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_solver_set_option(octo_fmm_solver_t* s, const char* key, int value)
+{
+    if (!s || !key) return OCTO_FMM_EINVAL;
+    if (!std::strcmp(key, "f2_fused")) {
+        if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
+        s->f2_fused = value;
+        return OCTO_FMM_OK;
+    }
+    if (!std::strcmp(key, "kernel")) {       // 0 = slab-fed kernel (default), 1 = direct kernel, on the levels that do not run one warp per cell
+        if (value != 0 && value != 1) return OCTO_FMM_EINVAL;
+        for (SolverLevel& l : s->lev) {
+            if (l.fmm->kernel == 2 || l.n % 8) continue;
+            l.fmm->kernel = value;
+            if (l.fmm2) l.fmm2->kernel = value;
+        }
+        return OCTO_FMM_OK;
+    }
+    return OCTO_FMM_EINVAL;
 }
 
 size_t octo_fmm_solver_host_scratch_bytes(const octo_fmm_solver_config* cfg)

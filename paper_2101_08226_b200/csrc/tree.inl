@@ -273,7 +273,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     for (int n = cfg->n0 / 2; n >= 2 && rc == OCTO_FMM_OK; n /= 2) {
         h *= 2.0;
         SolverLevel l;
-        l.n = n; l.h = h; l.fmm = nullptr;
+        l.n = n; l.h = h; l.fmm = nullptr; l.fmm2 = nullptr; l.raw2 = nullptr;
         octo_fmm_config mc = level_config(sc, n, h, OCTO_FMM_MULTIPOLE);
         const size_t nc = (size_t)n * n * n;
         l.ws_bytes = sizes_of(mc, CF_ANY_SIZE).total;

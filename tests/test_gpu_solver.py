@@ -174,3 +174,37 @@ def test_second_right_hand_side_32(env, theta):
     e_phi, e_g = _errors(out.cpu().numpy(), ref)
     assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
     s.close()
+
+
+@pytest.mark.parametrize("theta,n", [(0.5, 32), (0.35, 32), (0.5, 64)])
+def test_both_right_hand_sides_in_one_call(env, theta, n):
+    """octo_fmm_solver_solve2 (f2: L81-83, Alg. 1): (phi, g) of the density AND d(phi)/dt of its time derivative from
+    ONE call -- against oracle.solve and oracle.solve_rhs2 at 1e-12, with the fused kernel on the one-warp-per-cell levels
+    only (default) and on every level ("f2_fused" = 1), and against the two separate calls."""
+    p, torch = env
+    h = 1.0 / n
+    rng = np.random.default_rng(12 + n)
+    mass = rng.uniform(0.5, 1.5, (n, n, n)) * h ** 3
+    dm = rng.uniform(-1.0, 1.0, (n, n, n)) * h ** 3
+    dm -= dm.mean()
+    ref = oracle.solve(n, h, theta, mass, True)
+    ref2 = oracle.solve_rhs2(n, h, theta, mass, dm)[0]
+    s = p.OctoFMMSolver(n, h, theta, True, two_rhs=True)
+    m_d, dm_d = torch.from_numpy(mass).cuda(), torch.from_numpy(dm).cuda()
+    sep = s.solve(m_d).clone()
+    sep2 = s.solve_rhs2(dm_d).clone()
+    for fused in (0, 1):
+        s.set_option("f2_fused", fused)
+        out, dphi = s.solve2(m_d, dm_d)
+        torch.cuda.synchronize()
+        assert s.status() == p.OK
+        e_phi, e_g = _errors(out.cpu().numpy(), ref)
+        e2 = np.abs(dphi.cpu().numpy() - ref2).max() / np.abs(ref2).max()
+        assert e_phi < TOL and e_g < TOL and e2 < TOL, (fused, e_phi, e_g, e2)
+        assert float((out - sep).abs().max() / sep.abs().max()) < 1e-13
+        assert float((dphi - sep2).abs().max() / sep2.abs().max()) < 1e-13
+    s.close()
+    plain = p.OctoFMMSolver(n, h, theta, True)
+    with pytest.raises(p.OctoFmmError):                      # needs the second set of buffers
+        plain.solve2(m_d, dm_d)
+    plain.close()
