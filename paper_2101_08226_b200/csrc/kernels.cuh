@@ -85,6 +85,8 @@ struct Params {
     double hmul[2 * REACH_MAX + 1];   // (double)(-d) * h for d = -5..5  (= (i_A - i_B) h), per handle
     const int* tile_list;        // levels of an adaptive tree: the bricks (ids in the dense enumeration) that have work;
                                  // nullptr = all ntiles bricks.  With a list, ntiles is its length.
+    int tile_offset;             // tensor-core monopole kernels without a list: first tile of this launch (the host entry
+                                 // points launch the level in chunks of z-tiles so that the copy out overlaps the rest)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -964,7 +966,7 @@ p2p_monopole_dmma_kernel(const __grid_constant__ CUtensorMap tmap, const Params 
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
     const int bx = (p.ox + MT_X - 1) / MT_X, by = (p.oy + MT_Y - 1) / MT_Y;
-    const int b = p.tile_list ? p.tile_list[blockIdx.x] : blockIdx.x;       // tree levels: only the tiles that hold leaf cells
+    const int b = p.tile_list ? p.tile_list[blockIdx.x] : (int)blockIdx.x + p.tile_offset;   // tree levels: only the tiles that hold leaf cells
     const int x0 = p.lo[0] + (b % bx) * MT_X, y0 = p.lo[1] + ((b / bx) % by) * MT_Y, z0 = p.lo[2] + (b / (bx * by)) * DT_Z;
 
     if (threadIdx.x == 0) {

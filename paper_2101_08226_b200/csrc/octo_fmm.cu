@@ -296,6 +296,8 @@ struct octo_fmm {
     const unsigned char* tree_kind;   // device [n^3]; non-null: the slab-fed kernel runs in MODE_TREE
     const int* tile_list;             // device; null = every brick (multipole) / tile (monopole)
     int tile_count;
+    int mono_zt_begin, mono_zt_end;   // tensor-core monopole kernels: z-tiles [begin, end) of this launch; end = 0: all
+    int* pinned_flag;      // pinned host word the host entry points read the device flag through (no pageable copy)
     bool pipeline_ready;   // the side streams and events below all exist
     cudaStream_t s_h2d, s_d2h;
     cudaEvent_t ev_in[32], ev_out[32], ev_begin, ev_end;
@@ -352,6 +354,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->host_chunk = 12;
     h->host_launches = 0;
     h->tree_kind = nullptr; h->tile_list = nullptr; h->tile_count = 0;
+    h->mono_zt_begin = 0; h->mono_zt_end = 0; h->pinned_flag = nullptr;
     h->pipeline_ready = false;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
     for (int i = 0; i < MAX_CHUNKS; ++i) { h->ev_in[i] = nullptr; h->ev_out[i] = nullptr; }
@@ -486,6 +489,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.pL = nullptr; P.pC = nullptr; P.poff = nullptr; P.hc = cfg->h;
     P.leaf = nullptr;
     P.tile_list = nullptr;
+    P.tile_offset = 0;
     for (int d = 0; d <= 2 * REACH_MAX; ++d) P.hmul[d] = h->hmul[d];
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
@@ -706,10 +710,18 @@ int octo_fmm_interact(octo_fmm_t* h)
             Q.tile_list = h->tile_list;
             if (h->tile_count > 0)
                 p2p_monopole_dmma_kernel<false><<<h->tile_count, DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, Q, h->T, h->dl, h->outL);
-        } else if (h->mono_kernel == 0 && P.pL) // complete solve: leaf evaluation fused into the epilogue (solver.inl)
-            p2p_monopole_dmma_kernel<true><<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
-        else if (h->mono_kernel == 0)
-            p2p_monopole_dmma_kernel<false><<<dmma_blocks(P), DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, P, h->T, h->dl, h->outL);
+        } else if (h->mono_kernel == 0) {
+            // all tiles, or (host entry points) the z-tiles [mono_zt_begin, mono_zt_end) only
+            const int per_z = ((P.ox + MT_X - 1) / MT_X) * ((P.oy + MT_Y - 1) / MT_Y);
+            Params Q = P;
+            int blocks = dmma_blocks(P);
+            if (h->mono_zt_end > 0) { Q.tile_offset = h->mono_zt_begin * per_z; blocks = (h->mono_zt_end - h->mono_zt_begin) * per_z; }
+            if (blocks <= 0) return OCTO_FMM_EINVAL;
+            if (P.pL)      // complete solve: leaf evaluation fused into the epilogue (solver.inl)
+                p2p_monopole_dmma_kernel<true><<<blocks, DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, Q, h->T, h->dl, h->outL);
+            else
+                p2p_monopole_dmma_kernel<false><<<blocks, DMMA_THREADS, DMMA_SMEM, h->stream>>>(h->tmap2, Q, h->T, h->dl, h->outL);
+        }
         else
             p2p_monopole_kernel<<<mono_blocks(P), MONO_THREADS, MONO_SMEM, h->stream>>>(h->tmap, P, h->W, h->outL);
     } else if (h->kernel == 1) {
@@ -925,6 +937,7 @@ int octo_fmm_destroy(octo_fmm_t* h)
     }
     if (h->ev_begin) cudaEventDestroy(h->ev_begin);
     if (h->ev_end) cudaEventDestroy(h->ev_end);
+    if (h->pinned_flag) cudaFreeHost(h->pinned_flag);
     delete h;
     return e == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
@@ -970,6 +983,23 @@ int octo_fmm_interaction_count(const octo_fmm_t* h, unsigned long long* n)
     return OCTO_FMM_OK;
 }
 
+// side streams and events of the host entry points, created piece by piece; whatever exists is destroyed by
+// octo_fmm_destroy (the handle is zero-initialised)
+static int ensure_pipeline(octo_fmm_t* h)
+{
+    if (h->pipeline_ready) return OCTO_FMM_OK;
+    if (!h->s_h2d && cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (!h->s_d2h && cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
+    for (int i = 0; i < MAX_CHUNKS; ++i)
+        if ((!h->ev_in[i] && cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming) != cudaSuccess) ||
+            (!h->ev_out[i] && cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming) != cudaSuccess)) return OCTO_FMM_ECUDA;
+    if ((!h->ev_begin && cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming) != cudaSuccess) ||
+        (!h->ev_end && cudaEventCreateWithFlags(&h->ev_end, cudaEventDisableTiming) != cudaSuccess)) return OCTO_FMM_ECUDA;
+    if (!h->pinned_flag && cudaHostAlloc((void**)&h->pinned_flag, 2 * sizeof(int), cudaHostAllocDefault) != cudaSuccess) return OCTO_FMM_ECUDA;
+    h->pipeline_ready = true;
+    return OCTO_FMM_OK;
+}
+
 // Whole step on host buffers, pipelined over slabs of z-layers (multipole kind, staged kernel):
 // the host->device copy of slab c+1, the staging + interaction kernels of slab c and the
 // device->host copy of slab c-1 run concurrently on three streams (PCIe is full duplex), so the
@@ -980,17 +1010,7 @@ static int run_host_pipelined(octo_fmm_t* h, const double* mom_h, const double* 
                               double* d_m, double* d_c, double* d_L, double* d_C)
 {
     const Params& P = h->prm;
-    if (!h->pipeline_ready) {
-        // created piece by piece; whatever exists is destroyed by octo_fmm_destroy (the handle is zero-initialised)
-        if (!h->s_h2d && cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
-        if (!h->s_d2h && cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
-        for (int i = 0; i < MAX_CHUNKS; ++i)
-            if ((!h->ev_in[i] && cudaEventCreateWithFlags(&h->ev_in[i], cudaEventDisableTiming) != cudaSuccess) ||
-                (!h->ev_out[i] && cudaEventCreateWithFlags(&h->ev_out[i], cudaEventDisableTiming) != cudaSuccess)) return OCTO_FMM_ECUDA;
-        if ((!h->ev_begin && cudaEventCreateWithFlags(&h->ev_begin, cudaEventDisableTiming) != cudaSuccess) ||
-            (!h->ev_end && cudaEventCreateWithFlags(&h->ev_end, cudaEventDisableTiming) != cudaSuccess)) return OCTO_FMM_ECUDA;
-        h->pipeline_ready = true;
-    }
+    if (ensure_pipeline(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     int zc = h->host_chunk;
     while ((P.oz + zc - 1) / zc + 4 > MAX_CHUNKS) zc += TILE_Z;
     // Slab boundaries.  The bus is the bottleneck, so what the pipeline adds to the pure copy time is its fill (the
@@ -1089,9 +1109,36 @@ int octo_fmm_run_host(octo_fmm_t* h, const double* moments_host, const double* c
     double* d_L = (double*)w; w += align_up(ocell * (multi ? 20 : 4) * 8);
     double* d_C = multi ? (double*)w : nullptr;
     if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (ensure_pipeline(h) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     if (multi && h->kernel == 0 && h->host_chunk > 0) {
         const int rc = run_host_pipelined(h, moments_host, com_off_host, L_host, Lcorr_host, d_m, d_c, d_L, d_C);
         if (rc != OCTO_FMM_OK) return rc;
+    } else if (!multi && h->mono_kernel == 0 && !h->tile_list && h->host_chunk > 0) {
+        // monopole kind on the tensor-core kernel: the level is launched in chunks of z-tiles and every chunk of the
+        // result goes back on a side stream while the next chunks are computed (the outputs are 4x the inputs)
+        if (cudaMemcpyAsync(d_m, moments_host, ncell * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+        int rc = octo_fmm_set_moments(h, d_m, nullptr);
+        if (rc != OCTO_FMM_OK) return rc;
+        double* const keepL = h->outL;
+        h->outL = d_L;
+        const int ztiles = (P.oz + DT_Z - 1) / DT_Z, nchunk = std::min(8, ztiles);
+        const size_t oplane = (size_t)P.ox * P.oy;
+        for (int c = 0; c < nchunk && rc == OCTO_FMM_OK; ++c) {
+            const int a = (int)((long long)ztiles * c / nchunk), b = (int)((long long)ztiles * (c + 1) / nchunk);
+            h->mono_zt_begin = a; h->mono_zt_end = b;
+            rc = octo_fmm_interact(h);
+            if (rc != OCTO_FMM_OK) break;
+            const int z0 = a * DT_Z, z1 = std::min(b * DT_Z, P.oz);
+            if (cudaEventRecord(h->ev_out[c], h->stream) != cudaSuccess || cudaStreamWaitEvent(h->s_d2h, h->ev_out[c], 0) != cudaSuccess ||
+                cudaMemcpy2DAsync(L_host + (size_t)z0 * oplane, ocell * 8, d_L + (size_t)z0 * oplane, ocell * 8,
+                                  (size_t)(z1 - z0) * oplane * 8, 4, cudaMemcpyDeviceToHost, h->s_d2h) != cudaSuccess)
+                rc = OCTO_FMM_ECUDA;
+        }
+        h->mono_zt_begin = 0; h->mono_zt_end = 0;
+        h->outL = keepL;
+        if (rc == OCTO_FMM_OK && (cudaEventRecord(h->ev_end, h->s_d2h) != cudaSuccess || cudaStreamWaitEvent(h->stream, h->ev_end, 0) != cudaSuccess))
+            rc = OCTO_FMM_ECUDA;
+        if (rc != OCTO_FMM_OK) { cudaStreamSynchronize(h->s_d2h); return rc; }
     } else {
         if (cudaMemcpyAsync(d_m, moments_host, ncell * (multi ? 20 : 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess)
             return OCTO_FMM_ECUDA;
@@ -1109,12 +1156,12 @@ int octo_fmm_run_host(octo_fmm_t* h, const double* moments_host, const double* c
         if (Lcorr_host && cudaMemcpyAsync(Lcorr_host, d_C, ocell * 3 * 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess)
             return OCTO_FMM_ECUDA;
     }
+    // the device flag word rides home behind the results, into pinned memory: one synchronisation, no pageable copy
+    if (cudaMemcpyAsync(h->pinned_flag, h->flags, sizeof(int), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     h->state = 1;                       // the results went to the host; nothing is kept in the scratch
     h->resL = h->L; h->resC = h->C;
-    int f = 0;
-    if (cudaMemcpy(&f, h->flags, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
-    return (f & 1) ? OCTO_FMM_EMASS : OCTO_FMM_OK;
+    return (h->pinned_flag[0] & 1) ? OCTO_FMM_EMASS : OCTO_FMM_OK;
 }
 
 int octo_fmm_set_option(octo_fmm_t* h, const char* key, int value)

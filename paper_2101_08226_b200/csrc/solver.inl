@@ -59,6 +59,8 @@ struct octo_fmm_solver {
     cudaStream_t stream;
     unsigned long long n_interactions;
     bool have_centres;    // solve() has run: lev[].off hold the expansion centres of the density
+    cudaStream_t s_d2h;   // solve_host(): side stream of the copies out (created on first use)
+    cudaEvent_t ev_chunk[16], ev_done;
     int f2_fused;         // solve2(): 0 = fused kernel on the one-warp-per-cell levels only (default), 1 = also on the
                           // finer levels (m2l_direct2_kernel instead of two launches of the slab-fed kernel)
 };
@@ -90,6 +92,10 @@ int octo_fmm_solver_destroy(octo_fmm_solver_t* s)
         if (l.fmm && octo_fmm_destroy(l.fmm) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
         if (l.fmm2 && octo_fmm_destroy(l.fmm2) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
     }
+    if (s->s_d2h) cudaStreamDestroy(s->s_d2h);
+    for (cudaEvent_t& e : s->ev_chunk)
+        if (e) cudaEventDestroy(e);
+    if (s->ev_done) cudaEventDestroy(s->ev_done);
     delete s;
     return rc;
 }
@@ -109,6 +115,8 @@ int octo_fmm_solver_create(const octo_fmm_solver_config* cfg, octo_fmm_solver_t*
     s->n_interactions = 0;
     s->have_centres = false;
     s->f2_fused = 0;
+    s->s_d2h = nullptr; s->ev_done = nullptr;
+    for (cudaEvent_t& e : s->ev_chunk) e = nullptr;
     char* w = (char*)cfg->workspace;
     {
         octo_fmm_config lc = level_config(*cfg, cfg->n, cfg->h, OCTO_FMM_MONOPOLE);
@@ -146,7 +154,10 @@ int octo_fmm_solver_create(const octo_fmm_solver_config* cfg, octo_fmm_solver_t*
     return OCTO_FMM_OK;
 }
 
-int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
+// out_host != nullptr (octo_fmm_solver_solve_host): the leaf kernel is launched in chunks of z-tiles and every chunk of
+// `out` is copied to out_host on a side stream as soon as it is complete, so that the 32 bytes per leaf that go back over
+// the bus overlap the rest of the leaf level instead of following it.
+static int solver_solve_impl(octo_fmm_solver_t* s, const double* mass, double* out, double* out_host)
 {
     if (!s || !mass || !out) return OCTO_FMM_EINVAL;
     if (((uintptr_t)mass % 16) || ((uintptr_t)out % 16)) return OCTO_FMM_EINVAL;     // double2 accesses
@@ -189,7 +200,34 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
     const bool fused_eval = s->leaf->mono_kernel == 0;
     s->leaf->outL = out;
     if (fused_eval) set_parent(s->leaf, s->lev[0]);
-    rc = octo_fmm_interact(s->leaf);
+    if (fused_eval && out_host) {
+        constexpr int NCHUNK = 8;
+        const int n = s->cfg.n, ztiles = (n + DT_Z - 1) / DT_Z;
+        const size_t plane = (size_t)n * n, ncell = plane * n;
+        rc = OCTO_FMM_OK;
+        if (!s->s_d2h && cudaStreamCreateWithFlags(&s->s_d2h, cudaStreamNonBlocking) != cudaSuccess) rc = OCTO_FMM_ECUDA;
+        for (int c = 0; c < NCHUNK && rc == OCTO_FMM_OK; ++c)
+            if (!s->ev_chunk[c] && cudaEventCreateWithFlags(&s->ev_chunk[c], cudaEventDisableTiming) != cudaSuccess) rc = OCTO_FMM_ECUDA;
+        if (rc == OCTO_FMM_OK && !s->ev_done && cudaEventCreateWithFlags(&s->ev_done, cudaEventDisableTiming) != cudaSuccess) rc = OCTO_FMM_ECUDA;
+        for (int c = 0; c < NCHUNK && rc == OCTO_FMM_OK; ++c) {
+            const int a = (int)((long long)ztiles * c / NCHUNK), b = (int)((long long)ztiles * (c + 1) / NCHUNK);
+            if (a == b) continue;
+            s->leaf->mono_zt_begin = a; s->leaf->mono_zt_end = b;
+            rc = octo_fmm_interact(s->leaf);
+            if (rc != OCTO_FMM_OK) break;
+            const int z0 = a * DT_Z, z1 = std::min(b * DT_Z, n);
+            if (cudaEventRecord(s->ev_chunk[c], st) != cudaSuccess || cudaStreamWaitEvent(s->s_d2h, s->ev_chunk[c], 0) != cudaSuccess ||
+                cudaMemcpy2DAsync(out_host + (size_t)z0 * plane, ncell * 8, out + (size_t)z0 * plane, ncell * 8,
+                                  (size_t)(z1 - z0) * plane * 8, 4, cudaMemcpyDeviceToHost, s->s_d2h) != cudaSuccess)
+                rc = OCTO_FMM_ECUDA;
+        }
+        s->leaf->mono_zt_begin = 0; s->leaf->mono_zt_end = 0;
+        if (rc == OCTO_FMM_OK && (cudaEventRecord(s->ev_done, s->s_d2h) != cudaSuccess || cudaStreamWaitEvent(st, s->ev_done, 0) != cudaSuccess))
+            rc = OCTO_FMM_ECUDA;
+        if (rc != OCTO_FMM_OK && s->s_d2h) cudaStreamSynchronize(s->s_d2h);     // nothing of this call stays in flight
+    } else {
+        rc = octo_fmm_interact(s->leaf);
+    }
     if (fused_eval) clear_parent(s->leaf);
     s->leaf->outL = keep;
     if (rc != OCTO_FMM_OK) return rc;
@@ -201,6 +239,11 @@ int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
     }
     s->have_centres = true;
     return OCTO_FMM_OK;
+}
+
+int octo_fmm_solver_solve(octo_fmm_solver_t* s, const double* mass, double* out)
+{
+    return solver_solve_impl(s, mass, out, nullptr);
 }
 
 // Second right-hand side (L81-83): the same passes with the sources d(mass)/dt, about the centres the last solve()
@@ -372,9 +415,10 @@ int octo_fmm_solver_solve_host(octo_fmm_solver_t* s, const double* mass_host, do
     double* d_m = (double*)scratch;
     double* d_o = (double*)((char*)scratch + align_up(nc * 8));
     if (cudaMemcpyAsync(d_m, mass_host, nc * 8, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
-    const int rc = octo_fmm_solver_solve(s, d_m, d_o);
+    const bool piped = s->leaf->mono_kernel == 0;      // the tensor-core leaf kernel: copies out overlap the leaf level
+    const int rc = solver_solve_impl(s, d_m, d_o, piped ? out_host : nullptr);
     if (rc != OCTO_FMM_OK) return rc;
-    if (cudaMemcpyAsync(out_host, d_o, nc * 4 * 8, cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (!piped && cudaMemcpyAsync(out_host, d_o, nc * 4 * 8, cudaMemcpyDeviceToHost, s->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     if (cudaStreamSynchronize(s->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     return OCTO_FMM_OK;
 }

@@ -818,3 +818,27 @@ def test_binding_refuses_tensors_the_c_abi_would_misread(env):
     with pytest.raises(ValueError):
         s.solve(torch.ones((16, 16, 8), dtype=torch.float64, device="cuda"))
     s.close()
+
+
+@pytest.mark.parametrize("n,chunk", [((40, 24, 16), 12), ((32, 32, 72), 12), ((32, 32, 72), 0)])
+def test_monopole_host_entry_point_in_chunks_of_z_tiles(env, n, chunk):
+    """octo_fmm_run_host, monopole kind: the tensor-core kernel is launched in chunks of z-tiles with the copies out on a
+    side stream (host_chunk > 0) or in one piece (0); either way bit-identical to the device-pointer route, twice in a row
+    (the side stream and its events are reused), on grids whose z-extent is and is not a multiple of the 8-layer tiles."""
+    p, torch = env
+    w = fi.config4(ncell=max(n))
+    mass = np.ascontiguousarray(w.moments[0][:n[2], :n[1], :n[0]])
+    f = p.OctoFMM(n, w.h, 0.5, p.MONOPOLE)
+    ref, _ = f.solve(torch.from_numpy(mass).cuda())
+    torch.cuda.synchronize()
+    f.set_option("host_chunk", chunk)
+    nb = p.octo_fmm_host_scratch_bytes(f.cfg)
+    scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    m_h = torch.from_numpy(mass).pin_memory()
+    o_h = torch.full((4,) + f.out_shape, float("nan"), dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        p.octo_fmm_run_host(f.handle, m_h, None, o_h, None, scratch, nb)
+        assert f.status() == p.OK
+        assert np.array_equal(o_h.numpy(), ref.cpu().numpy())
+        o_h.fill_(float("nan"))
+    f.close()
