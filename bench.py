@@ -396,7 +396,7 @@ def run_tree(args):
         Fa += mg.abs().sum()
     net_force = float(F.abs().max() / Fa)
     # end to end through the host-buffer entry point (pinned host arrays, every level)
-    nb = p.octo_fmm_tree_host_scratch_bytes(t.cfg)
+    nb = p.octo_fmm_tree_host_scratch_bytes(t.handle)
     scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
     m_h = [torch.from_numpy(m).pin_memory() for m in tree.mass]
     o_h = [torch.empty((4,) + (tree.n(l),) * 3, dtype=torch.float64).pin_memory() for l in range(depth)]

@@ -359,6 +359,35 @@ class Tree:
         return np.concatenate(pos), np.concatenate(ms), np.concatenate(lv), np.concatenate(idx)
 
 
+def tree_boxes(tree, margin: int = 0):
+    """Per level the bounding box (lo_x, lo_y, lo_z, n_x, n_y, n_z), aligned to the 8^3 sub-grids and grown by `margin`
+    sub-grids, of the cells that exist on that level of a tree given on whole lattices; level 0: the whole lattice."""
+    out = []
+    for l in range(tree.depth):
+        n = tree.n(l)
+        if l == 0 or not (tree.kind[l] != TREE_ABSENT).any():
+            out.append((0, 0, 0, n, n, n) if l == 0 else (0, 0, 0, 8, 8, 8))
+            continue
+        k, j, i = np.nonzero(tree.kind[l] != TREE_ABSENT)
+        b = []
+        for v in (i, j, k):
+            lo = max((int(v.min()) // 8 - margin) * 8, 0)
+            hi = min((int(v.max()) // 8 + 1 + margin) * 8, n)
+            b.append((lo, hi - lo))
+        out.append((b[0][0], b[1][0], b[2][0], b[0][1], b[1][1], b[2][1]))
+    return out
+
+
+def crop_tree(tree, boxes):
+    """(kind, mass) lists of the tree's levels restricted to the boxes (contiguous copies)."""
+    kind, mass = [], []
+    for l, b in enumerate(boxes):
+        sl = (slice(b[2], b[2] + b[5]), slice(b[1], b[1] + b[4]), slice(b[0], b[0] + b[3]))
+        kind.append(np.ascontiguousarray(tree.kind[l][sl]))
+        mass.append(np.ascontiguousarray(tree.mass[l][sl]))
+    return kind, mass
+
+
 def _expand8(a):
     return np.repeat(np.repeat(np.repeat(a, 8, 0), 8, 1), 8, 2)
 
@@ -460,3 +489,65 @@ def star_tree(n0: int = 16, depth: int = 3, stars=None, radius_factor: float = 1
             w |= rr < radius_factor * s.radius / (1.5 ** l)
         return w
     return make_tree(n0, depth, want, lambda X, Y, Z: field_density(stars, X, Y, Z))
+
+
+def nested_tree(n0: int = 16, depth: int = 9, centre=(0.37, 0.52, 0.61), reach: float = 1.6, star_radius: float = 0.05,
+                box: float = 1.0):
+    """A DEEP tree built directly in boxes (the paper's production runs use 9 levels, L684; a 2048^3 lattice cannot be
+    held whole): on every level the sub-grids whose centre lies within `reach` sub-grid widths of `centre` are refined, so
+    that each level is a window of a few sub-grids around the same point; proper nesting over the 26 neighbours is
+    enforced bottom-up on the sparse sets of sub-grids.  Density: one n = 1.5 polytrope of radius `star_radius` at
+    `centre` over the 1e-10 floor.  Returns (boxes, kind, mass) with kind[l], mass[l] of shape [n_z][n_y][n_x] of box l."""
+    assert n0 % 8 == 0 and depth >= 1
+    refined = []                                   # per level: set of refined sub-grids (lattice coordinates)
+    for l in range(depth - 1):
+        s = (n0 // 8) << l                         # sub-grids per axis
+        w = box / s
+        c = [centre[a] / w for a in range(3)]      # centre in sub-grid units
+        r = set()
+        lo = [max(int(c[a] - reach - 1), 0) for a in range(3)]
+        hi = [min(int(c[a] + reach + 2), s) for a in range(3)]
+        for K in range(lo[2], hi[2]):
+            for J in range(lo[1], hi[1]):
+                for I in range(lo[0], hi[0]):
+                    if (I + 0.5 - c[0]) ** 2 + (J + 0.5 - c[1]) ** 2 + (K + 0.5 - c[2]) ** 2 < reach * reach:
+                        r.add((I, J, K))
+        refined.append(r)
+    refined.append(set())
+    if depth > 1:
+        refined[0] = {(I, J, K) for K in range(n0 // 8) for J in range(n0 // 8) for I in range(n0 // 8)} if n0 <= 16 else refined[0]
+    # bottom-up: every 26-neighbour of a refined sub-grid must exist, i.e. its parent must be refined
+    for l in range(depth - 2, 0, -1):
+        s = (n0 // 8) << l
+        for (I, J, K) in list(refined[l]):
+            for dz in (-1, 0, 1):
+                for dy in (-1, 0, 1):
+                    for dx in (-1, 0, 1):
+                        q = (I + dx, J + dy, K + dz)
+                        if 0 <= q[0] < s and 0 <= q[1] < s and 0 <= q[2] < s:
+                            refined[l - 1].add((q[0] // 2, q[1] // 2, q[2] // 2))
+    # top-down: a sub-grid exists iff its parent is refined; refined sub-grids must exist
+    exists = [{(I, J, K) for K in range(n0 // 8) for J in range(n0 // 8) for I in range(n0 // 8)}]
+    for l in range(depth - 1):
+        refined[l] &= exists[l]
+        exists.append({(2 * I + a, 2 * J + b, 2 * K + c) for (I, J, K) in refined[l] for a in (0, 1) for b in (0, 1) for c in (0, 1)})
+    star = [Star(tuple(centre), star_radius, 1.0)]
+    boxes, kind, mass = [], [], []
+    for l in range(depth):
+        n = n0 << l
+        h = box / n
+        if not exists[l]:
+            boxes.append((0, 0, 0, 8, 8, 8)); kind.append(np.zeros((8, 8, 8), np.uint8)); mass.append(np.zeros((8, 8, 8)))
+            continue
+        lo = [min(q[a] for q in exists[l]) for a in range(3)]
+        hi = [max(q[a] for q in exists[l]) + 1 for a in range(3)]
+        b = (8 * lo[0], 8 * lo[1], 8 * lo[2], 8 * (hi[0] - lo[0]), 8 * (hi[1] - lo[1]), 8 * (hi[2] - lo[2]))
+        sub = np.zeros((hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0]), np.uint8)
+        for (I, J, K) in exists[l]:
+            sub[K - lo[2], J - lo[1], I - lo[0]] = TREE_REFINED if (I, J, K) in refined[l] else TREE_LEAF
+        k = _expand8(sub)
+        x = [(np.arange(b[3 + a]) + b[a] + 0.5) * h for a in range(3)]
+        Z, Y, X = np.meshgrid(x[2], x[1], x[0], indexing="ij")
+        m = np.where(k == TREE_LEAF, field_density(star, X, Y, Z) * h ** 3, 0.0)
+        boxes.append(b); kind.append(np.ascontiguousarray(k)); mass.append(np.ascontiguousarray(m))
+    return boxes, kind, mass

@@ -281,31 +281,39 @@ int octo_fmm_solver_num_levels(const octo_fmm_solver_t *s, int *multipole_levels
  * Every pair is taken once in each direction with antisymmetric forces: linear momentum, and with the correction
  * angular momentum, are conserved as on a uniform grid (L125, L127); a fully refined tree IS the uniform solve.
  *
- * Layout: tree level l = 0 .. depth-1 is a dense lattice [n_l][n_l][n_l], n_l = n0 2^l, h_l = h0 / 2^l, x fastest.
+ * Layout: tree level l = 0 .. depth-1 lives on the lattice of n_l = n0 2^l cells per axis, h_l = h0 / 2^l.  Its arrays
+ * cover a BOX of that lattice, box[6 l ..] = (lo_x, lo_y, lo_z, n_x, n_y, n_z) in cells of level l, all multiples of 8,
+ * n >= 8, inside the lattice; box = NULL: every level is its whole lattice.  Level 0 must be the whole lattice.  Cells
+ * outside a level's box do not exist on that level, so a deep tree costs memory and passes in proportion to the boxes,
+ * not to the lattices (the paper's 9 levels, L684: a 2048^3 lattice with a box of a few hundred cells around a star).
+ * Arrays are [n_z][n_y][n_x] of the box, x fastest.
  * kind[l] (uint8, HOST memory, read at create() only): 0 the cell does not exist on this level, 1 leaf, 2 refined;
  * constant over every aligned 8^3 sub-grid; every cell of level 0 exists; a cell exists on level l+1 iff its parent
- * is refined; no refined cell on the last level (else EINVAL).  Proper nesting over the 26 neighbours of a sub-grid
- * is the caller's duty (a leaf next to a sub-grid two levels finer is not detected).  Above level 0 the uniform
- * levels n0/2 .. 2 are built by the library.
- * mass[l]: DEVICE [n_l^3], read at the leaf cells only; out[l]: DEVICE [4][n_l^3] = (phi, g_x, g_y, g_z) at the
- * leaf cells, zeros elsewhere.  mass and out are HOST arrays of `depth` device pointers, all 16-byte aligned.
+ * is refined (so the 8 child sub-grids of a refined sub-grid lie inside the next box); no refined cell on the last
+ * level (else EINVAL).  Proper nesting over the 26 neighbours of a sub-grid is the caller's duty (a leaf next to a
+ * sub-grid two levels finer is not detected).  Above level 0 the uniform levels n0/2 .. 2 are built by the library.
+ * mass[l]: DEVICE [box cells], read at the leaf cells only; out[l]: DEVICE [4][box cells] = (phi, g_x, g_y, g_z) at
+ * the leaf cells, zeros elsewhere.  mass and out are HOST arrays of `depth` device pointers, all 16-byte aligned.
  * The caller lends the workspace; everything is enqueued on cfg.stream; create() synchronises the stream once (it
  * uploads the topology from pageable memory).  One handle is not thread-safe. */
 typedef struct octo_fmm_tree octo_fmm_tree_t;
 typedef struct {
-    int n0;                 /* cells per axis of level 0: a power of two, 8 <= n0, n0 2^(depth-1) <= 2048      */
-    int depth;              /* number of tree levels, 1..10                                                    */
+    int n0;                 /* cells per axis of level 0: a power of two, 8 <= n0 <= 2048                      */
+    int depth;              /* number of tree levels, 1..12 (lattice of the last level <= 2^20 cells per axis;  */
+                            /* every box <= 4096 cells per axis)                                               */
     double h0;              /* cell width of level 0                                                           */
     double theta;           /* opening angle, 1/3 < theta < 1                                                  */
     int am_correction;      /* 0/1 (L127)                                                                      */
     int device;
     void *stream;           /* cudaStream_t, borrowed                                                          */
     void *workspace;        /* device memory, 256-byte aligned, borrowed for the handle's lifetime             */
-    size_t workspace_bytes; /* >= octo_fmm_tree_workspace_bytes(cfg, kind_host)                                */
+    size_t workspace_bytes; /* >= octo_fmm_tree_workspace_bytes(cfg, kind_host, box)                           */
 } octo_fmm_tree_config;
 
-size_t octo_fmm_tree_workspace_bytes(const octo_fmm_tree_config *cfg, const unsigned char *const *kind_host); /* 0 if invalid */
-int octo_fmm_tree_create(const octo_fmm_tree_config *cfg, const unsigned char *const *kind_host, octo_fmm_tree_t **out);
+size_t octo_fmm_tree_workspace_bytes(const octo_fmm_tree_config *cfg, const unsigned char *const *kind_host,
+                                     const int *box);                                              /* 0 if invalid */
+int octo_fmm_tree_create(const octo_fmm_tree_config *cfg, const unsigned char *const *kind_host, const int *box,
+                         octo_fmm_tree_t **out);
 /* Asynchronous on the stream. */
 int octo_fmm_tree_solve(octo_fmm_tree_t *t, const double *const *mass, double *const *out);
 /* The same solve, and the ordered pairs it evaluates, counted on the device for the bit-exact check of the pair set:
@@ -315,8 +323,8 @@ int octo_fmm_tree_interaction_counts(octo_fmm_tree_t *t, const double *const *ma
                                      unsigned long long counts[3]);
 /* The same with HOST buffers (mass_host[l], out_host[l]: host arrays of the layouts above; pinned memory makes the
  * copies asynchronous): H2D of the masses of every level that has leaves, solve, D2H of every out[l], stream
- * synchronise.  scratch: device, >= octo_fmm_tree_host_scratch_bytes(cfg), 256-byte aligned, borrowed for the call. */
-size_t octo_fmm_tree_host_scratch_bytes(const octo_fmm_tree_config *cfg);
+ * synchronise.  scratch: device, >= octo_fmm_tree_host_scratch_bytes(t), 256-byte aligned, borrowed for the call. */
+size_t octo_fmm_tree_host_scratch_bytes(const octo_fmm_tree_t *t);
 int octo_fmm_tree_solve_host(octo_fmm_tree_t *t, const double *const *mass_host, double *const *out_host, void *scratch,
                              size_t scratch_bytes);
 /* Synchronises the stream; OCTO_FMM_EMASS if the correction met an existing cell of mass <= 0. */

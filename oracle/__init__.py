@@ -364,17 +364,22 @@ def _ub(a):
     return a.ctypes.data_as(ctypes.POINTER(ctypes.c_ubyte))
 
 
+def _n3(n):
+    """(nx, ny, nz) from an int (cubic) or a 3-tuple."""
+    return (int(n),) * 3 if np.isscalar(n) else tuple(int(v) for v in n)
+
+
 def tree_interact_multipole(n, h, theta, moments, com_off, kind, am_correction=True):
     """Same-level multipole step on one level of a tree (kind: 0 absent, 1 leaf, 2 refined): every existing cell takes
     the existing cells of its Eq. 15 list, except that two leaves do not meet here.  Returns (L, Lcorr, count)."""
-    n = int(n)
+    nx, ny, nz = _n3(n)
     moments = np.ascontiguousarray(moments, dtype=np.float64)
     com_off = np.ascontiguousarray(com_off, dtype=np.float64)
     kind = np.ascontiguousarray(kind, dtype=np.uint8)
-    assert moments.shape == (20, n, n, n) and com_off.shape == (3, n, n, n) and kind.shape == (n, n, n)
-    Lout, Lc = np.zeros((20, n, n, n)), np.zeros((3, n, n, n))
+    assert moments.shape == (20, nz, ny, nx) and com_off.shape == (3, nz, ny, nx) and kind.shape == (nz, ny, nx)
+    Lout, Lc = np.zeros((20, nz, ny, nx)), np.zeros((3, nz, ny, nx))
     cnt = ctypes.c_ulonglong(0)
-    _check(lib().fmm_oracle_tree_interact_multipole(_i3((n, n, n)), float(h), float(theta), int(bool(am_correction)),
+    _check(lib().fmm_oracle_tree_interact_multipole(_i3((nx, ny, nz)), float(h), float(theta), int(bool(am_correction)),
                                                     _dp(moments), _dp(com_off), _ub(kind), _dp(Lout), _dp(Lc),
                                                     ctypes.byref(cnt)), "tree_interact_multipole")
     return Lout, Lc, cnt.value
@@ -382,13 +387,13 @@ def tree_interact_multipole(n, h, theta, moments, com_off, kind, am_correction=T
 
 def tree_leaf_p2p(n, h, theta, kind, mass):
     """Point-mass sum of the leaf cells of one level over the leaf-level list.  Returns (out[4][n][n][n], count)."""
-    n = int(n)
+    nx, ny, nz = _n3(n)
     kind = np.ascontiguousarray(kind, dtype=np.uint8)
     mass = np.ascontiguousarray(mass, dtype=np.float64)
-    assert kind.shape == (n, n, n) and mass.shape == (n, n, n)
-    out = np.zeros((4, n, n, n))
+    assert kind.shape == (nz, ny, nx) and mass.shape == (nz, ny, nx)
+    out = np.zeros((4, nz, ny, nx))
     cnt = ctypes.c_ulonglong(0)
-    _check(lib().fmm_oracle_tree_leaf_p2p(_i3((n, n, n)), float(h), float(theta), _ub(kind), _dp(mass), _dp(out),
+    _check(lib().fmm_oracle_tree_leaf_p2p(_i3((nx, ny, nz)), float(h), float(theta), _ub(kind), _dp(mass), _dp(out),
                                           ctypes.byref(cnt)), "tree_leaf_p2p")
     return out, cnt.value
 
@@ -396,14 +401,15 @@ def tree_leaf_p2p(n, h, theta, kind, mass):
 def tree_cross_level(nc, hc, theta, kind_c, mass_c, kind_f, mass_f, out_c, out_f):
     """Point-mass pairs across a refinement boundary: a coarse leaf and the 8 children of every refined cell of its
     near field, both directions; ADDED to out_c [4][nc]^3 and out_f [4][2 nc]^3.  Returns the number of ordered pairs."""
-    nc = int(nc)
+    cx, cy, cz = _n3(nc)
     for a in (kind_c, kind_f):
         assert a.dtype == np.uint8 and a.flags["C_CONTIGUOUS"]
     for a in (mass_c, mass_f, out_c, out_f):
         assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
-    assert kind_c.shape == (nc,) * 3 and kind_f.shape == (2 * nc,) * 3 and out_c.shape == (4,) + (nc,) * 3
+    assert kind_c.shape == (cz, cy, cx) and kind_f.shape == (2 * cz, 2 * cy, 2 * cx) and out_c.shape == (4, cz, cy, cx)
+    assert out_f.shape == (4, 2 * cz, 2 * cy, 2 * cx) and mass_f.shape == kind_f.shape and mass_c.shape == kind_c.shape
     cnt = ctypes.c_ulonglong(0)
-    _check(lib().fmm_oracle_tree_cross_level(_i3((nc, nc, nc)), float(hc), float(theta), _ub(kind_c), _dp(mass_c), _ub(kind_f),
+    _check(lib().fmm_oracle_tree_cross_level(_i3((cx, cy, cz)), float(hc), float(theta), _ub(kind_c), _dp(mass_c), _ub(kind_f),
                                              _dp(mass_f), _dp(out_c), _dp(out_f), ctypes.byref(cnt)), "tree_cross_level")
     return cnt.value
 
@@ -417,34 +423,66 @@ def direct_sum_points(pos, mass):
     return out
 
 
-def solve_tree(n0, h0, theta, kind, mass, am_correction=True, coarsest=2):
+def _embed(arr, box, frame):
+    """arr [..., nz, ny, nx] living on box = (lo_x, lo_y, lo_z, n_x, n_y, n_z) of a lattice, placed into zeros of the
+    frame (same convention); the parts of the box outside the frame are dropped."""
+    out = np.zeros(arr.shape[:-3] + (frame[5], frame[4], frame[3]), dtype=arr.dtype)
+    src, dst = [], []
+    for a in (2, 1, 0):                     # z, y, x
+        lo = max(box[a], frame[a]); hi = min(box[a] + box[3 + a], frame[a] + frame[3 + a])
+        if hi <= lo:
+            return out
+        src.append(slice(lo - box[a], hi - box[a])); dst.append(slice(lo - frame[a], hi - frame[a]))
+    out[(Ellipsis,) + tuple(dst)] = arr[(Ellipsis,) + tuple(src)]
+    return out
+
+
+def _extract(arr, frame, box):
+    """Inverse of _embed for a box that lies inside the frame."""
+    sl = tuple(slice(box[a] - frame[a], box[a] - frame[a] + box[3 + a]) for a in (2, 1, 0))
+    return np.ascontiguousarray(arr[(Ellipsis,) + sl])
+
+
+def solve_tree(n0, h0, theta, kind, mass, am_correction=True, coarsest=2, box=None):
     """The gravity solve on an adaptive oct-tree of 8^3 sub-grids ("The FMM adapts naturally to an
-    oct-tree based adaptive mesh refinement"; L287-291; reading R9).  Level l = 0 .. len(kind)-1 is a dense
-    [n_l]^3 lattice, n_l = n0 2^l, h_l = h0 / 2^l, with kind[l] (0 absent, 1 leaf, 2 refined) and mass[l] (leaf masses);
-    above level 0 the uniform levels n0/2 .. `coarsest` as in solve().  Steps, in the paper's order (L125):
+    oct-tree based adaptive mesh refinement"; L287-291; reading R9).  Level l = 0 .. len(kind)-1 lives on the
+    lattice of n_l = n0 2^l cells per axis, h_l = h0 / 2^l, with kind[l] (0 absent, 1 leaf, 2 refined) and mass[l] (leaf
+    masses); above level 0 the uniform levels n0/2 .. `coarsest` as in solve().  box = None: every array is its whole
+    lattice [n_l]^3; else box[l] = (lo_x, lo_y, lo_z, n_x, n_y, n_z): the arrays of level l cover that box only and cells
+    outside it do not exist (level 0: the whole lattice).  Steps, in the paper's order (L125):
       upward    leaf = point mass at its geometric centre; refined cell = M2M of its 8 children (leaf or refined);
       downward  every existing cell: same-level step over its Eq. 15 list (two leaves excepted) + its parent's
                 expansion (L2L), the correction carried beside it;
       leaves    phi = L0 + point-mass sums, g = -(L1 + correction) + point-mass sums, the sums being (a) the leaves of
                 its own level on the leaf-level list, (b) the children of the refined cells of its near field, (c) the
                 coarser leaves in the near field of its parent.
-    Returns (out, counts): out[l] = [4][n_l]^3 = (phi, g) at the leaf cells of level l (0 elsewhere);
+    The parent <-> child steps (M2M, L2L, cross-level pairs) are the dense ones applied to the child arrays embedded in
+    the frame of the children of the parent's box (zeros outside the child's box: absent cells).
+    Returns (out, counts): out[l] = [4] + shape of level l = (phi, g) at the leaf cells of level l (0 elsewhere);
     counts = {"m2l": .., "p2p": .., "cross": .., and per tree level "m2l_levels", "p2p_levels", "cross_levels"} ordered pairs
     ("m2l" includes the uniform levels above level 0)."""
     D = len(kind)
     n0 = int(n0)
+    if box is None:
+        box = [(0, 0, 0) + (n0 << l,) * 3 for l in range(D)]
+    box = [tuple(int(v) for v in b) for b in box]
+    assert box[0] == (0, 0, 0, n0, n0, n0)
+    shp = [(b[5], b[4], b[3]) for b in box]
     kind = [np.ascontiguousarray(k, dtype=np.uint8) for k in kind]
+    for l in range(D):
+        assert kind[l].shape == shp[l] and np.shape(mass[l]) == shp[l]
     mass = [np.ascontiguousarray(np.where(k == 1, m, 0.0), dtype=np.float64) for k, m in zip(kind, mass)]
-    ns = [n0 << l for l in range(D)]
     hs = [float(h0) / (1 << l) for l in range(D)]
+    # the frame of the children of level l's box, on the lattice of level l + 1
+    cframe = [tuple(2 * v for v in b) for b in box]
     # ---- upward pass over the tree levels ----
     mom, off = [None] * D, [None] * D
     for l in range(D - 1, -1, -1):
-        n = ns[l]
-        m = np.zeros((20, n, n, n)); m[0] = mass[l]
-        o = np.zeros((3, n, n, n))
+        m = np.zeros((20,) + shp[l]); m[0] = mass[l]
+        o = np.zeros((3,) + shp[l])
         if l < D - 1:
-            pm, po = m2m((2 * n,) * 3, hs[l + 1], mom[l + 1], off[l + 1])
+            f = cframe[l]
+            pm, po = m2m((f[3], f[4], f[5]), hs[l + 1], _embed(mom[l + 1], box[l + 1], f), _embed(off[l + 1], box[l + 1], f))
             ref = kind[l] == 2
             m = np.where(ref[None], pm, m)
             o = np.where(ref[None], po, o)
@@ -467,28 +505,38 @@ def solve_tree(n0, h0, theta, kind, mass, am_correction=True, coarsest=2):
             l2l((nl, nl, nl), hl, L_par, corr_par, off_par, up_o[lv], L, corr)
         L_par, corr_par, off_par = L, corr, up_o[lv]
     # ---- downward pass over the tree levels, leaves evaluated on the way ----
-    out = [None] * D
+    out, exp = [None] * D, [None] * D
     for l in range(D):
-        n, h = ns[l], hs[l]
-        Lf, Lc, c = tree_interact_multipole(n, h, theta, mom[l], off[l], kind[l], am_correction)
+        n3, h = (box[l][3], box[l][4], box[l][5]), hs[l]
+        Lf, Lc, c = tree_interact_multipole(n3, h, theta, mom[l], off[l], kind[l], am_correction)
         counts["m2l"] += c
         counts["m2l_levels"].append(c)
         L = Lf.copy(); L[1:4] -= Lc
         corr = Lc.copy()
         if L_par is not None:
-            l2l((n, n, n), h, L_par, corr_par, off_par, off[l], L, corr)
-        o, c = tree_leaf_p2p(n, h, theta, kind[l], mass[l])
+            if l == 0:
+                l2l(n3, h, L_par, corr_par, off_par, off[l], L, corr)
+            else:
+                f = cframe[l - 1]                  # the parent's arrays cover box[l-1]; this level embedded in its children's frame
+                Le, ce = _embed(L, box[l], f), _embed(corr, box[l], f)
+                l2l((f[3], f[4], f[5]), h, L_par, corr_par, off_par, _embed(off[l], box[l], f), Le, ce)
+                L, corr = _extract(Le, f, box[l]), _extract(ce, f, box[l])
+        o, c = tree_leaf_p2p(n3, h, theta, kind[l], mass[l])
         counts["p2p"] += c
         counts["p2p_levels"].append(c)
         out[l] = o
         L_par, corr_par, off_par = L, corr, off[l]
-        mom[l] = (L, corr)                         # kept for the leaf evaluation below
+        exp[l] = (L, corr)
     for l in range(D - 1):
-        c = tree_cross_level(ns[l], hs[l], theta, kind[l], mass[l], kind[l + 1], mass[l + 1], out[l], out[l + 1])
+        f = cframe[l]
+        of = _embed(out[l + 1], box[l + 1], f)
+        c = tree_cross_level((box[l][3], box[l][4], box[l][5]), hs[l], theta, kind[l], mass[l], _embed(kind[l + 1], box[l + 1], f),
+                             _embed(mass[l + 1], box[l + 1], f), out[l], of)
+        out[l + 1] = _extract(of, f, box[l + 1])
         counts["cross"] += c
         counts["cross_levels"].append(c)
     for l in range(D):
-        L, corr = mom[l]
+        L, corr = exp[l]
         leaf = kind[l] == 1
         out[l][0] += np.where(leaf, L[0], 0.0)
         out[l][1:4] -= np.where(leaf[None], L[1:4] + corr, 0.0)

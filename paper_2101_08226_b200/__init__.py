@@ -89,12 +89,12 @@ class _Library:
         tcfgp = ctypes.POINTER(octo_fmm_tree_config)
         vpp = ctypes.POINTER(ctypes.c_void_p)
         lib.octo_fmm_tree_workspace_bytes.restype = ctypes.c_size_t
-        lib.octo_fmm_tree_workspace_bytes.argtypes = [tcfgp, vpp]
-        lib.octo_fmm_tree_create.argtypes = [tcfgp, vpp, ctypes.POINTER(vp)]
+        lib.octo_fmm_tree_workspace_bytes.argtypes = [tcfgp, vpp, ip]
+        lib.octo_fmm_tree_create.argtypes = [tcfgp, vpp, ip, ctypes.POINTER(vp)]
         lib.octo_fmm_tree_solve.argtypes = [vp, vpp, vpp]
         lib.octo_fmm_tree_interaction_counts.argtypes = [vp, vpp, vpp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_tree_host_scratch_bytes.restype = ctypes.c_size_t
-        lib.octo_fmm_tree_host_scratch_bytes.argtypes = [tcfgp]
+        lib.octo_fmm_tree_host_scratch_bytes.argtypes = [vp]
         lib.octo_fmm_tree_solve_host.argtypes = [vp, vpp, vpp, vp, ctypes.c_size_t]
         lib.octo_fmm_tree_status.argtypes = [vp]
         lib.octo_fmm_tree_launches.argtypes = [vp, ip]
@@ -542,13 +542,23 @@ def _ptr_array(items):
     return arr
 
 
-def octo_fmm_tree_workspace_bytes(cfg, kind_host):
-    return int(_lib.octo_fmm_tree_workspace_bytes(ctypes.byref(cfg), _ptr_array(kind_host)))
+def _box_array(box, depth):
+    """depth x 6 C ints (lo_x, lo_y, lo_z, n_x, n_y, n_z) or None (every level is its whole lattice)."""
+    if box is None:
+        return None
+    flat = [int(v) for b in box for v in b]
+    if len(flat) != 6 * depth:
+        raise ValueError("octo_fmm: box needs 6 integers per level")
+    return (ctypes.c_int * len(flat))(*flat)
 
 
-def octo_fmm_tree_create(cfg, kind_host):
+def octo_fmm_tree_workspace_bytes(cfg, kind_host, box=None):
+    return int(_lib.octo_fmm_tree_workspace_bytes(ctypes.byref(cfg), _ptr_array(kind_host), _box_array(box, cfg.depth)))
+
+
+def octo_fmm_tree_create(cfg, kind_host, box=None):
     h = _vp()
-    rc = _lib.octo_fmm_tree_create(ctypes.byref(cfg), _ptr_array(kind_host), ctypes.byref(h))
+    rc = _lib.octo_fmm_tree_create(ctypes.byref(cfg), _ptr_array(kind_host), _box_array(box, cfg.depth), ctypes.byref(h))
     if rc != OK:
         raise OctoFmmError("octo_fmm_tree_create", rc)
     return h
@@ -568,8 +578,8 @@ def octo_fmm_tree_interaction_counts(t, mass, out):
     return {"m2l": int(c[0]), "p2p": int(c[1]), "cross": int(c[2])}
 
 
-def octo_fmm_tree_host_scratch_bytes(cfg):
-    return int(_lib.octo_fmm_tree_host_scratch_bytes(ctypes.byref(cfg)))
+def octo_fmm_tree_host_scratch_bytes(t):
+    return int(_lib.octo_fmm_tree_host_scratch_bytes(t))
 
 
 def octo_fmm_tree_solve_host(t, mass_host, out_host, scratch, scratch_bytes):
@@ -598,9 +608,10 @@ def octo_fmm_tree_destroy(t):
 
 class OctoFMMTree:
     """Owns the workspace tensor and the handle of a solve on an adaptive tree.  kind: list of numpy uint8 arrays
-    [n_l]^3 (host; 0 absent, 1 leaf, 2 refined), one per level."""
+    (host; 0 absent, 1 leaf, 2 refined), one per level; box: None (kind[l] is the whole lattice [n_l]^3) or per level
+    (lo_x, lo_y, lo_z, n_x, n_y, n_z) in cells, kind[l] then has shape [n_z][n_y][n_x]."""
 
-    def __init__(self, n0, h0, theta, kind, am_correction=True, device=0, stream=None):
+    def __init__(self, n0, h0, theta, kind, am_correction=True, device=0, stream=None, box=None):
         import numpy as np
         import torch
         if not torch.cuda.is_available():
@@ -610,30 +621,34 @@ class OctoFMMTree:
         self.device = torch.device("cuda", device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self.kind = [np.ascontiguousarray(k, dtype=np.uint8) for k in kind]
+        self.box = None if box is None else [tuple(int(v) for v in b) for b in box]
+        self.shape = [(self.n0 << l,) * 3 if self.box is None else (self.box[l][5], self.box[l][4], self.box[l][3])
+                      for l in range(self.depth)]
         for l, k in enumerate(self.kind):
-            if k.shape != (self.n0 << l,) * 3:
-                raise ValueError("octo_fmm: kind[%d] must have shape %s" % (l, ((self.n0 << l,) * 3,)))
+            if k.shape != self.shape[l]:
+                raise ValueError("octo_fmm: kind[%d] must have shape %s" % (l, (self.shape[l],)))
         cfg = make_tree_config(n0, self.depth, h0, theta, am_correction, device=device, stream=self.stream.cuda_stream)
-        nbytes = octo_fmm_tree_workspace_bytes(cfg, self.kind)
+        nbytes = octo_fmm_tree_workspace_bytes(cfg, self.kind, self.box)
         if nbytes == 0:
             raise OctoFmmError("octo_fmm_tree_workspace_bytes", EINVAL)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         cfg.workspace, cfg.workspace_bytes = self.workspace.data_ptr(), nbytes
         self.cfg = cfg
-        self.handle = octo_fmm_tree_create(cfg, self.kind)
+        self.handle = octo_fmm_tree_create(cfg, self.kind, self.box)
 
-    def n(self, l):
-        return self.n0 << l
+    def cells(self, l):
+        s = self.shape[l]
+        return s[0] * s[1] * s[2]
 
     def _check(self, mass, out):
         if len(mass) != self.depth or len(out) != self.depth:
             raise ValueError("octo_fmm: one mass and one out tensor per level")
         for l in range(self.depth):
-            _check_device_tensor(mass[l], "mass[%d]" % l, self.torch.float64, self.n(l) ** 3, self.device, self.stream)
-            _check_device_tensor(out[l], "out[%d]" % l, self.torch.float64, 4 * self.n(l) ** 3, self.device, self.stream)
+            _check_device_tensor(mass[l], "mass[%d]" % l, self.torch.float64, self.cells(l), self.device, self.stream)
+            _check_device_tensor(out[l], "out[%d]" % l, self.torch.float64, 4 * self.cells(l), self.device, self.stream)
 
     def empty_out(self):
-        return [self.torch.empty((4,) + (self.n(l),) * 3, dtype=self.torch.float64, device=self.device) for l in range(self.depth)]
+        return [self.torch.empty((4,) + self.shape[l], dtype=self.torch.float64, device=self.device) for l in range(self.depth)]
 
     def solve(self, mass, out=None):
         out = self.empty_out() if out is None else out

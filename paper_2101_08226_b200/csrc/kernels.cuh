@@ -87,6 +87,10 @@ struct Params {
                                  // nullptr = all ntiles bricks.  With a list, ntiles is its length.
     int tile_offset;             // tensor-core monopole kernels without a list: first tile of this launch (the host entry
                                  // points launch the level in chunks of z-tiles so that the copy out overlaps the rest)
+    // fused L2L epilogue: extents of the parent arrays and the shift between the two index lattices,
+    //   parent index = (child index >> 1) + psh   (uniform solve: pdim = n / 2, psh = 0; a level of the adaptive tree
+    //   stored as a BOX of its lattice: psh = box_lo(child) / 2 - box_lo(parent))
+    int pdim[3], psh[3];
 };
 
 // ------------------------------------------------------------------------------------------
@@ -272,9 +276,9 @@ __device__ __forceinline__ void store_target(const Params& p, const Acc& acc, co
     const long long ocell = (long long)p.ox * p.oy * p.oz;
     const long long o = ((long long)(k - p.lo[2]) * p.oy + (gy - p.lo[1])) * p.ox + (gx - p.lo[0]);
     if constexpr (FUSE_L2L) {
-        const int pnx = p.nx >> 1, pny = p.ny >> 1;
-        const long long pcell = (long long)pnx * pny * (p.nz >> 1);
-        const long long P = ((long long)(k >> 1) * pny + (gy >> 1)) * pnx + (gx >> 1);
+        const int pnx = p.pdim[0], pny = p.pdim[1];
+        const long long pcell = (long long)pnx * pny * p.pdim[2];
+        const long long P = ((long long)((k >> 1) + p.psh[2]) * pny + ((gy >> 1) + p.psh[1])) * pnx + ((gx >> 1) + p.psh[0]);
         double pL[20], sh[20], e[3];
         e[0] = ((double)(gx & 1) - 0.5) * p.hc + dA[0] - p.poff[P];
         e[1] = ((double)(gy & 1) - 0.5) * p.hc + dA[1] - p.poff[pcell + P];

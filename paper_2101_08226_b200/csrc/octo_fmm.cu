@@ -490,6 +490,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.leaf = nullptr;
     P.tile_list = nullptr;
     P.tile_offset = 0;
+    for (int a = 0; a < 3; ++a) { P.pdim[a] = cfg->n[a] / 2; P.psh[a] = 0; }
     for (int d = 0; d <= 2 * REACH_MAX; ++d) P.hmul[d] = h->hmul[d];
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {

@@ -24,24 +24,33 @@ namespace octo {
 // GIVEN (second right-hand side, L81-83: d(rho)/dt expanded about the centres of rho): delta_P is read from poff
 // instead of being computed and written; coff are then the children's centres from the first right-hand side.
 // ------------------------------------------------------------------------------------------
-template <bool LEAF, bool GIVEN = false>
+// Child arrays stored as a BOX of their lattice (levels of the adaptive tree): cbox = extents of the child arrays and the
+// (even) shift of the child index, child = 2 * parent + (a,b,c) + sh; children outside the box do not exist (zero mass).
+// The uniform solve passes a null box: the child arrays are exactly twice the parent's.
+struct ChildBox { int n[3]; int sh[3]; };
+
+template <bool LEAF, bool GIVEN = false, bool BOXED = false>
 __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm, const double* __restrict__ coff,
                                                   double* __restrict__ pm, double* __restrict__ poff, int pnx, int pny, int pnz,
-                                                  double hc)
+                                                  double hc, const ChildBox cb = ChildBox())
 {
     // grid = (ceil(pnx / blockDim.x), pny, pnz): no integer divisions
-    const long long pcell = (long long)pnx * pny * pnz, ccell = 8 * pcell;
+    const long long pcell = (long long)pnx * pny * pnz;
     const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y, K = blockIdx.z;
     if (I >= pnx) return;
     const long long P = ((long long)K * pny + J) * pnx + I;
-    const int cnx = 2 * pnx, cny = 2 * pny;
+    const int cnx = BOXED ? cb.n[0] : 2 * pnx, cny = BOXED ? cb.n[1] : 2 * pny, cnz = BOXED ? cb.n[2] : 2 * pnz;
+    const long long ccell = (long long)cnx * cny * cnz;
     long long cell[8];
     double rel[8][3], m0s[8];
     double mass = 0.0, com[3] = {0.0, 0.0, 0.0};
+    // all eight children are inside the child box or none is (the shift is even and so are the extents)
+    const int cx0 = 2 * I + (BOXED ? cb.sh[0] : 0), cy0 = 2 * J + (BOXED ? cb.sh[1] : 0), cz0 = 2 * K + (BOXED ? cb.sh[2] : 0);
+    const bool inside = !BOXED || (cx0 >= 0 && cy0 >= 0 && cz0 >= 0 && cx0 < cnx && cy0 < cny && cz0 < cnz);
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         const int a[3] = {c & 1, (c >> 1) & 1, (c >> 2) & 1};
-        cell[c] = ((long long)(2 * K + a[2]) * cny + (2 * J + a[1])) * cnx + (2 * I + a[0]);
+        cell[c] = inside ? ((long long)(cz0 + a[2]) * cny + (cy0 + a[1])) * cnx + (cx0 + a[0]) : (long long)a[0];
         double m0;
         if (LEAF) {          // the two x-children are one aligned double2 (cm is 16-byte aligned, cnx is even)
             const double2 pair = *reinterpret_cast<const double2*>(cm + (cell[c] - a[0]));
@@ -49,11 +58,13 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
         } else {
             m0 = cm[cell[c]];
         }
+        if (BOXED && !inside) m0 = 0.0;
         m0s[c] = m0;
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
-            rel[c][i] = ((double)a[i] - 0.5) * hc + (LEAF ? 0.0 : coff[i * ccell + cell[c]]);
-            com[i] += m0 * rel[c][i] + (LEAF ? 0.0 : cm[(1 + i) * ccell + cell[c]]);
+            const bool none = LEAF || (BOXED && !inside);
+            rel[c][i] = ((double)a[i] - 0.5) * hc + (none ? 0.0 : coff[i * ccell + cell[c]]);
+            com[i] += m0 * rel[c][i] + (none ? 0.0 : cm[(1 + i) * ccell + cell[c]]);
         }
         mass += m0;
     }
@@ -74,7 +85,7 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
         double M[20];
         M[0] = m0s[c];
 #pragma unroll
-        for (int t = 1; t < 20; ++t) M[t] = LEAF ? 0.0 : cm[t * ccell + cell[c]];
+        for (int t = 1; t < 20; ++t) M[t] = (LEAF || (BOXED && !inside)) ? 0.0 : cm[t * ccell + cell[c]];
         double d[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) d[i] = rel[c][i] - dP[i];

@@ -48,20 +48,23 @@ __global__ void __launch_bounds__(256) tree_leaf_moments_kernel(const unsigned c
 }
 
 struct TreeFinishArgs {
-    int n;                          // cells per axis of this level
+    int n[3];                       // extents of this level's arrays (a box of its lattice, multiples of 8)
     double h;                       // its cell width
-    const unsigned char* kind;      // [n^3]
-    const unsigned char* nodeflag;  // [(n/8)^3]
-    const double* lm;               // masked masses of this level (not used here; kept for symmetry)
-    double* out;                    // [4][n^3]: in = leaf-leaf point-mass sums of the tensor-core kernel; out = (phi, g)
-    const double* L;                // this level's finished expansions [20][n^3] (correction beside, parent's part included)
-    const double* C;                // [3][n^3]
-    const double* pL;               // parent level [20][(n/2)^3], pC [3][..], poff [3][..]
+    const unsigned char* kind;      // [nz][ny][nx]
+    const unsigned char* nodeflag;  // [(nz/8)][(ny/8)][(nx/8)]
+    double* out;                    // [4][cells]: in = leaf-leaf point-mass sums of the tensor-core kernel; out = (phi, g)
+    const double* L;                // this level's finished expansions [20][cells] (correction beside, parent's part included)
+    const double* C;                // [3][cells]
+    const double* pL;               // parent level [20][pn cells], pC [3][..], poff [3][..]
     const double* pC;
     const double* poff;
-    const unsigned char* kind_f;    // level below: [(2n)^3] or null
+    int pn[3];                      // extents of the parent arrays;  parent index = (index >> 1) + psh
+    int psh[3];
+    const unsigned char* kind_f;    // level below, or null: [fn cells];  child index = 2 * index + (a,b,c) + fsh
     const double* mass_f;           // its masked masses
-    const unsigned char* kind_c;    // level above: [(n/2)^3] or null
+    int fn[3];
+    int fsh[3];
+    const unsigned char* kind_c;    // level above (= the parent arrays' level), or null: [pn cells]
     const double* mass_c;
     unsigned long long* count;      // null, or counts[2] += cross-level pairs taken (ordered)
 };
@@ -71,22 +74,25 @@ struct TreeFinishArgs {
 //   this level's own L (sub-grids flagged NODE_OWN_L: Eq. 15 partners that are refined + the parent's shifted expansion,
 //   already added by the fused L2L epilogue) or else the parent's expansion evaluated at the leaf centre;
 //   + the children of the refined cells of its near field (NODE_OWN_L) and the coarser leaves in the near field of its
-//   parent (NODE_COARSE_NBR), as point masses:  x_A - x_b = ((double)(2 i_A - i_b) + 0.5) * (h / 2) per axis.
+//   parent (NODE_COARSE_NBR), as point masses:  x_A - x_b = ((double)(2 i_A - i_b) + 0.5) * (h / 2) per axis, i the
+//   index on the level's own LATTICE (the box shifts drop out of the difference: 2 i_A - i_b = 2 (A - B) - (a,b,c) for
+//   the child (a,b,c) of B).
 // Cells that are not leaves get zeros.  The near-field offsets come from the constant bank (c_near).
 __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishArgs a)
 {
-    const int n = a.n;
+    const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
     const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
-    if (i >= n) return;
-    const long long ncell = (long long)n * n * n;
-    const long long cell = ((long long)k * n + j) * n + i;
+    if (i >= nx) return;
+    const long long ncell = (long long)nx * ny * nz;
+    const long long cell = ((long long)k * ny + j) * nx + i;
     if (a.kind[cell] != KIND_LEAF) {
 #pragma unroll
         for (int c = 0; c < 4; ++c) a.out[c * ncell + cell] = 0.0;
         return;
     }
-    const int nn = n >> 3;
-    const unsigned char flag = a.nodeflag[((long long)(k >> 3) * nn + (j >> 3)) * nn + (i >> 3)];
+    const unsigned char flag = a.nodeflag[((long long)(k >> 3) * (ny >> 3) + (j >> 3)) * (nx >> 3) + (i >> 3)];
+    const int pi = (i >> 1) + a.psh[0], pj = (j >> 1) + a.psh[1], pk = (k >> 1) + a.psh[2];   // parent, in the parent arrays
+    const long long pcell = (long long)a.pn[0] * a.pn[1] * a.pn[2];
     double v[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) v[c] = a.out[c * ncell + cell];
@@ -95,9 +101,7 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
 #pragma unroll
         for (int c = 0; c < 3; ++c) v[1 + c] -= a.L[(1 + c) * ncell + cell] + a.C[c * ncell + cell];
     } else {
-        const int pn = n >> 1;
-        const long long pcell = ncell >> 3;
-        const long long P = ((long long)(k >> 1) * pn + (j >> 1)) * pn + (i >> 1);
+        const long long P = ((long long)pk * a.pn[1] + pj) * a.pn[0] + pi;
         double Lp[20], sh[20], e[3];
 #pragma unroll
         for (int t = 0; t < 20; ++t) Lp[t] = a.pL[t * pcell + P];
@@ -113,20 +117,20 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
     if ((flag & NODE_OWN_L) && a.kind_f) {
         // the children of the refined cells of the near field
         const int cls = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
-        const int fn = 2 * n;
         const double hf = 0.5 * a.h;
         double s[4] = {0.0, 0.0, 0.0, 0.0};
         for (int q = 0; q < c_near_count[cls]; ++q) {
             const char4 d = c_near[cls][q];
             const int bi = i + d.x, bj = j + d.y, bk = k + d.z;
-            if (bi < 0 || bj < 0 || bk < 0 || bi >= n || bj >= n || bk >= n) continue;
-            if (a.kind[((long long)bk * n + bj) * n + bi] != KIND_REFINED) continue;
+            if (bi < 0 || bj < 0 || bk < 0 || bi >= nx || bj >= ny || bk >= nz) continue;
+            if (a.kind[((long long)bk * ny + bj) * nx + bi] != KIND_REFINED) continue;
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
-                const int ci = 2 * bi + (c & 1), cj = 2 * bj + ((c >> 1) & 1), ck = 2 * bk + (c >> 2);
-                const double m = a.mass_f[((long long)ck * fn + cj) * fn + ci];
-                const double Rx = ((double)(2 * i - ci) + 0.5) * hf, Ry = ((double)(2 * j - cj) + 0.5) * hf,
-                             Rz = ((double)(2 * k - ck) + 0.5) * hf;
+                const int ax = c & 1, ay = (c >> 1) & 1, az = c >> 2;
+                const int ci = 2 * bi + ax + a.fsh[0], cj = 2 * bj + ay + a.fsh[1], ck = 2 * bk + az + a.fsh[2];   // in the fine arrays
+                const double m = a.mass_f[((long long)ck * a.fn[1] + cj) * a.fn[0] + ci];
+                const double Rx = ((double)(-2 * d.x - ax) + 0.5) * hf, Ry = ((double)(-2 * d.y - ay) + 0.5) * hf,
+                             Rz = ((double)(-2 * d.z - az) + 0.5) * hf;
                 const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = sqrt(r2), w3 = -m / (r2 * r);
                 s[0] += -m / r; s[1] += w3 * Rx; s[2] += w3 * Ry; s[3] += w3 * Rz;
                 ++taken;
@@ -137,19 +141,19 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
     }
     if ((flag & NODE_COARSE_NBR) && a.kind_c) {
         // the coarser leaves in the near field of the parent
-        const int pi = i >> 1, pj = j >> 1, pk = k >> 1, pn = n >> 1;
-        const int cls = (pi & 1) + 2 * (pj & 1) + 4 * (pk & 1);
+        const int cls = (pi & 1) + 2 * (pj & 1) + 4 * (pk & 1);       // psh is even: the parity of the lattice index
         const double hf = a.h;                       // this level is the fine one of the pair
         double s[4] = {0.0, 0.0, 0.0, 0.0};
         for (int q = 0; q < c_near_count[cls]; ++q) {
             const char4 d = c_near[cls][q];
             const int ai = pi + d.x, aj = pj + d.y, ak = pk + d.z;
-            if (ai < 0 || aj < 0 || ak < 0 || ai >= pn || aj >= pn || ak >= pn) continue;
-            const long long A = ((long long)ak * pn + aj) * pn + ai;
+            if (ai < 0 || aj < 0 || ak < 0 || ai >= a.pn[0] || aj >= a.pn[1] || ak >= a.pn[2]) continue;
+            const long long A = ((long long)ak * a.pn[1] + aj) * a.pn[0] + ai;
             if (a.kind_c[A] != KIND_LEAF) continue;
             const double m = a.mass_c[A];
-            const double Rx = -(((double)(2 * ai - i) + 0.5) * hf), Ry = -(((double)(2 * aj - j) + 0.5) * hf),
-                         Rz = -(((double)(2 * ak - k) + 0.5) * hf);
+            // x_b - x_A = -(x_A - x_b),  2 i_A - i_b = 2 (parent + d) - (2 parent + (a,b,c)) = 2 d - (a,b,c)
+            const double Rx = -(((double)(2 * d.x - (i & 1)) + 0.5) * hf), Ry = -(((double)(2 * d.y - (j & 1)) + 0.5) * hf),
+                         Rz = -(((double)(2 * d.z - (k & 1)) + 0.5) * hf);
             const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = sqrt(r2), w3 = -m / (r2 * r);
             s[0] += -m / r; s[1] += w3 * Rx; s[2] += w3 * Ry; s[3] += w3 * Rz;
             ++taken;
@@ -165,20 +169,21 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
 // Pair counter of one level, for the bit-exact check of the pair set against the oracle: counts[0] += ordered pairs of the
 // multipole step (both exist, on the Eq. 15 list, not two leaves), counts[1] += leaf-leaf point-mass pairs (leaf-level list).
 // The Eq. 15 list is in the constant bank as (dx, dy, dz) of c_entries, the near field as c_near.
-__global__ void __launch_bounds__(128) tree_count_kernel(const unsigned char* __restrict__ kind, int n, unsigned long long* __restrict__ counts)
+__global__ void __launch_bounds__(128) tree_count_kernel(const unsigned char* __restrict__ kind, int nx, int ny, int nz,
+                                                         unsigned long long* __restrict__ counts)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
     unsigned long long m2l = 0, p2p = 0;
-    if (i < n) {
-        const unsigned char ka = kind[((long long)k * n + j) * n + i];
+    if (i < nx) {
+        const unsigned char ka = kind[((long long)k * ny + j) * nx + i];
         if (ka != KIND_ABSENT) {
             const int cls = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
             const int s_end = c_begin[cls][2 * REACH_MAX + 1];
             for (int s = c_begin[cls][0]; s < s_end; ++s) {
                 const StEntry e = c_entries[cls * MAX_LIST + s];
                 const int bi = i + e.dx, bj = j + e.dy, bk = k + e.dz;
-                if (bi < 0 || bj < 0 || bk < 0 || bi >= n || bj >= n || bk >= n) continue;
-                const unsigned char kb = kind[((long long)bk * n + bj) * n + bi];
+                if (bi < 0 || bj < 0 || bk < 0 || bi >= nx || bj >= ny || bk >= nz) continue;
+                const unsigned char kb = kind[((long long)bk * ny + bj) * nx + bi];
                 if (kb == KIND_ABSENT) continue;
                 if (ka == KIND_LEAF && kb == KIND_LEAF) ++p2p; else ++m2l;
             }
@@ -186,8 +191,8 @@ __global__ void __launch_bounds__(128) tree_count_kernel(const unsigned char* __
                 for (int q = 0; q < c_near_count[cls]; ++q) {
                     const char4 d = c_near[cls][q];
                     const int bi = i + d.x, bj = j + d.y, bk = k + d.z;
-                    if (bi < 0 || bj < 0 || bk < 0 || bi >= n || bj >= n || bk >= n) continue;
-                    if (kind[((long long)bk * n + bj) * n + bi] == KIND_LEAF) ++p2p;
+                    if (bi < 0 || bj < 0 || bk < 0 || bi >= nx || bj >= ny || bk >= nz) continue;
+                    if (kind[((long long)bk * ny + bj) * nx + bi] == KIND_LEAF) ++p2p;
                 }
         }
     }

@@ -12,20 +12,23 @@
 namespace {
 
 struct TreeLevel {
-    int n;
+    int n[3];                   // extents of this level's arrays: a BOX of the level's lattice (multiples of 8)
+    int lo[3];                  // lower corner of the box on the lattice (multiples of 8)
+    int psh[3];                 // parent index in the parent level's arrays = (index >> 1) + psh
     double h;
     bool has_refined, has_leaf;
-    unsigned char* kind;        // device [n^3]
-    unsigned char* nodeflag;    // device [(n/8)^3]
-    double* lm;                 // device [n^3] masked masses (leaf: m, else 0)
-    double* raw;                // device [20][n^3] (null on a level without refined cells)
-    double* off;                // device [3][n^3]
+    unsigned char* kind;        // device [nz][ny][nx]
+    unsigned char* nodeflag;    // device, per sub-grid
+    double* lm;                 // device [cells] masked masses (leaf: m, else 0)
+    double* raw;                // device [20][cells] (null on a level without refined cells)
+    double* off;                // device [3][cells]
     octo_fmm* fmm;              // multipole handle (null without refined cells)
     octo_fmm* leaf;             // monopole handle, leaf-level list (null without leaves)
     int* m2l_tiles;  int n_m2l_tiles;     // bricks of the slab-fed kernel that have work
     int* p2p_tiles;  int n_p2p_tiles;     // 16 x 16 x 8 tiles of the tensor-core kernel that hold leaves
     std::vector<int> h_m2l_tiles, h_p2p_tiles;
     std::vector<unsigned char> h_nodeflag;
+    size_t cells() const { return (size_t)n[0] * n[1] * n[2]; }
 };
 
 struct TreePlan {
@@ -38,8 +41,8 @@ inline bool tree_config_ok(const octo_fmm_tree_config* c)
 {
     if (!c) return false;
     if (c->n0 < 8 || c->n0 > 2048 || (c->n0 & (c->n0 - 1))) return false;       // a power of two >= 8
-    if (c->depth < 1 || c->depth > 10) return false;
-    if (((long long)c->n0 << (c->depth - 1)) > 2048) return false;
+    if (c->depth < 1 || c->depth > 12) return false;
+    if (((long long)c->n0 << (c->depth - 1)) > (1 << 20)) return false;          // lattice indices stay far from 2^31
     if (!(c->h0 > 0.0) || !std::isfinite(c->h0)) return false;
     if (!(c->theta > 1.0 / 3.0 && c->theta < 1.0)) return false;
     return true;
@@ -53,8 +56,16 @@ octo_fmm_solver_config as_solver_config(const octo_fmm_tree_config& t)
     return s;
 }
 
-// Topology checks, per-sub-grid flags, tile lists and the workspace size.  kind_host[l] = [n_l^3] on the HOST.
-TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* kind_host)
+octo_fmm_config box_config(const octo_fmm_solver_config& sc, const int n[3], double h, int kind)
+{
+    octo_fmm_config c = level_config(sc, n[0], h, kind);
+    for (int a = 0; a < 3; ++a) c.n[a] = n[a];
+    return c;
+}
+
+// Topology checks, per-sub-grid flags, tile lists and the workspace size.  kind_host[l] = [nz][ny][nx] of level l's box on
+// the HOST; box = null (every level is its whole lattice) or depth x 6 ints (lo_x, lo_y, lo_z, n_x, n_y, n_z).
+TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* kind_host, const int* box)
 {
     TreePlan P;
     P.ok = false;
@@ -62,108 +73,127 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
     const int D = cfg.depth;
     P.lev.resize(D);
     const octo_fmm_solver_config sc = as_solver_config(cfg);
+    // kind of the sub-grid with LATTICE coordinates (I, J, K) of level l: absent outside the box
+    auto node_kind = [&](int l, int I, int J, int K) -> unsigned char {
+        const TreeLevel& L = P.lev[l];
+        const int i = 8 * I - L.lo[0], j = 8 * J - L.lo[1], k = 8 * K - L.lo[2];
+        if (i < 0 || j < 0 || k < 0 || i >= L.n[0] || j >= L.n[1] || k >= L.n[2]) return KIND_ABSENT;
+        return kind_host[l][((size_t)k * L.n[1] + j) * L.n[0] + i];
+    };
     for (int l = 0; l < D; ++l) {
         TreeLevel& L = P.lev[l];
-        L.n = cfg.n0 << l;
-        L.h = cfg.h0 / (double)(1 << l);
+        const long long lat = (long long)cfg.n0 << l;
+        for (int a = 0; a < 3; ++a) {
+            L.lo[a] = box ? box[6 * l + a] : 0;
+            L.n[a] = box ? box[6 * l + 3 + a] : (int)lat;
+            if (L.lo[a] < 0 || L.n[a] < 8 || (L.lo[a] % 8) || (L.n[a] % 8) || (long long)L.lo[a] + L.n[a] > lat || L.n[a] > 4096) return P;
+            if (l == 0 && (L.lo[a] != 0 || L.n[a] != cfg.n0)) return P;      // level 0 is the whole lattice
+            L.psh[a] = l > 0 ? L.lo[a] / 2 - P.lev[l - 1].lo[a] : 0;
+        }
+        L.h = cfg.h0 / (double)(1LL << l);
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
-        const int n = L.n, nn = n / 8;
         L.has_refined = L.has_leaf = false;
-        // kinds are constant over sub-grids, children exist iff the parent is refined, the last level has no refined cell
-        for (int K = 0; K < nn; ++K)
-            for (int J = 0; J < nn; ++J)
-                for (int I = 0; I < nn; ++I) {
-                    const unsigned char v = k[((size_t)(8 * K) * n + 8 * J) * n + 8 * I];
+        // kinds are constant over sub-grids, a cell exists iff its parent is refined, the last level has no refined cell
+        for (int K = 0; K < L.n[2] / 8; ++K)
+            for (int J = 0; J < L.n[1] / 8; ++J)
+                for (int I = 0; I < L.n[0] / 8; ++I) {
+                    const unsigned char v = k[((size_t)(8 * K) * L.n[1] + 8 * J) * L.n[0] + 8 * I];
                     if (v > 2) return P;
                     for (int c = 0; c < 8; ++c)
                         for (int b = 0; b < 8; ++b)
                             for (int a = 0; a < 8; ++a)
-                                if (k[((size_t)(8 * K + c) * n + 8 * J + b) * n + 8 * I + a] != v) return P;
+                                if (k[((size_t)(8 * K + c) * L.n[1] + 8 * J + b) * L.n[0] + 8 * I + a] != v) return P;
                     if (l == 0 && v == KIND_ABSENT) return P;
                     if (l == D - 1 && v == KIND_REFINED) return P;
                     if (l > 0) {
-                        const unsigned char* kp = kind_host[l - 1];
-                        const int pn = n / 2;
-                        const unsigned char pv = kp[((size_t)(4 * K) * pn + 4 * J) * pn + 4 * I];
+                        const unsigned char pv = node_kind(l - 1, (L.lo[0] / 8 + I) / 2, (L.lo[1] / 8 + J) / 2, (L.lo[2] / 8 + K) / 2);
                         if ((v != KIND_ABSENT) != (pv == KIND_REFINED)) return P;
                     }
                     L.has_refined |= v == KIND_REFINED;
                     L.has_leaf |= v == KIND_LEAF;
                 }
+        // every refined sub-grid of the level above has all its children inside this level's box
+        if (l > 0) {
+            const TreeLevel& U = P.lev[l - 1];
+            for (int K = 0; K < U.n[2] / 8; ++K)
+                for (int J = 0; J < U.n[1] / 8; ++J)
+                    for (int I = 0; I < U.n[0] / 8; ++I) {
+                        if (kind_host[l - 1][((size_t)(8 * K) * U.n[1] + 8 * J) * U.n[0] + 8 * I] != KIND_REFINED) continue;
+                        for (int c = 0; c < 8; ++c)
+                            if (node_kind(l, 2 * (U.lo[0] / 8 + I) + (c & 1), 2 * (U.lo[1] / 8 + J) + ((c >> 1) & 1),
+                                          2 * (U.lo[2] / 8 + K) + (c >> 2)) == KIND_ABSENT)
+                                return P;
+                    }
+        }
     }
+    if (P.lev[D - 1].has_refined) return P;
     // flags: NODE_OWN_L = leaf sub-grid with a refined 26-neighbour; NODE_COARSE_NBR = the parent sub-grid has a leaf 26-neighbour
     for (int l = 0; l < D; ++l) {
         TreeLevel& L = P.lev[l];
-        const int n = L.n, nn = n / 8;
-        const unsigned char* k = kind_host[l];
-        auto node_kind = [&](const unsigned char* kk, int m, int I, int J, int K) { return kk[((size_t)(8 * K) * m + 8 * J) * m + 8 * I]; };
-        L.h_nodeflag.assign((size_t)nn * nn * nn, 0);
-        for (int K = 0; K < nn; ++K)
-            for (int J = 0; J < nn; ++J)
-                for (int I = 0; I < nn; ++I) {
-                    if (node_kind(k, n, I, J, K) != KIND_LEAF) continue;
+        const int nnx = L.n[0] / 8, nny = L.n[1] / 8, nnz = L.n[2] / 8;
+        const int gx0 = L.lo[0] / 8, gy0 = L.lo[1] / 8, gz0 = L.lo[2] / 8;
+        L.h_nodeflag.assign((size_t)nnx * nny * nnz, 0);
+        for (int K = 0; K < nnz; ++K)
+            for (int J = 0; J < nny; ++J)
+                for (int I = 0; I < nnx; ++I) {
+                    if (node_kind(l, gx0 + I, gy0 + J, gz0 + K) != KIND_LEAF) continue;
                     unsigned char f = 0;
                     for (int c = -1; c <= 1; ++c)
                         for (int b = -1; b <= 1; ++b)
                             for (int a = -1; a <= 1; ++a) {
-                                const int i2 = I + a, j2 = J + b, k2 = K + c;
-                                if (i2 >= 0 && j2 >= 0 && k2 >= 0 && i2 < nn && j2 < nn && k2 < nn && node_kind(k, n, i2, j2, k2) == KIND_REFINED)
-                                    f |= NODE_OWN_L;
-                                if (l > 0) {
-                                    const int pnn = nn / 2, pi = I / 2 + a, pj = J / 2 + b, pk = K / 2 + c;
-                                    if (pi >= 0 && pj >= 0 && pk >= 0 && pi < pnn && pj < pnn && pk < pnn &&
-                                        node_kind(kind_host[l - 1], n / 2, pi, pj, pk) == KIND_LEAF)
-                                        f |= NODE_COARSE_NBR;
-                                }
+                                if (node_kind(l, gx0 + I + a, gy0 + J + b, gz0 + K + c) == KIND_REFINED) f |= NODE_OWN_L;
+                                if (l > 0 && node_kind(l - 1, (gx0 + I) / 2 + a, (gy0 + J) / 2 + b, (gz0 + K) / 2 + c) == KIND_LEAF)
+                                    f |= NODE_COARSE_NBR;
                             }
-                    L.h_nodeflag[((size_t)K * nn + J) * nn + I] = f;
+                    L.h_nodeflag[((size_t)K * nny + J) * nnx + I] = f;
                 }
-        auto node_works = [&](int I, int J, int K) {   // its cells take part in the multipole step of this level
-            const unsigned char v = node_kind(k, n, I, J, K);
-            return v == KIND_REFINED || (v == KIND_LEAF && (L.h_nodeflag[((size_t)K * nn + J) * nn + I] & NODE_OWN_L));
+        auto node_works = [&](int I, int J, int K) {   // local sub-grid: its cells take part in the multipole step of this level
+            if (I >= nnx || J >= nny || K >= nnz) return false;
+            const unsigned char v = node_kind(l, gx0 + I, gy0 + J, gz0 + K);
+            return v == KIND_REFINED || (v == KIND_LEAF && (L.h_nodeflag[((size_t)K * nny + J) * nnx + I] & NODE_OWN_L));
         };
         // bricks of the slab-fed kernel: 16 x 8 x 3 cells, dense enumeration t = (ty * tiles_x + tx) * tiles_z + tz
         if (L.has_refined) {
-            const int tx_n = (n + TILE_X - 1) / TILE_X, ty_n = (n + TILE_Y - 1) / TILE_Y, tz_n = (n + TILE_Z - 1) / TILE_Z;
+            const int tx_n = (L.n[0] + TILE_X - 1) / TILE_X, ty_n = (L.n[1] + TILE_Y - 1) / TILE_Y, tz_n = (L.n[2] + TILE_Z - 1) / TILE_Z;
             for (int ty = 0; ty < ty_n; ++ty)
                 for (int tx = 0; tx < tx_n; ++tx)
                     for (int tz = 0; tz < tz_n; ++tz) {
                         bool work = false;
-                        const int z0 = tz * TILE_Z, z1 = std::min(z0 + TILE_Z, n) - 1;
+                        const int z0 = tz * TILE_Z, z1 = std::min(z0 + TILE_Z, L.n[2]) - 1;
                         for (int K = z0 / 8; K <= z1 / 8 && !work; ++K)
-                            for (int I = (tx * TILE_X) / 8; I <= std::min(tx * TILE_X + TILE_X - 1, n - 1) / 8 && !work; ++I)
+                            for (int I = (tx * TILE_X) / 8; I <= std::min(tx * TILE_X + TILE_X - 1, L.n[0] - 1) / 8 && !work; ++I)
                                 work = node_works(I, (ty * TILE_Y) / 8, K);
                         if (work) L.h_m2l_tiles.push_back((ty * tx_n + tx) * tz_n + tz);
                     }
         }
         // tiles of the tensor-core leaf kernel: 16 x 16 x 8 cells, b = (tz * by + ty) * bx + tx
         if (L.has_leaf) {
-            const int bx = (n + MT_X - 1) / MT_X, by = (n + MT_Y - 1) / MT_Y, bz = (n + DT_Z - 1) / DT_Z;
+            const int bx = (L.n[0] + MT_X - 1) / MT_X, by = (L.n[1] + MT_Y - 1) / MT_Y, bz = (L.n[2] + DT_Z - 1) / DT_Z;
             for (int tz = 0; tz < bz; ++tz)
                 for (int ty = 0; ty < by; ++ty)
                     for (int tx = 0; tx < bx; ++tx) {
                         bool work = false;
-                        for (int J = 2 * ty; J <= std::min(2 * ty + 1, nn - 1) && !work; ++J)
-                            for (int I = 2 * tx; I <= std::min(2 * tx + 1, nn - 1) && !work; ++I)
-                                work = node_kind(k, n, I, J, tz) == KIND_LEAF;
+                        for (int J = 2 * ty; J <= std::min(2 * ty + 1, nny - 1) && !work; ++J)
+                            for (int I = 2 * tx; I <= std::min(2 * tx + 1, nnx - 1) && !work; ++I)
+                                work = node_kind(l, gx0 + I, gy0 + J, gz0 + tz) == KIND_LEAF;
                         if (work) L.h_p2p_tiles.push_back((tz * by + ty) * bx + tx);
                     }
         }
         L.n_m2l_tiles = (int)L.h_m2l_tiles.size();
         L.n_p2p_tiles = (int)L.h_p2p_tiles.size();
         // workspace of this level
-        const size_t nc = (size_t)n * n * n;
-        P.bytes += align_up(nc) + align_up((size_t)nn * nn * nn) + align_up(nc * 8);           // kind, nodeflag, lm
+        const size_t nc = L.cells();
+        P.bytes += align_up(nc) + align_up((size_t)nnx * nny * nnz) + align_up(nc * 8);           // kind, nodeflag, lm
         P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4);
         if (L.has_refined) {
-            octo_fmm_config mc = level_config(sc, n, L.h, OCTO_FMM_MULTIPOLE);
+            octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
             P.bytes += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
         }
         if (L.has_leaf) {
-            octo_fmm_config lc = level_config(sc, n, L.h, OCTO_FMM_MONOPOLE);
+            octo_fmm_config lc = box_config(sc, L.n, L.h, OCTO_FMM_MONOPOLE);
             P.bytes += sizes_of(lc, CF_LEAF_LIST).total;
         }
     }
@@ -193,10 +223,10 @@ struct octo_fmm_tree {
 
 extern "C" {
 
-size_t octo_fmm_tree_workspace_bytes(const octo_fmm_tree_config* cfg, const unsigned char* const* kind_host)
+size_t octo_fmm_tree_workspace_bytes(const octo_fmm_tree_config* cfg, const unsigned char* const* kind_host, const int* box)
 {
     if (!tree_config_ok(cfg) || !kind_host) return 0;
-    const TreePlan P = tree_plan(*cfg, kind_host);
+    const TreePlan P = tree_plan(*cfg, kind_host, box);
     return P.ok ? P.bytes : 0;
 }
 
@@ -214,12 +244,12 @@ int octo_fmm_tree_destroy(octo_fmm_tree_t* t)
     return rc;
 }
 
-int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* const* kind_host, octo_fmm_tree_t** out)
+int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* const* kind_host, const int* box, octo_fmm_tree_t** out)
 {
     if (!out) return OCTO_FMM_EINVAL;
     *out = nullptr;
     if (!tree_config_ok(cfg) || !kind_host) return OCTO_FMM_EINVAL;
-    TreePlan P = tree_plan(*cfg, kind_host);
+    TreePlan P = tree_plan(*cfg, kind_host, box);
     if (!P.ok) return OCTO_FMM_EINVAL;
     if (!cfg->workspace || cfg->workspace_bytes < P.bytes || ((uintptr_t)cfg->workspace % ALIGN)) return OCTO_FMM_EINVAL;
     if (cudaSetDevice(cfg->device) != cudaSuccess) return OCTO_FMM_ECUDA;
@@ -235,7 +265,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     int rc = OCTO_FMM_OK;
     for (size_t l = 0; l < t->lev.size() && rc == OCTO_FMM_OK; ++l) {
         TreeLevel& L = t->lev[l];
-        const size_t nc = (size_t)L.n * L.n * L.n, nn = (size_t)(L.n / 8) * (L.n / 8) * (L.n / 8);
+        const size_t nc = L.cells(), nn = (size_t)(L.n[0] / 8) * (L.n[1] / 8) * (L.n[2] / 8);
         L.kind = (unsigned char*)w; w += align_up(nc);
         L.nodeflag = (unsigned char*)w; w += align_up(nn);
         L.lm = (double*)w; w += align_up(nc * 8);
@@ -249,7 +279,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
             break;
         }
         if (L.has_refined) {
-            octo_fmm_config mc = level_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
+            octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
             mc.workspace = w; mc.workspace_bytes = sizes_of(mc, CF_ANY_SIZE).total; w += mc.workspace_bytes;
             L.raw = (double*)w; w += align_up(nc * 20 * 8);
             L.off = (double*)w; w += align_up(nc * 3 * 8);
@@ -261,7 +291,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
             L.fmm->tile_count = L.n_m2l_tiles;
         }
         if (L.has_leaf) {
-            octo_fmm_config lc = level_config(sc, L.n, L.h, OCTO_FMM_MONOPOLE);
+            octo_fmm_config lc = box_config(sc, L.n, L.h, OCTO_FMM_MONOPOLE);
             lc.workspace = w; lc.workspace_bytes = sizes_of(lc, CF_LEAF_LIST).total; w += lc.workspace_bytes;
             rc = create_internal(&lc, CF_LEAF_LIST, &L.leaf);
             if (rc != OCTO_FMM_OK) break;
@@ -300,17 +330,19 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
     // ---- upward pass: finest level first ----
     for (int l = D - 1; l >= 0; --l) {
         TreeLevel& L = t->lev[l];
-        const long long nc = (long long)L.n * L.n * L.n;
+        const long long nc = (long long)L.cells();
         if (L.has_refined) {
             TreeLevel& F = t->lev[l + 1];
-            const dim3 blocks((unsigned)((L.n + 127) / 128), (unsigned)L.n, (unsigned)L.n);
-            if (F.raw) m2m_kernel<false><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n, L.n, L.n, F.h);
-            else       m2m_kernel<true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n, L.n, L.n, F.h);
+            ChildBox cb;
+            for (int a = 0; a < 3; ++a) { cb.n[a] = F.n[a]; cb.sh[a] = -2 * F.psh[a]; }
+            const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
+            if (F.raw) m2m_kernel<false, false, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
+            else       m2m_kernel<true, false, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
         }
         tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
-    // ---- the uniform levels above level 0: up ... ----
+    // ---- the uniform levels above level 0 (the whole lattice): up ... ----
     for (size_t lv = 0; lv < t->up.size(); ++lv) {
         SolverLevel& l = t->up[lv];
         const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
@@ -349,15 +381,22 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         // parent arrays of this level: the tree level above, or the finest uniform level
         // (a level above without refined cells means that this level is empty: nothing reads the parent arrays then)
         const double *pL = nullptr, *pC = nullptr, *poff = nullptr;
-        if (l > 0 && t->lev[l - 1].fmm) { pL = t->lev[l - 1].fmm->L; pC = t->lev[l - 1].fmm->C; poff = t->lev[l - 1].off; }
-        else if (l == 0)                { pL = t->up[0].fmm->L; pC = t->up[0].fmm->C; poff = t->up[0].off; }
+        int pn[3] = {L.n[0] / 2, L.n[1] / 2, L.n[2] / 2};
+        if (l > 0 && t->lev[l - 1].fmm) {
+            pL = t->lev[l - 1].fmm->L; pC = t->lev[l - 1].fmm->C; poff = t->lev[l - 1].off;
+            for (int a = 0; a < 3; ++a) pn[a] = t->lev[l - 1].n[a];
+        } else if (l == 0) {
+            pL = t->up[0].fmm->L; pC = t->up[0].fmm->C; poff = t->up[0].off;
+        }
         if (!pL && (L.has_refined || L.has_leaf)) return OCTO_FMM_ESTATE;
         if (L.fmm && L.n_m2l_tiles > 0) {
             if ((rc = octo_fmm_set_moments(L.fmm, L.raw, L.off)) != OCTO_FMM_OK) return rc;
-            const long long nc = (long long)L.n * L.n * L.n;
-            stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, L.fmm->src, L.n, L.n, L.n);
+            const long long nc = (long long)L.cells();
+            stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, L.fmm->src, L.n[0], L.n[1], L.n[2]);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
-            L.fmm->prm.pL = pL; L.fmm->prm.pC = pC; L.fmm->prm.poff = poff;
+            Params& Q = L.fmm->prm;
+            Q.pL = pL; Q.pC = pC; Q.poff = poff;
+            for (int a = 0; a < 3; ++a) { Q.pdim[a] = pn[a]; Q.psh[a] = L.psh[a]; }
             rc = octo_fmm_interact(L.fmm);
             clear_parent(L.fmm);
             if (rc != OCTO_FMM_OK) return rc;
@@ -376,13 +415,19 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             BankLock guard(hb);
             if (bank_acquire(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
             TreeFinishArgs a;
-            a.n = L.n; a.h = L.h; a.kind = L.kind; a.nodeflag = L.nodeflag; a.lm = L.lm; a.out = out[l];
+            std::memset(&a, 0, sizeof a);
+            for (int c = 0; c < 3; ++c) { a.n[c] = L.n[c]; a.pn[c] = pn[c]; a.psh[c] = L.psh[c]; }
+            a.h = L.h; a.kind = L.kind; a.nodeflag = L.nodeflag; a.out = out[l];
             a.L = L.fmm ? L.fmm->L : nullptr; a.C = L.fmm ? L.fmm->C : nullptr;
             a.pL = pL; a.pC = pC; a.poff = poff;
-            a.kind_f = l + 1 < D ? t->lev[l + 1].kind : nullptr; a.mass_f = l + 1 < D ? t->lev[l + 1].lm : nullptr;
-            a.kind_c = l > 0 ? t->lev[l - 1].kind : nullptr;     a.mass_c = l > 0 ? t->lev[l - 1].lm : nullptr;
+            if (l + 1 < D) {
+                TreeLevel& F = t->lev[l + 1];
+                a.kind_f = F.kind; a.mass_f = F.lm;
+                for (int c = 0; c < 3; ++c) { a.fn[c] = F.n[c]; a.fsh[c] = -2 * F.psh[c]; }
+            }
+            if (l > 0) { a.kind_c = t->lev[l - 1].kind; a.mass_c = t->lev[l - 1].lm; }
             a.count = count ? t->counts : nullptr;
-            const dim3 blocks((unsigned)((L.n + 127) / 128), (unsigned)L.n, (unsigned)L.n);
+            const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
             tree_leaf_finish_kernel<<<blocks, 128, 0, st>>>(a);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
             if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
@@ -392,8 +437,8 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             octo_fmm* hb = L.fmm ? L.fmm : t->up[0].fmm;
             BankLock guard(hb);
             if (bank_acquire(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
-            const dim3 blocks((unsigned)((L.n + 127) / 128), (unsigned)L.n, (unsigned)L.n);
-            tree_count_kernel<<<blocks, 128, 0, st>>>(L.kind, L.n, t->counts);
+            const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
+            tree_count_kernel<<<blocks, 128, 0, st>>>(L.kind, L.n[0], L.n[1], L.n[2], t->counts);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
             if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
         }
@@ -425,14 +470,11 @@ int octo_fmm_tree_interaction_counts(octo_fmm_tree_t* t, const double* const* ma
     return OCTO_FMM_OK;
 }
 
-size_t octo_fmm_tree_host_scratch_bytes(const octo_fmm_tree_config* cfg)
+size_t octo_fmm_tree_host_scratch_bytes(const octo_fmm_tree_t* t)
 {
-    if (!tree_config_ok(cfg)) return 0;
+    if (!t) return 0;
     size_t total = 0;
-    for (int l = 0; l < cfg->depth; ++l) {
-        const size_t n = (size_t)cfg->n0 << l, nc = n * n * n;
-        total += align_up(nc * 8) + align_up(nc * 4 * 8);
-    }
+    for (const TreeLevel& L : t->lev) total += align_up(L.cells() * 8) + align_up(L.cells() * 4 * 8);
     return total;
 }
 
@@ -440,7 +482,7 @@ int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host,
                              size_t scratch_bytes)
 {
     if (!t || !mass_host || !out_host || !scratch) return OCTO_FMM_EINVAL;
-    if (scratch_bytes < octo_fmm_tree_host_scratch_bytes(&t->cfg) || ((uintptr_t)scratch % ALIGN)) return OCTO_FMM_EINVAL;
+    if (scratch_bytes < octo_fmm_tree_host_scratch_bytes(t) || ((uintptr_t)scratch % ALIGN)) return OCTO_FMM_EINVAL;
     if (cudaSetDevice(t->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
     const int D = (int)t->lev.size();
     std::vector<const double*> m(D);
@@ -449,7 +491,7 @@ int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host,
     cudaStream_t st = t->stream;
     for (int l = 0; l < D; ++l) {
         if (!mass_host[l] || !out_host[l]) return OCTO_FMM_EINVAL;
-        const size_t nc = (size_t)t->lev[l].n * t->lev[l].n * t->lev[l].n;
+        const size_t nc = t->lev[l].cells();
         double* dm = (double*)w; w += align_up(nc * 8);
         o[l] = (double*)w; w += align_up(nc * 4 * 8);
         m[l] = dm;
@@ -459,7 +501,7 @@ int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host,
     const int rc = tree_solve_impl(t, m.data(), o.data(), false);
     if (rc != OCTO_FMM_OK) return rc;
     for (int l = 0; l < D; ++l) {
-        const size_t nc = (size_t)t->lev[l].n * t->lev[l].n * t->lev[l].n;
+        const size_t nc = t->lev[l].cells();
         if (cudaMemcpyAsync(out_host[l], o[l], nc * 4 * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     if (cudaStreamSynchronize(st) != cudaSuccess) return OCTO_FMM_ECUDA;

@@ -24,10 +24,15 @@ def env():
     return p, torch
 
 
-def _run(env, tree, theta, correction, counts=True):
+def _run(env, tree, theta, correction, counts=True, box=None):
+    """tree: fmm_inputs.Tree on whole lattices, or (n0, h0, kind, mass) with box given."""
     p, torch = env
-    t = p.OctoFMMTree(tree.n0, tree.h0, theta, tree.kind, correction)
-    mass = [torch.from_numpy(m).cuda() for m in tree.mass]
+    if box is None:
+        n0, h0, kind, masses = tree.n0, tree.h0, tree.kind, tree.mass
+    else:
+        n0, h0, kind, masses = tree
+    t = p.OctoFMMTree(n0, h0, theta, kind, correction, box=box)
+    mass = [torch.from_numpy(m).cuda() for m in masses]
     if counts:
         cnt, out = t.interaction_counts(mass)
     else:
@@ -127,3 +132,62 @@ def test_bad_topologies_are_refused(env):
             p.OctoFMMTree(tree.n0, tree.h0, 0.5, bad)
     with pytest.raises(ValueError):
         p.OctoFMMTree(tree.n0, tree.h0, 0.5, [k[:4] for k in tree.kind])
+
+
+def _compare_lists(kind, got, ref):
+    gmax = max(np.abs(r[1:]).max() for r in ref)
+    worst_phi = worst_g = 0.0
+    for l in range(len(kind)):
+        leaf = kind[l] == fi.TREE_LEAF
+        assert np.all(got[l][:, ~leaf] == 0.0)
+        if leaf.any():
+            worst_phi = max(worst_phi, float((np.abs(got[l][0] - ref[l][0])[leaf] / np.abs(ref[l][0])[leaf]).max()))
+            worst_g = max(worst_g, float(np.abs(got[l][1:] - ref[l][1:])[:, leaf].max() / gmax))
+    return worst_phi, worst_g
+
+
+@pytest.mark.parametrize("which", ["star", "seeded"])
+def test_levels_stored_as_boxes(env, which):
+    """The same trees with every level stored as the bounding box of its cells (boxes that shrink and move from level to
+    level): pair counts and numbers against the oracle, and bit-identical to the whole-lattice run of the library."""
+    tree = fi.star_tree(32, 4) if which == "star" else fi.seeded_tree(3, depth=4, frac=0.25)
+    boxes = fi.tree_boxes(tree)
+    kind, mass = fi.crop_tree(tree, boxes)
+    ref, cref = oracle.solve_tree(tree.n0, tree.h0, 0.5, kind, mass, True, box=boxes)
+    got, cnt = _run(env, (tree.n0, tree.h0, kind, mass), 0.5, True, box=boxes)
+    assert cnt == {k: cref[k] for k in ("m2l", "p2p", "cross")}
+    e_phi, e_g = _compare_lists(kind, got, ref)
+    assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+    whole, _ = _run(env, tree, 0.5, True, counts=False)
+    for l, b in enumerate(boxes):
+        assert np.array_equal(whole[l][:, b[2]:b[2] + b[5], b[1]:b[1] + b[4], b[0]:b[0] + b[3]], got[l])
+
+
+def test_nine_level_tree(env):
+    """The paper's production depth (9 levels, L684): 16^3 base cells, a 4096^3 lattice at the bottom, every level a box of
+    at most 64 cells per axis around the star -- 1.2 million leaves on eight levels, against the oracle."""
+    boxes, kind, mass = fi.nested_tree(16, 9)
+    ref, cref = oracle.solve_tree(16, 1.0 / 16, 0.5, kind, mass, True, box=boxes)
+    got, cnt = _run(env, (16, 1.0 / 16, kind, mass), 0.5, True, box=boxes)
+    assert cnt == {k: cref[k] for k in ("m2l", "p2p", "cross")}
+    e_phi, e_g = _compare_lists(kind, got, ref)
+    assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+
+
+def test_bad_boxes_are_refused(env):
+    p, torch = env
+    tree = fi.star_tree(32, 3)
+    boxes = fi.tree_boxes(tree)
+    kind, mass = fi.crop_tree(tree, boxes)
+    bad = [list(b) for b in boxes]
+    bad[1][0] += 4                                             # not aligned to the sub-grids
+    with pytest.raises(p.OctoFmmError):
+        p.OctoFMMTree(tree.n0, tree.h0, 0.5, kind, box=bad)
+    bad = [list(b) for b in boxes]
+    bad[2][0] += 8                                             # shifted: the children of a refined sub-grid fall outside / kinds disagree
+    with pytest.raises(p.OctoFmmError):
+        p.OctoFMMTree(tree.n0, tree.h0, 0.5, kind, box=bad)
+    bad = [list(b) for b in boxes]
+    bad[0][3] = 16                                             # level 0 must be the whole lattice
+    with pytest.raises((p.OctoFmmError, ValueError)):
+        p.OctoFMMTree(tree.n0, tree.h0, 0.5, [kind[0][:, :, :16].copy()] + kind[1:], box=bad)
