@@ -359,16 +359,27 @@ def run_tree(args):
     build.build()
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
-    n0 = args.ncell or 64
-    depth = 3
-    tree = fi.star_tree(n0, depth)
-    t = p.OctoFMMTree(tree.n0, tree.h0, args.theta, tree.kind, True, device=local, stream=stream)
-    mass = [torch.from_numpy(m).to(dev) for m in tree.mass]
+    if args.workload == "tree9":
+        # the paper's production depth (9 levels, L684): every level a window of a few sub-grids around one star
+        n0, depth = args.ncell or 16, 9
+        boxes, kinds, masses = fi.nested_tree(n0, depth)
+        h0 = 1.0 / n0
+        what = "9-level tree around one star (windows of <= 64 cells per axis on every level; %d^3 lattice at the bottom)" % (n0 << 8)
+    else:
+        n0, depth = args.ncell or 64, 3
+        dense = fi.star_tree(n0, depth)
+        boxes = fi.tree_boxes(dense)
+        kinds, masses = fi.crop_tree(dense, boxes)
+        h0 = dense.h0
+        what = "two-star field refined around the stars, %d^3 base cells, %d levels (%d^3-equivalent)" % (n0, depth, n0 << (depth - 1))
+        del dense
+    t = p.OctoFMMTree(n0, h0, args.theta, kinds, True, device=local, stream=stream, box=boxes)
+    mass = [torch.from_numpy(m).to(dev) for m in masses]
     out = t.empty_out()
     cnt, _ = t.interaction_counts(mass, out)
     n_int = cnt["m2l"] + cnt["p2p"] + cnt["cross"]
     launches = t.launches()
-    leaves = [int((k == fi.TREE_LEAF).sum()) for k in tree.kind]
+    leaves = [int((k == fi.TREE_LEAF).sum()) for k in kinds]
     for _ in range(max(args.warmup, 3)):
         t.solve(mass, out)
     torch.cuda.synchronize()
@@ -391,28 +402,37 @@ def run_tree(args):
     F = torch.zeros(3, dtype=torch.float64, device=dev)
     Fa = torch.zeros((), dtype=torch.float64, device=dev)
     for l in range(depth):
-        mg = mass[l][None] * out[l][1:4] * torch.from_numpy(tree.kind[l] == fi.TREE_LEAF).to(dev)[None]
+        mg = mass[l][None] * out[l][1:4] * torch.from_numpy(kinds[l] == fi.TREE_LEAF).to(dev)[None]
         F += mg.sum(dim=(1, 2, 3))
         Fa += mg.abs().sum()
     net_force = float(F.abs().max() / Fa)
     # end to end through the host-buffer entry point (pinned host arrays, every level)
     nb = p.octo_fmm_tree_host_scratch_bytes(t.handle)
     scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
-    m_h = [torch.from_numpy(m).pin_memory() for m in tree.mass]
-    o_h = [torch.empty((4,) + (tree.n(l),) * 3, dtype=torch.float64).pin_memory() for l in range(depth)]
+    m_h = [torch.from_numpy(m).pin_memory() for m in masses]
+    o_h = [torch.empty((4,) + t.shape[l], dtype=torch.float64).pin_memory() for l in range(depth)]
     p.octo_fmm_tree_solve_host(t.handle, m_h, o_h, scratch, nb)
     t0 = time.perf_counter()
     for _ in range(max(args.e2e_steps, 1)):
         p.octo_fmm_tree_solve_host(t.handle, m_h, o_h, scratch, nb)
     e2e_ms = 1e3 * (time.perf_counter() - t0) / max(args.e2e_steps, 1)
-    h2d = sum(int(m.numel() * 8) for m, k in zip(m_h, tree.kind) if (k == fi.TREE_LEAF).any())
+    h2d = sum(int(m.numel() * 8) for m, k in zip(m_h, kinds) if (k == fi.TREE_LEAF).any())
     d2h = sum(int(o.numel() * 8) for o in o_h)
     same = all(bool(torch.equal(o_h[l], out[l].cpu())) for l in range(depth))
-    # the oracle's tree solve on the host cores, on the same refinement pattern one octave down (n0 / 2)
-    small = fi.star_tree(max(n0 // 2, 16), depth)
+    # the oracle's tree solve on the host cores: the same tree for the 9-level workload, the same refinement pattern one
+    # octave down (n0 / 2) for the two-star field
     oracle.lib()
+    if args.workload == "tree9":
+        o_n0, o_h0, o_kinds, o_masses, o_boxes = n0, h0, kinds, masses, boxes
+        o_what = "oracle.solve_tree of the same tree"
+    else:
+        small = fi.star_tree(max(n0 // 2, 16), depth)
+        o_boxes = fi.tree_boxes(small)
+        o_kinds, o_masses = fi.crop_tree(small, o_boxes)
+        o_n0, o_h0 = small.n0, small.h0
+        o_what = "oracle.solve_tree of the same pattern at %d^3 base cells" % small.n0
     t0 = time.perf_counter()
-    _, cref = oracle.solve_tree(small.n0, small.h0, args.theta, small.kind, small.mass, True)
+    _, cref = oracle.solve_tree(o_n0, o_h0, args.theta, o_kinds, o_masses, True, box=o_boxes)
     t_ref = time.perf_counter() - t0
     cnt_ref = cref["m2l"] + cref["p2p"] + cref["cross"]
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -422,9 +442,9 @@ def run_tree(args):
     line = {"metric": METRIC, "value": n_int / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "adaptive-tree solve, two-star field refined around the stars, %d^3 base cells, %d levels "
-                                   "(%d^3-equivalent), theta=%g, correction on" % (n0, depth, n0 << (depth - 1), args.theta),
+            "config": {"workload": "adaptive-tree solve, %s, theta=%g, correction on" % (what, args.theta),
                        "interactions_per_step": n_int, "pairs": cnt, "leaf_cells_per_level": leaves,
+                       "boxes": [list(b) for b in boxes],
                        "leaf_cells_per_s": sum(leaves) / (ms * 1e-3),
                        "l2": "arrays of the fine levels larger than L2", "net_force_over_sum_abs_force": net_force,
                        "host_entry_bit_identical": same},
@@ -434,8 +454,7 @@ def run_tree(args):
                          "note": "useful flops only: %d per multipole pair, 8 per point-mass pair; pairs the kernels mask "
                                  "(two leaves in a brick of the multipole step) are executed but not counted" % f_multi},
             "cpu_baseline": {"value": cnt_ref / t_ref, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                             "sample": "oracle.solve_tree of the same pattern at %d^3 base cells (%d interactions) in %.1f s" % (
-                                 small.n0, cnt_ref, t_ref)},
+                             "sample": "%s (%d interactions) in %.1f s" % (o_what, cnt_ref, t_ref)},
             "e2e": {"value": n_int / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms},
             "clocks": clocks, "gpu_launches": launches * args.steps}
@@ -832,7 +851,7 @@ def main():
         run_reference(args)
     elif args.workload == "solve":
         run_solve(args)
-    elif args.workload == "tree":
+    elif args.workload in ("tree", "tree9"):
         run_tree(args)
     elif args.coupled:
         run_coupled(args)
