@@ -23,8 +23,8 @@ namespace octo {
 
 constexpr unsigned char KIND_ABSENT = 0, KIND_LEAF = 1, KIND_REFINED = 2;
 // per sub-grid flags, computed on the host at create()
-constexpr unsigned char NODE_OWN_L = 1;          // leaf sub-grid with a refined sub-grid among its 26 neighbours: its cells have refined
-                                                 // partners in the level's multipole step (tree_leaf_m2l_kernel) and may have refined near-field cells
+constexpr unsigned char NODE_OWN_L = 1;          // leaf sub-grid with a refined sub-grid among its 26 neighbours: its cells take part in
+                                                 // the level's multipole step (refined partners) and may have refined near-field cells
 constexpr unsigned char NODE_COARSE_NBR = 2;     // the parent sub-grid has a LEAF sub-grid among its 26 neighbours one level up
 
 // Moments of the cells that are not refined: a leaf is the point mass at its geometric centre (M0 = m, everything else
@@ -47,70 +47,14 @@ __global__ void __launch_bounds__(256) tree_leaf_moments_kernel(const unsigned c
     for (int c = 0; c < 3; ++c) off[c * ncell + cell] = 0.0;
 }
 
-// The multipole step of the LEAF cells of a level: a leaf A takes the cells of its Eq. 15 list that are REFINED (two leaves
-// meet as point masses in the tensor-core kernel, absent cells are all-zero records), through the general pair formula;
-// being a point mass at its geometric centre it needs only phi = L0 and g = -(L1 + correction) of the result, which are
-// ADDED to out (after the tensor-core kernel has written the leaf-leaf sums).  Only the sub-grids flagged NODE_OWN_L have
-// refined cells within reach, and of their list entries typically a fifth: so instead of running these targets through the
-// brick kernel (every entry evaluated, most of them masked) one WARP takes one cell, the lanes split the list, skip the
-// entries that do not count, and the partial sums are combined by a butterfly of shuffles (the pattern of
-// m2l_warp_kernel).  Block = one sub-grid of `nodes` (8 warps x 64 cells).  Sources: the staged array of the level (kind
-// flag in the padding slot), global memory.
-template <bool CORR>
-__global__ void __launch_bounds__(256) tree_leaf_m2l_kernel(const __grid_constant__ Params p, const int* __restrict__ nodes,
-                                                            double* __restrict__ out)
-{
-    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
-    const int lane = threadIdx.x & 31;
-    const int nnx = p.nx >> 3, nny = p.ny >> 3;
-    const int node = nodes[blockIdx.x];
-    const int x0 = 8 * (node % nnx), y0 = 8 * ((node / nnx) % nny), z0 = 8 * (node / (nnx * nny));
-    const long long plane = (long long)p.ny * p.nx, ncell = plane * p.nz;
-    const double2* S2 = reinterpret_cast<const double2*>(p.S);
-    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
-    const double tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};     // a leaf has no octupole: n3 = M3_B
-    for (int c = warp; c < 512; c += 8) {
-        const int gx = x0 + (c & 7), gy = y0 + ((c >> 3) & 7), k = z0 + (c >> 6);
-        const int cls = (gx & 1) + 2 * (gy & 1) + 4 * (k & 1);
-        Acc acc;
-        acc_zero(acc);
-        const int s_end = c_begin[cls][2 * REACH_MAX + 1];
-#pragma unroll 1
-        for (int s = c_begin[cls][0] + lane; s < s_end; s += 32) {
-            const StEntry e = c_entries[cls * MAX_LIST + s];
-            const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
-            if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
-            if (p.leaf[(long long)sz * plane + (long long)sy * p.nx + sx] != KIND_REFINED) continue;   // a leaf, or nothing there
-            const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
-            double src[16], bx_, by_, bz_;
-            OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
-            const double x = p.hmul[e.dx + REACH_MAX] - bx_;        // the leaf's own offset is zero
-            const double y = p.hmul[e.dy + REACH_MAX] - by_;
-            const double z = p.hmul[e.dz + REACH_MAX] - bz_;
-            if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
-            else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
-        }
-        double v[4] = {acc.l0 + acc.l0b, acc.l1[0] + (CORR ? acc.c[0] : 0.0), acc.l1[1] + (CORR ? acc.c[1] : 0.0),
-                       acc.l1[2] + (CORR ? acc.c[2] : 0.0)};
-#pragma unroll
-        for (int t = 0; t < 4; ++t)
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) v[t] += __shfl_xor_sync(0xffffffffu, v[t], o);
-        if (lane == 0) {
-            const long long cell = (long long)k * plane + (long long)gy * p.nx + gx;
-            out[cell] += v[0];
-#pragma unroll
-            for (int t = 0; t < 3; ++t) out[(1 + t) * ncell + cell] -= v[1 + t];
-        }
-    }
-}
-
 struct TreeFinishArgs {
     int n[3];                       // extents of this level's arrays (a box of its lattice, multiples of 8)
     double h;                       // its cell width
     const unsigned char* kind;      // [nz][ny][nx]
     const unsigned char* nodeflag;  // [(nz/8)][(ny/8)][(nx/8)]
     double* out;                    // [4][cells]: in = leaf-leaf point-mass sums of the tensor-core kernel; out = (phi, g)
+    const double* L;                // this level's finished expansions [20][cells] (correction beside, parent's part included)
+    const double* C;                // [3][cells]
     const double* pL;               // parent level [20][pn cells], pC [3][..], poff [3][..]
     const double* pC;
     const double* poff;
@@ -126,8 +70,9 @@ struct TreeFinishArgs {
 };
 
 // Leaf finish, one thread per cell of the level.  For a leaf A:
-//   phi = [what is in out: leaf-leaf sum + tree_leaf_m2l_kernel's refined partners] + the parent's expansion evaluated at
-//   the leaf centre,  g = [..] - (L1 + correction);
+//   phi = [leaf-leaf sum] + expansion at its centre,  g = [leaf-leaf sum] - (L1 + correction), where the expansion is
+//   this level's own L (sub-grids flagged NODE_OWN_L: Eq. 15 partners that are refined + the parent's shifted expansion,
+//   already added by the fused L2L epilogue) or else the parent's expansion evaluated at the leaf centre;
 //   + the children of the refined cells of its near field (NODE_OWN_L) and the coarser leaves in the near field of its
 //   parent (NODE_COARSE_NBR), as point masses:  x_A - x_b = ((double)(2 i_A - i_b) + 0.5) * (h / 2) per axis, i the
 //   index on the level's own LATTICE (the box shifts drop out of the difference: 2 i_A - i_b = 2 (A - B) - (a,b,c) for
@@ -151,7 +96,11 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
     double v[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) v[c] = a.out[c * ncell + cell];
-    {
+    if (flag & NODE_OWN_L) {
+        v[0] += a.L[cell];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) v[1 + c] -= a.L[(1 + c) * ncell + cell] + a.C[c * ncell + cell];
+    } else {
         const long long P = ((long long)pk * a.pn[1] + pj) * a.pn[0] + pi;
         double Lp[20], sh[20], e[3];
 #pragma unroll

@@ -26,8 +26,7 @@ struct TreeLevel {
     octo_fmm* leaf;             // monopole handle, leaf-level list (null without leaves)
     int* m2l_tiles;  int n_m2l_tiles;     // bricks of the slab-fed kernel that have work
     int* p2p_tiles;  int n_p2p_tiles;     // 16 x 16 x 8 tiles of the tensor-core kernel that hold leaves
-    int* own_nodes;  int n_own_nodes;     // leaf sub-grids with refined cells within reach (NODE_OWN_L), ids in the box's sub-grid lattice
-    std::vector<int> h_m2l_tiles, h_p2p_tiles, h_own_nodes;
+    std::vector<int> h_m2l_tiles, h_p2p_tiles;
     std::vector<unsigned char> h_nodeflag;
     size_t cells() const { return (size_t)n[0] * n[1] * n[2]; }
 };
@@ -94,7 +93,6 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.h = cfg.h0 / (double)(1LL << l);
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
-        L.own_nodes = nullptr; L.n_own_nodes = 0;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
         L.has_refined = L.has_leaf = false;
@@ -151,13 +149,11 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
                                     f |= NODE_COARSE_NBR;
                             }
                     L.h_nodeflag[((size_t)K * nny + J) * nnx + I] = f;
-                    if (f & NODE_OWN_L) L.h_own_nodes.push_back((K * nny + J) * nnx + I);
                 }
-        // the brick kernel takes the REFINED sub-grids (all 20 coefficients, handed down to the children); the leaves next to
-        // them take their refined partners in tree_leaf_m2l_kernel (phi and g only, and only the entries that count)
-        auto node_works = [&](int I, int J, int K) {
+        auto node_works = [&](int I, int J, int K) {   // local sub-grid: its cells take part in the multipole step of this level
             if (I >= nnx || J >= nny || K >= nnz) return false;
-            return node_kind(l, gx0 + I, gy0 + J, gz0 + K) == KIND_REFINED;
+            const unsigned char v = node_kind(l, gx0 + I, gy0 + J, gz0 + K);
+            return v == KIND_REFINED || (v == KIND_LEAF && (L.h_nodeflag[((size_t)K * nny + J) * nnx + I] & NODE_OWN_L));
         };
         // bricks of the slab-fed kernel: 16 x 8 x 3 cells, dense enumeration t = (ty * tiles_x + tx) * tiles_z + tz
         if (L.has_refined) {
@@ -188,11 +184,10 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         }
         L.n_m2l_tiles = (int)L.h_m2l_tiles.size();
         L.n_p2p_tiles = (int)L.h_p2p_tiles.size();
-        L.n_own_nodes = (int)L.h_own_nodes.size();
         // workspace of this level
         const size_t nc = L.cells();
         P.bytes += align_up(nc) + align_up((size_t)nnx * nny * nnz) + align_up(nc * 8);           // kind, nodeflag, lm
-        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4) + align_up((size_t)L.n_own_nodes * 4 + 4);
+        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4);
         if (L.has_refined) {
             octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
             P.bytes += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
@@ -276,9 +271,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         L.lm = (double*)w; w += align_up(nc * 8);
         L.m2l_tiles = (int*)w; w += align_up((size_t)L.n_m2l_tiles * 4 + 4);
         L.p2p_tiles = (int*)w; w += align_up((size_t)L.n_p2p_tiles * 4 + 4);
-        L.own_nodes = (int*)w; w += align_up((size_t)L.n_own_nodes * 4 + 4);
-        if ((L.n_own_nodes && cudaMemcpyAsync(L.own_nodes, L.h_own_nodes.data(), (size_t)L.n_own_nodes * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
-            cudaMemcpyAsync(L.kind, kind_host[l], nc, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+        if (cudaMemcpyAsync(L.kind, kind_host[l], nc, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             cudaMemcpyAsync(L.nodeflag, L.h_nodeflag.data(), nn, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             (L.n_m2l_tiles && cudaMemcpyAsync(L.m2l_tiles, L.h_m2l_tiles.data(), (size_t)L.n_m2l_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
             (L.n_p2p_tiles && cudaMemcpyAsync(L.p2p_tiles, L.h_p2p_tiles.data(), (size_t)L.n_p2p_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)) {
@@ -324,7 +317,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     // the topology arrays were copied from pageable host memory: make sure they have left it before returning
     if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
-    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_own_nodes.clear(); }
+    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); }
     *out = t;
     return OCTO_FMM_OK;
 }
@@ -342,7 +335,6 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             TreeLevel& F = t->lev[l + 1];
             ChildBox cb;
             for (int a = 0; a < 3; ++a) { cb.n[a] = F.n[a]; cb.sh[a] = -2 * F.psh[a]; }
-            cb.pkind = L.kind;
             const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
             if (F.raw) m2m_kernel<false, false, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
             else       m2m_kernel<true, false, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
@@ -417,17 +409,6 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             L.leaf->outL = keep;
             if (rc != OCTO_FMM_OK) return rc;
         }
-        // the leaves next to refined sub-grids: their refined partners of the Eq. 15 list (phi and g, added to out[l])
-        if (L.fmm && L.leaf && L.n_own_nodes > 0 && L.n_m2l_tiles > 0) {
-            BankLock guard(L.fmm);
-            if (bank_acquire(L.fmm) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
-            Params Q = L.fmm->prm;
-            Q.leaf = L.kind;
-            if (L.fmm->cfg.am_correction) tree_leaf_m2l_kernel<true><<<L.n_own_nodes, 256, 0, st>>>(Q, L.own_nodes, out[l]);
-            else                          tree_leaf_m2l_kernel<false><<<L.n_own_nodes, 256, 0, st>>>(Q, L.own_nodes, out[l]);
-            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
-            if (bank_reader_done(L.fmm) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
-        }
         // leaf finish (also zeroes the cells of out[l] that are not leaves); reads the near field from the constant bank
         {
             octo_fmm* hb = L.fmm ? L.fmm : (L.leaf ? L.leaf : t->up[0].fmm);
@@ -437,6 +418,7 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             std::memset(&a, 0, sizeof a);
             for (int c = 0; c < 3; ++c) { a.n[c] = L.n[c]; a.pn[c] = pn[c]; a.psh[c] = L.psh[c]; }
             a.h = L.h; a.kind = L.kind; a.nodeflag = L.nodeflag; a.out = out[l];
+            a.L = L.fmm ? L.fmm->L : nullptr; a.C = L.fmm ? L.fmm->C : nullptr;
             a.pL = pL; a.pC = pC; a.poff = poff;
             if (l + 1 < D) {
                 TreeLevel& F = t->lev[l + 1];
@@ -546,7 +528,6 @@ int octo_fmm_tree_launches(const octo_fmm_tree_t* t, int* launches)
     for (const TreeLevel& l : t->lev) {
         n += 1 + (l.has_refined ? 1 : 0);                                  // leaf moments, M2M
         if (l.fmm && l.n_m2l_tiles > 0) n += 3;                            // stage, flags, multipole step
-        if (l.fmm && l.leaf && l.n_own_nodes > 0 && l.n_m2l_tiles > 0) n += 1;   // leaves next to refined sub-grids
         if (l.leaf) n += 2;                                                // stage, leaf-leaf sums
         n += 1;                                                            // leaf finish
     }
