@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(256) stage_leaf_flags_kernel(const unsigned ch
     const int y = (int)(r % ny), z = (int)(r / ny);
     const long long plane = (long long)ny * nx;
     double2* dst = reinterpret_cast<double2*>(S) + ((long long)z * NPAIR + (NPAIR - 1)) * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1);
-    dst->y = leaf[cell] == 1 ? 1.0 : 0.0;       // mixed level: 0 / 1; tree level: the cell's kind, 1 = leaf
+    dst->y = (double)leaf[cell];                // mixed level: 0 / 1 (1 = leaf); tree level: the cell's kind (0 absent, 1 leaf, 2 refined)
 }
 
 // ------------------------------------------------------------------------------------------
@@ -384,29 +384,50 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         {                                                                                   \
             const StEntry e_ = c_entries[s];                                                \
             ++s;                                                                            \
-            double bx_, by_, bz_, fl_ = 0.0;                                                \
-            if (MODE != MODE_PLAIN) { OCTO_LOAD_SOURCE_F(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
-            else       { OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_); }  \
-            P.x = p.hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                                \
-            P.y = p.hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                                \
-            P.z = Rz0 - bz_;                                                                \
-            P.w = pair_head(P.x, P.y, P.z);                                                 \
-            if (MODE == MODE_MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;             \
-            if (MODE == MODE_TREE && leafA && fl_ != 0.0) P.w = 0.0;                        \
+            bool masked_ = false;                                                           \
+            P.live = true;                                                                  \
+            if (MODE == MODE_TREE) {                                                        \
+                /* the partner's kind first: absent, or a leaf meeting a leaf -> this lane takes nothing; if that holds \
+                   for the whole warp (kinds are constant over sub-grids: the usual case next to a refinement boundary) \
+                   the pair is skipped altogether */                                        \
+                const double kb_ = (sl + e_.off)[9 * SLAB_PLANE].y;                         \
+                masked_ = !present || kb_ == 0.0 || (leafA && kb_ == 1.0);                  \
+                P.live = !__all_sync(0xffffffffu, masked_);                                 \
+            }                                                                               \
+            if (P.live) {                                                                   \
+                double bx_, by_, bz_, fl_ = 0.0;                                            \
+                if (MODE != MODE_PLAIN) { OCTO_LOAD_SOURCE_F(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
+                else       { OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_); }  \
+                P.x = p.hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                            \
+                P.y = p.hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                            \
+                P.z = Rz0 - bz_;                                                            \
+                P.w = pair_head(P.x, P.y, P.z);                                             \
+                if (MODE == MODE_MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;         \
+                if (MODE == MODE_TREE && masked_) P.w = 0.0;                                \
+            }                                                                               \
         }
-        struct Fetched { double src[16]; double x, y, z, w; } A, B;
-        if (ensure()) {
+        struct Fetched { double src[16]; double x, y, z, w; bool live; } A, B;
+#define OCTO_BODY(P) { if (MODE != MODE_TREE || P.live) m2l_pair<CORR, DIPOLE>(acc, P.x, P.y, P.z, P.w, P.src, tA); }
+        if constexpr (MODE == MODE_TREE) {
+            // no hand pipelining here: with whole pairs skipped the two-deep scheme would have to keep both fetched pairs
+            // alive across a branch (it spills 2 KB); three warps per sub-partition cover the head of a pair instead
+            while (ensure()) {
+                OCTO_FETCH(A);
+                OCTO_BODY(A);
+            }
+        } else if (ensure()) {
             OCTO_FETCH(A);
             for (;;) {
                 if (!ensure()) break;
                 OCTO_FETCH(B);
-                m2l_pair<CORR, DIPOLE>(acc, A.x, A.y, A.z, A.w, A.src, tA);
+                OCTO_BODY(A);
                 if (!ensure()) { A = B; break; }
                 OCTO_FETCH(A);
-                m2l_pair<CORR, DIPOLE>(acc, B.x, B.y, B.z, B.w, B.src, tA);
+                OCTO_BODY(B);
             }
-            m2l_pair<CORR, DIPOLE>(acc, A.x, A.y, A.z, A.w, A.src, tA);
+            OCTO_BODY(A);
         }
+#undef OCTO_BODY
 #undef OCTO_FETCH
 
         if (present) store_target<CORR, FUSE_L2L>(p, acc, tA, dA, gx, gy, k);

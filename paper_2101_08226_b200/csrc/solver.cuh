@@ -27,7 +27,8 @@ namespace octo {
 // Child arrays stored as a BOX of their lattice (levels of the adaptive tree): cbox = extents of the child arrays and the
 // (even) shift of the child index, child = 2 * parent + (a,b,c) + sh; children outside the box do not exist (zero mass).
 // The uniform solve passes a null box: the child arrays are exactly twice the parent's.
-struct ChildBox { int n[3]; int sh[3]; };
+struct ChildBox { int n[3]; int sh[3]; const unsigned char* pkind; };   // pkind (may be null): kind of every parent cell; only
+                                                                        // the refined ones (2) are built from children
 
 template <bool LEAF, bool GIVEN = false, bool BOXED = false>
 __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm, const double* __restrict__ coff,
@@ -39,6 +40,7 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
     const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y, K = blockIdx.z;
     if (I >= pnx) return;
     const long long P = ((long long)K * pny + J) * pnx + I;
+    if (BOXED && cb.pkind && cb.pkind[P] != 2) return;      // a leaf or absent parent: tree_leaf_moments_kernel writes it
     const int cnx = BOXED ? cb.n[0] : 2 * pnx, cny = BOXED ? cb.n[1] : 2 * pny, cnz = BOXED ? cb.n[2] : 2 * pnz;
     const long long ccell = (long long)cnx * cny * cnz;
     long long cell[8];

@@ -335,6 +335,7 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             TreeLevel& F = t->lev[l + 1];
             ChildBox cb;
             for (int a = 0; a < 3; ++a) { cb.n[a] = F.n[a]; cb.sh[a] = -2 * F.psh[a]; }
+            cb.pkind = L.kind;
             const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
             if (F.raw) m2m_kernel<false, false, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
             else       m2m_kernel<true, false, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
