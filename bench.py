@@ -362,9 +362,10 @@ def run_tree(args):
     if args.workload == "tree9":
         # the paper's production depth (9 levels, L684): every level a window of a few sub-grids around one star
         n0, depth = args.ncell or 16, 9
-        boxes, kinds, masses = fi.nested_tree(n0, depth)
+        boxes, kinds, masses = fi.nested_tree(n0, depth, reach=2.6)     # 1.8 M leaf cells: the paper's "2 - 8 M cells" (L916)
         h0 = 1.0 / n0
-        what = "9-level tree around one star (windows of <= 64 cells per axis on every level; %d^3 lattice at the bottom)" % (n0 << 8)
+        what = "9-level tree around one star (windows of <= %d cells per axis on every level; %d^3 lattice at the bottom)" % (
+            max(max(b[3:]) for b in boxes[1:]), n0 << 8)
     else:
         n0, depth = args.ncell or 64, 3
         dense = fi.star_tree(n0, depth)
