@@ -131,8 +131,8 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
                 const double m = a.mass_f[((long long)ck * a.fn[1] + cj) * a.fn[0] + ci];
                 const double Rx = ((double)(-2 * d.x - ax) + 0.5) * hf, Ry = ((double)(-2 * d.y - ay) + 0.5) * hf,
                              Rz = ((double)(-2 * d.z - az) + 0.5) * hf;
-                const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = sqrt(r2), w3 = -m / (r2 * r);
-                s[0] += -m / r; s[1] += w3 * Rx; s[2] += w3 * Ry; s[3] += w3 * Rz;
+                const double w = rsqrt_fast(Rx * Rx + Ry * Ry + Rz * Rz), mw = -m * w, w3 = mw * (w * w);   // 1/r to < 1 ulp (m2l_math.cuh)
+                s[0] += mw; s[1] += w3 * Rx; s[2] += w3 * Ry; s[3] += w3 * Rz;
                 ++taken;
             }
         }
@@ -154,8 +154,8 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
             // x_b - x_A = -(x_A - x_b),  2 i_A - i_b = 2 (parent + d) - (2 parent + (a,b,c)) = 2 d - (a,b,c)
             const double Rx = -(((double)(2 * d.x - (i & 1)) + 0.5) * hf), Ry = -(((double)(2 * d.y - (j & 1)) + 0.5) * hf),
                          Rz = -(((double)(2 * d.z - (k & 1)) + 0.5) * hf);
-            const double r2 = Rx * Rx + Ry * Ry + Rz * Rz, r = sqrt(r2), w3 = -m / (r2 * r);
-            s[0] += -m / r; s[1] += w3 * Rx; s[2] += w3 * Ry; s[3] += w3 * Rz;
+            const double w = rsqrt_fast(Rx * Rx + Ry * Ry + Rz * Rz), mw = -m * w, w3 = mw * (w * w);
+            s[0] += mw; s[1] += w3 * Rx; s[2] += w3 * Ry; s[3] += w3 * Rz;
             ++taken;
         }
 #pragma unroll

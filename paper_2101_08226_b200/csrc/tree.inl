@@ -158,16 +158,27 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         // bricks of the slab-fed kernel: 16 x 8 x 3 cells, dense enumeration t = (ty * tiles_x + tx) * tiles_z + tz
         if (L.has_refined) {
             const int tx_n = (L.n[0] + TILE_X - 1) / TILE_X, ty_n = (L.n[1] + TILE_Y - 1) / TILE_Y, tz_n = (L.n[2] + TILE_Z - 1) / TILE_Z;
+            std::vector<std::pair<double, int>> weighted;
             for (int ty = 0; ty < ty_n; ++ty)
                 for (int tx = 0; tx < tx_n; ++tx)
                     for (int tz = 0; tz < tz_n; ++tz) {
-                        bool work = false;
+                        // estimated work of the brick: its cells in refined sub-grids count fully, those in leaf sub-grids next
+                        // to refined ones about a fifth (most of their list entries are skipped)
+                        double weight = 0.0;
                         const int z0 = tz * TILE_Z, z1 = std::min(z0 + TILE_Z, L.n[2]) - 1;
-                        for (int K = z0 / 8; K <= z1 / 8 && !work; ++K)
-                            for (int I = (tx * TILE_X) / 8; I <= std::min(tx * TILE_X + TILE_X - 1, L.n[0] - 1) / 8 && !work; ++I)
-                                work = node_works(I, (ty * TILE_Y) / 8, K);
-                        if (work) L.h_m2l_tiles.push_back((ty * tx_n + tx) * tz_n + tz);
+                        for (int K = z0 / 8; K <= z1 / 8; ++K)
+                            for (int I = (tx * TILE_X) / 8; I <= std::min(tx * TILE_X + TILE_X - 1, L.n[0] - 1) / 8; ++I) {
+                                if (!node_works(I, (ty * TILE_Y) / 8, K)) continue;
+                                const int layers = std::min(z1, 8 * K + 7) - std::max(z0, 8 * K) + 1;
+                                const bool refined = node_kind(l, gx0 + I, gy0 + (ty * TILE_Y) / 8, gz0 + K) == KIND_REFINED;
+                                weight += (refined ? 1.0 : 0.2) * 64.0 * layers;
+                            }
+                        if (weight > 0.0) weighted.push_back(std::make_pair(-weight, (ty * tx_n + tx) * tz_n + tz));
                     }
+            // heaviest bricks first: the persistent CTAs take the list round-robin, so that every CTA gets its share of the
+            // bricks that are full of refined cells instead of whoever comes first in lattice order getting three of them
+            std::sort(weighted.begin(), weighted.end());
+            for (const auto& wt : weighted) L.h_m2l_tiles.push_back(wt.second);
         }
         // tiles of the tensor-core leaf kernel: 16 x 16 x 8 cells, b = (tz * by + ty) * bx + tx
         if (L.has_leaf) {
