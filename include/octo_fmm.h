@@ -27,8 +27,8 @@
  *
  * Memory and ownership: every pointer marked "device" is device memory on cfg.device owned by
  * the caller; the library never allocates or frees device memory (the caller lends it a
- * workspace) and never synchronises the stream except in octo_fmm_destroy and
- * octo_fmm_status.  All work is enqueued on cfg.stream (a cudaStream_t).  Inputs may be reused
+ * workspace) and never synchronises the stream except in octo_fmm_destroy, octo_fmm_status, the
+ * counters that read a device word, the *_host entry points and (MONOPOLE handles, tree) create.  All work is enqueued on cfg.stream (a cudaStream_t).  Inputs may be reused
  * by the caller once the stream has passed set_moments; outputs are complete once the stream
  * has passed get_expansions.  One handle is not thread-safe; DIFFERENT handles may be driven from
  * different streams and host threads at the same time.  Everything that depends on a handle's cell
@@ -74,8 +74,10 @@ typedef struct {
 size_t octo_fmm_workspace_bytes(const octo_fmm_config *cfg);
 
 /* Builds the 8 per-parity interaction lists from Eq. 15 (L131-135) on the host and the TMA
- * descriptors of the workspace; no device allocation.  EINVAL: bad sizes / theta / NULL /
- * workspace too small or misaligned.  ECUDA: no usable device. */
+ * descriptors of the workspace; no device allocation.  MONOPOLE handles also upload the tables of
+ * the tensor-core kernel (weights of the 11^3 offsets, operand fragments) into the workspace and
+ * synchronise cfg.stream once for it (the tables come from pageable host memory).  EINVAL: bad sizes
+ * / theta / NULL / workspace too small or misaligned.  ECUDA: no usable device. */
 int octo_fmm_create(const octo_fmm_config *cfg, octo_fmm_t **out);
 
 /* Stage the sources: re-lays the caller's moments into the workspace

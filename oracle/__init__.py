@@ -541,3 +541,65 @@ def solve_tree(n0, h0, theta, kind, mass, am_correction=True, coarsest=2, box=No
         out[l][0] += np.where(leaf, L[0], 0.0)
         out[l][1:4] -= np.where(leaf[None], L[1:4] + corr, 0.0)
     return out, counts
+
+
+# ---- the five calls of the boundary on host arrays: one harness drives the oracle and the library -------
+class _OracleConfig(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int * 3), ("out_lo", ctypes.c_int * 3), ("out_hi", ctypes.c_int * 3), ("h", ctypes.c_double),
+                ("theta", ctypes.c_double), ("kind", ctypes.c_int), ("am_correction", ctypes.c_int)]
+
+
+class Oracle:
+    """The oracle behind the call sequence of the library's boundary -- create / set_moments / interact / get_expansions /
+    destroy (`fmm_oracle_*` in fmm_oracle.c) -- with the method names of paper_2101_08226_b200.OctoFMM, on numpy arrays."""
+    MULTIPOLE, MONOPOLE = 0, 1
+
+    def __init__(self, n, h, theta, kind=0, am_correction=True, out_lo=(0, 0, 0), out_hi=(0, 0, 0)):
+        L = lib()
+        L.fmm_oracle_create.argtypes = [ctypes.POINTER(_OracleConfig), ctypes.POINTER(ctypes.c_void_p)]
+        dp = ctypes.POINTER(ctypes.c_double)
+        L.fmm_oracle_set_moments.argtypes = [ctypes.c_void_p, dp, dp]
+        L.fmm_oracle_interact.argtypes = [ctypes.c_void_p]
+        L.fmm_oracle_get_expansions.argtypes = [ctypes.c_void_p, dp, dp]
+        L.fmm_oracle_destroy.argtypes = [ctypes.c_void_p]
+        L.fmm_oracle_handle_interaction_count.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_ulonglong)]
+        c = _OracleConfig()
+        for a in range(3):
+            c.n[a], c.out_lo[a], c.out_hi[a] = int(n[a]), int(out_lo[a]), int(out_hi[a])
+        c.h, c.theta, c.kind, c.am_correction = float(h), float(theta), int(kind), int(bool(am_correction))
+        self.kind, self.n = int(kind), tuple(int(v) for v in n)
+        whole = all(v == 0 for v in tuple(out_lo) + tuple(out_hi))
+        lo, hi = ((0, 0, 0), self.n) if whole else (tuple(out_lo), tuple(out_hi))
+        self.out_shape = (hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0])
+        self.handle = ctypes.c_void_p()
+        _check(L.fmm_oracle_create(ctypes.byref(c), ctypes.byref(self.handle)), "create")
+
+    def set_moments(self, moments, com_off=None):
+        moments = np.ascontiguousarray(moments, dtype=np.float64)
+        com = None if com_off is None else np.ascontiguousarray(com_off, dtype=np.float64)
+        _check(lib().fmm_oracle_set_moments(self.handle, _dp(moments), None if com is None else _dp(com)), "set_moments")
+
+    def interact(self):
+        _check(lib().fmm_oracle_interact(self.handle), "interact")
+
+    def get_expansions(self):
+        Lo = np.zeros(((20 if self.kind == 0 else 4),) + self.out_shape)
+        Lc = np.zeros((3,) + self.out_shape) if self.kind == 0 else None
+        _check(lib().fmm_oracle_get_expansions(self.handle, _dp(Lo), None if Lc is None else _dp(Lc)), "get_expansions")
+        return Lo, Lc
+
+    def interaction_count(self):
+        n = ctypes.c_ulonglong(0)
+        _check(lib().fmm_oracle_handle_interaction_count(self.handle, ctypes.byref(n)), "interaction_count")
+        return int(n.value)
+
+    def close(self):
+        if self.handle:
+            lib().fmm_oracle_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -875,3 +875,106 @@ int fmm_oracle_direct_sum_points(long np, const double *pos, const double *mass,
     }
     return ORC_OK;
 }
+
+/* ====================================================================================== */
+/* The five calls of the boundary on HOST pointers, under this file's own     */
+/* prefix, so that one harness can drive the oracle and the library alike:                  */
+/*   fmm_oracle_create / set_moments / interact / get_expansions / destroy.                 */
+/* Thin state around the functions above: set_moments copies the caller's arrays, interact  */
+/* calls fmm_oracle_interact_multipole or fmm_oracle_interact_monopole on the copy.         */
+/* ====================================================================================== */
+typedef struct {
+    int n[3];
+    int out_lo[3], out_hi[3];   /* all zero: the whole grid */
+    double h, theta;
+    int kind;                   /* 0 multipole, 1 monopole */
+    int am_correction;
+} fmm_oracle_config;
+
+typedef struct fmm_oracle_handle {
+    fmm_oracle_config cfg;
+    int lo[3], hi[3];
+    size_t ncell, ocell;
+    double *mom, *com, *L, *C;
+    unsigned long long count;
+    int state;                  /* 0 created, 1 sources set, 2 interacted */
+} fmm_oracle_t;
+
+int fmm_oracle_destroy(fmm_oracle_t *o)
+{
+    if (!o) return ORC_EINVAL;
+    free(o->mom); free(o->com); free(o->L); free(o->C);
+    free(o);
+    return ORC_OK;
+}
+
+int fmm_oracle_create(const fmm_oracle_config *cfg, fmm_oracle_t **out)
+{
+    if (!cfg || !out) return ORC_EINVAL;
+    *out = NULL;
+    if (cfg->kind != 0 && cfg->kind != 1) return ORC_EINVAL;
+    if (!(cfg->h > 0.0) || !(cfg->theta > 1.0 / 3.0 && cfg->theta < 1.0)) return ORC_EINVAL;
+    fmm_oracle_t *o = (fmm_oracle_t *)calloc(1, sizeof *o);
+    if (!o) return ORC_EINVAL;
+    o->cfg = *cfg;
+    int whole = 1;
+    for (int a = 0; a < 3; ++a) whole = whole && cfg->out_lo[a] == 0 && cfg->out_hi[a] == 0;
+    for (int a = 0; a < 3; ++a) {
+        o->lo[a] = whole ? 0 : cfg->out_lo[a];
+        o->hi[a] = whole ? cfg->n[a] : cfg->out_hi[a];
+    }
+    if (!check_region(cfg->n, o->lo, o->hi)) { free(o); return ORC_EINVAL; }
+    o->ncell = (size_t)cfg->n[0] * cfg->n[1] * cfg->n[2];
+    o->ocell = (size_t)(o->hi[0] - o->lo[0]) * (o->hi[1] - o->lo[1]) * (o->hi[2] - o->lo[2]);
+    const size_t nm = cfg->kind == 0 ? 20 : 1, nl = cfg->kind == 0 ? 20 : 4;
+    o->mom = (double *)malloc(nm * o->ncell * sizeof(double));
+    o->com = (double *)calloc(3 * o->ncell, sizeof(double));
+    o->L = (double *)malloc(nl * o->ocell * sizeof(double));
+    o->C = (double *)calloc(3 * o->ocell, sizeof(double));
+    if (!o->mom || !o->com || !o->L || !o->C) { fmm_oracle_destroy(o); return ORC_EINVAL; }
+    *out = o;
+    return ORC_OK;
+}
+
+int fmm_oracle_set_moments(fmm_oracle_t *o, const double *moments, const double *com_off)
+{
+    if (!o || !moments) return ORC_EINVAL;
+    memcpy(o->mom, moments, (o->cfg.kind == 0 ? 20 : 1) * o->ncell * sizeof(double));
+    if (com_off) memcpy(o->com, com_off, 3 * o->ncell * sizeof(double));
+    else memset(o->com, 0, 3 * o->ncell * sizeof(double));
+    o->state = 1;
+    return ORC_OK;
+}
+
+int fmm_oracle_interact(fmm_oracle_t *o)
+{
+    if (!o) return ORC_EINVAL;
+    if (o->state < 1) return ORC_EMASS + 1;        /* "state" error, distinct from EINVAL / EMASS */
+    int rc;
+    if (o->cfg.kind == 0)
+        rc = fmm_oracle_interact_multipole(o->cfg.n, o->lo, o->hi, o->cfg.h, o->cfg.theta, o->cfg.am_correction, o->mom, o->com,
+                                           o->L, o->C, &o->count);
+    else
+        rc = fmm_oracle_interact_monopole(o->cfg.n, o->lo, o->hi, o->cfg.h, o->cfg.theta, o->mom, o->L, &o->count);
+    if (rc == ORC_OK || rc == ORC_EMASS) o->state = 2;
+    return rc;
+}
+
+int fmm_oracle_get_expansions(fmm_oracle_t *o, double *L, double *Lcorr)
+{
+    if (!o || !L) return ORC_EINVAL;
+    if (o->state < 2) return ORC_EMASS + 1;
+    memcpy(L, o->L, (o->cfg.kind == 0 ? 20 : 4) * o->ocell * sizeof(double));
+    if (Lcorr) {
+        if (o->cfg.kind != 0) return ORC_EINVAL;
+        memcpy(Lcorr, o->C, 3 * o->ocell * sizeof(double));
+    }
+    return ORC_OK;
+}
+
+int fmm_oracle_handle_interaction_count(const fmm_oracle_t *o, unsigned long long *n)
+{
+    if (!o || !n || o->state < 2) return ORC_EINVAL;
+    *n = o->count;
+    return ORC_OK;
+}

@@ -842,3 +842,59 @@ def test_monopole_host_entry_point_in_chunks_of_z_tiles(env, n, chunk):
         assert np.array_equal(o_h.numpy(), ref.cpu().numpy())
         o_h.fill_(float("nan"))
     f.close()
+
+
+@pytest.mark.parametrize("correction", [True, False])
+def test_mixed_level_kernels_agree_with_each_other(env, correction):
+    """octo_fmm_interact_mixed has two implementations (the slab-fed kernel over the leaf-level lists; the Eq. 15 step
+    followed by m2l_near_kernel): the same pairs with the same dipole decision, so they agree to round-off -- on sources
+    WITHOUT dipole moments (device-checked path without the dipole terms in both) and WITH them."""
+    p, torch = env
+    w, leaf = _mixed_level(43, 32)
+    lf = torch.from_numpy(leaf).cuda()
+    for with_dipoles in (False, True):
+        mom = w.moments.copy()
+        if with_dipoles:
+            mom[1:4] = np.random.default_rng(7).normal(size=mom[1:4].shape) * mom[0] * w.h * 0.05 * (leaf == 0)
+        res = []
+        for kernel in (0, 1, 2):
+            f = p.OctoFMM(w.n, w.h, 0.5, p.MULTIPOLE, correction)
+            f.set_option("kernel", kernel)
+            f.set_moments(torch.from_numpy(mom).cuda(), torch.from_numpy(w.com_off).cuda())
+            f.interact_mixed(lf)
+            L, Lc = f.get_expansions()
+            torch.cuda.synchronize()
+            assert f.status() == p.OK and f.dipole_terms_used() == with_dipoles
+            res.append((L.cpu().numpy(), Lc.cpu().numpy()))
+            f.close()
+        for L, Lc in res[1:]:
+            assert parity_error(L, res[0][0]) < 1e-13
+            assert np.abs(Lc - res[0][1]).max() <= 1e-13 * max(np.abs(res[0][0][1:4]).max(), 1e-300)
+
+
+def _five_calls(make, moments, com_off):
+    """ONE harness for both implementations: create -> set_moments -> interact -> get_expansions -> destroy."""
+    obj = make()
+    obj.set_moments(moments, com_off)
+    obj.interact()
+    L, Lc = obj.get_expansions()
+    cnt = obj.interaction_count()
+    obj.close()
+    return L, Lc, cnt
+
+
+@pytest.mark.parametrize("kind", ["multipole", "monopole"])
+def test_one_harness_drives_the_oracle_and_the_library(env, kind):
+    p, torch = env
+    w = fi.config2(ncell=32)
+    region = dict(out_lo=(8, 8, 0), out_hi=(24, 32, 16))
+    if kind == "multipole":
+        a = _five_calls(lambda: oracle.Oracle(w.n, w.h, 0.5, oracle.Oracle.MULTIPOLE, True, **region), w.moments, w.com_off)
+        b = _five_calls(lambda: p.OctoFMM(w.n, w.h, 0.5, p.MULTIPOLE, True, **region),
+                        torch.from_numpy(w.moments).cuda(), torch.from_numpy(w.com_off).cuda())
+        assert a[2] == b[2]
+        check(b[0].cpu().numpy(), b[1].cpu().numpy(), a[0], a[1])
+    else:
+        a = _five_calls(lambda: oracle.Oracle(w.n, w.h, 0.5, oracle.Oracle.MONOPOLE, **region), w.moments[:1], None)
+        b = _five_calls(lambda: p.OctoFMM(w.n, w.h, 0.5, p.MONOPOLE, **region), torch.from_numpy(w.moments[:1].copy()).cuda(), None)
+        assert a[2] == b[2] and parity_error(b[0].cpu().numpy(), a[0]) < TOL

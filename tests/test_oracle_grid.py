@@ -213,3 +213,30 @@ def test_condition_output_is_the_sum_of_absolute_terms():
             tot[20:] += np.abs(c)
         got = La[:, k - 4, j - 4, i - 4]
         assert np.abs(got - tot).max() <= 1e-13 * tot.max()
+
+
+def test_the_five_calls_of_the_boundary_on_the_oracle():
+    """the oracle behind create / set_moments / interact / get_expansions / destroy gives what its plain
+    entry points give (bit for bit), for both kinds, whole grid and a sub-region; interact before set_moments and
+    get_expansions before interact are refused."""
+    w = fi.config1(seed=11, ncell=16)
+    for lo, hi in (((0, 0, 0), (0, 0, 0)), ((8, 0, 8), (16, 8, 16))):
+        o = oracle.Oracle(w.n, w.h, 0.5, oracle.Oracle.MULTIPOLE, True, lo, hi)
+        with pytest.raises(RuntimeError):
+            o.interact()
+        o.set_moments(w.moments, w.com_off)
+        with pytest.raises(RuntimeError):
+            o.get_expansions()
+        o.interact()
+        L, Lc = o.get_expansions()
+        rlo, rhi = (None, None) if hi == (0, 0, 0) else (lo, hi)
+        Lr, Lcr, cnt = oracle.interact_multipole(w.n, w.h, 0.5, w.moments, w.com_off, rlo, rhi, True)
+        assert np.array_equal(L, Lr) and np.array_equal(Lc, Lcr) and o.interaction_count() == cnt
+        o.close()
+    m = oracle.Oracle(w.n, w.h, 0.35, oracle.Oracle.MONOPOLE)
+    m.set_moments(w.moments[:1])
+    m.interact()
+    out, none = m.get_expansions()
+    ref, cnt = oracle.interact_monopole(w.n, w.h, 0.35, w.moments[0])
+    assert none is None and np.array_equal(out, ref) and m.interaction_count() == cnt
+    m.close()
