@@ -517,6 +517,10 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         cudaError_t e6 = cudaFuncSetAttribute(m2l_staged_kernel<false, false, MODE_MIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e7 = cudaFuncSetAttribute(m2l_staged_kernel<true, true, MODE_TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e8 = cudaFuncSetAttribute(m2l_staged_kernel<false, true, MODE_TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
+        if (cudaFuncSetAttribute(m2l_staged_kernel<true, false, MODE_TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM) != cudaSuccess ||
+            cudaFuncSetAttribute(m2l_staged_kernel<false, false, MODE_TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM) != cudaSuccess) {
+            delete h; return OCTO_FMM_ECUDA;
+        }
         if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess || e5 != cudaSuccess || e6 != cudaSuccess ||
             e7 != cudaSuccess || e8 != cudaSuccess) {
             delete h; return OCTO_FMM_ECUDA;
@@ -664,11 +668,18 @@ static int launch_staged(octo_fmm_t* h, int kb, int ke, bool mixed = false)
     if (h->tile_list) { P.tile_list = h->tile_list; P.ntiles = h->tile_count; }     // whole-grid launches only (tree levels)
     const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
     if (grid == 0) return OCTO_FMM_OK;
-    if (h->tree_kind) {    // a level of the adaptive tree: absent cells, leaf-leaf pairs left to the leaf kernel, parent's expansion fused in
-        if (!P.pL) return OCTO_FMM_ESTATE;
+    if (h->tree_kind) {    // a level of the adaptive tree: absent cells, leaf-leaf pairs left to the leaf kernel
         P.leaf = h->tree_kind;
-        if (h->cfg.am_correction) m2l_staged_kernel<true, true, MODE_TREE><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-        else                      m2l_staged_kernel<false, true, MODE_TREE><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        // one brick per CTA, heaviest first: the levels of a tree run side by side on streams of their own, and the block
+        // scheduler packs their bricks onto the SMs as they come free (the ring fill per brick is 3 % of a full brick)
+        const int tgrid = (int)P.ntiles;
+        if (P.pL) {        // the parent's expansion added in the epilogue (levels one after the other)
+            if (h->cfg.am_correction) m2l_staged_kernel<true, true, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+            else                      m2l_staged_kernel<false, true, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        } else {
+            if (h->cfg.am_correction) m2l_staged_kernel<true, false, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+            else                      m2l_staged_kernel<false, false, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        }
     } else if (mixed) {    // one level of an adaptive mesh: leaf-level lists, near-field entries conditional on the leaf flags
         if (h->cfg.am_correction) m2l_staged_kernel<true, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
         else                      m2l_staged_kernel<false, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);

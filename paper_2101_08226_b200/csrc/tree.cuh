@@ -47,14 +47,55 @@ __global__ void __launch_bounds__(256) tree_leaf_moments_kernel(const unsigned c
     for (int c = 0; c < 3; ++c) off[c * ncell + cell] = 0.0;
 }
 
+// L2L on a tree level stored as a box: what the fused epilogue of the brick kernel does when the levels run one after the
+// other, as a pass of its own so that the multipole steps of ALL levels can run side by side and only this cheap chain is
+// sequential.  For every existing cell: the correction is taken out of L1 and carried beside it, the parent's expansion,
+// Taylor-shifted to the cell's expansion centre, and the parent's correction are added.
+//   parent index = (index >> 1) + psh;   e = ((a,b,c) - 1/2) h + delta - delta_P
+struct TreeL2LArgs {
+    int n[3], pn[3], psh[3];
+    double h;
+    const unsigned char* kind;
+    double* L; double* C; const double* off;             // this level: [20], [3], [3] x cells
+    const double* pL; const double* pC; const double* poff;
+};
+
+__global__ void __launch_bounds__(128) tree_l2l_kernel(const TreeL2LArgs a)
+{
+    const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    if (i >= nx) return;
+    const long long ncell = (long long)nx * ny * nz, cell = ((long long)k * ny + j) * nx + i;
+    if (a.kind[cell] != KIND_REFINED) return;             // leaves take the parent's expansion in the leaf finish
+    const long long pcell = (long long)a.pn[0] * a.pn[1] * a.pn[2];
+    const long long P = ((long long)((k >> 1) + a.psh[2]) * a.pn[1] + ((j >> 1) + a.psh[1])) * a.pn[0] + ((i >> 1) + a.psh[0]);
+    double e[3], Lp[20], sh[20], C[3];
+    e[0] = ((double)(i & 1) - 0.5) * a.h + a.off[cell] - a.poff[P];
+    e[1] = ((double)(j & 1) - 0.5) * a.h + a.off[ncell + cell] - a.poff[pcell + P];
+    e[2] = ((double)(k & 1) - 0.5) * a.h + a.off[2 * ncell + cell] - a.poff[2 * pcell + P];
+#pragma unroll
+    for (int t = 0; t < 20; ++t) Lp[t] = a.pL[t * pcell + P];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) C[c] = a.C[c * ncell + cell];
+    taylor_shift<3>(Lp, e, sh);
+#pragma unroll
+    for (int t = 0; t < 20; ++t) {
+        double v = a.L[t * ncell + cell];
+        if (t >= 1 && t <= 3) v -= C[t - 1];
+        a.L[t * ncell + cell] = v + sh[t];
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) a.C[c * ncell + cell] = C[c] + a.pC[c * pcell + P];
+}
+
 struct TreeFinishArgs {
     int n[3];                       // extents of this level's arrays (a box of its lattice, multiples of 8)
     double h;                       // its cell width
     const unsigned char* kind;      // [nz][ny][nx]
     const unsigned char* nodeflag;  // [(nz/8)][(ny/8)][(nx/8)]
     double* out;                    // [4][cells]: in = leaf-leaf point-mass sums of the tensor-core kernel; out = (phi, g)
-    const double* L;                // this level's finished expansions [20][cells] (correction beside, parent's part included)
-    const double* C;                // [3][cells]
+    const double* L;                // this level's own multipole step [20][cells], as stored by the brick kernel (correction
+                                    // folded into L1); read at the leaves of sub-grids flagged NODE_OWN_L only
     const double* pL;               // parent level [20][pn cells], pC [3][..], poff [3][..]
     const double* pC;
     const double* poff;
@@ -71,8 +112,8 @@ struct TreeFinishArgs {
 
 // Leaf finish, one thread per cell of the level.  For a leaf A:
 //   phi = [leaf-leaf sum] + expansion at its centre,  g = [leaf-leaf sum] - (L1 + correction), where the expansion is
-//   this level's own L (sub-grids flagged NODE_OWN_L: Eq. 15 partners that are refined + the parent's shifted expansion,
-//   already added by the fused L2L epilogue) or else the parent's expansion evaluated at the leaf centre;
+//   the parent's, evaluated at the leaf centre, plus -- in sub-grids flagged NODE_OWN_L -- this level's own multipole step
+//   (the refined cells of the Eq. 15 list);
 //   + the children of the refined cells of its near field (NODE_OWN_L) and the coarser leaves in the near field of its
 //   parent (NODE_COARSE_NBR), as point masses:  x_A - x_b = ((double)(2 i_A - i_b) + 0.5) * (h / 2) per axis, i the
 //   index on the level's own LATTICE (the box shifts drop out of the difference: 2 i_A - i_b = 2 (A - B) - (a,b,c) for
@@ -97,10 +138,13 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
 #pragma unroll
     for (int c = 0; c < 4; ++c) v[c] = a.out[c * ncell + cell];
     if (flag & NODE_OWN_L) {
+        // this level's own multipole step (refined partners of the Eq. 15 list), as the brick kernel stored it: the
+        // correction folded into L1
         v[0] += a.L[cell];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) v[1 + c] -= a.L[(1 + c) * ncell + cell] + a.C[c * ncell + cell];
-    } else {
+        for (int c = 0; c < 3; ++c) v[1 + c] -= a.L[(1 + c) * ncell + cell];
+    }
+    {
         const long long P = ((long long)pk * a.pn[1] + pj) * a.pn[0] + pi;
         double Lp[20], sh[20], e[3];
 #pragma unroll

@@ -28,6 +28,10 @@ struct TreeLevel {
     int* p2p_tiles;  int n_p2p_tiles;     // 16 x 16 x 8 tiles of the tensor-core kernel that hold leaves
     std::vector<int> h_m2l_tiles, h_p2p_tiles;
     std::vector<unsigned char> h_nodeflag;
+    // the multipole step and the leaf-leaf sums of a level depend on the upward pass only: they run on streams of their
+    // own, side by side with those of the other levels; the L2L / leaf-finish chain on the caller's stream waits for them
+    cudaStream_t s_m2l, s_leaf;
+    cudaEvent_t ev_m2l, ev_leaf;
     size_t cells() const { return (size_t)n[0] * n[1] * n[2]; }
 };
 
@@ -93,6 +97,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.h = cfg.h0 / (double)(1LL << l);
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
+        L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
         L.has_refined = L.has_leaf = false;
@@ -229,6 +234,7 @@ struct octo_fmm_tree {
     std::vector<SolverLevel> up;       // uniform levels n0/2, ..., 2
     unsigned long long* counts;        // device [3]: m2l, p2p, cross
     cudaStream_t stream;
+    cudaEvent_t ev_up;                 // the upward pass of a solve is complete
     bool solved;
 };
 
@@ -251,6 +257,13 @@ int octo_fmm_tree_destroy(octo_fmm_tree_t* t)
     }
     for (SolverLevel& l : t->up)
         if (l.fmm && octo_fmm_destroy(l.fmm) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
+    for (TreeLevel& l : t->lev) {
+        if (l.s_m2l) cudaStreamDestroy(l.s_m2l);
+        if (l.s_leaf) cudaStreamDestroy(l.s_leaf);
+        if (l.ev_m2l) cudaEventDestroy(l.ev_m2l);
+        if (l.ev_leaf) cudaEventDestroy(l.ev_leaf);
+    }
+    if (t->ev_up) cudaEventDestroy(t->ev_up);
     delete t;
     return rc;
 }
@@ -269,6 +282,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     t->cfg = *cfg;
     t->stream = (cudaStream_t)cfg->stream;
     t->solved = false;
+    t->ev_up = nullptr;
     t->lev = std::move(P.lev);
     const octo_fmm_solver_config sc = as_solver_config(*cfg);
     char* w = (char*)cfg->workspace;
@@ -289,8 +303,13 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
             rc = OCTO_FMM_ECUDA;
             break;
         }
+        if (cudaStreamCreateWithFlags(&L.s_m2l, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&L.s_leaf, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&L.ev_m2l, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&L.ev_leaf, cudaEventDisableTiming) != cudaSuccess) { rc = OCTO_FMM_ECUDA; break; }
         if (L.has_refined) {
             octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
+            mc.stream = L.s_m2l;
             mc.workspace = w; mc.workspace_bytes = sizes_of(mc, CF_ANY_SIZE).total; w += mc.workspace_bytes;
             L.raw = (double*)w; w += align_up(nc * 20 * 8);
             L.off = (double*)w; w += align_up(nc * 3 * 8);
@@ -303,6 +322,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         }
         if (L.has_leaf) {
             octo_fmm_config lc = box_config(sc, L.n, L.h, OCTO_FMM_MONOPOLE);
+            lc.stream = L.s_leaf;
             lc.workspace = w; lc.workspace_bytes = sizes_of(lc, CF_LEAF_LIST).total; w += lc.workspace_bytes;
             rc = create_internal(&lc, CF_LEAF_LIST, &L.leaf);
             if (rc != OCTO_FMM_OK) break;
@@ -325,6 +345,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         t->up.push_back(l);
     }
     t->counts = (unsigned long long*)w;
+    if (rc == OCTO_FMM_OK && cudaEventCreateWithFlags(&t->ev_up, cudaEventDisableTiming) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     // the topology arrays were copied from pageable host memory: make sure they have left it before returning
     if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
@@ -354,7 +375,33 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
-    // ---- the uniform levels above level 0 (the whole lattice): up ... ----
+    // ---- side by side, each level on streams of its own: staging + multipole step (its own level only; the parent's
+    //      expansion comes in the chain below), and the leaf-leaf point-mass sums ----
+    if (cudaEventRecord(t->ev_up, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    for (int l = 0; l < D; ++l) {
+        TreeLevel& L = t->lev[l];
+        if (L.fmm && L.n_m2l_tiles > 0) {
+            if (cudaStreamWaitEvent(L.s_m2l, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+            if ((rc = octo_fmm_set_moments(L.fmm, L.raw, L.off)) != OCTO_FMM_OK) return rc;
+            const long long nc = (long long)L.cells();
+            stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_m2l>>>(L.kind, L.fmm->src, L.n[0], L.n[1], L.n[2]);
+            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+            clear_parent(L.fmm);
+            if ((rc = octo_fmm_interact(L.fmm)) != OCTO_FMM_OK) return rc;
+            if (cudaEventRecord(L.ev_m2l, L.s_m2l) != cudaSuccess) return OCTO_FMM_ECUDA;
+        }
+        if (L.leaf) {
+            if (cudaStreamWaitEvent(L.s_leaf, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+            if ((rc = octo_fmm_set_moments(L.leaf, L.lm, nullptr)) != OCTO_FMM_OK) return rc;
+            double* const keep = L.leaf->outL;
+            L.leaf->outL = out[l];
+            rc = octo_fmm_interact(L.leaf);
+            L.leaf->outL = keep;
+            if (rc != OCTO_FMM_OK) return rc;
+            if (cudaEventRecord(L.ev_leaf, L.s_leaf) != cudaSuccess) return OCTO_FMM_ECUDA;
+        }
+    }
+    // ---- meanwhile on the caller's stream: the uniform levels above level 0 (the whole lattice), up ... ----
     for (size_t lv = 0; lv < t->up.size(); ++lv) {
         SolverLevel& l = t->up[lv];
         const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
@@ -387,7 +434,8 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     if (count && cudaMemsetAsync(t->counts, 0, 3 * sizeof(unsigned long long), st) != cudaSuccess) return OCTO_FMM_ECUDA;
-    // ---- tree levels, coarsest first ----
+    // ---- the chain on the caller's stream, coarsest level first: L2L into the refined cells, then the leaf finish ----
+    octo_fmm* const hb = t->up[0].fmm;      // a multipole handle on the caller's stream: the bank's book-keeping for the chain
     for (int l = 0; l < D; ++l) {
         TreeLevel& L = t->lev[l];
         // parent arrays of this level: the tree level above, or the finest uniform level
@@ -401,36 +449,25 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             pL = t->up[0].fmm->L; pC = t->up[0].fmm->C; poff = t->up[0].off;
         }
         if (!pL && (L.has_refined || L.has_leaf)) return OCTO_FMM_ESTATE;
+        const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
         if (L.fmm && L.n_m2l_tiles > 0) {
-            if ((rc = octo_fmm_set_moments(L.fmm, L.raw, L.off)) != OCTO_FMM_OK) return rc;
-            const long long nc = (long long)L.cells();
-            stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, L.fmm->src, L.n[0], L.n[1], L.n[2]);
+            if (cudaStreamWaitEvent(st, L.ev_m2l, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+            TreeL2LArgs q;
+            for (int c = 0; c < 3; ++c) { q.n[c] = L.n[c]; q.pn[c] = pn[c]; q.psh[c] = L.psh[c]; }
+            q.h = L.h; q.kind = L.kind; q.L = L.fmm->L; q.C = L.fmm->C; q.off = L.off; q.pL = pL; q.pC = pC; q.poff = poff;
+            tree_l2l_kernel<<<blocks, 128, 0, st>>>(q);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
-            Params& Q = L.fmm->prm;
-            Q.pL = pL; Q.pC = pC; Q.poff = poff;
-            for (int a = 0; a < 3; ++a) { Q.pdim[a] = pn[a]; Q.psh[a] = L.psh[a]; }
-            rc = octo_fmm_interact(L.fmm);
-            clear_parent(L.fmm);
-            if (rc != OCTO_FMM_OK) return rc;
         }
-        if (L.leaf) {
-            if ((rc = octo_fmm_set_moments(L.leaf, L.lm, nullptr)) != OCTO_FMM_OK) return rc;
-            double* const keep = L.leaf->outL;
-            L.leaf->outL = out[l];
-            rc = octo_fmm_interact(L.leaf);
-            L.leaf->outL = keep;
-            if (rc != OCTO_FMM_OK) return rc;
-        }
+        if (L.leaf && cudaStreamWaitEvent(st, L.ev_leaf, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
         // leaf finish (also zeroes the cells of out[l] that are not leaves); reads the near field from the constant bank
         {
-            octo_fmm* hb = L.fmm ? L.fmm : (L.leaf ? L.leaf : t->up[0].fmm);
             BankLock guard(hb);
             if (bank_acquire(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
             TreeFinishArgs a;
             std::memset(&a, 0, sizeof a);
             for (int c = 0; c < 3; ++c) { a.n[c] = L.n[c]; a.pn[c] = pn[c]; a.psh[c] = L.psh[c]; }
             a.h = L.h; a.kind = L.kind; a.nodeflag = L.nodeflag; a.out = out[l];
-            a.L = L.fmm ? L.fmm->L : nullptr; a.C = L.fmm ? L.fmm->C : nullptr;
+            a.L = L.fmm ? L.fmm->L : nullptr;
             a.pL = pL; a.pC = pC; a.poff = poff;
             if (l + 1 < D) {
                 TreeLevel& F = t->lev[l + 1];
@@ -439,19 +476,12 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             }
             if (l > 0) { a.kind_c = t->lev[l - 1].kind; a.mass_c = t->lev[l - 1].lm; }
             a.count = count ? t->counts : nullptr;
-            const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
             tree_leaf_finish_kernel<<<blocks, 128, 0, st>>>(a);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
-            if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
-        }
-        if (count) {
-            // the Eq. 15 list with its (dx, dy, dz) is the multipole flavour of the bank: any multipole handle brings it
-            octo_fmm* hb = L.fmm ? L.fmm : t->up[0].fmm;
-            BankLock guard(hb);
-            if (bank_acquire(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
-            const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
-            tree_count_kernel<<<blocks, 128, 0, st>>>(L.kind, L.n[0], L.n[1], L.n[2], t->counts);
-            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+            if (count) {
+                tree_count_kernel<<<blocks, 128, 0, st>>>(L.kind, L.n[0], L.n[1], L.n[2], t->counts);
+                if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+            }
             if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
         }
     }
@@ -539,7 +569,7 @@ int octo_fmm_tree_launches(const octo_fmm_tree_t* t, int* launches)
     int n = 0;
     for (const TreeLevel& l : t->lev) {
         n += 1 + (l.has_refined ? 1 : 0);                                  // leaf moments, M2M
-        if (l.fmm && l.n_m2l_tiles > 0) n += 3;                            // stage, flags, multipole step
+        if (l.fmm && l.n_m2l_tiles > 0) n += 4;                            // stage, flags, multipole step, L2L
         if (l.leaf) n += 2;                                                // stage, leaf-leaf sums
         n += 1;                                                            // leaf finish
     }
