@@ -191,3 +191,47 @@ def test_bad_boxes_are_refused(env):
     bad[0][3] = 16                                             # level 0 must be the whole lattice
     with pytest.raises((p.OctoFmmError, ValueError)):
         p.OctoFMMTree(tree.n0, tree.h0, 0.5, [kind[0][:, :, :16].copy()] + kind[1:], box=bad)
+
+
+@pytest.mark.parametrize("theta,correction", [(0.35, True), (0.7, False)])
+def test_boxes_at_other_opening_angles(env, theta, correction):
+    """Boxes + the widest (reach 5) and the narrowest lists, correction on and off."""
+    tree = fi.star_tree(32, 3)
+    boxes = fi.tree_boxes(tree)
+    kind, mass = fi.crop_tree(tree, boxes)
+    ref, cref = oracle.solve_tree(tree.n0, tree.h0, theta, kind, mass, correction, box=boxes)
+    got, cnt = _run(env, (tree.n0, tree.h0, kind, mass), theta, correction, box=boxes)
+    assert cnt == {k: cref[k] for k in ("m2l", "p2p", "cross")}
+    e_phi, e_g = _compare_lists(kind, got, ref)
+    assert e_phi < TOL and e_g < TOL, (e_phi, e_g)
+
+
+def test_repeated_and_concurrent_solves_are_deterministic(env):
+    """The levels of a solve run side by side on streams of the library's own; two trees are driven from two caller
+    streams at the same time, several solves each without host synchronisation in between: every solve of a tree gives
+    bit-identical results, equal to a solve run alone."""
+    p, torch = env
+    trees = [fi.seeded_tree(1), fi.seeded_tree(2, depth=4, frac=0.3)]
+    alone = []
+    for tr in trees:
+        got, _ = _run(env, tr, 0.5, True, counts=False)
+        alone.append(got)
+    streams = [torch.cuda.Stream() for _ in trees]
+    handles, masses, outs = [], [], []
+    for tr, st in zip(trees, streams):
+        h = p.OctoFMMTree(tr.n0, tr.h0, 0.5, tr.kind, True, stream=st)
+        with torch.cuda.stream(st):
+            masses.append([torch.from_numpy(m).cuda() for m in tr.mass])
+        outs.append([h.empty_out() for _ in range(3)])
+        handles.append(h)
+    torch.cuda.synchronize()
+    for rnd in range(3):
+        for i in (0, 1):
+            handles[i].solve(masses[i], outs[i][rnd])
+    torch.cuda.synchronize()
+    for i, tr in enumerate(trees):
+        assert handles[i].status() == p.OK
+        for rnd in range(3):
+            for l in range(tr.depth):
+                assert np.array_equal(outs[i][rnd][l].cpu().numpy(), alone[i][l])
+        handles[i].close()
