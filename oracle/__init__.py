@@ -603,3 +603,81 @@ class Oracle:
             self.close()
         except Exception:
             pass
+
+
+def solve_tree_rhs2(n0, h0, theta, kind, mass, dmass, coarsest=2, box=None):
+    """Second right-hand side on the adaptive tree (Alg. 1: "Compute g, phi, and d(phi)/dt using
+    the FMM"): the tree, lists and EXPANSION CENTRES of solve_tree(.., mass) -- the centres of mass of `mass` -- with the
+    signed point sources dmass[l] at the leaf centres, no angular-momentum correction (readings R6, R7 of solve_rhs2, on
+    the tree of R9).  Same arguments as solve_tree.  Returns out[l] = [4] + shape of level l = (d(phi)/dt, -grad of it)
+    at the leaf cells."""
+    D = len(kind)
+    n0 = int(n0)
+    if box is None:
+        box = [(0, 0, 0) + (n0 << l,) * 3 for l in range(D)]
+    box = [tuple(int(v) for v in b) for b in box]
+    shp = [(b[5], b[4], b[3]) for b in box]
+    kind = [np.ascontiguousarray(k, dtype=np.uint8) for k in kind]
+    mass = [np.ascontiguousarray(np.where(k == 1, m, 0.0), dtype=np.float64) for k, m in zip(kind, mass)]
+    dmass = [np.ascontiguousarray(np.where(k == 1, m, 0.0), dtype=np.float64) for k, m in zip(kind, dmass)]
+    hs = [float(h0) / (1 << l) for l in range(D)]
+    cframe = [tuple(2 * v for v in b) for b in box]
+    # ---- upward: the density fixes the centres; d(rho)/dt is expanded about them ----
+    mom, mom2, off = [None] * D, [None] * D, [None] * D
+    for l in range(D - 1, -1, -1):
+        m = np.zeros((20,) + shp[l]); m[0] = mass[l]
+        m2 = np.zeros((20,) + shp[l]); m2[0] = dmass[l]
+        o = np.zeros((3,) + shp[l])
+        if l < D - 1:
+            f = cframe[l]
+            cm, co = _embed(mom[l + 1], box[l + 1], f), _embed(off[l + 1], box[l + 1], f)
+            pm, po = m2m((f[3], f[4], f[5]), hs[l + 1], cm, co)
+            ref = kind[l] == 2
+            o = np.where(ref[None], po, o)
+            pm2 = m2m_about((f[3], f[4], f[5]), hs[l + 1], _embed(mom2[l + 1], box[l + 1], f), co, np.ascontiguousarray(o))
+            m = np.where(ref[None], pm, m)
+            m2 = np.where(ref[None], pm2, m2)
+        mom[l], mom2[l], off[l] = np.ascontiguousarray(m), np.ascontiguousarray(m2), np.ascontiguousarray(o)
+    up_n, up_h, up_m, up_m2, up_o = [n0], [hs[0]], [mom[0]], [mom2[0]], [off[0]]
+    while up_n[-1] > coarsest:
+        nc, hc = up_n[-1], up_h[-1]
+        pm, po = m2m((nc, nc, nc), hc, up_m[-1], up_o[-1])
+        pm2 = m2m_about((nc, nc, nc), hc, up_m2[-1], up_o[-1], po)
+        up_n.append(nc // 2); up_h.append(2.0 * hc); up_m.append(pm); up_m2.append(pm2); up_o.append(po)
+    # ---- downward: the uniform levels, then the tree levels; no correction ----
+    L_par = off_par = None
+    for lv in range(len(up_n) - 1, 0, -1):
+        nl, hl = up_n[lv], up_h[lv]
+        L, Lc, _ = interact_multipole((nl, nl, nl), hl, theta, up_m2[lv], up_o[lv], None, None, False)
+        L = L.copy()
+        if L_par is not None:
+            l2l((nl, nl, nl), hl, L_par, np.zeros((3,) + L_par.shape[1:]), off_par, up_o[lv], L, np.zeros_like(Lc))
+        L_par, off_par = L, up_o[lv]
+    out, exp = [None] * D, [None] * D
+    for l in range(D):
+        n3, h = (box[l][3], box[l][4], box[l][5]), hs[l]
+        L, Lc, _ = tree_interact_multipole(n3, h, theta, mom2[l], off[l], kind[l], False)
+        L = L.copy()
+        if L_par is not None:
+            zp = np.zeros((3,) + L_par.shape[1:])
+            if l == 0:
+                l2l(n3, h, L_par, zp, off_par, off[l], L, np.zeros_like(Lc))
+            else:
+                f = cframe[l - 1]
+                Le = _embed(L, box[l], f)
+                l2l((f[3], f[4], f[5]), h, L_par, zp, off_par, _embed(off[l], box[l], f), Le, np.zeros((3,) + Le.shape[1:]))
+                L = _extract(Le, f, box[l])
+        out[l], _ = tree_leaf_p2p(n3, h, theta, kind[l], dmass[l])
+        L_par, off_par = L, off[l]
+        exp[l] = L
+    for l in range(D - 1):
+        f = cframe[l]
+        of = _embed(out[l + 1], box[l + 1], f)
+        tree_cross_level((box[l][3], box[l][4], box[l][5]), hs[l], theta, kind[l], dmass[l], _embed(kind[l + 1], box[l + 1], f),
+                         _embed(dmass[l + 1], box[l + 1], f), out[l], of)
+        out[l + 1] = _extract(of, f, box[l + 1])
+    for l in range(D):
+        leaf = kind[l] == 1
+        out[l][0] += np.where(leaf, exp[l][0], 0.0)
+        out[l][1:4] -= np.where(leaf[None], exp[l][1:4], 0.0)
+    return out

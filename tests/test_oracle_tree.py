@@ -306,3 +306,48 @@ def test_nine_level_tree_in_boxes():
     phi = -(ms[None, :] / np.sqrt(r2)).sum(1)
     e = np.abs(res[pick, 0] - phi) / np.abs(phi)
     assert e.max() < 3 * 2.66e-2 and np.median(e) < 1.5e-3 and e.mean() < 6e-3
+
+
+def test_second_right_hand_side_on_the_tree():
+    """oracle.solve_tree_rhs2 (L81-83 on the adaptive mesh): d(mass)/dt = alpha * mass gives alpha x the solve without the
+    correction, leaf by leaf to round-off (the centres are the density's); linear in the sources; a fully refined tree is
+    oracle.solve_rhs2 bit for bit; with levels stored as boxes the same numbers bit for bit; against the exact signed point
+    sum within the truncation level."""
+    tree = fi.seeded_tree(6, n0=8, depth=3, frac=0.5)
+    assert (tree.kind[1] == LEAF).any() and (tree.kind[2] == LEAF).any()
+    alpha = -0.37
+    base, _ = oracle.solve_tree(tree.n0, tree.h0, 0.5, tree.kind, tree.mass, False)
+    got = oracle.solve_tree_rhs2(tree.n0, tree.h0, 0.5, tree.kind, tree.mass, [alpha * m for m in tree.mass])
+    for l in range(tree.depth):
+        leaf = tree.kind[l] == LEAF
+        if leaf.any():
+            assert np.abs(got[l] - alpha * base[l])[:, leaf].max() <= 2e-15 * np.abs(base[l])[:, leaf].max()
+    rng = np.random.default_rng(2)
+    d1 = [rng.normal(size=m.shape) * m for m in tree.mass]
+    d2 = [rng.normal(size=m.shape) * m for m in tree.mass]
+    a = oracle.solve_tree_rhs2(tree.n0, tree.h0, 0.5, tree.kind, tree.mass, d1)
+    b = oracle.solve_tree_rhs2(tree.n0, tree.h0, 0.5, tree.kind, tree.mass, d2)
+    c = oracle.solve_tree_rhs2(tree.n0, tree.h0, 0.5, tree.kind, tree.mass, [x + 2.0 * y for x, y in zip(d1, d2)])
+    for l in range(tree.depth):
+        assert np.abs(c[l] - (a[l] + 2.0 * b[l])).max() <= 1e-12 * max(np.abs(c[l]).max(), 1e-300)
+    # boxes
+    boxes = fi.tree_boxes(tree)
+    kind, mass = fi.crop_tree(tree, boxes)
+    dcrop = [np.ascontiguousarray(x[bx[2]:bx[2] + bx[5], bx[1]:bx[1] + bx[4], bx[0]:bx[0] + bx[3]]) for x, bx in zip(d1, boxes)]
+    ab = oracle.solve_tree_rhs2(tree.n0, tree.h0, 0.5, kind, mass, dcrop, box=boxes)
+    for l, bx in enumerate(boxes):
+        assert np.array_equal(a[l][:, bx[2]:bx[2] + bx[5], bx[1]:bx[1] + bx[4], bx[0]:bx[0] + bx[3]], ab[l])
+    # exact signed point sum
+    pos, ms, lv, idx = tree.leaf_points()
+    dm = np.concatenate([d1[l][tree.kind[l] == LEAF] for l in range(tree.depth)])
+    res = np.concatenate([a[l][0][tree.kind[l] == LEAF] for l in range(tree.depth)])
+    ex = oracle.direct_sum_points(pos, dm)[:, 0]
+    scale = np.abs(oracle.direct_sum_points(pos, np.abs(dm))[:, 0])         # signed random sources cancel: the size of what is summed
+    assert (np.abs(res - ex) / scale).max() < 1e-3
+    # fully refined: the uniform second right-hand side
+    n, h = 16, 1.0 / 16
+    m = rng.uniform(0.5, 1.5, (n, n, n)) * h ** 3
+    dm = rng.normal(size=(n, n, n)) * h ** 3
+    k2 = [np.full((8,) * 3, REFINED, np.uint8), np.full((16,) * 3, LEAF, np.uint8)]
+    full = oracle.solve_tree_rhs2(8, 1.0 / 8, 0.5, k2, [np.zeros((8,) * 3), m], [np.zeros((8,) * 3), dm])
+    assert np.array_equal(full[1], oracle.solve_rhs2(n, h, 0.5, m, dm))
