@@ -318,6 +318,12 @@ int octo_fmm_tree_create(const octo_fmm_tree_config *cfg, const unsigned char *c
                          octo_fmm_tree_t **out);
 /* Asynchronous on the stream. */
 int octo_fmm_tree_solve(octo_fmm_tree_t *t, const double *const *mass, double *const *out);
+/* Second right-hand side on the tree (L81-83, Alg. 1): dmass[l] DEVICE [box cells], the time derivative of the leaf
+ * masses (any sign); dphi_dt[l] DEVICE [box cells]: the potential of these sources at the leaf cells, zeros elsewhere
+ * (only the potential of this solve is used, Eq. 3).  Same tree, lists and EXPANSION CENTRES as the last
+ * octo_fmm_tree_solve on this handle (ESTATE if there was none), no angular-momentum correction.  Overwrites the
+ * per-level results of solve().  Asynchronous on the stream. */
+int octo_fmm_tree_solve_rhs2(octo_fmm_tree_t *t, const double *const *dmass, double *const *dphi_dt);
 /* The same solve, and the ordered pairs it evaluates, counted on the device for the bit-exact check of the pair set:
  * counts[0] multipole pairs of all levels (uniform levels included), counts[1] leaf-leaf point-mass pairs of one
  * level, counts[2] point-mass pairs across a refinement boundary.  Synchronises the stream. */

@@ -92,6 +92,7 @@ class _Library:
         lib.octo_fmm_tree_workspace_bytes.argtypes = [tcfgp, vpp, ip]
         lib.octo_fmm_tree_create.argtypes = [tcfgp, vpp, ip, ctypes.POINTER(vp)]
         lib.octo_fmm_tree_solve.argtypes = [vp, vpp, vpp]
+        lib.octo_fmm_tree_solve_rhs2.argtypes = [vp, vpp, vpp]
         lib.octo_fmm_tree_interaction_counts.argtypes = [vp, vpp, vpp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_tree_host_scratch_bytes.restype = ctypes.c_size_t
         lib.octo_fmm_tree_host_scratch_bytes.argtypes = [vp]
@@ -570,6 +571,12 @@ def octo_fmm_tree_solve(t, mass, out):
         raise OctoFmmError("octo_fmm_tree_solve", rc)
 
 
+def octo_fmm_tree_solve_rhs2(t, dmass, dphi_dt):
+    rc = _lib.octo_fmm_tree_solve_rhs2(t, _ptr_array(dmass), _ptr_array(dphi_dt))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_tree_solve_rhs2", rc)
+
+
 def octo_fmm_tree_interaction_counts(t, mass, out):
     c = (ctypes.c_ulonglong * 3)()
     rc = _lib.octo_fmm_tree_interaction_counts(t, _ptr_array(mass), _ptr_array(out), c)
@@ -655,6 +662,18 @@ class OctoFMMTree:
         self._check(mass, out)
         octo_fmm_tree_solve(self.handle, mass, out)
         return out
+
+    def solve_rhs2(self, dmass, dphi_dt=None):
+        """d(phi)/dt per level ([box shape]) of the sources dmass on the tree and centres of the last solve()."""
+        if dphi_dt is None:
+            dphi_dt = [self.torch.empty(self.shape[l], dtype=self.torch.float64, device=self.device) for l in range(self.depth)]
+        if len(dmass) != self.depth or len(dphi_dt) != self.depth:
+            raise ValueError("octo_fmm: one dmass and one dphi_dt tensor per level")
+        for l in range(self.depth):
+            _check_device_tensor(dmass[l], "dmass[%d]" % l, self.torch.float64, self.cells(l), self.device, self.stream)
+            _check_device_tensor(dphi_dt[l], "dphi_dt[%d]" % l, self.torch.float64, self.cells(l), self.device, self.stream)
+        octo_fmm_tree_solve_rhs2(self.handle, dmass, dphi_dt)
+        return dphi_dt
 
     def interaction_counts(self, mass, out=None):
         out = self.empty_out() if out is None else out

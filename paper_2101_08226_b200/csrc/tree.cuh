@@ -108,6 +108,8 @@ struct TreeFinishArgs {
     const unsigned char* kind_c;    // level above (= the parent arrays' level), or null: [pn cells]
     const double* mass_c;
     unsigned long long* count;      // null, or counts[2] += cross-level pairs taken (ordered)
+    double* phi_only;               // null, or (second right-hand side) [cells]: only the potential is wanted; out is then
+                                    // read (the leaf-leaf sums) but not written
 };
 
 // Leaf finish, one thread per cell of the level.  For a leaf A:
@@ -127,6 +129,7 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
     const long long ncell = (long long)nx * ny * nz;
     const long long cell = ((long long)k * ny + j) * nx + i;
     if (a.kind[cell] != KIND_LEAF) {
+        if (a.phi_only) { a.phi_only[cell] = 0.0; return; }
 #pragma unroll
         for (int c = 0; c < 4; ++c) a.out[c * ncell + cell] = 0.0;
         return;
@@ -205,8 +208,12 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
 #pragma unroll
         for (int c = 0; c < 4; ++c) v[c] += s[c];
     }
+    if (a.phi_only) {
+        a.phi_only[cell] = v[0];
+    } else {
 #pragma unroll
-    for (int c = 0; c < 4; ++c) a.out[c * ncell + cell] = v[c];
+        for (int c = 0; c < 4; ++c) a.out[c * ncell + cell] = v[c];
+    }
     if (a.count && taken) atomicAdd(a.count + 2, taken);
 }
 

@@ -354,11 +354,28 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     return OCTO_FMM_OK;
 }
 
-static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double* const* out, bool count)
+// rhs2 (second right-hand side, L81-83): the sources are d(mass)/dt, expanded about the centres the last solve left in the
+// off arrays (M2M with GIVEN centres), no correction; out[l] is then [cells]: the potential only.
+static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double* const* out, bool count, bool rhs2 = false)
 {
     const int D = (int)t->lev.size();
     cudaStream_t st = t->stream;
     int rc;
+    // the level handles run without the correction for the second right-hand side (it belongs to the force, L127)
+    struct CorrGuard {
+        octo_fmm_tree_t* t; bool on; std::vector<int> keep;
+        CorrGuard(octo_fmm_tree_t* t_, bool on_) : t(t_), on(on_) {
+            if (!on) return;
+            for (TreeLevel& l : t->lev) { keep.push_back(l.fmm ? l.fmm->cfg.am_correction : 0); if (l.fmm) l.fmm->cfg.am_correction = 0; }
+            for (SolverLevel& l : t->up) { keep.push_back(l.fmm->cfg.am_correction); l.fmm->cfg.am_correction = 0; }
+        }
+        ~CorrGuard() {
+            if (!on) return;
+            size_t i = 0;
+            for (TreeLevel& l : t->lev) { if (l.fmm) l.fmm->cfg.am_correction = keep[i]; ++i; }
+            for (SolverLevel& l : t->up) l.fmm->cfg.am_correction = keep[i++];
+        }
+    } corr_guard(t, rhs2);
     // ---- upward pass: finest level first ----
     for (int l = D - 1; l >= 0; --l) {
         TreeLevel& L = t->lev[l];
@@ -369,9 +386,15 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             for (int a = 0; a < 3; ++a) { cb.n[a] = F.n[a]; cb.sh[a] = -2 * F.psh[a]; }
             cb.pkind = L.kind;
             const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
-            if (F.raw) m2m_kernel<false, false, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
-            else       m2m_kernel<true, false, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
+            if (rhs2) {
+                if (F.raw) m2m_kernel<false, true, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
+                else       m2m_kernel<true, true, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
+            } else {
+                if (F.raw) m2m_kernel<false, false, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
+                else       m2m_kernel<true, false, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
+            }
         }
+        // (the offsets of the cells that are not refined are zero for both right-hand sides: rewriting them is harmless)
         tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
@@ -394,7 +417,7 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             if (cudaStreamWaitEvent(L.s_leaf, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
             if ((rc = octo_fmm_set_moments(L.leaf, L.lm, nullptr)) != OCTO_FMM_OK) return rc;
             double* const keep = L.leaf->outL;
-            L.leaf->outL = out[l];
+            if (!rhs2) L.leaf->outL = out[l];          // second right-hand side: the four sums go to the handle's own buffer
             rc = octo_fmm_interact(L.leaf);
             L.leaf->outL = keep;
             if (rc != OCTO_FMM_OK) return rc;
@@ -407,8 +430,15 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
         if (lv == 0) {
             TreeLevel& B = t->lev[0];
-            if (B.raw) m2m_kernel<false><<<blocks, 128, 0, st>>>(B.raw, B.off, l.raw, l.off, l.n, l.n, l.n, B.h);
-            else       m2m_kernel<true><<<blocks, 128, 0, st>>>(B.lm, nullptr, l.raw, l.off, l.n, l.n, l.n, B.h);
+            if (rhs2) {
+                if (B.raw) m2m_kernel<false, true><<<blocks, 128, 0, st>>>(B.raw, B.off, l.raw, l.off, l.n, l.n, l.n, B.h);
+                else       m2m_kernel<true, true><<<blocks, 128, 0, st>>>(B.lm, nullptr, l.raw, l.off, l.n, l.n, l.n, B.h);
+            } else {
+                if (B.raw) m2m_kernel<false><<<blocks, 128, 0, st>>>(B.raw, B.off, l.raw, l.off, l.n, l.n, l.n, B.h);
+                else       m2m_kernel<true><<<blocks, 128, 0, st>>>(B.lm, nullptr, l.raw, l.off, l.n, l.n, l.n, B.h);
+            }
+        } else if (rhs2) {
+            m2m_kernel<false, true><<<blocks, 128, 0, st>>>(t->up[lv - 1].raw, t->up[lv - 1].off, l.raw, l.off, l.n, l.n, l.n, t->up[lv - 1].h);
         } else {
             m2m_kernel<false><<<blocks, 128, 0, st>>>(t->up[lv - 1].raw, t->up[lv - 1].off, l.raw, l.off, l.n, l.n, l.n, t->up[lv - 1].h);
         }
@@ -466,7 +496,9 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             TreeFinishArgs a;
             std::memset(&a, 0, sizeof a);
             for (int c = 0; c < 3; ++c) { a.n[c] = L.n[c]; a.pn[c] = pn[c]; a.psh[c] = L.psh[c]; }
-            a.h = L.h; a.kind = L.kind; a.nodeflag = L.nodeflag; a.out = out[l];
+            a.h = L.h; a.kind = L.kind; a.nodeflag = L.nodeflag;
+            a.out = rhs2 ? (L.leaf ? L.leaf->L : nullptr) : out[l];
+            a.phi_only = rhs2 ? out[l] : nullptr;
             a.L = L.fmm ? L.fmm->L : nullptr;
             a.pL = pL; a.pC = pC; a.poff = poff;
             if (l + 1 < D) {
@@ -485,8 +517,18 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
         }
     }
-    t->solved = true;
+    if (!rhs2) t->solved = true;
     return OCTO_FMM_OK;
+}
+
+int octo_fmm_tree_solve_rhs2(octo_fmm_tree_t* t, const double* const* dmass, double* const* dphi_dt)
+{
+    if (!t || !dmass || !dphi_dt) return OCTO_FMM_EINVAL;
+    for (size_t l = 0; l < t->lev.size(); ++l)
+        if (!dmass[l] || !dphi_dt[l] || ((uintptr_t)dmass[l] % 16) || ((uintptr_t)dphi_dt[l] % 16)) return OCTO_FMM_EINVAL;
+    if (!t->solved) return OCTO_FMM_ESTATE;          // the centres are the density's: solve() first
+    if (cudaSetDevice(t->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    return tree_solve_impl(t, dmass, dphi_dt, false, true);
 }
 
 int octo_fmm_tree_solve(octo_fmm_tree_t* t, const double* const* mass, double* const* out)

@@ -235,3 +235,40 @@ def test_repeated_and_concurrent_solves_are_deterministic(env):
             for l in range(tr.depth):
                 assert np.array_equal(outs[i][rnd][l].cpu().numpy(), alone[i][l])
         handles[i].close()
+
+
+@pytest.mark.parametrize("boxed", [False, True])
+def test_second_right_hand_side_on_the_tree(env, boxed):
+    """octo_fmm_tree_solve_rhs2 (L81-83 on the adaptive mesh): d(phi)/dt of signed sources on the tree and centres of the
+    density's solve, against oracle.solve_tree_rhs2 at 1e-12 of the largest value; the density's solve is unchanged by it
+    (bit-identical before and after); ESTATE before the first solve."""
+    p, torch = env
+    tree = fi.star_tree(32, 3) if boxed else fi.seeded_tree(2)
+    rng = np.random.default_rng(8)
+    dm = [rng.normal(size=m.shape) * m for m in tree.mass]
+    if boxed:
+        boxes = fi.tree_boxes(tree)
+        kind, mass = fi.crop_tree(tree, boxes)
+        dm = [np.ascontiguousarray(x[b[2]:b[2] + b[5], b[1]:b[1] + b[4], b[0]:b[0] + b[3]]) for x, b in zip(dm, boxes)]
+    else:
+        boxes, kind, mass = None, tree.kind, tree.mass
+    ref = oracle.solve_tree_rhs2(tree.n0, tree.h0, 0.5, kind, mass, dm, box=boxes)
+    t = p.OctoFMMTree(tree.n0, tree.h0, 0.5, kind, True, box=boxes)
+    m_d = [torch.from_numpy(m).cuda() for m in mass]
+    d_d = [torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in dm]
+    with pytest.raises(p.OctoFmmError):
+        t.solve_rhs2(d_d)
+    before = [o.clone() for o in t.solve(m_d)]
+    got = t.solve_rhs2(d_d)
+    after = t.solve(m_d)
+    torch.cuda.synchronize()
+    assert t.status() == p.OK
+    scale = max(np.abs(r[0]).max() for r in ref)
+    for l in range(tree.depth):
+        leaf = kind[l] == fi.TREE_LEAF
+        g = got[l].cpu().numpy()
+        assert np.all(g[~leaf] == 0.0)
+        if leaf.any():
+            assert np.abs(g - ref[l][0])[leaf].max() < TOL * scale
+        assert torch.equal(before[l], after[l])
+    t.close()
