@@ -407,6 +407,20 @@ def run_tree(args):
         F += mg.sum(dim=(1, 2, 3))
         Fa += mg.abs().sum()
     net_force = float(F.abs().max() / Fa)
+    # the second right-hand side (L81-83) on the same tree and centres, timed beside the solve (not part of `value`)
+    dm = [m * (2.0 * torch.rand(m.shape, dtype=torch.float64, device=dev, generator=torch.Generator(device=dev).manual_seed(7 + l)) - 1.0)
+          for l, m in enumerate(mass)]
+    dphi = t.solve_rhs2(dm)
+    torch.cuda.synchronize()
+    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev2.record(stream)
+    for _ in range(args.steps):
+        t.solve_rhs2(dm, dphi)
+    ev3.record(stream)
+    torch.cuda.synchronize()
+    rhs2_ms = ev2.elapsed_time(ev3) / args.steps
+    t.solve(mass, out)
+    torch.cuda.synchronize()
     # end to end through the host-buffer entry point (pinned host arrays, every level)
     nb = p.octo_fmm_tree_host_scratch_bytes(t.handle)
     scratch = torch.empty(nb, dtype=torch.uint8, device=dev)
@@ -458,6 +472,8 @@ def run_tree(args):
                              "sample": "%s (%d interactions) in %.1f s" % (o_what, cnt_ref, t_ref)},
             "e2e": {"value": n_int / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": e2e_ms},
+            "second_rhs": {"ms_per_solve": rhs2_ms, "note": "octo_fmm_tree_solve_rhs2: d(phi)/dt from d(mass)/dt on the same tree "
+                                                            "and centres, correction off, dipole terms on; not part of value"},
             "clocks": clocks, "gpu_launches": launches * args.steps}
     print(json.dumps(line))
     t.close()
