@@ -499,14 +499,21 @@ def run_coupled(args):
     if world > 1:
         dist.barrier()
     import paper_2101_08226_b200 as p
-    from paper_2101_08226_b200.sharded import HALO, ShardedLevel
+    from paper_2101_08226_b200.sharded import HALO, PeerShardedLevel, ShardedLevel
     w = make_workload(args.workload, args.theta, args.ncell, args.seed + rank)     # rank r's slab of the tall domain
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
-    lvl = ShardedLevel(w.n, w.h, args.theta, True, rank=rank, world=world, device=local, stream=stream)
+    peer = args.halo == "peer"
+    if peer:       # no exchange: the kernel reads the neighbours' staged layers through peer memory (CUDA IPC)
+        lvl = PeerShardedLevel(w.n, w.h, args.theta, True, rank=rank, world=world, device=local, stream=stream)
+        own_m = torch.from_numpy(w.moments).to(dev)
+        own_c = torch.from_numpy(w.com_off).to(dev)
+    else:
+        lvl = ShardedLevel(w.n, w.h, args.theta, True, rank=rank, world=world, device=local, stream=stream)
+        own_m, own_c = lvl.moments, lvl.com_off
+        own_m.copy_(torch.from_numpy(w.moments))               # the producer writes into the owned views, once
+        own_c.copy_(torch.from_numpy(w.com_off))
     lvl.fmm.set_option("dipole_terms", 1)
-    lvl.moments.copy_(torch.from_numpy(w.moments))             # the producer writes into the owned views, once
-    lvl.com_off.copy_(torch.from_numpy(w.com_off))
     L = torch.empty((20,) + lvl.fmm.out_shape, dtype=torch.float64, device=dev)
     Lc = torch.empty((3,) + lvl.fmm.out_shape, dtype=torch.float64, device=dev)
     lvl.fmm.bind_outputs(L, Lc)
@@ -516,8 +523,14 @@ def run_coupled(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    def step():
+        if peer:
+            lvl.step(own_m, own_c, L, Lc)
+        else:
+            lvl.step(None, None, L, Lc)
+
     for _ in range(max(args.warmup, 3)):
-        lvl.step(None, None, L, Lc)
+        step()
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -528,7 +541,7 @@ def run_coupled(args):
     t0 = time.perf_counter()
     ev0.record(stream)
     for _ in range(args.steps):
-        lvl.step(None, None, L, Lc)
+        step()
     ev1.record(stream)
     barrier()
     clocks = sampler.stop(t0, time.perf_counter()) if rank == 0 else None
@@ -543,9 +556,9 @@ def run_coupled(args):
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        lvl.moments.copy_(m_h, non_blocking=True)
-        lvl.com_off.copy_(c_h, non_blocking=True)
-        lvl.step(None, None, L, Lc)
+        own_m.copy_(m_h, non_blocking=True)
+        own_c.copy_(c_h, non_blocking=True)
+        step()
         L_h.copy_(L, non_blocking=True)
         torch.cuda.synchronize()
     barrier()
@@ -562,8 +575,10 @@ def run_coupled(args):
                           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                           "config": {"workload": "%s stacked in z: %d x %d x %d cells, theta=%g, correction on" % (
                               w.name, w.n[0], w.n[1], w.n[2] * world, args.theta),
-                              "parallelism": "z-slabs, one in-place halo exchange per step (%d bytes sent by this rank, "
-                                             "%d layers of 23 doubles per cell per neighbour)" % (lvl.halo_bytes_sent, HALO),
+                              "parallelism": ("z-slabs, no exchange: the kernel's TMA loads read the neighbours' staged layers "
+                                              "through peer memory (CUDA IPC); two host barriers per step") if peer else (
+                                             "z-slabs, one in-place halo exchange per step (%d bytes sent by this rank, "
+                                             "%d layers of 23 doubles per cell per neighbour)" % (lvl.halo_bytes_sent, HALO)),
                               "l2": "inputs larger than L2" if w.moments.nbytes > 126e6 else "inputs smaller than L2"},
                           "roofline": {"bound": "alu", "kernel": "m2l_staged_kernel<correction> on every rank (step incl. exchange and staging)",
                                        "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None},
@@ -861,6 +876,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--coupled", action="store_true",
                     help="N > 1: ONE problem in z-slabs with a halo exchange per step instead of independent problems")
+    ap.add_argument("--halo", default="exchange", choices=["exchange", "peer"],
+                    help="with --coupled: how a rank gets its neighbours' boundary layers")
     ap.add_argument("--ref-seconds", type=float, default=12.0,
                     help="CPU seconds of oracle work per cpu_baseline sample / per --impl reference step")
     args = ap.parse_args()

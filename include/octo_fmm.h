@@ -122,6 +122,40 @@ int octo_fmm_dmma_table(double theta, double h, int leaf, int which, int cap_chu
  * skipped: isolated boundary, L321). */
 int octo_fmm_interaction_count(const octo_fmm_t *h, unsigned long long *n);
 
+/* ---- f4: one uniform level sharded into z-slabs, the halo read from PEER MEMORY (the step needs
+ * "boundary data from sibling sub-grids" -- here the sub-grids of the neighbouring ranks) ----
+ * Rank r holds the z-layers of its slab in a handle of its own (n = {nx, ny, nz_local}; whole-slab output region).
+ * octo_fmm_set_neighbours tells the handle where the staged source arrays of the slabs below (z < 0) and above
+ * (z >= nz_local) live; octo_fmm_interact then treats the three slabs as one grid: the slab-fed kernel's TMA loads fetch
+ * the layers within the stencil's reach straight from the neighbours' arrays -- over NVLink when those sit on another
+ * GPU -- while it computes; there is no exchange step, no packing and no halo storage.  NULL = the isolated domain
+ * boundary on that side (L321).  Results are identical to one handle over the three slabs (same kernel, same order).
+ *   octo_fmm_peer: `sources`, `flags` = what octo_fmm_staged_sources returned for the neighbour's handle, as DEVICE
+ *   pointers valid in the calling process (same process: as they are, with peer access enabled between the devices;
+ *   another process: through the octo_fmm_ipc_* helpers below); nz = the neighbour's z-extent (>= 5).  The neighbour's
+ *   handle must have the same nx, ny, h, theta, kind = MULTIPOLE and am_correction.  Pointers are borrowed.
+ * Ordering is the caller's: every rank's set_moments must have COMPLETED (stream synchronised + a barrier across ranks)
+ * before any rank's interact, and no rank may stage again before its neighbours' interact has completed.
+ * Errors: EINVAL for a monopole handle, a handle whose output region is too small for the slab-fed kernel, nz < 5 or
+ * null/misaligned pointers.  With neighbours set, octo_fmm_run_host and octo_fmm_interact_mixed return ESTATE.
+ * octo_fmm_interaction_count counts the pairs with partners in the neighbouring slabs too. */
+typedef struct octo_fmm_peer {
+    const double *sources;
+    const int *flags;
+    int nz;
+} octo_fmm_peer;
+int octo_fmm_staged_sources(const octo_fmm_t *h, octo_fmm_peer *self);
+int octo_fmm_set_neighbours(octo_fmm_t *h, const octo_fmm_peer *below, const octo_fmm_peer *above);
+
+/* CUDA IPC plumbing for one process per GPU: export yields the 64-byte handle of the ALLOCATION that holds dev_ptr
+ * (e.g. the workspace) and dev_ptr's offset in it; import maps that allocation into the calling process (peer access is
+ * enabled lazily) and returns its base (for octo_fmm_ipc_close) and the pointer at the offset.  The exporter keeps the
+ * memory alive until every importer has closed.  Host-side, synchronous; ECUDA if the memory cannot be shared (it must
+ * come from cudaMalloc, which is what torch's caching allocator uses unless expandable segments are on). */
+int octo_fmm_ipc_export(const void *dev_ptr, unsigned char handle[64], unsigned long long *offset);
+int octo_fmm_ipc_import(const unsigned char handle[64], unsigned long long offset, void **base, void **dev_ptr);
+int octo_fmm_ipc_close(void *base);
+
 /* Synchronises the stream and reports device-side conditions of the last interact():
  * OCTO_FMM_EMASS if am_correction met a target mass <= 0, ECUDA on a CUDA error, else OK. */
 int octo_fmm_status(octo_fmm_t *h);

@@ -34,6 +34,10 @@ class octo_fmm_config(ctypes.Structure):
                 ("stream", ctypes.c_void_p), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t)]
 
 
+class octo_fmm_peer(ctypes.Structure):
+    _fields_ = [("sources", ctypes.c_void_p), ("flags", ctypes.c_void_p), ("nz", ctypes.c_int)]
+
+
 class octo_fmm_tree_config(ctypes.Structure):
     _fields_ = [("n0", ctypes.c_int), ("depth", ctypes.c_int), ("h0", ctypes.c_double), ("theta", ctypes.c_double),
                 ("am_correction", ctypes.c_int), ("device", ctypes.c_int), ("stream", ctypes.c_void_p),
@@ -77,6 +81,12 @@ class _Library:
         lib.octo_fmm_dmma_table.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, vp, vp]
         lib.octo_fmm_interaction_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
         lib.octo_fmm_status.argtypes = [vp]
+        peerp = ctypes.POINTER(octo_fmm_peer)
+        lib.octo_fmm_staged_sources.argtypes = [vp, peerp]
+        lib.octo_fmm_set_neighbours.argtypes = [vp, peerp, peerp]
+        lib.octo_fmm_ipc_export.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(ctypes.c_ulonglong)]
+        lib.octo_fmm_ipc_import.argtypes = [ctypes.c_char_p, ctypes.c_ulonglong, ctypes.POINTER(vp), ctypes.POINTER(vp)]
+        lib.octo_fmm_ipc_close.argtypes = [vp]
         lib.octo_fmm_run_host.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_size_t]
         lib.octo_fmm_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
         lib.octo_fmm_launch_info.argtypes = [vp, ip, ip, ip, ip, ip]
@@ -277,6 +287,55 @@ def octo_fmm_interaction_count(h):
     if rc != OK:
         raise OctoFmmError("octo_fmm_interaction_count", rc)
     return int(n.value)
+
+
+def octo_fmm_staged_sources(h):
+    """(sources pointer, flags pointer, nz) of the handle's staged array: what a z-neighbour needs."""
+    me = octo_fmm_peer()
+    rc = _lib.octo_fmm_staged_sources(h, ctypes.byref(me))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_staged_sources", rc)
+    return int(me.sources), int(me.flags), int(me.nz)
+
+
+def _peer(p):
+    if p is None:
+        return None
+    return ctypes.byref(octo_fmm_peer(int(p[0]), int(p[1]), int(p[2])))
+
+
+def octo_fmm_set_neighbours(h, below, above):
+    """below / above: None (domain boundary) or (sources pointer, flags pointer, nz) valid in this process."""
+    rc = _lib.octo_fmm_set_neighbours(h, _peer(below), _peer(above))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_set_neighbours", rc)
+
+
+def octo_fmm_ipc_export(dev_ptr):
+    """(64-byte handle of the allocation holding dev_ptr, offset of dev_ptr in it)."""
+    buf = ctypes.create_string_buffer(64)
+    off = ctypes.c_ulonglong(0)
+    rc = _lib.octo_fmm_ipc_export(ctypes.c_void_p(int(dev_ptr)), buf, ctypes.byref(off))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_ipc_export", rc)
+    return buf.raw, int(off.value)
+
+
+def octo_fmm_ipc_import(handle, offset):
+    """(base of the mapped allocation, pointer at the offset); close the base with octo_fmm_ipc_close."""
+    if len(handle) != 64:
+        raise ValueError("a CUDA IPC handle has 64 bytes")
+    base, ptr = ctypes.c_void_p(0), ctypes.c_void_p(0)
+    rc = _lib.octo_fmm_ipc_import(bytes(handle), int(offset), ctypes.byref(base), ctypes.byref(ptr))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_ipc_import", rc)
+    return int(base.value), int(ptr.value)
+
+
+def octo_fmm_ipc_close(base):
+    rc = _lib.octo_fmm_ipc_close(ctypes.c_void_p(int(base)))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_ipc_close", rc)
 
 
 def octo_fmm_run_host(h, moments_host, com_off_host, L_host, Lcorr_host, scratch, scratch_bytes):
@@ -789,6 +848,16 @@ class OctoFMM:
 
     def interaction_count(self):
         return octo_fmm_interaction_count(self.handle)
+
+    def staged_sources(self):
+        return octo_fmm_staged_sources(self.handle)
+
+    def set_neighbours(self, below=None, above=None):
+        """z-neighbours whose staged layers interact() reads in place of a halo: None, another OctoFMM of this process
+        (kept alive here), or (sources pointer, flags pointer, nz) as octo_fmm_ipc_import returned them."""
+        self._neighbours = (below, above)
+        as_peer = lambda p: p.staged_sources() if isinstance(p, OctoFMM) else p
+        octo_fmm_set_neighbours(self.handle, as_peer(below), as_peer(above))
 
     def launch_info(self):
         return octo_fmm_launch_info(self.handle)

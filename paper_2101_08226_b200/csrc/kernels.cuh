@@ -91,7 +91,15 @@ struct Params {
     //   parent index = (child index >> 1) + psh   (uniform solve: pdim = n / 2, psh = 0; a level of the adaptive tree
     //   stored as a BOX of its lattice: psh = box_lo(child) / 2 - box_lo(parent))
     int pdim[3], psh[3];
+    // z-slab sharding with the halo read from peer memory (f4, octo_fmm_set_neighbours): source layers exist for
+    // z in [zmin, zmax]; z < 0 lies in the slab below (its layer z + nz_below), z >= nz in the slab above.  Without
+    // neighbours zmin = 0, zmax = nz - 1.  nflags: the neighbours' flag words (their sources may carry dipoles).
+    int zmin, zmax, nz_below;
+    const int* nflags[2];
 };
+
+// the tensor maps of the slab-fed kernel: the handle's own staged array and, with neighbours, theirs
+struct SlabMaps { CUtensorMap own, below, above; };
 
 // ------------------------------------------------------------------------------------------
 // a2: stage the sources
@@ -330,7 +338,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         const bool layer_on = k < p.ke;                // warp-uniform
         const bool active = layer_on && gx < p.hi[0] && gy < p.hi[1];
         const int cls = cls_xy + ((k & 1) << 2);
-        const int z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.nz - 1);
+        const int z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.zmax);
 
         double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         bool leafA = false;
@@ -350,7 +358,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         // (class, dz).  The loop is software-pipelined by hand: `fetch` loads pair s+1 from shared
         // memory and runs its head (separation, r^2, 1/r) while the body of pair s executes, so the
         // dependent head chain is hidden although only two warps share a sub-partition's FP64 pipe.
-        int zz = max(k0 - p.reach, 0) - 1;
+        int zz = max(k0 - p.reach, p.zmin) - 1;
         int s = 0, s_end = 0;
         bool open = false;
         uint32_t b = 0;
@@ -436,7 +444,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
 
 template <bool CORR, bool FUSE_L2L = false, int MODE = MODE_PLAIN>
 __global__ void __launch_bounds__(STAGED_THREADS, 1)
-m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ Params p)
+m2l_staged_kernel(const __grid_constant__ SlabMaps maps, const __grid_constant__ Params p)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double2* slab0 = reinterpret_cast<double2*>(smem_raw);
@@ -463,12 +471,17 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
             for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
                 int x0, y0, k0;
                 decode_tile(p, t, x0, y0, k0);
-                const int z_lo = max(k0 - p.reach, 0), z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.nz - 1);
+                const int z_lo = max(k0 - p.reach, p.zmin), z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.zmax);
                 for (int zz = z_lo; zz <= z_hi; ++zz) {
                     const uint32_t b = it % NSTAGE;
                     if (it >= NSTAGE) mbar_wait_backoff(&empty[b], ((it / NSTAGE) - 1) & 1);
                     mbar_arrive_expect_tx(&full[b], SLAB_BYTES);
-                    tma_load_slab(slab0 + (size_t)b * SLAB_ELEMS, &tmap, &full[b], (x0 >> 1) - 3, 2 * (y0 - REACH_MAX), zz);
+                    // a layer of a neighbouring z-slab comes straight from that rank's staged array (peer memory)
+                    const CUtensorMap* m = &maps.own;
+                    int zc = zz;
+                    if (zz < 0) { m = &maps.below; zc = zz + p.nz_below; }
+                    else if (zz >= p.nz) { m = &maps.above; zc = zz - p.nz; }
+                    tma_load_slab(slab0 + (size_t)b * SLAB_ELEMS, m, &full[b], (x0 >> 1) - 3, 2 * (y0 - REACH_MAX), zc);
                     ++it;
                 }
             }
@@ -480,7 +493,9 @@ m2l_staged_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     // Sources expanded about their centre of mass have no dipole moment: the staging kernel raises bit 1 of
     // the flags if any cell has |M1_i| > DIPOLE_TOL |M| h, and only then (or when the caller forces it) the
     // 27 dipole terms are evaluated.  The branch is uniform over the grid.
-    const bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
+    bool dipole = p.force_dipole || ((*(volatile const int*)(p.flags + 1)) & 2);
+    if (p.nflags[0] && ((*(volatile const int*)(p.nflags[0] + 1)) & 2)) dipole = true;
+    if (p.nflags[1] && ((*(volatile const int*)(p.nflags[1] + 1)) & 2)) dipole = true;
     if (dipole) staged_consume<CORR, true, FUSE_L2L, MODE>(p, slab0, full, empty, warp, lane);
     else        staged_consume<CORR, false, FUSE_L2L, MODE>(p, slab0, full, empty, warp, lane);
 }

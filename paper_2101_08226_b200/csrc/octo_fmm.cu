@@ -275,7 +275,9 @@ struct octo_fmm {
     int mono_kernel;       // 0 tensor-core instruction (default), 1 DFMA
     bool mixed;            // the last interaction was octo_fmm_interact_mixed
     unsigned long long n_interactions;
-    CUtensorMap tmap;
+    CUtensorMap tmap;      // monopole: the mass tile box of p2p_monopole_kernel
+    SlabMaps maps;         // multipole: own staged array (+ the neighbours' with octo_fmm_set_neighbours)
+    bool has_neighbours;
     Params prm;
     double* src;
     double* L;             // workspace result buffers
@@ -324,6 +326,46 @@ size_t octo_fmm_host_scratch_bytes(const octo_fmm_config* cfg)
     if (cfg->kind == OCTO_FMM_MULTIPOLE)
         return align_up(ncell * 20 * 8) + align_up(ncell * 3 * 8) + align_up(ocell * 20 * 8) + align_up(ocell * 3 * 8);
     return align_up(ncell * 8) + align_up(ocell * 4 * 8);
+}
+
+// interaction count: per-axis closed form over the lists; partners outside the grid are skipped, where the grid's
+// z-extent is [zmin, zmax] (beyond [0, nz) with neighbouring z-slabs, octo_fmm_set_neighbours)
+static unsigned long long count_interactions(const octo_fmm* h, int zmin, int zmax)
+{
+    unsigned long long cnt[3][2][2 * REACH_MAX + 1];
+    for (int a = 0; a < 3; ++a) {
+        const int amin = a == 2 ? zmin : 0, amax = a == 2 ? zmax : h->cfg.n[a] - 1;
+        for (int par = 0; par < 2; ++par)
+            for (int d = -REACH_MAX; d <= REACH_MAX; ++d) {
+                unsigned long long c = 0;
+                for (int i = h->lo[a]; i < h->hi[a]; ++i)
+                    if ((i & 1) == par && i + d >= amin && i + d <= amax) ++c;
+                cnt[a][par][d + REACH_MAX] = c;
+            }
+    }
+    unsigned long long total = 0;
+    for (int p = 0; p < 8; ++p)
+        for (const Offset3& o : h->list[p])
+            total += cnt[0][p & 1][o.d[0] + REACH_MAX] * cnt[1][(p >> 1) & 1][o.d[1] + REACH_MAX] *
+                     cnt[2][(p >> 2) & 1][o.d[2] + REACH_MAX];
+    return total;
+}
+
+// TMA descriptor of a staged multipole array S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
+//      {2 (pair), nx/2 (xh), 2 ny (y*2 + xpar), 10 (cp), nz}
+static int encode_slab_map(CUtensorMap* map, const double* S, int nx, int ny, int nz)
+{
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return OCTO_FMM_ECUDA;
+    const cuuint64_t nxh = (cuuint64_t)nx / 2, nxy = (cuuint64_t)nx * ny;
+    cuuint64_t dims[5] = {2, nxh, 2 * (cuuint64_t)ny, (cuuint64_t)NPAIR, (cuuint64_t)nz};
+    cuuint64_t strides[4] = {16, nxh * 16, nxy * 16, nxy * 16 * NPAIR};
+    cuuint32_t box[5] = {2, SLAB_XH, 2 * SLAB_Y, NPAIR, 1};
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    std::memset(map, 0, sizeof(*map));
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void*)S, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
 
 static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** out)
@@ -447,24 +489,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
         if (h->list_sig_mixed == 0) h->list_sig_mixed = 2;
     }
 
-    // ---- interaction count: per-axis closed form over the lists (out-of-grid partners skipped) ----
-    {
-        unsigned long long cnt[3][2][2 * REACH_MAX + 1];
-        for (int a = 0; a < 3; ++a)
-            for (int par = 0; par < 2; ++par)
-                for (int d = -REACH_MAX; d <= REACH_MAX; ++d) {
-                    unsigned long long c = 0;
-                    for (int i = h->lo[a]; i < h->hi[a]; ++i)
-                        if ((i & 1) == par && i + d >= 0 && i + d < cfg->n[a]) ++c;
-                    cnt[a][par][d + REACH_MAX] = c;
-                }
-        unsigned long long total = 0;
-        for (int p = 0; p < 8; ++p)
-            for (const Offset3& o : h->list[p])
-                total += cnt[0][p & 1][o.d[0] + REACH_MAX] * cnt[1][(p >> 1) & 1][o.d[1] + REACH_MAX] *
-                         cnt[2][(p >> 2) & 1][o.d[2] + REACH_MAX];
-        h->n_interactions = total;
-    }
+    h->has_neighbours = false;
+    h->n_interactions = count_interactions(h, 0, cfg->n[2] - 1);
 
     // ---- workspace partition ----
     char* w = (char*)cfg->workspace;
@@ -493,22 +519,12 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.tile_offset = 0;
     for (int a = 0; a < 3; ++a) { P.pdim[a] = cfg->n[a] / 2; P.psh[a] = 0; }
     for (int d = 0; d <= 2 * REACH_MAX; ++d) P.hmul[d] = h->hmul[d];
+    P.zmin = 0; P.zmax = cfg->n[2] - 1; P.nz_below = 0;
+    P.nflags[0] = nullptr; P.nflags[1] = nullptr;
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
-        // ---- TMA descriptor of S[z][cp][y][xpar][xh][2]; tensor dims (fastest first):
-        //      {2 (pair), nx/2 (xh), 2 ny (y*2 + xpar), 10 (cp), nz}
-        EncodeTiledFn enc = encode_tiled_fn();
-        if (!enc) { delete h; return OCTO_FMM_ECUDA; }
-        const cuuint64_t nxh = (cuuint64_t)cfg->n[0] / 2, nxy = (cuuint64_t)cfg->n[0] * cfg->n[1];
-        cuuint64_t dims[5] = {2, nxh, 2 * (cuuint64_t)cfg->n[1], (cuuint64_t)NPAIR, (cuuint64_t)cfg->n[2]};
-        cuuint64_t strides[4] = {16, nxh * 16, nxy * 16, nxy * 16 * NPAIR};
-        cuuint32_t box[5] = {2, SLAB_XH, 2 * SLAB_Y, NPAIR, 1};
-        cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-        std::memset(&h->tmap, 0, sizeof(h->tmap));
-        CUresult r = enc(&h->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void*)h->src, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) { delete h; return OCTO_FMM_ECUDA; }
+        if (encode_slab_map(&h->maps.own, h->src, cfg->n[0], cfg->n[1], cfg->n[2]) != OCTO_FMM_OK) { delete h; return OCTO_FMM_ECUDA; }
+        h->maps.below = h->maps.own; h->maps.above = h->maps.own;
         cudaError_t e1 = cudaFuncSetAttribute(m2l_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e2 = cudaFuncSetAttribute(m2l_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
         cudaError_t e3 = cudaFuncSetAttribute(m2l_staged_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, STAGED_SMEM);
@@ -674,21 +690,21 @@ static int launch_staged(octo_fmm_t* h, int kb, int ke, bool mixed = false)
         // scheduler packs their bricks onto the SMs as they come free (the ring fill per brick is 3 % of a full brick)
         const int tgrid = (int)P.ntiles;
         if (P.pL) {        // the parent's expansion added in the epilogue (levels one after the other)
-            if (h->cfg.am_correction) m2l_staged_kernel<true, true, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-            else                      m2l_staged_kernel<false, true, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+            if (h->cfg.am_correction) m2l_staged_kernel<true, true, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
+            else                      m2l_staged_kernel<false, true, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
         } else {
-            if (h->cfg.am_correction) m2l_staged_kernel<true, false, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-            else                      m2l_staged_kernel<false, false, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+            if (h->cfg.am_correction) m2l_staged_kernel<true, false, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
+            else                      m2l_staged_kernel<false, false, MODE_TREE><<<tgrid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
         }
     } else if (mixed) {    // one level of an adaptive mesh: leaf-level lists, near-field entries conditional on the leaf flags
-        if (h->cfg.am_correction) m2l_staged_kernel<true, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-        else                      m2l_staged_kernel<false, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        if (h->cfg.am_correction) m2l_staged_kernel<true, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
+        else                      m2l_staged_kernel<false, false, MODE_MIXED><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
     } else if (P.pL) {     // complete solve: L2L fused into the epilogue (solver.inl sets the parent arrays)
-        if (h->cfg.am_correction) m2l_staged_kernel<true, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-        else                      m2l_staged_kernel<false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        if (h->cfg.am_correction) m2l_staged_kernel<true, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
+        else                      m2l_staged_kernel<false, true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
     } else {
-        if (h->cfg.am_correction) m2l_staged_kernel<true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
-        else                      m2l_staged_kernel<false><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->tmap, P);
+        if (h->cfg.am_correction) m2l_staged_kernel<true><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
+        else                      m2l_staged_kernel<false><<<grid, STAGED_THREADS, STAGED_SMEM, h->stream>>>(h->maps, P);
     }
     return cudaGetLastError() == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
 }
@@ -815,7 +831,7 @@ __global__ void __launch_bounds__(256) count_near_kernel(const Params p, const u
 int octo_fmm_interact_mixed(octo_fmm_t* h, const unsigned char* leaf)
 {
     if (!h || !leaf || h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
-    if (h->state < 1) return OCTO_FMM_ESTATE;
+    if (h->state < 1 || h->has_neighbours) return OCTO_FMM_ESTATE;
     if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
     if (h->kernel == 0) {
         // slab-fed kernel: one pass over the leaf-level lists; the partner's leaf flag travels in the padding slot of its record
@@ -934,6 +950,11 @@ int octo_fmm_dipole_terms_used(octo_fmm_t* h, int* used)
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     int f = 0;
     if (cudaMemcpy(&f, h->flags + 1, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
+    for (const int* nf : {h->prm.nflags[0], h->prm.nflags[1]}) {      // the neighbours' sources count too (f4)
+        int g = 0;
+        if (nf && cudaMemcpy(&g, nf + 1, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) return OCTO_FMM_ECUDA;
+        f |= g;
+    }
     *used = (h->prm.force_dipole || (f & 2)) ? 1 : 0;
     return OCTO_FMM_OK;
 }
@@ -993,6 +1014,78 @@ int octo_fmm_interaction_count(const octo_fmm_t* h, unsigned long long* n)
 {
     if (!h || !n) return OCTO_FMM_EINVAL;
     *n = h->n_interactions;
+    return OCTO_FMM_OK;
+}
+
+// ---- f4: z-slab sharding with the halo read from peer memory ----
+int octo_fmm_staged_sources(const octo_fmm_t* h, octo_fmm_peer* self)
+{
+    if (!h || !self || h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
+    self->sources = h->src;
+    self->flags = h->flags;
+    self->nz = h->cfg.n[2];
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_set_neighbours(octo_fmm_t* h, const octo_fmm_peer* below, const octo_fmm_peer* above)
+{
+    if (!h || h->cfg.kind != OCTO_FMM_MULTIPOLE) return OCTO_FMM_EINVAL;
+    // the slab-fed kernel over the whole x-y plane of a plain uniform level only
+    if (h->kernel != 0 || h->tree_kind || h->tile_list) return OCTO_FMM_EINVAL;
+    for (const octo_fmm_peer* nb : {below, above})
+        if (nb && (!nb->sources || !nb->flags || nb->nz < h->reach || ((uintptr_t)nb->sources % 16))) return OCTO_FMM_EINVAL;
+    if (cudaSetDevice(h->cfg.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    SlabMaps m = h->maps;
+    m.below = m.own; m.above = m.own;
+    if (below && encode_slab_map(&m.below, below->sources, h->cfg.n[0], h->cfg.n[1], below->nz) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    if (above && encode_slab_map(&m.above, above->sources, h->cfg.n[0], h->cfg.n[1], above->nz) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+    h->maps = m;
+    Params& P = h->prm;
+    // only the layers within the stencil's reach are ever read
+    P.zmin = below ? -h->reach : 0;
+    P.zmax = h->cfg.n[2] - 1 + (above ? h->reach : 0);
+    P.nz_below = below ? below->nz : 0;
+    P.nflags[0] = below ? below->flags : nullptr;
+    P.nflags[1] = above ? above->flags : nullptr;
+    h->has_neighbours = below || above;
+    h->n_interactions = count_interactions(h, P.zmin, P.zmax);
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_ipc_export(const void* dev_ptr, unsigned char handle[64], unsigned long long* offset)
+{
+    if (!dev_ptr || !handle || !offset) return OCTO_FMM_EINVAL;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handles are 64 bytes");
+    CUdeviceptr base = 0;
+    size_t size = 0;
+    typedef CUresult (*RangeFn)(CUdeviceptr*, size_t*, CUdeviceptr);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return OCTO_FMM_ECUDA;
+    if (((RangeFn)fn)(&base, &size, (CUdeviceptr)(uintptr_t)dev_ptr) != CUDA_SUCCESS) return OCTO_FMM_ECUDA;
+    cudaIpcMemHandle_t hd;
+    if (cudaIpcGetMemHandle(&hd, (void*)(uintptr_t)base) != cudaSuccess) { cudaGetLastError(); return OCTO_FMM_ECUDA; }
+    std::memcpy(handle, &hd, 64);
+    *offset = (unsigned long long)((uintptr_t)dev_ptr - (uintptr_t)base);
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_ipc_import(const unsigned char handle[64], unsigned long long offset, void** base, void** dev_ptr)
+{
+    if (!handle || !base || !dev_ptr) return OCTO_FMM_EINVAL;
+    cudaIpcMemHandle_t hd;
+    std::memcpy(&hd, handle, 64);
+    void* b = nullptr;
+    if (cudaIpcOpenMemHandle(&b, hd, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { cudaGetLastError(); return OCTO_FMM_ECUDA; }
+    *base = b;
+    *dev_ptr = (char*)b + offset;
+    return OCTO_FMM_OK;
+}
+
+int octo_fmm_ipc_close(void* base)
+{
+    if (!base) return OCTO_FMM_EINVAL;
+    if (cudaIpcCloseMemHandle(base) != cudaSuccess) { cudaGetLastError(); return OCTO_FMM_ECUDA; }
     return OCTO_FMM_OK;
 }
 
@@ -1109,6 +1202,7 @@ int octo_fmm_run_host(octo_fmm_t* h, const double* moments_host, const double* c
                       double* Lcorr_host, void* scratch, size_t scratch_bytes)
 {
     if (!h || !moments_host || !L_host || !scratch) return OCTO_FMM_EINVAL;
+    if (h->has_neighbours) return OCTO_FMM_ESTATE;     // the neighbours' staging is ordered by the caller, not by this call
     if (scratch_bytes < octo_fmm_host_scratch_bytes(&h->cfg) || ((uintptr_t)scratch % ALIGN)) return OCTO_FMM_EINVAL;
     const Params& P = h->prm;
     const size_t ncell = (size_t)P.nx * P.ny * P.nz, ocell = (size_t)P.ox * P.oy * P.oz;

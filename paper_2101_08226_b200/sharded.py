@@ -129,3 +129,69 @@ class ShardedLevel:
 
     def close(self):
         self.fmm.close()
+
+
+class PeerShardedLevel:
+    """The same step with NO exchange and no halo storage (octo_fmm.h, octo_fmm_set_neighbours): every rank stages only
+    its own slab; at construction the ranks trade the CUDA IPC handles of their workspaces once, and from then on the
+    slab-fed kernel's TMA loads fetch the neighbours' boundary layers straight from their staged arrays (over NVLink when
+    they sit on other GPUs) while it computes.  Per step: set_moments, a barrier (every slab staged), interact.
+    A second barrier at the start of the next step keeps a rank from staging over layers a neighbour is still reading.
+    Results are bit-identical to ShardedLevel's and to one handle over the whole grid.
+
+    One process per GPU; `group` may be a gloo or an NCCL group (it carries 100 bytes per rank once, then barriers)."""
+
+    def __init__(self, n_local, h, theta, am_correction=True, rank=0, world=1, group=None, device=0, stream=None):
+        from . import (MULTIPOLE, OctoFMM, octo_fmm_ipc_export, octo_fmm_ipc_import)
+        nx, ny, nzl = (int(v) for v in n_local)
+        if nzl % 8 or nzl < HALO:
+            raise ValueError("nz_local must be a multiple of 8")
+        self.rank, self.world, self.group = int(rank), int(world), group
+        self.n_local = (nx, ny, nzl)
+        self.fmm = OctoFMM((nx, ny, nzl), h, theta, MULTIPOLE, am_correction, device=device, stream=stream)
+        self._bases = []
+        self._dirty = False
+        if self.world > 1:
+            import torch.distributed as dist
+            src, flg, nz = self.fmm.staged_sources()
+            ws = self.fmm.workspace.data_ptr()
+            handle, off = octo_fmm_ipc_export(ws)
+            everyone = [None] * self.world
+            dist.all_gather_object(everyone, (handle, off, src - ws, flg - ws, nz), group=group)
+            peers = {}
+            for r in (self.rank - 1, self.rank + 1):
+                if 0 <= r < self.world:
+                    hd, o, dsrc, dflg, pnz = everyone[r]
+                    base, pws = octo_fmm_ipc_import(hd, o)
+                    self._bases.append(base)
+                    peers[r] = (pws + dsrc, pws + dflg, pnz)
+            self.fmm.set_neighbours(peers.get(self.rank - 1), peers.get(self.rank + 1))
+
+    def _barrier(self):
+        if self.world > 1:
+            import torch.distributed as dist
+            self.fmm.stream.synchronize()
+            dist.barrier(group=self.group)
+
+    def step(self, moments, com_off, L=None, Lcorr=None):
+        """moments [20][nz_local][ny][nx], com_off [3][...] of the OWNED slab.  Returns (L, Lcorr) of the owned slab."""
+        if self._dirty:
+            self._barrier()            # the neighbours have finished reading my previous sources
+        self.fmm.set_moments(moments, com_off)
+        self._barrier()                # every rank's slab is staged
+        self.fmm.interact()
+        self._dirty = True
+        return self.fmm.get_expansions(L, Lcorr)
+
+    def interaction_count(self):
+        return self.fmm.interaction_count()
+
+    def close(self):
+        from . import octo_fmm_ipc_close
+        if self._dirty:
+            self._barrier()
+            self._dirty = False
+        self.fmm.close()
+        for b in self._bases:
+            octo_fmm_ipc_close(b)
+        self._bases = []

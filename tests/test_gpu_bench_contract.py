@@ -44,3 +44,14 @@ def test_bench_line(workload):
     assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
     assert e["value"] < d["value"] * 1.5                       # copies are inside the e2e region
     assert {"sm_mhz", "sm_max_mhz", "reasons"} <= set(d["clocks"]) and d["gpu_launches"] > 0
+
+
+@pytest.mark.parametrize("halo", ["exchange", "peer"])
+def test_coupled_line(halo):
+    """--coupled (one problem in z-slabs, f4) carries the full key set in both halo modes; at N = 1 there are no neighbours."""
+    d = run_bench("--coupled", "--halo", halo, "--workload", "cfg2", "--ncell", "32", "--steps", "2", "--warmup", "1",
+                  "--e2e-steps", "1", "--ref-seconds", "0.2")
+    assert BASE_KEYS <= set(d), BASE_KEYS - set(d)
+    assert d["value"] > 0 and d["n_gpus"] == 1 and d["scaling"] == "weak" and d["roofline"]["bound"] == "alu"
+    assert ("peer memory" in d["config"]["parallelism"]) == (halo == "peer")
+    assert d["e2e"]["value"] > 0 and d["e2e"]["h2d_bytes_per_step"] > 0 and d["gpu_launches"] > 0
