@@ -47,9 +47,10 @@ constexpr int STAGED_SMEM = NSTAGE * SLAB_BYTES + 64;
 static_assert(STAGED_SMEM <= 227 * 1024, "shared memory per CTA");
 
 struct StEntry {
-    int off;                 // shared-memory offset relative to the thread's base (multipole: double2 units in
-                             // the slab; monopole: doubles in the mass tile)
-    signed char dx, dy, dz, d2;   // d2: monopole handles |Delta|^2; mixed-level lists 1 = near-field entry (not well separated)
+    int off;                 // multipole: shared-memory offset of the source relative to the thread's base in the slab, in
+                             // BYTES; monopole: offset in the mass tile (doubles, low 16 bits) + index of the weights (high 16)
+    signed char dx, dy, dz, d2;   // the offset.  MULTIPOLE lists hold 8 dx, 8 dy, 8 dz: byte offsets into Params::hmul, ready
+                                  // for the list walk of the slab-fed kernel (cell offsets: entry_cells());   // d2: monopole handles |Delta|^2; mixed-level lists 1 = near-field entry (not well separated)
 };
 
 // Stencil tables (the interaction lists of the 8 parity classes, Eq. 15) in constant memory.  They depend on
@@ -96,7 +97,29 @@ struct Params {
     // neighbours zmin = 0, zmax = nz - 1.  nflags: the neighbours' flag words (their sources may carry dipoles).
     int zmin, zmax, nz_below;
     const int* nflags[2];
+    // zr[pz] = {first, last} dz with a list entry for targets of z-parity pz (theta = 0.5: {-4, 5} for even layers, {-5, 4}
+    // for odd ones): the slabs a brick streams are the union over its layers, not k0 - reach .. k0 + TILE_Z - 1 + reach
+    int zr[2][2];
 };
+
+// (double)(-d) * h for a multipole list entry's field d8 = 8 d
+__device__ __forceinline__ double hmul_at(const Params& p, int d8)
+{
+    return *reinterpret_cast<const double*>(reinterpret_cast<const char*>(p.hmul) + 8 * REACH_MAX + d8);
+}
+
+// the z-range of source layers the brick at k0 needs (the same on the producer and the consumer side)
+__device__ __forceinline__ void brick_z_range(const Params& p, int k0, int& z_lo, int& z_hi)
+{
+    int lo = k0 + p.zr[k0 & 1][0], hi = k0 + p.zr[k0 & 1][1];
+#pragma unroll
+    for (int l = 1; l < TILE_Z; ++l) {
+        const int k = k0 + l;
+        if (k < p.ke) { lo = min(lo, k + p.zr[k & 1][0]); hi = max(hi, k + p.zr[k & 1][1]); }
+    }
+    z_lo = max(lo, p.zmin);
+    z_hi = min(hi, p.zmax);
+}
 
 // the tensor maps of the slab-fed kernel: the handle's own staged array and, with neighbours, theirs
 struct SlabMaps { CUtensorMap own, below, above; };
@@ -338,7 +361,8 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         const bool layer_on = k < p.ke;                // warp-uniform
         const bool active = layer_on && gx < p.hi[0] && gy < p.hi[1];
         const int cls = cls_xy + ((k & 1) << 2);
-        const int z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.zmax);
+        int z_lo, z_hi;
+        brick_z_range(p, k0, z_lo, z_hi);
 
         double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         bool leafA = false;
@@ -358,7 +382,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         // (class, dz).  The loop is software-pipelined by hand: `fetch` loads pair s+1 from shared
         // memory and runs its head (separation, r^2, 1/r) while the body of pair s executes, so the
         // dependent head chain is hidden although only two warps share a sub-partition's FP64 pipe.
-        int zz = max(k0 - p.reach, p.zmin) - 1;
+        int zz = z_lo - 1;
         int s = 0, s_end = 0;
         bool open = false;
         uint32_t b = 0;
@@ -382,32 +406,33 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
                 if (layer_on && dz >= -p.reach && dz <= p.reach) {
                     sl = slab0 + (size_t)b * SLAB_ELEMS + tbase;
                     Rz0 = p.hmul[dz + REACH_MAX] + dA[2];
-                    s = cls * MAX_LIST + c_begin[cls][dz + REACH_MAX];
-                    s_end = cls * MAX_LIST + c_begin[cls][dz + REACH_MAX + 1];
+                    s = (cls * MAX_LIST + c_begin[cls][dz + REACH_MAX]) * (int)sizeof(StEntry);       // byte offsets
+                    s_end = (cls * MAX_LIST + c_begin[cls][dz + REACH_MAX + 1]) * (int)sizeof(StEntry);
                 }
             }
             return true;
         };
 #define OCTO_FETCH(P)                                                                       \
         {                                                                                   \
-            const StEntry e_ = c_entries[s];                                                \
-            ++s;                                                                            \
+            const StEntry e_ = *reinterpret_cast<const StEntry*>(reinterpret_cast<const char*>(c_entries) + s); \
+            s += (int)sizeof(StEntry);                                                      \
+            const double2* q_ = reinterpret_cast<const double2*>(reinterpret_cast<const char*>(sl) + e_.off); \
             bool masked_ = false;                                                           \
             P.live = true;                                                                  \
             if (MODE == MODE_TREE) {                                                        \
                 /* the partner's kind first: absent, or a leaf meeting a leaf -> this lane takes nothing; if that holds \
                    for the whole warp (kinds are constant over sub-grids: the usual case next to a refinement boundary) \
                    the pair is skipped altogether */                                        \
-                const double kb_ = (sl + e_.off)[9 * SLAB_PLANE].y;                         \
+                const double kb_ = q_[9 * SLAB_PLANE].y;                                      \
                 masked_ = !present || kb_ == 0.0 || (leafA && kb_ == 1.0);                  \
                 P.live = !__all_sync(0xffffffffu, masked_);                                 \
             }                                                                               \
             if (P.live) {                                                                   \
                 double bx_, by_, bz_, fl_ = 0.0;                                            \
-                if (MODE != MODE_PLAIN) { OCTO_LOAD_SOURCE_F(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
-                else       { OCTO_LOAD_SOURCE(sl + e_.off, SLAB_PLANE, P.src, bx_, by_, bz_); }  \
-                P.x = p.hmul[e_.dx + REACH_MAX] + (dA[0] - bx_);                            \
-                P.y = p.hmul[e_.dy + REACH_MAX] + (dA[1] - by_);                            \
+                if (MODE != MODE_PLAIN) { OCTO_LOAD_SOURCE_F(q_, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
+                else       { OCTO_LOAD_SOURCE(q_, SLAB_PLANE, P.src, bx_, by_, bz_); }      \
+                P.x = hmul_at(p, e_.dx) + (dA[0] - bx_);                                    \
+                P.y = hmul_at(p, e_.dy) + (dA[1] - by_);                                    \
                 P.z = Rz0 - bz_;                                                            \
                 P.w = pair_head(P.x, P.y, P.z);                                             \
                 if (MODE == MODE_MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;         \
@@ -471,7 +496,8 @@ m2l_staged_kernel(const __grid_constant__ SlabMaps maps, const __grid_constant__
             for (long long t = blockIdx.x; t < p.ntiles; t += gridDim.x) {
                 int x0, y0, k0;
                 decode_tile(p, t, x0, y0, k0);
-                const int z_lo = max(k0 - p.reach, p.zmin), z_hi = min(min(k0 + TILE_Z, p.ke) - 1 + p.reach, p.zmax);
+                int z_lo, z_hi;
+                brick_z_range(p, k0, z_lo, z_hi);
                 for (int zz = z_lo; zz <= z_hi; ++zz) {
                     const uint32_t b = it % NSTAGE;
                     if (it >= NSTAGE) mbar_wait_backoff(&empty[b], ((it / NSTAGE) - 1) & 1);
@@ -530,14 +556,14 @@ __global__ void __launch_bounds__(256) m2l_direct_kernel(const __grid_constant__
 #pragma unroll 1
         for (int s = c_begin[cls][0]; s < s_end; ++s) {
             const StEntry e = c_entries[cls * MAX_LIST + s];
-            const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+            const int sx = gx + (e.dx >> 3), sy = gy + (e.dy >> 3), sz = k + (e.dz >> 3);
             if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
             const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
             double src[16], bx_, by_, bz_;
             OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
-            const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
-            const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
-            const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+            const double x = hmul_at(p, e.dx) + (dA[0] - bx_);
+            const double y = hmul_at(p, e.dy) + (dA[1] - by_);
+            const double z = hmul_at(p, e.dz) + (dA[2] - bz_);
             if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
             else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
         }
@@ -642,14 +668,14 @@ __global__ void __launch_bounds__(256) m2l_warp_kernel(const __grid_constant__ P
 #pragma unroll 1
     for (int s = c_begin[cls][0] + lane; s < s_end; s += 32) {
         const StEntry e = c_entries[cls * MAX_LIST + s];
-        const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+        const int sx = gx + (e.dx >> 3), sy = gy + (e.dy >> 3), sz = k + (e.dz >> 3);
         if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
         const double2* q = S2 + (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
         double src[16], bx_, by_, bz_;
         OCTO_LOAD_SOURCE(q, plane, src, bx_, by_, bz_);
-        const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
-        const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
-        const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+        const double x = hmul_at(p, e.dx) + (dA[0] - bx_);
+        const double y = hmul_at(p, e.dy) + (dA[1] - by_);
+        const double z = hmul_at(p, e.dz) + (dA[2] - bz_);
         if (dipole) m2l_pair<CORR, true>(acc, x, y, z, pair_head(x, y, z), src, tA);
         else        m2l_pair<CORR, false>(acc, x, y, z, pair_head(x, y, z), src, tA);
     }
@@ -704,15 +730,15 @@ __global__ void __launch_bounds__(256) m2l_warp2_kernel(const __grid_constant__ 
 #pragma unroll 1
     for (int s = c_begin[cls][0] + lane; s < s_end; s += 32) {
         const StEntry e = c_entries[cls * MAX_LIST + s];
-        const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+        const int sx = gx + (e.dx >> 3), sy = gy + (e.dy >> 3), sz = k + (e.dz >> 3);
         if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
         const long long o = (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
         double src[16], src2[16], bx_, by_, bz_;
         OCTO_LOAD_SOURCE(S1 + o, plane, src, bx_, by_, bz_);
         OCTO_LOAD_SOURCE2(S2 + o, plane, src2);
-        const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
-        const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
-        const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+        const double x = hmul_at(p, e.dx) + (dA[0] - bx_);
+        const double y = hmul_at(p, e.dy) + (dA[1] - by_);
+        const double z = hmul_at(p, e.dz) + (dA[2] - bz_);
         const double w = pair_head(x, y, z);
         if (dipole) m2l_pair<CORR, true>(acc, x, y, z, w, src, tA);
         else        m2l_pair<CORR, false>(acc, x, y, z, w, src, tA);
@@ -765,15 +791,15 @@ __global__ void __launch_bounds__(256) m2l_direct2_kernel(const __grid_constant_
 #pragma unroll 1
         for (int s = c_begin[cls][0]; s < s_end; ++s) {
             const StEntry e = c_entries[cls * MAX_LIST + s];
-            const int sx = gx + e.dx, sy = gy + e.dy, sz = k + e.dz;
+            const int sx = gx + (e.dx >> 3), sy = gy + (e.dy >> 3), sz = k + (e.dz >> 3);
             if (sx < 0 || sy < 0 || sz < 0 || sx >= p.nx || sy >= p.ny || sz >= p.nz) continue;
             const long long o = (long long)sz * NPAIR * plane + (long long)sy * p.nx + (sx & 1) * (p.nx >> 1) + (sx >> 1);
             double src[16], src2[16], bx_, by_, bz_;
             OCTO_LOAD_SOURCE(S1 + o, plane, src, bx_, by_, bz_);
             OCTO_LOAD_SOURCE2(S2 + o, plane, src2);
-            const double x = p.hmul[e.dx + REACH_MAX] + (dA[0] - bx_);
-            const double y = p.hmul[e.dy + REACH_MAX] + (dA[1] - by_);
-            const double z = p.hmul[e.dz + REACH_MAX] + (dA[2] - bz_);
+            const double x = hmul_at(p, e.dx) + (dA[0] - bx_);
+            const double y = hmul_at(p, e.dy) + (dA[1] - by_);
+            const double z = hmul_at(p, e.dz) + (dA[2] - bz_);
             const double w = pair_head(x, y, z);
             if (dipole) m2l_pair<CORR, true>(acc, x, y, z, w, src, tA);
             else        m2l_pair<CORR, false>(acc, x, y, z, w, src, tA);

@@ -54,6 +54,10 @@ __device__ __forceinline__ void acc_zero(Acc& a)
     for (int i = 0; i < 7; ++i) a.l3[i] = 0.0;
 }
 
+// constants that are not 32-bit immediates: as literals they are rebuilt by two moves per pair, from the constant bank
+// they are an operand of the instruction
+__constant__ double c_fold[2] = {-7.0 / 3.0, 0.375};
+
 // 1/sqrt(x) to ~1 ulp for normal positive x
 __device__ __forceinline__ double rsqrt_fast(double x)
 {
@@ -61,7 +65,7 @@ __device__ __forceinline__ double rsqrt_fast(double x)
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double t = x * y;
     const double e = fma(-t, y, 1.0);
-    const double p = fma(0.375, e, 0.5);
+    const double p = fma(c_fold[1], e, 0.5);
     const double q = e * p;
     return fma(y, q, y);
 }
@@ -124,109 +128,137 @@ __device__ __forceinline__ double pair_head(const double x, const double y, cons
 
 // Body of one ordered pair with the correction ON.  Instead of generating the components of D2, D3, D4 and
 // multiplying each by every source component, everything a source contributes is written as a radial factor times
-// products of components of R, with the source's mass folded into the radial factors:
-//   L0   += -M w + d1 (m1.R) + d2 S + d3 C                 S = q~_jk R_j R_k,  C = n_jkl R_j R_k R_l  (see below)
-//   L1_i += (M d1 + d2 (m1.R) + d3 S) R_i + d1 m1_i + 2 d2 V_i        V_i = q~_ij R_j
-//   L2_ij += c1 d_ij + c2 R_i R_j + h_i R_j + h_j R_i      c1 = M d1 + d2 (m1.R),  c2 = M d2 + d3 (m1.R),  h = d2 m1
-//   L3_ijk += M d2 (d_ij R_k + d_ik R_j + d_jk R_i) + M d3 R_i R_j R_k
-//   dL1_i += d4 C R_i + 3 d3 Q_i,  L0 += d3 C              n = N'_B - M_B (N'_A / M_A),  Q_i = n_ijk R_j R_k  (L127)
-// with m1 = -M1 (staged), q~ = 1/2 trace-free M2, N' = -1/6 trace-free M3.  These are the sums of the header of
-// this file with D2_ij = d1 d_ij + d2 R_i R_j etc. multiplied out (the quadrupole and dipole parts use that D2 and
-// D3 are trace-free); the independent components of L2 and L3 are accumulated as in the component form, each
-// completed per pair.  120 FP64 instructions per pair without the dipole terms and 141 with them, against 129 / 157
-// for the component-by-component contraction; the oracle keeps the component form.
+// products of components of R, with the source's mass folded into the radial factors (e_n = M d_n):
+//   L0   += -M w + d1 (m1.R) + d2 S + d3 C                 V_i = q~_ij R_j,  S = R.V,  Q_i = n_ijk R_j R_k,  C = R.Q
+//   L1_i += k1 R_i + d1 m1_i + 2 d2 V_i                    k1 = c1 + d3 S
+//   L2_ij += c1 d_ij + v_i R_j + h_j R_i                   c1 = e1 + d2 (m1.R),  c2 = e2 + d3 (m1.R),  h = d2 m1,  v = c2 R + h
+//   L3_ijk += e2 (d_ij R_k + d_ik R_j + d_jk R_i) + e3 R_i R_j R_k
+//   dL1_i += d4 C R_i + 3 d3 Q_i,  L0 += d3 C              n = N'_B - M_B (N'_A / M_A)   (L127)
+// with m1 = -M1 (staged), q~ = 1/2 trace-free M2, N' = -1/6 trace-free M3, d1 = 1/r^3, d2 = -3/r^5, d3 = 15/r^7,
+// d4 = -105/r^9.  These are the sums of the header of this file with D2_ij = d1 d_ij + d2 R_i R_j etc. multiplied out
+// (the quadrupole and dipole parts use that D2 and D3 are trace-free).  What keeps the instruction count down:
+//   - L3 is trace-free pair by pair (5 d2 + d3 r^2 = 0), so seven components carry it; the seven WITHOUT a repeated
+//     triple index (xxy xxz xyy yyz xzz yzz xyz) need only f_ii = e3 R_i^2 + e2, never the 3 e2 of xxx, yyy, zzz;
+//     acc_finish rebuilds xxx = -(xyy + xzz) etc.;
+//   - the diagonal of L2 is completed per pair (c1 and c2 x^2 cancel to a large extent; summing them separately over
+//     the list would lose those digits);
+//   - a.c holds ONE THIRD of the correction, d3 Q_i + (d4 / 3) C R_i (acc_finish multiplies by 3); -7/3 and the 0.375
+//     of rsqrt_fast come from the constant bank (c_fold), so no instruction rebuilds them.
+// 130 FP64 instructions per pair with the dipole terms (82 DFMA, 35 DMUL, 13 DADD: 212 flop) and 113 without, against
+// 157 / 129 for the component-by-component contraction; the oracle keeps the component form.
+//
+// ORDER OF THE STATEMENTS.  An FP64 instruction occupies the pipe for 2 cycles, and for 3 if all three of its source
+// registers have to be read fresh (profiles/r02_sass_cost_model.md); an operand is free when the previous instruction
+// of the warp read the same register in the same slot.  ptxas decides the final order, but it starts from the order of
+// the source, so the statements below stand in the order that a search over dependency-respecting permutations found
+// to give the fewest pipe cycles in the SASS of m2l_staged_kernel (python -m paper_2101_08226_b200.sass_cost_model:
+// 41 of 82 DFMAs with three fresh registers instead of 59 for the "natural" order of the formulas above).  Each
+// statement is one term of those formulas; names as above, n_ijk / p_ij (= x^2 - z^2, y^2 - z^2, 2xy, 2xz, 2yz) for
+// the cubic form.
 template <bool DIPOLE>
 __device__ __forceinline__ void m2l_pair_folded(Acc& a, const double x, const double y, const double z, const double w,
                                                   const double (&s)[16], const double (&tA)[7])
 {
-    const double w2 = w * w;                  // 1/r^2
-    const double d1 = w * w2;                 // 1/r^3
-    const double d2 = d1 * (-3.0 * w2);       // -3/r^5
-    const double d3 = d2 * (-5.0 * w2);       // 15/r^7
+    const double w2 = w * w;
+    const double x2 = x + x;
+    const double k3 = -3.0 * w2;
+    const double m1y = DIPOLE ? s[C_M1Y] : 0.0;
     const double m0 = s[C_M0];
-    const double qxx = s[C_QXX], qxy = s[C_QXY], qxz = s[C_QXZ], qyy = s[C_QYY], qyz = s[C_QYZ];
-    const double e1 = m0 * d1, e2 = m0 * d2, e3 = m0 * d3;
-    a.l0 = fma(m0, -w, a.l0);
-
-    // products of R shared by the quadrupole and octupole parts
+    const double qyz = s[C_QYZ];
+    const double d1 = w * w2;
+    const double y2 = y + y;
+    const double d2 = d1 * k3;
+    const double pyz = y2 * z;
+    const double e2 = m0 * d2;
+    const double qxy = s[C_QXY];
+    const double pxz = x2 * z;
+    const double nxxz = fma(-m0, tA[2], s[C_OXXZ]);
+    const double k7 = c_fold[0] * w2;
+    const double qxx = s[C_QXX];
+    const double k5 = -5.0 * w2;
+    const double d3 = d2 * k5;
     const double zz = z * z;
-    const double pa = fma(x, x, -zz), pb = fma(y, y, -zz);              // x^2 - z^2, y^2 - z^2
-    const double x2 = x + x, y2 = y + y;
-    const double pxy = x2 * y, pxz = x2 * z, pyz = y2 * z;              // 2xy, 2xz, 2yz
-
-    // ---- quadrupole: S = q~ : R R (q~ trace-free),  V = q~ R ----
-    const double S = fma(qyz, pyz, fma(qxz, pxz, fma(qxy, pxy, fma(qyy, pb, qxx * pa))));
-    a.l0b = fma(d2, S, a.l0b);
+    if (DIPOLE) a.l1[1] = fma(d1, m1y, a.l1[1]);
+    const double e3 = m0 * d3;
+    const double m1x = DIPOLE ? s[C_M1X] : 0.0;
+    const double hy = DIPOLE ? d2 * m1y : 0.0;
+    const double e3y = e3 * y;
+    const double qxz = s[C_QXZ];
+    const double e3x = e3 * x;
+    const double nxxy = fma(-m0, tA[1], s[C_OXXY]);
+    const double qyy = s[C_QYY];
+    const double fxx = fma(e3x, x, e2);
+    const double nxyz = fma(-m0, tA[4], s[C_OXYZ]);
+    const double fyy = fma(e3y, y, e2);
+    const double nxyy = fma(-m0, tA[3], s[C_OXYY]);
+    const double m1z = DIPOLE ? s[C_M1Z] : 0.0;
     const double qzz = -(qxx + qyy);
-    const double Vx = fma(qxz, z, fma(qxy, y, qxx * x));
-    const double Vy = fma(qyz, z, fma(qyy, y, qxy * x));
+    const double e3z = e3 * z;
+    const double e1 = m0 * d1;
+    const double fzz = fma(e3z, z, e2);
+    if (DIPOLE) a.l1[2] = fma(d1, m1z, a.l1[2]);
+    const double ar = DIPOLE ? fma(m1z, z, fma(m1y, y, m1x * x)) : 0.0;
+    const double d3k7 = d3 * k7;
+    const double nxxx = fma(-m0, tA[0], s[C_OXXX]);
+    const double pxy = x2 * y;
+    const double pa = fma(x, x, -zz);
+    const double c2 = DIPOLE ? fma(d3, ar, e2) : e2;
+    const double nxzz = -(nxxx + nxyy);
+    const double hx = DIPOLE ? d2 * m1x : 0.0;
     const double Vz = fma(qzz, z, fma(qyz, y, qxz * x));
-    const double u2 = d2 + d2;
-
-    // ---- monopole and dipole coefficients of the R-monomials ----
-    double c1 = e1, c2 = e2;
-    if (DIPOLE) {
-        const double m1x = s[C_M1X], m1y = s[C_M1Y], m1z = s[C_M1Z];
-        const double ar = fma(m1z, z, fma(m1y, y, m1x * x));            // m1 . R
-        a.l0 = fma(d1, ar, a.l0);
-        c1 = fma(d2, ar, e1);
-        c2 = fma(d3, ar, e2);
-        a.l1[0] = fma(d1, m1x, a.l1[0]);
-        a.l1[1] = fma(d1, m1y, a.l1[1]);
-        a.l1[2] = fma(d1, m1z, a.l1[2]);
-        const double hx = d2 * m1x, hy = d2 * m1y, hz = d2 * m1z;
-        a.l2[0] = fma(hx, x2, a.l2[0]);
-        a.l2[1] = fma(hy, x, fma(hx, y, a.l2[1]));
-        a.l2[2] = fma(hz, x, fma(hx, z, a.l2[2]));
-        a.l2[3] = fma(hy, y2, a.l2[3]);
-        a.l2[4] = fma(hz, y, fma(hy, z, a.l2[4]));
-    }
-    // ---- L1 ----
-    const double k1 = fma(d3, S, c1);
-    a.l1[0] = fma(u2, Vx, fma(k1, x, a.l1[0]));
-    a.l1[1] = fma(u2, Vy, fma(k1, y, a.l1[1]));
-    a.l1[2] = fma(u2, Vz, fma(k1, z, a.l1[2]));
-    // ---- L2_ij += c1 d_ij + c2 R_i R_j: the diagonal is completed per pair (c1 and c2 x^2 cancel to a large extent;
-    //      summing them separately over the list would lose those digits) ----
-    const double c2x = c2 * x, c2y = c2 * y;
-    a.l2[0] += fma(c2x, x, c1);
-    a.l2[1] = fma(c2x, y, a.l2[1]);
-    a.l2[2] = fma(c2x, z, a.l2[2]);
-    a.l2[3] += fma(c2y, y, c1);
-    a.l2[4] = fma(c2y, z, a.l2[4]);
-    // ---- L3_ijk += M d2 (d_ij R_k + d_ik R_j + d_jk R_i) + M d3 R_i R_j R_k, again completed per pair ----
-    const double e3x = e3 * x, e3y = e3 * y, e2t = 3.0 * e2;
-    const double fxx3 = fma(e3x, x, e2t), fxx1 = fma(e3x, x, e2);      // M (d3 x^2 + 3 d2), M (d3 x^2 + d2)
-    const double fyy3 = fma(e3y, y, e2t), fyy1 = fma(e3y, y, e2);
+    a.l3[2] = fma(fyy, x, a.l3[2]);
+    const double nyyz = fma(-m0, tA[6], s[C_OYYZ]);
+    a.l3[5] = fma(fzz, y, a.l3[5]);
+    const double vx = DIPOLE ? fma(c2, x, hx) : c2 * x;
+    const double vy = DIPOLE ? fma(c2, y, hy) : c2 * y;
+    a.l2[1] = fma(vx, y, a.l2[1]);
+    const double nyyy = fma(-m0, tA[5], s[C_OYYY]);
+    const double hz = DIPOLE ? d2 * m1z : 0.0;
+    a.l0 = fma(m0, -w, a.l0);
+    a.l2[2] = fma(vx, z, a.l2[2]);
+    const double c1 = DIPOLE ? fma(d2, ar, e1) : e1;
+    a.l3[4] = fma(fzz, x, a.l3[4]);
+    const double Vx = fma(qxz, z, fma(qxy, y, qxx * x));
+    if (DIPOLE) a.l0 = fma(d1, ar, a.l0);
     const double e3xy = e3x * y;
-    a.l3[0] = fma(fxx3, x, a.l3[0]);      // xxx
-    a.l3[1] = fma(fxx1, y, a.l3[1]);      // xxy
-    a.l3[2] = fma(fxx1, z, a.l3[2]);      // xxz
-    a.l3[3] = fma(fyy1, x, a.l3[3]);      // xyy
-    a.l3[4] = fma(e3xy, z, a.l3[4]);      // xyz
-    a.l3[5] = fma(fyy3, y, a.l3[5]);      // yyy
-    a.l3[6] = fma(fyy1, z, a.l3[6]);      // yyz
-
-    // ---- octupole term of L0 and the correction (L127) through the cubic form of n3 ----
-    // n = N'_B - M_B (N'_A / M_A): -1/6 x trace-free part of n3 = M3_B - (M_B / M_A) M3_A.  D3 and D4 are
-    // trace-free, so only this part of n3 matters, and with Q_i = n_ijk R_j R_k, C = Q.R:
-    //   -1/6 n3 :. D3          = d3 C                      (-> L0; the part M_B N'_A/M_A of the source's own
-    //                                                          octupole is added per cell in acc_finish)
-    //   -1/6 n3_jkl D4_ijkl    = d4 C R_i + 3 d3 Q_i       (-> dL1_i; D4_ijkl = d/dR_i D3_jkl, d(d3)/dR_i = d4 R_i)
-    const double nxxx = fma(-m0, tA[0], s[C_OXXX]), nxxy = fma(-m0, tA[1], s[C_OXXY]), nxxz = fma(-m0, tA[2], s[C_OXXZ]);
-    const double nxyy = fma(-m0, tA[3], s[C_OXYY]), nxyz = fma(-m0, tA[4], s[C_OXYZ]);
-    const double nyyy = fma(-m0, tA[5], s[C_OYYY]), nyyz = fma(-m0, tA[6], s[C_OYYZ]);
-    const double nxzz = -(nxxx + nxyy), nyzz = -(nxxy + nyyy);          // trace-free: n_izz = -n_ixx - n_iyy
+    const double Vy = fma(qyz, z, fma(qyy, y, qxy * x));
+    a.l2[3] += fma(vy, y, c1);
+    const double S = fma(z, Vz, fma(y, Vy, x * Vx));
+    a.l3[3] = fma(fyy, z, a.l3[3]);
+    if (DIPOLE) a.l2[3] = fma(hy, y, a.l2[3]);
+    a.l3[6] = fma(e3xy, z, a.l3[6]);
+    const double pb = fma(y, y, -zz);
+    if (DIPOLE) a.l2[1] = fma(hy, x, a.l2[1]);
+    a.l2[4] = fma(vy, z, a.l2[4]);
+    const double k1 = fma(d3, S, c1);
+    const double u2 = d2 + d2;
     const double Qx = fma(nxyz, pyz, fma(nxxz, pxz, fma(nxxy, pxy, fma(nxyy, pb, nxxx * pa))));
+    a.l3[0] = fma(fxx, y, a.l3[0]);
+    a.l1[2] = fma(k1, z, a.l1[2]);
+    a.l2[0] += fma(vx, x, c1);
+    if (DIPOLE) a.l1[0] = fma(d1, m1x, a.l1[0]);
+    a.l0b = fma(d2, S, a.l0b);
+    const double nyzz = -(nxxy + nyyy);
     const double Qy = fma(nyyz, pyz, fma(nxyz, pxz, fma(nxyy, pxy, fma(nyyy, pb, nxxy * pa))));
+    a.l3[1] = fma(fxx, z, a.l3[1]);
     const double Qz = fma(nyzz, pyz, fma(nxzz, pxz, fma(nxyz, pxy, fma(nyyz, pb, nxxz * pa))));
     const double C = fma(z, Qz, fma(y, Qy, x * Qx));
+    a.l1[2] = fma(u2, Vz, a.l1[2]);
+    a.l1[0] = fma(k1, x, a.l1[0]);
+    if (DIPOLE) a.l2[4] = fma(hz, y, a.l2[4]);
+    const double t4 = d3k7 * C;
+    a.l1[1] = fma(k1, y, a.l1[1]);
+    if (DIPOLE) a.l2[2] = fma(hz, x, a.l2[2]);
     a.l0 = fma(d3, C, a.l0);
-    const double t4 = (d3 * (-7.0 * w2)) * C;                           // d4 C,  d4 = -105/r^9
-    const double t3 = 3.0 * d3;
-    a.c[0] = fma(t3, Qx, fma(t4, x, a.c[0]));
-    a.c[1] = fma(t3, Qy, fma(t4, y, a.c[1]));
-    a.c[2] = fma(t3, Qz, fma(t4, z, a.c[2]));
+    a.c[0] = fma(t4, x, a.c[0]);
+    a.c[0] = fma(d3, Qx, a.c[0]);
+    a.c[1] = fma(t4, y, a.c[1]);
+    a.c[1] = fma(d3, Qy, a.c[1]);
+    a.c[2] = fma(t4, z, a.c[2]);
+    if (DIPOLE) a.l2[0] = fma(hx, x, a.l2[0]);
+    a.c[2] = fma(d3, Qz, a.c[2]);
+    a.l1[0] = fma(u2, Vx, a.l1[0]);
+    a.l1[1] = fma(u2, Vy, a.l1[1]);
 }
 
 // Body of one ordered pair A <- B.  (x,y,z) = R = z_A - z_B, w = 1/|R|; s[0..15] staged source
@@ -323,14 +355,25 @@ __device__ __forceinline__ void acc_finish(const Acc& a, const double (&tA)[7], 
     L[0] = a.l0 + a.l0b;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
-        C[i] = CORR ? a.c[i] : 0.0;
-        L[1 + i] = CORR ? a.l1[i] + a.c[i] : a.l1[i];
+        C[i] = CORR ? 3.0 * a.c[i] : 0.0;              // m2l_pair_folded accumulates a third of it
+        L[1 + i] = CORR ? a.l1[i] + C[i] : a.l1[i];
     }
     double l2[5], l3[7];
 #pragma unroll
     for (int i = 0; i < 5; ++i) l2[i] = a.l2[i];
+    double xzz, yzz;
+    if (CORR) {
+        // m2l_pair_folded carries xxy xxz xyy yyz xzz yzz xyz; the repeated-index components follow from the traces
+        l3[1] = a.l3[0]; l3[2] = a.l3[1]; l3[3] = a.l3[2]; l3[6] = a.l3[3]; l3[4] = a.l3[6];
+        xzz = a.l3[4]; yzz = a.l3[5];
+        l3[0] = -(l3[3] + xzz);                        // xxx = -(xyy + xzz)
+        l3[5] = -(l3[1] + yzz);                        // yyy = -(xxy + yzz)
+    } else {
 #pragma unroll
-    for (int i = 0; i < 7; ++i) l3[i] = a.l3[i];
+        for (int i = 0; i < 7; ++i) l3[i] = a.l3[i];
+        xzz = -(l3[0] + l3[3]);                        // xzz = -(xxx + xyy)
+        yzz = -(l3[1] + l3[5]);                        // yzz = -(xxy + yyy)
+    }
     if (CORR) {
         // the sources' octupoles entered L0 only through n = N'_B - M_B tA; the rest, sum_B M_B (tA :. D3(R_B)) =
         // tA :. L3, is added here, with tA taken to the reduced form that contracts with the 7 independent
@@ -348,9 +391,9 @@ __device__ __forceinline__ void acc_finish(const Acc& a, const double (&tA)[7], 
     L[4] = l2[0]; L[5] = l2[1]; L[6] = l2[2]; L[7] = l2[3]; L[8] = l2[4];
     L[9] = -(l2[0] + l2[3]);                           // zz = -(xx + yy)
     L[10] = l3[0]; L[11] = l3[1]; L[12] = l3[2]; L[13] = l3[3]; L[14] = l3[4];
-    L[15] = -(l3[0] + l3[3]);                          // xzz = -(xxx + xyy)
+    L[15] = xzz;
     L[16] = l3[5]; L[17] = l3[6];
-    L[18] = -(l3[1] + l3[5]);                          // yzz = -(xxy + yyy)
+    L[18] = yzz;
     L[19] = -(l3[2] + l3[6]);                          // zzz = -(xxz + yyz)
 }
 

@@ -442,8 +442,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
             for (size_t s2 = 0; s2 < full.size(); ++s2) {
                 const int dx = full[s2].d[0], dy = full[s2].d[1], dz = full[s2].d[2];
                 StEntry e;
-                e.off = (py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1);
-                e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz;
+                e.off = ((py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1)) * 16;   // bytes
+                e.dx = (signed char)(8 * dx); e.dy = (signed char)(8 * dy); e.dz = (signed char)(8 * dz);
                 e.d2 = well_separated((long long)dx * dx + (long long)dy * dy + (long long)dz * dz, cfg->theta) ? 0 : 1;
                 h->entries_mixed[(size_t)p * MAX_LIST + s2] = e;
             }
@@ -464,7 +464,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
             StEntry e;
             // shared-memory offset of the source relative to the thread's base (see kernels.cuh)
             if (cfg->kind == OCTO_FMM_MULTIPOLE) {
-                e.off = (py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1);   // double2 units
+                e.off = ((py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1)) * 16;   // bytes
+                e.dx = (signed char)(8 * dx); e.dy = (signed char)(8 * dy); e.dz = (signed char)(8 * dz);      // see StEntry
                 e.d2 = 0;
             } else {
                 // monopole: offset in the de-interleaved mass tile (doubles, low 16 bits) and index of the offset's
@@ -473,8 +474,8 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
                 const int widx = ((dz + REACH_MAX) * (2 * REACH_MAX + 1) + (dy + REACH_MAX)) * (2 * REACH_MAX + 1) + (dx + REACH_MAX);
                 e.off = (toff & 0xffff) | (widx << 16);
                 e.d2 = (signed char)(dx * dx + dy * dy + dz * dz);
+                e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz;
             }
-            e.dx = (signed char)dx; e.dy = (signed char)dy; e.dz = (signed char)dz;
             h->entries[(size_t)p * MAX_LIST + s] = e;
         }
     }
@@ -520,6 +521,17 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     for (int a = 0; a < 3; ++a) { P.pdim[a] = cfg->n[a] / 2; P.psh[a] = 0; }
     for (int d = 0; d <= 2 * REACH_MAX; ++d) P.hmul[d] = h->hmul[d];
     P.zmin = 0; P.zmax = cfg->n[2] - 1; P.nz_below = 0;
+    for (int pz = 0; pz < 2; ++pz) {       // dz-extent of the lists (Eq. 15 list and leaf-level list) per z-parity of the target
+        int lo = REACH_MAX, hi = -REACH_MAX;
+        for (int c = 4 * pz; c < 4 * pz + 4; ++c)
+            for (int dz = -REACH_MAX; dz <= REACH_MAX; ++dz) {
+                const bool any = h->begin[c][dz + REACH_MAX + 1] > h->begin[c][dz + REACH_MAX] ||
+                                 (cfg->kind == OCTO_FMM_MULTIPOLE && h->begin_mixed[c][dz + REACH_MAX + 1] > h->begin_mixed[c][dz + REACH_MAX]);
+                if (any) { lo = std::min(lo, dz); hi = std::max(hi, dz); }
+            }
+        if (lo > hi) { lo = 0; hi = 0; }
+        P.zr[pz][0] = lo; P.zr[pz][1] = hi;
+    }
     P.nflags[0] = nullptr; P.nflags[1] = nullptr;
 
     if (cfg->kind == OCTO_FMM_MULTIPOLE && !small) {
@@ -1401,24 +1413,36 @@ int octo_fmm_fp64_issue_probe(int device, void* stream, void* scratch, int mode,
     return OCTO_FMM_OK;
 }
 
-int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int* flops, int* fp64_instructions)
+// flops: the ALGORITHMIC count per pair, frozen at the operation list of the round-1 kernels (DFMA = 2,
+// DADD/DMUL = 1) so that rooflines stay comparable from version to version; executed / fp64_instructions: what the
+// hot loops of THIS library execute per pair, counted in their SASS (python -m paper_2101_08226_b200.sass_cost_model).
+static int op_counts(int kind, int am_correction, int dipole_terms, int* flops, int* executed, int* fp64_instructions)
 {
-    // Counted from the operation list of m2l_pair<> + the separation.
-    int f, i;
-    if (kind == OCTO_FMM_MONOPOLE) { f = 8; i = 4; }
+    int f, x, i;
+    if (kind == OCTO_FMM_MONOPOLE) { f = 8; x = 8; i = 4; }
     else if (kind == OCTO_FMM_MULTIPOLE) {
-        // counted in the SASS of the hot loops (cuobjdump), per pair
         if (am_correction) {
-            if (dipole_terms) { f = 224; i = 138; }   // 86 DFMA + 38 DMUL + 14 DADD
-            else              { f = 188; i = 118; }   // 70 DFMA + 34 DMUL + 14 DADD
+            if (dipole_terms) { f = 224; x = 212; i = 130; }   // frozen: 86 DFMA + 38 DMUL + 14 DADD; now 82 + 35 + 13
+            else              { f = 188; x = 180; i = 113; }   // frozen: 70 + 34 + 14; now 67 + 33 + 13
         } else {
-            if (dipole_terms) { f = 202; i = 118; }   // 84 DFMA + 26 DMUL +  8 DADD
-            else              { f = 146; i = 90; }    // 56 DFMA + 26 DMUL +  8 DADD
+            if (dipole_terms) { f = 202; x = 202; i = 118; }   // 84 DFMA + 26 DMUL +  8 DADD
+            else              { f = 146; x = 146; i = 90; }    // 56 DFMA + 26 DMUL +  8 DADD
         }
     } else return OCTO_FMM_EINVAL;
     if (flops) *flops = f;
+    if (executed) *executed = x;
     if (fp64_instructions) *fp64_instructions = i;
     return OCTO_FMM_OK;
+}
+
+int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int* flops, int* fp64_instructions)
+{
+    return op_counts(kind, am_correction, dipole_terms, flops, nullptr, fp64_instructions);
+}
+
+int octo_fmm_executed_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int* executed_flops)
+{
+    return op_counts(kind, am_correction, dipole_terms, nullptr, executed_flops, nullptr);
 }
 
 int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int* fp64_instructions)

@@ -219,7 +219,7 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
 
 // Pair counter of one level, for the bit-exact check of the pair set against the oracle: counts[0] += ordered pairs of the
 // multipole step (both exist, on the Eq. 15 list, not two leaves), counts[1] += leaf-leaf point-mass pairs (leaf-level list).
-// The Eq. 15 list is in the constant bank as (dx, dy, dz) of c_entries, the near field as c_near.
+// The Eq. 15 list is in the constant bank as 8 x (dx, dy, dz) of c_entries (a multipole list), the near field as c_near.
 __global__ void __launch_bounds__(128) tree_count_kernel(const unsigned char* __restrict__ kind, int nx, int ny, int nz,
                                                          unsigned long long* __restrict__ counts)
 {
@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(128) tree_count_kernel(const unsigned char* __
             const int s_end = c_begin[cls][2 * REACH_MAX + 1];
             for (int s = c_begin[cls][0]; s < s_end; ++s) {
                 const StEntry e = c_entries[cls * MAX_LIST + s];
-                const int bi = i + e.dx, bj = j + e.dy, bk = k + e.dz;
+                const int bi = i + (e.dx >> 3), bj = j + (e.dy >> 3), bk = k + (e.dz >> 3);    // multipole lists hold 8 d
                 if (bi < 0 || bj < 0 || bk < 0 || bi >= nx || bj >= ny || bk >= nz) continue;
                 const unsigned char kb = kind[((long long)bk * ny + bj) * nx + bi];
                 if (kb == KIND_ABSENT) continue;
