@@ -308,7 +308,7 @@ struct octo_fmm {
 
 extern "C" {
 
-const char* octo_fmm_version(void) { return "octo_fmm 0.2 (sm_100a)"; }
+const char* octo_fmm_version(void) { return "octo_fmm 0.3 (sm_100a)"; }
 
 size_t octo_fmm_workspace_bytes(const octo_fmm_config* cfg)
 {
