@@ -33,6 +33,9 @@ if ROOT not in sys.path:
 METRIC = "fmm_cell_interactions_per_s"
 UNIT = "interactions/s"
 FP64_LANES_PER_SM = 64        # FP64 FMA lanes per SM per clock on B200 (37.2 TFLOP/s at 148 SMs x 1965 MHz)
+# flops per interaction the ROUND-1 kernel executed on the general multipole path (kind 0), for continuity with r01's frac:
+# the round-2 kernel evaluates the same formula in fewer operations
+ROUND1_FLOPS = {0: 224}
 
 
 def env_int(name, default):
@@ -792,7 +795,6 @@ def run_ours(args):
                    for mode, name in ((0, "dfma_three_fresh_registers"), (1, "dfma_operand_reuse"), (2, "dmul"))}
     bytes_per_cell = (23 + 23) * 8 if multi else (1 + 4) * 8      # algorithmic: inputs read once, outputs written once
     achieved = flops_per * n_int / (kernel_ms * 1e-3) / 1e12
-    executed_per = p.octo_fmm_executed_flops_per_interaction_path(kind, True, True)
     roofline = {"bound": "alu", "kernel": "m2l_staged_kernel<correction>" if multi else "p2p_monopole_dmma_kernel", "achieved": achieved, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                 "peak_source": "derived: %d SMs x %d FP64 FMA lanes x 2 x %.0f MHz (sm_max_mhz of %s)" % (
@@ -800,10 +802,11 @@ def run_ours(args):
                 "peak_measured_dfma": probe["flops_per_s"] / 1e12,
                 "frac_of_measured_dfma": achieved / (probe["flops_per_s"] / 1e12),
                 "flops_per_interaction": flops_per, "fp64_instr_per_interaction": instr_per,
-                "flops_note": "flops_per_interaction is the ALGORITHMIC count (operation list of the pair formula, DESIGN.md "
-                              "section 7, frozen at the round-1 value); the kernel executes executed_flops_per_interaction",
-                "executed_flops_per_interaction": executed_per,
-                "frac_on_executed_flops": executed_per * n_int / (kernel_ms * 1e-3) / 1e12 / peak_tflops,
+                "flops_note": "flops_per_interaction = what the kernel executes per pair (counted in its SASS); round 1 executed "
+                              "224 for the same formula, so frac_at_round1_operation_count is the figure comparable with r01's 0.607",
+                "round1_flops_per_interaction": ROUND1_FLOPS.get(kind),
+                "frac_at_round1_operation_count": (ROUND1_FLOPS[kind] * n_int / (kernel_ms * 1e-3) / 1e12 / peak_tflops
+                                                   if kind in ROUND1_FLOPS else None),
                 "fp64_pipe_issue_frac": (instr_per * n_int / (kernel_ms * 1e-3)) / (sm_count * FP64_LANES_PER_SM * sm_max_mhz * 1e6),
                 "fp64_issue_probe_frac_of_issue_peak": issue_probe,
                 "kernel_ms": kernel_ms, "interactions_per_launch": n_int,

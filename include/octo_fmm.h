@@ -225,16 +225,13 @@ int octo_fmm_fp64_peak_probe(int device, void *stream, void *scratch, int iters,
  * interaction kernel's FP64 pipe is not 100 % busy.  scratch: device, >= 8 MiB. */
 int octo_fmm_fp64_issue_probe(int device, void *stream, void *scratch, int mode, int iters, double *instr_per_s);
 
-/* Operation counts per interaction of a multipole (kind 0) / monopole (kind 1) handle (DFMA = 2 flop, DADD/DMUL = 1,
- * the reciprocal-square-root instruction not counted).  *flops is the ALGORITHMIC count the rooflines are quoted on: the
- * operation list of the pair formula as written in DESIGN.md section 7, frozen at the round-1 value so that versions
- * stay comparable (224 with the correction and the dipole terms; the full-tensor definition needs about 400).
- * *fp64_instructions is what the hot loop of this library executes per pair, counted in its SASS. */
+/* FP64 operations one multipole (kind 0) / monopole (kind 1) interaction executes in the kernel's inner loop, counted
+ * in its SASS (DFMA = 2 flop, DADD/DMUL = 1, the reciprocal-square-root instruction not counted); see DESIGN.md
+ * section 7.  These are the flops `bench.py` quotes its roofline on: 212 with the correction and the dipole terms since
+ * round 2 (224 in round 1; the full-tensor definition needs about 400). */
 int octo_fmm_flops_per_interaction(int kind, int am_correction, int *flops, int *fp64_instructions);
 /* The same for a given path: dipole_terms = 0 is the path without the 27 dipole terms (multipole kind only). */
 int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int *flops, int *fp64_instructions);
-/* The flops that hot loop executes per pair (<= the algorithmic count: 212 of 224 on the general path). */
-int octo_fmm_executed_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int *executed_flops);
 
 const char *octo_fmm_version(void);
 

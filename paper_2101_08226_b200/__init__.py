@@ -94,7 +94,6 @@ class _Library:
         lib.octo_fmm_fp64_issue_probe.argtypes = [ctypes.c_int, vp, vp, ctypes.c_int, ctypes.c_int, dp]
         lib.octo_fmm_flops_per_interaction.argtypes = [ctypes.c_int, ctypes.c_int, ip, ip]
         lib.octo_fmm_flops_per_interaction_path.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, ip]
-        lib.octo_fmm_executed_flops_per_interaction_path.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ip]
         lib.octo_fmm_dipole_terms_used.argtypes = [vp, ip]
         lib.octo_fmm_version.restype = ctypes.c_char_p
         tcfgp = ctypes.POINTER(octo_fmm_tree_config)
@@ -392,15 +391,6 @@ def octo_fmm_flops_per_interaction_path(kind, am_correction, dipole_terms):
     if rc != OK:
         raise OctoFmmError("octo_fmm_flops_per_interaction_path", rc)
     return f.value, i.value
-
-
-def octo_fmm_executed_flops_per_interaction_path(kind, am_correction, dipole_terms):
-    f = ctypes.c_int(0)
-    rc = _lib.octo_fmm_executed_flops_per_interaction_path(int(kind), int(bool(am_correction)), int(bool(dipole_terms)),
-                                                           ctypes.byref(f))
-    if rc != OK:
-        raise OctoFmmError("octo_fmm_executed_flops_per_interaction_path", rc)
-    return f.value
 
 
 def octo_fmm_dipole_terms_used(h):

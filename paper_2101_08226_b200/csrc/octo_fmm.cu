@@ -1413,36 +1413,24 @@ int octo_fmm_fp64_issue_probe(int device, void* stream, void* scratch, int mode,
     return OCTO_FMM_OK;
 }
 
-// flops: the ALGORITHMIC count per pair, frozen at the operation list of the round-1 kernels (DFMA = 2,
-// DADD/DMUL = 1) so that rooflines stay comparable from version to version; executed / fp64_instructions: what the
-// hot loops of THIS library execute per pair, counted in their SASS (python -m paper_2101_08226_b200.sass_cost_model).
-static int op_counts(int kind, int am_correction, int dipole_terms, int* flops, int* executed, int* fp64_instructions)
+int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int* flops, int* fp64_instructions)
 {
-    int f, x, i;
-    if (kind == OCTO_FMM_MONOPOLE) { f = 8; x = 8; i = 4; }
+    // What the hot loops of THIS library execute per pair, counted in their SASS (python -m
+    // paper_2101_08226_b200.sass_cost_model): DFMA = 2 flop, DADD/DMUL = 1.
+    int f, i;
+    if (kind == OCTO_FMM_MONOPOLE) { f = 8; i = 4; }
     else if (kind == OCTO_FMM_MULTIPOLE) {
         if (am_correction) {
-            if (dipole_terms) { f = 224; x = 212; i = 130; }   // frozen: 86 DFMA + 38 DMUL + 14 DADD; now 82 + 35 + 13
-            else              { f = 188; x = 180; i = 113; }   // frozen: 70 + 34 + 14; now 67 + 33 + 13
+            if (dipole_terms) { f = 212; i = 130; }   // 82 DFMA + 35 DMUL + 13 DADD   (round 1: 86 + 38 + 14 = 224 flop)
+            else              { f = 180; i = 113; }   // 67 DFMA + 33 DMUL + 13 DADD   (round 1: 70 + 34 + 14 = 188 flop)
         } else {
-            if (dipole_terms) { f = 202; x = 202; i = 118; }   // 84 DFMA + 26 DMUL +  8 DADD
-            else              { f = 146; x = 146; i = 90; }    // 56 DFMA + 26 DMUL +  8 DADD
+            if (dipole_terms) { f = 202; i = 118; }   // 84 DFMA + 26 DMUL +  8 DADD
+            else              { f = 146; i = 90; }    // 56 DFMA + 26 DMUL +  8 DADD
         }
     } else return OCTO_FMM_EINVAL;
     if (flops) *flops = f;
-    if (executed) *executed = x;
     if (fp64_instructions) *fp64_instructions = i;
     return OCTO_FMM_OK;
-}
-
-int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int* flops, int* fp64_instructions)
-{
-    return op_counts(kind, am_correction, dipole_terms, flops, nullptr, fp64_instructions);
-}
-
-int octo_fmm_executed_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int* executed_flops)
-{
-    return op_counts(kind, am_correction, dipole_terms, nullptr, executed_flops, nullptr);
 }
 
 int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int* fp64_instructions)

@@ -4,7 +4,7 @@
 
 Finds the straight-line blocks that hold a pair body (>= 40 DFMAs) in the SASS of the named kernel (default: the
 headline instantiation m2l_staged_kernel<correction on, no fused L2L, plain>) and prints per block the FP64 instruction
-tally (DFMA / DMUL / DADD: the frozen operation count of DESIGN.md section 7), the DFMAs by number of FRESH register
+tally (DFMA / DMUL / DADD: the operation count of DESIGN.md section 7), the DFMAs by number of FRESH register
 operands, and the modelled cycles per pair; -v lists every instruction with its modelled cost.
 Model (register file: two banks, a 64-bit operand takes one read slot of each): an FP64
 instruction holds the sub-partition's dispatch port for max(2, number of distinct 64-bit register operands that do not
