@@ -63,8 +63,8 @@ def test_slabs_match_the_oracle_and_the_whole_grid(world):
     assert HALO == 8
 
 
-@pytest.mark.parametrize("world,theta", [(2, 0.5), (4, 0.5), (3, 0.35)])
-def test_peer_memory_halos_in_one_process(world, theta):
+@pytest.mark.parametrize("heights,theta", [((16, 16), 0.5), ((16, 16, 16, 16), 0.5), ((16, 16, 16), 0.35), ((8, 24, 16), 0.5)])
+def test_peer_memory_halos_in_one_process(heights, theta):
     """octo_fmm_set_neighbours: every slab has a handle of its own that stages only its own layers; interact() fetches
     the neighbours' layers through their staged arrays.  Bit-identical to one handle over the whole grid; matches the
     ORACLE on the layers next to the cuts; counts add up; one slab WITHOUT dipole moments next to one WITH them takes
@@ -73,8 +73,10 @@ def test_peer_memory_halos_in_one_process(world, theta):
     from paper_2101_08226_b200 import build
     build.build()
     import paper_2101_08226_b200 as p
-    nzl = 16
-    nz = nzl * world
+    world = len(heights)                              # slabs of unequal height too: a neighbour's layer index differs from mine
+    z0s = [sum(heights[:r]) for r in range(world)]
+    nz = sum(heights)
+    nzl = heights[0]
     w = fi.config2(ncell=64)
     hm = np.ascontiguousarray(w.moments[:, :nz, :32, :32])
     hc = np.ascontiguousarray(w.com_off[:, :nz, :32, :32])
@@ -85,11 +87,11 @@ def test_peer_memory_halos_in_one_process(world, theta):
     whole = p.OctoFMM(n, w.h, theta, p.MULTIPOLE, True)
     whole.set_option("kernel", 0)
     Lw, Cw = whole.solve(mom, com)
-    slabs = [p.OctoFMM((32, 32, nzl), w.h, theta, p.MULTIPOLE, True) for _ in range(world)]
+    slabs = [p.OctoFMM((32, 32, heights[r]), w.h, theta, p.MULTIPOLE, True) for r in range(world)]
     for r, s in enumerate(slabs):
         s.set_option("kernel", 0)
         s.set_neighbours(slabs[r - 1] if r > 0 else None, slabs[r + 1] if r < world - 1 else None)
-        s.set_moments(mom[:, r * nzl:(r + 1) * nzl].contiguous(), com[:, r * nzl:(r + 1) * nzl].contiguous())
+        s.set_moments(mom[:, z0s[r]:z0s[r] + heights[r]].contiguous(), com[:, z0s[r]:z0s[r] + heights[r]].contiguous())
     torch.cuda.synchronize()
     total = 0
     for r, s in enumerate(slabs):
@@ -98,11 +100,11 @@ def test_peer_memory_halos_in_one_process(world, theta):
         torch.cuda.synchronize()
         assert s.status() == p.OK
         assert s.dipole_terms_used()                 # slab 0 has none of its own: it takes the terms for its neighbour's
-        own = slice(r * nzl, (r + 1) * nzl)
+        own = slice(z0s[r], z0s[r] + heights[r])
         assert torch.equal(L, Lw[:, own]) and torch.equal(C, Cw[:, own])
         Lh, Ch = L.cpu().numpy(), C.cpu().numpy()
-        for z0 in (0, nzl - 8):
-            glo, ghi = (8, 8, r * nzl + z0), (24, 24, r * nzl + z0 + 8)
+        for z0 in sorted({0, heights[r] - 8}):
+            glo, ghi = (8, 8, z0s[r] + z0), (24, 24, z0s[r] + z0 + 8)
             Lr, Lcr, _ = oracle.interact_multipole(n, w.h, theta, hm, hc, glo, ghi, True)
             sl = (slice(None), slice(z0, z0 + 8), slice(8, 24), slice(8, 24))
             assert parity_error(Lh[sl], Lr) < 1e-12 and np.abs(Ch[sl] - Lcr).max() <= 1e-12 * np.abs(Lr[1:4]).max()
