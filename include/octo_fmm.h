@@ -53,7 +53,8 @@ extern "C" {
 typedef struct octo_fmm octo_fmm_t; /* opaque handle */
 
 enum { OCTO_FMM_OK = 0, OCTO_FMM_EINVAL = 1, OCTO_FMM_ESTATE = 2, OCTO_FMM_ENOMEM = 3, OCTO_FMM_ECUDA = 4,
-       OCTO_FMM_EMASS = 5 /* am_correction with a target cell of mass <= 0 (division M_B/M_A, L127) */ };
+       OCTO_FMM_EMASS = 5 /* am_correction with a target cell of mass <= 0 (division M_B/M_A, L127) */,
+       OCTO_FMM_ESIZE = 6 /* octo_fmm_interact_static: the grid has more cells than OCTO_FMM_STATIC_MAX_CELLS */ };
 enum { OCTO_FMM_MULTIPOLE = 0, OCTO_FMM_MONOPOLE = 1 };
 
 typedef struct {
@@ -234,6 +235,29 @@ int octo_fmm_flops_per_interaction(int kind, int am_correction, int *flops, int 
 int octo_fmm_flops_per_interaction_path(int kind, int am_correction, int dipole_terms, int *flops, int *fp64_instructions);
 
 const char *octo_fmm_version(void);
+
+/* ---- the interaction step WITHOUT any allocation ------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it) and have no workspace to lend: the same step as octo_fmm_set_moments + octo_fmm_interact (PAPER.md L125-137,
+ * multipole kind), one call, with its scratch (staged sources, flag words) in a static device array inside the library.
+ * The library holds that array, OCTO_FMM_STATIC_MAX_CELLS x 344 bytes + 1.3 KB = 11.3 MB, on every GPU that loads it,
+ * until the process exits.  The call allocates no device memory: no cudaMalloc / cudaFree / allocating library routine;
+ * a call with a configuration other than the previous one's on that device builds a new handle in HOST memory and
+ * first waits for the previous configuration's stream.
+ *   cfg: as for octo_fmm_create (n multiples of 8, theta, h, am_correction, out_lo/out_hi, device, stream), kind =
+ *   OCTO_FMM_MULTIPOLE; workspace and workspace_bytes are ignored.  moments [20][nz][ny][nx], com_off [3][nz][ny][nx]
+ *   (NULL: geometric centres), L [20][out cells], Lcorr [3][out cells] or NULL: DEVICE pointers of the caller,
+ *   borrowed for the call; the results are complete when cfg->stream has run the two kernels (the call does not wait).
+ * Errors: OCTO_FMM_ESIZE if n[0] n[1] n[2] > OCTO_FMM_STATIC_MAX_CELLS (nothing is launched); EINVAL for a bad
+ * configuration, the monopole kind or null moments / L; ECUDA.  octo_fmm_static_status(device) synchronises the stream
+ * of the last call on that device and reports EMASS like octo_fmm_status (ESTATE before the first call).
+ * EVERY call on a device shares the one array, which keeps the contents of the call before (the call clears what must
+ * start at zero): calls serialise on the host, but two calls whose kernels OVERLAP on the GPU -- different streams
+ * without an ordering between them -- race on it.  One stream, or an event between the calls. */
+#define OCTO_FMM_STATIC_MAX_CELLS 32768 /* e.g. 32 x 32 x 32 */
+int octo_fmm_static_max_cells(void);
+int octo_fmm_interact_static(const octo_fmm_config *cfg, const double *moments, const double *com_off, double *L, double *Lcorr);
+int octo_fmm_static_status(int device);
 
 /* ---- complete uniform-grid solve ------------------------------------
  * "The multipoles of each cell are composed of the multipoles of its child cells ... The expansion of

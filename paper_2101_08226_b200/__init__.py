@@ -16,9 +16,10 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libocto_fmm.so")
 
-OK, EINVAL, ESTATE, ENOMEM, ECUDA, EMASS = 0, 1, 2, 3, 4, 5
+OK, EINVAL, ESTATE, ENOMEM, ECUDA, EMASS, ESIZE = 0, 1, 2, 3, 4, 5, 6
 MULTIPOLE, MONOPOLE = 0, 1
-_STATUS = {0: "OK", 1: "EINVAL", 2: "ESTATE", 3: "ENOMEM", 4: "ECUDA", 5: "EMASS"}
+_STATUS = {0: "OK", 1: "EINVAL", 2: "ESTATE", 3: "ENOMEM", 4: "ECUDA", 5: "EMASS",
+           6: "ESIZE: more cells than the static scratch of octo_fmm_interact_static holds"}
 
 
 class OctoFmmError(RuntimeError):
@@ -96,6 +97,9 @@ class _Library:
         lib.octo_fmm_flops_per_interaction_path.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ip, ip]
         lib.octo_fmm_dipole_terms_used.argtypes = [vp, ip]
         lib.octo_fmm_version.restype = ctypes.c_char_p
+        lib.octo_fmm_static_max_cells.argtypes = []
+        lib.octo_fmm_interact_static.argtypes = [cfgp, vp, vp, vp, vp]
+        lib.octo_fmm_static_status.argtypes = [ctypes.c_int]
         tcfgp = ctypes.POINTER(octo_fmm_tree_config)
         vpp = ctypes.POINTER(ctypes.c_void_p)
         lib.octo_fmm_tree_workspace_bytes.restype = ctypes.c_size_t
@@ -336,6 +340,21 @@ def octo_fmm_ipc_close(base):
     rc = _lib.octo_fmm_ipc_close(ctypes.c_void_p(int(base)))
     if rc != OK:
         raise OctoFmmError("octo_fmm_ipc_close", rc)
+
+
+def octo_fmm_static_max_cells():
+    return int(_lib.octo_fmm_static_max_cells())
+
+
+def octo_fmm_interact_static(cfg, moments, com_off, L, Lcorr=None):
+    """The step without any allocation: scratch in the library's static device array (octo_fmm.h)."""
+    rc = _lib.octo_fmm_interact_static(ctypes.byref(cfg), _ptr(moments), _ptr(com_off), _ptr(L), _ptr(Lcorr))
+    if rc != OK:
+        raise OctoFmmError("octo_fmm_interact_static", rc)
+
+
+def octo_fmm_static_status(device=0):
+    return int(_lib.octo_fmm_static_status(int(device)))
 
 
 def octo_fmm_run_host(h, moments_host, com_off_host, L_host, Lcorr_host, scratch, scratch_bytes):

@@ -1438,6 +1438,80 @@ int octo_fmm_flops_per_interaction(int kind, int am_correction, int* flops, int*
     return octo_fmm_flops_per_interaction_path(kind, am_correction, 1, flops, fp64_instructions);
 }
 
+// ---- the entry point that allocates nothing (octo_fmm.h: octo_fmm_interact_static) ----
+// Its scratch -- the staged sources, the flag words, and the result slots a handle's workspace has -- lives in ONE
+// file-scope device array: every GPU that loads the library holds these bytes until the process exits.  In host code
+// the NAME of the array is a host-side stand-in, not a device address; the address is taken once per device, with that
+// device current, by cudaGetSymbolAddress (below) and only that pointer is handed to kernels and to the tensor map.
+constexpr size_t STATIC_SCRATCH_BYTES =
+    ((size_t)OCTO_FMM_STATIC_MAX_CELLS * (NPAIR * 2 + 20 + 3) * sizeof(double) + 4 * ALIGN + ALIGN - 1) / ALIGN * ALIGN;
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_SCRATCH_BYTES];
+
+struct StaticPath {
+    void* scratch = nullptr;       // device address of g_static_scratch on this device
+    octo_fmm* h = nullptr;         // handle over the scratch for the configuration of the last call (host memory only)
+    octo_fmm_config key{};
+};
+static StaticPath g_static[MAX_DEVICES];
+static std::mutex g_static_mu;
+
+static bool same_static_config(const octo_fmm_config& a, const octo_fmm_config& b)
+{
+    for (int c = 0; c < 3; ++c)
+        if (a.n[c] != b.n[c] || a.out_lo[c] != b.out_lo[c] || a.out_hi[c] != b.out_hi[c]) return false;
+    return a.h == b.h && a.theta == b.theta && a.kind == b.kind && a.am_correction == b.am_correction && a.device == b.device &&
+           a.stream == b.stream;
+}
+
+int octo_fmm_static_max_cells(void) { return OCTO_FMM_STATIC_MAX_CELLS; }
+
+int octo_fmm_interact_static(const octo_fmm_config* cfg, const double* moments, const double* com_off, double* L, double* Lcorr)
+{
+    if (!cfg || !moments || !L || cfg->kind != OCTO_FMM_MULTIPOLE || !config_ok(cfg)) return OCTO_FMM_EINVAL;
+    const long long ncell = (long long)cfg->n[0] * cfg->n[1] * cfg->n[2];
+    if (ncell > OCTO_FMM_STATIC_MAX_CELLS) return OCTO_FMM_ESIZE;
+    octo_fmm_config c = *cfg;
+    c.workspace = nullptr; c.workspace_bytes = 0;
+    if (sizes_of(c).total > STATIC_SCRATCH_BYTES) return OCTO_FMM_ESIZE;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || c.device < 0 || c.device >= ndev || c.device >= MAX_DEVICES) return OCTO_FMM_ECUDA;
+    if (cudaSetDevice(c.device) != cudaSuccess) return OCTO_FMM_ECUDA;
+    std::lock_guard<std::mutex> guard(g_static_mu);
+    StaticPath& sp = g_static[c.device];
+    if (!sp.scratch) {         // set-up, once per device, with that device current
+        void* ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return OCTO_FMM_ECUDA; }
+        if ((uintptr_t)ptr % ALIGN) return OCTO_FMM_ECUDA;
+        sp.scratch = ptr;
+    }
+    if (!sp.h || !same_static_config(sp.key, c)) {
+        // another configuration: a new handle over the same scratch (host memory only; the old one is drained first,
+        // its kernels still read the array)
+        if (sp.h) { octo_fmm* old = sp.h; sp.h = nullptr; if (octo_fmm_destroy(old) != OCTO_FMM_OK) return OCTO_FMM_ECUDA; }
+        c.workspace = sp.scratch; c.workspace_bytes = STATIC_SCRATCH_BYTES;
+        octo_fmm* h = nullptr;
+        const int rc = create_internal(&c, 0, &h);
+        if (rc != OCTO_FMM_OK) return rc;
+        sp.h = h; sp.key = c;
+    }
+    octo_fmm* h = sp.h;
+    int rc = octo_fmm_bind_outputs(h, L, Lcorr);
+    if (rc != OCTO_FMM_OK) return rc;
+    // the array keeps the last call's contents: the two flag words start at zero, every staged record of the grid is
+    // rewritten by the staging kernel, and nothing outside the grid is read (TMA zero-fills / explicit in-grid tests)
+    if (cudaMemsetAsync(h->flags, 0, 2 * sizeof(int), h->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if ((rc = octo_fmm_set_moments(h, moments, com_off)) != OCTO_FMM_OK) return rc;
+    return octo_fmm_interact(h);
+}
+
+int octo_fmm_static_status(int device)
+{
+    if (device < 0 || device >= MAX_DEVICES) return OCTO_FMM_EINVAL;
+    std::lock_guard<std::mutex> guard(g_static_mu);
+    if (!g_static[device].h) return OCTO_FMM_ESTATE;
+    return octo_fmm_status(g_static[device].h);
+}
+
 }  // extern "C"
 
 #include "solver.inl"
