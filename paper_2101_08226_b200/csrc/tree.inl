@@ -32,6 +32,9 @@ struct TreeLevel {
     // own, side by side with those of the other levels; the L2L / leaf-finish chain on the caller's stream waits for them
     cudaStream_t s_m2l, s_leaf;
     cudaEvent_t ev_m2l, ev_leaf;
+    bool m2l_on_main;                  // few bricks (a level near the top): its multipole step runs in the main stream's chain
+    cudaEvent_t ev_rdy;                // on the main stream: this level's raw moments and leaf masses are there (upward pass)
+    cudaEvent_t ev_par;                // on the main stream: the PARENT level's expansions are complete (leaf finish may start)
     size_t cells() const { return (size_t)n[0] * n[1] * n[2]; }
 };
 
@@ -97,7 +100,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.h = cfg.h0 / (double)(1LL << l);
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
-        L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr;
+        L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr; L.ev_par = nullptr; L.ev_rdy = nullptr;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
         L.has_refined = L.has_leaf = false;
@@ -233,7 +236,10 @@ struct octo_fmm_tree {
     std::vector<TreeLevel> lev;        // tree levels, coarsest first
     std::vector<SolverLevel> up;       // uniform levels n0/2, ..., 2
     unsigned long long* counts;        // device [3]: m2l, p2p, cross
-    cudaStream_t stream;
+    cudaStream_t stream;               // the solve's own main stream (high priority): upward pass, uniform levels, L2L chain
+    cudaStream_t pool_m2l[3], pool_leaf[2];   // the levels share a few side streams (see octo_fmm_tree_create)
+    cudaStream_t user;                 // the caller's stream (cfg.stream): a solve starts after and is joined into it
+    cudaEvent_t ev_user;               // hand-over between the two
     cudaEvent_t ev_up;                 // the upward pass of a solve is complete
     bool solved;
 };
@@ -258,12 +264,16 @@ int octo_fmm_tree_destroy(octo_fmm_tree_t* t)
     for (SolverLevel& l : t->up)
         if (l.fmm && octo_fmm_destroy(l.fmm) != OCTO_FMM_OK) rc = OCTO_FMM_ECUDA;
     for (TreeLevel& l : t->lev) {
-        if (l.s_m2l) cudaStreamDestroy(l.s_m2l);
-        if (l.s_leaf) cudaStreamDestroy(l.s_leaf);
         if (l.ev_m2l) cudaEventDestroy(l.ev_m2l);
         if (l.ev_leaf) cudaEventDestroy(l.ev_leaf);
+        if (l.ev_par) cudaEventDestroy(l.ev_par);
+        if (l.ev_rdy) cudaEventDestroy(l.ev_rdy);
     }
     if (t->ev_up) cudaEventDestroy(t->ev_up);
+    if (t->ev_user) cudaEventDestroy(t->ev_user);
+    for (cudaStream_t& q : t->pool_m2l) if (q) cudaStreamDestroy(q);
+    for (cudaStream_t& q : t->pool_leaf) if (q) cudaStreamDestroy(q);
+    if (t->stream) cudaStreamDestroy(t->stream);
     delete t;
     return rc;
 }
@@ -280,11 +290,37 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     octo_fmm_tree* t = new (std::nothrow) octo_fmm_tree();
     if (!t) return OCTO_FMM_ENOMEM;
     t->cfg = *cfg;
-    t->stream = (cudaStream_t)cfg->stream;
+    t->user = (cudaStream_t)cfg->stream;
+    t->stream = nullptr;
     t->solved = false;
-    t->ev_up = nullptr;
+    t->ev_up = nullptr; t->ev_user = nullptr;
     t->lev = std::move(P.lev);
-    const octo_fmm_solver_config sc = as_solver_config(*cfg);
+    // Streams.  The multipole steps of the levels are long CTAs that fill every SM (one per SM, 100 us each); whatever
+    // else a solve launches is short and must not queue behind them: it runs on streams of the HIGHEST priority (the
+    // block scheduler hands a freed SM to them first), the multipole steps on streams of the lowest.
+    int prio_least = 0, prio_greatest = 0;
+    if (cudaDeviceGetStreamPriorityRange(&prio_least, &prio_greatest) != cudaSuccess ||
+        cudaStreamCreateWithPriority(&t->stream, cudaStreamNonBlocking, prio_greatest) != cudaSuccess ||
+        cudaEventCreateWithFlags(&t->ev_user, cudaEventDisableTiming) != cudaSuccess) { octo_fmm_tree_destroy(t); return OCTO_FMM_ECUDA; }
+    // FEW side streams, shared by the levels (three for the multipole steps, leaf stream l % 2): a device runs only a
+    // handful of hardware work queues (8 by default), and streams beyond that number alias onto the same queue -- with one
+    // stream pair per level (19 streams at 9 levels) a level's multipole step started only when ANOTHER level's had
+    // ended.
+    for (cudaStream_t& q : t->pool_m2l)
+        if (cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_least) != cudaSuccess) { octo_fmm_tree_destroy(t); return OCTO_FMM_ECUDA; }
+    // (the leaf streams one step below the main stream: the short L2L chain must not queue behind a leaf finish)
+    const int prio_leaf = prio_greatest < prio_least ? prio_greatest + 1 : prio_greatest;
+    for (cudaStream_t& q : t->pool_leaf)
+        if (cudaStreamCreateWithPriority(&q, cudaStreamNonBlocking, prio_leaf) != cudaSuccess) { octo_fmm_tree_destroy(t); return OCTO_FMM_ECUDA; }
+    // multipole streams: the levels with at least one brick per SM take turns on the three, SHALLOWEST first (the L2L chain
+    // goes down the tree: what is left when the last multipole step ends is then one level's L2L and two leaf finishes);
+    // the small levels at the top run inside the main stream's chain, which needs them first anyway
+    int big_rank = 0;
+    std::vector<int> m2l_stream(t->lev.size(), -1);
+    for (size_t l = 0; l < t->lev.size(); ++l)
+        if (t->lev[l].n_m2l_tiles >= 148) m2l_stream[l] = big_rank++ % 3;
+    octo_fmm_solver_config sc = as_solver_config(*cfg);
+    sc.stream = t->stream;
     char* w = (char*)cfg->workspace;
     cudaStream_t st = t->stream;
     int rc = OCTO_FMM_OK;
@@ -303,10 +339,13 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
             rc = OCTO_FMM_ECUDA;
             break;
         }
-        if (cudaStreamCreateWithFlags(&L.s_m2l, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaStreamCreateWithFlags(&L.s_leaf, cudaStreamNonBlocking) != cudaSuccess ||
+        L.m2l_on_main = m2l_stream[l] < 0;
+        L.s_m2l = L.m2l_on_main ? t->stream : t->pool_m2l[m2l_stream[l]];
+        L.s_leaf = t->pool_leaf[l % 2];
+        if (cudaEventCreateWithFlags(&L.ev_rdy, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&L.ev_m2l, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&L.ev_leaf, cudaEventDisableTiming) != cudaSuccess) { rc = OCTO_FMM_ECUDA; break; }
+            cudaEventCreateWithFlags(&L.ev_leaf, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&L.ev_par, cudaEventDisableTiming) != cudaSuccess) { rc = OCTO_FMM_ECUDA; break; }
         if (L.has_refined) {
             octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
             mc.stream = L.s_m2l;
@@ -356,11 +395,24 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
 
 // rhs2 (second right-hand side, L81-83): the sources are d(mass)/dt, expanded about the centres the last solve left in the
 // off arrays (M2M with GIVEN centres), no correction; out[l] is then [cells]: the potential only.
+// hand-over between the caller's stream and the solve's main stream
+static int tree_enter(octo_fmm_tree_t* t)
+{
+    return cudaEventRecord(t->ev_user, t->user) == cudaSuccess && cudaStreamWaitEvent(t->stream, t->ev_user, 0) == cudaSuccess
+               ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
+}
+static int tree_leave(octo_fmm_tree_t* t)
+{
+    return cudaEventRecord(t->ev_user, t->stream) == cudaSuccess && cudaStreamWaitEvent(t->user, t->ev_user, 0) == cudaSuccess
+               ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
+}
+
 static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double* const* out, bool count, bool rhs2 = false)
 {
     const int D = (int)t->lev.size();
     cudaStream_t st = t->stream;
     int rc;
+    if ((rc = tree_enter(t)) != OCTO_FMM_OK) return rc;
     // the level handles run without the correction for the second right-hand side (it belongs to the force, L127)
     struct CorrGuard {
         octo_fmm_tree_t* t; bool on; std::vector<int> keep;
@@ -397,24 +449,28 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         // (the offsets of the cells that are not refined are zero for both right-hand sides: rewriting them is harmless)
         tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        // this level's multipole step and leaf sums need nothing of the coarser levels: they may start now
+        if (cudaEventRecord(L.ev_rdy, st) != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     // ---- side by side, each level on streams of its own: staging + multipole step (its own level only; the parent's
     //      expansion comes in the chain below), and the leaf-leaf point-mass sums ----
     if (cudaEventRecord(t->ev_up, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    auto multipole_step = [&](TreeLevel& L) -> int {
+        if (cudaStreamWaitEvent(L.s_m2l, L.ev_rdy, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+        int r = octo_fmm_set_moments(L.fmm, L.raw, L.off);
+        if (r != OCTO_FMM_OK) return r;
+        const long long nc = (long long)L.cells();
+        stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_m2l>>>(L.kind, L.fmm->src, L.n[0], L.n[1], L.n[2]);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        clear_parent(L.fmm);
+        if ((r = octo_fmm_interact(L.fmm)) != OCTO_FMM_OK) return r;
+        return cudaEventRecord(L.ev_m2l, L.s_m2l) == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
+    };
     for (int l = 0; l < D; ++l) {
         TreeLevel& L = t->lev[l];
-        if (L.fmm && L.n_m2l_tiles > 0) {
-            if (cudaStreamWaitEvent(L.s_m2l, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
-            if ((rc = octo_fmm_set_moments(L.fmm, L.raw, L.off)) != OCTO_FMM_OK) return rc;
-            const long long nc = (long long)L.cells();
-            stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_m2l>>>(L.kind, L.fmm->src, L.n[0], L.n[1], L.n[2]);
-            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
-            clear_parent(L.fmm);
-            if ((rc = octo_fmm_interact(L.fmm)) != OCTO_FMM_OK) return rc;
-            if (cudaEventRecord(L.ev_m2l, L.s_m2l) != cudaSuccess) return OCTO_FMM_ECUDA;
-        }
+        if (L.fmm && L.n_m2l_tiles > 0 && !L.m2l_on_main && (rc = multipole_step(L)) != OCTO_FMM_OK) return rc;
         if (L.leaf) {
-            if (cudaStreamWaitEvent(L.s_leaf, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+            if (cudaStreamWaitEvent(L.s_leaf, L.ev_rdy, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
             if ((rc = octo_fmm_set_moments(L.leaf, L.lm, nullptr)) != OCTO_FMM_OK) return rc;
             double* const keep = L.leaf->outL;
             if (!rhs2) L.leaf->outL = out[l];          // second right-hand side: the four sums go to the handle's own buffer
@@ -464,8 +520,11 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     if (count && cudaMemsetAsync(t->counts, 0, 3 * sizeof(unsigned long long), st) != cudaSuccess) return OCTO_FMM_ECUDA;
-    // ---- the chain on the caller's stream, coarsest level first: L2L into the refined cells, then the leaf finish ----
-    octo_fmm* const hb = t->up[0].fmm;      // a multipole handle on the caller's stream: the bank's book-keeping for the chain
+    // ---- the chain on the caller's stream, coarsest level first: L2L into the REFINED cells of each level (21 us per
+    //      level).  The leaf finish of a level (66 us) needs its parent level's finished expansions, its own multipole
+    //      step at the LEAF cells (which the L2L of its own level does not touch) and its leaf-leaf sums: it runs on the
+    //      level's leaf stream, beside the chain and the finishes of the other levels ----
+    octo_fmm* const hb = t->up[0].fmm;      // a multipole handle of the tree's theta: the bank's book-keeping for the finishes
     for (int l = 0; l < D; ++l) {
         TreeLevel& L = t->lev[l];
         // parent arrays of this level: the tree level above, or the finest uniform level
@@ -480,7 +539,11 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         }
         if (!pL && (L.has_refined || L.has_leaf)) return OCTO_FMM_ESTATE;
         const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
-        if (L.fmm && L.n_m2l_tiles > 0) {
+        // here the caller's stream holds the parent's finished expansions (and, for level 0, the cleared counters)
+        if (cudaEventRecord(L.ev_par, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+        const bool own_step = L.fmm && L.n_m2l_tiles > 0;
+        if (own_step && L.m2l_on_main && (rc = multipole_step(L)) != OCTO_FMM_OK) return rc;
+        if (own_step) {
             if (cudaStreamWaitEvent(st, L.ev_m2l, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
             TreeL2LArgs q;
             for (int c = 0; c < 3; ++c) { q.n[c] = L.n[c]; q.pn[c] = pn[c]; q.psh[c] = L.psh[c]; }
@@ -488,10 +551,19 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             tree_l2l_kernel<<<blocks, 128, 0, st>>>(q);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
         }
-        if (L.leaf && cudaStreamWaitEvent(st, L.ev_leaf, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
-        // leaf finish (also zeroes the cells of out[l] that are not leaves); reads the near field from the constant bank
+        // leaf finish on the level's leaf stream, behind its leaf-leaf sums (also zeroes the cells of out[l] that are not
+        // leaves); reads the near field from the constant bank
         {
+            cudaStream_t sf = L.s_leaf;
+            if (cudaStreamWaitEvent(sf, L.ev_par, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+            if (!L.leaf && cudaStreamWaitEvent(sf, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;   // nothing else ordered it yet
+            if (own_step && cudaStreamWaitEvent(sf, L.ev_m2l, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
             BankLock guard(hb);
+            struct OnStream {          // the bank's book-keeping goes by the handle's stream: lend it the finish's stream
+                octo_fmm* h; cudaStream_t keep;
+                OnStream(octo_fmm* h_, cudaStream_t s) : h(h_), keep(h_->stream) { h->stream = s; }
+                ~OnStream() { h->stream = keep; }
+            } lend(hb, sf);
             if (bank_acquire(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
             TreeFinishArgs a;
             std::memset(&a, 0, sizeof a);
@@ -508,15 +580,20 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             }
             if (l > 0) { a.kind_c = t->lev[l - 1].kind; a.mass_c = t->lev[l - 1].lm; }
             a.count = count ? t->counts : nullptr;
-            tree_leaf_finish_kernel<<<blocks, 128, 0, st>>>(a);
+            tree_leaf_finish_kernel<<<blocks, 128, 0, sf>>>(a);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
             if (count) {
-                tree_count_kernel<<<blocks, 128, 0, st>>>(L.kind, L.n[0], L.n[1], L.n[2], t->counts);
+                tree_count_kernel<<<blocks, 128, 0, sf>>>(L.kind, L.n[0], L.n[1], L.n[2], t->counts);
                 if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
             }
             if (bank_reader_done(hb) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
+            if (cudaEventRecord(L.ev_leaf, sf) != cudaSuccess) return OCTO_FMM_ECUDA;
         }
     }
+    // the solve is complete on the caller's stream when every level's finish is
+    for (int l = 0; l < D; ++l)
+        if (cudaStreamWaitEvent(st, t->lev[l].ev_leaf, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if ((rc = tree_leave(t)) != OCTO_FMM_OK) return rc;
     if (!rhs2) t->solved = true;
     return OCTO_FMM_OK;
 }
@@ -573,6 +650,7 @@ int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host,
     std::vector<double*> o(D);
     char* w = (char*)scratch;
     cudaStream_t st = t->stream;
+    if (tree_enter(t) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     for (int l = 0; l < D; ++l) {
         if (!mass_host[l] || !out_host[l]) return OCTO_FMM_EINVAL;
         const size_t nc = t->lev[l].cells();
