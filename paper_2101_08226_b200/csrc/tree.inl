@@ -33,6 +33,7 @@ struct TreeLevel {
     cudaStream_t s_m2l, s_leaf;
     cudaEvent_t ev_m2l, ev_leaf;
     bool m2l_on_main;                  // few bricks (a level near the top): its multipole step runs in the main stream's chain
+    cudaEvent_t ev_lm;                 // on the leaf stream: this level's leaf masses (and the moments of its non-refined cells)
     cudaEvent_t ev_rdy;                // on the main stream: this level's raw moments and leaf masses are there (upward pass)
     cudaEvent_t ev_par;                // on the main stream: the PARENT level's expansions are complete (leaf finish may start)
     size_t cells() const { return (size_t)n[0] * n[1] * n[2]; }
@@ -100,7 +101,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.h = cfg.h0 / (double)(1LL << l);
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
-        L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr; L.ev_par = nullptr; L.ev_rdy = nullptr;
+        L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr; L.ev_par = nullptr; L.ev_rdy = nullptr; L.ev_lm = nullptr;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
         L.has_refined = L.has_leaf = false;
@@ -240,7 +241,7 @@ struct octo_fmm_tree {
     cudaStream_t pool_m2l[3], pool_leaf[2];   // the levels share a few side streams (see octo_fmm_tree_create)
     cudaStream_t user;                 // the caller's stream (cfg.stream): a solve starts after and is joined into it
     cudaEvent_t ev_user;               // hand-over between the two
-    cudaEvent_t ev_up;                 // the upward pass of a solve is complete
+    cudaEvent_t ev_up;                 // a solve has begun on the main stream (the side streams start behind it)
     bool solved;
 };
 
@@ -268,6 +269,7 @@ int octo_fmm_tree_destroy(octo_fmm_tree_t* t)
         if (l.ev_leaf) cudaEventDestroy(l.ev_leaf);
         if (l.ev_par) cudaEventDestroy(l.ev_par);
         if (l.ev_rdy) cudaEventDestroy(l.ev_rdy);
+        if (l.ev_lm) cudaEventDestroy(l.ev_lm);
     }
     if (t->ev_up) cudaEventDestroy(t->ev_up);
     if (t->ev_user) cudaEventDestroy(t->ev_user);
@@ -343,6 +345,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         L.s_m2l = L.m2l_on_main ? t->stream : t->pool_m2l[m2l_stream[l]];
         L.s_leaf = t->pool_leaf[l % 2];
         if (cudaEventCreateWithFlags(&L.ev_rdy, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&L.ev_lm, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&L.ev_m2l, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&L.ev_leaf, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&L.ev_par, cudaEventDisableTiming) != cudaSuccess) { rc = OCTO_FMM_ECUDA; break; }
@@ -428,12 +431,23 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             for (SolverLevel& l : t->up) l.fmm->cfg.am_correction = keep[i++];
         }
     } corr_guard(t, rhs2);
-    // ---- upward pass: finest level first ----
+    // ---- upward pass.  The leaf masses of a level depend on nothing: every level writes them on its leaf stream, side by
+    //      side (and its leaf-leaf sums follow there); the main stream carries only the M2M chain, finest level first ----
+    if (cudaEventRecord(t->ev_up, st) != cudaSuccess) return OCTO_FMM_ECUDA;       // the solve has begun
     for (int l = D - 1; l >= 0; --l) {
         TreeLevel& L = t->lev[l];
         const long long nc = (long long)L.cells();
+        if (cudaStreamWaitEvent(L.s_leaf, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+        // (the offsets of the cells that are not refined are zero for both right-hand sides: rewriting them is harmless)
+        tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_leaf>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
+        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (cudaEventRecord(L.ev_lm, L.s_leaf) != cudaSuccess) return OCTO_FMM_ECUDA;
+    }
+    for (int l = D - 1; l >= 0; --l) {
+        TreeLevel& L = t->lev[l];
         if (L.has_refined) {
             TreeLevel& F = t->lev[l + 1];
+            if (cudaStreamWaitEvent(st, F.ev_lm, 0) != cudaSuccess) return OCTO_FMM_ECUDA;      // the children that are leaves
             ChildBox cb;
             for (int a = 0; a < 3; ++a) { cb.n[a] = F.n[a]; cb.sh[a] = -2 * F.psh[a]; }
             cb.pkind = L.kind;
@@ -445,16 +459,15 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
                 if (F.raw) m2m_kernel<false, false, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
                 else       m2m_kernel<true, false, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
             }
+            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
         }
-        // (the offsets of the cells that are not refined are zero for both right-hand sides: rewriting them is harmless)
-        tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
-        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
-        // this level's multipole step and leaf sums need nothing of the coarser levels: they may start now
+        // this level's moments are complete (refined cells: M2M; the others: its leaf masses): its multipole step needs
+        // nothing of the coarser levels and may start now
+        if (cudaStreamWaitEvent(st, L.ev_lm, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
         if (cudaEventRecord(L.ev_rdy, st) != cudaSuccess) return OCTO_FMM_ECUDA;
     }
-    // ---- side by side, each level on streams of its own: staging + multipole step (its own level only; the parent's
-    //      expansion comes in the chain below), and the leaf-leaf point-mass sums ----
-    if (cudaEventRecord(t->ev_up, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    // ---- side by side: staging + multipole step per level (its own level only; the parent's expansion comes in the chain
+    //      below), and the leaf-leaf point-mass sums ----
     auto multipole_step = [&](TreeLevel& L) -> int {
         if (cudaStreamWaitEvent(L.s_m2l, L.ev_rdy, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
         int r = octo_fmm_set_moments(L.fmm, L.raw, L.off);
@@ -470,7 +483,7 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         TreeLevel& L = t->lev[l];
         if (L.fmm && L.n_m2l_tiles > 0 && !L.m2l_on_main && (rc = multipole_step(L)) != OCTO_FMM_OK) return rc;
         if (L.leaf) {
-            if (cudaStreamWaitEvent(L.s_leaf, L.ev_rdy, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+            // (behind this level's leaf masses in the same stream)
             if ((rc = octo_fmm_set_moments(L.leaf, L.lm, nullptr)) != OCTO_FMM_OK) return rc;
             double* const keep = L.leaf->outL;
             if (!rhs2) L.leaf->outL = out[l];          // second right-hand side: the four sums go to the handle's own buffer
