@@ -35,6 +35,7 @@ struct Offset3 { signed char d[3]; };
 // Eq. 15 with distances in units of the (parent) cell width: theta' = 1/|Delta| < theta.
 inline bool well_separated(long long d2, double theta) { return (double)d2 * theta * theta > 1.0; }
 inline int floor_div2(int v) { return v >> 1; }   // arithmetic shift: floor for negatives too
+inline int floor_div8(int v) { return v >> 3; }
 
 // partner list of parity class (px,py,pz): cells well separated, parents not (L135)
 // leaf: the leaf-level list of the complete solve -- every Delta != 0 whose parents are not well separated

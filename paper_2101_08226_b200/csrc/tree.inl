@@ -27,6 +27,9 @@ struct TreeLevel {
     int* m2l_tiles;  int n_m2l_tiles;     // bricks of the slab-fed kernel that have work
     int* p2p_tiles;  int n_p2p_tiles;     // 16 x 16 x 8 tiles of the tensor-core kernel that hold leaves
     std::vector<int> h_m2l_tiles, h_p2p_tiles;
+    unsigned char* brick_on;              // device [bricks of the dense enumeration]: 1 = the multipole step ran on this brick
+    std::vector<unsigned char> h_brick_on;
+    int btx, btz;                         // bricks per x-row and per z-column of that enumeration
     std::vector<unsigned char> h_nodeflag;
     // the multipole step and the leaf-leaf sums of a level depend on the upward pass only: they run on streams of their
     // own, side by side with those of the other levels; the L2L / leaf-finish chain on the caller's stream waits for them
@@ -101,6 +104,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.h = cfg.h0 / (double)(1LL << l);
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
+        L.brick_on = nullptr; L.btx = 0; L.btz = 0;
         L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr; L.ev_par = nullptr; L.ev_rdy = nullptr; L.ev_lm = nullptr;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
@@ -182,8 +186,24 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
                                 const bool refined = node_kind(l, gx0 + I, gy0 + (ty * TILE_Y) / 8, gz0 + K) == KIND_REFINED;
                                 weight += (refined ? 1.0 : 0.2) * 64.0 * layers;
                             }
-                        if (weight > 0.0) weighted.push_back(std::make_pair(-weight, (ty * tx_n + tx) * tz_n + tz));
+                        if (weight <= 0.0) continue;
+                        // a brick of leaf cells only has work if a refined cell lies within the lists' reach of it (the
+                        // sub-grid flag says "within a sub-grid": 8 cells, and a sub-grid has 2 x 1 x 3 bricks)
+                        bool near_refined = false;
+                        const int xa = tx * TILE_X - REACH_MAX, xb = std::min(tx * TILE_X + TILE_X, L.n[0]) - 1 + REACH_MAX;
+                        const int ya = ty * TILE_Y - REACH_MAX, yb = std::min(ty * TILE_Y + TILE_Y, L.n[1]) - 1 + REACH_MAX;
+                        const int za = z0 - REACH_MAX, zb = z1 + REACH_MAX;
+                        for (int K = floor_div8(za); K <= floor_div8(zb) && !near_refined; ++K)
+                            for (int J = floor_div8(ya); J <= floor_div8(yb) && !near_refined; ++J)
+                                for (int I = floor_div8(xa); I <= floor_div8(xb) && !near_refined; ++I)
+                                    near_refined = I >= 0 && J >= 0 && K >= 0 && I < nnx && J < nny && K < nnz &&
+                                                   node_kind(l, gx0 + I, gy0 + J, gz0 + K) == KIND_REFINED;
+                        if (!near_refined) continue;
+                        weighted.push_back(std::make_pair(-weight, (ty * tx_n + tx) * tz_n + tz));
                     }
+            L.btx = tx_n; L.btz = tz_n;
+            L.h_brick_on.assign((size_t)tx_n * ty_n * tz_n, 0);
+            for (const auto& wt : weighted) L.h_brick_on[wt.second] = 1;
             // heaviest bricks first: the persistent CTAs take the list round-robin, so that every CTA gets its share of the
             // bricks that are full of refined cells instead of whoever comes first in lattice order getting three of them
             std::sort(weighted.begin(), weighted.end());
@@ -207,7 +227,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         // workspace of this level
         const size_t nc = L.cells();
         P.bytes += align_up(nc) + align_up((size_t)nnx * nny * nnz) + align_up(nc * 8);           // kind, nodeflag, lm
-        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4);
+        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4) + align_up(L.h_brick_on.size() + 4);
         if (L.has_refined) {
             octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
             P.bytes += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
@@ -334,10 +354,12 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         L.lm = (double*)w; w += align_up(nc * 8);
         L.m2l_tiles = (int*)w; w += align_up((size_t)L.n_m2l_tiles * 4 + 4);
         L.p2p_tiles = (int*)w; w += align_up((size_t)L.n_p2p_tiles * 4 + 4);
+        L.brick_on = (unsigned char*)w; w += align_up(L.h_brick_on.size() + 4);
         if (cudaMemcpyAsync(L.kind, kind_host[l], nc, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             cudaMemcpyAsync(L.nodeflag, L.h_nodeflag.data(), nn, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             (L.n_m2l_tiles && cudaMemcpyAsync(L.m2l_tiles, L.h_m2l_tiles.data(), (size_t)L.n_m2l_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
-            (L.n_p2p_tiles && cudaMemcpyAsync(L.p2p_tiles, L.h_p2p_tiles.data(), (size_t)L.n_p2p_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)) {
+            (L.n_p2p_tiles && cudaMemcpyAsync(L.p2p_tiles, L.h_p2p_tiles.data(), (size_t)L.n_p2p_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
+            (!L.h_brick_on.empty() && cudaMemcpyAsync(L.brick_on, L.h_brick_on.data(), L.h_brick_on.size(), cudaMemcpyHostToDevice, st) != cudaSuccess)) {
             rc = OCTO_FMM_ECUDA;
             break;
         }
@@ -391,7 +413,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     // the topology arrays were copied from pageable host memory: make sure they have left it before returning
     if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
-    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); }
+    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_brick_on.clear(); }
     *out = t;
     return OCTO_FMM_OK;
 }
@@ -585,6 +607,7 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             a.out = rhs2 ? (L.leaf ? L.leaf->L : nullptr) : out[l];
             a.phi_only = rhs2 ? out[l] : nullptr;
             a.L = L.fmm ? L.fmm->L : nullptr;
+            a.brick_on = L.fmm ? L.brick_on : nullptr; a.btx = L.btx; a.btz = L.btz;
             a.pL = pL; a.pC = pC; a.poff = poff;
             if (l + 1 < D) {
                 TreeLevel& F = t->lev[l + 1];
