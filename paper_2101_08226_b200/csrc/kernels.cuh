@@ -412,7 +412,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
             }
             return true;
         };
-#define OCTO_FETCH(P)                                                                       \
+#define OCTO_FETCH(P, SKIP)                                                                 \
         {                                                                                   \
             const StEntry e_ = *reinterpret_cast<const StEntry*>(reinterpret_cast<const char*>(c_entries) + s); \
             s += (int)sizeof(StEntry);                                                      \
@@ -425,7 +425,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
                    the pair is skipped altogether */                                        \
                 const double kb_ = q_[9 * SLAB_PLANE].y;                                      \
                 masked_ = !present || kb_ == 0.0 || (leafA && kb_ == 1.0);                  \
-                P.live = !__all_sync(0xffffffffu, masked_);                                 \
+                if (SKIP) P.live = !__all_sync(0xffffffffu, masked_);                       \
             }                                                                               \
             if (P.live) {                                                                   \
                 double bx_, by_, bz_, fl_ = 0.0;                                            \
@@ -440,37 +440,35 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
             }                                                                               \
         }
         struct Fetched { double src[16]; double x, y, z, w; bool live; } A, B;
-#define OCTO_BODY(P) { if (MODE != MODE_TREE || P.live) m2l_pair<CORR, DIPOLE>(acc, P.x, P.y, P.z, P.w, P.src, tA); }
-        if constexpr (MODE == MODE_TREE) {
-            // no hand pipelining here: with whole pairs skipped the two-deep scheme would have to keep both fetched pairs
-            // alive across a branch (it spills 2 KB); three warps per sub-partition cover the head of a pair instead
-            if (__all_sync(0xffffffffu, !present || leafA)) {
-                // a warp of LEAF targets (the shell of leaves around a refined region: most bricks of a level).  A leaf has
-                // no children: of its expansion only L0 and L1 (+ correction) are ever used -- the leaf finish evaluates
-                // them at the cell centre.  The order-2 and order-3 sums are discarded after the loop, which makes them dead:
-                // the compiler drops their instructions from this copy of the loop (83 instead of 117 per pair)
-                while (ensure()) {
-                    OCTO_FETCH(A);
-                    OCTO_BODY(A);
-                }
-#pragma unroll
-                for (int i = 0; i < 5; ++i) acc.l2[i] = 0.0;
-#pragma unroll
-                for (int i = 0; i < 7; ++i) acc.l3[i] = 0.0;
-            } else {
-                while (ensure()) {
-                    OCTO_FETCH(A);
-                    OCTO_BODY(A);
-                }
+#define OCTO_BODY(P) m2l_pair<CORR, DIPOLE>(acc, P.x, P.y, P.z, P.w, P.src, tA)
+        bool leaf_warp = false;
+        if constexpr (MODE == MODE_TREE) leaf_warp = __all_sync(0xffffffffu, !present || leafA);
+        if (leaf_warp) {
+            // MODE_TREE, a warp of LEAF targets (the shell of leaves around a refined region: most bricks of a level).  Most of
+            // its list entries meet leaves or nothing: a pair that is masked for the whole warp is skipped (one LDS and a
+            // vote instead of 340 cycles).  No hand pipelining here: with whole pairs skipped the two-deep scheme would have
+            // to keep both fetched pairs alive across a branch (it spills 2 KB).  And a leaf has no children: of its
+            // expansion only L0 and L1 (+ correction) are ever used -- the leaf finish evaluates them at the cell centre.
+            // The order-2 and order-3 sums are discarded after the loop, which makes them dead: the compiler drops their
+            // instructions from this copy of the loop (83 instead of 117 per pair)
+            while (ensure()) {
+                OCTO_FETCH(A, true);
+                if (A.live) OCTO_BODY(A);
             }
+#pragma unroll
+            for (int i = 0; i < 5; ++i) acc.l2[i] = 0.0;
+#pragma unroll
+            for (int i = 0; i < 7; ++i) acc.l3[i] = 0.0;
         } else if (ensure()) {
-            OCTO_FETCH(A);
+            // every other warp (MODE_TREE: its targets are refined cells, for which every partner that exists counts):
+            // the pipelined loop over all entries; a lane whose pair does not count has 1/r = 0
+            OCTO_FETCH(A, false);
             for (;;) {
                 if (!ensure()) break;
-                OCTO_FETCH(B);
+                OCTO_FETCH(B, false);
                 OCTO_BODY(A);
                 if (!ensure()) { A = B; break; }
-                OCTO_FETCH(A);
+                OCTO_FETCH(A, false);
                 OCTO_BODY(B);
             }
             OCTO_BODY(A);
