@@ -261,6 +261,139 @@ __device__ __forceinline__ void m2l_pair_folded(Acc& a, const double x, const do
     a.l1[1] = fma(u2, Vy, a.l1[1]);
 }
 
+// Body of one ordered pair with the correction OFF, component form: the contractions
+//   L0     += M D0 - M1.D1 + 1/2 M2:D2 - 1/6 M3:.D3
+//   L1_i   += M D1_i - M1_j D2_ij + 1/2 M2_jk D3_ijk
+//   L2_ij  += M D2_ij - M1_k D3_ijk            (xx xy xz yy yz)
+//   L3_ijk += M D3_ijk                         (xxx xxy xxz xyy xyz yyy yyz)
+// with the components of D generated one after the other (D2_ij = d1 d_ij + d2 R_i R_j, D3 likewise, zz / xzz / yzz from the
+// traces) and every accumulation that uses a component written as a statement of its own; L0 alternates between two
+// partial sums.  One statement per line, in an order found like the one of m2l_pair_folded (order_search): what counts is
+// how often consecutive DFMAs share an operand slot (operand-reuse cache).
+template <bool DIPOLE>
+__device__ __forceinline__ void m2l_pair_components(Acc& a, const double x, const double y, const double z, const double w,
+                                                     const double (&s)[16])
+{
+    const double w2 = w * w;
+    const double d1 = w * w2;
+    const double d2 = d1 * (-3.0 * w2);
+    const double d3 = d2 * (-5.0 * w2);
+    const double m0 = s[C_M0];
+    const double m1x = s[C_M1X];
+    const double m1y = s[C_M1Y];
+    const double m1z = s[C_M1Z];
+    const double qxx = s[C_QXX];
+    const double qxy = s[C_QXY];
+    const double qxz = s[C_QXZ];
+    const double qyy = s[C_QYY];
+    const double qyz = s[C_QYZ];
+    const double oxxx = s[C_OXXX];
+    const double oxxy = s[C_OXXY];
+    const double oxxz = s[C_OXXZ];
+    const double oxyy = s[C_OXYY];
+    const double oxyz = s[C_OXYZ];
+    const double oyyy = s[C_OYYY];
+    const double oyyz = s[C_OYYZ];
+    a.l0 = fma(m0, -w, a.l0);
+    const double D1x = d1 * x;
+    const double D1y = d1 * y;
+    const double D1z = d1 * z;
+    a.l1[0] = fma(m0, D1x, a.l1[0]);
+    if (DIPOLE) a.l0b = fma(m1x, D1x, a.l0b);
+    a.l1[1] = fma(m0, D1y, a.l1[1]);
+    if (DIPOLE) a.l0 = fma(m1y, D1y, a.l0);
+    a.l1[2] = fma(m0, D1z, a.l1[2]);
+    if (DIPOLE) a.l0b = fma(m1z, D1z, a.l0b);
+    const double ax = d2 * x;
+    const double ay = d2 * y;
+    const double az = d2 * z;
+    const double Dxx = fma(ax, x, d1);
+    const double Dyy = fma(ay, y, d1);
+    const double Dzz = fma(az, z, d1);
+    const double Dxy = ax * y;
+    const double Dxz = ax * z;
+    const double Dyz = ay * z;
+    a.l2[0] = fma(m0, Dxx, a.l2[0]);
+    if (DIPOLE) a.l1[0] = fma(m1x, Dxx, a.l1[0]);
+    a.l0 = fma(qxx, Dxx, a.l0);
+    a.l2[1] = fma(m0, Dxy, a.l2[1]);
+    if (DIPOLE) a.l1[1] = fma(m1x, Dxy, a.l1[1]);
+    if (DIPOLE) a.l1[0] = fma(m1y, Dxy, a.l1[0]);
+    a.l0b = fma(qxy, Dxy, a.l0b);
+    a.l2[2] = fma(m0, Dxz, a.l2[2]);
+    if (DIPOLE) a.l1[2] = fma(m1x, Dxz, a.l1[2]);
+    if (DIPOLE) a.l1[0] = fma(m1z, Dxz, a.l1[0]);
+    a.l0 = fma(qxz, Dxz, a.l0);
+    a.l2[3] = fma(m0, Dyy, a.l2[3]);
+    if (DIPOLE) a.l1[1] = fma(m1y, Dyy, a.l1[1]);
+    a.l0b = fma(qyy, Dyy, a.l0b);
+    a.l2[4] = fma(m0, Dyz, a.l2[4]);
+    if (DIPOLE) a.l1[2] = fma(m1y, Dyz, a.l1[2]);
+    if (DIPOLE) a.l1[1] = fma(m1z, Dyz, a.l1[1]);
+    a.l0 = fma(qyz, Dyz, a.l0);
+    if (DIPOLE) a.l1[2] = fma(m1z, Dzz, a.l1[2]);
+    const double bx = d3 * x;
+    const double by = d3 * y;
+    const double bxx = bx * x;
+    const double bxy = bx * y;
+    const double byy = by * y;
+    const double ax3 = 3.0 * ax;
+    const double ay3 = 3.0 * ay;
+    const double Dxxx = fma(bxx, x, ax3);
+    const double Dxxy = fma(bxx, y, ay);
+    const double Dxxz = fma(bxx, z, az);
+    a.l3[0] = fma(m0, Dxxx, a.l3[0]);
+    if (DIPOLE) a.l2[0] = fma(m1x, Dxxx, a.l2[0]);
+    a.l1[0] = fma(qxx, Dxxx, a.l1[0]);
+    a.l0b = fma(oxxx, Dxxx, a.l0b);
+    a.l3[1] = fma(m0, Dxxy, a.l3[1]);
+    if (DIPOLE) a.l2[1] = fma(m1x, Dxxy, a.l2[1]);
+    if (DIPOLE) a.l2[0] = fma(m1y, Dxxy, a.l2[0]);
+    a.l1[1] = fma(qxx, Dxxy, a.l1[1]);
+    a.l1[0] = fma(qxy, Dxxy, a.l1[0]);
+    a.l0 = fma(oxxy, Dxxy, a.l0);
+    a.l3[2] = fma(m0, Dxxz, a.l3[2]);
+    if (DIPOLE) a.l2[2] = fma(m1x, Dxxz, a.l2[2]);
+    if (DIPOLE) a.l2[0] = fma(m1z, Dxxz, a.l2[0]);
+    a.l1[2] = fma(qxx, Dxxz, a.l1[2]);
+    a.l1[0] = fma(qxz, Dxxz, a.l1[0]);
+    a.l0b = fma(oxxz, Dxxz, a.l0b);
+    const double Dxyy = fma(bxy, y, ax);
+    const double Dxyz = bxy * z;
+    a.l3[3] = fma(m0, Dxyy, a.l3[3]);
+    if (DIPOLE) a.l2[3] = fma(m1x, Dxyy, a.l2[3]);
+    if (DIPOLE) a.l2[1] = fma(m1y, Dxyy, a.l2[1]);
+    a.l1[0] = fma(qyy, Dxyy, a.l1[0]);
+    a.l1[1] = fma(qxy, Dxyy, a.l1[1]);
+    a.l0 = fma(oxyy, Dxyy, a.l0);
+    a.l3[4] = fma(m0, Dxyz, a.l3[4]);
+    if (DIPOLE) a.l2[4] = fma(m1x, Dxyz, a.l2[4]);
+    if (DIPOLE) a.l2[2] = fma(m1y, Dxyz, a.l2[2]);
+    if (DIPOLE) a.l2[1] = fma(m1z, Dxyz, a.l2[1]);
+    a.l1[0] = fma(qyz, Dxyz, a.l1[0]);
+    a.l1[1] = fma(qxz, Dxyz, a.l1[1]);
+    a.l1[2] = fma(qxy, Dxyz, a.l1[2]);
+    a.l0b = fma(oxyz, Dxyz, a.l0b);
+    const double Dyyy = fma(byy, y, ay3);
+    const double Dyyz = fma(byy, z, az);
+    a.l3[5] = fma(m0, Dyyy, a.l3[5]);
+    if (DIPOLE) a.l2[3] = fma(m1y, Dyyy, a.l2[3]);
+    a.l1[1] = fma(qyy, Dyyy, a.l1[1]);
+    a.l0 = fma(oyyy, Dyyy, a.l0);
+    a.l3[6] = fma(m0, Dyyz, a.l3[6]);
+    if (DIPOLE) a.l2[4] = fma(m1y, Dyyz, a.l2[4]);
+    if (DIPOLE) a.l2[3] = fma(m1z, Dyyz, a.l2[3]);
+    a.l1[2] = fma(qyy, Dyyz, a.l1[2]);
+    a.l1[1] = fma(qyz, Dyyz, a.l1[1]);
+    a.l0b = fma(oyyz, Dyyz, a.l0b);
+    const double Dxzz = -(Dxxx + Dxyy);
+    const double Dyzz = -(Dxxy + Dyyy);
+    if (DIPOLE) a.l2[2] = fma(m1z, Dxzz, a.l2[2]);
+    a.l1[2] = fma(qxz, Dxzz, a.l1[2]);
+    if (DIPOLE) a.l2[4] = fma(m1z, Dyzz, a.l2[4]);
+    a.l1[2] = fma(qyz, Dyzz, a.l1[2]);
+}
+
 // Body of one ordered pair A <- B.  (x,y,z) = R = z_A - z_B, w = 1/|R|; s[0..15] staged source
 // components; tA[0..6] = staged third moments of the target divided by its mass (correction only).
 // DIPOLE = false leaves out the 27 terms with the source's dipole moment (and D2_zz, which only they need):
@@ -269,83 +402,8 @@ template <bool CORR, bool DIPOLE>
 __device__ __forceinline__ void m2l_pair(Acc& a, const double x, const double y, const double z, const double w,
                                          const double (&s)[16], const double (&tA)[7])
 {
-    if constexpr (CORR) {
-        m2l_pair_folded<DIPOLE>(a, x, y, z, w, s, tA);
-        return;
-    }
-    const double w2 = w * w;                  // 1/r^2
-    const double d1 = w * w2;                 // 1/r^3
-    const double d2 = d1 * (-3.0 * w2);       // -3/r^5
-    const double d3 = d2 * (-5.0 * w2);       // 15/r^7
-
-    const double m0 = s[C_M0], m1x = s[C_M1X], m1y = s[C_M1Y], m1z = s[C_M1Z];
-    const double qxx = s[C_QXX], qxy = s[C_QXY], qxz = s[C_QXZ], qyy = s[C_QYY], qyz = s[C_QYZ];
-    const double oxxx = s[C_OXXX], oxxy = s[C_OXXY], oxxz = s[C_OXXZ], oxyy = s[C_OXYY], oxyz = s[C_OXYZ],
-                 oyyy = s[C_OYYY], oyyz = s[C_OYYZ];
-
-    // The contractions
-    //   L0     += M D0 - M1.D1 + 1/2 M2:D2 - 1/6 M3:.D3
-    //   L1_i   += M D1_i - M1_j D2_ij + 1/2 M2_jk D3_ijk
-    //   L2_ij  += M D2_ij - M1_k D3_ijk            (xx xy xz yy yz)
-    //   L3_ijk += M D3_ijk                         (xxx xxy xxz xyy xyz yyy yyz)
-    // are written as RUNS that share one component of D, each right after that component is
-    // generated: a DFMA with three fresh register operands issues at 2/3 of the FP64 rate on
-    // sm_100 (register-read bound, measured), one that repeats an operand of the previous
-    // instruction in the same slot takes it from the operand-reuse cache and issues at full rate.
-    // Every run updates distinct accumulators; L0 alternates between two partial sums.
-
-    // ---- D0, D1 ----
-    a.l0 = fma(m0, -w, a.l0);
-    const double D1x = d1 * x, D1y = d1 * y, D1z = d1 * z;
-    a.l1[0] = fma(m0, D1x, a.l1[0]);  if (DIPOLE) a.l0b = fma(m1x, D1x, a.l0b);
-    a.l1[1] = fma(m0, D1y, a.l1[1]);  if (DIPOLE) a.l0 = fma(m1y, D1y, a.l0);
-    a.l1[2] = fma(m0, D1z, a.l1[2]);  if (DIPOLE) a.l0b = fma(m1z, D1z, a.l0b);
-
-    // ---- D2 (6 components; zz is needed by the dipole term of L1_z) ----
-    const double ax = d2 * x, ay = d2 * y, az = d2 * z;
-    const double Dxx = fma(ax, x, d1), Dyy = fma(ay, y, d1), Dzz = fma(az, z, d1);
-    const double Dxy = ax * y, Dxz = ax * z, Dyz = ay * z;
-    a.l2[0] = fma(m0, Dxx, a.l2[0]);  if (DIPOLE) a.l1[0] = fma(m1x, Dxx, a.l1[0]);  a.l0 = fma(qxx, Dxx, a.l0);
-    a.l2[1] = fma(m0, Dxy, a.l2[1]);  if (DIPOLE) a.l1[1] = fma(m1x, Dxy, a.l1[1]);  if (DIPOLE) a.l1[0] = fma(m1y, Dxy, a.l1[0]);
-    a.l0b = fma(qxy, Dxy, a.l0b);
-    a.l2[2] = fma(m0, Dxz, a.l2[2]);  if (DIPOLE) a.l1[2] = fma(m1x, Dxz, a.l1[2]);  if (DIPOLE) a.l1[0] = fma(m1z, Dxz, a.l1[0]);
-    a.l0 = fma(qxz, Dxz, a.l0);
-    a.l2[3] = fma(m0, Dyy, a.l2[3]);  if (DIPOLE) a.l1[1] = fma(m1y, Dyy, a.l1[1]);  a.l0b = fma(qyy, Dyy, a.l0b);
-    a.l2[4] = fma(m0, Dyz, a.l2[4]);  if (DIPOLE) a.l1[2] = fma(m1y, Dyz, a.l1[2]);  if (DIPOLE) a.l1[1] = fma(m1z, Dyz, a.l1[1]);
-    a.l0 = fma(qyz, Dyz, a.l0);
-    if (DIPOLE) a.l1[2] = fma(m1z, Dzz, a.l1[2]);
-
-    // ---- D3: 7 independent + xzz, yzz ----
-    const double bx = d3 * x, by = d3 * y;
-    const double bxx = bx * x, bxy = bx * y, byy = by * y;
-    const double ax3 = 3.0 * ax, ay3 = 3.0 * ay;
-    const double Dxxx = fma(bxx, x, ax3);
-    const double Dxxy = fma(bxx, y, ay);
-    const double Dxxz = fma(bxx, z, az);
-    a.l3[0] = fma(m0, Dxxx, a.l3[0]);  if (DIPOLE) a.l2[0] = fma(m1x, Dxxx, a.l2[0]);  a.l1[0] = fma(qxx, Dxxx, a.l1[0]);
-    if (!CORR) a.l0b = fma(oxxx, Dxxx, a.l0b);
-    a.l3[1] = fma(m0, Dxxy, a.l3[1]);  if (DIPOLE) a.l2[1] = fma(m1x, Dxxy, a.l2[1]);  if (DIPOLE) a.l2[0] = fma(m1y, Dxxy, a.l2[0]);
-    a.l1[1] = fma(qxx, Dxxy, a.l1[1]);  a.l1[0] = fma(qxy, Dxxy, a.l1[0]);  if (!CORR) a.l0 = fma(oxxy, Dxxy, a.l0);
-    a.l3[2] = fma(m0, Dxxz, a.l3[2]);  if (DIPOLE) a.l2[2] = fma(m1x, Dxxz, a.l2[2]);  if (DIPOLE) a.l2[0] = fma(m1z, Dxxz, a.l2[0]);
-    a.l1[2] = fma(qxx, Dxxz, a.l1[2]);  a.l1[0] = fma(qxz, Dxxz, a.l1[0]);  if (!CORR) a.l0b = fma(oxxz, Dxxz, a.l0b);
-    const double Dxyy = fma(bxy, y, ax);
-    const double Dxyz = bxy * z;
-    a.l3[3] = fma(m0, Dxyy, a.l3[3]);  if (DIPOLE) a.l2[3] = fma(m1x, Dxyy, a.l2[3]);  if (DIPOLE) a.l2[1] = fma(m1y, Dxyy, a.l2[1]);
-    a.l1[0] = fma(qyy, Dxyy, a.l1[0]);  a.l1[1] = fma(qxy, Dxyy, a.l1[1]);  if (!CORR) a.l0 = fma(oxyy, Dxyy, a.l0);
-    a.l3[4] = fma(m0, Dxyz, a.l3[4]);  if (DIPOLE) a.l2[4] = fma(m1x, Dxyz, a.l2[4]);  if (DIPOLE) a.l2[2] = fma(m1y, Dxyz, a.l2[2]);
-    if (DIPOLE) a.l2[1] = fma(m1z, Dxyz, a.l2[1]);  a.l1[0] = fma(qyz, Dxyz, a.l1[0]);  a.l1[1] = fma(qxz, Dxyz, a.l1[1]);
-    a.l1[2] = fma(qxy, Dxyz, a.l1[2]);  if (!CORR) a.l0b = fma(oxyz, Dxyz, a.l0b);
-    const double Dyyy = fma(byy, y, ay3);
-    const double Dyyz = fma(byy, z, az);
-    a.l3[5] = fma(m0, Dyyy, a.l3[5]);  if (DIPOLE) a.l2[3] = fma(m1y, Dyyy, a.l2[3]);  a.l1[1] = fma(qyy, Dyyy, a.l1[1]);
-    if (!CORR) a.l0 = fma(oyyy, Dyyy, a.l0);
-    a.l3[6] = fma(m0, Dyyz, a.l3[6]);  if (DIPOLE) a.l2[4] = fma(m1y, Dyyz, a.l2[4]);  if (DIPOLE) a.l2[3] = fma(m1z, Dyyz, a.l2[3]);
-    a.l1[2] = fma(qyy, Dyyz, a.l1[2]);  a.l1[1] = fma(qyz, Dyyz, a.l1[1]);  if (!CORR) a.l0b = fma(oyyz, Dyyz, a.l0b);
-    const double Dxzz = -(Dxxx + Dxyy);
-    const double Dyzz = -(Dxxy + Dyyy);
-    if (DIPOLE) a.l2[2] = fma(m1z, Dxzz, a.l2[2]);  a.l1[2] = fma(qxz, Dxzz, a.l1[2]);
-    if (DIPOLE) a.l2[4] = fma(m1z, Dyzz, a.l2[4]);  a.l1[2] = fma(qyz, Dyzz, a.l1[2]);
-
+    if constexpr (CORR) m2l_pair_folded<DIPOLE>(a, x, y, z, w, s, tA);
+    else                m2l_pair_components<DIPOLE>(a, x, y, z, w, s);
 }
 
 // Rebuild the 20 + 3 output coefficients from the accumulators.
