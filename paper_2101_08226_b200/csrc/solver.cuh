@@ -27,7 +27,9 @@ namespace octo {
 // Child arrays stored as a BOX of their lattice (levels of the adaptive tree): cbox = extents of the child arrays and the
 // (even) shift of the child index, child = 2 * parent + (a,b,c) + sh; children outside the box do not exist (zero mass).
 // The uniform solve passes a null box: the child arrays are exactly twice the parent's.
-struct ChildBox { int n[3]; int sh[3]; const unsigned char* pkind; };   // pkind (may be null): kind of every parent cell; only
+struct ChildBox { int n[3]; int sh[3]; const unsigned char* pkind; const int* nodes = nullptr; };
+// nodes (may be null): the refined 8^3 sub-grids of the parent level, x | y << 10 | z << 20 in sub-grid units: the grid is then
+// 4 blocks of 128 threads per listed sub-grid instead of one thread per cell of the box.    pkind (may be null): kind of every parent cell; only
                                                                         // the refined ones (2) are built from children
 
 template <bool LEAF, bool GIVEN = false, bool BOXED = false>
@@ -37,7 +39,13 @@ __global__ void __launch_bounds__(128) m2m_kernel(const double* __restrict__ cm,
 {
     // grid = (ceil(pnx / blockDim.x), pny, pnz): no integer divisions
     const long long pcell = (long long)pnx * pny * pnz;
-    const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y, K = blockIdx.z;
+    int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y, K = blockIdx.z;
+    if (BOXED && cb.nodes) {                               // only the refined sub-grids: every lane of every warp has work
+        const int node = cb.nodes[blockIdx.x >> 2];
+        I = 8 * (node & 1023) + (threadIdx.x & 7);
+        J = 8 * ((node >> 10) & 1023) + ((threadIdx.x >> 3) & 7);
+        K = 8 * (node >> 20) + 2 * (blockIdx.x & 3) + (threadIdx.x >> 6);
+    }
     if (I >= pnx) return;
     const long long P = ((long long)K * pny + J) * pnx + I;
     if (BOXED && cb.pkind && cb.pkind[P] != 2) return;      // a leaf or absent parent: tree_leaf_moments_kernel writes it

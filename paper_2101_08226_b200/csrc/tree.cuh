@@ -58,12 +58,15 @@ struct TreeL2LArgs {
     const unsigned char* kind;
     double* L; double* C; const double* off;             // this level: [20], [3], [3] x cells
     const double* pL; const double* pC; const double* poff;
+    const int* nodes;                  // the refined sub-grids of the level (x | y << 10 | z << 20): 4 blocks of 128 threads each
 };
 
 __global__ void __launch_bounds__(128) tree_l2l_kernel(const TreeL2LArgs a)
 {
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    const int node = a.nodes[blockIdx.x >> 2];
+    const int i = 8 * (node & 1023) + (threadIdx.x & 7), j = 8 * ((node >> 10) & 1023) + ((threadIdx.x >> 3) & 7),
+              k = 8 * (node >> 20) + 2 * (blockIdx.x & 3) + (threadIdx.x >> 6);
     if (i >= nx) return;
     const long long ncell = (long long)nx * ny * nz, cell = ((long long)k * ny + j) * nx + i;
     if (a.kind[cell] != KIND_REFINED) return;             // leaves take the parent's expansion in the leaf finish

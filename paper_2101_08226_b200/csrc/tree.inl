@@ -27,6 +27,8 @@ struct TreeLevel {
     int* m2l_tiles;  int n_m2l_tiles;     // bricks of the slab-fed kernel that have work
     int* p2p_tiles;  int n_p2p_tiles;     // 16 x 16 x 8 tiles of the tensor-core kernel that hold leaves
     std::vector<int> h_m2l_tiles, h_p2p_tiles;
+    int* ref_nodes;  int n_ref_nodes;     // device: the refined sub-grids of the level, x | y << 10 | z << 20 (box-local, sub-grid units)
+    std::vector<int> h_ref_nodes;
     unsigned char* brick_on;              // device [bricks of the dense enumeration]: 1 = the multipole step ran on this brick
     std::vector<unsigned char> h_brick_on;
     int btx, btz;                         // bricks per x-row and per z-column of that enumeration
@@ -105,6 +107,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
         L.brick_on = nullptr; L.btx = 0; L.btz = 0;
+        L.ref_nodes = nullptr; L.n_ref_nodes = 0;
         L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr; L.ev_par = nullptr; L.ev_rdy = nullptr; L.ev_lm = nullptr;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
@@ -152,6 +155,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         for (int K = 0; K < nnz; ++K)
             for (int J = 0; J < nny; ++J)
                 for (int I = 0; I < nnx; ++I) {
+                    if (node_kind(l, gx0 + I, gy0 + J, gz0 + K) == KIND_REFINED) L.h_ref_nodes.push_back(I | (J << 10) | (K << 20));
                     if (node_kind(l, gx0 + I, gy0 + J, gz0 + K) != KIND_LEAF) continue;
                     unsigned char f = 0;
                     for (int c = -1; c <= 1; ++c)
@@ -227,7 +231,9 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         // workspace of this level
         const size_t nc = L.cells();
         P.bytes += align_up(nc) + align_up((size_t)nnx * nny * nnz) + align_up(nc * 8);           // kind, nodeflag, lm
-        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4) + align_up(L.h_brick_on.size() + 4);
+        L.n_ref_nodes = (int)L.h_ref_nodes.size();
+        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4) + align_up(L.h_brick_on.size() + 4) +
+                   align_up((size_t)L.n_ref_nodes * 4 + 4);
         if (L.has_refined) {
             octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
             P.bytes += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
@@ -355,11 +361,13 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         L.m2l_tiles = (int*)w; w += align_up((size_t)L.n_m2l_tiles * 4 + 4);
         L.p2p_tiles = (int*)w; w += align_up((size_t)L.n_p2p_tiles * 4 + 4);
         L.brick_on = (unsigned char*)w; w += align_up(L.h_brick_on.size() + 4);
+        L.ref_nodes = (int*)w; w += align_up((size_t)L.n_ref_nodes * 4 + 4);
         if (cudaMemcpyAsync(L.kind, kind_host[l], nc, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             cudaMemcpyAsync(L.nodeflag, L.h_nodeflag.data(), nn, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             (L.n_m2l_tiles && cudaMemcpyAsync(L.m2l_tiles, L.h_m2l_tiles.data(), (size_t)L.n_m2l_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
             (L.n_p2p_tiles && cudaMemcpyAsync(L.p2p_tiles, L.h_p2p_tiles.data(), (size_t)L.n_p2p_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
-            (!L.h_brick_on.empty() && cudaMemcpyAsync(L.brick_on, L.h_brick_on.data(), L.h_brick_on.size(), cudaMemcpyHostToDevice, st) != cudaSuccess)) {
+            (!L.h_brick_on.empty() && cudaMemcpyAsync(L.brick_on, L.h_brick_on.data(), L.h_brick_on.size(), cudaMemcpyHostToDevice, st) != cudaSuccess) ||
+            (L.n_ref_nodes && cudaMemcpyAsync(L.ref_nodes, L.h_ref_nodes.data(), (size_t)L.n_ref_nodes * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)) {
             rc = OCTO_FMM_ECUDA;
             break;
         }
@@ -413,7 +421,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     // the topology arrays were copied from pageable host memory: make sure they have left it before returning
     if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
-    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_brick_on.clear(); }
+    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_brick_on.clear(); L.h_ref_nodes.clear(); }
     *out = t;
     return OCTO_FMM_OK;
 }
@@ -473,7 +481,8 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             ChildBox cb;
             for (int a = 0; a < 3; ++a) { cb.n[a] = F.n[a]; cb.sh[a] = -2 * F.psh[a]; }
             cb.pkind = L.kind;
-            const dim3 blocks((unsigned)((L.n[0] + 127) / 128), (unsigned)L.n[1], (unsigned)L.n[2]);
+            cb.nodes = L.ref_nodes;
+            const dim3 blocks(4u * (unsigned)L.n_ref_nodes);          // the refined sub-grids only: 512 parents = 4 blocks each
             if (rhs2) {
                 if (F.raw) m2m_kernel<false, true, true><<<blocks, 128, 0, st>>>(F.raw, F.off, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
                 else       m2m_kernel<true, true, true><<<blocks, 128, 0, st>>>(F.lm, nullptr, L.raw, L.off, L.n[0], L.n[1], L.n[2], F.h, cb);
@@ -583,7 +592,8 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             TreeL2LArgs q;
             for (int c = 0; c < 3; ++c) { q.n[c] = L.n[c]; q.pn[c] = pn[c]; q.psh[c] = L.psh[c]; }
             q.h = L.h; q.kind = L.kind; q.L = L.fmm->L; q.C = L.fmm->C; q.off = L.off; q.pL = pL; q.pC = pC; q.poff = poff;
-            tree_l2l_kernel<<<blocks, 128, 0, st>>>(q);
+            q.nodes = L.ref_nodes;
+            tree_l2l_kernel<<<4u * (unsigned)L.n_ref_nodes, 128, 0, st>>>(q);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
         }
         // leaf finish on the level's leaf stream, behind its leaf-leaf sums (also zeroes the cells of out[l] that are not
