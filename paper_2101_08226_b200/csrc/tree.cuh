@@ -115,6 +115,8 @@ struct TreeFinishArgs {
     unsigned long long* count;      // null, or counts[2] += cross-level pairs taken (ordered)
     double* phi_only;               // null, or (second right-hand side) [cells]: only the potential is wanted; out is then
                                     // read (the leaf-leaf sums) but not written
+    const int* nodes;               // the sub-grids of the listed leaf tiles (x | y << 10 | z << 20): 4 blocks of 128 threads each;
+                                    // the rest of the level's output was zero-filled before
 };
 
 // Leaf finish, one thread per cell of the level.  For a leaf A:
@@ -125,11 +127,15 @@ struct TreeFinishArgs {
 //   parent (NODE_COARSE_NBR), as point masses:  x_A - x_b = ((double)(2 i_A - i_b) + 0.5) * (h / 2) per axis, i the
 //   index on the level's own LATTICE (the box shifts drop out of the difference: 2 i_A - i_b = 2 (A - B) - (a,b,c) for
 //   the child (a,b,c) of B).
-// Cells that are not leaves get zeros.  The near-field offsets come from the constant bank (c_near).
+// Cells of the visited sub-grids that are not leaves get zeros (the rest of the level's output was zero-filled before the
+// leaf-leaf sums).  The near-field offsets come from the constant bank (c_near).
 __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishArgs a)
 {
     const int nx = a.n[0], ny = a.n[1], nz = a.n[2];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, k = blockIdx.z;
+    // a warp = 4 rows of one sub-grid: its flags, and with them every branch on them below, are the same for the warp
+    const int node = a.nodes[blockIdx.x >> 2];
+    const int i = 8 * (node & 1023) + (threadIdx.x & 7), j = 8 * ((node >> 10) & 1023) + ((threadIdx.x >> 3) & 7),
+              k = 8 * (node >> 20) + 2 * (blockIdx.x & 3) + (threadIdx.x >> 6);
     if (i >= nx) return;
     const long long ncell = (long long)nx * ny * nz;
     const long long cell = ((long long)k * ny + j) * nx + i;

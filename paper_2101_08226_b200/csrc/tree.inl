@@ -29,6 +29,8 @@ struct TreeLevel {
     std::vector<int> h_m2l_tiles, h_p2p_tiles;
     int* ref_nodes;  int n_ref_nodes;     // device: the refined sub-grids of the level, x | y << 10 | z << 20 (box-local, sub-grid units)
     std::vector<int> h_ref_nodes;
+    int* fin_nodes;  int n_fin_nodes;     // device: the sub-grids of the listed leaf tiles (whatever their kind): the cells the leaf
+    std::vector<int> h_fin_nodes;         // finish visits; every other cell of the level's output is zero-filled by a memset
     unsigned char* brick_on;              // device [bricks of the dense enumeration]: 1 = the multipole step ran on this brick
     std::vector<unsigned char> h_brick_on;
     int btx, btz;                         // bricks per x-row and per z-column of that enumeration
@@ -107,7 +109,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
         L.brick_on = nullptr; L.btx = 0; L.btz = 0;
-        L.ref_nodes = nullptr; L.n_ref_nodes = 0;
+        L.ref_nodes = nullptr; L.n_ref_nodes = 0; L.fin_nodes = nullptr; L.n_fin_nodes = 0;
         L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr; L.ev_par = nullptr; L.ev_rdy = nullptr; L.ev_lm = nullptr;
         const unsigned char* k = kind_host[l];
         if (!k) return P;
@@ -223,7 +225,10 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
                         for (int J = 2 * ty; J <= std::min(2 * ty + 1, nny - 1) && !work; ++J)
                             for (int I = 2 * tx; I <= std::min(2 * tx + 1, nnx - 1) && !work; ++I)
                                 work = node_kind(l, gx0 + I, gy0 + J, gz0 + tz) == KIND_LEAF;
-                        if (work) L.h_p2p_tiles.push_back((tz * by + ty) * bx + tx);
+                        if (!work) continue;
+                        L.h_p2p_tiles.push_back((tz * by + ty) * bx + tx);
+                        for (int J = 2 * ty; J <= std::min(2 * ty + 1, nny - 1); ++J)
+                            for (int I = 2 * tx; I <= std::min(2 * tx + 1, nnx - 1); ++I) L.h_fin_nodes.push_back(I | (J << 10) | (tz << 20));
                     }
         }
         L.n_m2l_tiles = (int)L.h_m2l_tiles.size();
@@ -232,8 +237,9 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         const size_t nc = L.cells();
         P.bytes += align_up(nc) + align_up((size_t)nnx * nny * nnz) + align_up(nc * 8);           // kind, nodeflag, lm
         L.n_ref_nodes = (int)L.h_ref_nodes.size();
+        L.n_fin_nodes = (int)L.h_fin_nodes.size();
         P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4) + align_up(L.h_brick_on.size() + 4) +
-                   align_up((size_t)L.n_ref_nodes * 4 + 4);
+                   align_up((size_t)L.n_ref_nodes * 4 + 4) + align_up((size_t)L.n_fin_nodes * 4 + 4);
         if (L.has_refined) {
             octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
             P.bytes += sizes_of(mc, CF_ANY_SIZE).total + align_up(nc * 20 * 8) + align_up(nc * 3 * 8);
@@ -362,12 +368,14 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         L.p2p_tiles = (int*)w; w += align_up((size_t)L.n_p2p_tiles * 4 + 4);
         L.brick_on = (unsigned char*)w; w += align_up(L.h_brick_on.size() + 4);
         L.ref_nodes = (int*)w; w += align_up((size_t)L.n_ref_nodes * 4 + 4);
+        L.fin_nodes = (int*)w; w += align_up((size_t)L.n_fin_nodes * 4 + 4);
         if (cudaMemcpyAsync(L.kind, kind_host[l], nc, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             cudaMemcpyAsync(L.nodeflag, L.h_nodeflag.data(), nn, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             (L.n_m2l_tiles && cudaMemcpyAsync(L.m2l_tiles, L.h_m2l_tiles.data(), (size_t)L.n_m2l_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
             (L.n_p2p_tiles && cudaMemcpyAsync(L.p2p_tiles, L.h_p2p_tiles.data(), (size_t)L.n_p2p_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
             (!L.h_brick_on.empty() && cudaMemcpyAsync(L.brick_on, L.h_brick_on.data(), L.h_brick_on.size(), cudaMemcpyHostToDevice, st) != cudaSuccess) ||
-            (L.n_ref_nodes && cudaMemcpyAsync(L.ref_nodes, L.h_ref_nodes.data(), (size_t)L.n_ref_nodes * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)) {
+            (L.n_ref_nodes && cudaMemcpyAsync(L.ref_nodes, L.h_ref_nodes.data(), (size_t)L.n_ref_nodes * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
+            (L.n_fin_nodes && cudaMemcpyAsync(L.fin_nodes, L.h_fin_nodes.data(), (size_t)L.n_fin_nodes * 4, cudaMemcpyHostToDevice, st) != cudaSuccess)) {
             rc = OCTO_FMM_ECUDA;
             break;
         }
@@ -421,7 +429,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     // the topology arrays were copied from pageable host memory: make sure they have left it before returning
     if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
-    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_brick_on.clear(); L.h_ref_nodes.clear(); }
+    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_brick_on.clear(); L.h_ref_nodes.clear(); L.h_fin_nodes.clear(); }
     *out = t;
     return OCTO_FMM_OK;
 }
@@ -472,6 +480,8 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_leaf>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
         if (cudaEventRecord(L.ev_lm, L.s_leaf) != cudaSuccess) return OCTO_FMM_ECUDA;
+        // the level's output: zero wherever the leaf finish does not go (it visits the sub-grids of the leaf tiles only)
+        if (cudaMemsetAsync(out[l], 0, (size_t)nc * (rhs2 ? 1 : 4) * sizeof(double), L.s_leaf) != cudaSuccess) return OCTO_FMM_ECUDA;
     }
     for (int l = D - 1; l >= 0; --l) {
         TreeLevel& L = t->lev[l];
@@ -626,7 +636,8 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             }
             if (l > 0) { a.kind_c = t->lev[l - 1].kind; a.mass_c = t->lev[l - 1].lm; }
             a.count = count ? t->counts : nullptr;
-            tree_leaf_finish_kernel<<<blocks, 128, 0, sf>>>(a);
+            a.nodes = L.fin_nodes;
+            if (L.n_fin_nodes > 0) tree_leaf_finish_kernel<<<4u * (unsigned)L.n_fin_nodes, 128, 0, sf>>>(a);
             if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
             if (count) {
                 tree_count_kernel<<<blocks, 128, 0, sf>>>(L.kind, L.n[0], L.n[1], L.n[2], t->counts);
@@ -737,7 +748,7 @@ int octo_fmm_tree_launches(const octo_fmm_tree_t* t, int* launches)
         n += 1 + (l.has_refined ? 1 : 0);                                  // leaf moments, M2M
         if (l.fmm && l.n_m2l_tiles > 0) n += 4;                            // stage, flags, multipole step, L2L
         if (l.leaf) n += 2;                                                // stage, leaf-leaf sums
-        n += 1;                                                            // leaf finish
+        if (l.n_fin_nodes > 0) n += 1;                                     // leaf finish
     }
     n += 4 * (int)t->up.size();
     *launches = n;
