@@ -99,7 +99,7 @@ struct TreeFinishArgs {
     double* out;                    // [4][cells]: in = leaf-leaf point-mass sums of the tensor-core kernel; out = (phi, g)
     const double* L;                // this level's own multipole step [20][cells], as stored by the brick kernel (correction
                                     // folded into L1); read at the leaves of sub-grids flagged NODE_OWN_L only, and there
-    const unsigned char* brick_on;  // only in the 16 x 8 x 3 bricks the step ran on: brick_on[((j / 8) btx + i / 16) btz + k / 3]
+    const unsigned char* brick_on;  // only in the 16 x 8 x 3 bricks the step ran on: brick_on[((j / TILE_Y) btx + i / TILE_X) btz + k / TILE_Z]
     int btx, btz;                   // (the others have no refined cell within the lists' reach: their part is exactly zero)
     const double* pL;               // parent level [20][pn cells], pC [3][..], poff [3][..]
     const double* pC;
@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
     double v[4];
 #pragma unroll
     for (int c = 0; c < 4; ++c) v[c] = a.out[c * ncell + cell];
-    if ((flag & NODE_OWN_L) && a.brick_on[((j >> 3) * a.btx + (i >> 4)) * a.btz + k / 3]) {
+    if ((flag & NODE_OWN_L) && a.brick_on[((j / TILE_Y) * a.btx + i / TILE_X) * a.btz + k / TILE_Z]) {
         // this level's own multipole step (refined partners of the Eq. 15 list), as the brick kernel stored it: the
         // correction folded into L1
         v[0] += a.L[cell];
