@@ -100,6 +100,9 @@ struct Params {
     // zr[pz] = {first, last} dz with a list entry for targets of z-parity pz (theta = 0.5: {-4, 5} for even layers, {-5, 4}
     // for odd ones): the slabs a brick streams are the union over its layers, not k0 - reach .. k0 + TILE_Z - 1 + reach
     int zr[2][2];
+    // levels of an adaptive tree (with tile_list): per listed brick, which of its source layers hold anything it can meet --
+    // bit i = layer k0 - REACH_MAX + i; the others are neither loaded nor walked.  nullptr = all.
+    const unsigned short* tile_zmask;
 };
 
 // (double)(-d) * h for a multipole list entry's field d8 = 8 d
@@ -363,6 +366,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         const int cls = cls_xy + ((k & 1) << 2);
         int z_lo, z_hi;
         brick_z_range(p, k0, z_lo, z_hi);
+        const unsigned zmask = (MODE == MODE_TREE && p.tile_zmask) ? p.tile_zmask[t] : 0xffffu;
 
         double dA[3] = {0.0, 0.0, 0.0}, tA[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
         bool leafA = false;
@@ -399,6 +403,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
                     open = false;
                 }
                 if (++zz > z_hi) return false;
+                if (MODE == MODE_TREE && !((zmask >> (zz - k0 + REACH_MAX)) & 1u)) continue;      // not loaded (producer: the same test)
                 b = it % NSTAGE;
                 mbar_wait(&full[b], (it / NSTAGE) & 1);
                 open = true;
@@ -511,7 +516,9 @@ m2l_staged_kernel(const __grid_constant__ SlabMaps maps, const __grid_constant__
                 decode_tile(p, t, x0, y0, k0);
                 int z_lo, z_hi;
                 brick_z_range(p, k0, z_lo, z_hi);
+                const unsigned zmask = (MODE == MODE_TREE && p.tile_zmask) ? p.tile_zmask[t] : 0xffffu;
                 for (int zz = z_lo; zz <= z_hi; ++zz) {
+                    if (MODE == MODE_TREE && !((zmask >> (zz - k0 + REACH_MAX)) & 1u)) continue;
                     const uint32_t b = it % NSTAGE;
                     if (it >= NSTAGE) mbar_wait_backoff(&empty[b], ((it / NSTAGE) - 1) & 1);
                     mbar_arrive_expect_tx(&full[b], SLAB_BYTES);

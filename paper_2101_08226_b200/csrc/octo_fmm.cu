@@ -299,6 +299,7 @@ struct octo_fmm {
     // a level of the adaptive tree solve (tree.inl): the kinds of its cells, and the bricks / tiles that have work
     const unsigned char* tree_kind;   // device [n^3]; non-null: the slab-fed kernel runs in MODE_TREE
     const int* tile_list;             // device; null = every brick (multipole) / tile (monopole)
+    const unsigned short* tile_zmask; // device, per listed brick (multipole, tree levels): source layers worth loading; null = all
     int tile_count;
     int mono_zt_begin, mono_zt_end;   // tensor-core monopole kernels: z-tiles [begin, end) of this launch; end = 0: all
     int* pinned_flag;      // pinned host word the host entry points read the device flag through (no pageable copy)
@@ -397,7 +398,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     h->mixed_counted = false;
     h->host_chunk = 12;
     h->host_launches = 0;
-    h->tree_kind = nullptr; h->tile_list = nullptr; h->tile_count = 0;
+    h->tree_kind = nullptr; h->tile_list = nullptr; h->tile_count = 0; h->tile_zmask = nullptr;
     h->mono_zt_begin = 0; h->mono_zt_end = 0; h->pinned_flag = nullptr;
     h->pipeline_ready = false;
     h->s_h2d = nullptr; h->s_d2h = nullptr;
@@ -518,6 +519,7 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
     P.pL = nullptr; P.pC = nullptr; P.poff = nullptr; P.hc = cfg->h;
     P.leaf = nullptr;
     P.tile_list = nullptr;
+    P.tile_zmask = nullptr;
     P.tile_offset = 0;
     for (int a = 0; a < 3; ++a) { P.pdim[a] = cfg->n[a] / 2; P.psh[a] = 0; }
     for (int d = 0; d <= 2 * REACH_MAX; ++d) P.hmul[d] = h->hmul[d];
@@ -694,7 +696,7 @@ static int launch_staged(octo_fmm_t* h, int kb, int ke, bool mixed = false)
     P.kb = kb; P.ke = ke;
     P.tiles_z = (ke - kb + TILE_Z - 1) / TILE_Z;
     P.ntiles = (long long)P.tiles_x * P.tiles_y * P.tiles_z;
-    if (h->tile_list) { P.tile_list = h->tile_list; P.ntiles = h->tile_count; }     // whole-grid launches only (tree levels)
+    if (h->tile_list) { P.tile_list = h->tile_list; P.tile_zmask = h->tile_zmask; P.ntiles = h->tile_count; }     // whole-grid launches only (tree levels)
     const int grid = (int)std::min<long long>(P.ntiles, h->sm_count);
     if (grid == 0) return OCTO_FMM_OK;
     if (h->tree_kind) {    // a level of the adaptive tree: absent cells, leaf-leaf pairs left to the leaf kernel

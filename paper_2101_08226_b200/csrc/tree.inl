@@ -27,6 +27,8 @@ struct TreeLevel {
     int* m2l_tiles;  int n_m2l_tiles;     // bricks of the slab-fed kernel that have work
     int* p2p_tiles;  int n_p2p_tiles;     // 16 x 16 x 8 tiles of the tensor-core kernel that hold leaves
     std::vector<int> h_m2l_tiles, h_p2p_tiles;
+    unsigned short* m2l_zmask;            // device, per listed brick: source layers that hold anything the brick can meet
+    std::vector<unsigned short> h_m2l_zmask;
     int* ref_nodes;  int n_ref_nodes;     // device: the refined sub-grids of the level, x | y << 10 | z << 20 (box-local, sub-grid units)
     std::vector<int> h_ref_nodes;
     int* fin_nodes;  int n_fin_nodes;     // device: the sub-grids of the listed leaf tiles (whatever their kind): the cells the leaf
@@ -109,6 +111,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         L.fmm = nullptr; L.leaf = nullptr; L.kind = nullptr; L.nodeflag = nullptr; L.lm = nullptr; L.raw = nullptr; L.off = nullptr;
         L.m2l_tiles = nullptr; L.p2p_tiles = nullptr; L.n_m2l_tiles = 0; L.n_p2p_tiles = 0;
         L.brick_on = nullptr; L.btx = 0; L.btz = 0;
+        L.m2l_zmask = nullptr;
         L.ref_nodes = nullptr; L.n_ref_nodes = 0; L.fin_nodes = nullptr; L.n_fin_nodes = 0;
         L.s_m2l = nullptr; L.s_leaf = nullptr; L.ev_m2l = nullptr; L.ev_leaf = nullptr; L.ev_par = nullptr; L.ev_rdy = nullptr; L.ev_lm = nullptr;
         const unsigned char* k = kind_host[l];
@@ -214,6 +217,31 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
             // bricks that are full of refined cells instead of whoever comes first in lattice order getting three of them
             std::sort(weighted.begin(), weighted.end());
             for (const auto& wt : weighted) L.h_m2l_tiles.push_back(wt.second);
+            // per brick, the source layers worth loading: a brick with refined targets meets every cell that exists, a
+            // brick of leaves only refined ones; layers whose 26 x 18 footprint holds none are left out (bit i = layer
+            // k0 - REACH_MAX + i).  Kinds are constant over sub-grids, so sub-grids are what is tested.
+            for (const int tile : L.h_m2l_tiles) {
+                const int tz = tile % tz_n, tx = (tile / tz_n) % tx_n, ty = tile / (tz_n * tx_n);
+                const int x0 = tx * TILE_X, y0 = ty * TILE_Y, k0 = tz * TILE_Z;
+                bool refined_targets = false;
+                for (int K = k0 / 8; K <= std::min(k0 + TILE_Z - 1, L.n[2] - 1) / 8 && !refined_targets; ++K)
+                    for (int I = x0 / 8; I <= std::min(x0 + TILE_X - 1, L.n[0] - 1) / 8 && !refined_targets; ++I)
+                        refined_targets = node_kind(l, gx0 + I, gy0 + y0 / 8, gz0 + K) == KIND_REFINED;
+                unsigned short mask = 0;
+                for (int i = 0; i < TILE_Z + 2 * REACH_MAX; ++i) {
+                    const int zz = k0 - REACH_MAX + i;
+                    if (zz < 0 || zz >= L.n[2]) continue;
+                    bool any = false;
+                    for (int J = floor_div8(y0 - REACH_MAX); J <= floor_div8(y0 + TILE_Y - 1 + REACH_MAX) && !any; ++J)
+                        for (int I = floor_div8(x0 - REACH_MAX); I <= floor_div8(x0 + TILE_X - 1 + REACH_MAX) && !any; ++I) {
+                            if (I < 0 || J < 0 || I >= nnx || J >= nny) continue;
+                            const unsigned char v = node_kind(l, gx0 + I, gy0 + J, gz0 + zz / 8);
+                            any = refined_targets ? v != KIND_ABSENT : v == KIND_REFINED;
+                        }
+                    if (any) mask |= (unsigned short)(1u << i);
+                }
+                L.h_m2l_zmask.push_back(mask);
+            }
         }
         // tiles of the tensor-core leaf kernel: 16 x 16 x 8 cells, b = (tz * by + ty) * bx + tx
         if (L.has_leaf) {
@@ -238,7 +266,7 @@ TreePlan tree_plan(const octo_fmm_tree_config& cfg, const unsigned char* const* 
         P.bytes += align_up(nc) + align_up((size_t)nnx * nny * nnz) + align_up(nc * 8);           // kind, nodeflag, lm
         L.n_ref_nodes = (int)L.h_ref_nodes.size();
         L.n_fin_nodes = (int)L.h_fin_nodes.size();
-        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4) + align_up(L.h_brick_on.size() + 4) +
+        P.bytes += align_up((size_t)L.n_m2l_tiles * 4 + 4) + align_up((size_t)L.n_m2l_tiles * 2 + 4) + align_up((size_t)L.n_p2p_tiles * 4 + 4) + align_up(L.h_brick_on.size() + 4) +
                    align_up((size_t)L.n_ref_nodes * 4 + 4) + align_up((size_t)L.n_fin_nodes * 4 + 4);
         if (L.has_refined) {
             octo_fmm_config mc = box_config(sc, L.n, L.h, OCTO_FMM_MULTIPOLE);
@@ -366,12 +394,14 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         L.lm = (double*)w; w += align_up(nc * 8);
         L.m2l_tiles = (int*)w; w += align_up((size_t)L.n_m2l_tiles * 4 + 4);
         L.p2p_tiles = (int*)w; w += align_up((size_t)L.n_p2p_tiles * 4 + 4);
+        L.m2l_zmask = (unsigned short*)w; w += align_up((size_t)L.n_m2l_tiles * 2 + 4);
         L.brick_on = (unsigned char*)w; w += align_up(L.h_brick_on.size() + 4);
         L.ref_nodes = (int*)w; w += align_up((size_t)L.n_ref_nodes * 4 + 4);
         L.fin_nodes = (int*)w; w += align_up((size_t)L.n_fin_nodes * 4 + 4);
         if (cudaMemcpyAsync(L.kind, kind_host[l], nc, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             cudaMemcpyAsync(L.nodeflag, L.h_nodeflag.data(), nn, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             (L.n_m2l_tiles && cudaMemcpyAsync(L.m2l_tiles, L.h_m2l_tiles.data(), (size_t)L.n_m2l_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
+            (L.n_m2l_tiles && cudaMemcpyAsync(L.m2l_zmask, L.h_m2l_zmask.data(), (size_t)L.n_m2l_tiles * 2, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
             (L.n_p2p_tiles && cudaMemcpyAsync(L.p2p_tiles, L.h_p2p_tiles.data(), (size_t)L.n_p2p_tiles * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
             (!L.h_brick_on.empty() && cudaMemcpyAsync(L.brick_on, L.h_brick_on.data(), L.h_brick_on.size(), cudaMemcpyHostToDevice, st) != cudaSuccess) ||
             (L.n_ref_nodes && cudaMemcpyAsync(L.ref_nodes, L.h_ref_nodes.data(), (size_t)L.n_ref_nodes * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) ||
@@ -398,6 +428,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
             L.fmm->kernel = 0;                 // the slab-fed kernel (MODE_TREE), whatever the size of the level
             L.fmm->tree_kind = L.kind;
             L.fmm->tile_list = L.m2l_tiles;
+            L.fmm->tile_zmask = L.m2l_zmask;
             L.fmm->tile_count = L.n_m2l_tiles;
         }
         if (L.has_leaf) {
@@ -429,7 +460,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     // the topology arrays were copied from pageable host memory: make sure they have left it before returning
     if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
-    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_brick_on.clear(); L.h_ref_nodes.clear(); L.h_fin_nodes.clear(); }
+    for (TreeLevel& L : t->lev) { L.h_m2l_tiles.clear(); L.h_p2p_tiles.clear(); L.h_nodeflag.clear(); L.h_brick_on.clear(); L.h_ref_nodes.clear(); L.h_fin_nodes.clear(); L.h_m2l_zmask.clear(); }
     *out = t;
     return OCTO_FMM_OK;
 }
