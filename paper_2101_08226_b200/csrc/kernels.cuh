@@ -50,7 +50,8 @@ struct StEntry {
     int off;                 // multipole: shared-memory offset of the source relative to the thread's base in the slab, in
                              // BYTES; monopole: offset in the mass tile (doubles, low 16 bits) + index of the weights (high 16)
     signed char dx, dy, dz, d2;   // the offset.  MULTIPOLE lists hold 8 dx, 8 dy, 8 dz: byte offsets into Params::hmul, ready
-                                  // for the list walk of the slab-fed kernel (cell offsets: entry_cells());   // d2: monopole handles |Delta|^2; mixed-level lists 1 = near-field entry (not well separated)
+                                  // for the list walk of the slab-fed kernel (cell offsets: entry_cells());   // d2: monopole handles |Delta|^2; mixed-level lists 1 = near-field entry (not well separated);
+                                  // multipole lists: the sub-grids the partners of a warp's targets fall into (bits 0-2 x, 3-5 y; MODE_TREE)
 };
 
 // Stencil tables (the interaction lists of the 8 parity classes, Eq. 15) in constant memory.  They depend on
@@ -342,7 +343,9 @@ __device__ __forceinline__ void store_target(const Params& p, const Acc& acc, co
 // since every term of the pair carries a power of 1/r it contributes exactly nothing.
 // MODE_TREE (a level of the adaptive tree solve, f3 reading R9): p.leaf holds the KIND of every cell (0 absent, 1 leaf,
 // 2 refined); absent cells are no targets (as sources their staged record is all zeros), and two leaves do not meet here
-// (they are point masses: the tensor-core leaf kernel takes them), again through 1/r = 0.
+// (they are point masses: the tensor-core leaf kernel takes them), again through 1/r = 0.  Kinds must be constant over
+// sub-grids of 8^3 cells (the tree solve checks it): list entries that count for no lane of a warp are found from the
+// kinds of the sub-grids around it and never fetched.
 constexpr int MODE_PLAIN = 0, MODE_MIXED = 1, MODE_TREE = 2;
 template <bool CORR, bool DIPOLE, bool FUSE_L2L, int MODE>
 __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, uint64_t* full, uint64_t* empty, int warp, int lane)
@@ -378,6 +381,31 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
             present = kd != 0;
         }
         if (present) load_target<CORR>(p, gx, gy, k, dA, tA);
+        // MODE_TREE: which list entries can count for this warp at all is known from the kinds of the SUB-GRIDS around it
+        // (kinds are constant over the 8^3 cells of a sub-grid).  The warp's targets lie in two sub-grids next to each
+        // other in x (lanes with lx < 4 / lx >= 4); a refined target meets every partner that exists, a leaf only refined
+        // ones, an absent one nothing.  nab[sz] has bit 4 (sy + 1) + (sx + 1) set if the partners that fall into the
+        // sub-grid (sx, sy, sz) away from their target's hold anything to meet; an entry knows (StEntry::d2) which (sx, sy)
+        // its partners fall into, its slab which sz.  Entries that meet nothing are passed over without a load or a vote
+        unsigned nab[3] = {0u, 0u, 0u};
+        if constexpr (MODE == MODE_TREE) {
+            const unsigned lo4 = 0x0f0f0f0fu;
+            const unsigned ref = __ballot_sync(0xffffffffu, present && !leafA), lf = __ballot_sync(0xffffffffu, present && leafA);
+            const int sx = (lane & 3) - 1, sy = ((lane >> 2) & 3) - 1;          // lanes 0..11: the 4 x 3 sub-grids of a layer
+            const int X = ((x0 >> 3) + sx) * 8, Y = ((y0 >> 3) + sy) * 8;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const int Z = ((k >> 3) + c - 1) * 8;
+                unsigned char kd = 0;
+                if (lane < 12 && layer_on && X >= 0 && Y >= 0 && Z >= 0 && X < p.nx && Y < p.ny && Z < p.nz)
+                    kd = p.leaf[((long long)Z * p.ny + Y) * p.nx + X];
+                const unsigned ex = __ballot_sync(0xffffffffu, kd != 0), rf = __ballot_sync(0xffffffffu, kd == 2);
+                const unsigned na = (ref & lo4) ? ex : ((lf & lo4) ? rf : 0u);
+                const unsigned nb = (ref & ~lo4) ? ex : ((lf & ~lo4) ? rf : 0u);
+                nab[c] = (na & 0x777u) | ((nb >> 1) & 0x777u);
+            }
+        }
+        unsigned nseg = 0u;
 
         Acc acc;
         acc_zero(acc);
@@ -395,6 +423,7 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
         // make (s < s_end) true by moving on to the next slab this layer uses; every slab of the
         // brick is waited for and released, used or not.  false at the end of the brick.
         auto ensure = [&]() -> bool {
+          for (;;) {
             while (s >= s_end) {
                 if (open) {                        // every load from this slab has been issued
                     __syncwarp();
@@ -413,71 +442,73 @@ __device__ __forceinline__ void staged_consume(const Params& p, double2* slab0, 
                     Rz0 = p.hmul[dz + REACH_MAX] + dA[2];
                     s = (cls * MAX_LIST + c_begin[cls][dz + REACH_MAX]) * (int)sizeof(StEntry);       // byte offsets
                     s_end = (cls * MAX_LIST + c_begin[cls][dz + REACH_MAX + 1]) * (int)sizeof(StEntry);
+                    if constexpr (MODE == MODE_TREE) {
+                        const int sz = ((k & 7) + dz + 8) >> 3;           // 0, 1, 2: the sub-grid layer below, of, above the target
+                        nseg = sz == 0 ? nab[0] : (sz == 1 ? nab[1] : nab[2]);
+                        if (nseg == 0u) s = s_end;             // nothing to meet in the sub-grid layer this slab lies in
+                    }
                 }
             }
-            return true;
+            if constexpr (MODE != MODE_TREE) return true;
+            else {
+                // pass over the entries whose partner sub-grids hold nothing to meet (all of it warp-uniform)
+                do {
+                    const unsigned d2 = (unsigned)reinterpret_cast<const StEntry*>(reinterpret_cast<const char*>(c_entries) + s)->d2;
+                    const unsigned pat = (d2 & 7u) * (((d2 >> 3) * 0x49u) & 0x111u);     // x bits into the rows of its y bits
+                    if (pat & nseg) return true;
+                    s += (int)sizeof(StEntry);
+                } while (s < s_end);
+            }
+          }
         };
-#define OCTO_FETCH(P, SKIP)                                                                 \
+#define OCTO_FETCH(P)                                                                       \
         {                                                                                   \
             const StEntry e_ = *reinterpret_cast<const StEntry*>(reinterpret_cast<const char*>(c_entries) + s); \
             s += (int)sizeof(StEntry);                                                      \
             const double2* q_ = reinterpret_cast<const double2*>(reinterpret_cast<const char*>(sl) + e_.off); \
-            bool masked_ = false;                                                           \
-            P.live = true;                                                                  \
-            if (MODE == MODE_TREE) {                                                        \
-                /* the partner's kind first: absent, or a leaf meeting a leaf -> this lane takes nothing; if that holds \
-                   for the whole warp (kinds are constant over sub-grids: the usual case next to a refinement boundary) \
-                   the pair is skipped altogether */                                        \
-                const double kb_ = q_[9 * SLAB_PLANE].y;                                      \
-                masked_ = !present || kb_ == 0.0 || (leafA && kb_ == 1.0);                  \
-                if (SKIP) P.live = !__all_sync(0xffffffffu, masked_);                       \
-            }                                                                               \
-            if (P.live) {                                                                   \
-                double bx_, by_, bz_, fl_ = 0.0;                                            \
-                if (MODE != MODE_PLAIN) { OCTO_LOAD_SOURCE_F(q_, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
-                else       { OCTO_LOAD_SOURCE(q_, SLAB_PLANE, P.src, bx_, by_, bz_); }      \
-                P.x = hmul_at(p, e_.dx) + (dA[0] - bx_);                                    \
-                P.y = hmul_at(p, e_.dy) + (dA[1] - by_);                                    \
-                P.z = Rz0 - bz_;                                                            \
-                P.w = pair_head(P.x, P.y, P.z);                                             \
-                if (MODE == MODE_MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;         \
-                if (MODE == MODE_TREE && masked_) P.w = 0.0;                                \
-            }                                                                               \
+            double bx_, by_, bz_, fl_ = 0.0;                                                \
+            if (MODE != MODE_PLAIN) { OCTO_LOAD_SOURCE_F(q_, SLAB_PLANE, P.src, bx_, by_, bz_, fl_); } \
+            else       { OCTO_LOAD_SOURCE(q_, SLAB_PLANE, P.src, bx_, by_, bz_); }          \
+            P.x = hmul_at(p, e_.dx) + (dA[0] - bx_);                                        \
+            P.y = hmul_at(p, e_.dy) + (dA[1] - by_);                                        \
+            P.z = Rz0 - bz_;                                                                \
+            P.w = pair_head(P.x, P.y, P.z);                                                 \
+            if (MODE == MODE_MIXED && e_.d2 && !leafA && fl_ == 0.0) P.w = 0.0;             \
+            /* MODE_TREE: the partner is absent, or a leaf meets a leaf -> this lane takes nothing */ \
+            if (MODE == MODE_TREE && (!present || fl_ == 0.0 || (leafA && fl_ == 1.0))) P.w = 0.0; \
         }
-        struct Fetched { double src[16]; double x, y, z, w; bool live; } A, B;
+        struct Fetched { double src[16]; double x, y, z, w; } A, B;
 #define OCTO_BODY(P) m2l_pair<CORR, DIPOLE>(acc, P.x, P.y, P.z, P.w, P.src, tA)
+        // the loop over the entries, software-pipelined two deep (see above); a lane whose pair does not count has 1/r = 0
+#define OCTO_LOOP()                                                                         \
+        if (ensure()) {                                                                     \
+            OCTO_FETCH(A);                                                                  \
+            for (;;) {                                                                      \
+                if (!ensure()) break;                                                       \
+                OCTO_FETCH(B);                                                              \
+                OCTO_BODY(A);                                                               \
+                if (!ensure()) { A = B; break; }                                            \
+                OCTO_FETCH(A);                                                              \
+                OCTO_BODY(B);                                                               \
+            }                                                                               \
+            OCTO_BODY(A);                                                                   \
+        }
         bool leaf_warp = false;
         if constexpr (MODE == MODE_TREE) leaf_warp = __all_sync(0xffffffffu, !present || leafA);
         if (leaf_warp) {
-            // MODE_TREE, a warp of LEAF targets (the shell of leaves around a refined region: most bricks of a level).  Most of
-            // its list entries meet leaves or nothing: a pair that is masked for the whole warp is skipped (one LDS and a
-            // vote instead of 340 cycles).  No hand pipelining here: with whole pairs skipped the two-deep scheme would have
-            // to keep both fetched pairs alive across a branch (it spills 2 KB).  And a leaf has no children: of its
-            // expansion only L0 and L1 (+ correction) are ever used -- the leaf finish evaluates them at the cell centre.
-            // The order-2 and order-3 sums are discarded after the loop, which makes them dead: the compiler drops their
-            // instructions from this copy of the loop (83 instead of 117 per pair)
-            while (ensure()) {
-                OCTO_FETCH(A, true);
-                if (A.live) OCTO_BODY(A);
-            }
+            // MODE_TREE, a warp of LEAF targets (the shell of leaves around a refined region: most bricks of a level).  A
+            // leaf has no children: of its expansion only L0 and L1 (+ correction) are ever used -- the leaf finish evaluates
+            // them at the cell centre.  The order-2 and order-3 sums are discarded after the loop, which makes them dead:
+            // the compiler drops their instructions from this copy of the loop (83 instead of 117 per pair)
+            OCTO_LOOP()
 #pragma unroll
             for (int i = 0; i < 5; ++i) acc.l2[i] = 0.0;
 #pragma unroll
             for (int i = 0; i < 7; ++i) acc.l3[i] = 0.0;
-        } else if (ensure()) {
-            // every other warp (MODE_TREE: its targets are refined cells, for which every partner that exists counts):
-            // the pipelined loop over all entries; a lane whose pair does not count has 1/r = 0
-            OCTO_FETCH(A, false);
-            for (;;) {
-                if (!ensure()) break;
-                OCTO_FETCH(B, false);
-                OCTO_BODY(A);
-                if (!ensure()) { A = B; break; }
-                OCTO_FETCH(A, false);
-                OCTO_BODY(B);
-            }
-            OCTO_BODY(A);
+        } else {
+            OCTO_LOOP()
         }
+#undef OCTO_LOOP
 #undef OCTO_BODY
 #undef OCTO_FETCH
 

@@ -468,7 +468,16 @@ static int create_internal(const octo_fmm_config* cfg, int flags, octo_fmm_t** o
             if (cfg->kind == OCTO_FMM_MULTIPOLE) {
                 e.off = ((py + dy + REACH_MAX) * SLAB_ROW + (((px + dx) & 1) ? SLAB_XH : 0) + ((px + dx + 6) >> 1)) * 16;   // bytes
                 e.dx = (signed char)(8 * dx); e.dy = (signed char)(8 * dy); e.dz = (signed char)(8 * dz);      // see StEntry
-                e.d2 = 0;
+                // which sub-grids (8 cells per axis) the partners of a warp's targets fall into, relative to the targets'
+                // own: a warp holds the 4 x 4 cells of one parity class of one sub-grid (twice), cell c = p + 2 j, so the
+                // partner c + d lies in sub-grid floor((p + d + 2 j) / 8) in {-1, 0, 1}.  Bits 0-2: x, bits 3-5: y
+                // (the levels of the adaptive tree skip entries whose partner sub-grids hold nothing to meet)
+                int xm = 0, ym = 0;
+                for (int j = 0; j < 4; ++j) {
+                    xm |= 1 << (floor_div8(px + dx + 2 * j) + 1);
+                    ym |= 1 << (floor_div8(py + dy + 2 * j) + 1);
+                }
+                e.d2 = (signed char)(xm | (ym << 3));
             } else {
                 // monopole: offset in the de-interleaved mass tile (doubles, low 16 bits) and index of the offset's
                 // weights (high 16 bits), see p2p_monopole_kernel
