@@ -1,6 +1,7 @@
 """Search for the statement order of m2l_pair_folded (developer tool; needs nvcc and cuobjdump, no GPU).
 
-    python -m paper_2101_08226_b200.order_search [--function folded|components] [--minutes M] [--seed S] [--random N] [--apply]
+    python -m paper_2101_08226_b200.order_search [--function folded|components] [--minutes M] [--seed S] [--random N]
+                                                 [--weights A B] [--apply]
 
 Why: the interaction kernel is bound by the FP64 pipe, and a DFMA whose three source registers all have to be read
 fresh holds the pipe for 3 cycles instead of 2.  Whether consecutive instructions share an
@@ -148,15 +149,20 @@ def score(args):
     return cyc if len(cyc) >= 6 else None
 
 
+WEIGHTS = (1.0, 0.25)       # of the general path and of the path without dipole terms (--weights A B)
+
+
 def objective(cyc):
-    return 1e9 if cyc is None else cyc[0] + cyc[1] + 0.25 * (cyc[3] + cyc[4])
+    return 1e9 if cyc is None else WEIGHTS[0] * (cyc[0] + cyc[1]) + WEIGHTS[1] * (cyc[3] + cyc[4])
 
 
 def main(argv):
     def opt(name, default):
         return type(default)(argv[argv.index(name) + 1]) if name in argv else default
-    global TARGET
+    global TARGET, WEIGHTS
     minutes, seed, nrandom = opt("--minutes", 10.0), opt("--seed", 1), opt("--random", 64)
+    if "--weights" in argv:
+        WEIGHTS = (float(argv[argv.index("--weights") + 1]), float(argv[argv.index("--weights") + 2]))
     TARGET = opt("--function", "folded")
     if TARGET not in TARGETS:
         raise SystemExit("order_search: --function folded | components")
