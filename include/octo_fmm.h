@@ -390,8 +390,10 @@ int octo_fmm_tree_solve_rhs2(octo_fmm_tree_t *t, const double *const *dmass, dou
 int octo_fmm_tree_interaction_counts(octo_fmm_tree_t *t, const double *const *mass, double *const *out,
                                      unsigned long long counts[3]);
 /* The same with HOST buffers (mass_host[l], out_host[l]: host arrays of the layouts above; pinned memory makes the
- * copies asynchronous): H2D of the masses of every level that has leaves, solve, D2H of every out[l], stream
- * synchronise.  scratch: device, >= octo_fmm_tree_host_scratch_bytes(t), 256-byte aligned, borrowed for the call. */
+ * copies asynchronous): H2D of the masses of every level that has leaves, solve, D2H of every out[l]; the copies
+ * overlap the solve (masses arrive deepest level first on the streams that read them, a level's output leaves as soon
+ * as its leaves are finished).  Returns when every out_host[l] is complete (synchronises the library's streams, not the
+ * caller's).  scratch: device, >= octo_fmm_tree_host_scratch_bytes(t), 256-byte aligned, borrowed for the call. */
 size_t octo_fmm_tree_host_scratch_bytes(const octo_fmm_tree_t *t);
 int octo_fmm_tree_solve_host(octo_fmm_tree_t *t, const double *const *mass_host, double *const *out_host, void *scratch,
                              size_t scratch_bytes);

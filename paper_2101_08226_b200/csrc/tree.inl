@@ -299,6 +299,7 @@ struct octo_fmm_tree {
     unsigned long long* counts;        // device [3]: m2l, p2p, cross
     cudaStream_t stream;               // the solve's own main stream (high priority): upward pass, uniform levels, L2L chain
     cudaStream_t pool_m2l[3], pool_leaf[2];   // the levels share a few side streams (see octo_fmm_tree_create)
+    cudaStream_t s_d2h;                // octo_fmm_tree_solve_host: the copies out (created on first use)
     cudaStream_t user;                 // the caller's stream (cfg.stream): a solve starts after and is joined into it
     cudaEvent_t ev_user;               // hand-over between the two
     cudaEvent_t ev_up;                 // a solve has begun on the main stream (the side streams start behind it)
@@ -335,6 +336,7 @@ int octo_fmm_tree_destroy(octo_fmm_tree_t* t)
     if (t->ev_user) cudaEventDestroy(t->ev_user);
     for (cudaStream_t& q : t->pool_m2l) if (q) cudaStreamDestroy(q);
     for (cudaStream_t& q : t->pool_leaf) if (q) cudaStreamDestroy(q);
+    if (t->s_d2h) cudaStreamDestroy(t->s_d2h);
     if (t->stream) cudaStreamDestroy(t->stream);
     delete t;
     return rc;
@@ -737,24 +739,34 @@ int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host,
     std::vector<const double*> m(D);
     std::vector<double*> o(D);
     char* w = (char*)scratch;
-    cudaStream_t st = t->stream;
-    if (tree_enter(t) != OCTO_FMM_OK) return OCTO_FMM_ECUDA;
     for (int l = 0; l < D; ++l) {
         if (!mass_host[l] || !out_host[l]) return OCTO_FMM_EINVAL;
         const size_t nc = t->lev[l].cells();
-        double* dm = (double*)w; w += align_up(nc * 8);
+        m[l] = (double*)w; w += align_up(nc * 8);
         o[l] = (double*)w; w += align_up(nc * 4 * 8);
-        m[l] = dm;
+    }
+    if (!t->s_d2h && cudaStreamCreateWithFlags(&t->s_d2h, cudaStreamNonBlocking) != cudaSuccess) return OCTO_FMM_ECUDA;
+    // The copies overlap the solve.  IN: a level's masses are read by one kernel only, the first one on the level's leaf
+    // stream -- they are copied on that stream, ahead of it, deepest level first (the upward pass starts at the bottom).
+    // OUT: a level's output is complete when its leaf finish is (ev_leaf), coarsest level first, long before the solve
+    // ends: it leaves on a copy stream from then on.
+    if (cudaEventRecord(t->ev_user, t->user) != cudaSuccess) return OCTO_FMM_ECUDA;
+    for (cudaStream_t q : t->pool_leaf)
+        if (cudaStreamWaitEvent(q, t->ev_user, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+    for (int l = D - 1; l >= 0; --l) {
+        TreeLevel& L = t->lev[l];
         // a level without leaves has nothing to bring (its masses are never read) and nothing to take back but zeros
-        if (t->lev[l].has_leaf && cudaMemcpyAsync(dm, mass_host[l], nc * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (L.has_leaf && cudaMemcpyAsync((double*)m[l], mass_host[l], L.cells() * 8, cudaMemcpyHostToDevice, L.s_leaf) != cudaSuccess)
+            return OCTO_FMM_ECUDA;
     }
     const int rc = tree_solve_impl(t, m.data(), o.data(), false);
     if (rc != OCTO_FMM_OK) return rc;
     for (int l = 0; l < D; ++l) {
-        const size_t nc = t->lev[l].cells();
-        if (cudaMemcpyAsync(out_host[l], o[l], nc * 4 * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return OCTO_FMM_ECUDA;
+        TreeLevel& L = t->lev[l];
+        if (cudaStreamWaitEvent(t->s_d2h, L.ev_leaf, 0) != cudaSuccess ||
+            cudaMemcpyAsync(out_host[l], o[l], L.cells() * 4 * 8, cudaMemcpyDeviceToHost, t->s_d2h) != cudaSuccess) return OCTO_FMM_ECUDA;
     }
-    if (cudaStreamSynchronize(st) != cudaSuccess) return OCTO_FMM_ECUDA;
+    if (cudaStreamSynchronize(t->s_d2h) != cudaSuccess || cudaStreamSynchronize(t->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     return OCTO_FMM_OK;
 }
 

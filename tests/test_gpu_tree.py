@@ -237,6 +237,35 @@ def test_repeated_and_concurrent_solves_are_deterministic(env):
         handles[i].close()
 
 
+def test_tree_solve_host_entry_point(env):
+    """octo_fmm_tree_solve_host (copies in on the leaf streams, solve, copies out level by level as the finishes end)
+    gives the device-pointer route's numbers bit for bit -- on two calls in a row with different masses (the second call
+    meets the first call's contents in the scratch), and a device-pointer solve afterwards is unchanged."""
+    p, torch = env
+    dense = fi.star_tree(32, 3)
+    boxes = fi.tree_boxes(dense)
+    kinds, masses = fi.crop_tree(dense, boxes)
+    t = p.OctoFMMTree(32, dense.h0, 0.5, kinds, True, box=boxes)
+    nb = p.octo_fmm_tree_host_scratch_bytes(t.handle)
+    scratch = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    depth = len(kinds)
+    for scale in (1.0, 0.37):
+        ms = [m * (scale if l % 2 == 0 else 1.0) for l, m in enumerate(masses)]
+        dev = [o.cpu().numpy() for o in t.solve([torch.from_numpy(m).cuda() for m in ms])]
+        m_h = [torch.from_numpy(np.ascontiguousarray(m)).pin_memory() for m in ms]
+        o_h = [torch.full((4,) + t.shape[l], float("nan"), dtype=torch.float64).pin_memory() for l in range(depth)]
+        p.octo_fmm_tree_solve_host(t.handle, m_h, o_h, scratch, nb)
+        for l in range(depth):
+            assert np.array_equal(o_h[l].numpy(), dev[l]), (scale, l)
+        again = [o.cpu().numpy() for o in t.solve([torch.from_numpy(m).cuda() for m in ms])]
+        for l in range(depth):
+            assert np.array_equal(again[l], dev[l])
+    assert t.status() == p.OK
+    with pytest.raises(p.OctoFmmError):
+        p.octo_fmm_tree_solve_host(t.handle, m_h, o_h, scratch, nb - 1)
+    t.close()
+
+
 @pytest.mark.parametrize("boxed", [False, True])
 def test_second_right_hand_side_on_the_tree(env, boxed):
     """octo_fmm_tree_solve_rhs2 (L81-83 on the adaptive mesh): d(phi)/dt of signed sources on the tree and centres of the
