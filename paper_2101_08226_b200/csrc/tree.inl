@@ -750,6 +750,13 @@ int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host,
     // stream -- they are copied on that stream, ahead of it, deepest level first (the upward pass starts at the bottom).
     // OUT: a level's output is complete when its leaf finish is (ev_leaf), coarsest level first, long before the solve
     // ends: it leaves on a copy stream from then on.
+    // (an error after the first copy is queued: whatever was queued still uses the caller's buffers -- wait for it)
+    auto fail = [&](int code) {
+        for (cudaStream_t q : t->pool_leaf) cudaStreamSynchronize(q);
+        cudaStreamSynchronize(t->s_d2h);
+        cudaStreamSynchronize(t->stream);
+        return code;
+    };
     if (cudaEventRecord(t->ev_user, t->user) != cudaSuccess) return OCTO_FMM_ECUDA;
     for (cudaStream_t q : t->pool_leaf)
         if (cudaStreamWaitEvent(q, t->ev_user, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
@@ -757,14 +764,14 @@ int octo_fmm_tree_solve_host(octo_fmm_tree_t* t, const double* const* mass_host,
         TreeLevel& L = t->lev[l];
         // a level without leaves has nothing to bring (its masses are never read) and nothing to take back but zeros
         if (L.has_leaf && cudaMemcpyAsync((double*)m[l], mass_host[l], L.cells() * 8, cudaMemcpyHostToDevice, L.s_leaf) != cudaSuccess)
-            return OCTO_FMM_ECUDA;
+            return fail(OCTO_FMM_ECUDA);
     }
     const int rc = tree_solve_impl(t, m.data(), o.data(), false);
-    if (rc != OCTO_FMM_OK) return rc;
+    if (rc != OCTO_FMM_OK) return fail(rc);
     for (int l = 0; l < D; ++l) {
         TreeLevel& L = t->lev[l];
         if (cudaStreamWaitEvent(t->s_d2h, L.ev_leaf, 0) != cudaSuccess ||
-            cudaMemcpyAsync(out_host[l], o[l], L.cells() * 4 * 8, cudaMemcpyDeviceToHost, t->s_d2h) != cudaSuccess) return OCTO_FMM_ECUDA;
+            cudaMemcpyAsync(out_host[l], o[l], L.cells() * 4 * 8, cudaMemcpyDeviceToHost, t->s_d2h) != cudaSuccess) return fail(OCTO_FMM_ECUDA);
     }
     if (cudaStreamSynchronize(t->s_d2h) != cudaSuccess || cudaStreamSynchronize(t->stream) != cudaSuccess) return OCTO_FMM_ECUDA;
     return OCTO_FMM_OK;
