@@ -28,11 +28,14 @@ constexpr unsigned char NODE_OWN_L = 1;          // leaf sub-grid with a refined
 constexpr unsigned char NODE_COARSE_NBR = 2;     // the parent sub-grid has a LEAF sub-grid among its 26 neighbours one level up
 
 // Moments of the cells that are not refined: a leaf is the point mass at its geometric centre (M0 = m, everything else
-// and the offset 0), an absent cell is all zeros.  The refined cells were written by m2m_kernel before.  lm (may be
-// null): the masked masses [n^3] (m at leaves, 0 elsewhere) for the leaf kernel's staging.
+// and the offset 0), an absent cell is all zeros.  The refined cells are written by m2m_kernel.  Only M0 ever changes from
+// solve to solve: the zeros of raw and off, and of the cell's staged record S (the slab-fed kernel's source array), are
+// written once, at octo_fmm_tree_create (tree_stage_init_kernel) -- per solve a cell that is not refined costs its mass in
+// raw, in lm and in the first component pair of its staged record, 41 bytes instead of the 570 of writing and staging all
+// 23 numbers.  lm (may be null): the masked masses [n^3] (m at leaves, 0 elsewhere) for the leaf kernel's staging.
 __global__ void __launch_bounds__(256) tree_leaf_moments_kernel(const unsigned char* __restrict__ kind, const double* __restrict__ mass,
-                                                                double* __restrict__ raw, double* __restrict__ off,
-                                                                double* __restrict__ lm, long long ncell)
+                                                                double* __restrict__ raw, double* __restrict__ lm,
+                                                                double* __restrict__ S, int nx, int ny, long long ncell)
 {
     const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (cell >= ncell) return;
@@ -41,10 +44,64 @@ __global__ void __launch_bounds__(256) tree_leaf_moments_kernel(const unsigned c
     if (lm) lm[cell] = m;
     if (kd == KIND_REFINED || !raw) return;
     raw[cell] = m;
+    const int x = (int)(cell % nx);
+    const long long r = cell / nx;
+    const int y = (int)(r % ny);
+    const long long z = r / ny;
+    const long long plane = (long long)ny * nx;
+    // (M0, -M1_x) of a point mass at the cell centre, as reduce_moments writes it
+    if (S) reinterpret_cast<double2*>(S)[z * NPAIR * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1)] = make_double2(m, -0.0);
+}
+
+// Once per tree: the staged record of every cell as staging would write it for all-zero moments, with the cell's kind in the
+// padding slot (0 absent, 1 leaf, 2 refined: what MODE_TREE reads beside a partner's moments).
+__global__ void __launch_bounds__(256) tree_stage_init_kernel(const unsigned char* __restrict__ kind, double* __restrict__ S,
+                                                              int nx, int ny, int nz, int corr)
+{
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= (long long)nx * ny * nz) return;
+    const int x = (int)(cell % nx);
+    const long long r = cell / nx;
+    const int y = (int)(r % ny);
+    const long long z = r / ny;
+    double M[20], s[20];
 #pragma unroll
-    for (int t = 1; t < 20; ++t) raw[t * ncell + cell] = 0.0;
+    for (int c = 0; c < 20; ++c) M[c] = 0.0;
+    reduce_moments(M, s, corr != 0);
+    s[C_DX] = 0.0; s[C_DY] = 0.0; s[C_DZ] = 0.0;
+    s[19] = (double)kind[cell];
+    const long long plane = (long long)ny * nx;
+    double2* dst = reinterpret_cast<double2*>(S) + z * NPAIR * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1);
 #pragma unroll
-    for (int c = 0; c < 3; ++c) off[c * ncell + cell] = 0.0;
+    for (int c = 0; c < NPAIR; ++c) dst[(long long)c * plane] = make_double2(s[2 * c], s[2 * c + 1]);
+}
+
+// Per solve: the REFINED cells of a level (the sub-grids of `nodes`, 4 blocks of 128 threads each), staged as
+// stage_multipole_kernel stages a cell -- moments reduced, dipole terms flagged, offsets -- with kind 2 in the padding slot.
+__global__ void __launch_bounds__(128) tree_stage_refined_kernel(const double* __restrict__ mom, const double* __restrict__ com,
+                                                                 double* __restrict__ S, int nx, int ny, int nz, double h,
+                                                                 int* __restrict__ flags, int corr, const int* __restrict__ nodes)
+{
+    const int node = nodes[blockIdx.x >> 2];
+    const int x = 8 * (node & 1023) + (threadIdx.x & 7), y = 8 * ((node >> 10) & 1023) + ((threadIdx.x >> 3) & 7),
+              z = 8 * (node >> 20) + 2 * (blockIdx.x & 3) + (threadIdx.x >> 6);
+    const long long ncell = (long long)nx * ny * nz;
+    const long long cell = ((long long)z * ny + y) * nx + x;
+    double M[20], s[20];
+#pragma unroll
+    for (int c = 0; c < 20; ++c) M[c] = mom[(long long)c * ncell + cell];
+    reduce_moments(M, s, corr != 0);
+    {
+        const double lim = DIPOLE_TOL * fabs(M[0]) * h;
+        if (fabs(M[1]) > lim || fabs(M[2]) > lim || fabs(M[3]) > lim) atomicOr(flags + 1, 2);
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) s[C_DX + c] = com[(long long)c * ncell + cell];
+    s[19] = (double)KIND_REFINED;
+    const long long plane = (long long)ny * nx;
+    double2* dst = reinterpret_cast<double2*>(S) + (long long)z * NPAIR * plane + (long long)y * nx + (x & 1) * (nx >> 1) + (x >> 1);
+#pragma unroll
+    for (int c = 0; c < NPAIR; ++c) dst[(long long)c * plane] = make_double2(s[2 * c], s[2 * c + 1]);
 }
 
 // L2L on a tree level stored as a box: what the fused epilogue of the brick kernel does when the levels run one after the

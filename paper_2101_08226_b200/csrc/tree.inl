@@ -432,6 +432,16 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
             L.fmm->tile_list = L.m2l_tiles;
             L.fmm->tile_zmask = L.m2l_zmask;
             L.fmm->tile_count = L.n_m2l_tiles;
+            // what never changes from solve to solve is written here, once: the zeros of the moments and offsets of the
+            // cells that are not refined (a leaf is a point mass at its centre) and their staged records, with every cell's
+            // kind in the padding slot (tree.cuh: tree_leaf_moments_kernel)
+            if (cudaMemsetAsync(L.raw, 0, nc * 20 * 8, st) != cudaSuccess || cudaMemsetAsync(L.off, 0, nc * 3 * 8, st) != cudaSuccess) {
+                rc = OCTO_FMM_ECUDA;
+                break;
+            }
+            tree_stage_init_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, st>>>(L.kind, L.fmm->src, L.n[0], L.n[1], L.n[2],
+                                                                              L.fmm->cfg.am_correction);
+            if (cudaGetLastError() != cudaSuccess) { rc = OCTO_FMM_ECUDA; break; }
         }
         if (L.has_leaf) {
             octo_fmm_config lc = box_config(sc, L.n, L.h, OCTO_FMM_MONOPOLE);
@@ -509,8 +519,9 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         TreeLevel& L = t->lev[l];
         const long long nc = (long long)L.cells();
         if (cudaStreamWaitEvent(L.s_leaf, t->ev_up, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
-        // (the offsets of the cells that are not refined are zero for both right-hand sides: rewriting them is harmless)
-        tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_leaf>>>(L.kind, mass[l], L.raw, L.off, L.lm, nc);
+        // (the cells that are not refined: mass into raw, lm and the staged record; their zeros date from create())
+        tree_leaf_moments_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_leaf>>>(L.kind, mass[l], L.raw, L.lm, L.fmm ? L.fmm->src : nullptr,
+                                                                                     L.n[0], L.n[1], nc);
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
         if (cudaEventRecord(L.ev_lm, L.s_leaf) != cudaSuccess) return OCTO_FMM_ECUDA;
         // the level's output: zero wherever the leaf finish does not go (it visits the sub-grids of the leaf tiles only)
@@ -544,11 +555,16 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
     //      below), and the leaf-leaf point-mass sums ----
     auto multipole_step = [&](TreeLevel& L) -> int {
         if (cudaStreamWaitEvent(L.s_m2l, L.ev_rdy, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
-        int r = octo_fmm_set_moments(L.fmm, L.raw, L.off);
-        if (r != OCTO_FMM_OK) return r;
-        const long long nc = (long long)L.cells();
-        stage_leaf_flags_kernel<<<(unsigned)((nc + 255) / 256), 256, 0, L.s_m2l>>>(L.kind, L.fmm->src, L.n[0], L.n[1], L.n[2]);
-        if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        // staging: the cells that are not refined were staged with their masses (tree_leaf_moments_kernel); the refined ones
+        // got their moments from M2M just now
+        int r;
+        if (cudaMemsetAsync(L.fmm->flags + 1, 0, sizeof(int), L.s_m2l) != cudaSuccess) return OCTO_FMM_ECUDA;
+        if (L.n_ref_nodes > 0) {
+            tree_stage_refined_kernel<<<4u * (unsigned)L.n_ref_nodes, 128, 0, L.s_m2l>>>(L.raw, L.off, L.fmm->src, L.n[0], L.n[1], L.n[2], L.fmm->cfg.h,
+                                                                                     L.fmm->flags, L.fmm->cfg.am_correction, L.ref_nodes);
+            if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        }
+        L.fmm->state = 1;
         clear_parent(L.fmm);
         if ((r = octo_fmm_interact(L.fmm)) != OCTO_FMM_OK) return r;
         return cudaEventRecord(L.ev_m2l, L.s_m2l) == cudaSuccess ? OCTO_FMM_OK : OCTO_FMM_ECUDA;
@@ -796,7 +812,7 @@ int octo_fmm_tree_launches(const octo_fmm_tree_t* t, int* launches)
     int n = 0;
     for (const TreeLevel& l : t->lev) {
         n += 1 + (l.has_refined ? 1 : 0);                                  // leaf moments, M2M
-        if (l.fmm && l.n_m2l_tiles > 0) n += 4;                            // stage, flags, multipole step, L2L
+        if (l.fmm && l.n_m2l_tiles > 0) n += 3;                            // stage (refined cells), multipole step, L2L
         if (l.leaf) n += 2;                                                // stage, leaf-leaf sums
         if (l.n_fin_nodes > 0) n += 1;                                     // leaf finish
     }
