@@ -229,16 +229,25 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
         for (int c = 0; c < 3; ++c) v[1 + c] -= sh[1 + c] + a.pC[c * pcell + P];
     }
     unsigned long long taken = 0;
+    const int lane = threadIdx.x & 31;
     if ((flag & NODE_OWN_L) && a.kind_f) {
-        // the children of the refined cells of the near field
+        // the children of the refined cells of the near field.  Kinds are constant over sub-grids and the warp's cells lie in
+        // one: which of the 27 sub-grids around it are refined is read once (a lane each, one ballot); a partner's kind is
+        // then a bit of that word -- no bounds test, no load per list entry
+        unsigned char kd = KIND_ABSENT;
+        {
+            const int X = 8 * ((i >> 3) + lane % 3 - 1), Y = 8 * ((j >> 3) + (lane / 3) % 3 - 1), Z = 8 * ((k >> 3) + lane / 9 - 1);
+            if (lane < 27 && X >= 0 && Y >= 0 && Z >= 0 && X < nx && Y < ny && Z < nz) kd = a.kind[((long long)Z * ny + Y) * nx + X];
+        }
+        const unsigned refined = __ballot_sync(0xffffffffu, kd == KIND_REFINED);
         const int cls = (i & 1) + 2 * (j & 1) + 4 * (k & 1);
         const double hf = 0.5 * a.h;
         double s[4] = {0.0, 0.0, 0.0, 0.0};
         for (int q = 0; q < c_near_count[cls]; ++q) {
             const char4 d = c_near[cls][q];
             const int bi = i + d.x, bj = j + d.y, bk = k + d.z;
-            if (bi < 0 || bj < 0 || bk < 0 || bi >= nx || bj >= ny || bk >= nz) continue;
-            if (a.kind[((long long)bk * ny + bj) * nx + bi] != KIND_REFINED) continue;
+            const int bit = ((((k & 7) + d.z) >> 3) + 1) * 9 + ((((j & 7) + d.y) >> 3) + 1) * 3 + ((((i & 7) + d.x) >> 3) + 1);
+            if (!((refined >> bit) & 1u)) continue;
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
                 const int ax = c & 1, ay = (c >> 1) & 1, az = c >> 2;
@@ -255,16 +264,24 @@ __global__ void __launch_bounds__(128) tree_leaf_finish_kernel(const TreeFinishA
         for (int c = 0; c < 4; ++c) v[c] += s[c];
     }
     if ((flag & NODE_COARSE_NBR) && a.kind_c) {
-        // the coarser leaves in the near field of the parent
+        // the coarser leaves in the near field of the parent (the parents of a sub-grid's cells lie in one sub-grid of the
+        // level above: the same word of 27 kinds, there)
+        unsigned char kd = KIND_ABSENT;
+        {
+            const int X = 8 * ((pi >> 3) + lane % 3 - 1), Y = 8 * ((pj >> 3) + (lane / 3) % 3 - 1), Z = 8 * ((pk >> 3) + lane / 9 - 1);
+            if (lane < 27 && X >= 0 && Y >= 0 && Z >= 0 && X < a.pn[0] && Y < a.pn[1] && Z < a.pn[2])
+                kd = a.kind_c[((long long)Z * a.pn[1] + Y) * a.pn[0] + X];
+        }
+        const unsigned coarse_leaf = __ballot_sync(0xffffffffu, kd == KIND_LEAF);
         const int cls = (pi & 1) + 2 * (pj & 1) + 4 * (pk & 1);       // psh is even: the parity of the lattice index
         const double hf = a.h;                       // this level is the fine one of the pair
         double s[4] = {0.0, 0.0, 0.0, 0.0};
         for (int q = 0; q < c_near_count[cls]; ++q) {
             const char4 d = c_near[cls][q];
             const int ai = pi + d.x, aj = pj + d.y, ak = pk + d.z;
-            if (ai < 0 || aj < 0 || ak < 0 || ai >= a.pn[0] || aj >= a.pn[1] || ak >= a.pn[2]) continue;
+            const int bit = ((((pk & 7) + d.z) >> 3) + 1) * 9 + ((((pj & 7) + d.y) >> 3) + 1) * 3 + ((((pi & 7) + d.x) >> 3) + 1);
+            if (!((coarse_leaf >> bit) & 1u)) continue;
             const long long A = ((long long)ak * a.pn[1] + aj) * a.pn[0] + ai;
-            if (a.kind_c[A] != KIND_LEAF) continue;
             const double m = a.mass_c[A];
             // x_b - x_A = -(x_A - x_b),  2 i_A - i_b = 2 (parent + d) - (2 parent + (a,b,c)) = 2 d - (a,b,c)
             const double Rx = -(((double)(2 * d.x - (i & 1)) + 0.5) * hf), Ry = -(((double)(2 * d.y - (j & 1)) + 0.5) * hf),
