@@ -303,6 +303,7 @@ struct octo_fmm_tree {
     cudaStream_t user;                 // the caller's stream (cfg.stream): a solve starts after and is joined into it
     cudaEvent_t ev_user;               // hand-over between the two
     cudaEvent_t ev_up;                 // a solve has begun on the main stream (the side streams start behind it)
+    cudaEvent_t ev_top_rdy, ev_top_m2l;   // the finest uniform level: its moments are there / its multipole step is done
     bool solved;
 };
 
@@ -333,6 +334,8 @@ int octo_fmm_tree_destroy(octo_fmm_tree_t* t)
         if (l.ev_lm) cudaEventDestroy(l.ev_lm);
     }
     if (t->ev_up) cudaEventDestroy(t->ev_up);
+    if (t->ev_top_rdy) cudaEventDestroy(t->ev_top_rdy);
+    if (t->ev_top_m2l) cudaEventDestroy(t->ev_top_m2l);
     if (t->ev_user) cudaEventDestroy(t->ev_user);
     for (cudaStream_t& q : t->pool_m2l) if (q) cudaStreamDestroy(q);
     for (cudaStream_t& q : t->pool_leaf) if (q) cudaStreamDestroy(q);
@@ -357,7 +360,7 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
     t->user = (cudaStream_t)cfg->stream;
     t->stream = nullptr;
     t->solved = false;
-    t->ev_up = nullptr; t->ev_user = nullptr;
+    t->ev_up = nullptr; t->ev_user = nullptr; t->ev_top_rdy = nullptr; t->ev_top_m2l = nullptr;
     t->lev = std::move(P.lev);
     // Streams.  The multipole steps of the levels are long CTAs that fill every SM (one per SM, 100 us each); whatever
     // else a solve launches is short and must not queue behind them: it runs on streams of the HIGHEST priority (the
@@ -468,7 +471,9 @@ int octo_fmm_tree_create(const octo_fmm_tree_config* cfg, const unsigned char* c
         t->up.push_back(l);
     }
     t->counts = (unsigned long long*)w;
-    if (rc == OCTO_FMM_OK && cudaEventCreateWithFlags(&t->ev_up, cudaEventDisableTiming) != cudaSuccess) rc = OCTO_FMM_ECUDA;
+    if (rc == OCTO_FMM_OK && (cudaEventCreateWithFlags(&t->ev_up, cudaEventDisableTiming) != cudaSuccess ||
+                              cudaEventCreateWithFlags(&t->ev_top_rdy, cudaEventDisableTiming) != cudaSuccess ||
+                              cudaEventCreateWithFlags(&t->ev_top_m2l, cudaEventDisableTiming) != cudaSuccess)) rc = OCTO_FMM_ECUDA;
     // the topology arrays were copied from pageable host memory: make sure they have left it before returning
     if (rc == OCTO_FMM_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = OCTO_FMM_ECUDA;
     if (rc != OCTO_FMM_OK) { octo_fmm_tree_destroy(t); return rc; }
@@ -584,6 +589,7 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
         }
     }
     // ---- meanwhile on the caller's stream: the uniform levels above level 0 (the whole lattice), up ... ----
+    const bool top_early = t->up.size() > 1 && t->up[0].fmm->kernel == 0;
     for (size_t lv = 0; lv < t->up.size(); ++lv) {
         SolverLevel& l = t->up[lv];
         const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
@@ -602,17 +608,36 @@ static int tree_solve_impl(octo_fmm_tree_t* t, const double* const* mass, double
             m2m_kernel<false><<<blocks, 128, 0, st>>>(t->up[lv - 1].raw, t->up[lv - 1].off, l.raw, l.off, l.n, l.n, l.n, t->up[lv - 1].h);
         }
         if (cudaGetLastError() != cudaSuccess) return OCTO_FMM_ECUDA;
+        // The finest uniform level, when it is big enough for the slab-fed kernel (32^3 above a 64^3 base: 88 bricks, 110 us),
+        // does not wait for its turn in the chain: its multipole step needs nothing but its own moments and starts now, on a
+        // leaf stream (high priority: the chain will want it before the bricks of the tree levels that already fill the SMs),
+        // while the main stream goes up to the root and comes down again; the L2L it had as an epilogue becomes a pass of its
+        // own in the chain (12 us)
+        if (lv == 0 && top_early) {
+            cudaStream_t sx = t->pool_leaf[1];
+            if (cudaEventRecord(t->ev_top_rdy, st) != cudaSuccess || cudaStreamWaitEvent(sx, t->ev_top_rdy, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+            struct Lend { octo_fmm* h; cudaStream_t keep; Lend(octo_fmm* h_, cudaStream_t s) : h(h_), keep(h_->stream) { h->stream = s; } ~Lend() { h->stream = keep; } } lend(l.fmm, sx);
+            if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
+            clear_parent(l.fmm);
+            if ((rc = octo_fmm_interact(l.fmm)) != OCTO_FMM_OK) return rc;
+            if (cudaEventRecord(t->ev_top_m2l, sx) != cudaSuccess) return OCTO_FMM_ECUDA;
+        }
     }
     // ---- ... and down, as in the uniform solve ----
     for (int lv = (int)t->up.size() - 1; lv >= 0; --lv) {
         SolverLevel& l = t->up[lv];
-        if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
         const bool has_parent = lv < (int)t->up.size() - 1;
-        const bool fused = has_parent && l.fmm->kernel == 0;
-        if (fused) set_parent(l.fmm, t->up[lv + 1]);
-        rc = octo_fmm_interact(l.fmm);
-        if (fused) clear_parent(l.fmm);
-        if (rc != OCTO_FMM_OK) return rc;
+        const bool early = lv == 0 && top_early;
+        const bool fused = has_parent && l.fmm->kernel == 0 && !early;
+        if (early) {
+            if (cudaStreamWaitEvent(st, t->ev_top_m2l, 0) != cudaSuccess) return OCTO_FMM_ECUDA;
+        } else {
+            if ((rc = octo_fmm_set_moments(l.fmm, l.raw, l.off)) != OCTO_FMM_OK) return rc;
+            if (fused) set_parent(l.fmm, t->up[lv + 1]);
+            rc = octo_fmm_interact(l.fmm);
+            if (fused) clear_parent(l.fmm);
+            if (rc != OCTO_FMM_OK) return rc;
+        }
         const dim3 blocks((unsigned)((l.n + 127) / 128), (unsigned)l.n, (unsigned)l.n);
         if (!has_parent)
             l2l_kernel<false><<<blocks, 128, 0, st>>>(l.fmm->L, l.fmm->C, l.off, nullptr, nullptr, nullptr, l.n, l.n, l.n, l.h);
