@@ -356,8 +356,11 @@ int octo_fmm_solver_num_levels(const octo_fmm_solver_t *s, int *multipole_levels
  * sub-grid two levels finer is not detected).  Above level 0 the uniform levels n0/2 .. 2 are built by the library.
  * mass[l]: DEVICE [box cells], read at the leaf cells only; out[l]: DEVICE [4][box cells] = (phi, g_x, g_y, g_z) at
  * the leaf cells, zeros elsewhere.  mass and out are HOST arrays of `depth` device pointers, all 16-byte aligned.
- * The caller lends the workspace; everything is enqueued on cfg.stream; create() synchronises the stream once (it
- * uploads the topology from pageable memory).  One handle is not thread-safe. */
+ * The caller lends the workspace.  create() uploads the topology from pageable memory and writes what no solve changes
+ * (the zeros and the kind of every cell that is not refined, in the levels' moment arrays and staged records) on a stream
+ * of the library's own, and synchronises it once.  A solve runs on streams of the library's own (its levels side by side),
+ * behind whatever cfg.stream held at the call, and cfg.stream waits for it: to the caller it is asynchronous work on
+ * cfg.stream.  One handle is not thread-safe. */
 typedef struct octo_fmm_tree octo_fmm_tree_t;
 typedef struct {
     int n0;                 /* cells per axis of level 0: a power of two, 8 <= n0 <= 2048                      */
